@@ -1,0 +1,156 @@
+/*
+ * gnep.h -- C ABI of libgnep_b200.so: the data-parallel hot path of GNEP (arxiv 2507.00528) on one
+ * NVIDIA B200 (sm_100a): full-batch NEP training loss, its analytic gradient over every trainable
+ * parameter, and the Adam update.
+ *
+ * Citations "P:n" are line numbers of the paper text; "R<k>" are the readings of silent or
+ * garbled passages listed in DESIGN.md.  All kernels behind these calls are hand-written CUDA; there is
+ * no CPU fallback: gnep_create fails with GNEP_ECUDA when no sm_100 device is usable.
+ *
+ * Conventions
+ *   - every call returns 0 (GNEP_OK) or a negative GNEP_E* code; gnep_last_error(h) then holds a
+ *     message (handle-owned string, never freed by the caller).  No C++ exception crosses the ABI.
+ *   - the caller owns every pointer it passes.  Inputs are copied during the call (they may be freed on
+ *     return); outputs are written only into caller-provided buffers.
+ *   - `is_device` != 0: array pointers are CUDA device pointers on the handle's device (e.g. torch
+ *     tensors); == 0: host pointers.  Small scalar outputs (loss_terms, P, step) are always host.
+ *   - all work is enqueued on the cudaStream_t given at create (NULL = default stream).  Calls that
+ *     return host data synchronise that stream; gnep_adam_step and gnep_loss_and_grad with
+ *     loss_terms == NULL and host-free arguments do not.
+ *   - units: Angstrom, eV, eV/Angstrom; virial in eV (total per structure).
+ *   - one handle = one model + one resident batch.  Not thread-safe per handle.
+ *
+ * Parameter vector theta (P floats, R6/S:8(c).2):
+ *   [ cR[I][J][n][k] (k fastest; I = species of the central atom, J = of the neighbour)
+ *   | cA[I][J][n][k]
+ *   | for each species t: W0_t[mu][nu] (nu fastest), b0_t[mu], w1_t[mu], b1_t ]         (P:718 Eq.D1.1)
+ * Descriptor index nu: 0..NR-1 radial q_n (Eq.5); NR+(l-1)*NA+n three-body q_nl, l=1..l_max
+ * (Eq.7); NR+l_max*NA+n four-body (R14).
+ */
+#ifndef GNEP_H
+#define GNEP_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GNEP_OK 0
+#define GNEP_EINVAL (-1)     /* bad spec / size / null pointer                         */
+#define GNEP_ESTATE (-2)     /* call out of order, e.g. loss before load               */
+#define GNEP_ECUDA (-3)      /* any CUDA error, or no sm_100 device                    */
+#define GNEP_ENOMEM (-4)
+#define GNEP_ERANGE (-5)     /* species id >= T, non-positive cell volume, too many pairs */
+#define GNEP_ENONFINITE (-6) /* NaN/Inf in the loss                                    */
+
+/* build limits (compile-time array sizes of the kernels) */
+#define GNEP_MAX_SPECIES 4
+#define GNEP_MAX_NFUNC 16    /* n_radial, n_angular                                    */
+#define GNEP_MAX_BASIS 16    /* n_basis_radial, n_basis_angular                        */
+#define GNEP_MAX_NEURONS 128
+
+typedef struct gnep_handle gnep_handle; /* opaque; owns all device memory it allocates */
+
+/* Model and loss specification (Eq.5-8; P:718 Eq.D1.1; Eq.9-12). */
+typedef struct {
+  int32_t n_species;                     /* T, 1..GNEP_MAX_SPECIES                                      */
+  int32_t n_radial, n_basis_radial;      /* NR functions n=0..NR-1, KR basis functions k=0..KR-1 (R1,R2) */
+  double rc_radial;                      /* radial cutoff r_c^R (Eq.2)                                   */
+  int32_t n_angular, n_basis_angular;    /* NA, KA (own coefficients cA, R4)                             */
+  double rc_angular;                     /* 0 < rc_angular <= rc_radial                                  */
+  int32_t l_max;                         /* 1..4 (Eq.7; l = 5..8 not built)                              */
+  int32_t use_4body;                     /* 0/1, needs l_max >= 2 (R14)                                  */
+  int32_t n_neurons;                     /* hidden width N_neu, 1..GNEP_MAX_NEURONS                      */
+  double lambda_e, lambda_f, lambda_v;   /* Eq.9 weights                                                 */
+  double lambda_2;                       /* weight of t_2 = mean(theta^2) (R22; not in the paper)        */
+  int32_t loss_mode;                     /* 0: mean-square, paper Eq.9-12; 1: RMSE per term (R21)        */
+  const float *q_scale;                  /* host, N_des entries, fixed input scaling G = q_scale*q, or NULL = ones (R15) */
+} gnep_model_spec;
+
+/* Create a model on the current CUDA device.  cuda_stream: a cudaStream_t (may be NULL).
+ * Parameters start at zero; optimiser state at zero, step 0.  EINVAL on a bad spec; ECUDA if the
+ * device is not compute capability 10.x. */
+int gnep_create(const gnep_model_spec *spec, void *cuda_stream, gnep_handle **out);
+int gnep_destroy(gnep_handle *h);
+
+/* Number of trainable parameters P and of descriptor components N_des. */
+int gnep_num_params(const gnep_handle *h, int64_t *P);
+int gnep_num_descriptors(const gnep_handle *h, int32_t *n_des);
+
+/* theta: P floats in the layout above. */
+int gnep_set_params(gnep_handle *h, const float *theta, int is_device);
+int gnep_get_params(const gnep_handle *h, float *theta, int is_device);
+
+/* Replace the fixed, non-trainable input scaling (HOST, N_des floats; R15).  The harness derives it from
+ * gnep_descriptors at the initial parameters, which needs a loaded batch, hence a call of its own. */
+int gnep_set_q_scale(gnep_handle *h, const float *q_scale);
+
+/* Load the training batch and build its neighbour lists on the GPU (Eq.2; R7-R9): periodic
+ * cell-list search, all images with |r_j + shift - r_i| < rc (strict), excluding only (i, zero
+ * shift); positions are first moved into the cell by whole lattice vectors.  Replaces any
+ * previous batch.  Positions are fixed during training, so this is off the epoch loop.
+ *   n_structs S >= 0; atom_offsets: S+1 ints, HOST, ascending, offsets[0] = 0, N = offsets[S]
+ *   positions N*3 doubles (x,y,z per atom); cells S*9 doubles (rows a, b, c); types N ints in [0,T)
+ *   ref_energy S doubles (total eV) or NULL; ref_force N*3 or NULL; ref_virial S*6 (total eV,
+ *   order xx,yy,zz,xy,yz,zx) or NULL.  A NULL reference removes that loss term.
+ * ERANGE: species id out of range, degenerate cell, >= 2^31 pairs.  */
+int gnep_load_batch(gnep_handle *h, int32_t n_structs, const int32_t *atom_offsets, const double *positions,
+                    const double *cells, const int32_t *types, const double *ref_energy,
+                    const double *ref_force, const double *ref_virial, int is_device);
+
+/* Replace only the reference values of the resident batch (same shapes / NULL rules as above). */
+int gnep_set_targets(gnep_handle *h, const double *ref_energy, const double *ref_force,
+                     const double *ref_virial, int is_device);
+
+/* Parity aid: the neighbour list in canonical order (rows by atom, entries ascending (j, sa, sb, sc)),
+ * which: 0 radial, 1 angular.  n_pairs (host, may be NULL) receives the pair count; row_ptr N+1 int64;
+ * j and shift3 (3 int8 per pair) hold `capacity` pairs; if capacity < n_pairs only n_pairs is set
+ * and EINVAL returned.  Any of row_ptr/j/shift3 may be NULL. */
+int gnep_neighbor_list(const gnep_handle *h, int which, int64_t *n_pairs, int64_t *row_ptr, int32_t *j,
+                       int8_t *shift3, int64_t capacity, int is_device);
+
+/* Parity aid: unscaled descriptors q[N][N_des] at the current parameters (Eq.5, Eq.7, R14). */
+int gnep_descriptors(gnep_handle *h, float *q, int is_device);
+
+/* Predictions at the current parameters: E_s (S), F (N*3, input atom order), W_s (S*6) (Eq.1, 3, 4;
+ * W_ab = -sum r_ij,a f_ij,b, R17).  Any output may be NULL. */
+int gnep_predict(gnep_handle *h, float *energy, float *force, float *virial, int is_device);
+
+/* One full-batch evaluation of the loss and of its analytic gradient (Eq.9-16, App.C/D in
+ * contraction-first form).  loss_terms (HOST, 5 floats: L, t_e, t_f, t_v, t_2)
+ * may be NULL (no synchronisation then); grad (P floats) may be NULL: the gradient always stays in
+ * the handle for gnep_adam_step.  ENONFINITE if loss_terms is requested and L is not finite. */
+int gnep_loss_and_grad(gnep_handle *h, float *loss_terms, float *grad, int is_device);
+
+/* Fused Adam update with the internal gradient (textbook, bias-corrected, step counted from 1; R23). */
+int gnep_adam_step(gnep_handle *h, float lr, float beta1, float beta2, float eps);
+
+/* One epoch = gnep_loss_and_grad + gnep_adam_step, `n_epochs` times, replayed from a CUDA graph;
+ * loss_terms (HOST, 5 floats, or NULL) receives the terms of the LAST epoch's loss evaluation. */
+int gnep_train_epochs(gnep_handle *h, int32_t n_epochs, float lr, float beta1, float beta2, float eps,
+                      float *loss_terms);
+
+/* Checkpoint / resume of the optimiser state (m, v: P floats each; either may be NULL). */
+int gnep_get_opt_state(const gnep_handle *h, float *m, float *v, int64_t *step, int is_device);
+int gnep_set_opt_state(gnep_handle *h, const float *m, const float *v, int64_t step, int is_device);
+
+/* Sizes of the resident batch: atoms, structures, radial pairs, angular pairs (any may be NULL). */
+int gnep_batch_info(const gnep_handle *h, int64_t *n_atoms, int64_t *n_structs, int64_t *n_pairs_radial,
+                    int64_t *n_pairs_angular);
+
+/* Kernel launches issued by this handle since creation (for bench.py's gpu_launches). */
+int gnep_launch_count(const gnep_handle *h, int64_t *n);
+
+/* Per-phase device times of the most recent gnep_loss_and_grad / gnep_adam_step pair measured with
+ * CUDA events on the handle's stream when profiling is on (gnep_set_profiling(h,1)).  names: array of
+ * `capacity` const char* (handle-owned), ms: `capacity` floats; *n receives the phase count. */
+int gnep_set_profiling(gnep_handle *h, int on);
+int gnep_phase_times(const gnep_handle *h, const char **names, float *ms, int32_t capacity, int32_t *n);
+
+/* Last error message of this handle (or of a failed gnep_create when h == NULL). */
+const char *gnep_last_error(const gnep_handle *h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GNEP_H */

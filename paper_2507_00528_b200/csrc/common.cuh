@@ -1,0 +1,171 @@
+// common.cuh -- shared device helpers of the GNEP B200 path (fp32 arithmetic, sm_100a).
+// Nothing here is shared with oracle/: the oracle is plain C fp64 and is written separately.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define GNEP_NLM 24           // (l,m) slots for l = 1..4
+#define GNEP_WARPS 8          // warps per CTA of the warp-per-atom kernels
+#define GNEP_TILE 8           // atoms per warp tile of the network kernels
+#define GNEP_MAX_SPECIES_C 4   // == GNEP_MAX_SPECIES of include/gnep.h
+
+// Model constants passed by value to every kernel.
+struct DevSpec {
+  int T, NR, KR, NA, KA, L, use4, Nn, Ndes, P;
+  int KRp, KAp;               // basis sizes padded to the template size of the pair kernels
+  int offA, offNet, netSize;  // parameter-vector offsets (include/gnep.h layout)
+  int ldW;                    // padded shared-memory row stride of W0 (odd -> conflict-free)
+  int loss_mode;
+  float rcRinv, rcAinv;
+  float lam_e, lam_f, lam_v, lam_2;
+};
+
+// 2*C_lm (C_lm = (2l+1)/(4 pi) * Chat_lm, zero for l > l_max), l of each slot, kappa4.
+__constant__ float c_C2[GNEP_NLM];
+__constant__ float c_lf[GNEP_NLM];
+__constant__ float c_kappa4;
+
+__device__ __forceinline__ int l_of_lm(int lm) { return lm < 3 ? 1 : lm < 8 ? 2 : lm < 15 ? 3 : 4; }
+
+// ---------------------------------------------------------------------------------------------
+// Chebyshev radial basis (paper Eq.6, App.A):  f_k = 1/2 (T_k(xi)+1) f_c,  xi = 2 (d/rc - 1)^2 - 1
+// ---------------------------------------------------------------------------------------------
+template <int KT>
+__device__ __forceinline__ void cheb_f(float d, float rcinv, float (&f)[KT]) {
+  float t = d * rcinv;
+  float x = t - 1.f;
+  float xi = 2.f * x * x - 1.f;
+  float hfc = 0.25f * (1.f + cospif(t));      // 1/2 f_c
+  float Tm2 = 1.f, Tm1 = xi;
+  f[0] = 2.f * hfc;
+  if (KT > 1) f[1] = hfc * (xi + 1.f);
+#pragma unroll
+  for (int k = 2; k < KT; ++k) {
+    float Tk = 2.f * xi * Tm1 - Tm2;
+    f[k] = hfc * (Tk + 1.f);
+    Tm2 = Tm1; Tm1 = Tk;
+  }
+}
+
+template <int KT>
+__device__ __forceinline__ void cheb_ffp(float d, float rcinv, float (&f)[KT], float (&fp)[KT]) {
+  float t = d * rcinv;
+  float x = t - 1.f;
+  float xi = 2.f * x * x - 1.f;
+  float dxi = 4.f * x * rcinv;
+  float s, c;
+  sincospif(t, &s, &c);
+  float hfc = 0.25f * (1.f + c);                          // 1/2 f_c
+  float hfcp = -0.25f * 3.14159265358979f * rcinv * s;    // 1/2 f_c'
+  float hdf = hfc * dxi;                                  // 1/2 f_c dxi/dd
+  float Tm2 = 1.f, Tm1 = xi, Dm2 = 0.f, Dm1 = 1.f;
+  f[0] = 2.f * hfc;  fp[0] = 2.f * hfcp;
+  if (KT > 1) { f[1] = hfc * (xi + 1.f); fp[1] = hdf + (xi + 1.f) * hfcp; }
+#pragma unroll
+  for (int k = 2; k < KT; ++k) {
+    float Tk = 2.f * xi * Tm1 - Tm2;
+    float Dk = 2.f * Tm1 + 2.f * xi * Dm1 - Dm2;
+    f[k] = hfc * (Tk + 1.f);
+    fp[k] = Dk * hdf + (Tk + 1.f) * hfcp;
+    Tm2 = Tm1; Tm1 = Tk; Dm2 = Dm1; Dm1 = Dk;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Real harmonics of a UNIT vector (paper App.B): emits, for each of the 24 (l,m) slots,
+// b = b_lm(rhat) and g = (grad b_lm)(rhat)  [polynomial gradient, r^2 terms differentiated, then r=1].
+// With B_lm = b_lm(r)/d^l:  B_lm = b,  grad B_lm = (g - l b rhat) / d.
+// F is called as f(lm, l, b, gx, gy, gz) with literal lm so that register arrays index statically.
+// ---------------------------------------------------------------------------------------------
+template <class F>
+__device__ __forceinline__ void blm_unit(float x, float y, float z, F f) {
+  float x2 = x * x, y2 = y * y, z2 = z * z;
+  float xy = x * y, xz = x * z, yz = y * z;
+  float d2 = x2 - y2;
+  // l = 1
+  f(0, 1, z, 0.f, 0.f, 1.f);
+  f(1, 1, x, 1.f, 0.f, 0.f);
+  f(2, 1, y, 0.f, 1.f, 0.f);
+  // l = 2
+  f(3, 2, 3.f * z2 - 1.f, -2.f * x, -2.f * y, 4.f * z);
+  f(4, 2, xz, z, 0.f, x);
+  f(5, 2, yz, 0.f, z, y);
+  f(6, 2, d2, 2.f * x, -2.f * y, 0.f);
+  f(7, 2, 2.f * xy, 2.f * y, 2.f * x, 0.f);
+  // l = 3
+  float a5 = 5.f * z2 - 1.f;
+  f(8, 3, (5.f * z2 - 3.f) * z, -6.f * xz, -6.f * yz, 9.f * z2 - 3.f);
+  f(9, 3, a5 * x, a5 - 2.f * x2, -2.f * xy, 8.f * xz);
+  f(10, 3, a5 * y, -2.f * xy, a5 - 2.f * y2, 8.f * yz);
+  f(11, 3, d2 * z, 2.f * xz, -2.f * yz, d2);
+  f(12, 3, 2.f * xy * z, 2.f * yz, 2.f * xz, 2.f * xy);
+  f(13, 3, (x2 - 3.f * y2) * x, 3.f * d2, -6.f * xy, 0.f);
+  f(14, 3, (3.f * x2 - y2) * y, 6.f * xy, 3.f * d2, 0.f);
+  // l = 4
+  float p = (7.f * z2 - 3.f) * z;
+  float w = 7.f * z2 - 1.f;
+  float c3 = 15.f * z2 - 3.f;
+  float cx = (x2 - 3.f * y2) * x, cy = (3.f * x2 - y2) * y;
+  f(15, 4, (35.f * z2 - 30.f) * z2 + 3.f, (12.f - 60.f * z2) * x, (12.f - 60.f * z2) * y, (80.f * z2 - 48.f) * z);
+  f(16, 4, p * x, p - 6.f * z * x2, -6.f * z * xy, c3 * x);
+  f(17, 4, p * y, -6.f * z * xy, p - 6.f * z * y2, c3 * y);
+  f(18, 4, w * d2, 2.f * x * (w - d2), -2.f * y * (w + d2), 12.f * z * d2);
+  f(19, 4, 2.f * w * xy, 2.f * y * (w - 2.f * x2), 2.f * x * (w - 2.f * y2), 24.f * xy * z);
+  f(20, 4, cx * z, 3.f * d2 * z, -6.f * xy * z, cx);
+  f(21, 4, cy * z, 6.f * xy * z, 3.f * d2 * z, cy);
+  f(22, 4, x2 * x2 - 6.f * x2 * y2 + y2 * y2, 4.f * cx, -4.f * cy, 0.f);
+  f(23, 4, 4.f * xy * d2, 4.f * cy, 4.f * cx, 0.f);
+}
+
+// 4-body cubic invariant of the l=2 moments s[0..4] (R14): P4, gradient, Hessian*t
+__device__ __forceinline__ float p4_value(const float *s) {
+  float s0 = s[0], s1 = s[1], s2 = s[2], s3 = s[3], s4 = s[4];
+  return s0 * s0 * s0 + 18.f * s0 * (s1 * s1 + s2 * s2) - 9.f * s0 * (s3 * s3 + s4 * s4) +
+         54.f * s3 * (s1 * s1 - s2 * s2) + 108.f * s1 * s2 * s4;
+}
+__device__ __forceinline__ void p4_grad(const float *s, float *g) {
+  float s0 = s[0], s1 = s[1], s2 = s[2], s3 = s[3], s4 = s[4];
+  g[0] = 3.f * s0 * s0 + 18.f * (s1 * s1 + s2 * s2) - 9.f * (s3 * s3 + s4 * s4);
+  g[1] = 36.f * s0 * s1 + 108.f * s3 * s1 + 108.f * s2 * s4;
+  g[2] = 36.f * s0 * s2 - 108.f * s3 * s2 + 108.f * s1 * s4;
+  g[3] = -18.f * s0 * s3 + 54.f * (s1 * s1 - s2 * s2);
+  g[4] = -18.f * s0 * s4 + 108.f * s1 * s2;
+}
+__device__ __forceinline__ void p4_hess_vec(const float *s, const float *t, float *h) {
+  float s0 = s[0], s1 = s[1], s2 = s[2], s3 = s[3], s4 = s[4];
+  h[0] = 6.f * s0 * t[0] + 36.f * s1 * t[1] + 36.f * s2 * t[2] - 18.f * s3 * t[3] - 18.f * s4 * t[4];
+  h[1] = 36.f * s1 * t[0] + (36.f * s0 + 108.f * s3) * t[1] + 108.f * s4 * t[2] + 108.f * s1 * t[3] + 108.f * s2 * t[4];
+  h[2] = 36.f * s2 * t[0] + 108.f * s4 * t[1] + (36.f * s0 - 108.f * s3) * t[2] - 108.f * s2 * t[3] + 108.f * s1 * t[4];
+  h[3] = -18.f * s3 * t[0] + 108.f * s1 * t[1] - 108.f * s2 * t[2] - 18.f * s0 * t[3];
+  h[4] = -18.f * s4 * t[0] + 108.f * s2 * t[1] + 108.f * s1 * t[2] - 18.f * s0 * t[4];
+}
+
+// Fixed-order warp reduction of K per-lane accumulators through shared memory:
+// returns sum over lanes of acc[lane_k] to lane k (k < K), 0 elsewhere.  buf: K*33 floats per warp.
+template <int K>
+__device__ __forceinline__ float warp_transpose_reduce(const float (&acc)[K], float *buf, int lane) {
+#pragma unroll
+  for (int k = 0; k < K; ++k) buf[k * 33 + lane] = acc[k];
+  __syncwarp();
+  float s = 0.f;
+  if (lane < K) {
+#pragma unroll 8
+    for (int i = 0; i < 32; ++i) s += buf[lane * 33 + i];
+  }
+  __syncwarp();
+  return s;
+}
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// stage the expansion coefficients c[I][J][n][k] into shared memory with k padded to KT (zeros)
+__device__ __forceinline__ void stage_coeff(float *dst, const float *src, int rows, int K, int KT) {
+  for (int x = threadIdx.x; x < rows * KT; x += blockDim.x) {
+    int r = x / KT, k = x - r * KT;
+    dst[x] = (k < K) ? src[r * K + k] : 0.f;
+  }
+}

@@ -1,0 +1,816 @@
+// gnep_api.cu -- C ABI of libgnep_b200.so (include/gnep.h) and the host orchestration of the hot path:
+// handle, resident batch, stream-ordered kernel sequence, CUDA graph of one epoch.
+// No CPU fallback: every step of the path runs in the kernels of this directory.
+#include "../../include/gnep.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "common.cuh"
+#include "neighbor.cuh"
+#include "net_kernels.cuh"
+#include "pair_kernels.cuh"
+#include "reduce_kernels.cuh"
+
+namespace {
+
+thread_local std::string g_create_error;
+
+struct Phase { const char *name; cudaEvent_t ev; };
+
+}  // namespace
+
+struct gnep_handle {
+  gnep_model_spec spec{};
+  DevSpec ds{};
+  cudaStream_t stream = nullptr;
+  bool own_stream = false;
+  mutable std::string err;
+  int device = 0;
+  int num_sms = 148;
+  // parameters and optimiser
+  float *theta = nullptr, *grad = nullptr, *m = nullptr, *v = nullptr, *qscale = nullptr;
+  long long *step_dev = nullptr;
+  float *terms = nullptr, *scales = nullptr;   // device: 5 loss terms, 4 seed multipliers
+  float *h_terms = nullptr;                    // pinned host
+  // batch
+  bool loaded = false;
+  int N = 0, S = 0;
+  int64_t nR = 0, nA = 0;
+  int hasE = 0, hasF = 0, hasV = 0;
+  std::vector<void *> batch_allocs;
+  int *perm = nullptr, *type_s = nullptr, *struct_s = nullptr, *segR = nullptr, *rowAs = nullptr, *revA = nullptr;
+  float4 *pairR = nullptr, *pairA = nullptr;
+  int64_t *exp_row[2] = {nullptr, nullptr};
+  int *exp_j[2] = {nullptr, nullptr}, *exp_sh[2] = {nullptr, nullptr};
+  int *srange = nullptr;
+  double *Eref = nullptr, *Wref = nullptr;
+  float *Fref_s = nullptr;
+  SpeciesMap sm{};
+  ReduceMap rm{};
+  int n_cta_net = 0, n_chunks = 0, n_ca_blocks = 0;
+  // per-atom state
+  float *q = nullptr, *Sn = nullptr, *x = nullptr, *Ei = nullptr, *Ep = nullptr, *etil = nullptr, *M1 = nullptr,
+        *M2 = nullptr, *D = nullptr, *Tn = nullptr, *gbar = nullptr, *Acoef = nullptr, *Bcoef = nullptr, *Wat = nullptr;
+  float4 *Fat = nullptr, *fpair = nullptr, *u = nullptr;
+  double *Es = nullptr, *Ws = nullptr, *parts = nullptr;
+  float *e_s = nullptr, *omega = nullptr;
+  float *partialCR = nullptr, *partialCA = nullptr, *partialW = nullptr, *partialB = nullptr;
+  // bookkeeping
+  int64_t launches = 0;
+  cudaGraphExec_t graph = nullptr;
+  float g_lr = 0, g_b1 = 0, g_b2 = 0, g_eps = 0;
+  int64_t graph_launches = 0;
+  bool prof = false;
+  std::vector<Phase> phases;
+  std::vector<const char *> phase_names;
+  std::vector<float> phase_ms;
+};
+
+namespace {
+
+int fail(const gnep_handle *h, int code, const std::string &msg) {
+  if (h) h->err = msg; else g_create_error = msg;
+  return code;
+}
+
+#define CK(call)                                                                                   \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess)                                                                         \
+      return fail(h, e_ == cudaErrorMemoryAllocation ? GNEP_ENOMEM : GNEP_ECUDA,                   \
+                  std::string(#call) + ": " + cudaGetErrorString(e_));                             \
+  } while (0)
+
+#define RET_IF(expr)            \
+  do {                          \
+    int rc_ = (expr);           \
+    if (rc_ != GNEP_OK) return rc_; \
+  } while (0)
+
+int padded_basis(int K) {
+  const int sizes[] = {4, 6, 8, 12, 16};
+  for (int s : sizes) if (K <= s) return s;
+  return -1;
+}
+
+#define DISPATCH_KT(KP, ...)                                    \
+  switch (KP) {                                                 \
+    case 4: { constexpr int KT = 4; __VA_ARGS__; } break;       \
+    case 6: { constexpr int KT = 6; __VA_ARGS__; } break;       \
+    case 8: { constexpr int KT = 8; __VA_ARGS__; } break;       \
+    case 12: { constexpr int KT = 12; __VA_ARGS__; } break;     \
+    default: { constexpr int KT = 16; __VA_ARGS__; } break;     \
+  }
+
+template <class T>
+int dalloc(gnep_handle *h, T **p, size_t n, bool batch) {
+  void *q = nullptr;
+  CK(cudaMalloc(&q, std::max<size_t>(n, 1) * sizeof(T)));
+  *p = (T *)q;
+  if (batch) h->batch_allocs.push_back(q);
+  return GNEP_OK;
+}
+
+void free_batch(gnep_handle *h) {
+  for (void *p : h->batch_allocs) cudaFree(p);
+  h->batch_allocs.clear();
+  h->loaded = false;
+  if (h->graph) { cudaGraphExecDestroy(h->graph); h->graph = nullptr; }
+}
+
+// ---- dynamic shared memory sizes (bytes) --------------------------------------------------------
+size_t smem_radial(const DevSpec &d) { return sizeof(float) * (d.T * d.T * d.NR * d.KRp + GNEP_WARPS * (d.KRp * 33 + d.KRp)); }
+size_t smem_ang_fwd(const DevSpec &d) {
+  return sizeof(float) * (((d.T * d.T * d.NA * d.KAp + 3) & ~3) + GNEP_WARPS * ((d.NA + GNEP_NLM) * 32 + d.NA * GNEP_NLM));
+}
+size_t smem_ang_force(const DevSpec &d) { return sizeof(float) * (((d.T * d.T * d.NA * d.KAp + 3) & ~3) + GNEP_WARPS * d.NA * GNEP_NLM); }
+size_t smem_ang_adj(const DevSpec &d) {
+  return sizeof(float) * (((d.T * d.T * d.NA * d.KAp + 3) & ~3) + GNEP_WARPS * ((2 * d.NA + 2 * GNEP_NLM) * 32 + 2 * d.NA * GNEP_NLM));
+}
+size_t smem_cgrad_ang(const DevSpec &d) {
+  int NAp = d.NA | 1, KTp = d.KAp + 1;
+  int nacc = d.T * d.T * d.NA * d.KAp;
+  return sizeof(float) * GNEP_WARPS * (((nacc + 3) & ~3) + 4 * d.NA * GNEP_NLM + 32 * (2 * NAp + 2 * KTp));
+}
+size_t smem_net_fwd(const DevSpec &d) {
+  return sizeof(float) * (net_smem_floats(d) + ((d.T * d.NR * d.KRp + 3) & ~3) + GNEP_WARPS * (d.Ndes + d.Nn + d.NR) * GNEP_TILE);
+}
+size_t smem_net_bwd(const DevSpec &d) {
+  return sizeof(float) * (net_smem_floats(d) + ((GNEP_WARPS * (2 * d.Nn + 1) + 3) & ~3) + GNEP_WARPS * (d.Ndes + d.Nn) * GNEP_TILE);
+}
+size_t smem_gemm_w0(const DevSpec &d) { return sizeof(float) * GW_SUB * 2 * (d.Nn + d.Ndes); }
+size_t smem_cgrad_rad(const DevSpec &d) { return sizeof(float) * CR_SUB * 2 * (d.NR + d.T * d.KRp); }
+
+template <class K>
+int set_smem(gnep_handle *h, K kernel, size_t bytes) {
+  if (bytes > 227 * 1024) return fail(h, GNEP_EINVAL, "model too large for shared memory staging");
+  CK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+  return GNEP_OK;
+}
+
+int configure_kernels(gnep_handle *h) {
+  const DevSpec &d = h->ds;
+  DISPATCH_KT(d.KRp, RET_IF(set_smem(h, k_radial_fwd<KT>, smem_radial(d))); RET_IF(set_smem(h, k_radial_adj<KT>, smem_radial(d))));
+  DISPATCH_KT(d.KAp, RET_IF(set_smem(h, k_angular_fwd<KT>, smem_ang_fwd(d))); RET_IF(set_smem(h, k_angular_force<KT>, smem_ang_force(d)));
+              RET_IF(set_smem(h, k_angular_adj<KT>, smem_ang_adj(d))); RET_IF(set_smem(h, k_cgrad_angular<KT>, smem_cgrad_ang(d))));
+  RET_IF(set_smem(h, k_net_fwd, smem_net_fwd(d)));
+  RET_IF(set_smem(h, k_net_bwd, smem_net_bwd(d)));
+  RET_IF(set_smem(h, k_gemm_w0, smem_gemm_w0(d)));
+  RET_IF(set_smem(h, k_cgrad_radial, smem_cgrad_rad(d)));
+  return GNEP_OK;
+}
+
+void mark(gnep_handle *h, const char *name) {
+  if (!h->prof) return;
+  Phase p; p.name = name;
+  cudaEventCreate(&p.ev);
+  cudaEventRecord(p.ev, h->stream);
+  h->phases.push_back(p);
+}
+void prof_begin(gnep_handle *h) {
+  if (!h->prof) return;
+  for (auto &p : h->phases) cudaEventDestroy(p.ev);
+  h->phases.clear();
+  mark(h, "begin");
+}
+void prof_collect(gnep_handle *h) {
+  if (!h->prof || h->phases.empty()) return;
+  cudaEventSynchronize(h->phases.back().ev);
+  h->phase_names.clear(); h->phase_ms.clear();
+  for (size_t i = 1; i < h->phases.size(); ++i) {
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, h->phases[i - 1].ev, h->phases[i].ev);
+    h->phase_names.push_back(h->phases[i].name);
+    h->phase_ms.push_back(ms);
+  }
+}
+
+inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+#define LAUNCH(h, kern, grid, block, smem, ...)                       \
+  do {                                                                \
+    if ((grid) > 0) {                                                 \
+      kern<<<(grid), (block), (smem), (h)->stream>>>(__VA_ARGS__);   \
+      (h)->launches++;                                                \
+    }                                                                 \
+  } while (0)
+
+// ---- the forward half: descriptors, network, forces, per-structure sums (rows a1-a4) --------------
+int enqueue_descriptors(gnep_handle *h) {
+  const DevSpec &d = h->ds;
+  int gridA = cdiv(h->N, GNEP_WARPS);
+  DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_fwd<KT>, gridA, GNEP_WARPS * 32, smem_radial(d), d, h->N, h->type_s, h->segR, h->pairR, h->theta, h->q, h->M1));
+  mark(h, "a1_radial_descriptor");
+  DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_fwd<KT>, gridA, GNEP_WARPS * 32, smem_ang_fwd(d), d, h->N, h->type_s, h->rowAs, h->pairA, h->theta, h->q, h->Sn));
+  mark(h, "a1_angular_descriptor");
+  return GNEP_OK;
+}
+
+LossCfg loss_cfg(const gnep_handle *h) {
+  LossCfg lc;
+  lc.S = h->S; lc.N = h->N; lc.T = h->ds.T; lc.P = h->ds.P;
+  lc.hasE = h->hasE; lc.hasF = h->hasF; lc.hasV = h->hasV; lc.loss_mode = h->ds.loss_mode;
+  lc.lam_e = h->spec.lambda_e; lc.lam_f = h->spec.lambda_f; lc.lam_v = h->spec.lambda_v; lc.lam_2 = h->spec.lambda_2;
+  return lc;
+}
+
+int enqueue_forward(gnep_handle *h) {
+  const DevSpec &d = h->ds;
+  int gridA = cdiv(h->N, GNEP_WARPS);
+  RET_IF(enqueue_descriptors(h));
+  LAUNCH(h, k_net_fwd, h->n_cta_net, GNEP_WARPS * 32, smem_net_fwd(d), d, h->sm, h->theta, h->qscale, h->q, h->x, h->Ei, h->Ep, h->etil);
+  mark(h, "a2_network_forward");
+  DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_force<KT>, gridA, GNEP_WARPS * 32, 0, d, h->N, h->type_s, h->segR, h->pairR, h->etil, h->Fat, h->Wat));
+  mark(h, "a3_radial_force");
+  DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_force<KT>, gridA, GNEP_WARPS * 32, smem_ang_force(d), d, h->N, h->type_s, h->rowAs, h->pairA, h->theta, h->Ep, h->Sn, h->fpair, h->Fat, h->Wat));
+  mark(h, "a3_angular_force");
+  LAUNCH(h, k_force_gather, gridA, GNEP_WARPS * 32, 0, h->N, h->rowAs, h->revA, h->fpair, h->Fat);
+  mark(h, "a3_force_gather");
+  LAUNCH(h, k_struct_reduce, h->S, 128, 0, loss_cfg(h), h->srange, h->Ei, h->Fat, h->Wat, h->Eref, h->Fref_s, h->Wref, h->Es, h->Ws, h->e_s, h->u, h->omega, h->parts);
+  LAUNCH(h, k_loss_final, 1, 256, 0, loss_cfg(h), h->parts, h->theta, h->terms, h->scales);
+  mark(h, "a4_loss_and_seeds");
+  return GNEP_OK;
+}
+
+// ---- the backward half (rows a5-a8) ----------------------------------------------------------------
+int enqueue_backward(gnep_handle *h) {
+  const DevSpec &d = h->ds;
+  int gridA = cdiv(h->N, GNEP_WARPS);
+  DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_adj<KT>, gridA, GNEP_WARPS * 32, smem_radial(d), d, h->N, h->type_s, h->struct_s, h->segR, h->pairR, h->theta, h->u, h->omega, h->scales, h->D, h->M2));
+  mark(h, "a5_radial_adjoint");
+  DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_adj<KT>, gridA, GNEP_WARPS * 32, smem_ang_adj(d), d, h->N, h->type_s, h->struct_s, h->rowAs, h->pairA, h->theta, h->u, h->omega, h->scales, h->Sn, h->Tn, h->D));
+  mark(h, "a5_angular_adjoint");
+  LAUNCH(h, k_net_bwd, h->n_cta_net, GNEP_WARPS * 32, smem_net_bwd(d), d, h->sm, h->theta, h->qscale, h->struct_s, h->e_s, h->scales, h->x, h->Ep, h->D, h->Acoef, h->Bcoef, h->gbar, h->partialB);
+  mark(h, "a6_network_backward");
+  LAUNCH(h, k_gemm_w0, h->n_chunks, 256, smem_gemm_w0(d), d, h->sm, h->qscale, h->q, h->D, h->Acoef, h->Bcoef, h->partialW);
+  mark(h, "a6_w0_gradient");
+  LAUNCH(h, k_cgrad_radial, h->n_chunks, 256, smem_cgrad_rad(d), d, h->sm, h->gbar, h->Ep, h->M1, h->M2, h->partialCR);
+  mark(h, "a7_radial_cgrad");
+  DISPATCH_KT(d.KAp, LAUNCH(h, k_cgrad_angular<KT>, h->n_ca_blocks, GNEP_WARPS * 32, smem_cgrad_ang(d), d, h->N, h->type_s, h->struct_s, h->rowAs, h->pairA, h->u, h->omega, h->scales, h->Ep, h->gbar, h->Sn, h->Tn, h->partialCA));
+  mark(h, "a7_angular_cgrad");
+  LAUNCH(h, k_grad_reduce, cdiv(d.P, 256), 256, 0, d, h->rm, h->theta, h->scales, h->partialCR, h->partialCA, h->partialW, h->partialB, h->grad);
+  mark(h, "a8_grad_reduce");
+  return GNEP_OK;
+}
+
+int enqueue_adam(gnep_handle *h, float lr, float b1, float b2, float eps) {
+  LAUNCH(h, k_adam, cdiv(h->ds.P, 256), 256, 0, h->ds.P, h->theta, h->m, h->v, h->grad, h->step_dev, lr, b1, b2, eps);
+  LAUNCH(h, k_step_inc, 1, 1, 0, h->step_dev);
+  mark(h, "a9_adam");
+  return GNEP_OK;
+}
+
+int check_launch(gnep_handle *h) {
+  CK(cudaGetLastError());
+  return GNEP_OK;
+}
+
+// copy helper: caller buffer <-> device
+int copy_in(gnep_handle *h, void *dst, const void *src, size_t bytes, int is_device) {
+  CK(cudaMemcpyAsync(dst, src, bytes, is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, h->stream));
+  if (!is_device) CK(cudaStreamSynchronize(h->stream));   // pageable host memory may be reused by the caller
+  return GNEP_OK;
+}
+int copy_out(const gnep_handle *hc, void *dst, const void *src, size_t bytes, int is_device) {
+  gnep_handle *h = const_cast<gnep_handle *>(hc);
+  CK(cudaMemcpyAsync(dst, src, bytes, is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return GNEP_OK;
+}
+
+int fetch_terms(gnep_handle *h, float *loss_terms) {
+  CK(cudaMemcpyAsync(h->h_terms, h->terms, 5 * sizeof(float), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  prof_collect(h);
+  for (int i = 0; i < 5; ++i) loss_terms[i] = h->h_terms[i];
+  if (!std::isfinite(loss_terms[0])) return fail(h, GNEP_ENONFINITE, "loss is not finite");
+  return GNEP_OK;
+}
+
+struct HostGeo { double h[3]; };
+
+int cell_geometry(const double *c, double *inv, double *hh) {
+  const double *a = c, *b = c + 3, *cc = c + 6;
+  auto cross = [](const double *u, const double *v, double *o) {
+    o[0] = u[1] * v[2] - u[2] * v[1]; o[1] = u[2] * v[0] - u[0] * v[2]; o[2] = u[0] * v[1] - u[1] * v[0];
+  };
+  auto dot = [](const double *u, const double *v) { return u[0] * v[0] + u[1] * v[1] + u[2] * v[2]; };
+  double bxc[3], cxa[3], axb[3];
+  cross(b, cc, bxc); cross(cc, a, cxa); cross(a, b, axb);
+  double V = dot(a, bxc);
+  if (!(std::fabs(V) > 0.0) || !std::isfinite(V)) return -1;
+  hh[0] = std::fabs(V) / std::sqrt(dot(bxc, bxc));
+  hh[1] = std::fabs(V) / std::sqrt(dot(cxa, cxa));
+  hh[2] = std::fabs(V) / std::sqrt(dot(axb, axb));
+  for (int k = 0; k < 3; ++k) { inv[k] = bxc[k] / V; inv[3 + k] = cxa[k] / V; inv[6 + k] = axb[k] / V; }
+  return 0;
+}
+
+}  // namespace
+
+// ====================================================================================================
+extern "C" {
+
+const char *gnep_last_error(const gnep_handle *h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+int gnep_create(const gnep_model_spec *spec, void *cuda_stream, gnep_handle **out) {
+  gnep_handle *h = nullptr;   // errors before the handle exists go to the thread-local string
+  if (!spec || !out) return fail(h, GNEP_EINVAL, "null spec or out");
+  *out = nullptr;
+  const gnep_model_spec &s = *spec;
+  if (s.n_species < 1 || s.n_species > GNEP_MAX_SPECIES) return fail(h, GNEP_EINVAL, "n_species out of range");
+  if (s.n_radial < 1 || s.n_radial > GNEP_MAX_NFUNC || s.n_angular < 1 || s.n_angular > GNEP_MAX_NFUNC)
+    return fail(h, GNEP_EINVAL, "n_radial / n_angular out of range");
+  if (s.n_basis_radial < 1 || s.n_basis_radial > GNEP_MAX_BASIS || s.n_basis_angular < 1 || s.n_basis_angular > GNEP_MAX_BASIS)
+    return fail(h, GNEP_EINVAL, "basis size out of range");
+  if (!(s.rc_radial > 0) || !(s.rc_angular > 0) || s.rc_angular > s.rc_radial) return fail(h, GNEP_EINVAL, "need 0 < rc_angular <= rc_radial");
+  if (s.l_max < 1 || s.l_max > 4) return fail(h, GNEP_EINVAL, "l_max must be 1..4");
+  if (s.use_4body && s.l_max < 2) return fail(h, GNEP_EINVAL, "use_4body needs l_max >= 2");
+  if (s.n_neurons < 1 || s.n_neurons > GNEP_MAX_NEURONS) return fail(h, GNEP_EINVAL, "n_neurons out of range");
+  if (s.loss_mode != 0 && s.loss_mode != 1) return fail(h, GNEP_EINVAL, "loss_mode must be 0 or 1");
+  if (s.lambda_e < 0 || s.lambda_f < 0 || s.lambda_v < 0 || s.lambda_2 < 0) return fail(h, GNEP_EINVAL, "negative loss weight");
+  int dev = 0;
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+    cudaGetLastError();
+    return fail(h, GNEP_ECUDA, "no CUDA device (this library has no CPU fallback)");
+  }
+  if (prop.major != 10) return fail(h, GNEP_ECUDA, "device is not compute capability 10.x (built for sm_100a only)");
+  h = new (std::nothrow) gnep_handle();
+  if (!h) return fail(nullptr, GNEP_ENOMEM, "out of host memory");
+  h->spec = s; h->spec.q_scale = nullptr;
+  h->device = dev; h->num_sms = prop.multiProcessorCount;
+  DevSpec &d = h->ds;
+  d.T = s.n_species; d.NR = s.n_radial; d.KR = s.n_basis_radial; d.NA = s.n_angular; d.KA = s.n_basis_angular;
+  d.L = s.l_max; d.use4 = s.use_4body ? 1 : 0; d.Nn = s.n_neurons;
+  d.Ndes = d.NR + d.NA * d.L + (d.use4 ? d.NA : 0);
+  d.KRp = padded_basis(d.KR); d.KAp = padded_basis(d.KA);
+  d.offA = d.T * d.T * d.NR * d.KR;
+  d.offNet = d.offA + d.T * d.T * d.NA * d.KA;
+  d.netSize = d.Nn * d.Ndes + 2 * d.Nn + 1;
+  d.P = d.offNet + d.T * d.netSize;
+  d.ldW = d.Ndes | 1;
+  d.loss_mode = s.loss_mode;
+  d.rcRinv = (float)(1.0 / s.rc_radial); d.rcAinv = (float)(1.0 / s.rc_angular);
+  d.lam_e = (float)s.lambda_e; d.lam_f = (float)s.lambda_f; d.lam_v = (float)s.lambda_v; d.lam_2 = (float)s.lambda_2;
+  auto bail = [&](int rc) { std::string e = h->err; gnep_destroy(h); g_create_error = e; return rc; };
+  if (cuda_stream) h->stream = (cudaStream_t)cuda_stream;
+  else {
+    if (cudaStreamCreate(&h->stream) != cudaSuccess) { h->err = "cudaStreamCreate failed"; return bail(GNEP_ECUDA); }
+    h->own_stream = true;
+  }
+  int rc;
+  if ((rc = configure_kernels(h)) != GNEP_OK) return bail(rc);
+  // constants: 2 C_lm with C_lm = (2l+1)/(4 pi) Chat_lm (R11-R12), kappa4 (R14)
+  {
+    const double chat[GNEP_NLM] = {1, 1, 1, 1.0 / 4, 3, 3, 3.0 / 4, 3.0 / 4, 1.0 / 4, 3.0 / 8, 3.0 / 8, 15.0 / 4, 15.0 / 4, 5.0 / 8,
+                                   5.0 / 8, 1.0 / 64, 5.0 / 8, 5.0 / 8, 5.0 / 16, 5.0 / 16, 35.0 / 8, 35.0 / 8, 35.0 / 64, 35.0 / 64};
+    float c2[GNEP_NLM], lf[GNEP_NLM];
+    const double pi = 3.14159265358979323846;
+    for (int lm = 0; lm < GNEP_NLM; ++lm) {
+      int l = lm < 3 ? 1 : lm < 8 ? 2 : lm < 15 ? 3 : 4;
+      lf[lm] = (float)l;
+      c2[lm] = l <= d.L ? (float)(2.0 * (2 * l + 1) / (4.0 * pi) * chat[lm]) : 0.f;
+    }
+    float k4 = (float)(-5.0 * std::sqrt(14.0) / (448.0 * pi * std::sqrt(pi)));
+    if (cudaMemcpyToSymbol(c_C2, c2, sizeof(c2)) != cudaSuccess || cudaMemcpyToSymbol(c_lf, lf, sizeof(lf)) != cudaSuccess ||
+        cudaMemcpyToSymbol(c_kappa4, &k4, sizeof(k4)) != cudaSuccess) { h->err = "cudaMemcpyToSymbol failed"; return bail(GNEP_ECUDA); }
+  }
+  if ((rc = dalloc(h, &h->theta, d.P, false)) || (rc = dalloc(h, &h->grad, d.P, false)) || (rc = dalloc(h, &h->m, d.P, false)) ||
+      (rc = dalloc(h, &h->v, d.P, false)) || (rc = dalloc(h, &h->qscale, d.Ndes, false)) || (rc = dalloc(h, &h->step_dev, 1, false)) ||
+      (rc = dalloc(h, &h->terms, 8, false)) || (rc = dalloc(h, &h->scales, 4, false)))
+    return bail(rc);
+  if (cudaMallocHost((void **)&h->h_terms, 8 * sizeof(float)) != cudaSuccess) { h->err = "cudaMallocHost failed"; return bail(GNEP_ENOMEM); }
+  std::vector<float> qs(d.Ndes, 1.f);
+  if (s.q_scale) for (int i = 0; i < d.Ndes; ++i) qs[i] = s.q_scale[i];
+  float ones[4] = {1.f, 1.f, 1.f, 1.f};
+  if (cudaMemsetAsync(h->theta, 0, d.P * sizeof(float), h->stream) != cudaSuccess ||
+      cudaMemsetAsync(h->grad, 0, d.P * sizeof(float), h->stream) != cudaSuccess ||
+      cudaMemsetAsync(h->m, 0, d.P * sizeof(float), h->stream) != cudaSuccess ||
+      cudaMemsetAsync(h->v, 0, d.P * sizeof(float), h->stream) != cudaSuccess ||
+      cudaMemsetAsync(h->step_dev, 0, sizeof(long long), h->stream) != cudaSuccess ||
+      cudaMemsetAsync(h->terms, 0, 8 * sizeof(float), h->stream) != cudaSuccess ||
+      cudaMemcpyAsync(h->scales, ones, sizeof(ones), cudaMemcpyHostToDevice, h->stream) != cudaSuccess ||
+      cudaMemcpyAsync(h->qscale, qs.data(), d.Ndes * sizeof(float), cudaMemcpyHostToDevice, h->stream) != cudaSuccess ||
+      cudaStreamSynchronize(h->stream) != cudaSuccess) { h->err = "initialisation copies failed"; return bail(GNEP_ECUDA); }
+  *out = h;
+  return GNEP_OK;
+}
+
+int gnep_destroy(gnep_handle *h) {
+  if (!h) return GNEP_OK;
+  if (h->stream) cudaStreamSynchronize(h->stream);
+  free_batch(h);
+  for (auto &p : h->phases) cudaEventDestroy(p.ev);
+  cudaFree(h->theta); cudaFree(h->grad); cudaFree(h->m); cudaFree(h->v); cudaFree(h->qscale); cudaFree(h->step_dev);
+  cudaFree(h->terms); cudaFree(h->scales);
+  if (h->h_terms) cudaFreeHost(h->h_terms);
+  if (h->own_stream && h->stream) cudaStreamDestroy(h->stream);
+  delete h;
+  return GNEP_OK;
+}
+
+int gnep_num_params(const gnep_handle *h, int64_t *P) {
+  if (!h || !P) return fail(h, GNEP_EINVAL, "null argument");
+  *P = h->ds.P;
+  return GNEP_OK;
+}
+int gnep_num_descriptors(const gnep_handle *h, int32_t *n) {
+  if (!h || !n) return fail(h, GNEP_EINVAL, "null argument");
+  *n = h->ds.Ndes;
+  return GNEP_OK;
+}
+
+int gnep_set_params(gnep_handle *h, const float *theta, int is_device) {
+  if (!h || !theta) return fail(h, GNEP_EINVAL, "null argument");
+  return copy_in(h, h->theta, theta, h->ds.P * sizeof(float), is_device);
+}
+int gnep_get_params(const gnep_handle *h, float *theta, int is_device) {
+  if (!h || !theta) return fail(h, GNEP_EINVAL, "null argument");
+  return copy_out(h, theta, h->theta, h->ds.P * sizeof(float), is_device);
+}
+int gnep_set_q_scale(gnep_handle *h, const float *q_scale) {
+  if (!h || !q_scale) return fail(h, GNEP_EINVAL, "null argument");
+  for (int i = 0; i < h->ds.Ndes; ++i)
+    if (!std::isfinite(q_scale[i])) return fail(h, GNEP_EINVAL, "q_scale not finite");
+  return copy_in(h, h->qscale, q_scale, h->ds.Ndes * sizeof(float), 0);
+}
+
+int gnep_get_opt_state(const gnep_handle *h, float *m, float *v, int64_t *step, int is_device) {
+  if (!h) return fail(h, GNEP_EINVAL, "null handle");
+  if (m) RET_IF(copy_out(h, m, h->m, h->ds.P * sizeof(float), is_device));
+  if (v) RET_IF(copy_out(h, v, h->v, h->ds.P * sizeof(float), is_device));
+  if (step) { long long s = 0; RET_IF(copy_out(h, &s, h->step_dev, sizeof(s), 0)); *step = s; }
+  return GNEP_OK;
+}
+int gnep_set_opt_state(gnep_handle *h, const float *m, const float *v, int64_t step, int is_device) {
+  if (!h || step < 0) return fail(h, GNEP_EINVAL, "null handle or negative step");
+  if (m) RET_IF(copy_in(h, h->m, m, h->ds.P * sizeof(float), is_device));
+  if (v) RET_IF(copy_in(h, h->v, v, h->ds.P * sizeof(float), is_device));
+  long long s = step;
+  return copy_in(h, h->step_dev, &s, sizeof(s), 0);
+}
+
+int gnep_set_targets(gnep_handle *h, const double *E, const double *F, const double *W, int is_device) {
+  if (!h) return fail(h, GNEP_EINVAL, "null handle");
+  if (!h->loaded) return fail(h, GNEP_ESTATE, "no batch loaded");
+  h->hasE = E != nullptr; h->hasF = F != nullptr; h->hasV = W != nullptr;
+  if (E && h->S) RET_IF(copy_in(h, h->Eref, E, h->S * sizeof(double), is_device));
+  if (W && h->S) RET_IF(copy_in(h, h->Wref, W, (size_t)h->S * 6 * sizeof(double), is_device));
+  if (F && h->N) {
+    double *tmp = nullptr;
+    const double *src = F;
+    if (!is_device) {
+      CK(cudaMalloc((void **)&tmp, (size_t)h->N * 3 * sizeof(double)));
+      cudaError_t e = cudaMemcpyAsync(tmp, F, (size_t)h->N * 3 * sizeof(double), cudaMemcpyHostToDevice, h->stream);
+      if (e != cudaSuccess) { cudaFree(tmp); return fail(h, GNEP_ECUDA, cudaGetErrorString(e)); }
+      src = tmp;
+    }
+    LAUNCH(h, k_permute_fref, cdiv(h->N, 256), 256, 0, h->N, h->perm, src, h->Fref_s);
+    cudaError_t e = cudaStreamSynchronize(h->stream);
+    if (tmp) cudaFree(tmp);
+    if (e != cudaSuccess) return fail(h, GNEP_ECUDA, cudaGetErrorString(e));
+  }
+  if (h->graph) { cudaGraphExecDestroy(h->graph); h->graph = nullptr; }   // hasE/F/V are baked into the graph
+  return GNEP_OK;
+}
+
+int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double *pos, const double *cells,
+                    const int32_t *types, const double *Eref, const double *Fref, const double *Wref, int is_device) {
+  if (!h) return fail(h, GNEP_EINVAL, "null handle");
+  if (S < 0 || !aoff) return fail(h, GNEP_EINVAL, "bad n_structs / atom_offsets");
+  if (aoff[0] != 0) return fail(h, GNEP_EINVAL, "atom_offsets[0] must be 0");
+  for (int s = 0; s < S; ++s) if (aoff[s + 1] < aoff[s]) return fail(h, GNEP_EINVAL, "atom_offsets not ascending");
+  const int N = aoff[S];
+  if (N > 0 && (!pos || !cells || !types)) return fail(h, GNEP_EINVAL, "null positions / cells / types");
+  CK(cudaStreamSynchronize(h->stream));
+  free_batch(h);
+  const DevSpec &d = h->ds;
+  const int T = d.T;
+  try {
+    // ---- host copies of the small arrays ----
+    std::vector<double> hcell((size_t)S * 9);
+    std::vector<int> htype(N);
+    if (S) CK(cudaMemcpy(hcell.data(), cells, hcell.size() * sizeof(double), is_device ? cudaMemcpyDeviceToHost : cudaMemcpyHostToHost));
+    if (N) CK(cudaMemcpy(htype.data(), types, (size_t)N * sizeof(int), is_device ? cudaMemcpyDeviceToHost : cudaMemcpyHostToHost));
+    for (int i = 0; i < N; ++i) if (htype[i] < 0 || htype[i] >= T) return fail(h, GNEP_ERANGE, "species id out of range");
+    // ---- per-structure geometry and bins ----
+    std::vector<StructGeo> geo(S);
+    std::vector<int> struct_of(N);
+    int total_bins = 0;
+    const double rc = h->spec.rc_radial;
+    for (int s = 0; s < S; ++s) {
+      StructGeo &g = geo[s];
+      double hh[3];
+      memcpy(g.cell, &hcell[(size_t)s * 9], 9 * sizeof(double));
+      if (cell_geometry(g.cell, g.inv, hh)) return fail(h, GNEP_ERANGE, "degenerate cell (zero volume)");
+      for (int a = 0; a < 3; ++a) g.nb[a] = std::max(1, (int)std::floor(hh[a] / rc));
+      while ((int64_t)g.nb[0] * g.nb[1] * g.nb[2] > 4096) {
+        int big = g.nb[0] >= g.nb[1] && g.nb[0] >= g.nb[2] ? 0 : (g.nb[1] >= g.nb[2] ? 1 : 2);
+        g.nb[big] = (g.nb[big] + 1) / 2;
+      }
+      for (int a = 0; a < 3; ++a) {
+        g.m[a] = std::max(1, (int)std::ceil(rc * g.nb[a] / hh[a]));
+        if (g.m[a] > 127) return fail(h, GNEP_ERANGE, "cell much smaller than the cutoff (more than 127 images per axis)");
+      }
+      g.bin_base = total_bins;
+      total_bins += g.nb[0] * g.nb[1] * g.nb[2];
+      g.a0 = aoff[s]; g.a1 = aoff[s + 1];
+      for (int i = g.a0; i < g.a1; ++i) struct_of[i] = s;
+    }
+    // ---- species sort (stable) ----
+    std::vector<int> perm(N), inv(N), type_s(N), struct_s(N);
+    {
+      std::vector<int> cnt(T + 1, 0);
+      for (int i = 0; i < N; ++i) cnt[htype[i] + 1]++;
+      for (int t = 0; t < T; ++t) cnt[t + 1] += cnt[t];
+      for (int t = 0; t <= GNEP_MAX_SPECIES_C; ++t) h->sm.start[t] = cnt[std::min(t, T)];
+      std::vector<int> cur(cnt.begin(), cnt.end() - 1);
+      for (int i = 0; i < N; ++i) { int a = cur[htype[i]]++; perm[a] = i; inv[i] = a; }
+      for (int a = 0; a < N; ++a) { type_s[a] = htype[perm[a]]; struct_s[a] = struct_of[perm[a]]; }
+    }
+    std::vector<int> srange((size_t)std::max(S, 1) * T * 2, 0);
+    {
+      std::vector<int> run(T);
+      for (int t = 0; t < T; ++t) run[t] = h->sm.start[t];
+      for (int s = 0; s < S; ++s) {
+        std::vector<int> c(T, 0);
+        for (int i = aoff[s]; i < aoff[s + 1]; ++i) c[htype[i]]++;
+        for (int t = 0; t < T; ++t) { srange[((size_t)s * T + t) * 2] = run[t]; run[t] += c[t]; srange[((size_t)s * T + t) * 2 + 1] = run[t]; }
+      }
+    }
+    h->N = N; h->S = S;
+    // ---- device inputs ----
+    double *d_pos_in = nullptr; bool own_pos = false;
+    if (N) {
+      if (is_device) d_pos_in = const_cast<double *>(pos);
+      else { CK(cudaMalloc((void **)&d_pos_in, (size_t)N * 3 * sizeof(double))); own_pos = true;
+             CK(cudaMemcpy(d_pos_in, pos, (size_t)N * 3 * sizeof(double), cudaMemcpyHostToDevice)); }
+    }
+    std::vector<void *> tmp;
+    auto talloc = [&](void **p, size_t bytes) -> cudaError_t { cudaError_t e = cudaMalloc(p, std::max<size_t>(bytes, 16)); if (e == cudaSuccess) tmp.push_back(*p); return e; };
+    auto tfree = [&]() { for (void *p : tmp) cudaFree(p); tmp.clear(); if (own_pos) { cudaFree(d_pos_in); own_pos = false; } };
+#define CKT(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { tfree(); free_batch(h); return fail(h, e_ == cudaErrorMemoryAllocation ? GNEP_ENOMEM : GNEP_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); } } while (0)
+    StructGeo *d_geo; int *d_struct_of, *d_type, *d_inv, *d_binid, *d_bin_count, *d_bin_start, *d_bin_cursor, *d_bin_atoms, *d_cntR, *d_cntA;
+    double *d_wpos;
+    CKT(talloc((void **)&d_geo, sizeof(StructGeo) * S)); CKT(talloc((void **)&d_struct_of, sizeof(int) * N));
+    CKT(talloc((void **)&d_type, sizeof(int) * N)); CKT(talloc((void **)&d_inv, sizeof(int) * N));
+    CKT(talloc((void **)&d_binid, sizeof(int) * N)); CKT(talloc((void **)&d_bin_count, sizeof(int) * (total_bins + 1)));
+    CKT(talloc((void **)&d_bin_start, sizeof(int) * (total_bins + 1))); CKT(talloc((void **)&d_bin_cursor, sizeof(int) * (total_bins + 1)));
+    CKT(talloc((void **)&d_bin_atoms, sizeof(int) * N)); CKT(talloc((void **)&d_cntR, sizeof(int) * N)); CKT(talloc((void **)&d_cntA, sizeof(int) * N));
+    CKT(talloc((void **)&d_wpos, sizeof(double) * 3 * N));
+    cudaStream_t st = h->stream;
+    if (S) CKT(cudaMemcpyAsync(d_geo, geo.data(), sizeof(StructGeo) * S, cudaMemcpyHostToDevice, st));
+    if (N) {
+      CKT(cudaMemcpyAsync(d_struct_of, struct_of.data(), sizeof(int) * N, cudaMemcpyHostToDevice, st));
+      CKT(cudaMemcpyAsync(d_type, htype.data(), sizeof(int) * N, cudaMemcpyHostToDevice, st));
+      CKT(cudaMemcpyAsync(d_inv, inv.data(), sizeof(int) * N, cudaMemcpyHostToDevice, st));
+    }
+    CKT(cudaMemsetAsync(d_bin_count, 0, sizeof(int) * (total_bins + 1), st));
+    CKT(cudaMemsetAsync(d_bin_cursor, 0, sizeof(int) * (total_bins + 1), st));
+    const int gN = cdiv(N, 128);
+    LAUNCH(h, k_wrap_bin, gN, 128, 0, N, d_struct_of, d_geo, d_pos_in, d_wpos, d_binid, d_bin_count);
+    std::vector<int> bins(total_bins + 1, 0);
+    CKT(cudaMemcpyAsync(bins.data(), d_bin_count, sizeof(int) * (total_bins + 1), cudaMemcpyDeviceToHost, st));
+    CKT(cudaStreamSynchronize(st));
+    { int run = 0; for (int b = 0; b <= total_bins; ++b) { int c = bins[b]; bins[b] = run; run += c; } }
+    CKT(cudaMemcpyAsync(d_bin_start, bins.data(), sizeof(int) * (total_bins + 1), cudaMemcpyHostToDevice, st));
+    LAUNCH(h, k_bin_fill, gN, 128, 0, N, d_binid, d_bin_start, d_bin_cursor, d_bin_atoms);
+    const double rcR2 = h->spec.rc_radial * h->spec.rc_radial, rcA2 = h->spec.rc_angular * h->spec.rc_angular;
+    LAUNCH(h, k_nbr_count, gN, 128, 0, N, d_struct_of, d_geo, d_wpos, d_binid, d_bin_start, d_bin_atoms, rcR2, rcA2, d_cntR, d_cntA);
+    std::vector<int> cR(N), cA(N);
+    if (N) {
+      CKT(cudaMemcpyAsync(cR.data(), d_cntR, sizeof(int) * N, cudaMemcpyDeviceToHost, st));
+      CKT(cudaMemcpyAsync(cA.data(), d_cntA, sizeof(int) * N, cudaMemcpyDeviceToHost, st));
+    }
+    CKT(cudaStreamSynchronize(st));
+    std::vector<int64_t> rowR(N + 1, 0), rowA(N + 1, 0);
+    for (int i = 0; i < N; ++i) { rowR[i + 1] = rowR[i] + cR[i]; rowA[i + 1] = rowA[i] + cA[i]; }
+    const int64_t nR = rowR[N], nA = rowA[N];
+    if (nR >= (int64_t)1 << 31) { tfree(); free_batch(h); return fail(h, GNEP_ERANGE, "2^31 or more radial pairs"); }
+    std::vector<int> rowRs(N + 1, 0), rowAs(N + 1, 0);
+    for (int a = 0; a < N; ++a) { rowRs[a + 1] = rowRs[a] + cR[perm[a]]; rowAs[a + 1] = rowAs[a] + cA[perm[a]]; }
+    h->nR = nR; h->nA = nA;
+    // ---- persistent batch arrays ----
+    int rc_;
+#define BA(ptr, n) if ((rc_ = dalloc(h, &(ptr), (n), true)) != GNEP_OK) { tfree(); free_batch(h); return rc_; }
+    BA(h->perm, N); BA(h->type_s, N); BA(h->struct_s, N); BA(h->segR, (size_t)N * (T + 1) + 1); BA(h->rowAs, N + 1); BA(h->revA, nA);
+    BA(h->pairR, nR); BA(h->pairA, nA);
+    BA(h->exp_row[0], N + 1); BA(h->exp_row[1], N + 1); BA(h->exp_j[0], nR); BA(h->exp_sh[0], nR); BA(h->exp_j[1], nA); BA(h->exp_sh[1], nA);
+    BA(h->srange, srange.size()); BA(h->Eref, S); BA(h->Wref, (size_t)S * 6); BA(h->Fref_s, (size_t)N * 3);
+    int *d_rowRs, *d_shA; unsigned long long *d_ekey; float *d_er;
+    CKT(talloc((void **)&d_rowRs, sizeof(int) * (N + 1))); CKT(talloc((void **)&d_shA, sizeof(int) * nA));
+    CKT(talloc((void **)&d_ekey, sizeof(unsigned long long) * nR)); CKT(talloc((void **)&d_er, sizeof(float) * 3 * nR));
+    CKT(cudaMemcpyAsync(h->exp_row[0], rowR.data(), sizeof(int64_t) * (N + 1), cudaMemcpyHostToDevice, st));
+    CKT(cudaMemcpyAsync(h->exp_row[1], rowA.data(), sizeof(int64_t) * (N + 1), cudaMemcpyHostToDevice, st));
+    CKT(cudaMemcpyAsync(d_rowRs, rowRs.data(), sizeof(int) * (N + 1), cudaMemcpyHostToDevice, st));
+    CKT(cudaMemcpyAsync(h->rowAs, rowAs.data(), sizeof(int) * (N + 1), cudaMemcpyHostToDevice, st));
+    if (N) {
+      CKT(cudaMemcpyAsync(h->perm, perm.data(), sizeof(int) * N, cudaMemcpyHostToDevice, st));
+      CKT(cudaMemcpyAsync(h->type_s, type_s.data(), sizeof(int) * N, cudaMemcpyHostToDevice, st));
+      CKT(cudaMemcpyAsync(h->struct_s, struct_s.data(), sizeof(int) * N, cudaMemcpyHostToDevice, st));
+    }
+    CKT(cudaMemcpyAsync(h->srange, srange.data(), sizeof(int) * srange.size(), cudaMemcpyHostToDevice, st));
+    LAUNCH(h, k_nbr_fill, gN, 128, 0, N, d_struct_of, d_geo, d_wpos, d_binid, d_bin_start, d_bin_atoms, rcR2, rcA2, h->exp_row[0], d_ekey, d_er);
+    LAUNCH(h, k_nbr_scatter, cdiv((int64_t)N * 32, 256), 256, 0, N, T, d_struct_of, d_geo, d_type, d_inv, h->exp_row[0], h->exp_row[1], d_rowRs,
+           h->rowAs, d_ekey, d_er, h->exp_j[0], h->exp_sh[0], h->exp_j[1], h->exp_sh[1], h->pairR, h->pairA, d_shA, h->segR);
+    LAUNCH(h, k_nbr_reverse, cdiv((int64_t)N * 32, 256), 256, 0, N, h->rowAs, h->pairA, d_shA, h->revA);
+    CKT(cudaGetLastError());
+    CKT(cudaStreamSynchronize(st));
+    tfree();
+    // ---- work decomposition of the network / gradient kernels ----
+    const int per_cta = GNEP_WARPS * GNEP_TILE;
+    h->sm.cta_base[0] = 0; h->sm.chunk_base[0] = 0;
+    for (int t = 0; t < GNEP_MAX_SPECIES_C; ++t) {
+      int nt = t < T ? h->sm.start[t + 1] - h->sm.start[t] : 0;
+      h->sm.cta_base[t + 1] = h->sm.cta_base[t] + cdiv(nt, per_cta);
+      int want = nt > 0 ? std::max(1, std::min(cdiv(nt, 256), (int)((2.0 * h->num_sms * nt) / std::max(N, 1) + 0.5))) : 0;
+      int ca = want > 0 ? ((cdiv(nt, want) + 31) / 32) * 32 : 32;
+      h->sm.chunk_atoms[t] = ca;
+      h->sm.chunk_base[t + 1] = h->sm.chunk_base[t] + (nt > 0 ? cdiv(nt, ca) : 0);
+    }
+    h->n_cta_net = h->sm.cta_base[GNEP_MAX_SPECIES_C];
+    h->n_chunks = h->sm.chunk_base[GNEP_MAX_SPECIES_C];
+    h->n_ca_blocks = std::max(1, std::min(cdiv(N, GNEP_WARPS), 2 * h->num_sms));
+    for (int t = 0; t <= GNEP_MAX_SPECIES_C; ++t) { h->rm.chunk_base[t] = h->sm.chunk_base[t]; h->rm.cta_base[t] = h->sm.cta_base[t]; }
+    h->rm.n_warps_ca = N > 0 ? h->n_ca_blocks * GNEP_WARPS : 0;
+    // ---- per-atom state ----
+    const size_t n = N;
+    BA(h->q, n * d.Ndes); BA(h->Sn, n * d.NA * GNEP_NLM); BA(h->x, n * d.Nn); BA(h->Ei, n); BA(h->Ep, n * d.Ndes);
+    BA(h->etil, n * T * d.KRp); BA(h->M1, n * T * d.KRp); BA(h->M2, n * T * d.KRp); BA(h->D, n * d.Ndes); BA(h->Tn, n * d.NA * GNEP_NLM);
+    BA(h->gbar, n * d.Ndes); BA(h->Acoef, n * d.Nn); BA(h->Bcoef, n * d.Nn); BA(h->Wat, n * 6);
+    BA(h->Fat, n); BA(h->fpair, nA); BA(h->u, n);
+    BA(h->Es, S); BA(h->Ws, (size_t)S * 6); BA(h->parts, (size_t)S * 3); BA(h->e_s, S); BA(h->omega, (size_t)S * 6);
+    BA(h->partialCR, (size_t)std::max(h->n_chunks, 1) * d.NR * T * d.KRp);
+    BA(h->partialCA, (size_t)std::max(h->rm.n_warps_ca, 1) * T * T * d.NA * d.KAp);
+    BA(h->partialW, (size_t)std::max(h->n_chunks, 1) * d.Nn * d.Ndes);
+    BA(h->partialB, (size_t)std::max(h->n_cta_net, 1) * (2 * d.Nn + 1));
+#undef BA
+#undef CKT
+    h->loaded = true;
+    return gnep_set_targets(h, Eref, Fref, Wref, is_device);
+  } catch (const std::bad_alloc &) {
+    free_batch(h);
+    return fail(h, GNEP_ENOMEM, "out of host memory");
+  }
+}
+
+int gnep_batch_info(const gnep_handle *h, int64_t *n_atoms, int64_t *n_structs, int64_t *nR, int64_t *nA) {
+  if (!h) return fail(h, GNEP_EINVAL, "null handle");
+  if (!h->loaded) return fail(h, GNEP_ESTATE, "no batch loaded");
+  if (n_atoms) *n_atoms = h->N;
+  if (n_structs) *n_structs = h->S;
+  if (nR) *nR = h->nR;
+  if (nA) *nA = h->nA;
+  return GNEP_OK;
+}
+
+int gnep_neighbor_list(const gnep_handle *h, int which, int64_t *n_pairs, int64_t *row_ptr, int32_t *j, int8_t *shift3,
+                       int64_t capacity, int is_device) {
+  if (!h || (which != 0 && which != 1)) return fail(h, GNEP_EINVAL, "bad argument");
+  if (!h->loaded) return fail(h, GNEP_ESTATE, "no batch loaded");
+  const int64_t np = which == 0 ? h->nR : h->nA;
+  if (n_pairs) *n_pairs = np;
+  if ((j || shift3) && capacity < np) return fail(h, GNEP_EINVAL, "capacity smaller than the pair count");
+  if (row_ptr) RET_IF(copy_out(h, row_ptr, h->exp_row[which], (size_t)(h->N + 1) * sizeof(int64_t), is_device));
+  if (j && np) RET_IF(copy_out(h, j, h->exp_j[which], (size_t)np * sizeof(int32_t), is_device));
+  if (shift3 && np) {
+    std::vector<int> packed(np);
+    RET_IF(copy_out(h, packed.data(), h->exp_sh[which], (size_t)np * sizeof(int), 0));
+    std::vector<int8_t> sh((size_t)np * 3);
+    for (int64_t p = 0; p < np; ++p) {
+      sh[3 * p] = (int8_t)(((packed[p] >> 16) & 255) - 128);
+      sh[3 * p + 1] = (int8_t)(((packed[p] >> 8) & 255) - 128);
+      sh[3 * p + 2] = (int8_t)((packed[p] & 255) - 128);
+    }
+    if (is_device) { gnep_handle *hh = const_cast<gnep_handle *>(h); return copy_in(hh, shift3, sh.data(), sh.size(), 0); }
+    memcpy(shift3, sh.data(), sh.size());
+  }
+  return GNEP_OK;
+}
+
+int gnep_descriptors(gnep_handle *h, float *q, int is_device) {
+  if (!h || !q) return fail(h, GNEP_EINVAL, "null argument");
+  if (!h->loaded) return fail(h, GNEP_ESTATE, "no batch loaded");
+  if (h->N == 0) return GNEP_OK;
+  RET_IF(enqueue_descriptors(h));
+  const size_t n = (size_t)h->N * h->ds.Ndes;
+  float *dst = q; float *tmp = nullptr;
+  if (!is_device) { CK(cudaMalloc((void **)&tmp, n * sizeof(float))); dst = tmp; }
+  LAUNCH(h, k_unpermute_rows, cdiv(n, 256), 256, 0, h->N, h->ds.Ndes, h->perm, h->q, dst);
+  int rc = check_launch(h);
+  if (rc == GNEP_OK && tmp) rc = copy_out(h, q, tmp, n * sizeof(float), 0);
+  else if (rc == GNEP_OK) { cudaError_t e = cudaStreamSynchronize(h->stream); if (e != cudaSuccess) rc = fail(h, GNEP_ECUDA, cudaGetErrorString(e)); }
+  if (tmp) cudaFree(tmp);
+  return rc;
+}
+
+int gnep_predict(gnep_handle *h, float *energy, float *force, float *virial, int is_device) {
+  if (!h) return fail(h, GNEP_EINVAL, "null handle");
+  if (!h->loaded) return fail(h, GNEP_ESTATE, "no batch loaded");
+  if (h->N > 0 || h->S > 0) { RET_IF(enqueue_forward(h)); RET_IF(check_launch(h)); }
+  std::vector<void *> tmp;
+  auto run = [&]() -> int {
+    if (energy && h->S) {
+      float *dst = energy;
+      if (!is_device) { CK(cudaMalloc((void **)&dst, h->S * sizeof(float))); tmp.push_back(dst); }
+      LAUNCH(h, k_d2f, cdiv(h->S, 256), 256, 0, h->S, h->Es, dst);
+      if (!is_device) RET_IF(copy_out(h, energy, dst, h->S * sizeof(float), 0));
+    }
+    if (virial && h->S) {
+      float *dst = virial;
+      if (!is_device) { CK(cudaMalloc((void **)&dst, (size_t)h->S * 6 * sizeof(float))); tmp.push_back(dst); }
+      LAUNCH(h, k_d2f, cdiv(h->S * 6, 256), 256, 0, h->S * 6, h->Ws, dst);
+      if (!is_device) RET_IF(copy_out(h, virial, dst, (size_t)h->S * 6 * sizeof(float), 0));
+    }
+    if (force && h->N) {
+      float *dst = force;
+      if (!is_device) { CK(cudaMalloc((void **)&dst, (size_t)h->N * 3 * sizeof(float))); tmp.push_back(dst); }
+      LAUNCH(h, k_unpermute_force, cdiv(h->N, 256), 256, 0, h->N, h->perm, h->Fat, dst);
+      if (!is_device) RET_IF(copy_out(h, force, dst, (size_t)h->N * 3 * sizeof(float), 0));
+    }
+    RET_IF(check_launch(h));
+    CK(cudaStreamSynchronize(h->stream));
+    return GNEP_OK;
+  };
+  int rc = run();
+  for (void *p : tmp) cudaFree(p);
+  return rc;
+}
+
+int gnep_loss_and_grad(gnep_handle *h, float *loss_terms, float *grad, int is_device) {
+  if (!h) return fail(h, GNEP_EINVAL, "null handle");
+  if (!h->loaded) return fail(h, GNEP_ESTATE, "no batch loaded");
+  prof_begin(h);
+  RET_IF(enqueue_forward(h));
+  RET_IF(enqueue_backward(h));
+  RET_IF(check_launch(h));
+  if (grad) RET_IF(copy_out(h, grad, h->grad, h->ds.P * sizeof(float), is_device));
+  if (loss_terms) RET_IF(fetch_terms(h, loss_terms));
+  return GNEP_OK;
+}
+
+int gnep_adam_step(gnep_handle *h, float lr, float beta1, float beta2, float eps) {
+  if (!h) return fail(h, GNEP_EINVAL, "null handle");
+  if (!(beta1 >= 0 && beta1 < 1 && beta2 >= 0 && beta2 < 1) || !(eps >= 0)) return fail(h, GNEP_EINVAL, "bad Adam constants");
+  RET_IF(enqueue_adam(h, lr, beta1, beta2, eps));
+  return check_launch(h);
+}
+
+int gnep_train_epochs(gnep_handle *h, int32_t n_epochs, float lr, float beta1, float beta2, float eps, float *loss_terms) {
+  if (!h || n_epochs < 0) return fail(h, GNEP_EINVAL, "bad argument");
+  if (!h->loaded) return fail(h, GNEP_ESTATE, "no batch loaded");
+  if (!(beta1 >= 0 && beta1 < 1 && beta2 >= 0 && beta2 < 1) || !(eps >= 0)) return fail(h, GNEP_EINVAL, "bad Adam constants");
+  if (h->graph && (h->g_lr != lr || h->g_b1 != beta1 || h->g_b2 != beta2 || h->g_eps != eps)) {
+    cudaGraphExecDestroy(h->graph); h->graph = nullptr;
+  }
+  if (!h->graph) {
+    bool prof = h->prof; h->prof = false;
+    int64_t before = h->launches;
+    cudaGraph_t g = nullptr;
+    CK(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
+    int rc = enqueue_forward(h);
+    if (rc == GNEP_OK) rc = enqueue_backward(h);
+    if (rc == GNEP_OK) rc = enqueue_adam(h, lr, beta1, beta2, eps);
+    cudaError_t e = cudaStreamEndCapture(h->stream, &g);
+    h->prof = prof;
+    h->graph_launches = h->launches - before;
+    h->launches = before;
+    if (rc != GNEP_OK) { if (g) cudaGraphDestroy(g); return rc; }
+    if (e != cudaSuccess) return fail(h, GNEP_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e));
+    e = cudaGraphInstantiate(&h->graph, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) { h->graph = nullptr; return fail(h, GNEP_ECUDA, std::string("graph instantiate: ") + cudaGetErrorString(e)); }
+    h->g_lr = lr; h->g_b1 = beta1; h->g_b2 = beta2; h->g_eps = eps;
+  }
+  for (int i = 0; i < n_epochs; ++i) { CK(cudaGraphLaunch(h->graph, h->stream)); h->launches += h->graph_launches; }
+  if (loss_terms) RET_IF(fetch_terms(h, loss_terms));
+  return GNEP_OK;
+}
+
+int gnep_launch_count(const gnep_handle *h, int64_t *n) {
+  if (!h || !n) return fail(h, GNEP_EINVAL, "null argument");
+  *n = h->launches;
+  return GNEP_OK;
+}
+
+int gnep_set_profiling(gnep_handle *h, int on) {
+  if (!h) return fail(h, GNEP_EINVAL, "null handle");
+  h->prof = on != 0;
+  return GNEP_OK;
+}
+int gnep_phase_times(const gnep_handle *h, const char **names, float *ms, int32_t capacity, int32_t *n) {
+  if (!h || !n) return fail(h, GNEP_EINVAL, "null argument");
+  gnep_handle *hh = const_cast<gnep_handle *>(h);
+  if (hh->prof && !hh->phases.empty()) prof_collect(hh);
+  *n = (int32_t)h->phase_ms.size();
+  for (int i = 0; i < *n && i < capacity; ++i) { if (names) names[i] = h->phase_names[i]; if (ms) ms[i] = h->phase_ms[i]; }
+  return GNEP_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,191 @@
+// reduce_kernels.cuh -- per-structure sums, loss terms and adjoint seeds (row a4), block->grid reduction of
+// the partial gradients (row a8), fused Adam (row a9), and the output un-permutation kernels.
+// All cross-CTA sums run in a fixed order with fp64 accumulators: no global atomics, bit-reproducible.
+#pragma once
+#include "common.cuh"
+
+struct LossCfg {
+  int S, N, T, P;
+  int hasE, hasF, hasV, loss_mode;
+  double lam_e, lam_f, lam_v, lam_2;
+};
+
+template <int NV>
+__device__ __forceinline__ void block_reduce_d(double (&v)[NV], double *sh /*[NV][nwarps]*/) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    double x = v[i];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    if (lane == 0) sh[i * nw + warp] = x;
+  }
+  __syncthreads();
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    double x = 0.0;
+    for (int w = 0; w < nw; ++w) x += sh[i * nw + w];
+    v[i] = x;
+  }
+  __syncthreads();
+}
+
+// a4: one CTA per structure.  E_s = sum E_i, W_s = sum W_i (Eq.1, Eq.4), residuals of Eq.10-12 and the
+// seeds e_s = 2 lam_e dE_s/(S N_s), u_i = 2 lam_f (F_i - Fref_i)/(3N), omega_s = 2 lam_v dW_s/(6 S N_s).
+__global__ void __launch_bounds__(128)
+k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const float *__restrict__ Ei,
+                const float4 *__restrict__ Fat, const float *__restrict__ Wat, const double *__restrict__ Eref,
+                const float *__restrict__ Fref_s, const double *__restrict__ Wref, double *__restrict__ Es,
+                double *__restrict__ Ws, float *__restrict__ e_s, float4 *__restrict__ u,
+                float *__restrict__ omega, double *__restrict__ parts /*[S][3]*/) {
+  __shared__ double sh[8 * 4];
+  const int s = blockIdx.x;
+  double v[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // E, W[6], sum |dF|^2
+  int Ns = 0;
+  const float cu = lc.hasF ? (float)(2.0 * lc.lam_f / (3.0 * (double)lc.N)) : 0.f;
+  for (int t = 0; t < lc.T; ++t) {
+    int b = srange[(s * lc.T + t) * 2], e = srange[(s * lc.T + t) * 2 + 1];
+    Ns += e - b;
+    for (int a = b + threadIdx.x; a < e; a += blockDim.x) {
+      v[0] += (double)Ei[a];
+#pragma unroll
+      for (int c = 0; c < 6; ++c) v[1 + c] += (double)Wat[(size_t)a * 6 + c];
+      float4 F = Fat[a];
+      float dx = 0.f, dy = 0.f, dz = 0.f;
+      if (lc.hasF) { dx = F.x - Fref_s[3 * (size_t)a]; dy = F.y - Fref_s[3 * (size_t)a + 1]; dz = F.z - Fref_s[3 * (size_t)a + 2]; }
+      v[7] += (double)dx * dx + (double)dy * dy + (double)dz * dz;
+      u[a] = make_float4(cu * dx, cu * dy, cu * dz, 0.f);
+    }
+  }
+  block_reduce_d<8>(v, sh);
+  if (threadIdx.x == 0) {
+    double ns = (double)Ns;
+    Es[s] = v[0];
+    double pe = 0.0, pv = 0.0, es = 0.0;
+    if (lc.hasE && Ns > 0) {
+      double dE = v[0] / ns - Eref[s] / ns;
+      pe = dE * dE;
+      es = 2.0 * lc.lam_e * dE / ((double)lc.S * ns);
+    }
+    e_s[s] = (float)es;
+    for (int c = 0; c < 6; ++c) {
+      Ws[s * 6 + c] = v[1 + c];
+      double om = 0.0;
+      if (lc.hasV && Ns > 0) {
+        double dW = (v[1 + c] - Wref[s * 6 + c]) / ns;
+        pv += dW * dW;
+        om = 2.0 * lc.lam_v * dW / (6.0 * (double)lc.S * ns);
+      }
+      omega[s * 6 + c] = (float)om;
+    }
+    parts[s * 3 + 0] = pe; parts[s * 3 + 1] = v[7]; parts[s * 3 + 2] = pv;
+  }
+}
+
+// a4: loss terms {L, t_e, t_f, t_v, t_2} (Eq.9-12 + L2) and the per-term seed multipliers
+// scales = {se, sf, sv, s2}: all 1 in mean-square mode, 1/(2 sqrt t_x) in RMSE mode (0 if t_x = 0).
+__global__ void __launch_bounds__(256)
+k_loss_final(LossCfg lc, const double *__restrict__ parts, const float *__restrict__ theta,
+             float *__restrict__ terms, float *__restrict__ scales) {
+  __shared__ double sh[4 * 8];
+  double v[4] = {0, 0, 0, 0};
+  for (int s = threadIdx.x; s < lc.S; s += blockDim.x) { v[0] += parts[s * 3]; v[1] += parts[s * 3 + 1]; v[2] += parts[s * 3 + 2]; }
+  for (int p = threadIdx.x; p < lc.P; p += blockDim.x) { double x = theta[p]; v[3] += x * x; }
+  block_reduce_d<4>(v, sh);
+  if (threadIdx.x == 0) {
+    double te = lc.S > 0 ? v[0] / lc.S : 0.0;
+    double tf = lc.N > 0 ? v[1] / (3.0 * lc.N) : 0.0;
+    double tv = lc.S > 0 ? v[2] / (6.0 * lc.S) : 0.0;
+    double t2 = v[3] / lc.P;
+    double L, sc[4] = {1, 1, 1, 1};
+    if (lc.loss_mode == 0) L = lc.lam_e * te + lc.lam_f * tf + lc.lam_v * tv + lc.lam_2 * t2;
+    else {
+      L = lc.lam_e * sqrt(te) + lc.lam_f * sqrt(tf) + lc.lam_v * sqrt(tv) + lc.lam_2 * sqrt(t2);
+      sc[0] = te > 0 ? 0.5 / sqrt(te) : 0; sc[1] = tf > 0 ? 0.5 / sqrt(tf) : 0;
+      sc[2] = tv > 0 ? 0.5 / sqrt(tv) : 0; sc[3] = t2 > 0 ? 0.5 / sqrt(t2) : 0;
+    }
+    terms[0] = (float)L; terms[1] = (float)te; terms[2] = (float)tf; terms[3] = (float)tv; terms[4] = (float)t2;
+    for (int i = 0; i < 4; ++i) scales[i] = (float)sc[i];
+  }
+}
+
+// a8: grad[p] = sum over the partial buffers that cover p (fixed order, fp64) + 2 lam_2 s2 theta_p / P.
+struct ReduceMap {
+  int chunk_base[GNEP_MAX_SPECIES_C + 1];   // K-chunks (W0, cR partials) per species
+  int cta_base[GNEP_MAX_SPECIES_C + 1];     // network CTAs (b0, w1, b1 partials) per species
+  int n_warps_ca;                           // partial rows of the angular c-gradient
+};
+__global__ void __launch_bounds__(256)
+k_grad_reduce(DevSpec sp, ReduceMap rm, const float *__restrict__ theta, const float *__restrict__ scales,
+              const float *__restrict__ partialCR, const float *__restrict__ partialCA,
+              const float *__restrict__ partialW, const float *__restrict__ partialB, float *__restrict__ grad) {
+  int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= sp.P) return;
+  double s = 0.0;
+  if (p < sp.offA) {                       // cR[I][J][n][k]
+    int k = p % sp.KR, r = p / sp.KR;
+    int n = r % sp.NR; r /= sp.NR;
+    int J = r % sp.T, I = r / sp.T;
+    int O = sp.NR * sp.T * sp.KRp, o = n * sp.T * sp.KRp + J * sp.KRp + k;
+    for (int c = rm.chunk_base[I]; c < rm.chunk_base[I + 1]; ++c) s += (double)partialCR[(size_t)c * O + o];
+  } else if (p < sp.offNet) {              // cA[I][J][n][k]
+    int x = p - sp.offA;
+    int k = x % sp.KA, r = x / sp.KA;      // r = (I*T+J)*NA + n
+    int O = sp.T * sp.T * sp.NA * sp.KAp, o = r * sp.KAp + k;
+    for (int w = 0; w < rm.n_warps_ca; ++w) s += (double)partialCA[(size_t)w * O + o];
+  } else {
+    int x = p - sp.offNet;
+    int t = x / sp.netSize, y = x - t * sp.netSize;
+    int nW = sp.Nn * sp.Ndes;
+    if (y < nW) {
+      for (int c = rm.chunk_base[t]; c < rm.chunk_base[t + 1]; ++c) s += (double)partialW[(size_t)c * nW + y];
+    } else {
+      int nb = 2 * sp.Nn + 1;
+      for (int c = rm.cta_base[t]; c < rm.cta_base[t + 1]; ++c) s += (double)partialB[(size_t)c * nb + (y - nW)];
+    }
+  }
+  s += 2.0 * (double)sp.lam_2 * (double)scales[3] * (double)theta[p] / (double)sp.P;
+  grad[p] = (float)s;
+}
+
+// a9: textbook Adam with bias correction (Kingma & Ba Alg.1); step counter on the device (graph-safe).
+__global__ void __launch_bounds__(256)
+k_adam(int P, float *__restrict__ theta, float *__restrict__ m, float *__restrict__ v,
+       const float *__restrict__ grad, const long long *__restrict__ step, float lr, float beta1, float beta2,
+       float eps) {
+  int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P) return;
+  double t = (double)(*step + 1);
+  float c1 = (float)(1.0 - pow((double)beta1, t)), c2 = (float)(1.0 - pow((double)beta2, t));
+  float g = grad[p];
+  float mm = beta1 * m[p] + (1.f - beta1) * g;
+  float vv = beta2 * v[p] + (1.f - beta2) * g * g;
+  m[p] = mm; v[p] = vv;
+  theta[p] -= lr * (mm / c1) / (sqrtf(vv / c2) + eps);
+}
+__global__ void k_step_inc(long long *step) { *step += 1; }
+
+// outputs back to the caller's atom order
+__global__ void k_unpermute_force(int N, const int *__restrict__ perm, const float4 *__restrict__ Fat, float *__restrict__ out) {
+  int a = blockIdx.x * blockDim.x + threadIdx.x;
+  if (a >= N) return;
+  float4 f = Fat[a];
+  size_t i = perm[a];
+  out[3 * i] = f.x; out[3 * i + 1] = f.y; out[3 * i + 2] = f.z;
+}
+__global__ void k_unpermute_rows(int N, int W, const int *__restrict__ perm, const float *__restrict__ in, float *__restrict__ out) {
+  size_t x = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (x >= (size_t)N * W) return;
+  size_t a = x / W, c = x - a * W;
+  out[(size_t)perm[a] * W + c] = in[x];
+}
+__global__ void k_permute_fref(int N, const int *__restrict__ perm, const double *__restrict__ in, float *__restrict__ out) {
+  int a = blockIdx.x * blockDim.x + threadIdx.x;
+  if (a >= N) return;
+  size_t i = perm[a];
+  out[3 * (size_t)a] = (float)in[3 * i]; out[3 * (size_t)a + 1] = (float)in[3 * i + 1]; out[3 * (size_t)a + 2] = (float)in[3 * i + 2];
+}
+__global__ void k_d2f(int n, const double *__restrict__ in, float *__restrict__ out) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = (float)in[i];
+}

@@ -1,0 +1,197 @@
+"""GPU parity tests: the CUDA path through the C ABI against the fp64 oracle on identical seeded inputs.
+
+Tolerances are BASELINE.json's: neighbour lists bit-exact; E, F, virial, loss 1e-5 relative; gradient
+1e-4 relative L2 and 1e-3 per component above 1e-6 absolute; parameters after 10 Adam steps 1e-4 relative
+(L2, R33).  "Relative" for vectors means max |diff| / max |reference|.
+"""
+import numpy as np
+import pytest
+
+import gnep_synth as gs
+from cases import labelled_case
+from oracle import gnep_oracle as orc
+
+pytestmark = pytest.mark.gpu
+
+
+def _gnep(spec, qs, b, labels, theta):
+    from paper_2507_00528_b200 import Gnep
+    g = Gnep(dict(spec, q_scale=qs))
+    E, F, W = labels
+    g.load_batch(b["atom_offsets"], b["positions"], b["cells"], b["types"], E, F, W)
+    g.set_params(theta.astype(np.float32))
+    return g
+
+
+def _rel(a, ref):
+    return float(np.max(np.abs(np.asarray(a, dtype=np.float64) - ref)) / max(np.max(np.abs(ref)), 1e-300))
+
+
+def _check_neighbors(g, ob):
+    for which in (0, 1):
+        rp, j, sh = g.neighbor_list(which)
+        orp, oj, osh, _ = ob.neighbors(which)
+        np.testing.assert_array_equal(rp, orp)
+        np.testing.assert_array_equal(j, oj)
+        np.testing.assert_array_equal(sh.astype(np.int32), osh)
+
+
+def _check_all(config, n_structs, adam_steps=10, spec_over=None):
+    spec, sp, b, ob, theta, qs, labels = labelled_case(config, n_structs=n_structs, spec_over=spec_over)
+    g = _gnep(spec, qs, b, labels, theta)
+    _check_neighbors(g, ob)
+    # descriptors
+    q = g.descriptors()
+    q_ref = orc.descriptors(sp, theta, ob)
+    assert np.max(np.abs(q - q_ref) / (np.abs(q_ref).max(axis=0) + 1e-30)) < 1e-5
+    # predictions
+    E, F, W = g.predict()
+    E_ref, F_ref, W_ref = orc.predict(sp, theta, qs, ob)
+    assert _rel(E, E_ref) < 1e-5 and _rel(F, F_ref) < 1e-5 and _rel(W, W_ref) < 1e-5
+    # loss and gradient
+    terms, grad = g.loss_and_grad(want_grad=True)
+    t_ref, g_ref = orc.loss_and_grad(sp, theta, qs, ob)
+    for a, r in zip(terms, t_ref):
+        assert abs(a - r) <= 1e-5 * abs(r) + 1e-12
+    assert np.linalg.norm(grad - g_ref) / np.linalg.norm(g_ref) < 1e-4
+    big = np.abs(g_ref) > 1e-6
+    assert np.max(np.abs(grad[big] - g_ref[big]) / np.abs(g_ref[big])) < 1e-3
+    assert np.max(np.abs(grad[~big] - g_ref[~big])) < 1e-6 if (~big).any() else True
+    # Adam trajectory, both through separate calls and through the graph
+    if adam_steps:
+        th = theta.copy(); m = np.zeros_like(th); v = np.zeros_like(th)
+        losses_ref, losses = [], []
+        for t in range(1, adam_steps + 1):
+            tr, gr = orc.loss_and_grad(sp, th, qs, ob)
+            losses_ref.append(tr[0])
+            orc.adam_step(th, m, v, gr, t, 1e-3)
+            tt, _ = g.loss_and_grad()
+            losses.append(tt[0])
+            g.adam_step(1e-3)
+        th_gpu = g.get_params().astype(np.float64)
+        assert np.linalg.norm(th_gpu - th) / np.linalg.norm(th) < 1e-4
+        np.testing.assert_allclose(losses, losses_ref, rtol=1e-4)
+        mm, vv, step = g.get_opt_state()
+        assert step == adam_steps
+        # CUDA-graph epochs give the same trajectory
+        g.set_params(theta.astype(np.float32))
+        g.set_opt_state(np.zeros_like(mm), np.zeros_like(vv), 0)
+        g.train_epochs(adam_steps, 1e-3)
+        th_graph = g.get_params().astype(np.float64)
+        assert np.linalg.norm(th_graph - th) / np.linalg.norm(th) < 1e-4
+    g.destroy()
+
+
+def test_config0_full():
+    _check_all(0, None)
+
+
+def test_config1_sample_with_4body():
+    _check_all(1, 6)
+
+
+def test_config2_liquid_sample():
+    _check_all(2, 4, adam_steps=3)
+
+
+def test_config3_mixed_sample():
+    _check_all(3, 9, adam_steps=3)
+
+
+def test_config4_liquid_sample():
+    _check_all(4, 3, adam_steps=2)
+
+
+def test_rmse_mode_and_missing_virial():
+    spec, sp, b, ob, theta, qs, (E, F, W) = labelled_case(0, n_structs=3, spec_over={"loss_mode": 1})
+    g = _gnep(spec, qs, b, (E, F, W), theta)
+    terms, grad = g.loss_and_grad(want_grad=True)
+    t_ref, g_ref = orc.loss_and_grad(sp, theta, qs, ob)
+    np.testing.assert_allclose(terms, t_ref, rtol=1e-5)
+    assert np.linalg.norm(grad - g_ref) / np.linalg.norm(g_ref) < 1e-4
+    g.set_targets(E, F, None)
+    ob.set_refs(E, F, None)
+    terms, grad = g.loss_and_grad(want_grad=True)
+    t_ref, g_ref = orc.loss_and_grad(sp, theta, qs, ob)
+    assert terms[3] == 0.0
+    np.testing.assert_allclose(terms, t_ref, rtol=1e-5, atol=1e-12)
+    assert np.linalg.norm(grad - g_ref) / np.linalg.norm(g_ref) < 1e-4
+    g.destroy()
+
+
+def test_small_l_and_odd_sizes():
+    """l_max = 2 without 4-body, odd function / basis counts (padding paths), three species."""
+    over = {"l_max": 2, "n_radial": 3, "n_basis_radial": 5, "n_angular": 11, "n_basis_angular": 7, "n_neurons": 37}
+    _check_all(0, 2, adam_steps=2, spec_over=over)
+
+
+def test_neighbors_small_triclinic_multi_image_and_wrap():
+    from paper_2507_00528_b200 import Gnep
+    rng = np.random.default_rng(7)
+    cell = np.array([[5.0, 0.0, 0.0], [1.2, 4.6, 0.0], [-0.7, 0.9, 5.3]])
+    frac = rng.uniform(0.02, 0.98, size=(9, 3))
+    pos = (frac + rng.integers(-2, 3, size=(9, 3))) @ cell          # some atoms outside the cell
+    spec = dict(gs.MODEL_SPECS[0], rc_radial=6.0, rc_angular=3.5)
+    sp = orc.make_spec(spec)
+    off = np.array([0, 9], np.int32); types = (np.arange(9) % 2).astype(np.int32)
+    ob = orc.Batch(sp, off, pos, cell.reshape(1, 9), types)
+    g = Gnep(spec)
+    g.load_batch(off, pos, cell.reshape(1, 9), types)
+    _check_neighbors(g, ob)
+    theta = gs.draw_params(spec, 0)
+    g.set_params(theta.astype(np.float32))
+    E, F, W = g.predict()
+    E_ref, F_ref, W_ref = orc.predict(sp, theta, None, ob)
+    assert _rel(E, E_ref) < 1e-5 and _rel(F, F_ref) < 2e-5 and _rel(W, W_ref) < 1e-5
+    g.destroy()
+
+
+def test_edge_cases_empty_isolated_and_errors():
+    from paper_2507_00528_b200 import Gnep, GnepError
+    spec = dict(gs.MODEL_SPECS[0])
+    g = Gnep(spec)
+    with pytest.raises(GnepError) as e:
+        g.loss_and_grad()
+    assert e.value.code == -2                                       # ESTATE: nothing loaded
+    # empty batch
+    g.load_batch(np.array([0], np.int32), np.zeros((0, 3)), np.zeros((0, 9)), np.zeros(0, np.int32))
+    assert g.batch_info()["n_atoms"] == 0
+    # one isolated atom: no neighbours, E = F(0) = w1.tanh(b0) + b1, F = 0
+    theta = gs.draw_params(spec, 0)
+    g.set_params(theta.astype(np.float32))
+    g.load_batch(np.array([0, 1], np.int32), np.array([[1.0, 2.0, 3.0]]), (np.eye(3) * 20).reshape(1, 9), np.zeros(1, np.int32))
+    assert g.batch_info()["n_pairs_radial"] == 0
+    E, F, W = g.predict()
+    nd, nn = gs.n_descriptors(spec), spec["n_neurons"]
+    net = theta[4 * 5 * 8 + 4 * 5 * 6:][:nd * nn + 2 * nn + 1]
+    b0, w1, b1 = net[nd * nn:nd * nn + nn], net[nd * nn + nn:nd * nn + 2 * nn], net[-1]
+    assert abs(E[0] - (w1 @ np.tanh(b0) + b1)) < 1e-6 and np.all(F == 0) and np.all(W == 0)
+    # bad species, degenerate cell
+    with pytest.raises(GnepError) as e:
+        g.load_batch(np.array([0, 1], np.int32), np.zeros((1, 3)), (np.eye(3) * 20).reshape(1, 9), np.array([7], np.int32))
+    assert e.value.code == -5
+    with pytest.raises(GnepError) as e:
+        g.load_batch(np.array([0, 1], np.int32), np.zeros((1, 3)), np.zeros((1, 9)), np.zeros(1, np.int32))
+    assert e.value.code == -5
+    g.destroy()
+
+
+def test_device_pointers_and_determinism():
+    """torch CUDA tensors go through unchanged; two evaluations are bit-identical (no atomics)."""
+    import torch
+    spec, sp, b, ob, theta, qs, (E, F, W) = labelled_case(1, n_structs=3)
+    from paper_2507_00528_b200 import Gnep
+    g = Gnep(dict(spec, q_scale=qs), stream=torch.cuda.current_stream())
+    dev = torch.device("cuda:0")
+    g.load_batch(b["atom_offsets"], torch.tensor(b["positions"], device=dev), torch.tensor(b["cells"], device=dev),
+                 torch.tensor(b["types"], device=dev), torch.tensor(E, device=dev), torch.tensor(F, device=dev),
+                 torch.tensor(W, device=dev))
+    g.set_params(torch.tensor(theta, dtype=torch.float32, device=dev))
+    grad1 = torch.empty(len(theta), dtype=torch.float32, device=dev)
+    grad2 = torch.empty_like(grad1)
+    t1, _ = g.loss_and_grad(grad=grad1)
+    t2, _ = g.loss_and_grad(grad=grad2)
+    assert torch.equal(grad1, grad2) and np.array_equal(t1, t2)
+    t_ref, g_ref = orc.loss_and_grad(sp, theta, qs, ob)
+    assert np.linalg.norm(grad1.cpu().numpy() - g_ref) / np.linalg.norm(g_ref) < 1e-4
+    g.destroy()
