@@ -166,14 +166,25 @@ def make_structure(config, s):
     return pos, cell, np.ascontiguousarray(types, dtype=np.int32)
 
 
-def make_batch(config, n_structs=None, first=0):
-    """Structures first .. first+n_structs-1 of a config, concatenated.
+def _make_structure_job(args):
+    return make_structure(*args)
+
+
+def make_batch(config, n_structs=None, first=0, workers=0):
+    """Structures first .. first+n_structs-1 of a config, concatenated.  Every structure depends only on
+    (config, s), so `workers` > 1 (processes) changes nothing but the wall time.
 
     Returns dict(atom_offsets i32 [S+1], positions f64 [N,3], cells f64 [S,9], types i32 [N])."""
     S = N_STRUCTS[config] if n_structs is None else int(n_structs)
+    jobs = [(config, s) for s in range(first, first + S)]
+    if workers and workers > 1 and S >= 4 * workers:
+        import multiprocessing as mp
+        with mp.get_context("fork").Pool(workers) as pool:
+            res = pool.map(_make_structure_job, jobs, chunksize=max(1, S // (8 * workers)))
+    else:
+        res = [make_structure(*j) for j in jobs]
     P, Cc, Tt, off = [], [], [], [0]
-    for s in range(first, first + S):
-        p, c, t = make_structure(config, s)
+    for p, c, t in res:
         P.append(p); Cc.append(c.reshape(9)); Tt.append(t); off.append(off[-1] + len(p))
     return dict(atom_offsets=np.asarray(off, dtype=np.int32),
                 positions=np.concatenate(P, axis=0) if P else np.zeros((0, 3)),

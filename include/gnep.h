@@ -130,6 +130,14 @@ int gnep_adam_step(gnep_handle *h, float lr, float beta1, float beta2, float eps
 int gnep_train_epochs(gnep_handle *h, int32_t n_epochs, float lr, float beta1, float beta2, float eps,
                       float *loss_terms);
 
+/* Multi-GPU by structure sharding: every rank holds its own structures and calls
+ * gnep_set_global_norm with the job-wide atom and structure counts (the normalisers N, N_str of Eq.10-12)
+ * and its share of the L2 term (1/world).  Each rank's loss terms and gradient are then partial sums: the
+ * caller all-reduces (sum) the P gradient floats, hands the result back with gnep_set_grad and calls
+ * gnep_adam_step on every rank.  Negative counts restore single-GPU behaviour.  loss_mode 0 only. */
+int gnep_set_global_norm(gnep_handle *h, int64_t n_atoms_global, int64_t n_structs_global, double l2_share);
+int gnep_set_grad(gnep_handle *h, const float *grad, int is_device);
+
 /* Checkpoint / resume of the optimiser state (m, v: P floats each; either may be NULL). */
 int gnep_get_opt_state(const gnep_handle *h, float *m, float *v, int64_t *step, int is_device);
 int gnep_set_opt_state(gnep_handle *h, const float *m, const float *v, int64_t step, int is_device);

@@ -18,7 +18,7 @@ EXPORTS = ["gnep_create", "gnep_destroy", "gnep_num_params", "gnep_num_descripto
            "gnep_get_params", "gnep_set_q_scale", "gnep_load_batch", "gnep_set_targets", "gnep_neighbor_list",
            "gnep_descriptors", "gnep_predict", "gnep_loss_and_grad", "gnep_adam_step", "gnep_train_epochs",
            "gnep_get_opt_state", "gnep_set_opt_state", "gnep_batch_info", "gnep_launch_count",
-           "gnep_set_profiling", "gnep_phase_times", "gnep_last_error"]
+           "gnep_set_profiling", "gnep_phase_times", "gnep_last_error", "gnep_set_global_norm", "gnep_set_grad"]
 
 ERRORS = {-1: "GNEP_EINVAL", -2: "GNEP_ESTATE", -3: "GNEP_ECUDA", -4: "GNEP_ENOMEM", -5: "GNEP_ERANGE",
           -6: "GNEP_ENONFINITE"}
@@ -73,6 +73,8 @@ def load_library(build_if_missing=True):
     L.gnep_get_opt_state.argtypes = [vp, vp, vp, C.POINTER(C.c_int64), C.c_int]
     L.gnep_set_opt_state.argtypes = [vp, vp, vp, C.c_int64, C.c_int]
     L.gnep_batch_info.argtypes = [vp] + [C.POINTER(C.c_int64)] * 4
+    L.gnep_set_global_norm.argtypes = [vp, C.c_int64, C.c_int64, C.c_double]
+    L.gnep_set_grad.argtypes = [vp, vp, C.c_int]
     L.gnep_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
     L.gnep_set_profiling.argtypes = [vp, C.c_int]
     L.gnep_phase_times.argtypes = [vp, C.POINTER(C.c_char_p), C.POINTER(C.c_float), C.c_int32, C.POINTER(C.c_int32)]
@@ -250,6 +252,14 @@ class Gnep:
         pt = None if terms is None else terms.ctypes.data_as(C.c_void_p)
         self._ck(self._L.gnep_train_epochs(self._h, int(n_epochs), lr, beta1, beta2, eps, pt))
         return terms
+
+    # ---- structure sharding over ranks ----
+    def set_global_norm(self, n_atoms_global, n_structs_global, l2_share):
+        self._ck(self._L.gnep_set_global_norm(self._h, int(n_atoms_global), int(n_structs_global), float(l2_share)))
+
+    def set_grad(self, grad):
+        p, dev, _k = _ptr(grad, np.float32)
+        self._ck(self._L.gnep_set_grad(self._h, p, dev))
 
     # ---- profiling ----
     def set_profiling(self, on):

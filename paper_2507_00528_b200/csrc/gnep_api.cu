@@ -42,6 +42,7 @@ struct gnep_handle {
   int N = 0, S = 0;
   int64_t nR = 0, nA = 0;
   int hasE = 0, hasF = 0, hasV = 0;
+  double Ng = -1, Sg = -1, l2_share = 1.0;   // job-wide normalisers when structures are sharded over ranks
   std::vector<void *> batch_allocs;
   int *perm = nullptr, *type_s = nullptr, *struct_s = nullptr, *segR = nullptr, *rowAs = nullptr, *revA = nullptr;
   float4 *pairR = nullptr, *pairA = nullptr;
@@ -216,6 +217,7 @@ LossCfg loss_cfg(const gnep_handle *h) {
   lc.S = h->S; lc.N = h->N; lc.T = h->ds.T; lc.P = h->ds.P;
   lc.hasE = h->hasE; lc.hasF = h->hasF; lc.hasV = h->hasV; lc.loss_mode = h->ds.loss_mode;
   lc.lam_e = h->spec.lambda_e; lc.lam_f = h->spec.lambda_f; lc.lam_v = h->spec.lambda_v; lc.lam_2 = h->spec.lambda_2;
+  lc.Ng = h->Ng >= 0 ? h->Ng : (double)h->N; lc.Sg = h->Sg >= 0 ? h->Sg : (double)h->S; lc.l2_share = h->l2_share;
   return lc;
 }
 
@@ -253,7 +255,7 @@ int enqueue_backward(gnep_handle *h) {
   mark(h, "a7_radial_cgrad");
   DISPATCH_KT(d.KAp, LAUNCH(h, k_cgrad_angular<KT>, h->n_ca_blocks, GNEP_WARPS * 32, smem_cgrad_ang(d), d, h->N, h->type_s, h->struct_s, h->rowAs, h->pairA, h->u, h->omega, h->scales, h->Ep, h->gbar, h->Sn, h->Tn, h->partialCA));
   mark(h, "a7_angular_cgrad");
-  LAUNCH(h, k_grad_reduce, cdiv(d.P, 256), 256, 0, d, h->rm, h->theta, h->scales, h->partialCR, h->partialCA, h->partialW, h->partialB, h->grad);
+  LAUNCH(h, k_grad_reduce, cdiv(d.P, 256), 256, 0, d, h->rm, (float)h->l2_share, h->theta, h->scales, h->partialCR, h->partialCA, h->partialW, h->partialB, h->grad);
   mark(h, "a8_grad_reduce");
   return GNEP_OK;
 }
@@ -791,6 +793,23 @@ int gnep_train_epochs(gnep_handle *h, int32_t n_epochs, float lr, float beta1, f
   for (int i = 0; i < n_epochs; ++i) { CK(cudaGraphLaunch(h->graph, h->stream)); h->launches += h->graph_launches; }
   if (loss_terms) RET_IF(fetch_terms(h, loss_terms));
   return GNEP_OK;
+}
+
+int gnep_set_global_norm(gnep_handle *h, int64_t n_atoms_global, int64_t n_structs_global, double l2_share) {
+  if (!h) return fail(h, GNEP_EINVAL, "null handle");
+  if (n_atoms_global < 0 || n_structs_global < 0) { h->Ng = h->Sg = -1; h->l2_share = 1.0; }
+  else {
+    if (h->ds.loss_mode != 0) return fail(h, GNEP_EINVAL, "sharded normalisation needs loss_mode 0 (RMSE mode needs the global terms before the seeds)");
+    if (!(l2_share >= 0 && l2_share <= 1)) return fail(h, GNEP_EINVAL, "l2_share must be in [0,1]");
+    h->Ng = (double)n_atoms_global; h->Sg = (double)n_structs_global; h->l2_share = l2_share;
+  }
+  if (h->graph) { cudaGraphExecDestroy(h->graph); h->graph = nullptr; }
+  return GNEP_OK;
+}
+
+int gnep_set_grad(gnep_handle *h, const float *grad, int is_device) {
+  if (!h || !grad) return fail(h, GNEP_EINVAL, "null argument");
+  return copy_in(h, h->grad, grad, h->ds.P * sizeof(float), is_device);
 }
 
 int gnep_launch_count(const gnep_handle *h, int64_t *n) {

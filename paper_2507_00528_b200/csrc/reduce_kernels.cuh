@@ -8,6 +8,8 @@ struct LossCfg {
   int S, N, T, P;
   int hasE, hasF, hasV, loss_mode;
   double lam_e, lam_f, lam_v, lam_2;
+  double Ng, Sg;      // atoms / structures of the WHOLE job (== N, S on one GPU): the normalisers of Eq.10-12
+  double l2_share;    // this rank's share of the L2 term (1 on one GPU, 1/world when structures are sharded)
 };
 
 template <int NV>
@@ -42,7 +44,7 @@ k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const 
   const int s = blockIdx.x;
   double v[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // E, W[6], sum |dF|^2
   int Ns = 0;
-  const float cu = lc.hasF ? (float)(2.0 * lc.lam_f / (3.0 * (double)lc.N)) : 0.f;
+  const float cu = lc.hasF ? (float)(2.0 * lc.lam_f / (3.0 * lc.Ng)) : 0.f;
   for (int t = 0; t < lc.T; ++t) {
     int b = srange[(s * lc.T + t) * 2], e = srange[(s * lc.T + t) * 2 + 1];
     Ns += e - b;
@@ -65,7 +67,7 @@ k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const 
     if (lc.hasE && Ns > 0) {
       double dE = v[0] / ns - Eref[s] / ns;
       pe = dE * dE;
-      es = 2.0 * lc.lam_e * dE / ((double)lc.S * ns);
+      es = 2.0 * lc.lam_e * dE / (lc.Sg * ns);
     }
     e_s[s] = (float)es;
     for (int c = 0; c < 6; ++c) {
@@ -74,7 +76,7 @@ k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const 
       if (lc.hasV && Ns > 0) {
         double dW = (v[1 + c] - Wref[s * 6 + c]) / ns;
         pv += dW * dW;
-        om = 2.0 * lc.lam_v * dW / (6.0 * (double)lc.S * ns);
+        om = 2.0 * lc.lam_v * dW / (6.0 * lc.Sg * ns);
       }
       omega[s * 6 + c] = (float)om;
     }
@@ -93,10 +95,10 @@ k_loss_final(LossCfg lc, const double *__restrict__ parts, const float *__restri
   for (int p = threadIdx.x; p < lc.P; p += blockDim.x) { double x = theta[p]; v[3] += x * x; }
   block_reduce_d<4>(v, sh);
   if (threadIdx.x == 0) {
-    double te = lc.S > 0 ? v[0] / lc.S : 0.0;
-    double tf = lc.N > 0 ? v[1] / (3.0 * lc.N) : 0.0;
-    double tv = lc.S > 0 ? v[2] / (6.0 * lc.S) : 0.0;
-    double t2 = v[3] / lc.P;
+    double te = lc.Sg > 0 ? v[0] / lc.Sg : 0.0;
+    double tf = lc.Ng > 0 ? v[1] / (3.0 * lc.Ng) : 0.0;
+    double tv = lc.Sg > 0 ? v[2] / (6.0 * lc.Sg) : 0.0;
+    double t2 = lc.l2_share * v[3] / lc.P;
     double L, sc[4] = {1, 1, 1, 1};
     if (lc.loss_mode == 0) L = lc.lam_e * te + lc.lam_f * tf + lc.lam_v * tv + lc.lam_2 * t2;
     else {
@@ -116,7 +118,7 @@ struct ReduceMap {
   int n_warps_ca;                           // partial rows of the angular c-gradient
 };
 __global__ void __launch_bounds__(256)
-k_grad_reduce(DevSpec sp, ReduceMap rm, const float *__restrict__ theta, const float *__restrict__ scales,
+k_grad_reduce(DevSpec sp, ReduceMap rm, float l2_share, const float *__restrict__ theta, const float *__restrict__ scales,
               const float *__restrict__ partialCR, const float *__restrict__ partialCA,
               const float *__restrict__ partialW, const float *__restrict__ partialB, float *__restrict__ grad) {
   int p = blockIdx.x * blockDim.x + threadIdx.x;
@@ -144,7 +146,7 @@ k_grad_reduce(DevSpec sp, ReduceMap rm, const float *__restrict__ theta, const f
       for (int c = rm.cta_base[t]; c < rm.cta_base[t + 1]; ++c) s += (double)partialB[(size_t)c * nb + (y - nW)];
     }
   }
-  s += 2.0 * (double)sp.lam_2 * (double)scales[3] * (double)theta[p] / (double)sp.P;
+  s += 2.0 * (double)l2_share * (double)sp.lam_2 * (double)scales[3] * (double)theta[p] / (double)sp.P;
   grad[p] = (float)s;
 }
 
