@@ -1,0 +1,534 @@
+// angular_kernels.cuh -- sweeps over the angular neighbour list (rows a1, a3, a5, a7 of DESIGN.md).
+//
+// Moment form.  g_n(d) = sum_k c[I][J][n][k] f_k(d) is linear in the basis, so with
+//   A1[J][k][lm] = sum_{j in J} f_k(d_ij) B_lm(rhat_ij)
+//   A2[J][k][lm] = sum_{j in J} f_k'(d_ij) (a_ij.rhat_ij) B_lm + f_k(d_ij) (grad B_lm . a_ij)
+// one has S_nlm = sum_{J,k} c A1 (Eq.8), T_nlm = sum_{J,k} c A2 (the summed factors of C3.9-C3.16) and
+//   dL/dcA[I][J][n][k] = sum_atoms sum_lm alpha_nlm A1[J][k][lm] + beta_nlm A2[J][k][lm]   (C2.5-C2.10, C3.12-C3.20)
+// so the coefficient gradient needs no pair sweep of its own.
+//
+// Mapping: a warp owns ANG_TA consecutive atoms; their pairs are contiguous in pairA, so phase 1 (lane = pair)
+// runs on full 32-pair chunks that cross atom boundaries, and phase 2 (lane = (k, 6 lm) register tile) walks the
+// (atom, species-segment) boundaries inside the chunk.  Shared rows have stride ANG_LD = 36 floats so that the
+// LDS.128 of 8 different rows hit 8 different bank quads.
+#pragma once
+#include "common.cuh"
+#include "pair_kernels.cuh"
+
+#define ANG_TA 16        // atoms per warp tile (fwd / adj)
+#define ANG_WARPS 4      // warps per CTA
+#define ANG_LD 36        // shared-memory row stride in floats
+#define ANG_NQ 16        // n padded to 16 in the transposed coefficient table
+
+// transposed coefficients ct[((I*T+J)*KT + k)*ANG_NQ + n] (zero padded) for the S/T/Gamma contractions
+__device__ __forceinline__ void stage_coeff_t(float *dst, const float *src, int T, int NA, int K, int KT) {
+  int tot = T * T * KT * ANG_NQ;
+  for (int x = threadIdx.x; x < tot; x += blockDim.x) {
+    int n = x % ANG_NQ, r = x / ANG_NQ;
+    int k = r % KT, ij = r / KT;
+    dst[x] = (n < NA && k < K) ? src[(ij * NA + n) * K + k] : 0.f;
+  }
+}
+
+// mask the components of a 4-pair group that fall outside [lo4, hi4)
+__device__ __forceinline__ float4 mask4(float4 v, int lo4, int hi4) {
+  v.x = (0 >= lo4 && 0 < hi4) ? v.x : 0.f;
+  v.y = (1 >= lo4 && 1 < hi4) ? v.y : 0.f;
+  v.z = (2 >= lo4 && 2 < hi4) ? v.z : 0.f;
+  v.w = (3 >= lo4 && 3 < hi4) ? v.w : 0.f;
+  return v;
+}
+__device__ __forceinline__ float dot4(const float4 &a, const float4 &b) { return a.x * b.x + a.y * b.y + a.z * b.z + a.w * b.w; }
+
+// X_nlm = sum_{J,k} c[I][J][n][k] A[J][k][lm] for one atom: lane = lm (24 lanes), NA outputs per lane.
+template <int KT>
+__device__ __forceinline__ void contract_moments(const DevSpec &sp, const float *ct, const float *As, int I, int lane,
+                                                 float (&out)[ANG_NQ]) {
+#pragma unroll
+  for (int n = 0; n < ANG_NQ; ++n) out[n] = 0.f;
+  if (lane >= GNEP_NLM) return;
+  const int nq = (sp.NA + 3) >> 2;
+  for (int J = 0; J < sp.T; ++J) {
+    const float *cj = ct + (I * sp.T + J) * KT * ANG_NQ;
+#pragma unroll
+    for (int k = 0; k < KT; ++k) {
+      float a = As[(J * KT + k) * GNEP_NLM + lane];
+#pragma unroll
+      for (int v = 0; v < ANG_NQ / 4; ++v) {
+        if (v < nq) {
+          float4 c4 = *(const float4 *)(cj + k * ANG_NQ + 4 * v);
+          out[4 * v] += c4.x * a; out[4 * v + 1] += c4.y * a; out[4 * v + 2] += c4.z * a; out[4 * v + 3] += c4.w * a;
+        }
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1 (angular): A1 moments, S_nlm (Eq.8), q_nl = sum_m C_lm S_nlm^2 (Eq.7), 4-body (R14)
+// ------------------------------------------------------------------------------------------------
+template <int KT>
+__global__ void __launch_bounds__(ANG_WARPS * 32)
+k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ segA,
+              const float4 *__restrict__ pairA, const float *__restrict__ theta, float *__restrict__ q,
+              float *__restrict__ S, float *__restrict__ A1) {
+  constexpr int R = (KT + 7) / 8;
+  extern __shared__ __align__(16) float smem[];
+  float *ct = smem;
+  const int nct = sp.T * sp.T * KT * ANG_NQ;
+  const int nA = sp.T * KT * GNEP_NLM;
+  const int per_warp = (KT + GNEP_NLM) * ANG_LD + nA + ((sp.NA * GNEP_NLM + 3) & ~3);
+  float *sf = smem + nct + (threadIdx.x >> 5) * per_warp;   // [KT][LD]
+  float *sB = sf + KT * ANG_LD;                              // [24][LD]
+  float *As = sB + GNEP_NLM * ANG_LD;                        // [T][KT][24]
+  float *sS = As + nA;                                       // [NA][24]
+  stage_coeff_t(ct, theta + sp.offA, sp.T, sp.NA, sp.KA, KT);
+  __syncthreads();
+  const int lane = threadIdx.x & 31;
+  const int a_lo = (blockIdx.x * ANG_WARPS + (threadIdx.x >> 5)) * ANG_TA;
+  if (a_lo >= N) return;
+  const int a_hi = min(a_lo + ANG_TA, N);
+  const int T1 = sp.T + 1;
+  const int P_lo = segA[a_lo * T1], P_hi = segA[(a_hi - 1) * T1 + sp.T];
+  const int kq = lane >> 2, lmq = lane & 3;
+  float acc[R][6];
+#pragma unroll
+  for (int r = 0; r < R; ++r)
+#pragma unroll
+    for (int i = 0; i < 6; ++i) acc[r][i] = 0.f;
+  int a = a_lo, J = 0;
+  int seg_end = segA[a * T1 + 1];
+
+  auto flush_segment = [&]() {   // accumulators of (a, J) -> global A1 and shared As, then reset
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      int k = kq + 8 * r;
+      if (k < KT) {
+        int o = (J * KT + k) * GNEP_NLM + 6 * lmq;
+        float *g = A1 + (size_t)a * nA + o;
+#pragma unroll
+        for (int i = 0; i < 6; i += 2) *(float2 *)(g + i) = make_float2(acc[r][i], acc[r][i + 1]);
+#pragma unroll
+        for (int i = 0; i < 6; ++i) { As[o + i] = acc[r][i]; acc[r][i] = 0.f; }
+      }
+    }
+  };
+  auto atom_epilogue = [&]() {   // S = c.A1, q_nl, q4 of atom a
+    __syncwarp();
+    const int I = type_s[a];
+    float sv[ANG_NQ];
+    contract_moments<KT>(sp, ct, As, I, lane, sv);
+    float *Sa = S + (size_t)a * sp.NA * GNEP_NLM;
+    if (lane < GNEP_NLM) {
+#pragma unroll
+      for (int n = 0; n < ANG_NQ; ++n)
+        if (n < sp.NA) { sS[n * GNEP_NLM + lane] = sv[n]; Sa[n * GNEP_NLM + lane] = sv[n]; }
+    }
+    __syncwarp();
+    float *qa = q + (size_t)a * sp.Ndes + sp.NR;
+    for (int o = lane; o < sp.NA * sp.L; o += 32) {
+      int l = o / sp.NA + 1, n = o - (l - 1) * sp.NA;
+      int lm0 = l * l - 1;
+      float v = 0.f;
+      for (int m = 0; m <= 2 * l; ++m) { float s = sS[n * GNEP_NLM + lm0 + m]; v += 0.5f * c_C2[lm0 + m] * s * s; }
+      qa[o] = v;
+    }
+    if (sp.use4 && lane < sp.NA) qa[sp.NA * sp.L + lane] = c_kappa4 * p4_value(sS + lane * GNEP_NLM + 3);
+    __syncwarp();
+  };
+  auto next_segment = [&]() {
+    flush_segment();
+    if (++J == sp.T) { atom_epilogue(); J = 0; ++a; }
+    seg_end = a < a_hi ? segA[a * T1 + J + 1] : 0x7fffffff;
+  };
+
+  for (int c0 = P_lo; c0 < P_hi; c0 += 32) {
+    const int p = c0 + lane;
+    if (p < P_hi) {
+      float4 r = pairA[p];
+      float d = sqrtf(r.x * r.x + r.y * r.y + r.z * r.z);
+      float rinv = 1.f / d;
+      float f[KT];
+      cheb_f<KT>(d, sp.rcAinv, f);
+#pragma unroll
+      for (int k = 0; k < KT; ++k) sf[k * ANG_LD + lane] = f[k];
+      blm_unit(r.x * rinv, r.y * rinv, r.z * rinv,
+               [&](int lm, int, float b, float, float, float) { sB[lm * ANG_LD + lane] = b; });
+    } else {   // keep masked lanes finite
+#pragma unroll
+      for (int k = 0; k < KT; ++k) sf[k * ANG_LD + lane] = 0.f;
+#pragma unroll
+      for (int lm = 0; lm < GNEP_NLM; ++lm) sB[lm * ANG_LD + lane] = 0.f;
+    }
+    __syncwarp();
+    const int chunk_end = min(c0 + 32, P_hi);
+    int pos = c0;
+    while (pos < chunk_end) {
+      while (seg_end <= pos) next_segment();
+      const int hi = min(seg_end, chunk_end);
+      const int g0 = (pos - c0) >> 2, g1 = (hi - 1 - c0) >> 2;
+      for (int g = g0; g <= g1; ++g) {
+        const int lo4 = pos - c0 - 4 * g, hi4 = hi - c0 - 4 * g;
+        const bool partial = lo4 > 0 || hi4 < 4;
+        float4 fv[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+          int k = kq + 8 * r;
+          fv[r] = k < KT ? *(const float4 *)(sf + k * ANG_LD + 4 * g) : make_float4(0.f, 0.f, 0.f, 0.f);
+          if (partial) fv[r] = mask4(fv[r], lo4, hi4);
+        }
+#pragma unroll
+        for (int i = 0; i < 6; ++i) {
+          float4 b = *(const float4 *)(sB + (6 * lmq + i) * ANG_LD + 4 * g);
+#pragma unroll
+          for (int r = 0; r < R; ++r) acc[r][i] += dot4(fv[r], b);
+        }
+      }
+      pos = hi;
+    }
+    __syncwarp();
+  }
+  while (a < a_hi) next_segment();
+}
+
+// ------------------------------------------------------------------------------------------------
+// a5 (angular): A2 moments with the pair adjoint a_ij, T_nlm = c.A2, D_(n,l) = sum_m 2 C_lm S_nlm T_nlm, D_4
+// ------------------------------------------------------------------------------------------------
+template <int KT>
+__global__ void __launch_bounds__(ANG_WARPS * 32)
+k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ struct_s,
+              const int *__restrict__ segA, const int *__restrict__ atomA, const float4 *__restrict__ pairA,
+              const float *__restrict__ theta, const float4 *__restrict__ u, const float *__restrict__ omega,
+              const float *__restrict__ scales, const float *__restrict__ S, float *__restrict__ Tn,
+              float *__restrict__ A2, float *__restrict__ D) {
+  constexpr int R = (KT + 7) / 8;
+  extern __shared__ __align__(16) float smem[];
+  float *ct = smem;
+  const int nct = sp.T * sp.T * KT * ANG_NQ;
+  const int nA = sp.T * KT * GNEP_NLM;
+  const int nS = (sp.NA * GNEP_NLM + 3) & ~3;
+  const int per_warp = (2 * KT + 2 * GNEP_NLM) * ANG_LD + nA + 2 * nS;
+  float *sf1 = smem + nct + (threadIdx.x >> 5) * per_warp;   // [KT][LD]  f_k' (a.rhat)
+  float *sf2 = sf1 + KT * ANG_LD;                             // [KT][LD]  f_k
+  float *sX = sf2 + KT * ANG_LD;                              // [24][LD]  B_lm
+  float *sY = sX + GNEP_NLM * ANG_LD;                         // [24][LD]  grad B_lm . a
+  float *As = sY + GNEP_NLM * ANG_LD;                         // [T][KT][24]
+  float *sS = As + nA;                                        // [NA][24]
+  float *sT = sS + nS;                                        // [NA][24]
+  stage_coeff_t(ct, theta + sp.offA, sp.T, sp.NA, sp.KA, KT);
+  __syncthreads();
+  const int lane = threadIdx.x & 31;
+  const int a_lo = (blockIdx.x * ANG_WARPS + (threadIdx.x >> 5)) * ANG_TA;
+  if (a_lo >= N) return;
+  const int a_hi = min(a_lo + ANG_TA, N);
+  const int T1 = sp.T + 1;
+  const int P_lo = segA[a_lo * T1], P_hi = segA[(a_hi - 1) * T1 + sp.T];
+  const int kq = lane >> 2, lmq = lane & 3;
+  const float sfF = scales[1], svV = scales[2];
+  float acc[R][6];
+#pragma unroll
+  for (int r = 0; r < R; ++r)
+#pragma unroll
+    for (int i = 0; i < 6; ++i) acc[r][i] = 0.f;
+  int a = a_lo, J = 0;
+  int seg_end = segA[a * T1 + 1];
+
+  auto flush_segment = [&]() {
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      int k = kq + 8 * r;
+      if (k < KT) {
+        int o = (J * KT + k) * GNEP_NLM + 6 * lmq;
+        float *g = A2 + (size_t)a * nA + o;
+#pragma unroll
+        for (int i = 0; i < 6; i += 2) *(float2 *)(g + i) = make_float2(acc[r][i], acc[r][i + 1]);
+#pragma unroll
+        for (int i = 0; i < 6; ++i) { As[o + i] = acc[r][i]; acc[r][i] = 0.f; }
+      }
+    }
+  };
+  auto atom_epilogue = [&]() {   // T = c.A2, D of atom a
+    const float *Sa = S + (size_t)a * sp.NA * GNEP_NLM;
+    for (int o = lane; o < sp.NA * GNEP_NLM; o += 32) sS[o] = Sa[o];
+    __syncwarp();
+    const int I = type_s[a];
+    float tv[ANG_NQ];
+    contract_moments<KT>(sp, ct, As, I, lane, tv);
+    float *Ta = Tn + (size_t)a * sp.NA * GNEP_NLM;
+    if (lane < GNEP_NLM) {
+#pragma unroll
+      for (int n = 0; n < ANG_NQ; ++n)
+        if (n < sp.NA) { sT[n * GNEP_NLM + lane] = tv[n]; Ta[n * GNEP_NLM + lane] = tv[n]; }
+    }
+    __syncwarp();
+    float *Da = D + (size_t)a * sp.Ndes + sp.NR;
+    for (int o = lane; o < sp.NA * sp.L; o += 32) {
+      int l = o / sp.NA + 1, n = o - (l - 1) * sp.NA;
+      int lm0 = l * l - 1;
+      float v = 0.f;
+      for (int m = 0; m <= 2 * l; ++m) v += c_C2[lm0 + m] * sS[n * GNEP_NLM + lm0 + m] * sT[n * GNEP_NLM + lm0 + m];
+      Da[o] = v;
+    }
+    if (sp.use4 && lane < sp.NA) {
+      float g4[5];
+      p4_grad(sS + lane * GNEP_NLM + 3, g4);
+      float v = 0.f;
+#pragma unroll
+      for (int m = 0; m < 5; ++m) v += g4[m] * sT[lane * GNEP_NLM + 3 + m];
+      Da[sp.NA * sp.L + lane] = c_kappa4 * v;
+    }
+    __syncwarp();
+  };
+  auto next_segment = [&]() {
+    flush_segment();
+    if (++J == sp.T) { atom_epilogue(); J = 0; ++a; }
+    seg_end = a < a_hi ? segA[a * T1 + J + 1] : 0x7fffffff;
+  };
+
+  for (int c0 = P_lo; c0 < P_hi; c0 += 32) {
+    const int p = c0 + lane;
+    if (p < P_hi) {
+      float4 r = pairA[p];
+      const int ai = atomA[p];
+      const int s = struct_s[ai];
+      float4 ui = u[ai], uj = u[__float_as_int(r.w)];
+      float d = sqrtf(r.x * r.x + r.y * r.y + r.z * r.z);
+      float rinv = 1.f / d;
+      const float *om = omega + s * 6;
+      float ax = sfF * (ui.x - uj.x) - svV * (om[0] * r.x + om[5] * r.z);
+      float ay = sfF * (ui.y - uj.y) - svV * (om[1] * r.y + om[3] * r.x);
+      float az = sfF * (ui.z - uj.z) - svV * (om[2] * r.z + om[4] * r.y);
+      float hx = r.x * rinv, hy = r.y * rinv, hz = r.z * rinv;
+      float ar = ax * hx + ay * hy + az * hz;
+      float f[KT], fp[KT];
+      cheb_ffp<KT>(d, sp.rcAinv, f, fp);
+#pragma unroll
+      for (int k = 0; k < KT; ++k) { sf1[k * ANG_LD + lane] = fp[k] * ar; sf2[k * ANG_LD + lane] = f[k]; }
+      blm_unit(hx, hy, hz, [&](int lm, int l, float b, float gx, float gy, float gz) {
+        sX[lm * ANG_LD + lane] = b;
+        sY[lm * ANG_LD + lane] = rinv * ((gx * ax + gy * ay + gz * az) - (float)l * b * ar);
+      });
+    } else {
+#pragma unroll
+      for (int k = 0; k < KT; ++k) { sf1[k * ANG_LD + lane] = 0.f; sf2[k * ANG_LD + lane] = 0.f; }
+#pragma unroll
+      for (int lm = 0; lm < GNEP_NLM; ++lm) { sX[lm * ANG_LD + lane] = 0.f; sY[lm * ANG_LD + lane] = 0.f; }
+    }
+    __syncwarp();
+    const int chunk_end = min(c0 + 32, P_hi);
+    int pos = c0;
+    while (pos < chunk_end) {
+      while (seg_end <= pos) next_segment();
+      const int hi = min(seg_end, chunk_end);
+      const int g0 = (pos - c0) >> 2, g1 = (hi - 1 - c0) >> 2;
+      for (int g = g0; g <= g1; ++g) {
+        const int lo4 = pos - c0 - 4 * g, hi4 = hi - c0 - 4 * g;
+        const bool partial = lo4 > 0 || hi4 < 4;
+        float4 f1[R], f2[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+          int k = kq + 8 * r;
+          const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+          f1[r] = k < KT ? *(const float4 *)(sf1 + k * ANG_LD + 4 * g) : z4;
+          f2[r] = k < KT ? *(const float4 *)(sf2 + k * ANG_LD + 4 * g) : z4;
+          if (partial) { f1[r] = mask4(f1[r], lo4, hi4); f2[r] = mask4(f2[r], lo4, hi4); }
+        }
+#pragma unroll
+        for (int i = 0; i < 6; ++i) {
+          float4 X = *(const float4 *)(sX + (6 * lmq + i) * ANG_LD + 4 * g);
+          float4 Y = *(const float4 *)(sY + (6 * lmq + i) * ANG_LD + 4 * g);
+#pragma unroll
+          for (int r = 0; r < R; ++r) acc[r][i] += dot4(f1[r], X) + dot4(f2[r], Y);
+        }
+      }
+      pos = hi;
+    }
+    __syncwarp();
+  }
+  while (a < a_hi) next_segment();
+}
+
+// ------------------------------------------------------------------------------------------------
+// a3 (angular): f_ij = sum_n sum_lm beta_nlm (g_n' B_lm rhat + g_n grad B_lm)   (C3.6 with C2.1-C2.3)
+// lane = pair over the packed pairs of FRC_TA atoms; beta of the tile's atoms lives in shared memory.
+// gam_lm = sum_n g_n beta_nlm, gamp_lm = sum_n g_n' beta_nlm, then one harmonic sweep.  Writes f_ij per pair.
+// ------------------------------------------------------------------------------------------------
+#define FRC_TA 8
+template <int KT>
+__global__ void __launch_bounds__(ANG_WARPS * 32)
+k_angular_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ segA,
+                const int *__restrict__ atomA, const float4 *__restrict__ pairA, const float *__restrict__ theta,
+                const float *__restrict__ Ep, const float *__restrict__ S, float4 *__restrict__ fpair) {
+  extern __shared__ __align__(16) float smem[];
+  float *cs = smem;
+  const int ncs = (sp.T * sp.T * sp.NA * KT + 3) & ~3;
+  const int nb = sp.NA * GNEP_NLM;
+  float *beta = smem + ncs + (threadIdx.x >> 5) * FRC_TA * nb;
+  stage_coeff(cs, theta + sp.offA, sp.T * sp.T * sp.NA, sp.KA, KT);
+  __syncthreads();
+  const int lane = threadIdx.x & 31;
+  const int a_lo = (blockIdx.x * ANG_WARPS + (threadIdx.x >> 5)) * FRC_TA;
+  if (a_lo >= N) return;
+  const int a_hi = min(a_lo + FRC_TA, N);
+  const int T1 = sp.T + 1;
+  const int P_lo = segA[a_lo * T1], P_hi = segA[(a_hi - 1) * T1 + sp.T];
+  if (P_lo == P_hi) return;
+  for (int a = a_lo; a < a_hi; ++a)
+    make_beta(sp, Ep + (size_t)a * sp.Ndes, S + (size_t)a * nb, beta + (a - a_lo) * nb, lane);
+  __syncwarp();
+  for (int p = P_lo + lane; p < P_hi; p += 32) {
+    float4 r = pairA[p];
+    const int a = atomA[p];
+    const int I = type_s[a];
+    const float *be = beta + (a - a_lo) * nb;
+    float d = sqrtf(r.x * r.x + r.y * r.y + r.z * r.z);
+    float rinv = 1.f / d;
+    int J = type_s[__float_as_int(r.w)];
+    float f[KT], fp[KT];
+    cheb_ffp<KT>(d, sp.rcAinv, f, fp);
+    const float *c = cs + (I * sp.T + J) * sp.NA * KT;
+    float gam[GNEP_NLM], gamp[GNEP_NLM];
+#pragma unroll
+    for (int lm = 0; lm < GNEP_NLM; ++lm) { gam[lm] = 0.f; gamp[lm] = 0.f; }
+    for (int n = 0; n < sp.NA; ++n) {
+      float g = 0.f, gp = 0.f;
+#pragma unroll
+      for (int k = 0; k < KT; ++k) { float cv = c[n * KT + k]; g += cv * f[k]; gp += cv * fp[k]; }
+#pragma unroll
+      for (int v = 0; v < GNEP_NLM / 4; ++v) {
+        float4 b4 = *(const float4 *)(be + n * GNEP_NLM + 4 * v);
+        gam[4 * v] += g * b4.x; gam[4 * v + 1] += g * b4.y; gam[4 * v + 2] += g * b4.z; gam[4 * v + 3] += g * b4.w;
+        gamp[4 * v] += gp * b4.x; gamp[4 * v + 1] += gp * b4.y; gamp[4 * v + 2] += gp * b4.z; gamp[4 * v + 3] += gp * b4.w;
+      }
+    }
+    float hx = r.x * rinv, hy = r.y * rinv, hz = r.z * rinv;
+    float sB = 0.f, sl = 0.f, vx = 0.f, vy = 0.f, vz = 0.f;
+    blm_unit(hx, hy, hz, [&](int lm, int l, float b, float gx, float gy, float gz) {
+      sB += gamp[lm] * b;
+      sl += (float)l * gam[lm] * b;
+      vx += gam[lm] * gx; vy += gam[lm] * gy; vz += gam[lm] * gz;
+    });
+    fpair[p] = make_float4(hx * sB + rinv * (vx - hx * sl), hy * sB + rinv * (vy - hy * sl),
+                           hz * sB + rinv * (vz - hz * sl), 0.f);
+  }
+}
+
+// F_i += sum_{p in row i} (f_p - f_rev(p)),  W_i -= sum_p r_p (x) f_p   (Eq.3, Eq.4 for the angular part; no
+// atomics).  Half a warp per atom.
+__global__ void __launch_bounds__(256)
+k_force_gather(int N, int T1, const int *__restrict__ segA, const int *__restrict__ revA,
+               const float4 *__restrict__ pairA, const float4 *__restrict__ fpair, float4 *__restrict__ Fat,
+               float *__restrict__ Wat) {
+  const int a = (blockIdx.x * blockDim.x + threadIdx.x) >> 4;
+  const int sub = threadIdx.x & 15;
+  float F[3] = {0.f, 0.f, 0.f}, W[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  if (a < N) {
+    const int p0 = segA[a * T1], p1 = segA[a * T1 + T1 - 1];
+    for (int p = p0 + sub; p < p1; p += 16) {
+      float4 f = fpair[p], g = fpair[revA[p]], r = pairA[p];
+      F[0] += f.x - g.x; F[1] += f.y - g.y; F[2] += f.z - g.z;
+      W[0] -= r.x * f.x; W[1] -= r.y * f.y; W[2] -= r.z * f.z;
+      W[3] -= r.x * f.y; W[4] -= r.y * f.z; W[5] -= r.z * f.x;
+    }
+  }
+#pragma unroll
+  for (int o = 8; o > 0; o >>= 1) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) F[c] += __shfl_xor_sync(0xffffffffu, F[c], o);
+#pragma unroll
+    for (int c = 0; c < 6; ++c) W[c] += __shfl_xor_sync(0xffffffffu, W[c], o);
+  }
+  if (a < N && sub == 0) {
+    float4 o = Fat[a];
+    Fat[a] = make_float4(o.x + F[0], o.y + F[1], o.z + F[2], 0.f);
+#pragma unroll
+    for (int c = 0; c < 6; ++c) Wat[(size_t)a * 6 + c] += W[c];
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a7 (angular): dL/dcA[I][J][n][k] = sum_atoms sum_lm alpha_nlm A1[J][k][lm] + beta_nlm A2[J][k][lm]
+//   alpha_nlm = gbar_(n,l) 2C_lm S_nlm + E'_(n,l) 2C_lm T_nlm (+ 4-body: gbar_4 k4 dP4/ds_m + E'_4 k4 (H4 T)_m)
+//   beta_nlm  = E'_(n,l) 2C_lm S_nlm (+ E'_4 k4 dP4/ds_m)
+// One warp per atom (grid-stride); lane = ((J,k) row, half of n).  Each warp keeps a [T][T][NA][KT] accumulator in
+// shared memory over the atoms it visits and writes one partial at the end (reduced by k_grad_reduce).
+// ------------------------------------------------------------------------------------------------
+template <int KT>
+__global__ void __launch_bounds__(ANG_WARPS * 32)
+k_cgrad_angular(DevSpec sp, int N, const int *__restrict__ type_s, const float *__restrict__ Ep,
+                const float *__restrict__ gbar, const float *__restrict__ S, const float *__restrict__ Tn,
+                const float *__restrict__ A1, const float *__restrict__ A2, float *__restrict__ partial) {
+  extern __shared__ __align__(16) float smem[];
+  const int nacc = sp.T * sp.T * sp.NA * KT;
+  const int nb = sp.NA * GNEP_NLM;
+  const int nA = sp.T * KT * GNEP_NLM;
+  const int per_warp = ((nacc + 3) & ~3) + 4 * ((nb + 3) & ~3);
+  float *accS = smem + (threadIdx.x >> 5) * per_warp;
+  float *sS = accS + ((nacc + 3) & ~3);
+  float *sT = sS + ((nb + 3) & ~3);
+  float *sAl = sT + ((nb + 3) & ~3);
+  float *sBe = sAl + ((nb + 3) & ~3);
+  const int lane = threadIdx.x & 31;
+  const int gw = blockIdx.x * ANG_WARPS + (threadIdx.x >> 5);
+  const int nw = gridDim.x * ANG_WARPS;
+  for (int o = lane; o < nacc; o += 32) accS[o] = 0.f;
+  __syncwarp();
+  const int rows = sp.T * KT;                      // (J,k) rows of A1/A2
+  const int nh = (sp.NA + 1) >> 1;                 // n's per half
+  for (int a = gw; a < N; a += nw) {
+    const int I = type_s[a];
+    const float *Sa = S + (size_t)a * nb, *Ta = Tn + (size_t)a * nb;
+    const float *Epa = Ep + (size_t)a * sp.Ndes, *gba = gbar + (size_t)a * sp.Ndes;
+    for (int o = lane; o < nb; o += 32) { sS[o] = Sa[o]; sT[o] = Ta[o]; }
+    __syncwarp();
+    for (int o = lane; o < nb; o += 32) {
+      int n = o / GNEP_NLM, lm = o - n * GNEP_NLM;
+      int l = l_of_lm(lm);
+      float al = 0.f, be = 0.f;
+      if (l <= sp.L) {
+        int v = sp.NR + (l - 1) * sp.NA + n;
+        float e1 = Epa[v];
+        al = c_C2[lm] * (gba[v] * sS[o] + e1 * sT[o]);
+        be = c_C2[lm] * e1 * sS[o];
+      }
+      if (sp.use4 && lm >= 3 && lm < 8) {
+        int v4 = sp.NR + sp.L * sp.NA + n;
+        float g4[5], hv[5];
+        p4_grad(sS + n * GNEP_NLM + 3, g4);
+        p4_hess_vec(sS + n * GNEP_NLM + 3, sT + n * GNEP_NLM + 3, hv);
+        int m = lm - 3;
+        float g = m == 0 ? g4[0] : m == 1 ? g4[1] : m == 2 ? g4[2] : m == 3 ? g4[3] : g4[4];
+        float h = m == 0 ? hv[0] : m == 1 ? hv[1] : m == 2 ? hv[2] : m == 3 ? hv[3] : hv[4];
+        float e4 = Epa[v4];
+        al += c_kappa4 * (gba[v4] * g + e4 * h);
+        be += c_kappa4 * e4 * g;
+      }
+      sAl[o] = al; sBe[o] = be;
+    }
+    __syncwarp();
+    // contraction: lane -> row = lane>>1 (+16 per round), half = lane&1 -> n in [half*nh, min(NA, half*nh+nh))
+    const int half = lane & 1;
+    const int n_lo = half * nh, n_hi = min(sp.NA, n_lo + nh);
+    for (int row = lane >> 1; row < rows; row += 16) {
+      const float4 *a1 = (const float4 *)(A1 + (size_t)a * nA + row * GNEP_NLM);
+      const float4 *a2 = (const float4 *)(A2 + (size_t)a * nA + row * GNEP_NLM);
+      float4 x1[6], x2[6];
+#pragma unroll
+      for (int v = 0; v < 6; ++v) { x1[v] = __ldg(a1 + v); x2[v] = __ldg(a2 + v); }
+      const int J = row / KT, k = row - J * KT;
+      float *dst = accS + ((I * sp.T + J) * sp.NA) * KT + k;
+      for (int n = n_lo; n < n_hi; ++n) {
+        float s = 0.f;
+#pragma unroll
+        for (int v = 0; v < 6; ++v) {
+          float4 al4 = *(const float4 *)(sAl + n * GNEP_NLM + 4 * v);
+          float4 be4 = *(const float4 *)(sBe + n * GNEP_NLM + 4 * v);
+          s += dot4(al4, x1[v]) + dot4(be4, x2[v]);
+        }
+        dst[n * KT] += s;
+      }
+    }
+    __syncwarp();
+  }
+  for (int o = lane; o < nacc; o += 32) partial[(size_t)gw * nacc + o] = accS[o];
+}

@@ -14,6 +14,7 @@
 #include "neighbor.cuh"
 #include "net_kernels.cuh"
 #include "pair_kernels.cuh"
+#include "angular_kernels.cuh"
 #include "reduce_kernels.cuh"
 
 namespace {
@@ -44,7 +45,7 @@ struct gnep_handle {
   int hasE = 0, hasF = 0, hasV = 0;
   double Ng = -1, Sg = -1, l2_share = 1.0;   // job-wide normalisers when structures are sharded over ranks
   std::vector<void *> batch_allocs;
-  int *perm = nullptr, *type_s = nullptr, *struct_s = nullptr, *segR = nullptr, *rowAs = nullptr, *revA = nullptr;
+  int *perm = nullptr, *type_s = nullptr, *struct_s = nullptr, *segR = nullptr, *rowAs = nullptr, *revA = nullptr, *segA = nullptr, *atomA = nullptr;
   float4 *pairR = nullptr, *pairA = nullptr;
   int64_t *exp_row[2] = {nullptr, nullptr};
   int *exp_j[2] = {nullptr, nullptr}, *exp_sh[2] = {nullptr, nullptr};
@@ -56,7 +57,7 @@ struct gnep_handle {
   int n_cta_net = 0, n_chunks = 0, n_ca_blocks = 0;
   // per-atom state
   float *q = nullptr, *Sn = nullptr, *x = nullptr, *Ei = nullptr, *Ep = nullptr, *etil = nullptr, *M1 = nullptr,
-        *M2 = nullptr, *D = nullptr, *Tn = nullptr, *gbar = nullptr, *Acoef = nullptr, *Bcoef = nullptr, *Wat = nullptr;
+        *M2 = nullptr, *D = nullptr, *Tn = nullptr, *A1 = nullptr, *A2 = nullptr, *gbar = nullptr, *Acoef = nullptr, *Bcoef = nullptr, *Wat = nullptr;
   float4 *Fat = nullptr, *fpair = nullptr, *u = nullptr;
   double *Es = nullptr, *Ws = nullptr, *parts = nullptr;
   float *e_s = nullptr, *omega = nullptr;
@@ -127,16 +128,15 @@ void free_batch(gnep_handle *h) {
 // ---- dynamic shared memory sizes (bytes) --------------------------------------------------------
 size_t smem_radial(const DevSpec &d) { return sizeof(float) * (d.T * d.T * d.NR * d.KRp + GNEP_WARPS * (d.KRp * 33 + d.KRp)); }
 size_t smem_ang_fwd(const DevSpec &d) {
-  return sizeof(float) * (((d.T * d.T * d.NA * d.KAp + 3) & ~3) + GNEP_WARPS * ((d.NA + GNEP_NLM) * 32 + d.NA * GNEP_NLM));
+  return sizeof(float) * (d.T * d.T * d.KAp * ANG_NQ + ANG_WARPS * ((d.KAp + GNEP_NLM) * ANG_LD + d.T * d.KAp * GNEP_NLM + ((d.NA * GNEP_NLM + 3) & ~3)));
 }
-size_t smem_ang_force(const DevSpec &d) { return sizeof(float) * (((d.T * d.T * d.NA * d.KAp + 3) & ~3) + GNEP_WARPS * d.NA * GNEP_NLM); }
+size_t smem_ang_force(const DevSpec &d) { return sizeof(float) * (((d.T * d.T * d.NA * d.KAp + 3) & ~3) + ANG_WARPS * FRC_TA * d.NA * GNEP_NLM); }
 size_t smem_ang_adj(const DevSpec &d) {
-  return sizeof(float) * (((d.T * d.T * d.NA * d.KAp + 3) & ~3) + GNEP_WARPS * ((2 * d.NA + 2 * GNEP_NLM) * 32 + 2 * d.NA * GNEP_NLM));
+  return sizeof(float) * (d.T * d.T * d.KAp * ANG_NQ + ANG_WARPS * ((2 * d.KAp + 2 * GNEP_NLM) * ANG_LD + d.T * d.KAp * GNEP_NLM + 2 * ((d.NA * GNEP_NLM + 3) & ~3)));
 }
 size_t smem_cgrad_ang(const DevSpec &d) {
-  int NAp = d.NA | 1, KTp = d.KAp + 1;
   int nacc = d.T * d.T * d.NA * d.KAp;
-  return sizeof(float) * GNEP_WARPS * (((nacc + 3) & ~3) + 4 * d.NA * GNEP_NLM + 32 * (2 * NAp + 2 * KTp));
+  return sizeof(float) * ANG_WARPS * (((nacc + 3) & ~3) + 4 * ((d.NA * GNEP_NLM + 3) & ~3));
 }
 size_t smem_net_fwd(const DevSpec &d) {
   return sizeof(float) * (net_smem_floats(d) + ((d.T * d.NR * d.KRp + 3) & ~3) + GNEP_WARPS * (d.Ndes + d.Nn + d.NR) * GNEP_TILE);
@@ -207,7 +207,7 @@ int enqueue_descriptors(gnep_handle *h) {
   int gridA = cdiv(h->N, GNEP_WARPS);
   DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_fwd<KT>, gridA, GNEP_WARPS * 32, smem_radial(d), d, h->N, h->type_s, h->segR, h->pairR, h->theta, h->q, h->M1));
   mark(h, "a1_radial_descriptor");
-  DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_fwd<KT>, gridA, GNEP_WARPS * 32, smem_ang_fwd(d), d, h->N, h->type_s, h->rowAs, h->pairA, h->theta, h->q, h->Sn));
+  DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_fwd<KT>, cdiv(h->N, ANG_WARPS * ANG_TA), ANG_WARPS * 32, smem_ang_fwd(d), d, h->N, h->type_s, h->segA, h->pairA, h->theta, h->q, h->Sn, h->A1));
   mark(h, "a1_angular_descriptor");
   return GNEP_OK;
 }
@@ -229,9 +229,9 @@ int enqueue_forward(gnep_handle *h) {
   mark(h, "a2_network_forward");
   DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_force<KT>, gridA, GNEP_WARPS * 32, 0, d, h->N, h->type_s, h->segR, h->pairR, h->etil, h->Fat, h->Wat));
   mark(h, "a3_radial_force");
-  DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_force<KT>, gridA, GNEP_WARPS * 32, smem_ang_force(d), d, h->N, h->type_s, h->rowAs, h->pairA, h->theta, h->Ep, h->Sn, h->fpair, h->Fat, h->Wat));
+  DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_force<KT>, cdiv(h->N, ANG_WARPS * FRC_TA), ANG_WARPS * 32, smem_ang_force(d), d, h->N, h->type_s, h->segA, h->atomA, h->pairA, h->theta, h->Ep, h->Sn, h->fpair));
   mark(h, "a3_angular_force");
-  LAUNCH(h, k_force_gather, gridA, GNEP_WARPS * 32, 0, h->N, h->rowAs, h->revA, h->fpair, h->Fat);
+  LAUNCH(h, k_force_gather, cdiv((int64_t)h->N * 16, 256), 256, 0, h->N, d.T + 1, h->segA, h->revA, h->pairA, h->fpair, h->Fat, h->Wat);
   mark(h, "a3_force_gather");
   LAUNCH(h, k_struct_reduce, h->S, 128, 0, loss_cfg(h), h->srange, h->Ei, h->Fat, h->Wat, h->Eref, h->Fref_s, h->Wref, h->Es, h->Ws, h->e_s, h->u, h->omega, h->parts);
   LAUNCH(h, k_loss_final, 1, 256, 0, loss_cfg(h), h->parts, h->theta, h->terms, h->scales);
@@ -245,7 +245,7 @@ int enqueue_backward(gnep_handle *h) {
   int gridA = cdiv(h->N, GNEP_WARPS);
   DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_adj<KT>, gridA, GNEP_WARPS * 32, smem_radial(d), d, h->N, h->type_s, h->struct_s, h->segR, h->pairR, h->theta, h->u, h->omega, h->scales, h->D, h->M2));
   mark(h, "a5_radial_adjoint");
-  DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_adj<KT>, gridA, GNEP_WARPS * 32, smem_ang_adj(d), d, h->N, h->type_s, h->struct_s, h->rowAs, h->pairA, h->theta, h->u, h->omega, h->scales, h->Sn, h->Tn, h->D));
+  DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_adj<KT>, cdiv(h->N, ANG_WARPS * ANG_TA), ANG_WARPS * 32, smem_ang_adj(d), d, h->N, h->type_s, h->struct_s, h->segA, h->atomA, h->pairA, h->theta, h->u, h->omega, h->scales, h->Sn, h->Tn, h->A2, h->D));
   mark(h, "a5_angular_adjoint");
   LAUNCH(h, k_net_bwd, h->n_cta_net, GNEP_WARPS * 32, smem_net_bwd(d), d, h->sm, h->theta, h->qscale, h->struct_s, h->e_s, h->scales, h->x, h->Ep, h->D, h->Acoef, h->Bcoef, h->gbar, h->partialB);
   mark(h, "a6_network_backward");
@@ -253,7 +253,7 @@ int enqueue_backward(gnep_handle *h) {
   mark(h, "a6_w0_gradient");
   LAUNCH(h, k_cgrad_radial, h->n_chunks, 256, smem_cgrad_rad(d), d, h->sm, h->gbar, h->Ep, h->M1, h->M2, h->partialCR);
   mark(h, "a7_radial_cgrad");
-  DISPATCH_KT(d.KAp, LAUNCH(h, k_cgrad_angular<KT>, h->n_ca_blocks, GNEP_WARPS * 32, smem_cgrad_ang(d), d, h->N, h->type_s, h->struct_s, h->rowAs, h->pairA, h->u, h->omega, h->scales, h->Ep, h->gbar, h->Sn, h->Tn, h->partialCA));
+  DISPATCH_KT(d.KAp, LAUNCH(h, k_cgrad_angular<KT>, h->n_ca_blocks, ANG_WARPS * 32, smem_cgrad_ang(d), d, h->N, h->type_s, h->Ep, h->gbar, h->Sn, h->Tn, h->A1, h->A2, h->partialCA));
   mark(h, "a7_angular_cgrad");
   LAUNCH(h, k_grad_reduce, cdiv(d.P, 256), 256, 0, d, h->rm, (float)h->l2_share, h->theta, h->scales, h->partialCR, h->partialCA, h->partialW, h->partialB, h->grad);
   mark(h, "a8_grad_reduce");
@@ -601,7 +601,7 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     // ---- persistent batch arrays ----
     int rc_;
 #define BA(ptr, n) if ((rc_ = dalloc(h, &(ptr), (n), true)) != GNEP_OK) { tfree(); free_batch(h); return rc_; }
-    BA(h->perm, N); BA(h->type_s, N); BA(h->struct_s, N); BA(h->segR, (size_t)N * (T + 1) + 1); BA(h->rowAs, N + 1); BA(h->revA, nA);
+    BA(h->perm, N); BA(h->type_s, N); BA(h->struct_s, N); BA(h->segR, (size_t)N * (T + 1) + 1); BA(h->rowAs, N + 1); BA(h->revA, nA); BA(h->segA, (size_t)N * (T + 1) + 1); BA(h->atomA, nA);
     BA(h->pairR, nR); BA(h->pairA, nA);
     BA(h->exp_row[0], N + 1); BA(h->exp_row[1], N + 1); BA(h->exp_j[0], nR); BA(h->exp_sh[0], nR); BA(h->exp_j[1], nA); BA(h->exp_sh[1], nA);
     BA(h->srange, srange.size()); BA(h->Eref, S); BA(h->Wref, (size_t)S * 6); BA(h->Fref_s, (size_t)N * 3);
@@ -620,7 +620,7 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     CKT(cudaMemcpyAsync(h->srange, srange.data(), sizeof(int) * srange.size(), cudaMemcpyHostToDevice, st));
     LAUNCH(h, k_nbr_fill, gN, 128, 0, N, d_struct_of, d_geo, d_wpos, d_binid, d_bin_start, d_bin_atoms, rcR2, rcA2, h->exp_row[0], d_ekey, d_er);
     LAUNCH(h, k_nbr_scatter, cdiv((int64_t)N * 32, 256), 256, 0, N, T, d_struct_of, d_geo, d_type, d_inv, h->exp_row[0], h->exp_row[1], d_rowRs,
-           h->rowAs, d_ekey, d_er, h->exp_j[0], h->exp_sh[0], h->exp_j[1], h->exp_sh[1], h->pairR, h->pairA, d_shA, h->segR);
+           h->rowAs, d_ekey, d_er, h->exp_j[0], h->exp_sh[0], h->exp_j[1], h->exp_sh[1], h->pairR, h->pairA, d_shA, h->segR, h->segA, h->atomA);
     LAUNCH(h, k_nbr_reverse, cdiv((int64_t)N * 32, 256), 256, 0, N, h->rowAs, h->pairA, d_shA, h->revA);
     CKT(cudaGetLastError());
     CKT(cudaStreamSynchronize(st));
@@ -638,13 +638,13 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     }
     h->n_cta_net = h->sm.cta_base[GNEP_MAX_SPECIES_C];
     h->n_chunks = h->sm.chunk_base[GNEP_MAX_SPECIES_C];
-    h->n_ca_blocks = std::max(1, std::min(cdiv(N, GNEP_WARPS), 2 * h->num_sms));
+    h->n_ca_blocks = std::max(1, std::min(cdiv(N, ANG_WARPS), 4 * h->num_sms));
     for (int t = 0; t <= GNEP_MAX_SPECIES_C; ++t) { h->rm.chunk_base[t] = h->sm.chunk_base[t]; h->rm.cta_base[t] = h->sm.cta_base[t]; }
-    h->rm.n_warps_ca = N > 0 ? h->n_ca_blocks * GNEP_WARPS : 0;
+    h->rm.n_warps_ca = N > 0 ? h->n_ca_blocks * ANG_WARPS : 0;
     // ---- per-atom state ----
     const size_t n = N;
     BA(h->q, n * d.Ndes); BA(h->Sn, n * d.NA * GNEP_NLM); BA(h->x, n * d.Nn); BA(h->Ei, n); BA(h->Ep, n * d.Ndes);
-    BA(h->etil, n * T * d.KRp); BA(h->M1, n * T * d.KRp); BA(h->M2, n * T * d.KRp); BA(h->D, n * d.Ndes); BA(h->Tn, n * d.NA * GNEP_NLM);
+    BA(h->etil, n * T * d.KRp); BA(h->M1, n * T * d.KRp); BA(h->M2, n * T * d.KRp); BA(h->D, n * d.Ndes); BA(h->Tn, n * d.NA * GNEP_NLM); BA(h->A1, n * T * d.KAp * GNEP_NLM); BA(h->A2, n * T * d.KAp * GNEP_NLM);
     BA(h->gbar, n * d.Ndes); BA(h->Acoef, n * d.Nn); BA(h->Bcoef, n * d.Nn); BA(h->Wat, n * 6);
     BA(h->Fat, n); BA(h->fpair, nA); BA(h->u, n);
     BA(h->Es, S); BA(h->Ws, (size_t)S * 6); BA(h->parts, (size_t)S * 3); BA(h->e_s, S); BA(h->omega, (size_t)S * 6);

@@ -147,7 +147,8 @@ __global__ void k_nbr_scatter(int N, int T, const int *__restrict__ struct_of, c
                               const unsigned long long *__restrict__ ekey, const float *__restrict__ er,
                               int *__restrict__ expR_j, int *__restrict__ expR_sh, int *__restrict__ expA_j,
                               int *__restrict__ expA_sh, float4 *__restrict__ pairR, float4 *__restrict__ pairA,
-                              int *__restrict__ shA, int *__restrict__ segR) {
+                              int *__restrict__ shA, int *__restrict__ segR, int *__restrict__ segA,
+                              int *__restrict__ atomA) {
   int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   int lane = threadIdx.x & 31;
   if (i >= N) return;
@@ -157,7 +158,7 @@ __global__ void k_nbr_scatter(int N, int T, const int *__restrict__ struct_of, c
   int baseRs = rowRs[a], baseAs = rowAs[a];
   int64_t baseA = rowA[i];
   const unsigned long long KM = KEY_ANG_BIT - 1;
-  int cntJ[4] = {0, 0, 0, 0};   // GNEP_MAX_SPECIES
+  int cntJ[4] = {0, 0, 0, 0}, cntJA[4] = {0, 0, 0, 0};   // GNEP_MAX_SPECIES
   for (int64_t e = r0 + lane; e < r1; e += 32) {
     unsigned long long ke = ekey[e];
     bool ang = (ke & KEY_ANG_BIT) != 0;
@@ -184,6 +185,8 @@ __global__ void k_nbr_scatter(int N, int T, const int *__restrict__ struct_of, c
       expA_j[baseA + rankCA] = j; expA_sh[baseA + rankCA] = sh;
       pairA[baseAs + rankIA] = rec;
       shA[baseAs + rankIA] = sh;
+      atomA[baseAs + rankIA] = a;
+      cntJA[J] += 1;
     }
     cntJ[J] += 1;
   }
@@ -197,6 +200,15 @@ __global__ void k_nbr_scatter(int N, int T, const int *__restrict__ struct_of, c
     run += c;
   }
   if (lane == 0) segR[a * (T + 1) + T] = run;
+  run = baseAs;
+  for (int t = 0; t < T; ++t) {
+    int c = cntJA[t];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+    if (lane == 0) segA[a * (T + 1) + t] = run;
+    run += c;
+  }
+  if (lane == 0) segA[a * (T + 1) + T] = run;
 }
 
 // reverse-pair index of the internal angular list: rev[p] = index of (j -> i, -shift).  Warp per atom.
