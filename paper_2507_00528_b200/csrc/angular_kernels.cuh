@@ -40,28 +40,52 @@ __device__ __forceinline__ float4 mask4(float4 v, int lo4, int hi4) {
 }
 __device__ __forceinline__ float dot4(const float4 &a, const float4 &b) { return a.x * b.x + a.y * b.y + a.z * b.z + a.w * b.w; }
 
-// X_nlm = sum_{J,k} c[I][J][n][k] A[J][k][lm] for one atom: lane = lm (24 lanes), NA outputs per lane.
-template <int KT>
-__device__ __forceinline__ void contract_moments(const DevSpec &sp, const float *ct, const float *As, int I, int lane,
-                                                 float (&out)[ANG_NQ]) {
+// Per-atom lane layout "(n, lmg)": lane = 3*nq + lmg (lanes 0..29), n = nb + nq for nb = 0, 10, ..., and the lane owns
+// lm in [8 lmg, 8 lmg + 8): lmg 0 = all of l=1 (i<3) and l=2; lmg 1 = all of l=3 (i<7) and the first slot of l=4;
+// lmg 2 = the rest of l=4.  Everything per-atom (S, T, beta, alpha, q_nl, D_nl) is produced in this layout with static
+// register indexing and 2*C_lm held in registers (no divergent constant-memory indexing in the hot loops).
+struct NLane {
+  int nq, lmg, la, lb, split;
+  bool act;
+  float c2[8];
+};
+__device__ __forceinline__ NLane make_nlane(int lane) {
+  NLane L;
+  L.nq = lane / 3; L.lmg = lane - 3 * L.nq; L.act = lane < 30;
+  L.la = L.lmg == 0 ? 1 : L.lmg == 1 ? 3 : 4;
+  L.lb = L.lmg == 0 ? 2 : 4;
+  L.split = L.lmg == 0 ? 3 : L.lmg == 1 ? 7 : 8;
 #pragma unroll
-  for (int n = 0; n < ANG_NQ; ++n) out[n] = 0.f;
-  if (lane >= GNEP_NLM) return;
-  const int nq = (sp.NA + 3) >> 2;
+  for (int i = 0; i < 8; ++i) L.c2[i] = c_C2[8 * (L.lmg < 3 ? L.lmg : 0) + i];
+  return L;
+}
+// E'-like value of descriptor (n, l) of one atom row (0 when l > l_max)
+__device__ __forceinline__ float desc_of(const DevSpec &sp, const float *__restrict__ row, int l, int n) {
+  return l <= sp.L ? row[sp.NR + (l - 1) * sp.NA + n] : 0.f;
+}
+// X[n][8 lmg .. +8] = sum_{J,k} c[I][J][n][k] A[J][k][lm]  (S = c.A1, T = c.A2)
+template <int KT>
+__device__ __forceinline__ void contract_nl(const DevSpec &sp, const float *ct, const float *As, int I, int n, int lmg,
+                                            float (&out)[8]) {
+#pragma unroll
+  for (int i = 0; i < 8; ++i) out[i] = 0.f;
   for (int J = 0; J < sp.T; ++J) {
-    const float *cj = ct + (I * sp.T + J) * KT * ANG_NQ;
+    const float *cj = ct + (I * sp.T + J) * KT * ANG_NQ + n;
+    const float *aj = As + J * KT * GNEP_NLM + 8 * lmg;
 #pragma unroll
     for (int k = 0; k < KT; ++k) {
-      float a = As[(J * KT + k) * GNEP_NLM + lane];
-#pragma unroll
-      for (int v = 0; v < ANG_NQ / 4; ++v) {
-        if (v < nq) {
-          float4 c4 = *(const float4 *)(cj + k * ANG_NQ + 4 * v);
-          out[4 * v] += c4.x * a; out[4 * v + 1] += c4.y * a; out[4 * v + 2] += c4.z * a; out[4 * v + 3] += c4.w * a;
-        }
-      }
+      float c = cj[k * ANG_NQ];
+      float4 a0 = *(const float4 *)(aj + k * GNEP_NLM), a1 = *(const float4 *)(aj + k * GNEP_NLM + 4);
+      out[0] += c * a0.x; out[1] += c * a0.y; out[2] += c * a0.z; out[3] += c * a0.w;
+      out[4] += c * a1.x; out[5] += c * a1.y; out[6] += c * a1.z; out[7] += c * a1.w;
     }
   }
+}
+// sums of w[i] over the lane's two l-blocks
+__device__ __forceinline__ void split_sums(const NLane &nl, const float (&w)[8], float &sa, float &sb) {
+  sa = 0.f; sb = 0.f;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) { if (i < nl.split) sa += w[i]; else sb += w[i]; }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -77,11 +101,10 @@ k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   float *ct = smem;
   const int nct = sp.T * sp.T * KT * ANG_NQ;
   const int nA = sp.T * KT * GNEP_NLM;
-  const int per_warp = (KT + GNEP_NLM) * ANG_LD + nA + ((sp.NA * GNEP_NLM + 3) & ~3);
+  const int per_warp = (KT + GNEP_NLM) * ANG_LD + nA;
   float *sf = smem + nct + (threadIdx.x >> 5) * per_warp;   // [KT][LD]
   float *sB = sf + KT * ANG_LD;                              // [24][LD]
   float *As = sB + GNEP_NLM * ANG_LD;                        // [T][KT][24]
-  float *sS = As + nA;                                       // [NA][24]
   stage_coeff_t(ct, theta + sp.offA, sp.T, sp.NA, sp.KA, KT);
   __syncthreads();
   const int lane = threadIdx.x & 31;
@@ -91,6 +114,7 @@ k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   const int T1 = sp.T + 1;
   const int P_lo = segA[a_lo * T1], P_hi = segA[(a_hi - 1) * T1 + sp.T];
   const int kq = lane >> 2, lmq = lane & 3;
+  const NLane nl = make_nlane(lane);
   float acc[R][6];
 #pragma unroll
   for (int r = 0; r < R; ++r)
@@ -116,24 +140,32 @@ k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   auto atom_epilogue = [&]() {   // S = c.A1, q_nl, q4 of atom a
     __syncwarp();
     const int I = type_s[a];
-    float sv[ANG_NQ];
-    contract_moments<KT>(sp, ct, As, I, lane, sv);
     float *Sa = S + (size_t)a * sp.NA * GNEP_NLM;
-    if (lane < GNEP_NLM) {
-#pragma unroll
-      for (int n = 0; n < ANG_NQ; ++n)
-        if (n < sp.NA) { sS[n * GNEP_NLM + lane] = sv[n]; Sa[n * GNEP_NLM + lane] = sv[n]; }
-    }
-    __syncwarp();
     float *qa = q + (size_t)a * sp.Ndes + sp.NR;
-    for (int o = lane; o < sp.NA * sp.L; o += 32) {
-      int l = o / sp.NA + 1, n = o - (l - 1) * sp.NA;
-      int lm0 = l * l - 1;
-      float v = 0.f;
-      for (int m = 0; m <= 2 * l; ++m) { float s = sS[n * GNEP_NLM + lm0 + m]; v += 0.5f * c_C2[lm0 + m] * s * s; }
-      qa[o] = v;
+    for (int nb = 0; nb < sp.NA; nb += 10) {
+      const int n = nb + nl.nq;
+      const bool on = nl.act && n < sp.NA;
+      float sv[8], qa_ = 0.f, qb_ = 0.f;
+      if (on) {
+        contract_nl<KT>(sp, ct, As, I, n, nl.lmg, sv);
+        *(float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg) = make_float4(sv[0], sv[1], sv[2], sv[3]);
+        *(float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg + 4) = make_float4(sv[4], sv[5], sv[6], sv[7]);
+        float w[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) w[i] = 0.5f * nl.c2[i] * sv[i] * sv[i];
+        split_sums(nl, w, qa_, qb_);
+      }
+      const float nxt = __shfl_down_sync(0xffffffffu, qa_, 1);     // the l=4 remainder held by (n, lmg 2)
+      if (on && nl.lmg == 0) {
+        qa[n] = qa_;
+        if (sp.L >= 2) qa[sp.NA + n] = qb_;
+        if (sp.use4) qa[sp.NA * sp.L + n] = c_kappa4 * p4_value(sv + 3);
+      }
+      if (on && nl.lmg == 1) {
+        if (sp.L >= 3) qa[2 * sp.NA + n] = qa_;
+        if (sp.L >= 4) qa[3 * sp.NA + n] = qb_ + nxt;
+      }
     }
-    if (sp.use4 && lane < sp.NA) qa[sp.NA * sp.L + lane] = c_kappa4 * p4_value(sS + lane * GNEP_NLM + 3);
     __syncwarp();
   };
   auto next_segment = [&]() {
@@ -206,15 +238,12 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   float *ct = smem;
   const int nct = sp.T * sp.T * KT * ANG_NQ;
   const int nA = sp.T * KT * GNEP_NLM;
-  const int nS = (sp.NA * GNEP_NLM + 3) & ~3;
-  const int per_warp = (2 * KT + 2 * GNEP_NLM) * ANG_LD + nA + 2 * nS;
+  const int per_warp = (2 * KT + 2 * GNEP_NLM) * ANG_LD + nA;
   float *sf1 = smem + nct + (threadIdx.x >> 5) * per_warp;   // [KT][LD]  f_k' (a.rhat)
   float *sf2 = sf1 + KT * ANG_LD;                             // [KT][LD]  f_k
   float *sX = sf2 + KT * ANG_LD;                              // [24][LD]  B_lm
   float *sY = sX + GNEP_NLM * ANG_LD;                         // [24][LD]  grad B_lm . a
   float *As = sY + GNEP_NLM * ANG_LD;                         // [T][KT][24]
-  float *sS = As + nA;                                        // [NA][24]
-  float *sT = sS + nS;                                        // [NA][24]
   stage_coeff_t(ct, theta + sp.offA, sp.T, sp.NA, sp.KA, KT);
   __syncthreads();
   const int lane = threadIdx.x & 31;
@@ -224,6 +253,7 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   const int T1 = sp.T + 1;
   const int P_lo = segA[a_lo * T1], P_hi = segA[(a_hi - 1) * T1 + sp.T];
   const int kq = lane >> 2, lmq = lane & 3;
+  const NLane nl = make_nlane(lane);
   const float sfF = scales[1], svV = scales[2];
   float acc[R][6];
 #pragma unroll
@@ -248,34 +278,40 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
     }
   };
   auto atom_epilogue = [&]() {   // T = c.A2, D of atom a
-    const float *Sa = S + (size_t)a * sp.NA * GNEP_NLM;
-    for (int o = lane; o < sp.NA * GNEP_NLM; o += 32) sS[o] = Sa[o];
     __syncwarp();
     const int I = type_s[a];
-    float tv[ANG_NQ];
-    contract_moments<KT>(sp, ct, As, I, lane, tv);
+    const float *Sa = S + (size_t)a * sp.NA * GNEP_NLM;
     float *Ta = Tn + (size_t)a * sp.NA * GNEP_NLM;
-    if (lane < GNEP_NLM) {
-#pragma unroll
-      for (int n = 0; n < ANG_NQ; ++n)
-        if (n < sp.NA) { sT[n * GNEP_NLM + lane] = tv[n]; Ta[n * GNEP_NLM + lane] = tv[n]; }
-    }
-    __syncwarp();
     float *Da = D + (size_t)a * sp.Ndes + sp.NR;
-    for (int o = lane; o < sp.NA * sp.L; o += 32) {
-      int l = o / sp.NA + 1, n = o - (l - 1) * sp.NA;
-      int lm0 = l * l - 1;
-      float v = 0.f;
-      for (int m = 0; m <= 2 * l; ++m) v += c_C2[lm0 + m] * sS[n * GNEP_NLM + lm0 + m] * sT[n * GNEP_NLM + lm0 + m];
-      Da[o] = v;
-    }
-    if (sp.use4 && lane < sp.NA) {
-      float g4[5];
-      p4_grad(sS + lane * GNEP_NLM + 3, g4);
-      float v = 0.f;
+    for (int nb = 0; nb < sp.NA; nb += 10) {
+      const int n = nb + nl.nq;
+      const bool on = nl.act && n < sp.NA;
+      float tv[8], sv[8], da = 0.f, db = 0.f;
+      if (on) {
+        float4 s0 = *(const float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg), s1 = *(const float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg + 4);
+        sv[0] = s0.x; sv[1] = s0.y; sv[2] = s0.z; sv[3] = s0.w; sv[4] = s1.x; sv[5] = s1.y; sv[6] = s1.z; sv[7] = s1.w;
+        contract_nl<KT>(sp, ct, As, I, n, nl.lmg, tv);
+        *(float4 *)(Ta + n * GNEP_NLM + 8 * nl.lmg) = make_float4(tv[0], tv[1], tv[2], tv[3]);
+        *(float4 *)(Ta + n * GNEP_NLM + 8 * nl.lmg + 4) = make_float4(tv[4], tv[5], tv[6], tv[7]);
+        float w[8];
 #pragma unroll
-      for (int m = 0; m < 5; ++m) v += g4[m] * sT[lane * GNEP_NLM + 3 + m];
-      Da[sp.NA * sp.L + lane] = c_kappa4 * v;
+        for (int i = 0; i < 8; ++i) w[i] = nl.c2[i] * sv[i] * tv[i];
+        split_sums(nl, w, da, db);
+      }
+      const float nxt = __shfl_down_sync(0xffffffffu, da, 1);
+      if (on && nl.lmg == 0) {
+        Da[n] = da;
+        if (sp.L >= 2) Da[sp.NA + n] = db;
+        if (sp.use4) {
+          float g4[5];
+          p4_grad(sv + 3, g4);
+          Da[sp.NA * sp.L + n] = c_kappa4 * (g4[0] * tv[3] + g4[1] * tv[4] + g4[2] * tv[5] + g4[3] * tv[6] + g4[4] * tv[7]);
+        }
+      }
+      if (on && nl.lmg == 1) {
+        if (sp.L >= 3) Da[2 * sp.NA + n] = da;
+        if (sp.L >= 4) Da[3 * sp.NA + n] = db + nxt;
+      }
     }
     __syncwarp();
   };
@@ -353,7 +389,7 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
 // lane = pair over the packed pairs of FRC_TA atoms; beta of the tile's atoms lives in shared memory.
 // gam_lm = sum_n g_n beta_nlm, gamp_lm = sum_n g_n' beta_nlm, then one harmonic sweep.  Writes f_ij per pair.
 // ------------------------------------------------------------------------------------------------
-#define FRC_TA 8
+#define FRC_TA 16
 template <int KT>
 __global__ void __launch_bounds__(ANG_WARPS * 32)
 k_angular_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ segA,
@@ -373,8 +409,32 @@ k_angular_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__
   const int T1 = sp.T + 1;
   const int P_lo = segA[a_lo * T1], P_hi = segA[(a_hi - 1) * T1 + sp.T];
   if (P_lo == P_hi) return;
-  for (int a = a_lo; a < a_hi; ++a)
-    make_beta(sp, Ep + (size_t)a * sp.Ndes, S + (size_t)a * nb, beta + (a - a_lo) * nb, lane);
+  {   // beta_nlm = E'_(n,l) 2C_lm S_nlm (+ E'_4 kappa4 dP4/ds_m), (n, lmg) lane layout
+    const NLane nl = make_nlane(lane);
+    for (int a = a_lo; a < a_hi; ++a) {
+      const float *Sa = S + (size_t)a * nb, *Epa = Ep + (size_t)a * sp.Ndes;
+      for (int n0 = 0; n0 < sp.NA; n0 += 10) {
+        const int n = n0 + nl.nq;
+        if (nl.act && n < sp.NA) {
+          float4 s0 = *(const float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg), s1 = *(const float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg + 4);
+          float sv[8] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w}, bv[8];
+          const float ea = desc_of(sp, Epa, nl.la, n), eb = desc_of(sp, Epa, nl.lb, n);
+#pragma unroll
+          for (int i = 0; i < 8; ++i) bv[i] = (i < nl.split ? ea : eb) * nl.c2[i] * sv[i];
+          if (sp.use4 && nl.lmg == 0) {
+            float g4[5];
+            p4_grad(sv + 3, g4);
+            const float e4 = c_kappa4 * Epa[sp.NR + sp.L * sp.NA + n];
+#pragma unroll
+            for (int m = 0; m < 5; ++m) bv[3 + m] += e4 * g4[m];
+          }
+          float *dst = beta + (a - a_lo) * nb + n * GNEP_NLM + 8 * nl.lmg;
+          *(float4 *)dst = make_float4(bv[0], bv[1], bv[2], bv[3]);
+          *(float4 *)(dst + 4) = make_float4(bv[4], bv[5], bv[6], bv[7]);
+        }
+      }
+    }
+  }
   __syncwarp();
   for (int p = P_lo + lane; p < P_hi; p += 32) {
     float4 r = pairA[p];
@@ -462,13 +522,12 @@ k_cgrad_angular(DevSpec sp, int N, const int *__restrict__ type_s, const float *
   const int nacc = sp.T * sp.T * sp.NA * KT;
   const int nb = sp.NA * GNEP_NLM;
   const int nA = sp.T * KT * GNEP_NLM;
-  const int per_warp = ((nacc + 3) & ~3) + 4 * ((nb + 3) & ~3);
+  const int per_warp = ((nacc + 3) & ~3) + 2 * ((nb + 3) & ~3);
   float *accS = smem + (threadIdx.x >> 5) * per_warp;
-  float *sS = accS + ((nacc + 3) & ~3);
-  float *sT = sS + ((nb + 3) & ~3);
-  float *sAl = sT + ((nb + 3) & ~3);
+  float *sAl = accS + ((nacc + 3) & ~3);
   float *sBe = sAl + ((nb + 3) & ~3);
   const int lane = threadIdx.x & 31;
+  const NLane nl = make_nlane(lane);
   const int gw = blockIdx.x * ANG_WARPS + (threadIdx.x >> 5);
   const int nw = gridDim.x * ANG_WARPS;
   for (int o = lane; o < nacc; o += 32) accS[o] = 0.f;
@@ -479,31 +538,37 @@ k_cgrad_angular(DevSpec sp, int N, const int *__restrict__ type_s, const float *
     const int I = type_s[a];
     const float *Sa = S + (size_t)a * nb, *Ta = Tn + (size_t)a * nb;
     const float *Epa = Ep + (size_t)a * sp.Ndes, *gba = gbar + (size_t)a * sp.Ndes;
-    for (int o = lane; o < nb; o += 32) { sS[o] = Sa[o]; sT[o] = Ta[o]; }
-    __syncwarp();
-    for (int o = lane; o < nb; o += 32) {
-      int n = o / GNEP_NLM, lm = o - n * GNEP_NLM;
-      int l = l_of_lm(lm);
-      float al = 0.f, be = 0.f;
-      if (l <= sp.L) {
-        int v = sp.NR + (l - 1) * sp.NA + n;
-        float e1 = Epa[v];
-        al = c_C2[lm] * (gba[v] * sS[o] + e1 * sT[o]);
-        be = c_C2[lm] * e1 * sS[o];
+    for (int n0 = 0; n0 < sp.NA; n0 += 10) {      // alpha, beta in the (n, lmg) lane layout
+      const int n = n0 + nl.nq;
+      if (nl.act && n < sp.NA) {
+        const int o = n * GNEP_NLM + 8 * nl.lmg;
+        float4 s0 = *(const float4 *)(Sa + o), s1 = *(const float4 *)(Sa + o + 4);
+        float4 t0 = *(const float4 *)(Ta + o), t1 = *(const float4 *)(Ta + o + 4);
+        float sv[8] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
+        float tv[8] = {t0.x, t0.y, t0.z, t0.w, t1.x, t1.y, t1.z, t1.w};
+        const float ea = desc_of(sp, Epa, nl.la, n), eb = desc_of(sp, Epa, nl.lb, n);
+        const float ga = desc_of(sp, gba, nl.la, n), gb = desc_of(sp, gba, nl.lb, n);
+        float al[8], be[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+          const float e1 = i < nl.split ? ea : eb, g1 = i < nl.split ? ga : gb;
+          al[i] = nl.c2[i] * (g1 * sv[i] + e1 * tv[i]);
+          be[i] = nl.c2[i] * e1 * sv[i];
+        }
+        if (sp.use4 && nl.lmg == 0) {
+          const int v4 = sp.NR + sp.L * sp.NA + n;
+          float g4[5], hv[5];
+          p4_grad(sv + 3, g4);
+          p4_hess_vec(sv + 3, tv + 3, hv);
+          const float e4 = c_kappa4 * Epa[v4], gb4 = c_kappa4 * gba[v4];
+#pragma unroll
+          for (int m = 0; m < 5; ++m) { al[3 + m] += gb4 * g4[m] + e4 * hv[m]; be[3 + m] += e4 * g4[m]; }
+        }
+        *(float4 *)(sAl + o) = make_float4(al[0], al[1], al[2], al[3]);
+        *(float4 *)(sAl + o + 4) = make_float4(al[4], al[5], al[6], al[7]);
+        *(float4 *)(sBe + o) = make_float4(be[0], be[1], be[2], be[3]);
+        *(float4 *)(sBe + o + 4) = make_float4(be[4], be[5], be[6], be[7]);
       }
-      if (sp.use4 && lm >= 3 && lm < 8) {
-        int v4 = sp.NR + sp.L * sp.NA + n;
-        float g4[5], hv[5];
-        p4_grad(sS + n * GNEP_NLM + 3, g4);
-        p4_hess_vec(sS + n * GNEP_NLM + 3, sT + n * GNEP_NLM + 3, hv);
-        int m = lm - 3;
-        float g = m == 0 ? g4[0] : m == 1 ? g4[1] : m == 2 ? g4[2] : m == 3 ? g4[3] : g4[4];
-        float h = m == 0 ? hv[0] : m == 1 ? hv[1] : m == 2 ? hv[2] : m == 3 ? hv[3] : hv[4];
-        float e4 = Epa[v4];
-        al += c_kappa4 * (gba[v4] * g + e4 * h);
-        be += c_kappa4 * e4 * g;
-      }
-      sAl[o] = al; sBe[o] = be;
     }
     __syncwarp();
     // contraction: lane -> row = lane>>1 (+16 per round), half = lane&1 -> n in [half*nh, min(NA, half*nh+nh))

@@ -128,15 +128,15 @@ void free_batch(gnep_handle *h) {
 // ---- dynamic shared memory sizes (bytes) --------------------------------------------------------
 size_t smem_radial(const DevSpec &d) { return sizeof(float) * (d.T * d.T * d.NR * d.KRp + GNEP_WARPS * (d.KRp * 33 + d.KRp)); }
 size_t smem_ang_fwd(const DevSpec &d) {
-  return sizeof(float) * (d.T * d.T * d.KAp * ANG_NQ + ANG_WARPS * ((d.KAp + GNEP_NLM) * ANG_LD + d.T * d.KAp * GNEP_NLM + ((d.NA * GNEP_NLM + 3) & ~3)));
+  return sizeof(float) * (d.T * d.T * d.KAp * ANG_NQ + ANG_WARPS * ((d.KAp + GNEP_NLM) * ANG_LD + d.T * d.KAp * GNEP_NLM));
 }
 size_t smem_ang_force(const DevSpec &d) { return sizeof(float) * (((d.T * d.T * d.NA * d.KAp + 3) & ~3) + ANG_WARPS * FRC_TA * d.NA * GNEP_NLM); }
 size_t smem_ang_adj(const DevSpec &d) {
-  return sizeof(float) * (d.T * d.T * d.KAp * ANG_NQ + ANG_WARPS * ((2 * d.KAp + 2 * GNEP_NLM) * ANG_LD + d.T * d.KAp * GNEP_NLM + 2 * ((d.NA * GNEP_NLM + 3) & ~3)));
+  return sizeof(float) * (d.T * d.T * d.KAp * ANG_NQ + ANG_WARPS * ((2 * d.KAp + 2 * GNEP_NLM) * ANG_LD + d.T * d.KAp * GNEP_NLM));
 }
 size_t smem_cgrad_ang(const DevSpec &d) {
   int nacc = d.T * d.T * d.NA * d.KAp;
-  return sizeof(float) * ANG_WARPS * (((nacc + 3) & ~3) + 4 * ((d.NA * GNEP_NLM + 3) & ~3));
+  return sizeof(float) * ANG_WARPS * (((nacc + 3) & ~3) + 2 * ((d.NA * GNEP_NLM + 3) & ~3));
 }
 size_t smem_net_fwd(const DevSpec &d) {
   return sizeof(float) * (net_smem_floats(d) + ((d.T * d.NR * d.KRp + 3) & ~3) + GNEP_WARPS * (d.Ndes + d.Nn + d.NR) * GNEP_TILE);

@@ -36,18 +36,19 @@ def phase_flops(spec, n_atoms, n_pairs_radial, n_pairs_angular):
     geom = 12                                      # d, 1/d, rhat
     f = {}
     f["a1_radial_descriptor"] = nR * (geom + _basis_f(KR) + KR) + N * 2 * T * KR * NR
-    f["a1_angular_descriptor"] = nA * (geom + _basis_f(KA) + 2 * NA * KA + HARM_B + 2 * NA * NLM) + N * (3 * NA * NLM + 60 * NA)
+    moments = 2 * T * KA * NA * NLM                  # S = c.A1 / T = c.A2 per atom (moment form)
+    f["a1_angular_descriptor"] = nA * (geom + _basis_f(KA) + HARM_B + 2 * KA * NLM) + N * (moments + 3 * NA * NLM + 60 * NA)
     f["a2_network_forward"] = N * (4 * Nn * Nd + 2 * T * KR * NR + 12 * Nn)
     f["a3_radial_force"] = nR * (geom + _basis_ffp(KR) + 4 * KR + 30)
     f["a3_angular_force"] = nA * (geom + _basis_ffp(KA) + 4 * NA * KA + 4 * NA * NLM + HARM_BG + 9 * NLM + 40) + N * 3 * NA * NLM
     f["a3_force_gather"] = nA * 3
     f["a4_loss_and_seeds"] = N * 20
     f["a5_radial_adjoint"] = nR * (geom + _basis_ffp(KR) + 2 * KR + 30) + N * 2 * T * KR * NR
-    f["a5_angular_adjoint"] = nA * (geom + _basis_ffp(KA) + 4 * NA * KA + HARM_BG + 8 * NLM + 4 * NA * NLM + 30) + N * 3 * NA * NLM
+    f["a5_angular_adjoint"] = nA * (geom + _basis_ffp(KA) + 2 * KA + HARM_BG + 8 * NLM + 4 * KA * NLM + 30) + N * (moments + 3 * NA * NLM)
     f["a6_network_backward"] = N * (4 * Nn * Nd + 16 * Nn + 2 * Nd)
     f["a6_w0_gradient"] = N * 4 * Nn * Nd
     f["a7_radial_cgrad"] = N * 4 * NR * T * KR
-    f["a7_angular_cgrad"] = nA * (geom + _basis_ffp(KA) + HARM_BG + 8 * NLM + 6 * NA * NLM + 4 * NA * KA + 30) + N * 10 * NA * NLM
+    f["a7_angular_cgrad"] = N * (2 * moments + 12 * NA * NLM)     # sum_lm alpha A1 + beta A2; no pair sweep
     f["a8_grad_reduce"] = 0
     f["a9_adam"] = 0
     return f
@@ -61,20 +62,21 @@ def phase_bytes(spec, n_atoms, n_pairs_radial, n_pairs_angular):
     N, nR, nA = n_atoms, n_pairs_radial, n_pairs_angular
     S_ = 4 * NA * NLM                 # bytes of S or T per atom
     M_ = 4 * T * KR                   # bytes of a radial moment row per atom
+    A_ = 4 * T * spec["n_basis_angular"] * NLM   # bytes of A1 or A2 per atom
     b = {}
     b["a1_radial_descriptor"] = 16 * nR + N * (M_ + 4 * NR)
-    b["a1_angular_descriptor"] = 16 * nA + N * (S_ + 4 * (Nd - NR))
+    b["a1_angular_descriptor"] = 16 * nA + N * (S_ + A_ + 4 * (Nd - NR))
     b["a2_network_forward"] = N * (4 * Nd + 4 * Nn + 4 + 4 * Nd + M_)
     b["a3_radial_force"] = (16 + 4 * KR) * nR + N * (M_ + 16 + 24)
-    b["a3_angular_force"] = (16 + 16) * nA + N * (S_ + 4 * Nd + 16 + 24)
-    b["a3_force_gather"] = (4 + 16) * nA + N * 32
+    b["a3_angular_force"] = (16 + 4 + 16) * nA + N * (S_ + 4 * Nd)
+    b["a3_force_gather"] = (4 + 16 + 16 + 16) * nA + N * 2 * (16 + 24)
     b["a4_loss_and_seeds"] = N * (4 + 16 + 24 + 12 + 16)
     b["a5_radial_adjoint"] = (16 + 16) * nR + N * (M_ + 4 * NR + 16)
-    b["a5_angular_adjoint"] = (16 + 16) * nA + N * (2 * S_ + 4 * (Nd - NR) + 16)
+    b["a5_angular_adjoint"] = (16 + 4 + 16) * nA + N * (2 * S_ + A_ + 4 * (Nd - NR) + 16)
     b["a6_network_backward"] = N * (4 * Nd * 3 + 4 * Nn * 3)
     b["a6_w0_gradient"] = N * (8 * Nn + 8 * Nd)
     b["a7_radial_cgrad"] = N * (8 * NR + 2 * M_)
-    b["a7_angular_cgrad"] = (16 + 16) * nA + N * (2 * S_ + 8 * Nd + 16)
+    b["a7_angular_cgrad"] = N * (2 * S_ + 2 * A_ + 8 * Nd)
     b["a8_grad_reduce"] = 0
     b["a9_adam"] = 0
     return b
