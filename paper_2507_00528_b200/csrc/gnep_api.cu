@@ -142,9 +142,10 @@ size_t smem_net_fwd(const DevSpec &d) {
   return sizeof(float) * (net_smem_floats(d) + ((d.T * d.NR * d.KRp + 3) & ~3) + GNEP_WARPS * (d.Ndes + d.Nn + d.NR) * GNEP_TILE);
 }
 size_t smem_net_bwd(const DevSpec &d) {
-  return sizeof(float) * (net_smem_floats(d) + ((GNEP_WARPS * (2 * d.Nn + 1) + 3) & ~3) + GNEP_WARPS * (d.Ndes + d.Nn) * GNEP_TILE);
+  return sizeof(float) * (net_smem_floats(d) + ((GNEP_WARPS * (2 * d.Nn + 1) + 3) & ~3) + GNEP_WARPS * (d.Ndes + d.Nn + 1) * GNEP_TILE);
 }
-size_t smem_gemm_w0(const DevSpec &d) { return sizeof(float) * GW_SUB * 2 * (d.Nn + d.Ndes); }
+size_t smem_gemm_w0(const DevSpec &d) { return sizeof(float) * GW_SUB * 2 * (gw_ldm(d) + gw_ldn(d)); }
+int threads_gemm_w0(const DevSpec &d) { return (((gw_ldm(d) >> 2) * (gw_ldn(d) >> 3) + 31) / 32) * 32; }
 size_t smem_cgrad_rad(const DevSpec &d) { return sizeof(float) * CR_SUB * 2 * (d.NR + d.T * d.KRp); }
 
 template <class K>
@@ -249,13 +250,13 @@ int enqueue_backward(gnep_handle *h) {
   mark(h, "a5_angular_adjoint");
   LAUNCH(h, k_net_bwd, h->n_cta_net, GNEP_WARPS * 32, smem_net_bwd(d), d, h->sm, h->theta, h->qscale, h->struct_s, h->e_s, h->scales, h->x, h->Ep, h->D, h->Acoef, h->Bcoef, h->gbar, h->partialB);
   mark(h, "a6_network_backward");
-  LAUNCH(h, k_gemm_w0, h->n_chunks, 256, smem_gemm_w0(d), d, h->sm, h->qscale, h->q, h->D, h->Acoef, h->Bcoef, h->partialW);
+  LAUNCH(h, k_gemm_w0, h->n_chunks, threads_gemm_w0(d), smem_gemm_w0(d), d, h->sm, h->qscale, h->q, h->D, h->Acoef, h->Bcoef, h->partialW);
   mark(h, "a6_w0_gradient");
   LAUNCH(h, k_cgrad_radial, h->n_chunks, 256, smem_cgrad_rad(d), d, h->sm, h->gbar, h->Ep, h->M1, h->M2, h->partialCR);
   mark(h, "a7_radial_cgrad");
   DISPATCH_KT(d.KAp, LAUNCH(h, k_cgrad_angular<KT>, h->n_ca_blocks, ANG_WARPS * 32, smem_cgrad_ang(d), d, h->N, h->type_s, h->Ep, h->gbar, h->Sn, h->Tn, h->A1, h->A2, h->partialCA));
   mark(h, "a7_angular_cgrad");
-  LAUNCH(h, k_grad_reduce, cdiv(d.P, 256), 256, 0, d, h->rm, (float)h->l2_share, h->theta, h->scales, h->partialCR, h->partialCA, h->partialW, h->partialB, h->grad);
+  LAUNCH(h, k_grad_reduce, cdiv(d.P, 8), 256, 0, d, h->rm, (float)h->l2_share, h->theta, h->scales, h->partialCR, h->partialCA, h->partialW, h->partialB, h->grad);
   mark(h, "a8_grad_reduce");
   return GNEP_OK;
 }

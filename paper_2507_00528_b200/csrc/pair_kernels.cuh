@@ -86,9 +86,20 @@ k_radial_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__r
       float f[KT], fp[KT];
       cheb_ffp<KT>(d, sp.rcRinv, f, fp);
       const float *ej = etil + (size_t)j * TK + I * KT;
+      float ejv[KT];
+      if (KT % 4 == 0) {
+#pragma unroll
+        for (int k = 0; k < KT / 4; ++k) {
+          float4 v = __ldg((const float4 *)ej + k);
+          ejv[4 * k] = v.x; ejv[4 * k + 1] = v.y; ejv[4 * k + 2] = v.z; ejv[4 * k + 3] = v.w;
+        }
+      } else {
+#pragma unroll
+        for (int k = 0; k < KT / 2; ++k) { float2 v = __ldg((const float2 *)ej + k); ejv[2 * k] = v.x; ejv[2 * k + 1] = v.y; }
+      }
       float si = 0.f, sj = 0.f;
 #pragma unroll
-      for (int k = 0; k < KT; ++k) { si += ei[k] * fp[k]; sj += __ldg(ej + k) * fp[k]; }
+      for (int k = 0; k < KT; ++k) { si += ei[k] * fp[k]; sj += ejv[k] * fp[k]; }
       float hx = r.x * rinv, hy = r.y * rinv, hz = r.z * rinv;
       float tot = si + sj;
       F[0] += tot * hx; F[1] += tot * hy; F[2] += tot * hz;
@@ -105,26 +116,6 @@ k_radial_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__r
     Fat[a] = make_float4(F[0], F[1], F[2], 0.f);
 #pragma unroll
     for (int c = 0; c < 6; ++c) Wat[(size_t)a * 6 + c] = W[c];
-  }
-}
-
-// beta_nlm = sum_{nu in n} E'_nu dq_nu/dS_nlm  for one atom, into per-warp shared memory [NA][24]
-__device__ __forceinline__ void make_beta(const DevSpec &sp, const float *__restrict__ Ep_a,
-                                          const float *__restrict__ S_a, float *beta, int lane) {
-  for (int o = lane; o < sp.NA * GNEP_NLM; o += 32) {
-    int n = o / GNEP_NLM, lm = o - n * GNEP_NLM;
-    int l = l_of_lm(lm);
-    float be = 0.f;
-    if (l <= sp.L) be = Ep_a[sp.NR + (l - 1) * sp.NA + n] * c_C2[lm] * S_a[o];
-    if (sp.use4 && lm >= 3 && lm < 8) {
-      float s5[5], g4[5];
-#pragma unroll
-      for (int m = 0; m < 5; ++m) s5[m] = S_a[n * GNEP_NLM + 3 + m];
-      p4_grad(s5, g4);
-      float g = lm == 3 ? g4[0] : lm == 4 ? g4[1] : lm == 5 ? g4[2] : lm == 6 ? g4[3] : g4[4];
-      be += Ep_a[sp.NR + sp.L * sp.NA + n] * c_kappa4 * g;
-    }
-    beta[o] = be;
   }
 }
 

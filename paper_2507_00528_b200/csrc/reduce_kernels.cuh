@@ -117,37 +117,49 @@ struct ReduceMap {
   int cta_base[GNEP_MAX_SPECIES_C + 1];     // network CTAs (b0, w1, b1 partials) per species
   int n_warps_ca;                           // partial rows of the angular c-gradient
 };
+// Block = 8 consecutive parameters x 32 row lanes: every lane sums rows lane, lane+32, ... of its parameter's partial
+// buffer in fp64, the 32 lane sums are added in lane order by one thread (fixed order -> bit-reproducible).
 __global__ void __launch_bounds__(256)
 k_grad_reduce(DevSpec sp, ReduceMap rm, float l2_share, const float *__restrict__ theta, const float *__restrict__ scales,
               const float *__restrict__ partialCR, const float *__restrict__ partialCA,
               const float *__restrict__ partialW, const float *__restrict__ partialB, float *__restrict__ grad) {
-  int p = blockIdx.x * blockDim.x + threadIdx.x;
-  if (p >= sp.P) return;
+  __shared__ double sh[32][9];
+  const int tx = threadIdx.x & 7, ty = threadIdx.x >> 3;
+  const int p = blockIdx.x * 8 + tx;
   double s = 0.0;
-  if (p < sp.offA) {                       // cR[I][J][n][k]
-    int k = p % sp.KR, r = p / sp.KR;
-    int n = r % sp.NR; r /= sp.NR;
-    int J = r % sp.T, I = r / sp.T;
-    int O = sp.NR * sp.T * sp.KRp, o = n * sp.T * sp.KRp + J * sp.KRp + k;
-    for (int c = rm.chunk_base[I]; c < rm.chunk_base[I + 1]; ++c) s += (double)partialCR[(size_t)c * O + o];
-  } else if (p < sp.offNet) {              // cA[I][J][n][k]
-    int x = p - sp.offA;
-    int k = x % sp.KA, r = x / sp.KA;      // r = (I*T+J)*NA + n
-    int O = sp.T * sp.T * sp.NA * sp.KAp, o = r * sp.KAp + k;
-    for (int w = 0; w < rm.n_warps_ca; ++w) s += (double)partialCA[(size_t)w * O + o];
-  } else {
-    int x = p - sp.offNet;
-    int t = x / sp.netSize, y = x - t * sp.netSize;
-    int nW = sp.Nn * sp.Ndes;
-    if (y < nW) {
-      for (int c = rm.chunk_base[t]; c < rm.chunk_base[t + 1]; ++c) s += (double)partialW[(size_t)c * nW + y];
+  if (p < sp.P) {
+    const float *base; size_t stride; int r0, r1;
+    if (p < sp.offA) {                       // cR[I][J][n][k]
+      int k = p % sp.KR, r = p / sp.KR;
+      int n = r % sp.NR; r /= sp.NR;
+      int J = r % sp.T, I = r / sp.T;
+      stride = (size_t)sp.NR * sp.T * sp.KRp;
+      base = partialCR + n * sp.T * sp.KRp + J * sp.KRp + k;
+      r0 = rm.chunk_base[I]; r1 = rm.chunk_base[I + 1];
+    } else if (p < sp.offNet) {              // cA[I][J][n][k]
+      int x = p - sp.offA;
+      int k = x % sp.KA, r = x / sp.KA;      // r = (I*T+J)*NA + n
+      stride = (size_t)sp.T * sp.T * sp.NA * sp.KAp;
+      base = partialCA + r * sp.KAp + k;
+      r0 = 0; r1 = rm.n_warps_ca;
     } else {
-      int nb = 2 * sp.Nn + 1;
-      for (int c = rm.cta_base[t]; c < rm.cta_base[t + 1]; ++c) s += (double)partialB[(size_t)c * nb + (y - nW)];
+      int x = p - sp.offNet;
+      int t = x / sp.netSize, y = x - t * sp.netSize;
+      int nW = sp.Nn * sp.Ndes;
+      if (y < nW) { stride = nW; base = partialW + y; r0 = rm.chunk_base[t]; r1 = rm.chunk_base[t + 1]; }
+      else { stride = 2 * sp.Nn + 1; base = partialB + (y - nW); r0 = rm.cta_base[t]; r1 = rm.cta_base[t + 1]; }
     }
+    for (int r = r0 + ty; r < r1; r += 32) s += (double)base[(size_t)r * stride];
   }
-  s += 2.0 * (double)l2_share * (double)sp.lam_2 * (double)scales[3] * (double)theta[p] / (double)sp.P;
-  grad[p] = (float)s;
+  sh[ty][tx] = s;
+  __syncthreads();
+  if (ty == 0 && p < sp.P) {
+    double t = 0.0;
+#pragma unroll
+    for (int r = 0; r < 32; ++r) t += sh[r][tx];
+    t += 2.0 * (double)l2_share * (double)sp.lam_2 * (double)scales[3] * (double)theta[p] / (double)sp.P;
+    grad[p] = (float)t;
+  }
 }
 
 // a9: textbook Adam with bias correction (Kingma & Ba Alg.1); step counter on the device (graph-safe).
