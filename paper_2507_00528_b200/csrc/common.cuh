@@ -6,7 +6,6 @@
 
 #define GNEP_NLM 24           // (l,m) slots for l = 1..4
 #define GNEP_WARPS 8          // warps per CTA of the warp-per-atom kernels
-#define GNEP_TILE 16          // atoms per warp tile of the network kernels
 #define GNEP_MAX_SPECIES_C 4   // == GNEP_MAX_SPECIES of include/gnep.h
 
 // Model constants passed by value to every kernel.

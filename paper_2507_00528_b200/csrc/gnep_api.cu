@@ -12,7 +12,7 @@
 
 #include "common.cuh"
 #include "neighbor.cuh"
-#include "net_kernels.cuh"
+#include "net_kernels.cuh"   // includes net_tc_kernels.cuh (tensor-core network)
 #include "pair_kernels.cuh"
 #include "angular_kernels.cuh"
 #include "reduce_kernels.cuh"
@@ -54,10 +54,10 @@ struct gnep_handle {
   float *Fref_s = nullptr;
   SpeciesMap sm{};
   ReduceMap rm{};
-  int n_cta_net = 0, n_chunks = 0, n_ca_blocks = 0;
+  int n_cta_net = 0, n_chunks = 0, n_ca_blocks = 0, n_gw = 0;
   // per-atom state
   float *q = nullptr, *Sn = nullptr, *x = nullptr, *Ei = nullptr, *Ep = nullptr, *etil = nullptr, *M1 = nullptr,
-        *M2 = nullptr, *D = nullptr, *Tn = nullptr, *A1 = nullptr, *A2 = nullptr, *gbar = nullptr, *Acoef = nullptr, *Bcoef = nullptr, *Wat = nullptr;
+        *M2 = nullptr, *D = nullptr, *Tn = nullptr, *A1 = nullptr, *A2 = nullptr, *gbar = nullptr, *pbuf = nullptr, *Wat = nullptr;
   float4 *Fat = nullptr, *fpair = nullptr, *u = nullptr;
   double *Es = nullptr, *Ws = nullptr, *parts = nullptr;
   float *e_s = nullptr, *omega = nullptr;
@@ -138,19 +138,14 @@ size_t smem_cgrad_ang(const DevSpec &d) {
   int nacc = d.T * d.T * d.NA * d.KAp;
   return sizeof(float) * ANG_WARPS * (((nacc + 3) & ~3) + 2 * ((d.NA * GNEP_NLM + 3) & ~3));
 }
-size_t smem_net_fwd(const DevSpec &d) {
-  return sizeof(float) * (net_smem_floats(d) + ((d.T * d.NR * d.KRp + 3) & ~3) + GNEP_WARPS * (d.Ndes + d.Nn + d.NR) * GNEP_TILE);
-}
-size_t smem_net_bwd(const DevSpec &d) {
-  return sizeof(float) * (net_smem_floats(d) + ((GNEP_WARPS * (2 * d.Nn + 1) + 3) & ~3) + GNEP_WARPS * (d.Ndes + d.Nn + 1) * GNEP_TILE);
-}
-size_t smem_gemm_w0(const DevSpec &d) { return sizeof(float) * GW_SUB * 2 * (gw_ldm(d) + gw_ldn(d)); }
-int threads_gemm_w0(const DevSpec &d) { return (((gw_ldm(d) >> 2) * (gw_ldn(d) >> 3) + 31) / 32) * 32; }
+size_t smem_net_fwd(const DevSpec &d) { return net_tc_smem_bytes(d, false); }
+size_t smem_net_bwd(const DevSpec &d) { return net_tc_smem_bytes(d, true); }
+size_t smem_gradw(const DevSpec &d) { return gradw_smem_bytes(d); }
 size_t smem_cgrad_rad(const DevSpec &d) { return sizeof(float) * CR_SUB * 2 * (d.NR + d.T * d.KRp); }
 
 template <class K>
 int set_smem(gnep_handle *h, K kernel, size_t bytes) {
-  if (bytes > 227 * 1024) return fail(h, GNEP_EINVAL, "model too large for shared memory staging");
+  if (bytes > 227 * 1024) return fail(h, GNEP_EINVAL, "model too large for shared memory staging (n_neurons x n_descriptors)");
   CK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
   return GNEP_OK;
 }
@@ -160,9 +155,13 @@ int configure_kernels(gnep_handle *h) {
   DISPATCH_KT(d.KRp, RET_IF(set_smem(h, k_radial_fwd<KT>, smem_radial(d))); RET_IF(set_smem(h, k_radial_adj<KT>, smem_radial(d))));
   DISPATCH_KT(d.KAp, RET_IF(set_smem(h, k_angular_fwd<KT>, smem_ang_fwd(d))); RET_IF(set_smem(h, k_angular_force<KT>, smem_ang_force(d)));
               RET_IF(set_smem(h, k_angular_adj<KT>, smem_ang_adj(d))); RET_IF(set_smem(h, k_cgrad_angular<KT>, smem_cgrad_ang(d))));
-  RET_IF(set_smem(h, k_net_fwd, smem_net_fwd(d)));
-  RET_IF(set_smem(h, k_net_bwd, smem_net_bwd(d)));
-  RET_IF(set_smem(h, k_gemm_w0, smem_gemm_w0(d)));
+  {   // TMEM budget of one k_net_tc warpgroup (256 columns): D1 + max(D1 corrections, D2 + D2 corrections)
+    const NetDims nd = net_dims(d);
+    if (nd.NnP + std::max(nd.NnP, 2 * nd.NdN) > 256) return fail(h, GNEP_EINVAL, "model too large for tensor memory (n_neurons, n_descriptors)");
+  }
+  RET_IF(set_smem(h, k_net_tc<false>, smem_net_fwd(d)));
+  RET_IF(set_smem(h, k_net_tc<true>, smem_net_bwd(d)));
+  RET_IF(set_smem(h, k_gradw_tc, smem_gradw(d)));
   RET_IF(set_smem(h, k_cgrad_radial, smem_cgrad_rad(d)));
   return GNEP_OK;
 }
@@ -226,7 +225,8 @@ int enqueue_forward(gnep_handle *h) {
   const DevSpec &d = h->ds;
   int gridA = cdiv(h->N, GNEP_WARPS);
   RET_IF(enqueue_descriptors(h));
-  LAUNCH(h, k_net_fwd, h->n_cta_net, GNEP_WARPS * 32, smem_net_fwd(d), d, h->sm, h->theta, h->qscale, h->q, h->x, h->Ei, h->Ep, h->etil);
+  LAUNCH(h, k_net_tc<false>, h->n_cta_net, 256, smem_net_fwd(d), d, h->sm, h->theta, h->qscale, h->q, h->x, h->Ei, h->Ep, h->etil,
+         (const int *)nullptr, (const float *)nullptr, (const float *)nullptr, (float *)nullptr, (float *)nullptr);
   mark(h, "a2_network_forward");
   DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_force<KT>, gridA, GNEP_WARPS * 32, 0, d, h->N, h->type_s, h->segR, h->pairR, h->etil, h->Fat, h->Wat));
   mark(h, "a3_radial_force");
@@ -248,9 +248,10 @@ int enqueue_backward(gnep_handle *h) {
   mark(h, "a5_radial_adjoint");
   DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_adj<KT>, cdiv(h->N, ANG_WARPS * ANG_TA), ANG_WARPS * 32, smem_ang_adj(d), d, h->N, h->type_s, h->struct_s, h->segA, h->atomA, h->pairA, h->theta, h->u, h->omega, h->scales, h->Sn, h->Tn, h->A2, h->D));
   mark(h, "a5_angular_adjoint");
-  LAUNCH(h, k_net_bwd, h->n_cta_net, GNEP_WARPS * 32, smem_net_bwd(d), d, h->sm, h->theta, h->qscale, h->struct_s, h->e_s, h->scales, h->x, h->Ep, h->D, h->Acoef, h->Bcoef, h->gbar, h->partialB);
+  LAUNCH(h, k_net_tc<true>, h->n_cta_net, 256, smem_net_bwd(d), d, h->sm, h->theta, h->qscale, h->D, h->x, (float *)nullptr, h->Ep, (float *)nullptr,
+         h->struct_s, h->e_s, h->scales, h->pbuf, h->gbar);
   mark(h, "a6_network_backward");
-  LAUNCH(h, k_gemm_w0, h->n_chunks, threads_gemm_w0(d), smem_gemm_w0(d), d, h->sm, h->qscale, h->q, h->D, h->Acoef, h->Bcoef, h->partialW);
+  LAUNCH(h, k_gradw_tc, h->n_gw, GW_THREADS, smem_gradw(d), d, h->sm, h->theta, h->qscale, h->struct_s, h->e_s, h->scales, h->q, h->D, h->x, h->pbuf, h->partialW, h->partialB);
   mark(h, "a6_w0_gradient");
   LAUNCH(h, k_cgrad_radial, h->n_chunks, 256, smem_cgrad_rad(d), d, h->sm, h->gbar, h->Ep, h->M1, h->M2, h->partialCR);
   mark(h, "a7_radial_cgrad");
@@ -627,32 +628,43 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     CKT(cudaStreamSynchronize(st));
     tfree();
     // ---- work decomposition of the network / gradient kernels ----
-    const int per_cta = GNEP_WARPS * GNEP_TILE;
-    h->sm.cta_base[0] = 0; h->sm.chunk_base[0] = 0;
+    int tiles_total = 0;
+    for (int t = 0; t < T; ++t) tiles_total += cdiv(h->sm.start[t + 1] - h->sm.start[t], 128);
+    h->sm.cta_base[0] = 0; h->sm.chunk_base[0] = 0; h->sm.gw_base[0] = 0;
     for (int t = 0; t < GNEP_MAX_SPECIES_C; ++t) {
       int nt = t < T ? h->sm.start[t + 1] - h->sm.start[t] : 0;
-      h->sm.cta_base[t + 1] = h->sm.cta_base[t] + cdiv(nt, per_cta);
+      // k_net_tc: persistent CTAs (two 128-atom tiles in flight each), shared out by tile count
+      int tiles = cdiv(nt, 128);
+      int nc = tiles > 0 ? std::max(1, std::min(cdiv(tiles, 2), (int)((double)h->num_sms * tiles / std::max(tiles_total, 1) + 0.5))) : 0;
+      h->sm.cta_base[t + 1] = h->sm.cta_base[t] + nc;
+      // k_cgrad_radial: K-chunks
       int want = nt > 0 ? std::max(1, std::min(cdiv(nt, 256), (int)((2.0 * h->num_sms * nt) / std::max(N, 1) + 0.5))) : 0;
       int ca = want > 0 ? ((cdiv(nt, want) + 31) / 32) * 32 : 32;
       h->sm.chunk_atoms[t] = ca;
       h->sm.chunk_base[t + 1] = h->sm.chunk_base[t] + (nt > 0 ? cdiv(nt, ca) : 0);
+      // k_gradw_tc: one contiguous atom range per CTA
+      int gwant = nt > 0 ? std::max(1, std::min(cdiv(nt, 4 * GW_KS), (int)((double)h->num_sms * nt / std::max(N, 1) + 0.5))) : 0;
+      int ga = gwant > 0 ? pad_to(cdiv(nt, gwant), GW_KS) : GW_KS;
+      h->sm.gw_atoms[t] = ga;
+      h->sm.gw_base[t + 1] = h->sm.gw_base[t] + (nt > 0 ? cdiv(nt, ga) : 0);
     }
     h->n_cta_net = h->sm.cta_base[GNEP_MAX_SPECIES_C];
     h->n_chunks = h->sm.chunk_base[GNEP_MAX_SPECIES_C];
+    h->n_gw = h->sm.gw_base[GNEP_MAX_SPECIES_C];
     h->n_ca_blocks = std::max(1, std::min(cdiv(N, ANG_WARPS), 4 * h->num_sms));
-    for (int t = 0; t <= GNEP_MAX_SPECIES_C; ++t) { h->rm.chunk_base[t] = h->sm.chunk_base[t]; h->rm.cta_base[t] = h->sm.cta_base[t]; }
+    for (int t = 0; t <= GNEP_MAX_SPECIES_C; ++t) { h->rm.chunk_base[t] = h->sm.chunk_base[t]; h->rm.gw_base[t] = h->sm.gw_base[t]; }
     h->rm.n_warps_ca = N > 0 ? h->n_ca_blocks * ANG_WARPS : 0;
     // ---- per-atom state ----
     const size_t n = N;
     BA(h->q, n * d.Ndes); BA(h->Sn, n * d.NA * GNEP_NLM); BA(h->x, n * d.Nn); BA(h->Ei, n); BA(h->Ep, n * d.Ndes);
     BA(h->etil, n * T * d.KRp); BA(h->M1, n * T * d.KRp); BA(h->M2, n * T * d.KRp); BA(h->D, n * d.Ndes); BA(h->Tn, n * d.NA * GNEP_NLM); BA(h->A1, n * T * d.KAp * GNEP_NLM); BA(h->A2, n * T * d.KAp * GNEP_NLM);
-    BA(h->gbar, n * d.Ndes); BA(h->Acoef, n * d.Nn); BA(h->Bcoef, n * d.Nn); BA(h->Wat, n * 6);
+    BA(h->gbar, n * d.Ndes); BA(h->pbuf, n * d.Nn); BA(h->Wat, n * 6);
     BA(h->Fat, n); BA(h->fpair, nA); BA(h->u, n);
     BA(h->Es, S); BA(h->Ws, (size_t)S * 6); BA(h->parts, (size_t)S * 3); BA(h->e_s, S); BA(h->omega, (size_t)S * 6);
     BA(h->partialCR, (size_t)std::max(h->n_chunks, 1) * d.NR * T * d.KRp);
     BA(h->partialCA, (size_t)std::max(h->rm.n_warps_ca, 1) * T * T * d.NA * d.KAp);
-    BA(h->partialW, (size_t)std::max(h->n_chunks, 1) * d.Nn * d.Ndes);
-    BA(h->partialB, (size_t)std::max(h->n_cta_net, 1) * (2 * d.Nn + 1));
+    BA(h->partialW, (size_t)std::max(h->n_gw, 1) * d.Nn * d.Ndes);
+    BA(h->partialB, (size_t)std::max(h->n_gw, 1) * (2 * d.Nn + 1));
 #undef BA
 #undef CKT
     h->loaded = true;

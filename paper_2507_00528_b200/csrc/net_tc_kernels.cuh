@@ -1,0 +1,524 @@
+// net_tc_kernels.cuh -- the per-atom tanh network (rows a2, a6 of DESIGN.md) on the sm_100a tensor cores.
+//
+// All three network contractions are batched over atoms and run as tcgen05.mma (kind::tf32, fp32 accumulators in
+// TMEM) in 3xTF32 (tc05.cuh), which keeps fp32-grade accuracy (parity tolerances of BASELINE.json hold unchanged):
+//   k_net_tc<false>  a2: Z = G W0^T -> x = tanh(Z + b0), E_i, C = w1 (1 - x^2) -> E' = s o (C W0), etil
+//   k_net_tc<true>   a6: p = (s o D) W0^T -> Hc = w1 d2 p -> h = s o (Hc W0), gbar = e E' + h      (D1.6, C3.8)
+//   k_gradw_tc       a6: dL/dW0 = sum_atoms A (x) G + Bc (x) sD, dL/db0 = sum A, dL/dw1 = sum V, dL/db1 = sum e
+//                        with A = w1 (e d1 + d2 p), Bc = w1 d1, V = e x + d1 p                    (D1.7-D1.17)
+// Atoms are sorted by species; a CTA works on one species and keeps that species' W0 (split hi/lo, in both operand
+// arrangements) resident in shared memory while it loops over 128-atom tiles (k_net_tc: two warpgroups, one tile
+// each, so that one tile's epilogue overlaps the other's loads and MMAs).
+#pragma once
+#include "common.cuh"
+#include "tc05.cuh"
+
+struct SpeciesMap {
+  int start[GNEP_MAX_SPECIES_C + 1];      // sorted-atom range of each species
+  int cta_base[GNEP_MAX_SPECIES_C + 1];   // k_net_tc: first (persistent) CTA of each species
+  int chunk_base[GNEP_MAX_SPECIES_C + 1]; // k_cgrad_radial: first K-chunk of each species
+  int chunk_atoms[GNEP_MAX_SPECIES_C];    // atoms per K-chunk
+  int gw_base[GNEP_MAX_SPECIES_C + 1];    // k_gradw_tc: first CTA of each species
+  int gw_atoms[GNEP_MAX_SPECIES_C];       // atoms per k_gradw_tc CTA (multiple of GW_KS)
+};
+
+__device__ __forceinline__ int species_of_block(const int *base, int T, int b) {
+  int t = 0;
+  while (t + 1 < T && b >= base[t + 1]) ++t;
+  return t;
+}
+
+__host__ __device__ inline int pad_to(int x, int m) { return (x + m - 1) / m * m; }
+
+// padded problem sizes of the tensor-core kernels
+struct NetDims {
+  int NnP;   // neurons padded to 16: N of the first contraction, K of the second
+  int NdK;   // descriptors padded to 8: K of the first contraction
+  int NdN;   // descriptors padded to 16: N of the second contraction
+  int abuf;  // floats of one warpgroup's operand buffer
+};
+__host__ __device__ inline NetDims net_dims(const DevSpec &sp) {
+  NetDims d;
+  d.NnP = pad_to(sp.Nn, 16); d.NdK = pad_to(sp.Ndes, 8); d.NdN = pad_to(sp.Ndes, 16);
+  d.abuf = 128 * (2 * d.NdK > d.NnP ? 2 * d.NdK : d.NnP);
+  return d;
+}
+__host__ __device__ inline size_t net_tc_smem_bytes(const DevSpec &sp, bool bwd) {
+  NetDims d = net_dims(sp);
+  size_t fl = 2 * (size_t)d.NdK * d.NnP + 2 * (size_t)d.NnP * d.NdN + 2 * d.NnP + d.NdN + 2 * (size_t)d.abuf;
+  if (!bwd) fl += pad_to(sp.T * sp.NR * sp.KRp, 4);
+  return fl * sizeof(float) + 128;
+}
+
+__device__ __forceinline__ void wg_barrier(int wg) { asm volatile("bar.sync %0, 128;" ::"r"(1 + wg) : "memory"); }
+
+// 4 consecutive values of a row of length W starting at column c (zeros beyond W); vectorised when rows are 16-byte aligned
+__device__ __forceinline__ float4 load_row4(const float *__restrict__ row, int W, int c, bool vec, bool valid) {
+  float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (!valid) return v;
+  if (vec && c + 4 <= W) return *(const float4 *)(row + c);
+  if (c < W) v.x = row[c];
+  if (c + 1 < W) v.y = row[c + 1];
+  if (c + 2 < W) v.z = row[c + 2];
+  if (c + 3 < W) v.w = row[c + 3];
+  return v;
+}
+__device__ __forceinline__ void store_row4(float *__restrict__ row, int W, int c, bool vec, float4 v) {
+  if (vec && c + 4 <= W) { *(float4 *)(row + c) = v; return; }
+  if (c < W) row[c] = v.x;
+  if (c + 1 < W) row[c + 1] = v.y;
+  if (c + 2 < W) row[c + 2] = v.z;
+  if (c + 3 < W) row[c + 3] = v.w;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a2 / a6: two chained contractions per 128-atom tile.  Thread r of a warpgroup owns atom row r (TMEM lane r).
+//   step 1  rows of `in_rows` (q or D), scaled by s, split hi/lo -> K-major operand tile [NdK/4][128][4]
+//   step 2  one thread: D1[128][NnP] = rows . W0^T            (3 MMAs per K = 8)
+//   step 3  epilogue 1 per (atom, neuron); the second A operand goes back hi -> TMEM (in place of D1), lo -> smem
+//   step 4  one thread: D2[128][NdN] = A2 . W0                (A hi from TMEM, lo from smem)
+//   step 5  epilogue 2 per (atom, descriptor)
+// ------------------------------------------------------------------------------------------------
+template <bool BWD>
+__global__ void __launch_bounds__(256, 1)
+k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float *__restrict__ qscale,
+         const float *__restrict__ in_rows, float *__restrict__ xbuf, float *__restrict__ Ei, float *__restrict__ Ep,
+         float *__restrict__ etil, const int *__restrict__ struct_s, const float *__restrict__ e_s,
+         const float *__restrict__ scales, float *__restrict__ pbuf, float *__restrict__ gbar) {
+  using namespace tc05;
+  extern __shared__ __align__(128) float smem[];
+  const NetDims nd = net_dims(sp);
+  const int NnP = nd.NnP, NdK = nd.NdK, NdN = nd.NdN;
+  float *W1h = smem, *W1l = W1h + NdK * NnP;             // B of contraction 1: [NdK/4][NnP][4]   (n = mu, k = nu)
+  float *W2h = W1l + NdK * NnP, *W2l = W2h + NnP * NdN;  // B of contraction 2: [NnP/4][NdN][4]   (n = nu, k = mu)
+  float *b0s = W2l + NnP * NdN, *w1s = b0s + NnP, *qss = w1s + NnP;
+  float *cRs = qss + NdN;                                 // forward only: cR[t][J][n][k], k padded to KRp
+  float *abuf0 = cRs + (BWD ? 0 : pad_to(sp.T * sp.NR * sp.KRp, 4));
+  uint64_t *bars = (uint64_t *)(abuf0 + 2 * nd.abuf);    // [wg][2]
+  uint32_t *tmem_slot = (uint32_t *)(bars + 4);
+  const int tid = threadIdx.x, warp = tid >> 5, wg = tid >> 7, r = tid & 127;
+  const int t = species_of_block(sm.cta_base, sp.T, blockIdx.x);
+  const float *net = theta + sp.offNet + (size_t)t * sp.netSize;
+
+  if (warp == 0) tmem_alloc(tmem_slot, 512);
+  if (tid == 32) {
+    for (int i = 0; i < 4; ++i) mbar_init(bars + i, 1);
+    fence_mbar_init();
+  }
+  // ---- stage this species' network (zero padded) ----
+  for (int x = tid; x < 2 * NdK * NnP + 2 * NnP * NdN; x += 256) smem[x] = 0.f;
+  __syncthreads();
+  for (int x = tid; x < sp.Nn * sp.Ndes; x += 256) {
+    const int mu = x / sp.Ndes, nu = x - mu * sp.Ndes;
+    float hi, lo;
+    split_tf32(net[x], hi, lo);
+    const int o1 = (nu >> 2) * NnP * 4 + mu * 4 + (nu & 3), o2 = (mu >> 2) * NdN * 4 + nu * 4 + (mu & 3);
+    W1h[o1] = hi; W1l[o1] = lo; W2h[o2] = hi; W2l[o2] = lo;
+  }
+  for (int x = tid; x < NnP; x += 256) {
+    b0s[x] = x < sp.Nn ? net[sp.Nn * sp.Ndes + x] : 0.f;
+    w1s[x] = x < sp.Nn ? net[sp.Nn * sp.Ndes + sp.Nn + x] : 0.f;
+  }
+  for (int x = tid; x < NdN; x += 256) qss[x] = x < sp.Ndes ? qscale[x] : 0.f;
+  if (!BWD)
+    for (int x = tid; x < sp.T * sp.NR * sp.KRp; x += 256) {
+      const int row = x / sp.KRp, k = x - row * sp.KRp;
+      cRs[x] = k < sp.KR ? theta[((size_t)t * sp.T * sp.NR + row) * sp.KR + k] : 0.f;
+    }
+  fence_async_smem();
+  fence_before_sync();
+  __syncthreads();
+  fence_after_sync();
+  const uint32_t tbase = *tmem_slot + (uint32_t)(wg * 256);
+  // TMEM columns of this warpgroup: D1 main [0,NnP) (later the hi part of the second A operand), D1 corrections
+  // [NnP,2NnP); after step 3 the corrections are dead and D2 main / corrections take [NnP,NnP+NdN) / [NnP+NdN,NnP+2NdN).
+  // (the accumulator truncates at every accumulation: the small 3xTF32 correction products get their own accumulator)
+  const uint32_t tD1 = tbase, tD1c = tbase + NnP, tD2 = tbase + NnP, tD2c = tD2 + NdN;
+  const int lane0 = (warp & 3) * 32;
+  float *abuf = abuf0 + wg * nd.abuf;
+  const uint32_t a1h = smem_u32(abuf), a1l = a1h + (uint32_t)NdK * 128u * 4u;
+  const uint32_t w1h_a = smem_u32(W1h), w1l_a = smem_u32(W1l), w2h_a = smem_u32(W2h), w2l_a = smem_u32(W2l);
+  const uint32_t id1 = idesc_tf32(128, NnP, 0, 0), id2 = idesc_tf32(128, NdN, 0, 0);
+  uint64_t *bar1 = bars + 2 * wg, *bar2 = bar1 + 1;
+  const float b1v = net[sp.Nn * sp.Ndes + 2 * sp.Nn];
+  const bool vecD = (sp.Ndes & 3) == 0, vecN = (sp.Nn & 3) == 0;
+  const int TK = sp.T * sp.KRp;
+  const bool vecT = (TK & 3) == 0;
+
+  const int n_t = sm.start[t + 1] - sm.start[t];
+  const int tiles = (n_t + 127) >> 7;
+  const int ncta = sm.cta_base[t + 1] - sm.cta_base[t];
+  uint32_t parity = 0;
+  for (int tile = (blockIdx.x - sm.cta_base[t]) * 2 + wg; tile < tiles; tile += 2 * ncta, parity ^= 1u) {
+    const int a = sm.start[t] + tile * 128 + r;
+    const bool valid = a < sm.start[t + 1];
+    // ---- step 1 ----
+    {
+      const float *row = in_rows + (size_t)a * sp.Ndes;
+      for (int c = 0; c < NdK / 4; ++c) {
+        float4 v = load_row4(row, sp.Ndes, 4 * c, vecD, valid);
+        const float4 s4 = *(const float4 *)(qss + 4 * c);
+        v.x *= s4.x; v.y *= s4.y; v.z *= s4.z; v.w *= s4.w;
+        float4 hi, lo;
+        split4(v, hi, lo);
+        *(float4 *)(abuf + (c * 128 + r) * 4) = hi;
+        *(float4 *)(abuf + NdK * 128 + (c * 128 + r) * 4) = lo;
+      }
+    }
+    float ev = 0.f;
+    if (BWD) ev = valid ? scales[0] * e_s[struct_s[a]] : 0.f;
+    fence_async_smem();
+    fence_before_sync();
+    wg_barrier(wg);
+    // ---- step 2 ----
+    if (r == 0) {
+      fence_after_sync();
+      for (int s = 0; s < NdK / 8; ++s) {
+        const uint64_t dah = desc_kmajor(a1h, 128, s), dal = desc_kmajor(a1l, 128, s);
+        const uint64_t dbh = desc_kmajor(w1h_a, NnP, s), dbl = desc_kmajor(w1l_a, NnP, s);
+        mma_ss(tD1, dah, dbh, id1, s > 0);
+        mma_ss(tD1c, dah, dbl, id1, s > 0);
+        mma_ss(tD1c, dal, dbh, id1, 1);
+      }
+      mma_commit(bar1);
+    }
+    if (!mbar_wait(bar1, parity)) __trap();
+    fence_after_sync();
+    // ---- step 3 ----
+    float eacc = 0.f;
+    for (int m0 = 0; m0 < NnP; m0 += 16) {
+      float z[16], ch[16], cl[16];
+      tmem_ld16(tmem_addr(tD1, lane0, m0), z);
+      tmem_ld16(tmem_addr(tD1c, lane0, m0), ch);
+#pragma unroll
+      for (int i = 0; i < 16; ++i) z[i] += ch[i];
+      if (!BWD) {
+        float xs[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+          const float xv = tanhf(z[i] + b0s[m0 + i]);
+          const float w1 = w1s[m0 + i];            // zero for padded neurons
+          xs[i] = xv;
+          eacc += w1 * xv;
+          split_tf32(w1 * (1.f - xv * xv), ch[i], cl[i]);
+        }
+        if (valid) {
+          float *xr = xbuf + (size_t)a * sp.Nn;
+#pragma unroll
+          for (int v = 0; v < 4; ++v) store_row4(xr, sp.Nn, m0 + 4 * v, vecN, make_float4(xs[4 * v], xs[4 * v + 1], xs[4 * v + 2], xs[4 * v + 3]));
+        }
+      } else {
+        const float *xr = xbuf + (size_t)a * sp.Nn;
+        float *pr = pbuf + (size_t)a * sp.Nn;
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+          const float4 x4 = load_row4(xr, sp.Nn, m0 + 4 * v, vecN, valid);
+          const float xv[4] = {x4.x, x4.y, x4.z, x4.w};
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const float d1 = 1.f - xv[i] * xv[i], d2 = -2.f * xv[i] * d1;
+            split_tf32(w1s[m0 + 4 * v + i] * d2 * z[4 * v + i], ch[4 * v + i], cl[4 * v + i]);
+          }
+          if (valid) store_row4(pr, sp.Nn, m0 + 4 * v, vecN, make_float4(z[4 * v], z[4 * v + 1], z[4 * v + 2], z[4 * v + 3]));
+        }
+      }
+      {
+        float h8[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) h8[i] = ch[i];
+        tmem_st8(tmem_addr(tD1, lane0, m0), h8);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) h8[i] = ch[8 + i];
+        tmem_st8(tmem_addr(tD1, lane0, m0 + 8), h8);
+      }
+#pragma unroll
+      for (int v = 0; v < 4; ++v)
+        *(float4 *)(abuf + (((m0 >> 2) + v) * 128 + r) * 4) = make_float4(cl[4 * v], cl[4 * v + 1], cl[4 * v + 2], cl[4 * v + 3]);
+    }
+    if (!BWD && valid) Ei[a] = eacc + b1v;
+    tmem_st_wait();
+    fence_async_smem();
+    fence_before_sync();
+    wg_barrier(wg);
+    // ---- step 4 ----
+    if (r == 0) {
+      fence_after_sync();
+      for (int s = 0; s < NnP / 8; ++s) {
+        const uint64_t dbh = desc_kmajor(w2h_a, NdN, s), dbl = desc_kmajor(w2l_a, NdN, s);
+        const uint32_t ta = tmem_addr(tD1, 0, 8 * s);
+        mma_ts(tD2, ta, dbh, id2, s > 0);
+        mma_ts(tD2c, ta, dbl, id2, s > 0);
+        mma_ss(tD2c, desc_kmajor(a1h, 128, s), dbh, id2, 1);
+      }
+      mma_commit(bar2);
+    }
+    if (!mbar_wait(bar2, parity)) __trap();
+    fence_after_sync();
+    // ---- step 5 ----
+    float epr[16];
+    for (int n0 = 0; n0 < NdN; n0 += 16) {
+      float v[16], vc[16];
+      tmem_ld16(tmem_addr(tD2, lane0, n0), v);
+      tmem_ld16(tmem_addr(tD2c, lane0, n0), vc);
+#pragma unroll
+      for (int i = 0; i < 16; ++i) v[i] = (v[i] + vc[i]) * qss[n0 + i];
+      if (!BWD) {
+        if (n0 == 0) {
+#pragma unroll
+          for (int i = 0; i < 16; ++i) epr[i] = v[i];
+        }
+        if (valid) {
+          float *er = Ep + (size_t)a * sp.Ndes;
+#pragma unroll
+          for (int q4 = 0; q4 < 4; ++q4) store_row4(er, sp.Ndes, n0 + 4 * q4, vecD, make_float4(v[4 * q4], v[4 * q4 + 1], v[4 * q4 + 2], v[4 * q4 + 3]));
+        }
+      } else {
+        const float *er = Ep + (size_t)a * sp.Ndes;
+        float *gr = gbar + (size_t)a * sp.Ndes;
+#pragma unroll
+        for (int q4 = 0; q4 < 4; ++q4) {
+          const float4 e4 = load_row4(er, sp.Ndes, n0 + 4 * q4, vecD, valid);
+          if (valid)
+            store_row4(gr, sp.Ndes, n0 + 4 * q4, vecD,
+                       make_float4(ev * e4.x + v[4 * q4], ev * e4.y + v[4 * q4 + 1], ev * e4.z + v[4 * q4 + 2], ev * e4.w + v[4 * q4 + 3]));
+        }
+      }
+    }
+    if (!BWD) {   // etil[J][k] = sum_n E'_n cR[t][J][n][k]  (input of the radial force pass)
+      float *et = etil + (size_t)a * TK;
+      for (int o = 0; o < TK; o += 4) {
+        float acc4[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const int oo = o + i;
+          if (oo < TK) {
+            const int J = oo / sp.KRp, k = oo - J * sp.KRp;
+            const float *c = cRs + (J * sp.NR) * sp.KRp + k;
+            float s = 0.f;
+#pragma unroll
+            for (int n = 0; n < 16; ++n)
+              if (n < sp.NR) s += epr[n] * c[n * sp.KRp];
+            acc4[i] = s;
+          }
+        }
+        if (valid) store_row4(et, TK, o, vecT, make_float4(acc4[0], acc4[1], acc4[2], acc4[3]));
+      }
+    }
+    fence_before_sync();   // the next tile's MMAs overwrite D1/D2 and the operand buffer after the barrier of step 1
+  }
+  fence_before_sync();
+  __syncthreads();
+  if (warp == 0) tmem_free(*tmem_slot, 512);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a6: the parameter gradients of the network as ONE contraction over atoms (K = atoms, D1.7-D1.17):
+//   D3[mu][nu]   = sum_a A[a][mu] G[a][nu] + Bc[a][mu] sD[a][nu]      (dL/dW0; column nu = Ndes carries G = 1 -> dL/db0)
+//   D4[mu][0]    = sum_a V[a][mu]                                       (dL/dw1)
+// A, Bc, V are formed on the fly from x, p and the energy seed e.  Each CTA owns a contiguous atom range of one
+// species; operands are staged K-major ([atoms/4][row][4]) in a two-stage ring of GW_KS atoms.
+// The tensor-core accumulator truncates at every accumulation, so the TMEM sums are kept short: a group of
+// GW_FLUSH stages accumulates into one of two TMEM sets (hi*hi products and the small 3xTF32 corrections in separate
+// accumulators) and is then added, with fp32 rounding, to register accumulators held by threads 0..127 (row mu).
+// One partial per CTA is written at the end (reduced in fixed order, fp64, by k_grad_reduce).
+// ------------------------------------------------------------------------------------------------
+#define GW_KS 16        // atoms per stage (2 MMA K-steps)
+#define GW_FLUSH 4      // stages per TMEM accumulation group
+#define GW_THREADS 256
+#define GW_MAXC 7       // 16-column chunks of the widest accumulator (NB <= 112)
+
+__host__ __device__ inline int gw_ncols(const DevSpec &sp) { return pad_to(sp.Ndes + 1, 16); }
+__host__ __device__ inline size_t gradw_smem_bytes(const DevSpec &sp) {
+  const int NB = gw_ncols(sp);
+  size_t stage = 6 * (size_t)(GW_KS / 4) * 128 * 4 + 4 * (size_t)(GW_KS / 4) * NB * 4;
+  return (2 * stage + (GW_KS / 4) * 16 * 4 + GW_THREADS) * sizeof(float) + 128;
+}
+
+__global__ void __launch_bounds__(GW_THREADS, 1)
+k_gradw_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float *__restrict__ qscale,
+           const int *__restrict__ struct_s, const float *__restrict__ e_s, const float *__restrict__ scales,
+           const float *__restrict__ q, const float *__restrict__ D, const float *__restrict__ x,
+           const float *__restrict__ p, float *__restrict__ partialW, float *__restrict__ partialB) {
+  using namespace tc05;
+  extern __shared__ __align__(128) float smem[];
+  constexpr int G4 = GW_KS / 4;                       // atom groups (16-byte K-chunks) per stage
+  const int NB = gw_ncols(sp);
+  const int tileA = G4 * 128 * 4, tileB = G4 * NB * 4; // floats per operand tile
+  const int stage_fl = 6 * tileA + 4 * tileB;
+  // stage layout: Ah Al Bh Bl Vh Vl (rows = mu, 128) | Gh Gl Dh Dl (rows = nu, NB)
+  float *ones = smem + 2 * stage_fl;                  // [G4][16][4]
+  float *esh = ones + G4 * 16 * 4;                    // [GW_THREADS]
+  uint64_t *bars = (uint64_t *)(esh + GW_THREADS);    // [0,1] stage free, [2,3] accumulation group done
+  uint32_t *tmem_slot = (uint32_t *)(bars + 4);
+  const int tid = threadIdx.x, warp = tid >> 5;
+  const int t = species_of_block(sm.gw_base, sp.T, blockIdx.x);
+  const float *net = theta + sp.offNet + (size_t)t * sp.netSize;
+  const float *w1g = net + sp.Nn * sp.Ndes + sp.Nn;
+  const int c0 = sm.start[t] + (blockIdx.x - sm.gw_base[t]) * sm.gw_atoms[t];
+  const int c1 = min(c0 + sm.gw_atoms[t], sm.start[t + 1]);
+  if (warp == 0) tmem_alloc(tmem_slot, 512);
+  if (tid == 32) {
+    for (int i = 0; i < 4; ++i) mbar_init(bars + i, 1);
+    fence_mbar_init();
+  }
+  for (int i = tid; i < 2 * stage_fl; i += GW_THREADS) smem[i] = 0.f;
+  for (int i = tid; i < G4 * 16 * 4; i += GW_THREADS) ones[i] = 1.f;
+  __syncthreads();
+  // the constant "G = 1" row (nu = Ndes) of both stages' Gh tiles
+  if (tid < 2 * G4 * 4) {
+    const int st = tid / (G4 * 4), rem = tid - st * G4 * 4, g = rem >> 2, i = rem & 3;
+    smem[st * stage_fl + 6 * tileA + (g * NB + sp.Ndes) * 4 + i] = 1.f;
+  }
+  fence_async_smem();
+  fence_before_sync();
+  __syncthreads();
+  fence_after_sync();
+  // TMEM set s (two of them): [0,NB) D3 main, [NB,2NB) D3 corrections, [2NB,2NB+16) D4 main, [2NB+16,2NB+32) D4 corr.
+  const int setc = 2 * NB + 32;
+  const uint32_t tb = *tmem_slot;
+  const uint32_t idW = idesc_tf32(128, NB, 0, 0), id1 = idesc_tf32(128, 16, 0, 0);
+  const uint32_t ones_a = smem_u32(ones);
+  const float se = scales[0];
+  const int nA = G4 * sp.Nn, nB = G4 * sp.Ndes;        // work items per stage
+  const int lane0 = (warp & 3) * 32;
+  float esum = 0.f;
+  float racc[GW_MAXC][16], rv = 0.f;                   // threads 0..127: row mu of D3, and D4[mu][0]
+#pragma unroll
+  for (int c = 0; c < GW_MAXC; ++c)
+#pragma unroll
+    for (int i = 0; i < 16; ++i) racc[c][i] = 0.f;
+
+  auto flush = [&](int g) {   // add accumulation group g (complete after its last commit) to the registers
+    if (tid < 128) {
+      if (!mbar_wait(bars + 2 + (g & 1), (uint32_t)((g >> 1) & 1))) __trap();
+      fence_after_sync();
+      const uint32_t ts = tb + (uint32_t)((g & 1) * setc);
+#pragma unroll
+      for (int c = 0; c < GW_MAXC; ++c)
+        if (c * 16 < NB) {
+          float m[16], k[16];
+          tmem_ld16(tmem_addr(ts, lane0, c * 16), m);
+          tmem_ld16(tmem_addr(ts, lane0, NB + c * 16), k);
+#pragma unroll
+          for (int i = 0; i < 16; ++i) racc[c][i] += m[i] + k[i];
+        }
+      float m8[8], k8[8];
+      tmem_ld8(tmem_addr(ts, lane0, 2 * NB), m8);
+      tmem_ld8(tmem_addr(ts, lane0, 2 * NB + 16), k8);
+      rv += m8[0] + k8[0];
+      fence_before_sync();
+    }
+  };
+
+  const int nst = (c1 - c0 + GW_KS - 1) / GW_KS;
+  const int ngroups = (nst + GW_FLUSH - 1) / GW_FLUSH;
+  for (int it = 0; it < nst; ++it) {
+    const int st = it & 1, g = it / GW_FLUSH, gi = it - g * GW_FLUSH;
+    float *sb = smem + st * stage_fl;
+    if (gi == 0 && g >= 1) flush(g - 1);
+    if (it >= 2 && !mbar_wait(bars + st, (uint32_t)(((it >> 1) - 1) & 1))) __trap();
+    const int a0 = c0 + it * GW_KS;
+    for (int w = tid; w < nA + nB; w += GW_THREADS) {
+      if (w < nA) {
+        const int ag = w / sp.Nn, mu = w - ag * sp.Nn;
+        const float w1 = w1g[mu];
+        float Av[4], Bv[4], Vv[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const int a = a0 + 4 * ag + i;
+          Av[i] = 0.f; Bv[i] = 0.f; Vv[i] = 0.f;
+          if (a < c1) {
+            const float ev = se * e_s[struct_s[a]];
+            const float xv = x[(size_t)a * sp.Nn + mu], pv = p[(size_t)a * sp.Nn + mu];
+            const float d1 = 1.f - xv * xv, d2 = -2.f * xv * d1;
+            Av[i] = w1 * (ev * d1 + d2 * pv);
+            Bv[i] = w1 * d1;
+            Vv[i] = ev * xv + d1 * pv;
+            if (mu == 0) esum += ev;
+          }
+        }
+        float4 hi, lo;
+        const int o = (ag * 128 + mu) * 4;
+        split4(make_float4(Av[0], Av[1], Av[2], Av[3]), hi, lo);
+        *(float4 *)(sb + o) = hi; *(float4 *)(sb + tileA + o) = lo;
+        split4(make_float4(Bv[0], Bv[1], Bv[2], Bv[3]), hi, lo);
+        *(float4 *)(sb + 2 * tileA + o) = hi; *(float4 *)(sb + 3 * tileA + o) = lo;
+        split4(make_float4(Vv[0], Vv[1], Vv[2], Vv[3]), hi, lo);
+        *(float4 *)(sb + 4 * tileA + o) = hi; *(float4 *)(sb + 5 * tileA + o) = lo;
+      } else {
+        const int wb = w - nA;
+        const int ag = wb / sp.Ndes, nu = wb - ag * sp.Ndes;
+        const float s = qscale[nu];
+        float Gv[4], Dv[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const int a = a0 + 4 * ag + i;
+          const bool ok = a < c1;
+          Gv[i] = ok ? s * q[(size_t)a * sp.Ndes + nu] : 0.f;
+          Dv[i] = ok ? s * D[(size_t)a * sp.Ndes + nu] : 0.f;
+        }
+        float4 hi, lo;
+        float *gb = sb + 6 * tileA;
+        const int o = (ag * NB + nu) * 4;
+        split4(make_float4(Gv[0], Gv[1], Gv[2], Gv[3]), hi, lo);
+        *(float4 *)(gb + o) = hi; *(float4 *)(gb + tileB + o) = lo;
+        split4(make_float4(Dv[0], Dv[1], Dv[2], Dv[3]), hi, lo);
+        *(float4 *)(gb + 2 * tileB + o) = hi; *(float4 *)(gb + 3 * tileB + o) = lo;
+      }
+    }
+    fence_async_smem();
+    fence_before_sync();
+    __syncthreads();
+    if (tid == 0) {
+      fence_after_sync();
+      const uint32_t ts = tb + (uint32_t)((g & 1) * setc);
+      const uint32_t tM = ts, tC = ts + NB, tV = ts + 2 * NB, tVc = tV + 16;
+      const uint32_t sa = smem_u32(sb), ga = sa + 6u * (uint32_t)tileA * 4u;
+      for (int s = 0; s < GW_KS / 8; ++s) {
+        const uint64_t Ah = desc_kmajor(sa, 128, s), Al = desc_kmajor(sa + tileA * 4, 128, s);
+        const uint64_t Bh = desc_kmajor(sa + 2 * tileA * 4, 128, s), Bl = desc_kmajor(sa + 3 * tileA * 4, 128, s);
+        const uint64_t Vh = desc_kmajor(sa + 4 * tileA * 4, 128, s), Vl = desc_kmajor(sa + 5 * tileA * 4, 128, s);
+        const uint64_t Gh = desc_kmajor(ga, NB, s), Gl = desc_kmajor(ga + tileB * 4, NB, s);
+        const uint64_t Dh = desc_kmajor(ga + 2 * tileB * 4, NB, s), Dl = desc_kmajor(ga + 3 * tileB * 4, NB, s);
+        const uint64_t On = desc_kmajor(ones_a, 16, s);
+        const uint32_t acc = (gi > 0 || s > 0) ? 1u : 0u;   // the first K-step of a group overwrites the set
+        mma_ss(tM, Ah, Gh, idW, acc);
+        mma_ss(tM, Bh, Dh, idW, 1);
+        mma_ss(tC, Ah, Gl, idW, acc);
+        mma_ss(tC, Al, Gh, idW, 1);
+        mma_ss(tC, Bh, Dl, idW, 1);
+        mma_ss(tC, Bl, Dh, idW, 1);
+        mma_ss(tV, Vh, On, id1, acc);
+        mma_ss(tVc, Vl, On, id1, acc);
+      }
+      mma_commit(bars + st);
+      if (gi == GW_FLUSH - 1 || it == nst - 1) mma_commit(bars + 2 + (g & 1));
+    }
+  }
+  if (ngroups > 0) flush(ngroups - 1);
+  esh[tid] = esum;
+  __syncthreads();
+  const int nb = 2 * sp.Nn + 1;
+  float *outW = partialW + (size_t)blockIdx.x * sp.Nn * sp.Ndes;
+  float *outB = partialB + (size_t)blockIdx.x * nb;
+  if (tid < sp.Nn) {
+    const int mu = tid;
+#pragma unroll
+    for (int c = 0; c < GW_MAXC; ++c)
+#pragma unroll
+      for (int i = 0; i < 16; ++i) {
+        const int nu = c * 16 + i;
+        if (nu < sp.Ndes) outW[mu * sp.Ndes + nu] = racc[c][i];
+        else if (nu == sp.Ndes) outB[mu] = racc[c][i];
+      }
+    outB[sp.Nn + mu] = rv;
+  }
+  if (tid == 0) {
+    float s = 0.f;
+    for (int i = 0; i < GW_THREADS; ++i) s += esh[i];
+    outB[2 * sp.Nn] = s;
+  }
+  fence_before_sync();
+  __syncthreads();
+  if (warp == 0) tmem_free(tb, 512);
+}

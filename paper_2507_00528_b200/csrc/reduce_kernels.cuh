@@ -114,7 +114,7 @@ k_loss_final(LossCfg lc, const double *__restrict__ parts, const float *__restri
 // a8: grad[p] = sum over the partial buffers that cover p (fixed order, fp64) + 2 lam_2 s2 theta_p / P.
 struct ReduceMap {
   int chunk_base[GNEP_MAX_SPECIES_C + 1];   // K-chunks (W0, cR partials) per species
-  int cta_base[GNEP_MAX_SPECIES_C + 1];     // network CTAs (b0, w1, b1 partials) per species
+  int gw_base[GNEP_MAX_SPECIES_C + 1];      // k_gradw_tc CTAs (W0, b0, w1, b1 partials) per species
   int n_warps_ca;                           // partial rows of the angular c-gradient
 };
 // Block = 8 consecutive parameters x 32 row lanes: every lane sums rows lane, lane+32, ... of its parameter's partial
@@ -146,8 +146,9 @@ k_grad_reduce(DevSpec sp, ReduceMap rm, float l2_share, const float *__restrict_
       int x = p - sp.offNet;
       int t = x / sp.netSize, y = x - t * sp.netSize;
       int nW = sp.Nn * sp.Ndes;
-      if (y < nW) { stride = nW; base = partialW + y; r0 = rm.chunk_base[t]; r1 = rm.chunk_base[t + 1]; }
-      else { stride = 2 * sp.Nn + 1; base = partialB + (y - nW); r0 = rm.cta_base[t]; r1 = rm.cta_base[t + 1]; }
+      r0 = rm.gw_base[t]; r1 = rm.gw_base[t + 1];
+      if (y < nW) { stride = nW; base = partialW + y; }
+      else { stride = 2 * sp.Nn + 1; base = partialB + (y - nW); }
     }
     for (int r = r0 + ty; r < r1; r += 32) s += (double)base[(size_t)r * stride];
   }
