@@ -57,7 +57,7 @@ struct gnep_handle {
   int n_cta_net = 0, n_chunks = 0, n_ca_blocks = 0, n_gw = 0;
   // per-atom state
   float *q = nullptr, *Sn = nullptr, *x = nullptr, *Ei = nullptr, *Ep = nullptr, *etil = nullptr, *M1 = nullptr,
-        *M2 = nullptr, *D = nullptr, *Tn = nullptr, *A1 = nullptr, *A2 = nullptr, *gbar = nullptr, *pbuf = nullptr, *Wat = nullptr;
+        *M2 = nullptr, *D = nullptr, *Tn = nullptr, *A1 = nullptr, *A2 = nullptr, *gbar = nullptr, *pbuf = nullptr, *eat = nullptr, *Wat = nullptr;
   float4 *Fat = nullptr, *fpair = nullptr, *u = nullptr;
   double *Es = nullptr, *Ws = nullptr, *parts = nullptr;
   float *e_s = nullptr, *omega = nullptr;
@@ -161,6 +161,7 @@ int configure_kernels(gnep_handle *h) {
   }
   RET_IF(set_smem(h, k_net_tc<false>, smem_net_fwd(d)));
   RET_IF(set_smem(h, k_net_tc<true>, smem_net_bwd(d)));
+  if (gradw_stages(d) < 2) return fail(h, GNEP_EINVAL, "model too large for shared memory staging (n_descriptors)");
   RET_IF(set_smem(h, k_gradw_tc, smem_gradw(d)));
   RET_IF(set_smem(h, k_cgrad_radial, smem_cgrad_rad(d)));
   return GNEP_OK;
@@ -248,10 +249,10 @@ int enqueue_backward(gnep_handle *h) {
   mark(h, "a5_radial_adjoint");
   DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_adj<KT>, cdiv(h->N, ANG_WARPS * ANG_TA), ANG_WARPS * 32, smem_ang_adj(d), d, h->N, h->type_s, h->struct_s, h->segA, h->atomA, h->pairA, h->theta, h->u, h->omega, h->scales, h->Sn, h->Tn, h->A2, h->D));
   mark(h, "a5_angular_adjoint");
-  LAUNCH(h, k_net_tc<true>, h->n_cta_net, 256, smem_net_bwd(d), d, h->sm, h->theta, h->qscale, h->D, h->x, (float *)nullptr, h->Ep, (float *)nullptr,
+  LAUNCH(h, k_net_tc<true>, h->n_cta_net, 256, smem_net_bwd(d), d, h->sm, h->theta, h->qscale, h->D, h->x, h->eat, h->Ep, (float *)nullptr,
          h->struct_s, h->e_s, h->scales, h->pbuf, h->gbar);
   mark(h, "a6_network_backward");
-  LAUNCH(h, k_gradw_tc, h->n_gw, GW_THREADS, smem_gradw(d), d, h->sm, h->theta, h->qscale, h->struct_s, h->e_s, h->scales, h->q, h->D, h->x, h->pbuf, h->partialW, h->partialB);
+  LAUNCH(h, k_gradw_tc, h->n_gw, GW_THREADS, smem_gradw(d), d, h->sm, gradw_stages(d), h->theta, h->qscale, h->eat, h->q, h->D, h->x, h->pbuf, h->partialW, h->partialB);
   mark(h, "a6_w0_gradient");
   LAUNCH(h, k_cgrad_radial, h->n_chunks, 256, smem_cgrad_rad(d), d, h->sm, h->gbar, h->Ep, h->M1, h->M2, h->partialCR);
   mark(h, "a7_radial_cgrad");
@@ -658,7 +659,7 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     const size_t n = N;
     BA(h->q, n * d.Ndes); BA(h->Sn, n * d.NA * GNEP_NLM); BA(h->x, n * d.Nn); BA(h->Ei, n); BA(h->Ep, n * d.Ndes);
     BA(h->etil, n * T * d.KRp); BA(h->M1, n * T * d.KRp); BA(h->M2, n * T * d.KRp); BA(h->D, n * d.Ndes); BA(h->Tn, n * d.NA * GNEP_NLM); BA(h->A1, n * T * d.KAp * GNEP_NLM); BA(h->A2, n * T * d.KAp * GNEP_NLM);
-    BA(h->gbar, n * d.Ndes); BA(h->pbuf, n * d.Nn); BA(h->Wat, n * 6);
+    BA(h->gbar, n * d.Ndes); BA(h->pbuf, n * d.Nn); BA(h->eat, n); BA(h->Wat, n * 6);
     BA(h->Fat, n); BA(h->fpair, nA); BA(h->u, n);
     BA(h->Es, S); BA(h->Ws, (size_t)S * 6); BA(h->parts, (size_t)S * 3); BA(h->e_s, S); BA(h->omega, (size_t)S * 6);
     BA(h->partialCR, (size_t)std::max(h->n_chunks, 1) * d.NR * T * d.KRp);

@@ -50,6 +50,13 @@ __host__ __device__ inline size_t net_tc_smem_bytes(const DevSpec &sp, bool bwd)
   return fl * sizeof(float) + 128;
 }
 
+// tanh(z) = 1 - 2 / (exp(2 z) + 1) with the hardware exp2 and reciprocal: absolute error <= ~1e-7 over the whole range
+// (the argument rounding of exp2 only matters where tanh is already saturated), about 6 instructions.
+__device__ __forceinline__ float tanh_fast(float z) {
+  const float e = exp2f(fminf(z * 2.885390081777927f, 126.f));   // exp(2 z), clamped below overflow
+  return 1.f - __fdividef(2.f, e + 1.f);
+}
+
 __device__ __forceinline__ void wg_barrier(int wg) { asm volatile("bar.sync %0, 128;" ::"r"(1 + wg) : "memory"); }
 
 // 4 consecutive values of a row of length W starting at column c (zeros beyond W); vectorised when rows are 16-byte aligned
@@ -155,18 +162,30 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
     // ---- step 1 ----
     {
       const float *row = in_rows + (size_t)a * sp.Ndes;
-      for (int c = 0; c < NdK / 4; ++c) {
-        float4 v = load_row4(row, sp.Ndes, 4 * c, vecD, valid);
-        const float4 s4 = *(const float4 *)(qss + 4 * c);
-        v.x *= s4.x; v.y *= s4.y; v.z *= s4.z; v.w *= s4.w;
-        float4 hi, lo;
-        split4(v, hi, lo);
-        *(float4 *)(abuf + (c * 128 + r) * 4) = hi;
-        *(float4 *)(abuf + NdK * 128 + (c * 128 + r) * 4) = lo;
+      for (int cb = 0; cb < NdK / 4; cb += 8) {     // 8 row chunks in flight per thread
+        float4 v8[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) v8[j] = load_row4(row, sp.Ndes, 4 * (cb + j), vecD, valid && cb + j < NdK / 4);
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const int c = cb + j;
+          if (c < NdK / 4) {
+            float4 v = v8[j];
+            const float4 s4 = *(const float4 *)(qss + 4 * c);
+            v.x *= s4.x; v.y *= s4.y; v.z *= s4.z; v.w *= s4.w;
+            float4 hi, lo;
+            split4(v, hi, lo);
+            *(float4 *)(abuf + (c * 128 + r) * 4) = hi;
+            *(float4 *)(abuf + NdK * 128 + (c * 128 + r) * 4) = lo;
+          }
+        }
       }
     }
     float ev = 0.f;
-    if (BWD) ev = valid ? scales[0] * e_s[struct_s[a]] : 0.f;
+    if (BWD) {
+      ev = valid ? scales[0] * e_s[struct_s[a]] : 0.f;
+      if (valid) Ei[a] = ev;   // backward: Ei is the per-atom energy-seed buffer read by k_gradw_tc
+    }
     fence_async_smem();
     fence_before_sync();
     wg_barrier(wg);
@@ -182,6 +201,11 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
       }
       mma_commit(bar1);
     }
+    float4 xnext[4];   // backward: the x row is fetched one 16-neuron chunk ahead of its use
+    if (BWD) {
+#pragma unroll
+      for (int v = 0; v < 4; ++v) xnext[v] = load_row4(xbuf + (size_t)a * sp.Nn, sp.Nn, 4 * v, vecN, valid);
+    }
     if (!mbar_wait(bar1, parity)) __trap();
     fence_after_sync();
     // ---- step 3 ----
@@ -196,7 +220,7 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
         float xs[16];
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
-          const float xv = tanhf(z[i] + b0s[m0 + i]);
+          const float xv = tanh_fast(z[i] + b0s[m0 + i]);
           const float w1 = w1s[m0 + i];            // zero for padded neurons
           xs[i] = xv;
           eacc += w1 * xv;
@@ -210,9 +234,15 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
       } else {
         const float *xr = xbuf + (size_t)a * sp.Nn;
         float *pr = pbuf + (size_t)a * sp.Nn;
+        float4 xcur[4];
 #pragma unroll
         for (int v = 0; v < 4; ++v) {
-          const float4 x4 = load_row4(xr, sp.Nn, m0 + 4 * v, vecN, valid);
+          xcur[v] = xnext[v];
+          xnext[v] = load_row4(xr, sp.Nn, m0 + 16 + 4 * v, vecN, valid && m0 + 16 < NnP);
+        }
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+          const float4 x4 = xcur[v];
           const float xv[4] = {x4.x, x4.y, x4.z, x4.w};
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
@@ -252,6 +282,11 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
       }
       mma_commit(bar2);
     }
+    float4 enext[4];   // backward: E' row, one 16-descriptor chunk ahead
+    if (BWD) {
+#pragma unroll
+      for (int v = 0; v < 4; ++v) enext[v] = load_row4(Ep + (size_t)a * sp.Ndes, sp.Ndes, 4 * v, vecD, valid);
+    }
     if (!mbar_wait(bar2, parity)) __trap();
     fence_after_sync();
     // ---- step 5 ----
@@ -275,9 +310,15 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
       } else {
         const float *er = Ep + (size_t)a * sp.Ndes;
         float *gr = gbar + (size_t)a * sp.Ndes;
+        float4 ecur[4];
 #pragma unroll
         for (int q4 = 0; q4 < 4; ++q4) {
-          const float4 e4 = load_row4(er, sp.Ndes, n0 + 4 * q4, vecD, valid);
+          ecur[q4] = enext[q4];
+          enext[q4] = load_row4(er, sp.Ndes, n0 + 16 + 4 * q4, vecD, valid && n0 + 16 < NdN);
+        }
+#pragma unroll
+        for (int q4 = 0; q4 < 4; ++q4) {
+          const float4 e4 = ecur[q4];
           if (valid)
             store_row4(gr, sp.Ndes, n0 + 4 * q4, vecD,
                        make_float4(ev * e4.x + v[4 * q4], ev * e4.y + v[4 * q4 + 1], ev * e4.z + v[4 * q4 + 2], ev * e4.w + v[4 * q4 + 3]));
@@ -315,8 +356,11 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
 // a6: the parameter gradients of the network as ONE contraction over atoms (K = atoms, D1.7-D1.17):
 //   D3[mu][nu]   = sum_a A[a][mu] G[a][nu] + Bc[a][mu] sD[a][nu]      (dL/dW0; column nu = Ndes carries G = 1 -> dL/db0)
 //   D4[mu][0]    = sum_a V[a][mu]                                       (dL/dw1)
-// A, Bc, V are formed on the fly from x, p and the energy seed e.  Each CTA owns a contiguous atom range of one
-// species; operands are staged K-major ([atoms/4][row][4]) in a two-stage ring of GW_KS atoms.
+// A, Bc, V are formed on the fly from x, p and the per-atom energy seed e.  Each CTA owns a contiguous atom range of
+// one species.  Warps 0..7 are producers: they stage the operands K-major ([atoms/4][row][4], hi/lo split) into a ring
+// of `nstage` stages of GW_KS atoms and arrive on the stage's "full" mbarrier; warp 8 issues the MMAs of a full stage
+// and commits to its "empty" mbarrier.  No CTA-wide barrier sits in the loop, so the global-load latency of one stage
+// overlaps the staging arithmetic and the MMAs of the others.
 // The tensor-core accumulator truncates at every accumulation, so the TMEM sums are kept short: a group of
 // GW_FLUSH stages accumulates into one of two TMEM sets (hi*hi products and the small 3xTF32 corrections in separate
 // accumulators) and is then added, with fp32 rounding, to register accumulators held by threads 0..127 (row mu).
@@ -324,21 +368,32 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
 // ------------------------------------------------------------------------------------------------
 #define GW_KS 16        // atoms per stage (2 MMA K-steps)
 #define GW_FLUSH 4      // stages per TMEM accumulation group
-#define GW_THREADS 256
+#define GW_PROD 256     // producer threads
+#define GW_THREADS (GW_PROD + 32)
 #define GW_MAXC 7       // 16-column chunks of the widest accumulator (NB <= 112)
 
 __host__ __device__ inline int gw_ncols(const DevSpec &sp) { return pad_to(sp.Ndes + 1, 16); }
+__host__ __device__ inline size_t gradw_stage_floats(const DevSpec &sp) {
+  return 6 * (size_t)(GW_KS / 4) * 128 * 4 + 4 * (size_t)(GW_KS / 4) * gw_ncols(sp) * 4;
+}
+__host__ __device__ inline int gradw_stages(const DevSpec &sp) {
+  const size_t fixed = ((GW_KS / 4) * 16 * 4 + GW_PROD) * sizeof(float) + 256;
+  int n = (int)((227 * 1024 - fixed) / (gradw_stage_floats(sp) * sizeof(float)));
+  return n > 4 ? 4 : n;
+}
 __host__ __device__ inline size_t gradw_smem_bytes(const DevSpec &sp) {
-  const int NB = gw_ncols(sp);
-  size_t stage = 6 * (size_t)(GW_KS / 4) * 128 * 4 + 4 * (size_t)(GW_KS / 4) * NB * 4;
-  return (2 * stage + (GW_KS / 4) * 16 * 4 + GW_THREADS) * sizeof(float) + 128;
+  return (gradw_stages(sp) * gradw_stage_floats(sp) + (GW_KS / 4) * 16 * 4 + GW_PROD) * sizeof(float) + 256;
+}
+
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(tc05::smem_u32(bar)) : "memory");
 }
 
 __global__ void __launch_bounds__(GW_THREADS, 1)
-k_gradw_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float *__restrict__ qscale,
-           const int *__restrict__ struct_s, const float *__restrict__ e_s, const float *__restrict__ scales,
-           const float *__restrict__ q, const float *__restrict__ D, const float *__restrict__ x,
-           const float *__restrict__ p, float *__restrict__ partialW, float *__restrict__ partialB) {
+k_gradw_tc(DevSpec sp, SpeciesMap sm, int nstage, const float *__restrict__ theta, const float *__restrict__ qscale,
+           const float *__restrict__ eat, const float *__restrict__ q, const float *__restrict__ D,
+           const float *__restrict__ x, const float *__restrict__ p, float *__restrict__ partialW,
+           float *__restrict__ partialB) {
   using namespace tc05;
   extern __shared__ __align__(128) float smem[];
   constexpr int G4 = GW_KS / 4;                       // atom groups (16-byte K-chunks) per stage
@@ -346,10 +401,11 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const flo
   const int tileA = G4 * 128 * 4, tileB = G4 * NB * 4; // floats per operand tile
   const int stage_fl = 6 * tileA + 4 * tileB;
   // stage layout: Ah Al Bh Bl Vh Vl (rows = mu, 128) | Gh Gl Dh Dl (rows = nu, NB)
-  float *ones = smem + 2 * stage_fl;                  // [G4][16][4]
-  float *esh = ones + G4 * 16 * 4;                    // [GW_THREADS]
-  uint64_t *bars = (uint64_t *)(esh + GW_THREADS);    // [0,1] stage free, [2,3] accumulation group done
-  uint32_t *tmem_slot = (uint32_t *)(bars + 4);
+  float *ones = smem + nstage * stage_fl;             // [G4][16][4]
+  float *esh = ones + G4 * 16 * 4;                    // [GW_PROD]
+  uint64_t *bars = (uint64_t *)(esh + GW_PROD);       // full[4], empty[4], group[2]
+  uint64_t *full = bars, *empty = bars + 4, *group = bars + 8;
+  uint32_t *tmem_slot = (uint32_t *)(bars + 10);
   const int tid = threadIdx.x, warp = tid >> 5;
   const int t = species_of_block(sm.gw_base, sp.T, blockIdx.x);
   const float *net = theta + sp.offNet + (size_t)t * sp.netSize;
@@ -358,14 +414,15 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const flo
   const int c1 = min(c0 + sm.gw_atoms[t], sm.start[t + 1]);
   if (warp == 0) tmem_alloc(tmem_slot, 512);
   if (tid == 32) {
-    for (int i = 0; i < 4; ++i) mbar_init(bars + i, 1);
+    for (int i = 0; i < 4; ++i) { mbar_init(full + i, GW_PROD); mbar_init(empty + i, 1); }
+    mbar_init(group, 1); mbar_init(group + 1, 1);
     fence_mbar_init();
   }
-  for (int i = tid; i < 2 * stage_fl; i += GW_THREADS) smem[i] = 0.f;
+  for (int i = tid; i < nstage * stage_fl; i += GW_THREADS) smem[i] = 0.f;
   for (int i = tid; i < G4 * 16 * 4; i += GW_THREADS) ones[i] = 1.f;
   __syncthreads();
-  // the constant "G = 1" row (nu = Ndes) of both stages' Gh tiles
-  if (tid < 2 * G4 * 4) {
+  // the constant "G = 1" row (nu = Ndes) of every stage's Gh tile
+  if (tid < nstage * G4 * 4) {
     const int st = tid / (G4 * 4), rem = tid - st * G4 * 4, g = rem >> 2, i = rem & 3;
     smem[st * stage_fl + 6 * tileA + (g * NB + sp.Ndes) * 4 + i] = 1.f;
   }
@@ -376,147 +433,161 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const flo
   // TMEM set s (two of them): [0,NB) D3 main, [NB,2NB) D3 corrections, [2NB,2NB+16) D4 main, [2NB+16,2NB+32) D4 corr.
   const int setc = 2 * NB + 32;
   const uint32_t tb = *tmem_slot;
-  const uint32_t idW = idesc_tf32(128, NB, 0, 0), id1 = idesc_tf32(128, 16, 0, 0);
-  const uint32_t ones_a = smem_u32(ones);
-  const float se = scales[0];
-  const int nA = G4 * sp.Nn, nB = G4 * sp.Ndes;        // work items per stage
-  const int lane0 = (warp & 3) * 32;
-  float esum = 0.f;
-  float racc[GW_MAXC][16], rv = 0.f;                   // threads 0..127: row mu of D3, and D4[mu][0]
-#pragma unroll
-  for (int c = 0; c < GW_MAXC; ++c)
-#pragma unroll
-    for (int i = 0; i < 16; ++i) racc[c][i] = 0.f;
-
-  auto flush = [&](int g) {   // add accumulation group g (complete after its last commit) to the registers
-    if (tid < 128) {
-      if (!mbar_wait(bars + 2 + (g & 1), (uint32_t)((g >> 1) & 1))) __trap();
-      fence_after_sync();
-      const uint32_t ts = tb + (uint32_t)((g & 1) * setc);
-#pragma unroll
-      for (int c = 0; c < GW_MAXC; ++c)
-        if (c * 16 < NB) {
-          float m[16], k[16];
-          tmem_ld16(tmem_addr(ts, lane0, c * 16), m);
-          tmem_ld16(tmem_addr(ts, lane0, NB + c * 16), k);
-#pragma unroll
-          for (int i = 0; i < 16; ++i) racc[c][i] += m[i] + k[i];
-        }
-      float m8[8], k8[8];
-      tmem_ld8(tmem_addr(ts, lane0, 2 * NB), m8);
-      tmem_ld8(tmem_addr(ts, lane0, 2 * NB + 16), k8);
-      rv += m8[0] + k8[0];
-      fence_before_sync();
-    }
-  };
-
   const int nst = (c1 - c0 + GW_KS - 1) / GW_KS;
   const int ngroups = (nst + GW_FLUSH - 1) / GW_FLUSH;
-  for (int it = 0; it < nst; ++it) {
-    const int st = it & 1, g = it / GW_FLUSH, gi = it - g * GW_FLUSH;
-    float *sb = smem + st * stage_fl;
-    if (gi == 0 && g >= 1) flush(g - 1);
-    if (it >= 2 && !mbar_wait(bars + st, (uint32_t)(((it >> 1) - 1) & 1))) __trap();
-    const int a0 = c0 + it * GW_KS;
-    for (int w = tid; w < nA + nB; w += GW_THREADS) {
-      if (w < nA) {
-        const int ag = w / sp.Nn, mu = w - ag * sp.Nn;
-        const float w1 = w1g[mu];
-        float Av[4], Bv[4], Vv[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          const int a = a0 + 4 * ag + i;
-          Av[i] = 0.f; Bv[i] = 0.f; Vv[i] = 0.f;
-          if (a < c1) {
-            const float ev = se * e_s[struct_s[a]];
-            const float xv = x[(size_t)a * sp.Nn + mu], pv = p[(size_t)a * sp.Nn + mu];
-            const float d1 = 1.f - xv * xv, d2 = -2.f * xv * d1;
-            Av[i] = w1 * (ev * d1 + d2 * pv);
-            Bv[i] = w1 * d1;
-            Vv[i] = ev * xv + d1 * pv;
-            if (mu == 0) esum += ev;
-          }
+
+  if (warp == GW_PROD / 32) {
+    // ================= MMA issuer (one thread) =================
+    if ((tid & 31) == 0) {
+      const uint32_t idW = idesc_tf32(128, NB, 0, 0), id1 = idesc_tf32(128, 16, 0, 0);
+      const uint32_t ones_a = smem_u32(ones);
+      for (int it = 0; it < nst; ++it) {
+        const int st = it % nstage, use = it / nstage, g = it / GW_FLUSH, gi = it - g * GW_FLUSH;
+        if (!mbar_wait(full + st, (uint32_t)(use & 1))) __trap();
+        fence_after_sync();
+        const uint32_t ts = tb + (uint32_t)((g & 1) * setc);
+        const uint32_t tM = ts, tC = ts + NB, tV = ts + 2 * NB, tVc = tV + 16;
+        const uint32_t sa = smem_u32(smem + st * stage_fl), ga = sa + 6u * (uint32_t)tileA * 4u;
+        for (int s = 0; s < GW_KS / 8; ++s) {
+          const uint64_t Ah = desc_kmajor(sa, 128, s), Al = desc_kmajor(sa + tileA * 4, 128, s);
+          const uint64_t Bh = desc_kmajor(sa + 2 * tileA * 4, 128, s), Bl = desc_kmajor(sa + 3 * tileA * 4, 128, s);
+          const uint64_t Vh = desc_kmajor(sa + 4 * tileA * 4, 128, s), Vl = desc_kmajor(sa + 5 * tileA * 4, 128, s);
+          const uint64_t Gh = desc_kmajor(ga, NB, s), Gl = desc_kmajor(ga + tileB * 4, NB, s);
+          const uint64_t Dh = desc_kmajor(ga + 2 * tileB * 4, NB, s), Dl = desc_kmajor(ga + 3 * tileB * 4, NB, s);
+          const uint64_t On = desc_kmajor(ones_a, 16, s);
+          const uint32_t acc = (gi > 0 || s > 0) ? 1u : 0u;   // the first K-step of a group overwrites the set
+          mma_ss(tM, Ah, Gh, idW, acc);
+          mma_ss(tM, Bh, Dh, idW, 1);
+          mma_ss(tC, Ah, Gl, idW, acc);
+          mma_ss(tC, Al, Gh, idW, 1);
+          mma_ss(tC, Bh, Dl, idW, 1);
+          mma_ss(tC, Bl, Dh, idW, 1);
+          mma_ss(tV, Vh, On, id1, acc);
+          mma_ss(tVc, Vl, On, id1, acc);
         }
-        float4 hi, lo;
-        const int o = (ag * 128 + mu) * 4;
-        split4(make_float4(Av[0], Av[1], Av[2], Av[3]), hi, lo);
-        *(float4 *)(sb + o) = hi; *(float4 *)(sb + tileA + o) = lo;
-        split4(make_float4(Bv[0], Bv[1], Bv[2], Bv[3]), hi, lo);
-        *(float4 *)(sb + 2 * tileA + o) = hi; *(float4 *)(sb + 3 * tileA + o) = lo;
-        split4(make_float4(Vv[0], Vv[1], Vv[2], Vv[3]), hi, lo);
-        *(float4 *)(sb + 4 * tileA + o) = hi; *(float4 *)(sb + 5 * tileA + o) = lo;
-      } else {
-        const int wb = w - nA;
-        const int ag = wb / sp.Ndes, nu = wb - ag * sp.Ndes;
-        const float s = qscale[nu];
-        float Gv[4], Dv[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          const int a = a0 + 4 * ag + i;
-          const bool ok = a < c1;
-          Gv[i] = ok ? s * q[(size_t)a * sp.Ndes + nu] : 0.f;
-          Dv[i] = ok ? s * D[(size_t)a * sp.Ndes + nu] : 0.f;
-        }
-        float4 hi, lo;
-        float *gb = sb + 6 * tileA;
-        const int o = (ag * NB + nu) * 4;
-        split4(make_float4(Gv[0], Gv[1], Gv[2], Gv[3]), hi, lo);
-        *(float4 *)(gb + o) = hi; *(float4 *)(gb + tileB + o) = lo;
-        split4(make_float4(Dv[0], Dv[1], Dv[2], Dv[3]), hi, lo);
-        *(float4 *)(gb + 2 * tileB + o) = hi; *(float4 *)(gb + 3 * tileB + o) = lo;
+        mma_commit(empty + st);
+        if (gi == GW_FLUSH - 1 || it == nst - 1) mma_commit(group + (g & 1));
       }
     }
-    fence_async_smem();
-    fence_before_sync();
-    __syncthreads();
-    if (tid == 0) {
-      fence_after_sync();
-      const uint32_t ts = tb + (uint32_t)((g & 1) * setc);
-      const uint32_t tM = ts, tC = ts + NB, tV = ts + 2 * NB, tVc = tV + 16;
-      const uint32_t sa = smem_u32(sb), ga = sa + 6u * (uint32_t)tileA * 4u;
-      for (int s = 0; s < GW_KS / 8; ++s) {
-        const uint64_t Ah = desc_kmajor(sa, 128, s), Al = desc_kmajor(sa + tileA * 4, 128, s);
-        const uint64_t Bh = desc_kmajor(sa + 2 * tileA * 4, 128, s), Bl = desc_kmajor(sa + 3 * tileA * 4, 128, s);
-        const uint64_t Vh = desc_kmajor(sa + 4 * tileA * 4, 128, s), Vl = desc_kmajor(sa + 5 * tileA * 4, 128, s);
-        const uint64_t Gh = desc_kmajor(ga, NB, s), Gl = desc_kmajor(ga + tileB * 4, NB, s);
-        const uint64_t Dh = desc_kmajor(ga + 2 * tileB * 4, NB, s), Dl = desc_kmajor(ga + 3 * tileB * 4, NB, s);
-        const uint64_t On = desc_kmajor(ones_a, 16, s);
-        const uint32_t acc = (gi > 0 || s > 0) ? 1u : 0u;   // the first K-step of a group overwrites the set
-        mma_ss(tM, Ah, Gh, idW, acc);
-        mma_ss(tM, Bh, Dh, idW, 1);
-        mma_ss(tC, Ah, Gl, idW, acc);
-        mma_ss(tC, Al, Gh, idW, 1);
-        mma_ss(tC, Bh, Dl, idW, 1);
-        mma_ss(tC, Bl, Dh, idW, 1);
-        mma_ss(tV, Vh, On, id1, acc);
-        mma_ss(tVc, Vl, On, id1, acc);
-      }
-      mma_commit(bars + st);
-      if (gi == GW_FLUSH - 1 || it == nst - 1) mma_commit(bars + 2 + (g & 1));
-    }
-  }
-  if (ngroups > 0) flush(ngroups - 1);
-  esh[tid] = esum;
-  __syncthreads();
-  const int nb = 2 * sp.Nn + 1;
-  float *outW = partialW + (size_t)blockIdx.x * sp.Nn * sp.Ndes;
-  float *outB = partialB + (size_t)blockIdx.x * nb;
-  if (tid < sp.Nn) {
-    const int mu = tid;
+  } else {
+    // ================= producers (and, for threads 0..127, the register accumulators) =================
+    const int nI = G4 * (sp.Nn + sp.Ndes), nA = G4 * sp.Nn;   // work items per stage: (atom group, mu) then (atom group, nu)
+    const int lane0 = (warp & 3) * 32;
+    float esum = 0.f;
+    float racc[GW_MAXC][16], rv = 0.f;                 // threads 0..127: row mu of D3, and D4[mu][0]
 #pragma unroll
     for (int c = 0; c < GW_MAXC; ++c)
 #pragma unroll
-      for (int i = 0; i < 16; ++i) {
-        const int nu = c * 16 + i;
-        if (nu < sp.Ndes) outW[mu * sp.Ndes + nu] = racc[c][i];
-        else if (nu == sp.Ndes) outB[mu] = racc[c][i];
+      for (int i = 0; i < 16; ++i) racc[c][i] = 0.f;
+    auto flush = [&](int g) {   // add accumulation group g (complete after its last commit) to the registers
+      if (tid < 128) {
+        if (!mbar_wait(group + (g & 1), (uint32_t)((g >> 1) & 1))) __trap();
+        fence_after_sync();
+        const uint32_t ts = tb + (uint32_t)((g & 1) * setc);
+#pragma unroll
+        for (int c = 0; c < GW_MAXC; ++c)
+          if (c * 16 < NB) {
+            float m[16], k[16];
+            tmem_ld16(tmem_addr(ts, lane0, c * 16), m);
+            tmem_ld16(tmem_addr(ts, lane0, NB + c * 16), k);
+#pragma unroll
+            for (int i = 0; i < 16; ++i) racc[c][i] += m[i] + k[i];
+          }
+        float m8[8], k8[8];
+        tmem_ld8(tmem_addr(ts, lane0, 2 * NB), m8);
+        tmem_ld8(tmem_addr(ts, lane0, 2 * NB + 16), k8);
+        rv += m8[0] + k8[0];
+        fence_before_sync();
       }
-    outB[sp.Nn + mu] = rv;
-  }
-  if (tid == 0) {
-    float s = 0.f;
-    for (int i = 0; i < GW_THREADS; ++i) s += esh[i];
-    outB[2 * sp.Nn] = s;
+    };
+    for (int it = 0; it < nst; ++it) {
+      const int st = it % nstage, use = it / nstage, g = it / GW_FLUSH, gi = it - g * GW_FLUSH;
+      float *sb = smem + st * stage_fl;
+      if (gi == 0 && g >= 1) flush(g - 1);
+      if (use > 0 && !mbar_wait(empty + st, (uint32_t)((use - 1) & 1))) __trap();
+      const int a0 = c0 + it * GW_KS;
+      for (int w0 = tid; w0 < nI; w0 += 2 * GW_PROD) {
+        float raw[2][8], e4[2][4], cf[2];
+        int col[2], ag[2];
+        bool isA[2], on[2];
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {   // gather: all global loads of two items in flight together
+          const int w = w0 + j * GW_PROD;
+          on[j] = w < nI;
+          isA[j] = w < nA;
+          const int wl = isA[j] ? w : w - nA, W = isA[j] ? sp.Nn : sp.Ndes;
+          ag[j] = wl / W; col[j] = wl - ag[j] * W;
+          const float *r0 = isA[j] ? x : q, *r1 = isA[j] ? p : D;
+          cf[j] = on[j] ? (isA[j] ? w1g[col[j]] : qscale[col[j]]) : 0.f;
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const int a = a0 + 4 * ag[j] + i;
+            const bool ok = on[j] && a < c1;
+            raw[j][i] = ok ? r0[(size_t)a * W + col[j]] : 0.f;
+            raw[j][4 + i] = ok ? r1[(size_t)a * W + col[j]] : 0.f;
+            e4[j][i] = (ok && isA[j]) ? eat[a] : 0.f;
+          }
+        }
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+          if (!on[j]) continue;
+          float4 hi, lo;
+          if (isA[j]) {
+            float Av[4], Bv[4], Vv[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              const float xv = raw[j][i], pv = raw[j][4 + i], ev = e4[j][i];
+              const float d1 = 1.f - xv * xv, d2 = -2.f * xv * d1;
+              Av[i] = cf[j] * (ev * d1 + d2 * pv);
+              Bv[i] = cf[j] * d1;
+              Vv[i] = ev * xv + d1 * pv;
+              if (a0 + 4 * ag[j] + i >= c1) Bv[i] = 0.f;   // atoms past the range: x = 0 would give Bc = w1
+              if (col[j] == 0) esum += ev;
+            }
+            const int o = (ag[j] * 128 + col[j]) * 4;
+            split4(make_float4(Av[0], Av[1], Av[2], Av[3]), hi, lo);
+            *(float4 *)(sb + o) = hi; *(float4 *)(sb + tileA + o) = lo;
+            split4(make_float4(Bv[0], Bv[1], Bv[2], Bv[3]), hi, lo);
+            *(float4 *)(sb + 2 * tileA + o) = hi; *(float4 *)(sb + 3 * tileA + o) = lo;
+            split4(make_float4(Vv[0], Vv[1], Vv[2], Vv[3]), hi, lo);
+            *(float4 *)(sb + 4 * tileA + o) = hi; *(float4 *)(sb + 5 * tileA + o) = lo;
+          } else {
+            float *gb = sb + 6 * tileA;
+            const int o = (ag[j] * NB + col[j]) * 4;
+            split4(make_float4(cf[j] * raw[j][0], cf[j] * raw[j][1], cf[j] * raw[j][2], cf[j] * raw[j][3]), hi, lo);
+            *(float4 *)(gb + o) = hi; *(float4 *)(gb + tileB + o) = lo;
+            split4(make_float4(cf[j] * raw[j][4], cf[j] * raw[j][5], cf[j] * raw[j][6], cf[j] * raw[j][7]), hi, lo);
+            *(float4 *)(gb + 2 * tileB + o) = hi; *(float4 *)(gb + 3 * tileB + o) = lo;
+          }
+        }
+      }
+      fence_async_smem();
+      mbar_arrive(full + st);
+    }
+    if (ngroups > 0) flush(ngroups - 1);
+    esh[tid] = esum;
+    // results: rows mu < Nn live in threads 0..127
+    asm volatile("bar.sync 1, %0;" ::"n"(GW_PROD) : "memory");
+    const int nb = 2 * sp.Nn + 1;
+    float *outW = partialW + (size_t)blockIdx.x * sp.Nn * sp.Ndes;
+    float *outB = partialB + (size_t)blockIdx.x * nb;
+    if (tid < sp.Nn) {
+      const int mu = tid;
+#pragma unroll
+      for (int c = 0; c < GW_MAXC; ++c)
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+          const int nu = c * 16 + i;
+          if (nu < sp.Ndes) outW[mu * sp.Ndes + nu] = racc[c][i];
+          else if (nu == sp.Ndes) outB[mu] = racc[c][i];
+        }
+      outB[sp.Nn + mu] = rv;
+    }
+    if (tid == 0) {
+      float s = 0.f;
+      for (int i = 0; i < GW_PROD; ++i) s += esh[i];
+      outB[2 * sp.Nn] = s;
+    }
   }
   fence_before_sync();
   __syncthreads();
