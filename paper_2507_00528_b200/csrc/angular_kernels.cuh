@@ -97,7 +97,7 @@ k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
               const float4 *__restrict__ pairA, const float *__restrict__ theta, float *__restrict__ q,
               float *__restrict__ S, float *__restrict__ A1) {
   constexpr int R = (KT + 7) / 8;
-  extern __shared__ __align__(16) float smem[];
+  extern __shared__ __align__(128) float smem[];
   float *ct = smem;
   const int nct = sp.T * sp.T * KT * ANG_NQ;
   const int nA = sp.T * KT * GNEP_NLM;
@@ -234,7 +234,7 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
               const float *__restrict__ scales, const float *__restrict__ S, float *__restrict__ Tn,
               float *__restrict__ A2, float *__restrict__ D) {
   constexpr int R = (KT + 7) / 8;
-  extern __shared__ __align__(16) float smem[];
+  extern __shared__ __align__(128) float smem[];
   float *ct = smem;
   const int nct = sp.T * sp.T * KT * ANG_NQ;
   const int nA = sp.T * KT * GNEP_NLM;
@@ -395,7 +395,7 @@ __global__ void __launch_bounds__(ANG_WARPS * 32)
 k_angular_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ segA,
                 const int *__restrict__ atomA, const float4 *__restrict__ pairA, const float *__restrict__ theta,
                 const float *__restrict__ Ep, const float *__restrict__ S, float4 *__restrict__ fpair) {
-  extern __shared__ __align__(16) float smem[];
+  extern __shared__ __align__(128) float smem[];
   float *cs = smem;
   const int ncs = (sp.T * sp.T * sp.NA * KT + 3) & ~3;
   const int nb = sp.NA * GNEP_NLM;
@@ -518,7 +518,7 @@ __global__ void __launch_bounds__(ANG_WARPS * 32)
 k_cgrad_angular(DevSpec sp, int N, const int *__restrict__ type_s, const float *__restrict__ Ep,
                 const float *__restrict__ gbar, const float *__restrict__ S, const float *__restrict__ Tn,
                 const float *__restrict__ A1, const float *__restrict__ A2, float *__restrict__ partial) {
-  extern __shared__ __align__(16) float smem[];
+  extern __shared__ __align__(128) float smem[];
   const int nacc = sp.T * sp.T * sp.NA * KT;
   const int nb = sp.NA * GNEP_NLM;
   const int nA = sp.T * KT * GNEP_NLM;

@@ -13,7 +13,7 @@
 __global__ void __launch_bounds__(256)
 k_cgrad_radial(DevSpec sp, SpeciesMap sm, const float *__restrict__ gbar, const float *__restrict__ Ep,
                const float *__restrict__ M1, const float *__restrict__ M2, float *__restrict__ partialC) {
-  extern __shared__ __align__(16) float smem[];
+  extern __shared__ __align__(128) float smem[];
   const int TK = sp.T * sp.KRp;
   float *gb = smem, *ep = gb + CR_SUB * sp.NR, *m1 = ep + CR_SUB * sp.NR, *m2 = m1 + CR_SUB * TK;
   const int t = species_of_block(sm.chunk_base, sp.T, blockIdx.x);

@@ -46,15 +46,17 @@ __host__ __device__ inline NetDims net_dims(const DevSpec &sp) {
 __host__ __device__ inline size_t net_tc_smem_bytes(const DevSpec &sp, bool bwd) {
   NetDims d = net_dims(sp);
   size_t fl = 2 * (size_t)d.NdK * d.NnP + 2 * (size_t)d.NnP * d.NdN + 2 * d.NnP + d.NdN + 2 * (size_t)d.abuf;
-  if (!bwd) fl += pad_to(sp.T * sp.NR * sp.KRp, 4);
+  if (!bwd) fl += 16 * sp.T * sp.KRp;
   return fl * sizeof(float) + 128;
 }
 
 // tanh(z) = 1 - 2 / (exp(2 z) + 1) with the hardware exp2 and reciprocal: absolute error <= ~1e-7 over the whole range
 // (the argument rounding of exp2 only matters where tanh is already saturated), about 6 instructions.
 __device__ __forceinline__ float tanh_fast(float z) {
-  const float e = exp2f(fminf(z * 2.885390081777927f, 126.f));   // exp(2 z), clamped below overflow
-  return 1.f - __fdividef(2.f, e + 1.f);
+  float e, rc;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(fminf(z * 2.885390081777927f, 126.f)));   // exp(2 z), no overflow
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rc) : "f"(e + 1.f));
+  return fmaf(-2.f, rc, 1.f);
 }
 
 __device__ __forceinline__ void wg_barrier(int wg) { asm volatile("bar.sync %0, 128;" ::"r"(1 + wg) : "memory"); }
@@ -99,8 +101,8 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
   float *W1h = smem, *W1l = W1h + NdK * NnP;             // B of contraction 1: [NdK/4][NnP][4]   (n = mu, k = nu)
   float *W2h = W1l + NdK * NnP, *W2l = W2h + NnP * NdN;  // B of contraction 2: [NnP/4][NdN][4]   (n = nu, k = mu)
   float *b0s = W2l + NnP * NdN, *w1s = b0s + NnP, *qss = w1s + NnP;
-  float *cRs = qss + NdN;                                 // forward only: cR[t][J][n][k], k padded to KRp
-  float *abuf0 = cRs + (BWD ? 0 : pad_to(sp.T * sp.NR * sp.KRp, 4));
+  float *cRs = qss + NdN;                                 // forward only: cR[t][J][n][k] as [J*KRp + k][16] (zero padded)
+  float *abuf0 = cRs + (BWD ? 0 : 16 * sp.T * sp.KRp);
   uint64_t *bars = (uint64_t *)(abuf0 + 2 * nd.abuf);    // [wg][2]
   uint32_t *tmem_slot = (uint32_t *)(bars + 4);
   const int tid = threadIdx.x, warp = tid >> 5, wg = tid >> 7, r = tid & 127;
@@ -128,9 +130,9 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
   }
   for (int x = tid; x < NdN; x += 256) qss[x] = x < sp.Ndes ? qscale[x] : 0.f;
   if (!BWD)
-    for (int x = tid; x < sp.T * sp.NR * sp.KRp; x += 256) {
-      const int row = x / sp.KRp, k = x - row * sp.KRp;
-      cRs[x] = k < sp.KR ? theta[((size_t)t * sp.T * sp.NR + row) * sp.KR + k] : 0.f;
+    for (int x = tid; x < 16 * sp.T * sp.KRp; x += 256) {
+      const int o = x >> 4, n = x & 15, J = o / sp.KRp, k = o - J * sp.KRp;
+      cRs[x] = (n < sp.NR && k < sp.KR) ? theta[(((size_t)t * sp.T + J) * sp.NR + n) * sp.KR + k] : 0.f;
     }
   fence_async_smem();
   fence_before_sync();
@@ -331,14 +333,14 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
         float acc4[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-          const int oo = o + i;
-          if (oo < TK) {
-            const int J = oo / sp.KRp, k = oo - J * sp.KRp;
-            const float *c = cRs + (J * sp.NR) * sp.KRp + k;
+          if (o + i < TK) {
+            const float4 *c4 = (const float4 *)(cRs + (o + i) * 16);
             float s = 0.f;
 #pragma unroll
-            for (int n = 0; n < 16; ++n)
-              if (n < sp.NR) s += epr[n] * c[n * sp.KRp];
+            for (int v = 0; v < 4; ++v) {
+              const float4 c = c4[v];
+              s += epr[4 * v] * c.x + epr[4 * v + 1] * c.y + epr[4 * v + 2] * c.z + epr[4 * v + 3] * c.w;
+            }
             acc4[i] = s;
           }
         }
@@ -363,14 +365,15 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
 // overlaps the staging arithmetic and the MMAs of the others.
 // The tensor-core accumulator truncates at every accumulation, so the TMEM sums are kept short: a group of
 // GW_FLUSH stages accumulates into one of two TMEM sets (hi*hi products and the small 3xTF32 corrections in separate
-// accumulators) and is then added, with fp32 rounding, to register accumulators held by threads 0..127 (row mu).
+// accumulators) and is then added, with fp32 rounding, to register accumulators (row mu: threads mu and 128 + mu).
 // One partial per CTA is written at the end (reduced in fixed order, fp64, by k_grad_reduce).
 // ------------------------------------------------------------------------------------------------
 #define GW_KS 16        // atoms per stage (2 MMA K-steps)
 #define GW_FLUSH 4      // stages per TMEM accumulation group
 #define GW_PROD 256     // producer threads
 #define GW_THREADS (GW_PROD + 32)
-#define GW_MAXC 7       // 16-column chunks of the widest accumulator (NB <= 112)
+#define GW_MAXC 4       // 16-column chunks of the accumulator held by one thread (NB <= 112: 7 chunks over two warpgroups)
+#define GW_MAXI 4       // work items per producer thread and stage: 4 (Nn + Ndes) <= GW_MAXI * GW_PROD
 
 __host__ __device__ inline int gw_ncols(const DevSpec &sp) { return pad_to(sp.Ndes + 1, 16); }
 __host__ __device__ inline size_t gradw_stage_floats(const DevSpec &sp) {
@@ -470,95 +473,105 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, int nstage, const float *__restrict__ thet
       }
     }
   } else {
-    // ================= producers (and, for threads 0..127, the register accumulators) =================
+    // ================= producers (which also hold the register accumulators) =================
     const int nI = G4 * (sp.Nn + sp.Ndes), nA = G4 * sp.Nn;   // work items per stage: (atom group, mu) then (atom group, nu)
     const int lane0 = (warp & 3) * 32;
     float esum = 0.f;
-    float racc[GW_MAXC][16], rv = 0.f;                 // threads 0..127: row mu of D3, and D4[mu][0]
+    // Row mu of D3 is held by two threads (TMEM lane mu is visible to warps w and w + 4): thread mu owns the column
+    // chunks [0, chalf), thread 128 + mu the chunks [chalf, nch) and D4[mu][0].
+    const int wgp = tid >> 7, nch = NB >> 4, chalf = (nch + 1) >> 1, cbeg = wgp ? chalf : 0, ccnt = wgp ? nch - chalf : chalf;
+    float racc[GW_MAXC][16], rv = 0.f;
 #pragma unroll
     for (int c = 0; c < GW_MAXC; ++c)
 #pragma unroll
       for (int i = 0; i < 16; ++i) racc[c][i] = 0.f;
     auto flush = [&](int g) {   // add accumulation group g (complete after its last commit) to the registers
-      if (tid < 128) {
-        if (!mbar_wait(group + (g & 1), (uint32_t)((g >> 1) & 1))) __trap();
-        fence_after_sync();
-        const uint32_t ts = tb + (uint32_t)((g & 1) * setc);
+      if (!mbar_wait(group + (g & 1), (uint32_t)((g >> 1) & 1))) __trap();
+      fence_after_sync();
+      const uint32_t ts = tb + (uint32_t)((g & 1) * setc);
 #pragma unroll
-        for (int c = 0; c < GW_MAXC; ++c)
-          if (c * 16 < NB) {
-            float m[16], k[16];
-            tmem_ld16(tmem_addr(ts, lane0, c * 16), m);
-            tmem_ld16(tmem_addr(ts, lane0, NB + c * 16), k);
+      for (int c = 0; c < GW_MAXC; ++c)
+        if (c < ccnt) {
+          float m[16], k[16];
+          tmem_ld16(tmem_addr(ts, lane0, (cbeg + c) * 16), m);
+          tmem_ld16(tmem_addr(ts, lane0, NB + (cbeg + c) * 16), k);
 #pragma unroll
-            for (int i = 0; i < 16; ++i) racc[c][i] += m[i] + k[i];
-          }
+          for (int i = 0; i < 16; ++i) racc[c][i] += m[i] + k[i];
+        }
+      if (wgp) {
         float m8[8], k8[8];
         tmem_ld8(tmem_addr(ts, lane0, 2 * NB), m8);
         tmem_ld8(tmem_addr(ts, lane0, 2 * NB + 16), k8);
         rv += m8[0] + k8[0];
-        fence_before_sync();
       }
+      fence_before_sync();
     };
+    // The work items of a stage are the same in every stage: (atom group ag, column) of the A-side (x, p -> A, Bc, V)
+    // followed by the B-side (q, D -> G, sD).  Each thread decodes its (up to GW_MAXI) items once.
+    int g_off[GW_MAXI], s_off[GW_MAXI], i_ag[GW_MAXI], i_kind[GW_MAXI];   // kind: 0 none, 1 A-side, 2 B-side
+    float i_cf[GW_MAXI];
+#pragma unroll
+    for (int j = 0; j < GW_MAXI; ++j) {
+      const int w = tid + j * GW_PROD;
+      i_kind[j] = w < nA ? 1 : (w < nI ? 2 : 0);
+      const int wl = w < nA ? w : w - nA, W = w < nA ? sp.Nn : sp.Ndes;
+      const int ag = i_kind[j] ? wl / W : 0, col = i_kind[j] ? wl - ag * W : 0;
+      i_ag[j] = 4 * ag;
+      g_off[j] = 4 * ag * W + col;
+      s_off[j] = i_kind[j] == 1 ? (ag * 128 + col) * 4 : 6 * tileA + (ag * NB + col) * 4;
+      i_cf[j] = i_kind[j] == 1 ? w1g[col] : (i_kind[j] == 2 ? qscale[col] : 0.f);
+      if (i_kind[j] == 1 && col == 0) i_kind[j] = 3;   // this item also sums the energy seeds (dL/db1)
+    }
     for (int it = 0; it < nst; ++it) {
       const int st = it % nstage, use = it / nstage, g = it / GW_FLUSH, gi = it - g * GW_FLUSH;
       float *sb = smem + st * stage_fl;
       if (gi == 0 && g >= 1) flush(g - 1);
-      if (use > 0 && !mbar_wait(empty + st, (uint32_t)((use - 1) & 1))) __trap();
       const int a0 = c0 + it * GW_KS;
-      for (int w0 = tid; w0 < nI; w0 += 2 * GW_PROD) {
-        float raw[2][8], e4[2][4], cf[2];
-        int col[2], ag[2];
-        bool isA[2], on[2];
+      const int nval = c1 - a0;                       // atoms of this stage inside the range (>= GW_KS except in the tail)
+      float raw[GW_MAXI][8], e4[GW_MAXI][4];
 #pragma unroll
-        for (int j = 0; j < 2; ++j) {   // gather: all global loads of two items in flight together
-          const int w = w0 + j * GW_PROD;
-          on[j] = w < nI;
-          isA[j] = w < nA;
-          const int wl = isA[j] ? w : w - nA, W = isA[j] ? sp.Nn : sp.Ndes;
-          ag[j] = wl / W; col[j] = wl - ag[j] * W;
-          const float *r0 = isA[j] ? x : q, *r1 = isA[j] ? p : D;
-          cf[j] = on[j] ? (isA[j] ? w1g[col[j]] : qscale[col[j]]) : 0.f;
+      for (int j = 0; j < GW_MAXI; ++j) {             // gather: all global loads of the stage in flight together
+        const bool isA = i_kind[j] & 1;
+        const int W = isA ? sp.Nn : sp.Ndes;
+        const float *r0 = (isA ? x : q) + (size_t)a0 * W + g_off[j];
+        const float *r1 = (isA ? p : D) + (size_t)a0 * W + g_off[j];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const bool ok = i_kind[j] != 0 && i_ag[j] + i < nval;
+          raw[j][i] = ok ? r0[i * W] : 0.f;
+          raw[j][4 + i] = ok ? r1[i * W] : 0.f;
+          e4[j][i] = (ok && isA) ? eat[a0 + i_ag[j] + i] : 0.f;
+        }
+      }
+      if (use > 0 && !mbar_wait(empty + st, (uint32_t)((use - 1) & 1))) __trap();
+#pragma unroll
+      for (int j = 0; j < GW_MAXI; ++j) {
+        if (i_kind[j] == 0) continue;
+        float4 hi, lo;
+        float *dst = sb + s_off[j];
+        const float cf = i_cf[j];
+        if (i_kind[j] & 1) {
+          float Av[4], Bv[4], Vv[4];
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
-            const int a = a0 + 4 * ag[j] + i;
-            const bool ok = on[j] && a < c1;
-            raw[j][i] = ok ? r0[(size_t)a * W + col[j]] : 0.f;
-            raw[j][4 + i] = ok ? r1[(size_t)a * W + col[j]] : 0.f;
-            e4[j][i] = (ok && isA[j]) ? eat[a] : 0.f;
+            const float xv = raw[j][i], pv = raw[j][4 + i], ev = e4[j][i];
+            const float d1 = 1.f - xv * xv, d2 = -2.f * xv * d1;
+            Av[i] = cf * (ev * d1 + d2 * pv);
+            Bv[i] = i_ag[j] + i < nval ? cf * d1 : 0.f;   // atoms past the range: x = 0 would give Bc = w1
+            Vv[i] = ev * xv + d1 * pv;
+            if (i_kind[j] == 3) esum += ev;
           }
-        }
-#pragma unroll
-        for (int j = 0; j < 2; ++j) {
-          if (!on[j]) continue;
-          float4 hi, lo;
-          if (isA[j]) {
-            float Av[4], Bv[4], Vv[4];
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-              const float xv = raw[j][i], pv = raw[j][4 + i], ev = e4[j][i];
-              const float d1 = 1.f - xv * xv, d2 = -2.f * xv * d1;
-              Av[i] = cf[j] * (ev * d1 + d2 * pv);
-              Bv[i] = cf[j] * d1;
-              Vv[i] = ev * xv + d1 * pv;
-              if (a0 + 4 * ag[j] + i >= c1) Bv[i] = 0.f;   // atoms past the range: x = 0 would give Bc = w1
-              if (col[j] == 0) esum += ev;
-            }
-            const int o = (ag[j] * 128 + col[j]) * 4;
-            split4(make_float4(Av[0], Av[1], Av[2], Av[3]), hi, lo);
-            *(float4 *)(sb + o) = hi; *(float4 *)(sb + tileA + o) = lo;
-            split4(make_float4(Bv[0], Bv[1], Bv[2], Bv[3]), hi, lo);
-            *(float4 *)(sb + 2 * tileA + o) = hi; *(float4 *)(sb + 3 * tileA + o) = lo;
-            split4(make_float4(Vv[0], Vv[1], Vv[2], Vv[3]), hi, lo);
-            *(float4 *)(sb + 4 * tileA + o) = hi; *(float4 *)(sb + 5 * tileA + o) = lo;
-          } else {
-            float *gb = sb + 6 * tileA;
-            const int o = (ag[j] * NB + col[j]) * 4;
-            split4(make_float4(cf[j] * raw[j][0], cf[j] * raw[j][1], cf[j] * raw[j][2], cf[j] * raw[j][3]), hi, lo);
-            *(float4 *)(gb + o) = hi; *(float4 *)(gb + tileB + o) = lo;
-            split4(make_float4(cf[j] * raw[j][4], cf[j] * raw[j][5], cf[j] * raw[j][6], cf[j] * raw[j][7]), hi, lo);
-            *(float4 *)(gb + 2 * tileB + o) = hi; *(float4 *)(gb + 3 * tileB + o) = lo;
-          }
+          split4(make_float4(Av[0], Av[1], Av[2], Av[3]), hi, lo);
+          *(float4 *)(dst) = hi; *(float4 *)(dst + tileA) = lo;
+          split4(make_float4(Bv[0], Bv[1], Bv[2], Bv[3]), hi, lo);
+          *(float4 *)(dst + 2 * tileA) = hi; *(float4 *)(dst + 3 * tileA) = lo;
+          split4(make_float4(Vv[0], Vv[1], Vv[2], Vv[3]), hi, lo);
+          *(float4 *)(dst + 4 * tileA) = hi; *(float4 *)(dst + 5 * tileA) = lo;
+        } else {
+          split4(make_float4(cf * raw[j][0], cf * raw[j][1], cf * raw[j][2], cf * raw[j][3]), hi, lo);
+          *(float4 *)(dst) = hi; *(float4 *)(dst + tileB) = lo;
+          split4(make_float4(cf * raw[j][4], cf * raw[j][5], cf * raw[j][6], cf * raw[j][7]), hi, lo);
+          *(float4 *)(dst + 2 * tileB) = hi; *(float4 *)(dst + 3 * tileB) = lo;
         }
       }
       fence_async_smem();
@@ -566,22 +579,24 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, int nstage, const float *__restrict__ thet
     }
     if (ngroups > 0) flush(ngroups - 1);
     esh[tid] = esum;
-    // results: rows mu < Nn live in threads 0..127
+    // results: row mu lives in threads mu and 128 + mu
     asm volatile("bar.sync 1, %0;" ::"n"(GW_PROD) : "memory");
     const int nb = 2 * sp.Nn + 1;
     float *outW = partialW + (size_t)blockIdx.x * sp.Nn * sp.Ndes;
     float *outB = partialB + (size_t)blockIdx.x * nb;
-    if (tid < sp.Nn) {
-      const int mu = tid;
+    if ((tid & 127) < sp.Nn) {
+      const int mu = tid & 127;
 #pragma unroll
       for (int c = 0; c < GW_MAXC; ++c)
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
-          const int nu = c * 16 + i;
-          if (nu < sp.Ndes) outW[mu * sp.Ndes + nu] = racc[c][i];
-          else if (nu == sp.Ndes) outB[mu] = racc[c][i];
+          const int nu = (cbeg + c) * 16 + i;
+          if (c < ccnt) {
+            if (nu < sp.Ndes) outW[mu * sp.Ndes + nu] = racc[c][i];
+            else if (nu == sp.Ndes) outB[mu] = racc[c][i];
+          }
         }
-      outB[sp.Nn + mu] = rv;
+      if (wgp) outB[sp.Nn + mu] = rv;
     }
     if (tid == 0) {
       float s = 0.f;

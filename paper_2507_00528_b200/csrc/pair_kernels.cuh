@@ -19,7 +19,7 @@ __global__ void __launch_bounds__(GNEP_WARPS * 32)
 k_radial_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ segR,
              const float4 *__restrict__ pairR, const float *__restrict__ theta, float *__restrict__ q,
              float *__restrict__ M1) {
-  extern __shared__ __align__(16) float smem[];
+  extern __shared__ __align__(128) float smem[];
   float *cs = smem;                                          // [T*T*NR][KT]
   int ncs = sp.T * sp.T * sp.NR * KT;
   float *wbuf = warp_smem(smem + ncs, KT * 33 + KT);          // reduce buffer + moment row
@@ -148,7 +148,7 @@ k_radial_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__res
              const int *__restrict__ segR, const float4 *__restrict__ pairR, const float *__restrict__ theta,
              const float4 *__restrict__ u, const float *__restrict__ omega, const float *__restrict__ scales,
              float *__restrict__ D, float *__restrict__ M2) {
-  extern __shared__ __align__(16) float smem[];
+  extern __shared__ __align__(128) float smem[];
   float *cs = smem;
   int ncs = sp.T * sp.T * sp.NR * KT;
   float *wbuf = warp_smem(smem + ncs, KT * 33 + KT);
