@@ -161,7 +161,7 @@ int configure_kernels(gnep_handle *h) {
   }
   RET_IF(set_smem(h, k_net_tc<false>, smem_net_fwd(d)));
   RET_IF(set_smem(h, k_net_tc<true>, smem_net_bwd(d)));
-  if (gradw_stages(d) < 2) return fail(h, GNEP_EINVAL, "model too large for shared memory staging (n_descriptors)");
+  if (gradw_nraw(d) < 2) return fail(h, GNEP_EINVAL, "model too large for shared memory staging (n_descriptors)");
   RET_IF(set_smem(h, k_gradw_tc, smem_gradw(d)));
   RET_IF(set_smem(h, k_cgrad_radial, smem_cgrad_rad(d)));
   return GNEP_OK;
@@ -252,7 +252,7 @@ int enqueue_backward(gnep_handle *h) {
   LAUNCH(h, k_net_tc<true>, h->n_cta_net, 256, smem_net_bwd(d), d, h->sm, h->theta, h->qscale, h->D, h->x, h->eat, h->Ep, (float *)nullptr,
          h->struct_s, h->e_s, h->scales, h->pbuf, h->gbar);
   mark(h, "a6_network_backward");
-  LAUNCH(h, k_gradw_tc, h->n_gw, GW_THREADS, smem_gradw(d), d, h->sm, gradw_stages(d), h->theta, h->qscale, h->eat, h->q, h->D, h->x, h->pbuf, h->partialW, h->partialB);
+  LAUNCH(h, k_gradw_tc, h->n_gw, GW_THREADS, smem_gradw(d), d, h->sm, gradw_nraw(d), h->theta, h->qscale, h->eat, h->q, h->D, h->x, h->pbuf, h->partialW, h->partialB);
   mark(h, "a6_w0_gradient");
   LAUNCH(h, k_cgrad_radial, h->n_chunks, 256, smem_cgrad_rad(d), d, h->sm, h->gbar, h->Ep, h->M1, h->M2, h->partialCR);
   mark(h, "a7_radial_cgrad");
@@ -657,15 +657,21 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     h->rm.n_warps_ca = N > 0 ? h->n_ca_blocks * ANG_WARPS : 0;
     // ---- per-atom state ----
     const size_t n = N;
-    BA(h->q, n * d.Ndes); BA(h->Sn, n * d.NA * GNEP_NLM); BA(h->x, n * d.Nn); BA(h->Ei, n); BA(h->Ep, n * d.Ndes);
-    BA(h->etil, n * T * d.KRp); BA(h->M1, n * T * d.KRp); BA(h->M2, n * T * d.KRp); BA(h->D, n * d.Ndes); BA(h->Tn, n * d.NA * GNEP_NLM); BA(h->A1, n * T * d.KAp * GNEP_NLM); BA(h->A2, n * T * d.KAp * GNEP_NLM);
-    BA(h->gbar, n * d.Ndes); BA(h->pbuf, n * d.Nn); BA(h->eat, n); BA(h->Wat, n * 6);
+    const size_t npad = n + GW_PAD_ROWS;   // k_gradw_tc bulk-copies whole windows of rows: zeroed rows past the end
+    BA(h->q, npad * d.Ndes); BA(h->Sn, n * d.NA * GNEP_NLM); BA(h->x, npad * d.Nn); BA(h->Ei, n); BA(h->Ep, n * d.Ndes);
+    BA(h->etil, n * T * d.KRp); BA(h->M1, n * T * d.KRp); BA(h->M2, n * T * d.KRp); BA(h->D, npad * d.Ndes); BA(h->Tn, n * d.NA * GNEP_NLM); BA(h->A1, n * T * d.KAp * GNEP_NLM); BA(h->A2, n * T * d.KAp * GNEP_NLM);
+    BA(h->gbar, n * d.Ndes); BA(h->pbuf, npad * d.Nn); BA(h->eat, npad); BA(h->Wat, n * 6);
     BA(h->Fat, n); BA(h->fpair, nA); BA(h->u, n);
     BA(h->Es, S); BA(h->Ws, (size_t)S * 6); BA(h->parts, (size_t)S * 3); BA(h->e_s, S); BA(h->omega, (size_t)S * 6);
     BA(h->partialCR, (size_t)std::max(h->n_chunks, 1) * d.NR * T * d.KRp);
     BA(h->partialCA, (size_t)std::max(h->rm.n_warps_ca, 1) * T * T * d.NA * d.KAp);
     BA(h->partialW, (size_t)std::max(h->n_gw, 1) * d.Nn * d.Ndes);
     BA(h->partialB, (size_t)std::max(h->n_gw, 1) * (2 * d.Nn + 1));
+    CKT(cudaMemsetAsync(h->q + n * d.Ndes, 0, sizeof(float) * GW_PAD_ROWS * d.Ndes, st));
+    CKT(cudaMemsetAsync(h->D + n * d.Ndes, 0, sizeof(float) * GW_PAD_ROWS * d.Ndes, st));
+    CKT(cudaMemsetAsync(h->x + n * d.Nn, 0, sizeof(float) * GW_PAD_ROWS * d.Nn, st));
+    CKT(cudaMemsetAsync(h->pbuf + n * d.Nn, 0, sizeof(float) * GW_PAD_ROWS * d.Nn, st));
+    CKT(cudaMemsetAsync(h->eat + n, 0, sizeof(float) * GW_PAD_ROWS, st));
 #undef BA
 #undef CKT
     h->loaded = true;

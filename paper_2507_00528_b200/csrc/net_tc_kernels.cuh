@@ -359,41 +359,70 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
 //   D3[mu][nu]   = sum_a A[a][mu] G[a][nu] + Bc[a][mu] sD[a][nu]      (dL/dW0; column nu = Ndes carries G = 1 -> dL/db0)
 //   D4[mu][0]    = sum_a V[a][mu]                                       (dL/dw1)
 // A, Bc, V are formed on the fly from x, p and the per-atom energy seed e.  Each CTA owns a contiguous atom range of
-// one species.  Warps 0..7 are producers: they stage the operands K-major ([atoms/4][row][4], hi/lo split) into a ring
-// of `nstage` stages of GW_KS atoms and arrive on the stage's "full" mbarrier; warp 8 issues the MMAs of a full stage
-// and commits to its "empty" mbarrier.  No CTA-wide barrier sits in the loop, so the global-load latency of one stage
-// overlaps the staging arithmetic and the MMAs of the others.
+// one species and walks it in windows of GW_KS atoms aligned to absolute multiples of GW_KS (so that every row block
+// is 16-byte aligned for any row length; atoms of a window outside the CTA's range are masked out).
+//   warp 9 (one thread)  bulk-copies (cp.async.bulk, mbarrier complete_tx) the raw rows x, p, q, D, e of a window --
+//                        five contiguous blocks -- into a ring of `nraw` raw stages;
+//   warps 0..7           turn a raw stage into the K-major operand tiles ([atoms/4][row][4], hi/lo split) of one of
+//                        GW_OPST operand stages and arrive on its "full" mbarrier;
+//   warp 8 (one thread)  issues the MMAs of a full operand stage and commits to its "empty" mbarrier.
+// No CTA-wide barrier and no exposed global-load latency sit in the loop.
 // The tensor-core accumulator truncates at every accumulation, so the TMEM sums are kept short: a group of
 // GW_FLUSH stages accumulates into one of two TMEM sets (hi*hi products and the small 3xTF32 corrections in separate
 // accumulators) and is then added, with fp32 rounding, to register accumulators (row mu: threads mu and 128 + mu).
 // One partial per CTA is written at the end (reduced in fixed order, fp64, by k_grad_reduce).
+// The bulk copies of the last window may read up to GW_KS rows past the end of the arrays: the host pads x, p, q, D, e
+// by GW_PAD_ROWS zeroed rows.
 // ------------------------------------------------------------------------------------------------
 #define GW_KS 16        // atoms per stage (2 MMA K-steps)
 #define GW_FLUSH 4      // stages per TMEM accumulation group
 #define GW_PROD 256     // producer threads
-#define GW_THREADS (GW_PROD + 32)
+#define GW_THREADS (GW_PROD + 64)
 #define GW_MAXC 4       // 16-column chunks of the accumulator held by one thread (NB <= 112: 7 chunks over two warpgroups)
 #define GW_MAXI 4       // work items per producer thread and stage: 4 (Nn + Ndes) <= GW_MAXI * GW_PROD
+#define GW_OPST 2       // operand stages
+#define GW_MAXRAW 6     // raw stages (at most)
+#define GW_PAD_ROWS 32  // zeroed rows the host appends to x, p, q, D, e
 
 __host__ __device__ inline int gw_ncols(const DevSpec &sp) { return pad_to(sp.Ndes + 1, 16); }
 __host__ __device__ inline size_t gradw_stage_floats(const DevSpec &sp) {
   return 6 * (size_t)(GW_KS / 4) * 128 * 4 + 4 * (size_t)(GW_KS / 4) * gw_ncols(sp) * 4;
 }
-__host__ __device__ inline int gradw_stages(const DevSpec &sp) {
-  const size_t fixed = ((GW_KS / 4) * 16 * 4 + GW_PROD) * sizeof(float) + 256;
-  int n = (int)((227 * 1024 - fixed) / (gradw_stage_floats(sp) * sizeof(float)));
-  return n > 4 ? 4 : n;
+__host__ __device__ inline size_t gradw_raw_floats(const DevSpec &sp) { return (size_t)GW_KS * (2 * sp.Nn + 2 * sp.Ndes + 1); }
+__host__ __device__ inline size_t gradw_fixed_bytes() { return ((GW_KS / 4) * 16 * 4 + GW_PROD) * sizeof(float) + 256; }
+__host__ __device__ inline int gradw_nraw(const DevSpec &sp) {
+  const long long left = 227ll * 1024 - (long long)gradw_fixed_bytes() - (long long)(GW_OPST * gradw_stage_floats(sp) * sizeof(float));
+  if (left <= 0) return 0;
+  const int n = (int)(left / (long long)(gradw_raw_floats(sp) * sizeof(float)));
+  return n > GW_MAXRAW ? GW_MAXRAW : n;
 }
 __host__ __device__ inline size_t gradw_smem_bytes(const DevSpec &sp) {
-  return (gradw_stages(sp) * gradw_stage_floats(sp) + (GW_KS / 4) * 16 * 4 + GW_PROD) * sizeof(float) + 256;
+  return (GW_OPST * gradw_stage_floats(sp) + gradw_nraw(sp) * gradw_raw_floats(sp)) * sizeof(float) + gradw_fixed_bytes();
 }
 
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(tc05::smem_u32(bar)) : "memory");
 }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(tc05::smem_u32(bar)), "r"(bytes) : "memory");
+}
+// contiguous global -> shared bulk copy (16-byte aligned addresses and size), completion counted on an mbarrier
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(tc05::smem_u32(dst)), "l"(__cvta_generic_to_global(src)), "r"(bytes), "r"(tc05::smem_u32(bar))
+               : "memory");
+}
+// 3xTF32 split with integer round-half-away (2 + 1 + 2 instructions): hi = tf32(x), lo = tf32(x - hi)
+__device__ __forceinline__ void split_fast(float x, float &hi, float &lo) {
+  hi = __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
+  lo = __uint_as_float((__float_as_uint(x - hi) + 0x1000u) & 0xffffe000u);
+}
+__device__ __forceinline__ void split4_fast(const float4 &x, float4 &hi, float4 &lo) {
+  split_fast(x.x, hi.x, lo.x); split_fast(x.y, hi.y, lo.y); split_fast(x.z, hi.z, lo.z); split_fast(x.w, hi.w, lo.w);
+}
 
 __global__ void __launch_bounds__(GW_THREADS, 1)
-k_gradw_tc(DevSpec sp, SpeciesMap sm, int nstage, const float *__restrict__ theta, const float *__restrict__ qscale,
+k_gradw_tc(DevSpec sp, SpeciesMap sm, int nraw, const float *__restrict__ theta, const float *__restrict__ qscale,
            const float *__restrict__ eat, const float *__restrict__ q, const float *__restrict__ D,
            const float *__restrict__ x, const float *__restrict__ p, float *__restrict__ partialW,
            float *__restrict__ partialB) {
@@ -403,29 +432,33 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, int nstage, const float *__restrict__ thet
   const int NB = gw_ncols(sp);
   const int tileA = G4 * 128 * 4, tileB = G4 * NB * 4; // floats per operand tile
   const int stage_fl = 6 * tileA + 4 * tileB;
-  // stage layout: Ah Al Bh Bl Vh Vl (rows = mu, 128) | Gh Gl Dh Dl (rows = nu, NB)
-  float *ones = smem + nstage * stage_fl;             // [G4][16][4]
+  const int raw_fl = GW_KS * (2 * sp.Nn + 2 * sp.Ndes + 1);
+  // operand stage: Ah Al Bh Bl Vh Vl (rows = mu, 128) | Gh Gl Dh Dl (rows = nu, NB);  raw stage: x | p | q | D | e
+  float *raw = smem + GW_OPST * stage_fl;
+  float *ones = raw + nraw * raw_fl;                  // [G4][16][4]
   float *esh = ones + G4 * 16 * 4;                    // [GW_PROD]
-  uint64_t *bars = (uint64_t *)(esh + GW_PROD);       // full[4], empty[4], group[2]
-  uint64_t *full = bars, *empty = bars + 4, *group = bars + 8;
-  uint32_t *tmem_slot = (uint32_t *)(bars + 10);
+  uint64_t *bars = (uint64_t *)(esh + GW_PROD);
+  uint64_t *full = bars, *empty = bars + 2, *group = bars + 4, *rfull = bars + 6, *rempty = bars + 6 + GW_MAXRAW;
+  uint32_t *tmem_slot = (uint32_t *)(bars + 6 + 2 * GW_MAXRAW);
   const int tid = threadIdx.x, warp = tid >> 5;
   const int t = species_of_block(sm.gw_base, sp.T, blockIdx.x);
   const float *net = theta + sp.offNet + (size_t)t * sp.netSize;
   const float *w1g = net + sp.Nn * sp.Ndes + sp.Nn;
   const int c0 = sm.start[t] + (blockIdx.x - sm.gw_base[t]) * sm.gw_atoms[t];
   const int c1 = min(c0 + sm.gw_atoms[t], sm.start[t + 1]);
+  const int w0 = c0 & ~(GW_KS - 1);                   // first window (absolute multiple of GW_KS)
   if (warp == 0) tmem_alloc(tmem_slot, 512);
   if (tid == 32) {
-    for (int i = 0; i < 4; ++i) { mbar_init(full + i, GW_PROD); mbar_init(empty + i, 1); }
+    for (int i = 0; i < GW_OPST; ++i) { mbar_init(full + i, GW_PROD); mbar_init(empty + i, 1); }
     mbar_init(group, 1); mbar_init(group + 1, 1);
+    for (int i = 0; i < GW_MAXRAW; ++i) { mbar_init(rfull + i, 1); mbar_init(rempty + i, GW_PROD); }
     fence_mbar_init();
   }
-  for (int i = tid; i < nstage * stage_fl; i += GW_THREADS) smem[i] = 0.f;
+  for (int i = tid; i < GW_OPST * stage_fl; i += GW_THREADS) smem[i] = 0.f;
   for (int i = tid; i < G4 * 16 * 4; i += GW_THREADS) ones[i] = 1.f;
   __syncthreads();
   // the constant "G = 1" row (nu = Ndes) of every stage's Gh tile
-  if (tid < nstage * G4 * 4) {
+  if (tid < GW_OPST * G4 * 4) {
     const int st = tid / (G4 * 4), rem = tid - st * G4 * 4, g = rem >> 2, i = rem & 3;
     smem[st * stage_fl + 6 * tileA + (g * NB + sp.Ndes) * 4 + i] = 1.f;
   }
@@ -436,16 +469,34 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, int nstage, const float *__restrict__ thet
   // TMEM set s (two of them): [0,NB) D3 main, [NB,2NB) D3 corrections, [2NB,2NB+16) D4 main, [2NB+16,2NB+32) D4 corr.
   const int setc = 2 * NB + 32;
   const uint32_t tb = *tmem_slot;
-  const int nst = (c1 - c0 + GW_KS - 1) / GW_KS;
+  const int nst = (c1 - w0 + GW_KS - 1) / GW_KS;
   const int ngroups = (nst + GW_FLUSH - 1) / GW_FLUSH;
 
-  if (warp == GW_PROD / 32) {
+  if (warp == GW_PROD / 32 + 1) {
+    // ================= bulk-copy issuer (one thread) =================
+    if ((tid & 31) == 0) {
+      const uint32_t bx = (uint32_t)(GW_KS * sp.Nn * sizeof(float)), bq = (uint32_t)(GW_KS * sp.Ndes * sizeof(float));
+      const uint32_t be = (uint32_t)(GW_KS * sizeof(float));
+      for (int it = 0; it < nst; ++it) {
+        const int rs = it % nraw, use = it / nraw;
+        if (use > 0 && !mbar_wait(rempty + rs, (uint32_t)((use - 1) & 1))) __trap();
+        const size_t a0 = (size_t)(w0 + it * GW_KS);
+        float *rb = raw + rs * raw_fl;
+        mbar_expect_tx(rfull + rs, 2 * bx + 2 * bq + be);
+        bulk_g2s(rb, x + a0 * sp.Nn, bx, rfull + rs);
+        bulk_g2s(rb + GW_KS * sp.Nn, p + a0 * sp.Nn, bx, rfull + rs);
+        bulk_g2s(rb + 2 * GW_KS * sp.Nn, q + a0 * sp.Ndes, bq, rfull + rs);
+        bulk_g2s(rb + 2 * GW_KS * sp.Nn + GW_KS * sp.Ndes, D + a0 * sp.Ndes, bq, rfull + rs);
+        bulk_g2s(rb + 2 * GW_KS * (sp.Nn + sp.Ndes), eat + a0, be, rfull + rs);
+      }
+    }
+  } else if (warp == GW_PROD / 32) {
     // ================= MMA issuer (one thread) =================
     if ((tid & 31) == 0) {
       const uint32_t idW = idesc_tf32(128, NB, 0, 0), id1 = idesc_tf32(128, 16, 0, 0);
       const uint32_t ones_a = smem_u32(ones);
       for (int it = 0; it < nst; ++it) {
-        const int st = it % nstage, use = it / nstage, g = it / GW_FLUSH, gi = it - g * GW_FLUSH;
+        const int st = it % GW_OPST, use = it / GW_OPST, g = it / GW_FLUSH, gi = it - g * GW_FLUSH;
         if (!mbar_wait(full + st, (uint32_t)(use & 1))) __trap();
         fence_after_sync();
         const uint32_t ts = tb + (uint32_t)((g & 1) * setc);
@@ -508,7 +559,7 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, int nstage, const float *__restrict__ thet
     };
     // The work items of a stage are the same in every stage: (atom group ag, column) of the A-side (x, p -> A, Bc, V)
     // followed by the B-side (q, D -> G, sD).  Each thread decodes its (up to GW_MAXI) items once.
-    int g_off[GW_MAXI], s_off[GW_MAXI], i_ag[GW_MAXI], i_kind[GW_MAXI];   // kind: 0 none, 1 A-side, 2 B-side
+    int r_off[GW_MAXI], s_off[GW_MAXI], i_ag[GW_MAXI], i_kind[GW_MAXI];   // kind: 0 none, 1 A-side, 2 B-side, 3 A-side + sum e
     float i_cf[GW_MAXI];
 #pragma unroll
     for (int j = 0; j < GW_MAXI; ++j) {
@@ -517,32 +568,22 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, int nstage, const float *__restrict__ thet
       const int wl = w < nA ? w : w - nA, W = w < nA ? sp.Nn : sp.Ndes;
       const int ag = i_kind[j] ? wl / W : 0, col = i_kind[j] ? wl - ag * W : 0;
       i_ag[j] = 4 * ag;
-      g_off[j] = 4 * ag * W + col;
+      r_off[j] = (i_kind[j] == 1 ? 0 : 2 * GW_KS * sp.Nn) + 4 * ag * W + col;
       s_off[j] = i_kind[j] == 1 ? (ag * 128 + col) * 4 : 6 * tileA + (ag * NB + col) * 4;
       i_cf[j] = i_kind[j] == 1 ? w1g[col] : (i_kind[j] == 2 ? qscale[col] : 0.f);
-      if (i_kind[j] == 1 && col == 0) i_kind[j] = 3;   // this item also sums the energy seeds (dL/db1)
+      if (i_kind[j] == 1 && col == 0) i_kind[j] = 3;
     }
+    const int e_off = 2 * GW_KS * (sp.Nn + sp.Ndes);
     for (int it = 0; it < nst; ++it) {
-      const int st = it % nstage, use = it / nstage, g = it / GW_FLUSH, gi = it - g * GW_FLUSH;
+      const int st = it % GW_OPST, use = it / GW_OPST, g = it / GW_FLUSH, gi = it - g * GW_FLUSH;
+      const int rs = it % nraw, ruse = it / nraw;
       float *sb = smem + st * stage_fl;
+      const float *rb = raw + rs * raw_fl;
       if (gi == 0 && g >= 1) flush(g - 1);
-      const int a0 = c0 + it * GW_KS;
-      const int nval = c1 - a0;                       // atoms of this stage inside the range (>= GW_KS except in the tail)
-      float raw[GW_MAXI][8], e4[GW_MAXI][4];
-#pragma unroll
-      for (int j = 0; j < GW_MAXI; ++j) {             // gather: all global loads of the stage in flight together
-        const bool isA = i_kind[j] & 1;
-        const int W = isA ? sp.Nn : sp.Ndes;
-        const float *r0 = (isA ? x : q) + (size_t)a0 * W + g_off[j];
-        const float *r1 = (isA ? p : D) + (size_t)a0 * W + g_off[j];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          const bool ok = i_kind[j] != 0 && i_ag[j] + i < nval;
-          raw[j][i] = ok ? r0[i * W] : 0.f;
-          raw[j][4 + i] = ok ? r1[i * W] : 0.f;
-          e4[j][i] = (ok && isA) ? eat[a0 + i_ag[j] + i] : 0.f;
-        }
-      }
+      const int a0 = w0 + it * GW_KS;
+      const int vlo = c0 - a0, vhi = c1 - a0;         // atoms [vlo, vhi) of the window belong to this CTA
+      const bool whole = vlo <= 0 && vhi >= GW_KS;
+      if (!mbar_wait(rfull + rs, (uint32_t)(ruse & 1))) __trap();
       if (use > 0 && !mbar_wait(empty + st, (uint32_t)((use - 1) & 1))) __trap();
 #pragma unroll
       for (int j = 0; j < GW_MAXI; ++j) {
@@ -551,31 +592,41 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, int nstage, const float *__restrict__ thet
         float *dst = sb + s_off[j];
         const float cf = i_cf[j];
         if (i_kind[j] & 1) {
+          const float *rx = rb + r_off[j], *rp = rx + GW_KS * sp.Nn;
+          const float4 e4 = *(const float4 *)(rb + e_off + i_ag[j]);
+          const float ee[4] = {e4.x, e4.y, e4.z, e4.w};
           float Av[4], Bv[4], Vv[4];
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
-            const float xv = raw[j][i], pv = raw[j][4 + i], ev = e4[j][i];
+            const bool ok = whole || (i_ag[j] + i >= vlo && i_ag[j] + i < vhi);
+            const float xv = rx[i * sp.Nn];
+            const float pv = ok ? rp[i * sp.Nn] : 0.f, ev = ok ? ee[i] : 0.f;
             const float d1 = 1.f - xv * xv, d2 = -2.f * xv * d1;
             Av[i] = cf * (ev * d1 + d2 * pv);
-            Bv[i] = i_ag[j] + i < nval ? cf * d1 : 0.f;   // atoms past the range: x = 0 would give Bc = w1
+            Bv[i] = ok ? cf * d1 : 0.f;
             Vv[i] = ev * xv + d1 * pv;
             if (i_kind[j] == 3) esum += ev;
           }
-          split4(make_float4(Av[0], Av[1], Av[2], Av[3]), hi, lo);
+          split4_fast(make_float4(Av[0], Av[1], Av[2], Av[3]), hi, lo);
           *(float4 *)(dst) = hi; *(float4 *)(dst + tileA) = lo;
-          split4(make_float4(Bv[0], Bv[1], Bv[2], Bv[3]), hi, lo);
+          split4_fast(make_float4(Bv[0], Bv[1], Bv[2], Bv[3]), hi, lo);
           *(float4 *)(dst + 2 * tileA) = hi; *(float4 *)(dst + 3 * tileA) = lo;
-          split4(make_float4(Vv[0], Vv[1], Vv[2], Vv[3]), hi, lo);
+          split4_fast(make_float4(Vv[0], Vv[1], Vv[2], Vv[3]), hi, lo);
           *(float4 *)(dst + 4 * tileA) = hi; *(float4 *)(dst + 5 * tileA) = lo;
         } else {
-          split4(make_float4(cf * raw[j][0], cf * raw[j][1], cf * raw[j][2], cf * raw[j][3]), hi, lo);
+          const float *rq = rb + r_off[j], *rD = rq + GW_KS * sp.Ndes;
+          float qv[4], dv[4];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) { qv[i] = cf * rq[i * sp.Ndes]; dv[i] = cf * rD[i * sp.Ndes]; }
+          split4_fast(make_float4(qv[0], qv[1], qv[2], qv[3]), hi, lo);
           *(float4 *)(dst) = hi; *(float4 *)(dst + tileB) = lo;
-          split4(make_float4(cf * raw[j][4], cf * raw[j][5], cf * raw[j][6], cf * raw[j][7]), hi, lo);
+          split4_fast(make_float4(dv[0], dv[1], dv[2], dv[3]), hi, lo);
           *(float4 *)(dst + 2 * tileB) = hi; *(float4 *)(dst + 3 * tileB) = lo;
         }
       }
       fence_async_smem();
       mbar_arrive(full + st);
+      mbar_arrive(rempty + rs);
     }
     if (ngroups > 0) flush(ngroups - 1);
     esh[tid] = esum;
