@@ -31,7 +31,7 @@ __device__ __forceinline__ int l_of_lm(int lm) { return lm < 3 ? 1 : lm < 8 ? 2 
 // ---------------------------------------------------------------------------------------------
 template <int KT>
 __device__ __forceinline__ void cheb_f(float d, float rcinv, float (&f)[KT]) {
-  float t = d * rcinv;
+  float t = fminf(d * rcinv, 1.f);            // real pairs have d < rc; the padding dummies of the angular list sit at 2 rc
   float x = t - 1.f;
   float xi = 2.f * x * x - 1.f;
   float hfc = 0.25f * (1.f + cospif(t));      // 1/2 f_c
@@ -48,7 +48,7 @@ __device__ __forceinline__ void cheb_f(float d, float rcinv, float (&f)[KT]) {
 
 template <int KT>
 __device__ __forceinline__ void cheb_ffp(float d, float rcinv, float (&f)[KT], float (&fp)[KT]) {
-  float t = d * rcinv;
+  float t = fminf(d * rcinv, 1.f);            // (see cheb_f) at t = 1: f_k = f_k' = 0 exactly
   float x = t - 1.f;
   float xi = 2.f * x * x - 1.f;
   float dxi = 4.f * x * rcinv;

@@ -41,7 +41,7 @@ struct gnep_handle {
   // batch
   bool loaded = false;
   int N = 0, S = 0;
-  int64_t nR = 0, nA = 0;
+  int64_t nR = 0, nA = 0, nAp = 0;   // nAp: angular pairs including the padding dummies
   int hasE = 0, hasF = 0, hasV = 0;
   double Ng = -1, Sg = -1, l2_share = 1.0;   // job-wide normalisers when structures are sharded over ranks
   std::vector<void *> batch_allocs;
@@ -604,17 +604,21 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     // ---- persistent batch arrays ----
     int rc_;
 #define BA(ptr, n) if ((rc_ = dalloc(h, &(ptr), (n), true)) != GNEP_OK) { tfree(); free_batch(h); return rc_; }
-    BA(h->perm, N); BA(h->type_s, N); BA(h->struct_s, N); BA(h->segR, (size_t)N * (T + 1) + 1); BA(h->rowAs, N + 1); BA(h->revA, nA); BA(h->segA, (size_t)N * (T + 1) + 1); BA(h->atomA, nA);
-    BA(h->pairR, nR); BA(h->pairA, nA);
+    BA(h->perm, N); BA(h->type_s, N); BA(h->struct_s, N); BA(h->segR, (size_t)N * (T + 1) + 1); BA(h->rowAs, N + 1); BA(h->segA, (size_t)N * (T + 1) + 1);
+    BA(h->pairR, nR);
     BA(h->exp_row[0], N + 1); BA(h->exp_row[1], N + 1); BA(h->exp_j[0], nR); BA(h->exp_sh[0], nR); BA(h->exp_j[1], nA); BA(h->exp_sh[1], nA);
     BA(h->srange, srange.size()); BA(h->Eref, S); BA(h->Wref, (size_t)S * 6); BA(h->Fref_s, (size_t)N * 3);
-    int *d_rowRs, *d_shA; unsigned long long *d_ekey; float *d_er;
+    // the angular list is first built unpadded (u) and then copied into its final layout, in which every (atom, J)
+    // segment is padded to a multiple of 4 pairs with zero-contribution dummies (k_pad_angular)
+    int *d_rowRs, *d_shA, *d_rowAu, *d_segAu, *d_atomAu; unsigned long long *d_ekey; float *d_er; float4 *d_pairAu;
     CKT(talloc((void **)&d_rowRs, sizeof(int) * (N + 1))); CKT(talloc((void **)&d_shA, sizeof(int) * nA));
+    CKT(talloc((void **)&d_rowAu, sizeof(int) * (N + 1))); CKT(talloc((void **)&d_segAu, sizeof(int) * ((size_t)N * (T + 1) + 1)));
+    CKT(talloc((void **)&d_atomAu, sizeof(int) * nA)); CKT(talloc((void **)&d_pairAu, sizeof(float4) * nA));
     CKT(talloc((void **)&d_ekey, sizeof(unsigned long long) * nR)); CKT(talloc((void **)&d_er, sizeof(float) * 3 * nR));
     CKT(cudaMemcpyAsync(h->exp_row[0], rowR.data(), sizeof(int64_t) * (N + 1), cudaMemcpyHostToDevice, st));
     CKT(cudaMemcpyAsync(h->exp_row[1], rowA.data(), sizeof(int64_t) * (N + 1), cudaMemcpyHostToDevice, st));
     CKT(cudaMemcpyAsync(d_rowRs, rowRs.data(), sizeof(int) * (N + 1), cudaMemcpyHostToDevice, st));
-    CKT(cudaMemcpyAsync(h->rowAs, rowAs.data(), sizeof(int) * (N + 1), cudaMemcpyHostToDevice, st));
+    CKT(cudaMemcpyAsync(d_rowAu, rowAs.data(), sizeof(int) * (N + 1), cudaMemcpyHostToDevice, st));
     if (N) {
       CKT(cudaMemcpyAsync(h->perm, perm.data(), sizeof(int) * N, cudaMemcpyHostToDevice, st));
       CKT(cudaMemcpyAsync(h->type_s, type_s.data(), sizeof(int) * N, cudaMemcpyHostToDevice, st));
@@ -623,8 +627,31 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     CKT(cudaMemcpyAsync(h->srange, srange.data(), sizeof(int) * srange.size(), cudaMemcpyHostToDevice, st));
     LAUNCH(h, k_nbr_fill, gN, 128, 0, N, d_struct_of, d_geo, d_wpos, d_binid, d_bin_start, d_bin_atoms, rcR2, rcA2, h->exp_row[0], d_ekey, d_er);
     LAUNCH(h, k_nbr_scatter, cdiv((int64_t)N * 32, 256), 256, 0, N, T, d_struct_of, d_geo, d_type, d_inv, h->exp_row[0], h->exp_row[1], d_rowRs,
-           h->rowAs, d_ekey, d_er, h->exp_j[0], h->exp_sh[0], h->exp_j[1], h->exp_sh[1], h->pairR, h->pairA, d_shA, h->segR, h->segA, h->atomA);
-    LAUNCH(h, k_nbr_reverse, cdiv((int64_t)N * 32, 256), 256, 0, N, h->rowAs, h->pairA, d_shA, h->revA);
+           d_rowAu, d_ekey, d_er, h->exp_j[0], h->exp_sh[0], h->exp_j[1], h->exp_sh[1], h->pairR, d_pairAu, d_shA, h->segR, d_segAu, d_atomAu);
+    CKT(cudaGetLastError());
+    std::vector<int> segAu((size_t)N * (T + 1) + 1, 0), segAp((size_t)N * (T + 1) + 1, 0);
+    if (N) CKT(cudaMemcpyAsync(segAu.data(), d_segAu, sizeof(int) * (size_t)N * (T + 1), cudaMemcpyDeviceToHost, st));
+    CKT(cudaStreamSynchronize(st));
+    int64_t nAp = 0;
+    for (int a = 0; a < N; ++a) {
+      for (int J = 0; J < T; ++J) {
+        segAp[(size_t)a * (T + 1) + J] = (int)nAp;
+        nAp += (segAu[(size_t)a * (T + 1) + J + 1] - segAu[(size_t)a * (T + 1) + J] + 3) / 4 * 4;
+      }
+      segAp[(size_t)a * (T + 1) + T] = (int)nAp;
+      rowAs[a] = segAp[(size_t)a * (T + 1)];
+    }
+    rowAs[N] = (int)nAp;
+    if (nAp >= (int64_t)1 << 31) { tfree(); free_batch(h); return fail(h, GNEP_ERANGE, "2^31 or more (padded) angular pairs"); }
+    h->nAp = nAp;
+    int *d_shAp;
+    CKT(talloc((void **)&d_shAp, sizeof(int) * nAp));
+    BA(h->revA, nAp); BA(h->atomA, nAp); BA(h->pairA, nAp);
+    CKT(cudaMemcpyAsync(h->rowAs, rowAs.data(), sizeof(int) * (N + 1), cudaMemcpyHostToDevice, st));
+    CKT(cudaMemcpyAsync(h->segA, segAp.data(), sizeof(int) * ((size_t)N * (T + 1) + 1), cudaMemcpyHostToDevice, st));
+    LAUNCH(h, k_pad_angular, cdiv((int64_t)N * 32, 256), 256, 0, N, T, d_segAu, h->segA, d_pairAu, d_shA, h->pairA, d_shAp, h->atomA,
+           (float)(2.0 * h->spec.rc_angular));
+    LAUNCH(h, k_nbr_reverse, cdiv((int64_t)N * 32, 256), 256, 0, N, h->rowAs, h->pairA, d_shAp, h->revA);
     CKT(cudaGetLastError());
     CKT(cudaStreamSynchronize(st));
     tfree();
@@ -661,7 +688,7 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     BA(h->q, npad * d.Ndes); BA(h->Sn, n * d.NA * GNEP_NLM); BA(h->x, npad * d.Nn); BA(h->Ei, n); BA(h->Ep, n * d.Ndes);
     BA(h->etil, n * T * d.KRp); BA(h->M1, n * T * d.KRp); BA(h->M2, n * T * d.KRp); BA(h->D, npad * d.Ndes); BA(h->Tn, n * d.NA * GNEP_NLM); BA(h->A1, n * T * d.KAp * GNEP_NLM); BA(h->A2, n * T * d.KAp * GNEP_NLM);
     BA(h->gbar, n * d.Ndes); BA(h->pbuf, npad * d.Nn); BA(h->eat, npad); BA(h->Wat, n * 6);
-    BA(h->Fat, n); BA(h->fpair, nA); BA(h->u, n);
+    BA(h->Fat, n); BA(h->fpair, h->nAp); BA(h->u, n);
     BA(h->Es, S); BA(h->Ws, (size_t)S * 6); BA(h->parts, (size_t)S * 3); BA(h->e_s, S); BA(h->omega, (size_t)S * 6);
     BA(h->partialCR, (size_t)std::max(h->n_chunks, 1) * d.NR * T * d.KRp);
     BA(h->partialCA, (size_t)std::max(h->rm.n_warps_ca, 1) * T * T * d.NA * d.KAp);
