@@ -126,7 +126,7 @@ void free_batch(gnep_handle *h) {
 }
 
 // ---- dynamic shared memory sizes (bytes) --------------------------------------------------------
-size_t smem_radial(const DevSpec &d) { return sizeof(float) * (d.T * d.T * d.NR * d.KRp + GNEP_WARPS * (d.KRp * 33 + d.KRp)); }
+size_t smem_radial(const DevSpec &d) { return sizeof(float) * (d.T * d.T * d.NR * d.KRp); }
 size_t smem_ang_fwd(const DevSpec &d) {
   return sizeof(float) * (d.T * d.T * d.KAp * ANG_NQ + ANG_WARPS * ((d.KAp + GNEP_NLM) * ANG_LD + d.T * d.KAp * GNEP_NLM));
 }
@@ -206,7 +206,7 @@ inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 int enqueue_descriptors(gnep_handle *h) {
   const DevSpec &d = h->ds;
   int gridA = cdiv(h->N, GNEP_WARPS);
-  DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_fwd<KT>, gridA, GNEP_WARPS * 32, smem_radial(d), d, h->N, h->type_s, h->segR, h->pairR, h->theta, h->q, h->M1));
+  DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_fwd<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, smem_radial(d), d, h->N, h->type_s, h->segR, h->pairR, h->theta, h->q, h->M1));
   mark(h, "a1_radial_descriptor");
   DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_fwd<KT>, cdiv(h->N, ANG_WARPS * ANG_TA), ANG_WARPS * 32, smem_ang_fwd(d), d, h->N, h->type_s, h->segA, h->pairA, h->theta, h->q, h->Sn, h->A1));
   mark(h, "a1_angular_descriptor");
@@ -229,7 +229,7 @@ int enqueue_forward(gnep_handle *h) {
   LAUNCH(h, k_net_tc<false>, h->n_cta_net, 256, smem_net_fwd(d), d, h->sm, h->theta, h->qscale, h->q, h->x, h->Ei, h->Ep, h->etil,
          (const int *)nullptr, (const float *)nullptr, (const float *)nullptr, (float *)nullptr, (float *)nullptr);
   mark(h, "a2_network_forward");
-  DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_force<KT>, gridA, GNEP_WARPS * 32, 0, d, h->N, h->type_s, h->segR, h->pairR, h->etil, h->Fat, h->Wat));
+  DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_force<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, 0, d, h->N, h->type_s, h->segR, h->pairR, h->etil, h->Fat, h->Wat));
   mark(h, "a3_radial_force");
   DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_force<KT>, cdiv(h->N, ANG_WARPS * FRC_TA), ANG_WARPS * 32, smem_ang_force(d), d, h->N, h->type_s, h->segA, h->atomA, h->pairA, h->theta, h->Ep, h->Sn, h->fpair));
   mark(h, "a3_angular_force");
@@ -245,7 +245,7 @@ int enqueue_forward(gnep_handle *h) {
 int enqueue_backward(gnep_handle *h) {
   const DevSpec &d = h->ds;
   int gridA = cdiv(h->N, GNEP_WARPS);
-  DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_adj<KT>, gridA, GNEP_WARPS * 32, smem_radial(d), d, h->N, h->type_s, h->struct_s, h->segR, h->pairR, h->theta, h->u, h->omega, h->scales, h->D, h->M2));
+  DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_adj<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, smem_radial(d), d, h->N, h->type_s, h->struct_s, h->segR, h->pairR, h->theta, h->u, h->omega, h->scales, h->D, h->M2));
   mark(h, "a5_radial_adjoint");
   DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_adj<KT>, cdiv(h->N, ANG_WARPS * ANG_TA), ANG_WARPS * 32, smem_ang_adj(d), d, h->N, h->type_s, h->struct_s, h->segA, h->atomA, h->pairA, h->theta, h->u, h->omega, h->scales, h->Sn, h->Tn, h->A2, h->D));
   mark(h, "a5_angular_adjoint");

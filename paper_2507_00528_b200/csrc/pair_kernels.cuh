@@ -1,7 +1,11 @@
 // pair_kernels.cuh -- radial sweeps over the neighbour list (rows a1, a3, a5) and helpers shared with angular_kernels.cuh.
-// One warp per atom.  Atoms are sorted by species (index "a"); pair records are
-// float4(r_ij.x, r_ij.y, r_ij.z, bits(a_j)).  Radial rows are split in species segments segR[a][J..J+1]
-// so that the neighbour species is warp-uniform; angular rows are processed in chunks of 32 pairs.
+// Atoms are sorted by species (index "a"); pair records are float4(r_ij.x, r_ij.y, r_ij.z, bits(a_j)); a radial row is
+// ordered by neighbour species, segR[a][J..J+1] bounding the species segments.
+// Mapping: ONE THREAD PER ATOM.  Everything a radial sweep produces is a per-atom sum over the row (moments M1/M2, F_i,
+// W_i), so a thread that walks its own row needs no cross-lane reduction at all, every lane is busy (rows of
+// neighbouring atoms have nearly equal lengths) and the per-pair work is the ~70-110 instructions of the basis
+// functions.  The 16-byte pair loads of a warp touch 32 different rows: each 32-byte sector is fetched once and its
+// second half is an L1 hit in the next iteration.
 #pragma once
 #include "common.cuh"
 
@@ -10,51 +14,98 @@ __device__ __forceinline__ float *warp_smem(float *base, int per_warp_floats) {
   return base + (threadIdx.x >> 5) * per_warp_floats;
 }
 
+#define RAD_THREADS 128
+
+template <int KT>
+__device__ __forceinline__ void store_row(float *__restrict__ dst, const float (&v)[KT]) {
+  if (KT % 4 == 0) {
+#pragma unroll
+    for (int k = 0; k < KT; k += 4) *(float4 *)(dst + k) = make_float4(v[k], v[k + 1], v[k + 2], v[k + 3]);
+  } else {
+#pragma unroll
+    for (int k = 0; k < KT; k += 2) *(float2 *)(dst + k) = make_float2(v[k], v[k + 1]);
+  }
+}
+template <int KT>
+__device__ __forceinline__ void load_row(const float *__restrict__ src, float (&v)[KT]) {
+  if (KT % 4 == 0) {
+#pragma unroll
+    for (int k = 0; k < KT; k += 4) { float4 t = *(const float4 *)(src + k); v[k] = t.x; v[k + 1] = t.y; v[k + 2] = t.z; v[k + 3] = t.w; }
+  } else {
+#pragma unroll
+    for (int k = 0; k < KT; k += 2) { float2 t = *(const float2 *)(src + k); v[k] = t.x; v[k + 1] = t.y; }
+  }
+}
+// out_n = sum_{J,k} cs[I][J][n][k] M[J][k] for n < NR, written to out[n] (row of q or D); M is the atom's moment row
+template <int KT>
+__device__ __forceinline__ void radial_contract(const DevSpec &sp, const float *cs, int I, const float *__restrict__ Mrow,
+                                                float *__restrict__ out) {
+  float o[16];
+#pragma unroll
+  for (int n = 0; n < 16; ++n) o[n] = 0.f;
+  for (int J = 0; J < sp.T; ++J) {
+    float m[KT];
+    load_row<KT>(Mrow + J * KT, m);
+    const float *c = cs + (size_t)(I * sp.T + J) * sp.NR * KT;
+#pragma unroll
+    for (int n = 0; n < 16; ++n)
+      if (n < sp.NR) {
+        float cv[KT];
+        load_row<KT>(c + n * KT, cv);
+#pragma unroll
+        for (int k = 0; k < KT; ++k) o[n] += cv[k] * m[k];
+      }
+  }
+#pragma unroll
+  for (int n = 0; n < 16; ++n)
+    if (n < sp.NR) out[n] = o[n];
+}
+
 // ------------------------------------------------------------------------------------------------
 // a1 (radial):  M1[a][J][k] = sum_{j in seg J} f_k(d_ij)  ;  q_n = sum_{J,k} cR[I][J][n][k] M1[J][k]
 // (paper Eq.5-6, in moment-factored form: g_n is linear in f_k)
 // ------------------------------------------------------------------------------------------------
 template <int KT>
-__global__ void __launch_bounds__(GNEP_WARPS * 32)
+__global__ void __launch_bounds__(RAD_THREADS)
 k_radial_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ segR,
              const float4 *__restrict__ pairR, const float *__restrict__ theta, float *__restrict__ q,
              float *__restrict__ M1) {
   extern __shared__ __align__(128) float smem[];
   float *cs = smem;                                          // [T*T*NR][KT]
-  int ncs = sp.T * sp.T * sp.NR * KT;
-  float *wbuf = warp_smem(smem + ncs, KT * 33 + KT);          // reduce buffer + moment row
-  float *mrow = wbuf + KT * 33;
   stage_coeff(cs, theta, sp.T * sp.T * sp.NR, sp.KR, KT);
   __syncthreads();
-  int lane = threadIdx.x & 31;
-  int a = blockIdx.x * GNEP_WARPS + (threadIdx.x >> 5);
+  const int a = blockIdx.x * RAD_THREADS + threadIdx.x;
   if (a >= N) return;
-  int I = type_s[a];
-  float qn = 0.f;
-  for (int J = 0; J < sp.T; ++J) {
-    int p0 = segR[a * (sp.T + 1) + J], p1 = segR[a * (sp.T + 1) + J + 1];
-    float acc[KT];
+  const int *sg = segR + (size_t)a * (sp.T + 1);
+  int p = sg[0], J = 0, jend = sg[1];
+  const int pend = sg[sp.T];
+  float *Mrow = M1 + (size_t)a * sp.T * KT;
+  float acc[KT];
+#pragma unroll
+  for (int k = 0; k < KT; ++k) acc[k] = 0.f;
+  float4 rn = p < pend ? pairR[p] : make_float4(1.f, 0.f, 0.f, 0.f);
+  while (p < pend) {
+    const float4 r = rn;
+    if (p + 1 < pend) rn = pairR[p + 1];
+    while (p >= jend) {                                      // species segment J complete
+      store_row<KT>(Mrow + J * KT, acc);
+#pragma unroll
+      for (int k = 0; k < KT; ++k) acc[k] = 0.f;
+      ++J; jend = sg[J + 1];
+    }
+    const float d = sqrtf(r.x * r.x + r.y * r.y + r.z * r.z);
+    float f[KT];
+    cheb_f<KT>(d, sp.rcRinv, f);
+#pragma unroll
+    for (int k = 0; k < KT; ++k) acc[k] += f[k];
+    ++p;
+  }
+  for (; J < sp.T; ++J) {
+    store_row<KT>(Mrow + J * KT, acc);
 #pragma unroll
     for (int k = 0; k < KT; ++k) acc[k] = 0.f;
-    for (int p = p0 + lane; p < p1; p += 32) {
-      float4 r = pairR[p];
-      float d = sqrtf(r.x * r.x + r.y * r.y + r.z * r.z);
-      float f[KT];
-      cheb_f<KT>(d, sp.rcRinv, f);
-#pragma unroll
-      for (int k = 0; k < KT; ++k) acc[k] += f[k];
-    }
-    float s = warp_transpose_reduce<KT>(acc, wbuf, lane);
-    if (lane < KT) { M1[(size_t)a * sp.T * KT + J * KT + lane] = s; mrow[lane] = s; }
-    __syncwarp();
-    if (lane < sp.NR) {
-      const float *c = cs + ((I * sp.T + J) * sp.NR + lane) * KT;
-#pragma unroll
-      for (int k = 0; k < KT; ++k) qn += c[k] * mrow[k];
-    }
-    __syncwarp();
   }
-  if (lane < sp.NR) q[(size_t)a * sp.Ndes + lane] = qn;
+  radial_contract<KT>(sp, cs, type_s[a], Mrow, q + (size_t)a * sp.Ndes);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -63,60 +114,45 @@ k_radial_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__res
 // etil_i[J][k] = sum_n E'_in cR[I][J][n][k] is produced by the network forward kernel.
 // ------------------------------------------------------------------------------------------------
 template <int KT>
-__global__ void __launch_bounds__(GNEP_WARPS * 32)
+__global__ void __launch_bounds__(RAD_THREADS)
 k_radial_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ segR,
                const float4 *__restrict__ pairR, const float *__restrict__ etil, float4 *__restrict__ Fat,
                float *__restrict__ Wat) {
-  int lane = threadIdx.x & 31;
-  int a = blockIdx.x * GNEP_WARPS + (threadIdx.x >> 5);
+  const int a = blockIdx.x * RAD_THREADS + threadIdx.x;
   if (a >= N) return;
-  int I = type_s[a];
-  float F[3] = {0.f, 0.f, 0.f}, W[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  const int I = type_s[a];
   const int TK = sp.T * KT;
-  for (int J = 0; J < sp.T; ++J) {
-    int p0 = segR[a * (sp.T + 1) + J], p1 = segR[a * (sp.T + 1) + J + 1];
-    float ei[KT];
+  const int *sg = segR + (size_t)a * (sp.T + 1);
+  int p = sg[0], J = 0, jend = sg[1];
+  const int pend = sg[sp.T];
+  float F[3] = {0.f, 0.f, 0.f}, W[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  float ei[KT];
+  load_row<KT>(etil + (size_t)a * TK, ei);
+  float4 rn = p < pend ? pairR[p] : make_float4(1.f, 0.f, 0.f, 0.f);
+  while (p < pend) {
+    const float4 r = rn;
+    if (p + 1 < pend) rn = pairR[p + 1];
+    while (p >= jend) { ++J; jend = sg[J + 1]; load_row<KT>(etil + (size_t)a * TK + J * KT, ei); }
+    float ejv[KT];
+    load_row<KT>(etil + (size_t)__float_as_int(r.w) * TK + I * KT, ejv);
+    const float d = sqrtf(r.x * r.x + r.y * r.y + r.z * r.z);
+    const float rinv = 1.f / d;
+    float f[KT], fp[KT];
+    cheb_ffp<KT>(d, sp.rcRinv, f, fp);
+    float si = 0.f, sj = 0.f;
 #pragma unroll
-    for (int k = 0; k < KT; ++k) ei[k] = __ldg(etil + (size_t)a * TK + J * KT + k);
-    for (int p = p0 + lane; p < p1; p += 32) {
-      float4 r = pairR[p];
-      int j = __float_as_int(r.w);
-      float d = sqrtf(r.x * r.x + r.y * r.y + r.z * r.z);
-      float rinv = 1.f / d;
-      float f[KT], fp[KT];
-      cheb_ffp<KT>(d, sp.rcRinv, f, fp);
-      const float *ej = etil + (size_t)j * TK + I * KT;
-      float ejv[KT];
-      if (KT % 4 == 0) {
-#pragma unroll
-        for (int k = 0; k < KT / 4; ++k) {
-          float4 v = __ldg((const float4 *)ej + k);
-          ejv[4 * k] = v.x; ejv[4 * k + 1] = v.y; ejv[4 * k + 2] = v.z; ejv[4 * k + 3] = v.w;
-        }
-      } else {
-#pragma unroll
-        for (int k = 0; k < KT / 2; ++k) { float2 v = __ldg((const float2 *)ej + k); ejv[2 * k] = v.x; ejv[2 * k + 1] = v.y; }
-      }
-      float si = 0.f, sj = 0.f;
-#pragma unroll
-      for (int k = 0; k < KT; ++k) { si += ei[k] * fp[k]; sj += ejv[k] * fp[k]; }
-      float hx = r.x * rinv, hy = r.y * rinv, hz = r.z * rinv;
-      float tot = si + sj;
-      F[0] += tot * hx; F[1] += tot * hy; F[2] += tot * hz;
-      float fx = si * hx, fy = si * hy, fz = si * hz;
-      W[0] -= r.x * fx; W[1] -= r.y * fy; W[2] -= r.z * fz;
-      W[3] -= r.x * fy; W[4] -= r.y * fz; W[5] -= r.z * fx;
-    }
+    for (int k = 0; k < KT; ++k) { si += ei[k] * fp[k]; sj += ejv[k] * fp[k]; }
+    const float hx = r.x * rinv, hy = r.y * rinv, hz = r.z * rinv;
+    const float tot = si + sj;
+    F[0] += tot * hx; F[1] += tot * hy; F[2] += tot * hz;
+    const float fx = si * hx, fy = si * hy, fz = si * hz;
+    W[0] -= r.x * fx; W[1] -= r.y * fy; W[2] -= r.z * fz;
+    W[3] -= r.x * fy; W[4] -= r.y * fz; W[5] -= r.z * fx;
+    ++p;
   }
+  Fat[a] = make_float4(F[0], F[1], F[2], 0.f);
 #pragma unroll
-  for (int c = 0; c < 3; ++c) F[c] = warp_sum(F[c]);
-#pragma unroll
-  for (int c = 0; c < 6; ++c) W[c] = warp_sum(W[c]);
-  if (lane == 0) {
-    Fat[a] = make_float4(F[0], F[1], F[2], 0.f);
-#pragma unroll
-    for (int c = 0; c < 6; ++c) Wat[(size_t)a * 6 + c] = W[c];
-  }
+  for (int c = 0; c < 6; c += 2) *(float2 *)(Wat + (size_t)a * 6 + c) = make_float2(W[c], W[c + 1]);
 }
 
 // pair adjoint a_ij = dL/df_ij = sf (u_i - u_j) - sv omega_s . r_ij   (DESIGN.md section 3 step 2)
@@ -143,51 +179,51 @@ __device__ __forceinline__ void pair_adjoint(const AdjCtx &c, const float4 &uj, 
 // a5 (radial): M2[a][J][k] = sum_j f_k'(d_ij) (a_ij . rhat_ij) ;  D_n = sum_{J,k} cR[I][J][n][k] M2[J][k]
 // ------------------------------------------------------------------------------------------------
 template <int KT>
-__global__ void __launch_bounds__(GNEP_WARPS * 32)
+__global__ void __launch_bounds__(RAD_THREADS)
 k_radial_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ struct_s,
              const int *__restrict__ segR, const float4 *__restrict__ pairR, const float *__restrict__ theta,
              const float4 *__restrict__ u, const float *__restrict__ omega, const float *__restrict__ scales,
              float *__restrict__ D, float *__restrict__ M2) {
   extern __shared__ __align__(128) float smem[];
   float *cs = smem;
-  int ncs = sp.T * sp.T * sp.NR * KT;
-  float *wbuf = warp_smem(smem + ncs, KT * 33 + KT);
-  float *mrow = wbuf + KT * 33;
   stage_coeff(cs, theta, sp.T * sp.T * sp.NR, sp.KR, KT);
   __syncthreads();
-  int lane = threadIdx.x & 31;
-  int a = blockIdx.x * GNEP_WARPS + (threadIdx.x >> 5);
+  const int a = blockIdx.x * RAD_THREADS + threadIdx.x;
   if (a >= N) return;
-  int I = type_s[a];
-  AdjCtx ac = make_adj(u, omega, scales, a, struct_s[a]);
-  float Dn = 0.f;
-  for (int J = 0; J < sp.T; ++J) {
-    int p0 = segR[a * (sp.T + 1) + J], p1 = segR[a * (sp.T + 1) + J + 1];
-    float acc[KT];
+  const AdjCtx ac = make_adj(u, omega, scales, a, struct_s[a]);
+  const int *sg = segR + (size_t)a * (sp.T + 1);
+  int p = sg[0], J = 0, jend = sg[1];
+  const int pend = sg[sp.T];
+  float *Mrow = M2 + (size_t)a * sp.T * KT;
+  float acc[KT];
+#pragma unroll
+  for (int k = 0; k < KT; ++k) acc[k] = 0.f;
+  float4 rn = p < pend ? pairR[p] : make_float4(1.f, 0.f, 0.f, 0.f);
+  while (p < pend) {
+    const float4 r = rn;
+    if (p + 1 < pend) rn = pairR[p + 1];
+    while (p >= jend) {
+      store_row<KT>(Mrow + J * KT, acc);
+#pragma unroll
+      for (int k = 0; k < KT; ++k) acc[k] = 0.f;
+      ++J; jend = sg[J + 1];
+    }
+    const float4 uj = u[__float_as_int(r.w)];
+    const float d = sqrtf(r.x * r.x + r.y * r.y + r.z * r.z);
+    const float rinv = 1.f / d;
+    float ax, ay, az;
+    pair_adjoint(ac, uj, r, ax, ay, az);
+    const float ar = (ax * r.x + ay * r.y + az * r.z) * rinv;
+    float f[KT], fp[KT];
+    cheb_ffp<KT>(d, sp.rcRinv, f, fp);
+#pragma unroll
+    for (int k = 0; k < KT; ++k) acc[k] += fp[k] * ar;
+    ++p;
+  }
+  for (; J < sp.T; ++J) {
+    store_row<KT>(Mrow + J * KT, acc);
 #pragma unroll
     for (int k = 0; k < KT; ++k) acc[k] = 0.f;
-    for (int p = p0 + lane; p < p1; p += 32) {
-      float4 r = pairR[p];
-      float4 uj = u[__float_as_int(r.w)];
-      float d = sqrtf(r.x * r.x + r.y * r.y + r.z * r.z);
-      float rinv = 1.f / d;
-      float ax, ay, az;
-      pair_adjoint(ac, uj, r, ax, ay, az);
-      float ar = (ax * r.x + ay * r.y + az * r.z) * rinv;
-      float f[KT], fp[KT];
-      cheb_ffp<KT>(d, sp.rcRinv, f, fp);
-#pragma unroll
-      for (int k = 0; k < KT; ++k) acc[k] += fp[k] * ar;
-    }
-    float s = warp_transpose_reduce<KT>(acc, wbuf, lane);
-    if (lane < KT) { M2[(size_t)a * sp.T * KT + J * KT + lane] = s; mrow[lane] = s; }
-    __syncwarp();
-    if (lane < sp.NR) {
-      const float *c = cs + ((I * sp.T + J) * sp.NR + lane) * KT;
-#pragma unroll
-      for (int k = 0; k < KT; ++k) Dn += c[k] * mrow[k];
-    }
-    __syncwarp();
   }
-  if (lane < sp.NR) D[(size_t)a * sp.Ndes + lane] = Dn;
+  radial_contract<KT>(sp, cs, type_s[a], Mrow, D + (size_t)a * sp.Ndes);
 }
