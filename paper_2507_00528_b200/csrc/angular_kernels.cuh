@@ -178,8 +178,8 @@ k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
     const int p = c0 + lane;
     if (p < P_hi) {
       float4 r = pairA[p];
-      float d = sqrtf(r.x * r.x + r.y * r.y + r.z * r.z);
-      float rinv = 1.f / d;
+      float d, rinv;
+      pair_len(r.x * r.x + r.y * r.y + r.z * r.z, d, rinv);
       float f[KT];
       cheb_f<KT>(d, sp.rcAinv, f);
 #pragma unroll
@@ -328,8 +328,8 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
       const int ai = atomA[p];
       const int s = struct_s[ai];
       float4 ui = u[ai], uj = u[__float_as_int(r.w)];
-      float d = sqrtf(r.x * r.x + r.y * r.y + r.z * r.z);
-      float rinv = 1.f / d;
+      float d, rinv;
+      pair_len(r.x * r.x + r.y * r.y + r.z * r.z, d, rinv);
       const float *om = omega + s * 6;
       float ax = sfF * (ui.x - uj.x) - svV * (om[0] * r.x + om[5] * r.z);
       float ay = sfF * (ui.y - uj.y) - svV * (om[1] * r.y + om[3] * r.x);
@@ -441,8 +441,8 @@ k_angular_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__
     const int a = atomA[p];
     const int I = type_s[a];
     const float *be = beta + (a - a_lo) * nb;
-    float d = sqrtf(r.x * r.x + r.y * r.y + r.z * r.z);
-    float rinv = 1.f / d;
+    float d, rinv;
+    pair_len(r.x * r.x + r.y * r.y + r.z * r.z, d, rinv);
     int J = type_s[__float_as_int(r.w)];
     float f[KT], fp[KT];
     cheb_ffp<KT>(d, sp.rcAinv, f, fp);

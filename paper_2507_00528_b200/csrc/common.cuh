@@ -27,46 +27,98 @@ __constant__ float c_kappa4;
 __device__ __forceinline__ int l_of_lm(int lm) { return lm < 3 ? 1 : lm < 8 ? 2 : lm < 15 ? 3 : 4; }
 
 // ---------------------------------------------------------------------------------------------
-// Chebyshev radial basis (paper Eq.6, App.A):  f_k = 1/2 (T_k(xi)+1) f_c,  xi = 2 (d/rc - 1)^2 - 1
+// Pair geometry: d = |r| and 1/d from one MUFU.RSQ and one Newton step (relative error ~1e-7, as sqrtf + division).
 // ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void pair_len(float d2, float &d, float &rinv) {
+  const float y = rsqrtf(d2);
+  const float e = fmaf(-d2 * y, y, 1.f);
+  rinv = fmaf(0.5f * y, e, y);
+  d = d2 * rinv;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Chebyshev radial basis (paper Eq.6, App.A):  f_k = 1/2 (T_k(xi)+1) f_c,  xi = 2 (d/rc - 1)^2 - 1,
+// f_c = 1/2 (1 + cos(pi d/rc)); d/rc is clamped at 1, where f_k = f_k' = 0 exactly
+// (real pairs have d < rc; the padding dummies of the angular list sit at 2 rc).
+// cheb_T / cheb_TD give the pieces, so that sums over pairs can be accumulated per Chebyshev term:
+//   f_0 = 2 hfc,  f_k = hfc T_k + hfc;   f_0' = 2 hfcp,  f_k' = D_k hdf + T_k hfcp + hfcp   (D_k = dT_k/dxi)
+// ---------------------------------------------------------------------------------------------
+#define GNEP_PI_F 3.14159265358979f
+// sin(pi t), cos(pi t) for t in [0, 1] from the Taylor polynomials about t = 1/2 (x = pi (t - 1/2), |x| <= pi/2):
+// cos(pi t) = -sin x, sin(pi t) = cos x; truncation 6e-8 / 7e-9 absolute, i.e. fp32 rounding level, in ~16 instructions
+// (sincospif spends about twice that on its general range reduction).
+__device__ __forceinline__ float cospi01(float t) {
+  const float x = GNEP_PI_F * (t - 0.5f), x2 = x * x;
+  float p = fmaf(x2, -2.5052108e-8f, 2.7557319e-6f);
+  p = fmaf(x2, p, -1.9841270e-4f);
+  p = fmaf(x2, p, 8.3333333e-3f);
+  p = fmaf(x2, p, -1.6666667e-1f);
+  return -fmaf(x * x2, p, x);
+}
+__device__ __forceinline__ void sincospi01(float t, float &sn, float &cs) {
+  const float x = GNEP_PI_F * (t - 0.5f), x2 = x * x;
+  float p = fmaf(x2, -2.5052108e-8f, 2.7557319e-6f);
+  p = fmaf(x2, p, -1.9841270e-4f);
+  p = fmaf(x2, p, 8.3333333e-3f);
+  p = fmaf(x2, p, -1.6666667e-1f);
+  cs = -fmaf(x * x2, p, x);
+  float c = fmaf(x2, 2.0876757e-9f, -2.7557319e-7f);
+  c = fmaf(x2, c, 2.4801587e-5f);
+  c = fmaf(x2, c, -1.3888889e-3f);
+  c = fmaf(x2, c, 4.1666667e-2f);
+  c = fmaf(x2, c, -0.5f);
+  sn = fmaf(x2, c, 1.f);
+}
 template <int KT>
-__device__ __forceinline__ void cheb_f(float d, float rcinv, float (&f)[KT]) {
-  float t = fminf(d * rcinv, 1.f);            // real pairs have d < rc; the padding dummies of the angular list sit at 2 rc
-  float x = t - 1.f;
-  float xi = 2.f * x * x - 1.f;
-  float hfc = 0.25f * (1.f + cospif(t));      // 1/2 f_c
-  float Tm2 = 1.f, Tm1 = xi;
-  f[0] = 2.f * hfc;
-  if (KT > 1) f[1] = hfc * (xi + 1.f);
+__device__ __forceinline__ void cheb_T(float d, float rcinv, float (&Tk)[KT], float &hfc) {
+  const float t = fminf(d * rcinv, 1.f);
+  const float x = t - 1.f;
+  const float xi = 2.f * x * x - 1.f;
+  hfc = t < 1.f ? 0.25f * (1.f + cospi01(t)) : 0.f;                 // 1/2 f_c
+  Tk[0] = 1.f;
+  if (KT > 1) Tk[1] = xi;
+#pragma unroll
+  for (int k = 2; k < KT; ++k) Tk[k] = 2.f * xi * Tk[k - 1] - Tk[k - 2];
+}
+template <int KT>
+__device__ __forceinline__ void cheb_TD(float d, float rcinv, float (&Tk)[KT], float (&Dk)[KT], float &hfc, float &hfcp,
+                                        float &hdf) {
+  const float t = fminf(d * rcinv, 1.f);
+  const float x = t - 1.f;
+  const float xi = 2.f * x * x - 1.f;
+  float sn, cs;
+  sincospi01(t, sn, cs);
+  const bool in = t < 1.f;
+  hfc = in ? 0.25f * (1.f + cs) : 0.f;                              // 1/2 f_c
+  hfcp = in ? -0.25f * GNEP_PI_F * rcinv * sn : 0.f;                // 1/2 f_c'
+  hdf = hfc * 4.f * x * rcinv;                                      // 1/2 f_c dxi/dd
+  Tk[0] = 1.f; Dk[0] = 0.f;
+  if (KT > 1) { Tk[1] = xi; Dk[1] = 1.f; }
 #pragma unroll
   for (int k = 2; k < KT; ++k) {
-    float Tk = 2.f * xi * Tm1 - Tm2;
-    f[k] = hfc * (Tk + 1.f);
-    Tm2 = Tm1; Tm1 = Tk;
+    Tk[k] = 2.f * xi * Tk[k - 1] - Tk[k - 2];
+    Dk[k] = 2.f * Tk[k - 1] + 2.f * xi * Dk[k - 1] - Dk[k - 2];
   }
 }
 
 template <int KT>
-__device__ __forceinline__ void cheb_ffp(float d, float rcinv, float (&f)[KT], float (&fp)[KT]) {
-  float t = fminf(d * rcinv, 1.f);            // (see cheb_f) at t = 1: f_k = f_k' = 0 exactly
-  float x = t - 1.f;
-  float xi = 2.f * x * x - 1.f;
-  float dxi = 4.f * x * rcinv;
-  float s, c;
-  sincospif(t, &s, &c);
-  float hfc = 0.25f * (1.f + c);                          // 1/2 f_c
-  float hfcp = -0.25f * 3.14159265358979f * rcinv * s;    // 1/2 f_c'
-  float hdf = hfc * dxi;                                  // 1/2 f_c dxi/dd
-  float Tm2 = 1.f, Tm1 = xi, Dm2 = 0.f, Dm1 = 1.f;
-  f[0] = 2.f * hfc;  fp[0] = 2.f * hfcp;
-  if (KT > 1) { f[1] = hfc * (xi + 1.f); fp[1] = hdf + (xi + 1.f) * hfcp; }
+__device__ __forceinline__ void cheb_f(float d, float rcinv, float (&f)[KT]) {
+  float Tk[KT], hfc;
+  cheb_T<KT>(d, rcinv, Tk, hfc);
+  f[0] = 2.f * hfc;
 #pragma unroll
-  for (int k = 2; k < KT; ++k) {
-    float Tk = 2.f * xi * Tm1 - Tm2;
-    float Dk = 2.f * Tm1 + 2.f * xi * Dm1 - Dm2;
-    f[k] = hfc * (Tk + 1.f);
-    fp[k] = Dk * hdf + (Tk + 1.f) * hfcp;
-    Tm2 = Tm1; Tm1 = Tk; Dm2 = Dm1; Dm1 = Dk;
+  for (int k = 1; k < KT; ++k) f[k] = fmaf(hfc, Tk[k], hfc);
+}
+
+template <int KT>
+__device__ __forceinline__ void cheb_ffp(float d, float rcinv, float (&f)[KT], float (&fp)[KT]) {
+  float Tk[KT], Dk[KT], hfc, hfcp, hdf;
+  cheb_TD<KT>(d, rcinv, Tk, Dk, hfc, hfcp, hdf);
+  f[0] = 2.f * hfc; fp[0] = 2.f * hfcp;
+#pragma unroll
+  for (int k = 1; k < KT; ++k) {
+    f[k] = fmaf(hfc, Tk[k], hfc);
+    fp[k] = fmaf(Dk[k], hdf, fmaf(Tk[k], hfcp, hfcp));
   }
 }
 

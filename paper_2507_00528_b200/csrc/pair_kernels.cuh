@@ -15,6 +15,43 @@ __device__ __forceinline__ float *warp_smem(float *base, int per_warp_floats) {
 }
 
 #define RAD_THREADS 128
+#define RAD_PF 4        // pairs per prefetch group: the loads of a group are issued one whole group ahead
+
+// Walk the row [p, pend) of one atom RAD_PF pairs at a time, the next group's records (64 contiguous bytes per lane)
+// already in flight; g = gather(r), the per-pair gather of neighbour data (e.g. u_j), is issued one pair ahead of its
+// use.  next_seg(J) is called whenever the walk leaves species segment J, body(r, g) for every pair.
+template <class Seg, class Gather, class Body>
+__device__ __forceinline__ void walk_row(const float4 *__restrict__ pairR, const int *__restrict__ sg, int T, Seg next_seg,
+                                         Gather gather, Body body) {
+  int p = sg[0], J = 0, jend = sg[1];
+  const int pend = sg[T];
+  const float4 dum = make_float4(1.f, 0.f, 0.f, 0.f);      // w = bits(0): a valid atom index for the gather
+  float4 nb[RAD_PF];
+#pragma unroll
+  for (int i = 0; i < RAD_PF; ++i) nb[i] = p + i < pend ? pairR[p + i] : dum;
+  auto gn = gather(nb[0]);
+  while (p < pend) {
+    float4 cb[RAD_PF];
+#pragma unroll
+    for (int i = 0; i < RAD_PF; ++i) cb[i] = nb[i];
+#pragma unroll
+    for (int i = 0; i < RAD_PF; ++i) nb[i] = p + RAD_PF + i < pend ? pairR[p + RAD_PF + i] : dum;
+#pragma unroll
+    for (int i = 0; i < RAD_PF; ++i) {
+      const auto gc = gn;
+      gn = gather(i + 1 < RAD_PF ? cb[i + 1 < RAD_PF ? i + 1 : 0] : nb[0]);
+      if (p + i < pend) {
+        while (p + i >= jend) { next_seg(J); ++J; jend = sg[J + 1]; }
+        body(cb[i], gc);
+      }
+    }
+    p += RAD_PF;
+  }
+  for (; J < T; ++J) next_seg(J);
+}
+
+template <int KT>
+struct RowRegs { float v[KT]; };
 
 template <int KT>
 __device__ __forceinline__ void store_row(float *__restrict__ dst, const float (&v)[KT]) {
@@ -77,40 +114,37 @@ k_radial_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__res
   const int a = blockIdx.x * RAD_THREADS + threadIdx.x;
   if (a >= N) return;
   const int *sg = segR + (size_t)a * (sp.T + 1);
-  int p = sg[0], J = 0, jend = sg[1];
-  const int pend = sg[sp.T];
   float *Mrow = M1 + (size_t)a * sp.T * KT;
+  // accumulated per Chebyshev term: acc[k] = sum hfc T_k (k >= 1), acc[0] = sum hfc;  f_0 = 2 hfc, f_k = hfc T_k + hfc
   float acc[KT];
 #pragma unroll
   for (int k = 0; k < KT; ++k) acc[k] = 0.f;
-  float4 rn = p < pend ? pairR[p] : make_float4(1.f, 0.f, 0.f, 0.f);
-  while (p < pend) {
-    const float4 r = rn;
-    if (p + 1 < pend) rn = pairR[p + 1];
-    while (p >= jend) {                                      // species segment J complete
-      store_row<KT>(Mrow + J * KT, acc);
+  walk_row(pairR, sg, sp.T,
+           [&](int J) {                                     // species segment J complete
+             float m[KT];
+             m[0] = 2.f * acc[0];
 #pragma unroll
-      for (int k = 0; k < KT; ++k) acc[k] = 0.f;
-      ++J; jend = sg[J + 1];
-    }
-    const float d = sqrtf(r.x * r.x + r.y * r.y + r.z * r.z);
-    float f[KT];
-    cheb_f<KT>(d, sp.rcRinv, f);
+             for (int k = 1; k < KT; ++k) m[k] = acc[k] + acc[0];
+             store_row<KT>(Mrow + J * KT, m);
 #pragma unroll
-    for (int k = 0; k < KT; ++k) acc[k] += f[k];
-    ++p;
-  }
-  for (; J < sp.T; ++J) {
-    store_row<KT>(Mrow + J * KT, acc);
+             for (int k = 0; k < KT; ++k) acc[k] = 0.f;
+           },
+           [](const float4 &) { return 0; },
+           [&](const float4 &r, int) {
+             float d, rinv, Tk[KT], hfc;
+             pair_len(r.x * r.x + r.y * r.y + r.z * r.z, d, rinv);
+             cheb_T<KT>(d, sp.rcRinv, Tk, hfc);
+             acc[0] += hfc;
 #pragma unroll
-    for (int k = 0; k < KT; ++k) acc[k] = 0.f;
-  }
+             for (int k = 1; k < KT; ++k) acc[k] = fmaf(hfc, Tk[k], acc[k]);
+           });
   radial_contract<KT>(sp, cs, type_s[a], Mrow, q + (size_t)a * sp.Ndes);
 }
 
 // ------------------------------------------------------------------------------------------------
 // a3 (radial): F_i += sum_j [ sum_k (etil_i[J][k] + etil_j[I][k]) f_k'(d) ] rhat_ij   (Eq.3 with C3.6),
-// per-atom virial  W_ab -= r_a f_ij,b  with f_ij = (sum_k etil_i[J][k] f_k') rhat   (Eq.4, R17).
+// virial W_ab -= r_a f_ij,b with f_ij = (sum_k etil_i[J][k] f_k') rhat (Eq.4, R17), booked per atom as half of the pair's
+// symmetric total (only the per-structure sum of W_i is ever used; see the kernel body).
 // etil_i[J][k] = sum_n E'_in cR[I][J][n][k] is produced by the network forward kernel.
 // ------------------------------------------------------------------------------------------------
 template <int KT>
@@ -123,33 +157,38 @@ k_radial_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__r
   const int I = type_s[a];
   const int TK = sp.T * KT;
   const int *sg = segR + (size_t)a * (sp.T + 1);
-  int p = sg[0], J = 0, jend = sg[1];
-  const int pend = sg[sp.T];
   float F[3] = {0.f, 0.f, 0.f}, W[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   float ei[KT];
   load_row<KT>(etil + (size_t)a * TK, ei);
-  float4 rn = p < pend ? pairR[p] : make_float4(1.f, 0.f, 0.f, 0.f);
-  while (p < pend) {
-    const float4 r = rn;
-    if (p + 1 < pend) rn = pairR[p + 1];
-    while (p >= jend) { ++J; jend = sg[J + 1]; load_row<KT>(etil + (size_t)a * TK + J * KT, ei); }
-    float ejv[KT];
-    load_row<KT>(etil + (size_t)__float_as_int(r.w) * TK + I * KT, ejv);
-    const float d = sqrtf(r.x * r.x + r.y * r.y + r.z * r.z);
-    const float rinv = 1.f / d;
-    float f[KT], fp[KT];
-    cheb_ffp<KT>(d, sp.rcRinv, f, fp);
-    float si = 0.f, sj = 0.f;
+  walk_row(pairR, sg, sp.T,
+           [&](int J) { if (J + 1 < sp.T) load_row<KT>(etil + (size_t)a * TK + (J + 1) * KT, ei); },
+           [&](const float4 &r) {
+             RowRegs<KT> g;
+             load_row<KT>(etil + (size_t)__float_as_int(r.w) * TK + I * KT, g.v);
+             return g;
+           },
+           [&](const float4 &r, const RowRegs<KT> &ej) {
+             float d, rinv, Tk[KT], Dk[KT], hfc, hfcp, hdf;
+             pair_len(r.x * r.x + r.y * r.y + r.z * r.z, d, rinv);
+             cheb_TD<KT>(d, sp.rcRinv, Tk, Dk, hfc, hfcp, hdf);
+             // tot = sum_k (etil_i[J][k] + etil_j[I][k]) f_k',  f_0' = 2 hfcp, f_k' = D_k hdf + (T_k + 1) hfcp
+             float sD = 0.f, sT = 2.f * (ei[0] + ej.v[0]);
 #pragma unroll
-    for (int k = 0; k < KT; ++k) { si += ei[k] * fp[k]; sj += ejv[k] * fp[k]; }
-    const float hx = r.x * rinv, hy = r.y * rinv, hz = r.z * rinv;
-    const float tot = si + sj;
-    F[0] += tot * hx; F[1] += tot * hy; F[2] += tot * hz;
-    const float fx = si * hx, fy = si * hy, fz = si * hz;
-    W[0] -= r.x * fx; W[1] -= r.y * fy; W[2] -= r.z * fz;
-    W[3] -= r.x * fy; W[4] -= r.y * fz; W[5] -= r.z * fx;
-    ++p;
-  }
+             for (int k = 1; k < KT; ++k) {
+               const float es = ei[k] + ej.v[k];
+               sD = fmaf(es, Dk[k], sD);
+               sT = fmaf(es, Tk[k] + 1.f, sT);
+             }
+             const float tot = sD * hdf + sT * hfcp;
+             const float hx = r.x * rinv, hy = r.y * rinv, hz = r.z * rinv;
+             F[0] += tot * hx; F[1] += tot * hy; F[2] += tot * hz;
+             // virial: sum_i W_i only enters per structure, and there sum_(i,j) r (x) rhat s_ij = 1/2 sum_(i,j) r (x) rhat
+             // (s_ij + s_ji) because (j,i) carries the same dyad -- so the atom books half of the pair's total
+             const float hf = 0.5f * tot;
+             const float fx = hf * hx, fy = hf * hy, fz = hf * hz;
+             W[0] -= r.x * fx; W[1] -= r.y * fy; W[2] -= r.z * fz;
+             W[3] -= r.x * fy; W[4] -= r.y * fz; W[5] -= r.z * fx;
+           });
   Fat[a] = make_float4(F[0], F[1], F[2], 0.f);
 #pragma unroll
   for (int c = 0; c < 6; c += 2) *(float2 *)(Wat + (size_t)a * 6 + c) = make_float2(W[c], W[c + 1]);
@@ -192,38 +231,34 @@ k_radial_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__res
   if (a >= N) return;
   const AdjCtx ac = make_adj(u, omega, scales, a, struct_s[a]);
   const int *sg = segR + (size_t)a * (sp.T + 1);
-  int p = sg[0], J = 0, jend = sg[1];
-  const int pend = sg[sp.T];
   float *Mrow = M2 + (size_t)a * sp.T * KT;
-  float acc[KT];
+  // accumulated per Chebyshev term with w1 = (a.rhat) hdf, w2 = (a.rhat) hfcp:
+  //   aD[k] = sum w1 D_k, aT[k] = sum w2 T_k (k >= 1), aT[0] = sum w2;  M2[0] = 2 aT[0], M2[k] = aD[k] + aT[k] + aT[0]
+  float aD[KT], aT[KT];
 #pragma unroll
-  for (int k = 0; k < KT; ++k) acc[k] = 0.f;
-  float4 rn = p < pend ? pairR[p] : make_float4(1.f, 0.f, 0.f, 0.f);
-  while (p < pend) {
-    const float4 r = rn;
-    if (p + 1 < pend) rn = pairR[p + 1];
-    while (p >= jend) {
-      store_row<KT>(Mrow + J * KT, acc);
+  for (int k = 0; k < KT; ++k) { aD[k] = 0.f; aT[k] = 0.f; }
+  walk_row(pairR, sg, sp.T,
+           [&](int J) {
+             float m[KT];
+             m[0] = 2.f * aT[0];
 #pragma unroll
-      for (int k = 0; k < KT; ++k) acc[k] = 0.f;
-      ++J; jend = sg[J + 1];
-    }
-    const float4 uj = u[__float_as_int(r.w)];
-    const float d = sqrtf(r.x * r.x + r.y * r.y + r.z * r.z);
-    const float rinv = 1.f / d;
-    float ax, ay, az;
-    pair_adjoint(ac, uj, r, ax, ay, az);
-    const float ar = (ax * r.x + ay * r.y + az * r.z) * rinv;
-    float f[KT], fp[KT];
-    cheb_ffp<KT>(d, sp.rcRinv, f, fp);
+             for (int k = 1; k < KT; ++k) m[k] = aD[k] + aT[k] + aT[0];
+             store_row<KT>(Mrow + J * KT, m);
 #pragma unroll
-    for (int k = 0; k < KT; ++k) acc[k] += fp[k] * ar;
-    ++p;
-  }
-  for (; J < sp.T; ++J) {
-    store_row<KT>(Mrow + J * KT, acc);
+             for (int k = 0; k < KT; ++k) { aD[k] = 0.f; aT[k] = 0.f; }
+           },
+           [&](const float4 &r) { return u[__float_as_int(r.w)]; },
+           [&](const float4 &r, const float4 &uj) {
+             float d, rinv, Tk[KT], Dk[KT], hfc, hfcp, hdf;
+             pair_len(r.x * r.x + r.y * r.y + r.z * r.z, d, rinv);
+             float ax, ay, az;
+             pair_adjoint(ac, uj, r, ax, ay, az);
+             const float ar = (ax * r.x + ay * r.y + az * r.z) * rinv;
+             cheb_TD<KT>(d, sp.rcRinv, Tk, Dk, hfc, hfcp, hdf);
+             const float w1 = ar * hdf, w2 = ar * hfcp;
+             aT[0] += w2;
 #pragma unroll
-    for (int k = 0; k < KT; ++k) acc[k] = 0.f;
-  }
+             for (int k = 1; k < KT; ++k) { aD[k] = fmaf(w1, Dk[k], aD[k]); aT[k] = fmaf(w2, Tk[k], aT[k]); }
+           });
   radial_contract<KT>(sp, cs, type_s[a], Mrow, D + (size_t)a * sp.Ndes);
 }
