@@ -534,8 +534,21 @@ k_cgrad_angular(DevSpec sp, int N, const int *__restrict__ type_s, const float *
   __syncwarp();
   const int rows = sp.T * KT;                      // (J,k) rows of A1/A2
   const int nh = (sp.NA + 1) >> 1;                 // n's per half
+  const int half = lane & 1;
+  const int n_lo = half * nh, n_hi = min(sp.NA, n_lo + nh);
   for (int a = gw; a < N; a += nw) {
     const int I = type_s[a];
+    // the moment rows of the first round are requested before alpha/beta are formed, so that their latency is hidden
+    float4 x1[6], x2[6];
+    {
+      const int row = lane >> 1;
+      if (row < rows) {
+        const float4 *a1 = (const float4 *)(A1 + (size_t)a * nA + row * GNEP_NLM);
+        const float4 *a2 = (const float4 *)(A2 + (size_t)a * nA + row * GNEP_NLM);
+#pragma unroll
+        for (int v = 0; v < 6; ++v) { x1[v] = __ldg(a1 + v); x2[v] = __ldg(a2 + v); }
+      }
+    }
     const float *Sa = S + (size_t)a * nb, *Ta = Tn + (size_t)a * nb;
     const float *Epa = Ep + (size_t)a * sp.Ndes, *gba = gbar + (size_t)a * sp.Ndes;
     for (int n0 = 0; n0 < sp.NA; n0 += 10) {      // alpha, beta in the (n, lmg) lane layout
@@ -572,25 +585,26 @@ k_cgrad_angular(DevSpec sp, int N, const int *__restrict__ type_s, const float *
     }
     __syncwarp();
     // contraction: lane -> row = lane>>1 (+16 per round), half = lane&1 -> n in [half*nh, min(NA, half*nh+nh))
-    const int half = lane & 1;
-    const int n_lo = half * nh, n_hi = min(sp.NA, n_lo + nh);
     for (int row = lane >> 1; row < rows; row += 16) {
-      const float4 *a1 = (const float4 *)(A1 + (size_t)a * nA + row * GNEP_NLM);
-      const float4 *a2 = (const float4 *)(A2 + (size_t)a * nA + row * GNEP_NLM);
-      float4 x1[6], x2[6];
+      if (row >= 16) {
+        const float4 *a1 = (const float4 *)(A1 + (size_t)a * nA + row * GNEP_NLM);
+        const float4 *a2 = (const float4 *)(A2 + (size_t)a * nA + row * GNEP_NLM);
 #pragma unroll
-      for (int v = 0; v < 6; ++v) { x1[v] = __ldg(a1 + v); x2[v] = __ldg(a2 + v); }
+        for (int v = 0; v < 6; ++v) { x1[v] = __ldg(a1 + v); x2[v] = __ldg(a2 + v); }
+      }
       const int J = row / KT, k = row - J * KT;
       float *dst = accS + ((I * sp.T + J) * sp.NA) * KT + k;
       for (int n = n_lo; n < n_hi; ++n) {
-        float s = 0.f;
+        float sa[2] = {0.f, 0.f}, sb[2] = {0.f, 0.f};   // four independent FMA chains
 #pragma unroll
         for (int v = 0; v < 6; ++v) {
-          float4 al4 = *(const float4 *)(sAl + n * GNEP_NLM + 4 * v);
-          float4 be4 = *(const float4 *)(sBe + n * GNEP_NLM + 4 * v);
-          s += dot4(al4, x1[v]) + dot4(be4, x2[v]);
+          const float4 al4 = *(const float4 *)(sAl + n * GNEP_NLM + 4 * v);
+          const float4 be4 = *(const float4 *)(sBe + n * GNEP_NLM + 4 * v);
+          float &s = sa[v & 1], &t = sb[v & 1];
+          s = fmaf(al4.x, x1[v].x, s); s = fmaf(al4.y, x1[v].y, s); s = fmaf(al4.z, x1[v].z, s); s = fmaf(al4.w, x1[v].w, s);
+          t = fmaf(be4.x, x2[v].x, t); t = fmaf(be4.y, x2[v].y, t); t = fmaf(be4.z, x2[v].z, t); t = fmaf(be4.w, x2[v].w, t);
         }
-        dst[n * KT] += s;
+        dst[n * KT] += (sa[0] + sa[1]) + (sb[0] + sb[1]);
       }
     }
     __syncwarp();
