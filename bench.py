@@ -197,16 +197,11 @@ def run_ours(args):
     N_glob, S_glob = N_local, S_local
     grad_t = torch.empty(P, dtype=torch.float32, device="cuda")
     if world > 1:
-        cnt = torch.tensor([N_local, S_local], dtype=torch.int64, device="cuda")
-        dist.all_reduce(cnt)
-        N_glob, S_glob = int(cnt[0]), int(cnt[1])
-        g.set_global_norm(N_glob, S_glob, 1.0 / world)
+        from paper_2507_00528_b200 import sharding
+        N_glob, S_glob = sharding.setup_sharded(g, dist, N_local, S_local, device="cuda")
 
     def step_multi():
-        g.loss_and_grad(want_terms=False, grad=grad_t)
-        dist.all_reduce(grad_t)
-        g.set_grad(grad_t)
-        g.adam_step(LR)
+        sharding.sharded_step(g, dist, grad_t, LR)
 
     def run_steps(k):
         if world == 1:

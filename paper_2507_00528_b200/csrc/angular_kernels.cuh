@@ -30,14 +30,6 @@ __device__ __forceinline__ void stage_coeff_t(float *dst, const float *src, int 
   }
 }
 
-// mask the components of a 4-pair group that fall outside [lo4, hi4)
-__device__ __forceinline__ float4 mask4(float4 v, int lo4, int hi4) {
-  v.x = (0 >= lo4 && 0 < hi4) ? v.x : 0.f;
-  v.y = (1 >= lo4 && 1 < hi4) ? v.y : 0.f;
-  v.z = (2 >= lo4 && 2 < hi4) ? v.z : 0.f;
-  v.w = (3 >= lo4 && 3 < hi4) ? v.w : 0.f;
-  return v;
-}
 __device__ __forceinline__ float dot4(const float4 &a, const float4 &b) { return a.x * b.x + a.y * b.y + a.z * b.z + a.w * b.w; }
 
 // Per-atom lane layout "(n, lmg)": lane = 3*nq + lmg (lanes 0..29), n = nb + nq for nb = 0, 10, ..., and the lane owns
@@ -198,16 +190,13 @@ k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
     while (pos < chunk_end) {
       while (seg_end <= pos) next_segment();
       const int hi = min(seg_end, chunk_end);
-      const int g0 = (pos - c0) >> 2, g1 = (hi - 1 - c0) >> 2;
-      for (int g = g0; g <= g1; ++g) {
-        const int lo4 = pos - c0 - 4 * g, hi4 = hi - c0 - 4 * g;
-        const bool partial = lo4 > 0 || hi4 < 4;
+      // segments are multiples of 4 pairs (k_pad_angular) and so are the chunk bounds: whole 4-pair groups only
+      for (int g = (pos - c0) >> 2; g < (hi - c0) >> 2; ++g) {
         float4 fv[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
           int k = kq + 8 * r;
           fv[r] = k < KT ? *(const float4 *)(sf + k * ANG_LD + 4 * g) : make_float4(0.f, 0.f, 0.f, 0.f);
-          if (partial) fv[r] = mask4(fv[r], lo4, hi4);
         }
 #pragma unroll
         for (int i = 0; i < 6; ++i) {
@@ -356,10 +345,7 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
     while (pos < chunk_end) {
       while (seg_end <= pos) next_segment();
       const int hi = min(seg_end, chunk_end);
-      const int g0 = (pos - c0) >> 2, g1 = (hi - 1 - c0) >> 2;
-      for (int g = g0; g <= g1; ++g) {
-        const int lo4 = pos - c0 - 4 * g, hi4 = hi - c0 - 4 * g;
-        const bool partial = lo4 > 0 || hi4 < 4;
+      for (int g = (pos - c0) >> 2; g < (hi - c0) >> 2; ++g) {   // whole 4-pair groups only (padded segments)
         float4 f1[R], f2[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
@@ -367,7 +353,6 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
           const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
           f1[r] = k < KT ? *(const float4 *)(sf1 + k * ANG_LD + 4 * g) : z4;
           f2[r] = k < KT ? *(const float4 *)(sf2 + k * ANG_LD + 4 * g) : z4;
-          if (partial) { f1[r] = mask4(f1[r], lo4, hi4); f2[r] = mask4(f2[r], lo4, hi4); }
         }
 #pragma unroll
         for (int i = 0; i < 6; ++i) {
