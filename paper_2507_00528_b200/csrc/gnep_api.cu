@@ -141,7 +141,7 @@ size_t smem_cgrad_ang(const DevSpec &d) {
 size_t smem_net_fwd(const DevSpec &d) { return net_tc_smem_bytes(d, false); }
 size_t smem_net_bwd(const DevSpec &d) { return net_tc_smem_bytes(d, true); }
 size_t smem_gradw(const DevSpec &d) { return gradw_smem_bytes(d); }
-size_t smem_cgrad_rad(const DevSpec &d) { return sizeof(float) * CR_SUB * 2 * (d.NR + d.T * d.KRp); }
+size_t smem_cgrad_rad(const DevSpec &d) { return cgrad_radial_smem_bytes(d); }
 
 template <class K>
 int set_smem(gnep_handle *h, K kernel, size_t bytes) {
@@ -254,7 +254,7 @@ int enqueue_backward(gnep_handle *h) {
   mark(h, "a6_network_backward");
   LAUNCH(h, k_gradw_tc, h->n_gw, GW_THREADS, smem_gradw(d), d, h->sm, gradw_nraw(d), h->theta, h->qscale, h->eat, h->q, h->D, h->x, h->pbuf, h->partialW, h->partialB);
   mark(h, "a6_w0_gradient");
-  LAUNCH(h, k_cgrad_radial, h->n_chunks, 256, smem_cgrad_rad(d), d, h->sm, h->gbar, h->Ep, h->M1, h->M2, h->partialCR);
+  LAUNCH(h, k_cgrad_radial, h->n_chunks, CR_THREADS, smem_cgrad_rad(d), d, h->sm, h->gbar, h->Ep, h->M1, h->M2, h->partialCR);
   mark(h, "a7_radial_cgrad");
   DISPATCH_KT(d.KAp, LAUNCH(h, k_cgrad_angular<KT>, h->n_ca_blocks, ANG_WARPS * 32, smem_cgrad_ang(d), d, h->N, h->type_s, h->Ep, h->gbar, h->Sn, h->Tn, h->A1, h->A2, h->partialCA));
   mark(h, "a7_angular_cgrad");
@@ -666,7 +666,7 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
       int nc = tiles > 0 ? std::max(1, std::min(cdiv(tiles, 2), (int)((double)h->num_sms * tiles / std::max(tiles_total, 1) + 0.5))) : 0;
       h->sm.cta_base[t + 1] = h->sm.cta_base[t] + nc;
       // k_cgrad_radial: K-chunks
-      int want = nt > 0 ? std::max(1, std::min(cdiv(nt, 256), (int)((2.0 * h->num_sms * nt) / std::max(N, 1) + 0.5))) : 0;
+      int want = nt > 0 ? std::max(1, std::min(cdiv(nt, 256), (int)((4.0 * h->num_sms * nt) / std::max(N, 1) + 0.5))) : 0;
       int ca = want > 0 ? ((cdiv(nt, want) + 31) / 32) * 32 : 32;
       h->sm.chunk_atoms[t] = ca;
       h->sm.chunk_base[t + 1] = h->sm.chunk_base[t] + (nt > 0 ? cdiv(nt, ca) : 0);
