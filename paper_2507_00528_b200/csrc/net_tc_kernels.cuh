@@ -59,6 +59,17 @@ __device__ __forceinline__ float tanh_fast(float z) {
   return fmaf(-2.f, rc, 1.f);
 }
 
+// 3xTF32 split with integer round-half-away (2 + 1 + 2 instructions): hi = tf32(x), lo = tf32(x - hi)
+__device__ __forceinline__ void split_fast(float x, float &hi, float &lo) {
+  hi = __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
+  lo = __uint_as_float((__float_as_uint(x - hi) + 0x1000u) & 0xffffe000u);
+}
+__device__ __forceinline__ void split4_fast(const float4 &x, float4 &hi, float4 &lo) {
+  split_fast(x.x, hi.x, lo.x); split_fast(x.y, hi.y, lo.y); split_fast(x.z, hi.z, lo.z); split_fast(x.w, hi.w, lo.w);
+}
+
+#define NET_PRE 16      // row chunks (float4) of the next tile held in registers
+
 __device__ __forceinline__ void wg_barrier(int wg) { asm volatile("bar.sync %0, 128;" ::"r"(1 + wg) : "memory"); }
 
 // 4 consecutive values of a row of length W starting at column c (zeros beyond W); vectorised when rows are 16-byte aligned
@@ -158,29 +169,40 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
   const int tiles = (n_t + 127) >> 7;
   const int ncta = sm.cta_base[t + 1] - sm.cta_base[t];
   uint32_t parity = 0;
+  float4 pre[NET_PRE];     // input row of the NEXT tile, requested while the current tile is in its epilogues
+  auto prefetch_row = [&](int tile_) {
+    const int a_ = sm.start[t] + tile_ * 128 + r;
+    const bool ok = tile_ < tiles && a_ < sm.start[t + 1];
+    const float *row_ = in_rows + (size_t)a_ * sp.Ndes;
+#pragma unroll
+    for (int c = 0; c < NET_PRE; ++c) pre[c] = load_row4(row_, sp.Ndes, 4 * c, vecD, ok && c < NdK / 4);
+  };
+  prefetch_row((blockIdx.x - sm.cta_base[t]) * 2 + wg);
   for (int tile = (blockIdx.x - sm.cta_base[t]) * 2 + wg; tile < tiles; tile += 2 * ncta, parity ^= 1u) {
     const int a = sm.start[t] + tile * 128 + r;
     const bool valid = a < sm.start[t + 1];
-    // ---- step 1 ----
+    // ---- step 1 ---- (the first NET_PRE row chunks were requested during the previous tile)
     {
       const float *row = in_rows + (size_t)a * sp.Ndes;
-      for (int cb = 0; cb < NdK / 4; cb += 8) {     // 8 row chunks in flight per thread
-        float4 v8[8];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) v8[j] = load_row4(row, sp.Ndes, 4 * (cb + j), vecD, valid && cb + j < NdK / 4);
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const int c = cb + j;
-          if (c < NdK / 4) {
-            float4 v = v8[j];
-            const float4 s4 = *(const float4 *)(qss + 4 * c);
-            v.x *= s4.x; v.y *= s4.y; v.z *= s4.z; v.w *= s4.w;
-            float4 hi, lo;
-            split4(v, hi, lo);
-            *(float4 *)(abuf + (c * 128 + r) * 4) = hi;
-            *(float4 *)(abuf + NdK * 128 + (c * 128 + r) * 4) = lo;
-          }
+      for (int c = 0; c < NET_PRE; ++c)
+        if (c < NdK / 4) {
+          float4 v = pre[c];
+          const float4 s4 = *(const float4 *)(qss + 4 * c);
+          v.x *= s4.x; v.y *= s4.y; v.z *= s4.z; v.w *= s4.w;
+          float4 hi, lo;
+          split4_fast(v, hi, lo);
+          *(float4 *)(abuf + (c * 128 + r) * 4) = hi;
+          *(float4 *)(abuf + NdK * 128 + (c * 128 + r) * 4) = lo;
         }
+      for (int c = NET_PRE; c < NdK / 4; ++c) {
+        float4 v = load_row4(row, sp.Ndes, 4 * c, vecD, valid);
+        const float4 s4 = *(const float4 *)(qss + 4 * c);
+        v.x *= s4.x; v.y *= s4.y; v.z *= s4.z; v.w *= s4.w;
+        float4 hi, lo;
+        split4_fast(v, hi, lo);
+        *(float4 *)(abuf + (c * 128 + r) * 4) = hi;
+        *(float4 *)(abuf + NdK * 128 + (c * 128 + r) * 4) = lo;
       }
     }
     float ev = 0.f;
@@ -203,6 +225,7 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
       }
       mma_commit(bar1);
     }
+    prefetch_row(tile + 2 * ncta);
     float4 xnext[4];   // backward: the x row is fetched one 16-neuron chunk ahead of its use
     if (BWD) {
 #pragma unroll
@@ -212,12 +235,18 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
     fence_after_sync();
     // ---- step 3 ----
     float eacc = 0.f;
+    uint32_t tz[16], tc[16];   // TMEM chunk m0 + 16 is in flight while chunk m0 is worked on
+    tmem_ld16_issue(tmem_addr(tD1, lane0, 0), tz);
+    tmem_ld16_issue(tmem_addr(tD1c, lane0, 0), tc);
     for (int m0 = 0; m0 < NnP; m0 += 16) {
       float z[16], ch[16], cl[16];
-      tmem_ld16(tmem_addr(tD1, lane0, m0), z);
-      tmem_ld16(tmem_addr(tD1c, lane0, m0), ch);
+      tmem_ld_wait(tz, tc);
 #pragma unroll
-      for (int i = 0; i < 16; ++i) z[i] += ch[i];
+      for (int i = 0; i < 16; ++i) z[i] = __uint_as_float(tz[i]) + __uint_as_float(tc[i]);
+      if (m0 + 16 < NnP) {
+        tmem_ld16_issue(tmem_addr(tD1, lane0, m0 + 16), tz);
+        tmem_ld16_issue(tmem_addr(tD1c, lane0, m0 + 16), tc);
+      }
       if (!BWD) {
         float xs[16];
 #pragma unroll
@@ -226,7 +255,7 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
           const float w1 = w1s[m0 + i];            // zero for padded neurons
           xs[i] = xv;
           eacc += w1 * xv;
-          split_tf32(w1 * (1.f - xv * xv), ch[i], cl[i]);
+          split_fast(w1 * (1.f - xv * xv), ch[i], cl[i]);
         }
         if (valid) {
           float *xr = xbuf + (size_t)a * sp.Nn;
@@ -249,7 +278,7 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
             const float d1 = 1.f - xv[i] * xv[i], d2 = -2.f * xv[i] * d1;
-            split_tf32(w1s[m0 + 4 * v + i] * d2 * z[4 * v + i], ch[4 * v + i], cl[4 * v + i]);
+            split_fast(w1s[m0 + 4 * v + i] * d2 * z[4 * v + i], ch[4 * v + i], cl[4 * v + i]);
           }
           if (valid) store_row4(pr, sp.Nn, m0 + 4 * v, vecN, make_float4(z[4 * v], z[4 * v + 1], z[4 * v + 2], z[4 * v + 3]));
         }
@@ -293,12 +322,17 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
     fence_after_sync();
     // ---- step 5 ----
     float epr[16];
+    tmem_ld16_issue(tmem_addr(tD2, lane0, 0), tz);
+    tmem_ld16_issue(tmem_addr(tD2c, lane0, 0), tc);
     for (int n0 = 0; n0 < NdN; n0 += 16) {
-      float v[16], vc[16];
-      tmem_ld16(tmem_addr(tD2, lane0, n0), v);
-      tmem_ld16(tmem_addr(tD2c, lane0, n0), vc);
+      float v[16];
+      tmem_ld_wait(tz, tc);
 #pragma unroll
-      for (int i = 0; i < 16; ++i) v[i] = (v[i] + vc[i]) * qss[n0 + i];
+      for (int i = 0; i < 16; ++i) v[i] = (__uint_as_float(tz[i]) + __uint_as_float(tc[i])) * qss[n0 + i];
+      if (n0 + 16 < NdN) {
+        tmem_ld16_issue(tmem_addr(tD2, lane0, n0 + 16), tz);
+        tmem_ld16_issue(tmem_addr(tD2c, lane0, n0 + 16), tc);
+      }
       if (!BWD) {
         if (n0 == 0) {
 #pragma unroll
@@ -412,15 +446,6 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
                ::"r"(tc05::smem_u32(dst)), "l"(__cvta_generic_to_global(src)), "r"(bytes), "r"(tc05::smem_u32(bar))
                : "memory");
 }
-// 3xTF32 split with integer round-half-away (2 + 1 + 2 instructions): hi = tf32(x), lo = tf32(x - hi)
-__device__ __forceinline__ void split_fast(float x, float &hi, float &lo) {
-  hi = __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
-  lo = __uint_as_float((__float_as_uint(x - hi) + 0x1000u) & 0xffffe000u);
-}
-__device__ __forceinline__ void split4_fast(const float4 &x, float4 &hi, float4 &lo) {
-  split_fast(x.x, hi.x, lo.x); split_fast(x.y, hi.y, lo.y); split_fast(x.z, hi.z, lo.z); split_fast(x.w, hi.w, lo.w);
-}
-
 __global__ void __launch_bounds__(GW_THREADS, 1)
 k_gradw_tc(DevSpec sp, SpeciesMap sm, int nraw, const float *__restrict__ theta, const float *__restrict__ qscale,
            const float *__restrict__ eat, const float *__restrict__ q, const float *__restrict__ D,
