@@ -8,7 +8,8 @@
 // so the coefficient gradient needs no pair sweep of its own.
 //
 // Mapping: a warp owns ANG_TA consecutive atoms; their pairs are contiguous in pairA, so phase 1 (lane = pair)
-// runs on full 32-pair chunks that cross atom boundaries, and phase 2 (lane = (k, 6 lm) register tile) walks the
+// runs on full 32-pair chunks that cross atom boundaries, and phase 2 (lane = (KT/4 k, 3 lm) register tile: the
+// shape with the fewest shared-memory operand loads per FMA for 32 lanes on an 8 x 24 output) walks the
 // (atom, species-segment) boundaries inside the chunk.  Shared rows have stride ANG_LD = 36 floats so that the
 // LDS.128 of 8 different rows hit 8 different bank quads.
 #pragma once
@@ -88,7 +89,7 @@ __global__ void __launch_bounds__(ANG_WARPS * 32)
 k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ segA,
               const float4 *__restrict__ pairA, const float *__restrict__ theta, float *__restrict__ q,
               float *__restrict__ S, float *__restrict__ A1) {
-  constexpr int R = (KT + 7) / 8;
+  constexpr int KQ = (KT + 3) / 4;      // k per lane: lane = (k quarter kq, lm eighth lmq) holds a KQ x 3 register tile
   extern __shared__ __align__(128) float smem[];
   float *ct = smem;
   const int nct = sp.T * sp.T * KT * ANG_NQ;
@@ -105,32 +106,30 @@ k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   const int a_hi = min(a_lo + ANG_TA, N);
   const int T1 = sp.T + 1;
   const int P_lo = segA[a_lo * T1], P_hi = segA[(a_hi - 1) * T1 + sp.T];
-  const int kq = lane >> 2, lmq = lane & 3;
+  const int kq = lane >> 3, lmq = lane & 7;
   const NLane nl = make_nlane(lane);
-  float acc[R][6];
+  float acc[KQ][3];
 #pragma unroll
-  for (int r = 0; r < R; ++r)
+  for (int r = 0; r < KQ; ++r)
 #pragma unroll
-    for (int i = 0; i < 6; ++i) acc[r][i] = 0.f;
+    for (int i = 0; i < 3; ++i) acc[r][i] = 0.f;
   int a = a_lo, J = 0;
   int seg_end = segA[a * T1 + 1];
 
   auto flush_segment = [&]() {   // accumulators of (a, J) -> global A1 and shared As, then reset
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-      int k = kq + 8 * r;
+    for (int r = 0; r < KQ; ++r) {
+      int k = kq * KQ + r;
       if (k < KT) {
-        int o = (J * KT + k) * GNEP_NLM + 6 * lmq;
-        float *g = A1 + (size_t)a * nA + o;
+        int o = (J * KT + k) * GNEP_NLM + 3 * lmq;
 #pragma unroll
-        for (int i = 0; i < 6; i += 2) *(float2 *)(g + i) = make_float2(acc[r][i], acc[r][i + 1]);
-#pragma unroll
-        for (int i = 0; i < 6; ++i) { As[o + i] = acc[r][i]; acc[r][i] = 0.f; }
+        for (int i = 0; i < 3; ++i) { As[o + i] = acc[r][i]; acc[r][i] = 0.f; }
       }
     }
   };
-  auto atom_epilogue = [&]() {   // S = c.A1, q_nl, q4 of atom a
+  auto atom_epilogue = [&]() {   // A1 -> global, S = c.A1, q_nl, q4 of atom a
     __syncwarp();
+    for (int x = lane; x < nA / 4; x += 32) ((float4 *)(A1 + (size_t)a * nA))[x] = ((const float4 *)As)[x];
     const int I = type_s[a];
     float *Sa = S + (size_t)a * sp.NA * GNEP_NLM;
     float *qa = q + (size_t)a * sp.Ndes + sp.NR;
@@ -192,17 +191,17 @@ k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
       const int hi = min(seg_end, chunk_end);
       // segments are multiples of 4 pairs (k_pad_angular) and so are the chunk bounds: whole 4-pair groups only
       for (int g = (pos - c0) >> 2; g < (hi - c0) >> 2; ++g) {
-        float4 fv[R];
+        float4 fv[KQ];
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-          int k = kq + 8 * r;
+        for (int r = 0; r < KQ; ++r) {
+          int k = kq * KQ + r;
           fv[r] = k < KT ? *(const float4 *)(sf + k * ANG_LD + 4 * g) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
 #pragma unroll
-        for (int i = 0; i < 6; ++i) {
-          float4 b = *(const float4 *)(sB + (6 * lmq + i) * ANG_LD + 4 * g);
+        for (int i = 0; i < 3; ++i) {
+          float4 b = *(const float4 *)(sB + (3 * lmq + i) * ANG_LD + 4 * g);
 #pragma unroll
-          for (int r = 0; r < R; ++r) acc[r][i] += dot4(fv[r], b);
+          for (int r = 0; r < KQ; ++r) acc[r][i] += dot4(fv[r], b);
         }
       }
       pos = hi;
@@ -222,7 +221,7 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
               const float *__restrict__ theta, const float4 *__restrict__ u, const float *__restrict__ omega,
               const float *__restrict__ scales, const float *__restrict__ S, float *__restrict__ Tn,
               float *__restrict__ A2, float *__restrict__ D) {
-  constexpr int R = (KT + 7) / 8;
+  constexpr int KQ = (KT + 3) / 4;      // k per lane: lane = (k quarter kq, lm eighth lmq) holds a KQ x 3 register tile
   extern __shared__ __align__(128) float smem[];
   float *ct = smem;
   const int nct = sp.T * sp.T * KT * ANG_NQ;
@@ -241,33 +240,31 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   const int a_hi = min(a_lo + ANG_TA, N);
   const int T1 = sp.T + 1;
   const int P_lo = segA[a_lo * T1], P_hi = segA[(a_hi - 1) * T1 + sp.T];
-  const int kq = lane >> 2, lmq = lane & 3;
+  const int kq = lane >> 3, lmq = lane & 7;
   const NLane nl = make_nlane(lane);
   const float sfF = scales[1], svV = scales[2];
-  float acc[R][6];
+  float acc[KQ][3];
 #pragma unroll
-  for (int r = 0; r < R; ++r)
+  for (int r = 0; r < KQ; ++r)
 #pragma unroll
-    for (int i = 0; i < 6; ++i) acc[r][i] = 0.f;
+    for (int i = 0; i < 3; ++i) acc[r][i] = 0.f;
   int a = a_lo, J = 0;
   int seg_end = segA[a * T1 + 1];
 
   auto flush_segment = [&]() {
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-      int k = kq + 8 * r;
+    for (int r = 0; r < KQ; ++r) {
+      int k = kq * KQ + r;
       if (k < KT) {
-        int o = (J * KT + k) * GNEP_NLM + 6 * lmq;
-        float *g = A2 + (size_t)a * nA + o;
+        int o = (J * KT + k) * GNEP_NLM + 3 * lmq;
 #pragma unroll
-        for (int i = 0; i < 6; i += 2) *(float2 *)(g + i) = make_float2(acc[r][i], acc[r][i + 1]);
-#pragma unroll
-        for (int i = 0; i < 6; ++i) { As[o + i] = acc[r][i]; acc[r][i] = 0.f; }
+        for (int i = 0; i < 3; ++i) { As[o + i] = acc[r][i]; acc[r][i] = 0.f; }
       }
     }
   };
-  auto atom_epilogue = [&]() {   // T = c.A2, D of atom a
+  auto atom_epilogue = [&]() {   // A2 -> global, T = c.A2, D of atom a
     __syncwarp();
+    for (int x = lane; x < nA / 4; x += 32) ((float4 *)(A2 + (size_t)a * nA))[x] = ((const float4 *)As)[x];
     const int I = type_s[a];
     const float *Sa = S + (size_t)a * sp.NA * GNEP_NLM;
     float *Ta = Tn + (size_t)a * sp.NA * GNEP_NLM;
@@ -346,20 +343,20 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
       while (seg_end <= pos) next_segment();
       const int hi = min(seg_end, chunk_end);
       for (int g = (pos - c0) >> 2; g < (hi - c0) >> 2; ++g) {   // whole 4-pair groups only (padded segments)
-        float4 f1[R], f2[R];
+        float4 f1[KQ], f2[KQ];
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-          int k = kq + 8 * r;
+        for (int r = 0; r < KQ; ++r) {
+          int k = kq * KQ + r;
           const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
           f1[r] = k < KT ? *(const float4 *)(sf1 + k * ANG_LD + 4 * g) : z4;
           f2[r] = k < KT ? *(const float4 *)(sf2 + k * ANG_LD + 4 * g) : z4;
         }
 #pragma unroll
-        for (int i = 0; i < 6; ++i) {
-          float4 X = *(const float4 *)(sX + (6 * lmq + i) * ANG_LD + 4 * g);
-          float4 Y = *(const float4 *)(sY + (6 * lmq + i) * ANG_LD + 4 * g);
+        for (int i = 0; i < 3; ++i) {
+          float4 X = *(const float4 *)(sX + (3 * lmq + i) * ANG_LD + 4 * g);
+          float4 Y = *(const float4 *)(sY + (3 * lmq + i) * ANG_LD + 4 * g);
 #pragma unroll
-          for (int r = 0; r < R; ++r) acc[r][i] += dot4(f1[r], X) + dot4(f2[r], Y);
+          for (int r = 0; r < KQ; ++r) acc[r][i] += dot4(f1[r], X) + dot4(f2[r], Y);
         }
       }
       pos = hi;
