@@ -20,6 +20,7 @@
 #define ANG_WARPS 4      // warps per CTA
 #define ANG_LD 36        // shared-memory row stride in floats
 #define ANG_NQ 16        // n padded to 16 in the transposed coefficient table
+#define ANG_SEGS (ANG_TA * GNEP_MAX_SPECIES_C)   // (atom, J) segments of a warp tile
 
 // transposed coefficients ct[((I*T+J)*KT + k)*ANG_NQ + n] (zero padded) for the S/T/Gamma contractions
 __device__ __forceinline__ void stage_coeff_t(float *dst, const float *src, int T, int NA, int K, int KT) {
@@ -56,24 +57,6 @@ __device__ __forceinline__ NLane make_nlane(int lane) {
 __device__ __forceinline__ float desc_of(const DevSpec &sp, const float *__restrict__ row, int l, int n) {
   return l <= sp.L ? row[sp.NR + (l - 1) * sp.NA + n] : 0.f;
 }
-// X[n][8 lmg .. +8] = sum_{J,k} c[I][J][n][k] A[J][k][lm]  (S = c.A1, T = c.A2)
-template <int KT>
-__device__ __forceinline__ void contract_nl(const DevSpec &sp, const float *ct, const float *As, int I, int n, int lmg,
-                                            float (&out)[8]) {
-#pragma unroll
-  for (int i = 0; i < 8; ++i) out[i] = 0.f;
-  for (int J = 0; J < sp.T; ++J) {
-    const float *cj = ct + (I * sp.T + J) * KT * ANG_NQ + n;
-    const float *aj = As + J * KT * GNEP_NLM + 8 * lmg;
-#pragma unroll
-    for (int k = 0; k < KT; ++k) {
-      float c = cj[k * ANG_NQ];
-      float4 a0 = *(const float4 *)(aj + k * GNEP_NLM), a1 = *(const float4 *)(aj + k * GNEP_NLM + 4);
-      out[0] += c * a0.x; out[1] += c * a0.y; out[2] += c * a0.z; out[3] += c * a0.w;
-      out[4] += c * a1.x; out[5] += c * a1.y; out[6] += c * a1.z; out[7] += c * a1.w;
-    }
-  }
-}
 // sums of w[i] over the lane's two l-blocks
 __device__ __forceinline__ void split_sums(const NLane &nl, const float (&w)[8], float &sa, float &sb) {
   sa = 0.f; sb = 0.f;
@@ -81,10 +64,48 @@ __device__ __forceinline__ void split_sums(const NLane &nl, const float (&w)[8],
   for (int i = 0; i < 8; ++i) { if (i < nl.split) sa += w[i]; else sb += w[i]; }
 }
 
+// Epilogue contraction X = c . A (S = c.A1, T = c.A2) without a second pass over shared memory: when a segment's
+// register tile acc[KQ][3] (k in the lane's quarter, 3 lm) is complete, the lane adds its part
+//   Xp[n][i] += sum_r c[I][J][n][k_r] acc[r][i]
+// for all n; at the end of the atom the four k-quarters are summed by two butterfly shuffles and X[n][lm] goes to
+// shared memory once (Xs[n][24]) for the per-(n, l) contractions.  (The straightforward form re-reads the whole
+// moment matrix from shared memory for every n-group and made the sweeps shared-memory-bandwidth bound.)
+template <int KT, int KQ, int NQ>
+__device__ __forceinline__ void xpart_add(const DevSpec &sp, const float *ct, int I, int J, int kq, const float (&acc)[KQ][3],
+                                          float (&Xp)[NQ][3]) {
+#pragma unroll
+  for (int r = 0; r < KQ; ++r) {
+    const int k = kq * KQ + r;
+    if (k < KT) {
+      const float *cp = ct + ((I * sp.T + J) * KT + k) * ANG_NQ;
+#pragma unroll
+      for (int n = 0; n < NQ; ++n) {
+        const float c = cp[n];                      // zero for n >= NA (zero-padded table)
+#pragma unroll
+        for (int i = 0; i < 3; ++i) Xp[n][i] = fmaf(c, acc[r][i], Xp[n][i]);
+      }
+    }
+  }
+}
+template <int NQ>
+__device__ __forceinline__ void xpart_finish(int kq, int lmq, float (&Xp)[NQ][3], float *Xs) {
+#pragma unroll
+  for (int n = 0; n < NQ; ++n)
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      float v = Xp[n][i];
+      v += __shfl_xor_sync(0xffffffffu, v, 8);
+      v += __shfl_xor_sync(0xffffffffu, v, 16);
+      if ((n & 3) == kq) Xs[n * GNEP_NLM + 3 * lmq + i] = v;
+      Xp[n][i] = 0.f;
+    }
+  __syncwarp();
+}
+
 // ------------------------------------------------------------------------------------------------
 // a1 (angular): A1 moments, S_nlm (Eq.8), q_nl = sum_m C_lm S_nlm^2 (Eq.7), 4-body (R14)
 // ------------------------------------------------------------------------------------------------
-template <int KT>
+template <int KT, int NQ>
 __global__ void __launch_bounds__(ANG_WARPS * 32)
 k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ segA,
               const float4 *__restrict__ pairA, const float *__restrict__ theta, float *__restrict__ q,
@@ -94,10 +115,12 @@ k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   float *ct = smem;
   const int nct = sp.T * sp.T * KT * ANG_NQ;
   const int nA = sp.T * KT * GNEP_NLM;
-  const int per_warp = (KT + GNEP_NLM) * ANG_LD + nA;
+  const int per_warp = (KT + GNEP_NLM) * ANG_LD + nA + ANG_NQ * GNEP_NLM + ANG_SEGS;
   float *sf = smem + nct + (threadIdx.x >> 5) * per_warp;   // [KT][LD]
   float *sB = sf + KT * ANG_LD;                              // [24][LD]
   float *As = sB + GNEP_NLM * ANG_LD;                        // [T][KT][24]
+  float *Xs = As + nA;                                       // [NQ][24]  S of the current atom
+  int *sEnd = (int *)(Xs + ANG_NQ * GNEP_NLM);               // segment ends of the tile
   stage_coeff_t(ct, theta + sp.offA, sp.T, sp.NA, sp.KA, KT);
   __syncthreads();
   const int lane = threadIdx.x & 31;
@@ -113,10 +136,18 @@ k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   for (int r = 0; r < KQ; ++r)
 #pragma unroll
     for (int i = 0; i < 3; ++i) acc[r][i] = 0.f;
+  float Xp[NQ][3];
+#pragma unroll
+  for (int n = 0; n < NQ; ++n)
+#pragma unroll
+    for (int i = 0; i < 3; ++i) Xp[n][i] = 0.f;
+  for (int x = lane; x < (a_hi - a_lo) * sp.T; x += 32) sEnd[x] = segA[(a_lo + x / sp.T) * T1 + x % sp.T + 1];
+  __syncwarp();
   int a = a_lo, J = 0;
-  int seg_end = segA[a * T1 + 1];
+  int seg_end = sEnd[0];
 
-  auto flush_segment = [&]() {   // accumulators of (a, J) -> global A1 and shared As, then reset
+  auto flush_segment = [&]() {   // accumulators of (a, J) -> S partial sums and shared As, then reset
+    xpart_add<KT, KQ, NQ>(sp, ct, type_s[a], J, kq, acc, Xp);
 #pragma unroll
     for (int r = 0; r < KQ; ++r) {
       int k = kq * KQ + r;
@@ -130,7 +161,7 @@ k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   auto atom_epilogue = [&]() {   // A1 -> global, S = c.A1, q_nl, q4 of atom a
     __syncwarp();
     for (int x = lane; x < nA / 4; x += 32) ((float4 *)(A1 + (size_t)a * nA))[x] = ((const float4 *)As)[x];
-    const int I = type_s[a];
+    xpart_finish<NQ>(kq, lmq, Xp, Xs);
     float *Sa = S + (size_t)a * sp.NA * GNEP_NLM;
     float *qa = q + (size_t)a * sp.Ndes + sp.NR;
     for (int nb = 0; nb < sp.NA; nb += 10) {
@@ -138,7 +169,10 @@ k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
       const bool on = nl.act && n < sp.NA;
       float sv[8], qa_ = 0.f, qb_ = 0.f;
       if (on) {
-        contract_nl<KT>(sp, ct, As, I, n, nl.lmg, sv);
+        {
+          const float4 s0 = *(const float4 *)(Xs + n * GNEP_NLM + 8 * nl.lmg), s1 = *(const float4 *)(Xs + n * GNEP_NLM + 8 * nl.lmg + 4);
+          sv[0] = s0.x; sv[1] = s0.y; sv[2] = s0.z; sv[3] = s0.w; sv[4] = s1.x; sv[5] = s1.y; sv[6] = s1.z; sv[7] = s1.w;
+        }
         *(float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg) = make_float4(sv[0], sv[1], sv[2], sv[3]);
         *(float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg + 4) = make_float4(sv[4], sv[5], sv[6], sv[7]);
         float w[8];
@@ -162,13 +196,15 @@ k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   auto next_segment = [&]() {
     flush_segment();
     if (++J == sp.T) { atom_epilogue(); J = 0; ++a; }
-    seg_end = a < a_hi ? segA[a * T1 + J + 1] : 0x7fffffff;
+    seg_end = a < a_hi ? sEnd[(a - a_lo) * sp.T + J] : 0x7fffffff;
   };
 
+  float4 rn = P_lo + lane < P_hi ? pairA[P_lo + lane] : make_float4(1.f, 0.f, 0.f, 0.f);
   for (int c0 = P_lo; c0 < P_hi; c0 += 32) {
     const int p = c0 + lane;
+    const float4 r = rn;
+    if (p + 32 < P_hi) rn = pairA[p + 32];                    // the next chunk's record is in flight during this chunk
     if (p < P_hi) {
-      float4 r = pairA[p];
       float d, rinv;
       pair_len(r.x * r.x + r.y * r.y + r.z * r.z, d, rinv);
       float f[KT];
@@ -214,7 +250,7 @@ k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
 // ------------------------------------------------------------------------------------------------
 // a5 (angular): A2 moments with the pair adjoint a_ij, T_nlm = c.A2, D_(n,l) = sum_m 2 C_lm S_nlm T_nlm, D_4
 // ------------------------------------------------------------------------------------------------
-template <int KT>
+template <int KT, int NQ>
 __global__ void __launch_bounds__(ANG_WARPS * 32)
 k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ struct_s,
               const int *__restrict__ segA, const int *__restrict__ atomA, const float4 *__restrict__ pairA,
@@ -226,12 +262,14 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   float *ct = smem;
   const int nct = sp.T * sp.T * KT * ANG_NQ;
   const int nA = sp.T * KT * GNEP_NLM;
-  const int per_warp = (2 * KT + 2 * GNEP_NLM) * ANG_LD + nA;
+  const int per_warp = (2 * KT + 2 * GNEP_NLM) * ANG_LD + nA + ANG_NQ * GNEP_NLM + ANG_SEGS;
   float *sf1 = smem + nct + (threadIdx.x >> 5) * per_warp;   // [KT][LD]  f_k' (a.rhat)
   float *sf2 = sf1 + KT * ANG_LD;                             // [KT][LD]  f_k
   float *sX = sf2 + KT * ANG_LD;                              // [24][LD]  B_lm
   float *sY = sX + GNEP_NLM * ANG_LD;                         // [24][LD]  grad B_lm . a
   float *As = sY + GNEP_NLM * ANG_LD;                         // [T][KT][24]
+  float *Xs = As + nA;                                        // [NQ][24]  T of the current atom
+  int *sEnd = (int *)(Xs + ANG_NQ * GNEP_NLM);                // segment ends of the tile
   stage_coeff_t(ct, theta + sp.offA, sp.T, sp.NA, sp.KA, KT);
   __syncthreads();
   const int lane = threadIdx.x & 31;
@@ -248,10 +286,18 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   for (int r = 0; r < KQ; ++r)
 #pragma unroll
     for (int i = 0; i < 3; ++i) acc[r][i] = 0.f;
+  float Xp[NQ][3];
+#pragma unroll
+  for (int n = 0; n < NQ; ++n)
+#pragma unroll
+    for (int i = 0; i < 3; ++i) Xp[n][i] = 0.f;
+  for (int x = lane; x < (a_hi - a_lo) * sp.T; x += 32) sEnd[x] = segA[(a_lo + x / sp.T) * T1 + x % sp.T + 1];
+  __syncwarp();
   int a = a_lo, J = 0;
-  int seg_end = segA[a * T1 + 1];
+  int seg_end = sEnd[0];
 
   auto flush_segment = [&]() {
+    xpart_add<KT, KQ, NQ>(sp, ct, type_s[a], J, kq, acc, Xp);
 #pragma unroll
     for (int r = 0; r < KQ; ++r) {
       int k = kq * KQ + r;
@@ -265,7 +311,7 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   auto atom_epilogue = [&]() {   // A2 -> global, T = c.A2, D of atom a
     __syncwarp();
     for (int x = lane; x < nA / 4; x += 32) ((float4 *)(A2 + (size_t)a * nA))[x] = ((const float4 *)As)[x];
-    const int I = type_s[a];
+    xpart_finish<NQ>(kq, lmq, Xp, Xs);
     const float *Sa = S + (size_t)a * sp.NA * GNEP_NLM;
     float *Ta = Tn + (size_t)a * sp.NA * GNEP_NLM;
     float *Da = D + (size_t)a * sp.Ndes + sp.NR;
@@ -276,7 +322,10 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
       if (on) {
         float4 s0 = *(const float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg), s1 = *(const float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg + 4);
         sv[0] = s0.x; sv[1] = s0.y; sv[2] = s0.z; sv[3] = s0.w; sv[4] = s1.x; sv[5] = s1.y; sv[6] = s1.z; sv[7] = s1.w;
-        contract_nl<KT>(sp, ct, As, I, n, nl.lmg, tv);
+        {
+          const float4 t0 = *(const float4 *)(Xs + n * GNEP_NLM + 8 * nl.lmg), t1 = *(const float4 *)(Xs + n * GNEP_NLM + 8 * nl.lmg + 4);
+          tv[0] = t0.x; tv[1] = t0.y; tv[2] = t0.z; tv[3] = t0.w; tv[4] = t1.x; tv[5] = t1.y; tv[6] = t1.z; tv[7] = t1.w;
+        }
         *(float4 *)(Ta + n * GNEP_NLM + 8 * nl.lmg) = make_float4(tv[0], tv[1], tv[2], tv[3]);
         *(float4 *)(Ta + n * GNEP_NLM + 8 * nl.lmg + 4) = make_float4(tv[4], tv[5], tv[6], tv[7]);
         float w[8];
@@ -304,16 +353,25 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   auto next_segment = [&]() {
     flush_segment();
     if (++J == sp.T) { atom_epilogue(); J = 0; ++a; }
-    seg_end = a < a_hi ? segA[a * T1 + J + 1] : 0x7fffffff;
+    seg_end = a < a_hi ? sEnd[(a - a_lo) * sp.T + J] : 0x7fffffff;
   };
 
+  // three-stage pipeline over chunks: records (r, atom) two chunks ahead, their gathers (u_i, u_j, structure) one
+  // chunk ahead, arithmetic on the current chunk
+  const float4 rdum = make_float4(1.f, 0.f, 0.f, 0.f);
+  float4 r1 = rdum, r2 = rdum, ui1 = rdum, uj1 = rdum;
+  int ai1 = 0, ai2 = 0, s1 = 0;
+  if (P_lo + lane < P_hi) { r1 = pairA[P_lo + lane]; ai1 = atomA[P_lo + lane]; }
+  if (P_lo + 32 + lane < P_hi) { r2 = pairA[P_lo + 32 + lane]; ai2 = atomA[P_lo + 32 + lane]; }
+  ui1 = u[ai1]; uj1 = u[__float_as_int(r1.w)]; s1 = struct_s[ai1];
   for (int c0 = P_lo; c0 < P_hi; c0 += 32) {
     const int p = c0 + lane;
+    const float4 r = r1, ui = ui1, uj = uj1;
+    const int s = s1;
+    r1 = r2; ai1 = ai2;
+    ui1 = u[ai1]; uj1 = u[__float_as_int(r1.w)]; s1 = struct_s[ai1];
+    if (p + 64 < P_hi) { r2 = pairA[p + 64]; ai2 = atomA[p + 64]; } else { r2 = rdum; ai2 = 0; }
     if (p < P_hi) {
-      float4 r = pairA[p];
-      const int ai = atomA[p];
-      const int s = struct_s[ai];
-      float4 ui = u[ai], uj = u[__float_as_int(r.w)];
       float d, rinv;
       pair_len(r.x * r.x + r.y * r.y + r.z * r.z, d, rinv);
       const float *om = omega + s * 6;

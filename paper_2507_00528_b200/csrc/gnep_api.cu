@@ -109,6 +109,11 @@ int padded_basis(int K) {
     default: { constexpr int KT = 16; __VA_ARGS__; } break;     \
   }
 
+// n (angular radial functions) padded to the register-array size of the angular sweeps
+#define DISPATCH_NQ(NA_, ...)                                   \
+  if ((NA_) <= 10) { constexpr int NQ = 10; __VA_ARGS__; }      \
+  else { constexpr int NQ = 16; __VA_ARGS__; }
+
 template <class T>
 int dalloc(gnep_handle *h, T **p, size_t n, bool batch) {
   void *q = nullptr;
@@ -128,11 +133,11 @@ void free_batch(gnep_handle *h) {
 // ---- dynamic shared memory sizes (bytes) --------------------------------------------------------
 size_t smem_radial(const DevSpec &d) { return sizeof(float) * (d.T * d.T * d.NR * d.KRp); }
 size_t smem_ang_fwd(const DevSpec &d) {
-  return sizeof(float) * (d.T * d.T * d.KAp * ANG_NQ + ANG_WARPS * ((d.KAp + GNEP_NLM) * ANG_LD + d.T * d.KAp * GNEP_NLM));
+  return sizeof(float) * (d.T * d.T * d.KAp * ANG_NQ + ANG_WARPS * ((d.KAp + GNEP_NLM) * ANG_LD + d.T * d.KAp * GNEP_NLM + ANG_NQ * GNEP_NLM + ANG_SEGS));
 }
 size_t smem_ang_force(const DevSpec &d) { return sizeof(float) * (((d.T * d.T * d.NA * d.KAp + 3) & ~3) + ANG_WARPS * FRC_TA * d.NA * GNEP_NLM); }
 size_t smem_ang_adj(const DevSpec &d) {
-  return sizeof(float) * (d.T * d.T * d.KAp * ANG_NQ + ANG_WARPS * ((2 * d.KAp + 2 * GNEP_NLM) * ANG_LD + d.T * d.KAp * GNEP_NLM));
+  return sizeof(float) * (d.T * d.T * d.KAp * ANG_NQ + ANG_WARPS * ((2 * d.KAp + 2 * GNEP_NLM) * ANG_LD + d.T * d.KAp * GNEP_NLM + ANG_NQ * GNEP_NLM + ANG_SEGS));
 }
 size_t smem_cgrad_ang(const DevSpec &d) {
   int nacc = d.T * d.T * d.NA * d.KAp;
@@ -153,8 +158,8 @@ int set_smem(gnep_handle *h, K kernel, size_t bytes) {
 int configure_kernels(gnep_handle *h) {
   const DevSpec &d = h->ds;
   DISPATCH_KT(d.KRp, RET_IF(set_smem(h, k_radial_fwd<KT>, smem_radial(d))); RET_IF(set_smem(h, k_radial_adj<KT>, smem_radial(d))));
-  DISPATCH_KT(d.KAp, RET_IF(set_smem(h, k_angular_fwd<KT>, smem_ang_fwd(d))); RET_IF(set_smem(h, k_angular_force<KT>, smem_ang_force(d)));
-              RET_IF(set_smem(h, k_angular_adj<KT>, smem_ang_adj(d))); RET_IF(set_smem(h, k_cgrad_angular<KT>, smem_cgrad_ang(d))));
+  DISPATCH_KT(d.KAp, RET_IF(set_smem(h, k_angular_force<KT>, smem_ang_force(d))); RET_IF(set_smem(h, k_cgrad_angular<KT>, smem_cgrad_ang(d)));
+              DISPATCH_NQ(d.NA, auto kf = k_angular_fwd<KT, NQ>; auto ka = k_angular_adj<KT, NQ>; RET_IF(set_smem(h, kf, smem_ang_fwd(d))); RET_IF(set_smem(h, ka, smem_ang_adj(d)))));
   {   // TMEM budget of one k_net_tc warpgroup (256 columns): D1 + max(D1 corrections, D2 + D2 corrections)
     const NetDims nd = net_dims(d);
     if (nd.NnP + std::max(nd.NnP, 2 * nd.NdN) > 256) return fail(h, GNEP_EINVAL, "model too large for tensor memory (n_neurons, n_descriptors)");
@@ -208,7 +213,7 @@ int enqueue_descriptors(gnep_handle *h) {
   int gridA = cdiv(h->N, GNEP_WARPS);
   DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_fwd<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, smem_radial(d), d, h->N, h->type_s, h->segR, h->pairR, h->theta, h->q, h->M1));
   mark(h, "a1_radial_descriptor");
-  DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_fwd<KT>, cdiv(h->N, ANG_WARPS * ANG_TA), ANG_WARPS * 32, smem_ang_fwd(d), d, h->N, h->type_s, h->segA, h->pairA, h->theta, h->q, h->Sn, h->A1));
+  DISPATCH_KT(d.KAp, DISPATCH_NQ(d.NA, auto kf = k_angular_fwd<KT, NQ>; LAUNCH(h, kf, cdiv(h->N, ANG_WARPS * ANG_TA), ANG_WARPS * 32, smem_ang_fwd(d), d, h->N, h->type_s, h->segA, h->pairA, h->theta, h->q, h->Sn, h->A1)));
   mark(h, "a1_angular_descriptor");
   return GNEP_OK;
 }
@@ -247,7 +252,7 @@ int enqueue_backward(gnep_handle *h) {
   int gridA = cdiv(h->N, GNEP_WARPS);
   DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_adj<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, smem_radial(d), d, h->N, h->type_s, h->struct_s, h->segR, h->pairR, h->theta, h->u, h->omega, h->scales, h->D, h->M2));
   mark(h, "a5_radial_adjoint");
-  DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_adj<KT>, cdiv(h->N, ANG_WARPS * ANG_TA), ANG_WARPS * 32, smem_ang_adj(d), d, h->N, h->type_s, h->struct_s, h->segA, h->atomA, h->pairA, h->theta, h->u, h->omega, h->scales, h->Sn, h->Tn, h->A2, h->D));
+  DISPATCH_KT(d.KAp, DISPATCH_NQ(d.NA, auto ka = k_angular_adj<KT, NQ>; LAUNCH(h, ka, cdiv(h->N, ANG_WARPS * ANG_TA), ANG_WARPS * 32, smem_ang_adj(d), d, h->N, h->type_s, h->struct_s, h->segA, h->atomA, h->pairA, h->theta, h->u, h->omega, h->scales, h->Sn, h->Tn, h->A2, h->D)));
   mark(h, "a5_angular_adjoint");
   LAUNCH(h, k_net_tc<true>, h->n_cta_net, 256, smem_net_bwd(d), d, h->sm, h->theta, h->qscale, h->D, h->x, h->eat, h->Ep, (float *)nullptr,
          h->struct_s, h->e_s, h->scales, h->pbuf, h->gbar);
