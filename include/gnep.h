@@ -138,6 +138,19 @@ int gnep_train_epochs(gnep_handle *h, int32_t n_epochs, float lr, float beta1, f
 int gnep_set_global_norm(gnep_handle *h, int64_t n_atoms_global, int64_t n_structs_global, double l2_share);
 int gnep_set_grad(gnep_handle *h, const float *grad, int is_device);
 
+/* Mini-batch training (the paper's regime is mini-batches of size 1).  A shared handle is a
+ * model of the same spec that SHARES the parent's device-resident parameter vector, gradient, Adam state (m, v, step)
+ * and q_scale, and owns its own resident batch: load one mini-batch into each shared handle once, then step through
+ * them (gnep_train_epochs(h_b, 1, lr(s), ...)) -- every step is one CUDA-graph launch on the parent's stream, nothing
+ * is reloaded, and all handles see the same parameters.  The parent must outlive its shared handles; gnep_set_q_scale /
+ * gnep_set_params on any of them affects all.  EINVAL on a NULL parent. */
+int gnep_create_shared(const gnep_handle *parent, gnep_handle **out);
+
+/* Learning-rate schedule of the paper (Eq.17): linear warm-up from lr_stop to lr_start over n_warmup steps,
+ * then cosine decay back to lr_stop at n_total.  Pure host arithmetic (fp64).  step is clamped to [0, n_total];
+ * EINVAL unless 0 <= n_warmup <= n_total and n_total >= 1. */
+int gnep_lr_schedule(int64_t step, int64_t n_warmup, int64_t n_total, double lr_start, double lr_stop, double *lr);
+
 /* Checkpoint / resume of the optimiser state (m, v: P floats each; either may be NULL). */
 int gnep_get_opt_state(const gnep_handle *h, float *m, float *v, int64_t *step, int is_device);
 int gnep_set_opt_state(gnep_handle *h, const float *m, const float *v, int64_t step, int is_device);

@@ -230,3 +230,15 @@ def adam_step(theta, m, v, grad, step, lr, beta1=0.9, beta2=0.999, eps=1e-8):
     grad = _f64(grad)
     lib().orc_adam_step(theta.size, _p(theta), _p(m), _p(v), _p(grad), int(step), float(lr),
                         float(beta1), float(beta2), float(eps))
+
+
+def lr_schedule(step, n_warmup, n_total, lr_start, lr_stop):
+    """Paper Eq.17 written out: linear warm-up from lr_stop to lr_start over n_warmup steps, then cosine
+    decay back to lr_stop at n_total.  Pinned in tests/test_oracle_schedule.py by its end points, the warm-up slope,
+    the cosine mid-point and monotonicity."""
+    s = min(max(int(step), 0), int(n_total))
+    if s < n_warmup:
+        return lr_stop + s / n_warmup * (lr_start - lr_stop)
+    if n_total == n_warmup:
+        return lr_start
+    return lr_stop + (lr_start - lr_stop) * 0.5 * (1.0 + np.cos(np.pi * (s - n_warmup) / (n_total - n_warmup)))

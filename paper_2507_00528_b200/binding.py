@@ -18,7 +18,8 @@ EXPORTS = ["gnep_create", "gnep_destroy", "gnep_num_params", "gnep_num_descripto
            "gnep_get_params", "gnep_set_q_scale", "gnep_load_batch", "gnep_set_targets", "gnep_neighbor_list",
            "gnep_descriptors", "gnep_predict", "gnep_loss_and_grad", "gnep_adam_step", "gnep_train_epochs",
            "gnep_get_opt_state", "gnep_set_opt_state", "gnep_batch_info", "gnep_launch_count",
-           "gnep_set_profiling", "gnep_phase_times", "gnep_last_error", "gnep_set_global_norm", "gnep_set_grad"]
+           "gnep_set_profiling", "gnep_phase_times", "gnep_last_error", "gnep_set_global_norm", "gnep_set_grad",
+           "gnep_create_shared", "gnep_lr_schedule"]
 
 ERRORS = {-1: "GNEP_EINVAL", -2: "GNEP_ESTATE", -3: "GNEP_ECUDA", -4: "GNEP_ENOMEM", -5: "GNEP_ERANGE",
           -6: "GNEP_ENONFINITE"}
@@ -75,6 +76,8 @@ def load_library(build_if_missing=True):
     L.gnep_batch_info.argtypes = [vp] + [C.POINTER(C.c_int64)] * 4
     L.gnep_set_global_norm.argtypes = [vp, C.c_int64, C.c_int64, C.c_double]
     L.gnep_set_grad.argtypes = [vp, vp, C.c_int]
+    L.gnep_create_shared.argtypes = [vp, C.POINTER(vp)]
+    L.gnep_lr_schedule.argtypes = [C.c_int64, C.c_int64, C.c_int64, C.c_double, C.c_double, C.POINTER(C.c_double)]
     L.gnep_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
     L.gnep_set_profiling.argtypes = [vp, C.c_int]
     L.gnep_phase_times.argtypes = [vp, C.POINTER(C.c_char_p), C.POINTER(C.c_float), C.c_int32, C.POINTER(C.c_int32)]
@@ -261,6 +264,16 @@ class Gnep:
         p, dev, _k = _ptr(grad, np.float32)
         self._ck(self._L.gnep_set_grad(self._h, p, dev))
 
+    # ---- mini-batches: handles that share this model's parameters and optimiser state ----
+    def create_shared(self):
+        """A handle with its own resident batch that shares this model's theta, gradient, Adam state and q_scale
+        (gnep_create_shared).  Keep the parent alive while its shared handles are in use."""
+        child = object.__new__(Gnep)
+        child._L, child._h, child._qs, child.spec = self._L, C.c_void_p(), self._qs, dict(self.spec)
+        child._parent = self
+        self._ck(self._L.gnep_create_shared(self._h, C.byref(child._h)))
+        return child
+
     # ---- profiling ----
     def set_profiling(self, on):
         self._ck(self._L.gnep_set_profiling(self._h, int(on)))
@@ -270,3 +283,13 @@ class Gnep:
         names = (C.c_char_p * cap)(); ms = (C.c_float * cap)(); n = C.c_int32()
         self._ck(self._L.gnep_phase_times(self._h, names, ms, cap, C.byref(n)))
         return [(names[i].decode(), float(ms[i])) for i in range(min(n.value, cap))]
+
+
+def lr_schedule(step, n_warmup, n_total, lr_start, lr_stop):
+    """Paper Eq.17 (linear warm-up, cosine decay) through the library's host function gnep_lr_schedule."""
+    L = load_library()
+    out = C.c_double()
+    rc = L.gnep_lr_schedule(int(step), int(n_warmup), int(n_total), float(lr_start), float(lr_stop), C.byref(out))
+    if rc != 0:
+        raise GnepError(rc, "gnep_lr_schedule: bad arguments")
+    return out.value

@@ -30,6 +30,7 @@ struct gnep_handle {
   DevSpec ds{};
   cudaStream_t stream = nullptr;
   bool own_stream = false;
+  bool shares_state = false;   // gnep_create_shared: theta, grad, m, v, q_scale, step belong to the parent
   mutable std::string err;
   int device = 0;
   int num_sms = 148;
@@ -37,6 +38,7 @@ struct gnep_handle {
   float *theta = nullptr, *grad = nullptr, *m = nullptr, *v = nullptr, *qscale = nullptr;
   long long *step_dev = nullptr;
   float *terms = nullptr, *scales = nullptr;   // device: 5 loss terms, 4 seed multipliers
+  float *lr_dev = nullptr;                     // device: learning rate read by k_adam
   float *h_terms = nullptr;                    // pinned host
   // batch
   bool loaded = false;
@@ -268,8 +270,9 @@ int enqueue_backward(gnep_handle *h) {
   return GNEP_OK;
 }
 
-int enqueue_adam(gnep_handle *h, float lr, float b1, float b2, float eps) {
-  LAUNCH(h, k_adam, cdiv(h->ds.P, 256), 256, 0, h->ds.P, h->theta, h->m, h->v, h->grad, h->step_dev, lr, b1, b2, eps);
+void set_lr(gnep_handle *h, float lr) { LAUNCH(h, k_set_scalar, 1, 1, 0, h->lr_dev, lr); }
+int enqueue_adam(gnep_handle *h, float b1, float b2, float eps) {
+  LAUNCH(h, k_adam, cdiv(h->ds.P, 256), 256, 0, h->ds.P, h->theta, h->m, h->v, h->grad, h->step_dev, h->lr_dev, b1, b2, eps);
   LAUNCH(h, k_step_inc, 1, 1, 0, h->step_dev);
   mark(h, "a9_adam");
   return GNEP_OK;
@@ -393,7 +396,7 @@ int gnep_create(const gnep_model_spec *spec, void *cuda_stream, gnep_handle **ou
   }
   if ((rc = dalloc(h, &h->theta, d.P, false)) || (rc = dalloc(h, &h->grad, d.P, false)) || (rc = dalloc(h, &h->m, d.P, false)) ||
       (rc = dalloc(h, &h->v, d.P, false)) || (rc = dalloc(h, &h->qscale, d.Ndes, false)) || (rc = dalloc(h, &h->step_dev, 1, false)) ||
-      (rc = dalloc(h, &h->terms, 8, false)) || (rc = dalloc(h, &h->scales, 4, false)))
+      (rc = dalloc(h, &h->terms, 8, false)) || (rc = dalloc(h, &h->scales, 4, false)) || (rc = dalloc(h, &h->lr_dev, 1, false)))
     return bail(rc);
   if (cudaMallocHost((void **)&h->h_terms, 8 * sizeof(float)) != cudaSuccess) { h->err = "cudaMallocHost failed"; return bail(GNEP_ENOMEM); }
   std::vector<float> qs(d.Ndes, 1.f);
@@ -417,11 +420,35 @@ int gnep_destroy(gnep_handle *h) {
   if (h->stream) cudaStreamSynchronize(h->stream);
   free_batch(h);
   for (auto &p : h->phases) cudaEventDestroy(p.ev);
-  cudaFree(h->theta); cudaFree(h->grad); cudaFree(h->m); cudaFree(h->v); cudaFree(h->qscale); cudaFree(h->step_dev);
-  cudaFree(h->terms); cudaFree(h->scales);
+  if (!h->shares_state) { cudaFree(h->theta); cudaFree(h->grad); cudaFree(h->m); cudaFree(h->v); cudaFree(h->qscale); cudaFree(h->step_dev); }
+  cudaFree(h->terms); cudaFree(h->scales); cudaFree(h->lr_dev);
   if (h->h_terms) cudaFreeHost(h->h_terms);
   if (h->own_stream && h->stream) cudaStreamDestroy(h->stream);
   delete h;
+  return GNEP_OK;
+}
+
+int gnep_create_shared(const gnep_handle *parent, gnep_handle **out) {
+  if (!parent || !out) return fail(parent, GNEP_EINVAL, "null parent or out");
+  gnep_model_spec s = parent->spec;
+  s.q_scale = nullptr;
+  gnep_handle *h = nullptr;
+  int rc = gnep_create(&s, (void *)parent->stream, &h);
+  if (rc != GNEP_OK) { parent->err = g_create_error; return rc; }
+  cudaFree(h->theta); cudaFree(h->grad); cudaFree(h->m); cudaFree(h->v); cudaFree(h->qscale); cudaFree(h->step_dev);
+  h->theta = parent->theta; h->grad = parent->grad; h->m = parent->m; h->v = parent->v; h->qscale = parent->qscale;
+  h->step_dev = parent->step_dev;
+  h->shares_state = true;
+  *out = h;
+  return GNEP_OK;
+}
+
+int gnep_lr_schedule(int64_t step, int64_t n_warmup, int64_t n_total, double lr_start, double lr_stop, double *lr) {
+  if (!lr || n_total < 1 || n_warmup < 0 || n_warmup > n_total) return GNEP_EINVAL;
+  const int64_t s = step < 0 ? 0 : (step > n_total ? n_total : step);
+  if (s < n_warmup) *lr = lr_stop + (double)s / (double)n_warmup * (lr_start - lr_stop);
+  else if (n_total == n_warmup) *lr = lr_start;
+  else *lr = lr_stop + (lr_start - lr_stop) * 0.5 * (1.0 + std::cos(3.14159265358979323846 * (double)(s - n_warmup) / (double)(n_total - n_warmup)));
   return GNEP_OK;
 }
 
@@ -812,7 +839,8 @@ int gnep_loss_and_grad(gnep_handle *h, float *loss_terms, float *grad, int is_de
 int gnep_adam_step(gnep_handle *h, float lr, float beta1, float beta2, float eps) {
   if (!h) return fail(h, GNEP_EINVAL, "null handle");
   if (!(beta1 >= 0 && beta1 < 1 && beta2 >= 0 && beta2 < 1) || !(eps >= 0)) return fail(h, GNEP_EINVAL, "bad Adam constants");
-  RET_IF(enqueue_adam(h, lr, beta1, beta2, eps));
+  if (h->g_lr != lr) { set_lr(h, lr); h->g_lr = lr; }
+  RET_IF(enqueue_adam(h, beta1, beta2, eps));
   return check_launch(h);
 }
 
@@ -820,7 +848,7 @@ int gnep_train_epochs(gnep_handle *h, int32_t n_epochs, float lr, float beta1, f
   if (!h || n_epochs < 0) return fail(h, GNEP_EINVAL, "bad argument");
   if (!h->loaded) return fail(h, GNEP_ESTATE, "no batch loaded");
   if (!(beta1 >= 0 && beta1 < 1 && beta2 >= 0 && beta2 < 1) || !(eps >= 0)) return fail(h, GNEP_EINVAL, "bad Adam constants");
-  if (h->graph && (h->g_lr != lr || h->g_b1 != beta1 || h->g_b2 != beta2 || h->g_eps != eps)) {
+  if (h->graph && (h->g_b1 != beta1 || h->g_b2 != beta2 || h->g_eps != eps)) {
     cudaGraphExecDestroy(h->graph); h->graph = nullptr;
   }
   if (!h->graph) {
@@ -830,7 +858,7 @@ int gnep_train_epochs(gnep_handle *h, int32_t n_epochs, float lr, float beta1, f
     CK(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
     int rc = enqueue_forward(h);
     if (rc == GNEP_OK) rc = enqueue_backward(h);
-    if (rc == GNEP_OK) rc = enqueue_adam(h, lr, beta1, beta2, eps);
+    if (rc == GNEP_OK) rc = enqueue_adam(h, beta1, beta2, eps);
     cudaError_t e = cudaStreamEndCapture(h->stream, &g);
     h->prof = prof;
     h->graph_launches = h->launches - before;
@@ -840,8 +868,9 @@ int gnep_train_epochs(gnep_handle *h, int32_t n_epochs, float lr, float beta1, f
     e = cudaGraphInstantiate(&h->graph, g, 0);
     cudaGraphDestroy(g);
     if (e != cudaSuccess) { h->graph = nullptr; return fail(h, GNEP_ECUDA, std::string("graph instantiate: ") + cudaGetErrorString(e)); }
-    h->g_lr = lr; h->g_b1 = beta1; h->g_b2 = beta2; h->g_eps = eps;
+    h->g_lr = -1.f; h->g_b1 = beta1; h->g_b2 = beta2; h->g_eps = eps;
   }
+  if (h->g_lr != lr) { set_lr(h, lr); h->g_lr = lr; }   // outside the graph: a schedule only rewrites the device scalar
   for (int i = 0; i < n_epochs; ++i) { CK(cudaGraphLaunch(h->graph, h->stream)); h->launches += h->graph_launches; }
   if (loss_terms) RET_IF(fetch_terms(h, loss_terms));
   return GNEP_OK;

@@ -166,10 +166,11 @@ k_grad_reduce(DevSpec sp, ReduceMap rm, float l2_share, const float *__restrict_
 // a9: textbook Adam with bias correction (Kingma & Ba Alg.1); step counter on the device (graph-safe).
 __global__ void __launch_bounds__(256)
 k_adam(int P, float *__restrict__ theta, float *__restrict__ m, float *__restrict__ v,
-       const float *__restrict__ grad, const long long *__restrict__ step, float lr, float beta1, float beta2,
-       float eps) {
+       const float *__restrict__ grad, const long long *__restrict__ step, const float *__restrict__ lr_p, float beta1,
+       float beta2, float eps) {
   int p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= P) return;
+  const float lr = *lr_p;          // device scalar: a learning-rate schedule changes it without re-building the epoch graph
   double t = (double)(*step + 1);
   float c1 = (float)(1.0 - pow((double)beta1, t)), c2 = (float)(1.0 - pow((double)beta2, t));
   float g = grad[p];
@@ -179,6 +180,7 @@ k_adam(int P, float *__restrict__ theta, float *__restrict__ m, float *__restric
   theta[p] -= lr * (mm / c1) / (sqrtf(vv / c2) + eps);
 }
 __global__ void k_step_inc(long long *step) { *step += 1; }
+__global__ void k_set_scalar(float *dst, float v) { *dst = v; }
 
 // outputs back to the caller's atom order
 __global__ void k_unpermute_force(int N, const int *__restrict__ perm, const float4 *__restrict__ Fat, float *__restrict__ out) {

@@ -1,0 +1,54 @@
+"""Mini-batch training through shared handles + the Eq.17 schedule (paper P:142) against the
+oracle: every mini-batch is its own resident batch on a handle that shares the parent's parameters and Adam state; a
+step is one graph-replayed epoch of that handle at lr(s)."""
+import numpy as np
+import pytest
+
+from cases import labelled_case
+from oracle import gnep_oracle as orc
+
+pytestmark = pytest.mark.gpu
+
+
+def _slice(b, labels, lo, hi):
+    off = b["atom_offsets"]; a0, a1 = off[lo], off[hi]
+    E, F, W = labels
+    return ((off[lo:hi + 1] - a0).astype(off.dtype), b["positions"][a0:a1], b["cells"][lo:hi], b["types"][a0:a1],
+            E[lo:hi], F[a0:a1], W[lo:hi])
+
+
+@pytest.mark.parametrize("config,n_structs,bs", [(1, 6, 2), (0, 4, 1)])
+def test_minibatch_trajectory_matches_oracle(config, n_structs, bs):
+    from paper_2507_00528_b200 import Gnep, lr_schedule
+    spec, sp, b, ob, theta, qs, labels = labelled_case(config, n_structs=n_structs)
+    nb = n_structs // bs
+    epochs, n_warm = 2, 2
+    n_total = epochs * nb
+    parent = Gnep(dict(spec, q_scale=qs))
+    parent.set_params(theta.astype(np.float32))
+    handles, obatches = [], []
+    for k in range(nb):
+        off, pos, cells, types, E, F, W = _slice(b, labels, k * bs, (k + 1) * bs)
+        h = parent if k == 0 else parent.create_shared()
+        h.load_batch(off, pos, cells, types, E, F, W)
+        handles.append(h)
+        o = orc.Batch(sp, off, pos, cells, types); o.set_refs(E, F, W)
+        obatches.append(o)
+    th = theta.copy(); m = np.zeros_like(th); v = np.zeros_like(th)
+    s = 0
+    for _ in range(epochs):
+        for k in range(nb):
+            lr = orc.lr_schedule(s, n_warm, n_total, 1e-3, 1e-5)
+            assert lr_schedule(s, n_warm, n_total, 1e-3, 1e-5) == pytest.approx(lr, rel=1e-14)
+            t_ref, g_ref = orc.loss_and_grad(sp, th, qs, obatches[k])
+            orc.adam_step(th, m, v, g_ref, s + 1, lr)
+            terms = handles[k].train_epochs(1, lr)
+            assert abs(terms[0] - t_ref[0]) <= 2e-5 * abs(t_ref[0])     # the loss the step saw (same parameters so far)
+            s += 1
+    for h in handles:                                                    # every handle sees the same shared state
+        th_gpu = h.get_params().astype(np.float64)
+        assert np.linalg.norm(th_gpu - th) / np.linalg.norm(th) < 1e-4
+        assert h.get_opt_state()[2] == n_total
+    for h in handles[1:]:
+        h.destroy()
+    parent.destroy()
