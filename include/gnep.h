@@ -151,6 +151,12 @@ int gnep_create_shared(const gnep_handle *parent, gnep_handle **out);
  * EINVAL unless 0 <= n_warmup <= n_total and n_total >= 1. */
 int gnep_lr_schedule(int64_t step, int64_t n_warmup, int64_t n_total, double lr_start, double lr_stop, double *lr);
 
+/* Held-out evaluation (paper Fig.2): forward pass only over the resident batch of this
+ * handle -- typically a shared handle holding the test set -- and the three root-mean-square errors against its
+ * references: rmse[0] energy per atom (eV/atom, over structures), rmse[1] force components (eV/A, over atoms x 3),
+ * rmse[2] virial per atom (eV/atom, over structures x 6).  A missing reference gives 0.  rmse: HOST, 3 floats. */
+int gnep_evaluate(gnep_handle *h, float *rmse);
+
 /* Checkpoint / resume of the optimiser state (m, v: P floats each; either may be NULL). */
 int gnep_get_opt_state(const gnep_handle *h, float *m, float *v, int64_t *step, int is_device);
 int gnep_set_opt_state(gnep_handle *h, const float *m, const float *v, int64_t step, int is_device);

@@ -19,7 +19,7 @@ EXPORTS = ["gnep_create", "gnep_destroy", "gnep_num_params", "gnep_num_descripto
            "gnep_descriptors", "gnep_predict", "gnep_loss_and_grad", "gnep_adam_step", "gnep_train_epochs",
            "gnep_get_opt_state", "gnep_set_opt_state", "gnep_batch_info", "gnep_launch_count",
            "gnep_set_profiling", "gnep_phase_times", "gnep_last_error", "gnep_set_global_norm", "gnep_set_grad",
-           "gnep_create_shared", "gnep_lr_schedule"]
+           "gnep_create_shared", "gnep_lr_schedule", "gnep_evaluate"]
 
 ERRORS = {-1: "GNEP_EINVAL", -2: "GNEP_ESTATE", -3: "GNEP_ECUDA", -4: "GNEP_ENOMEM", -5: "GNEP_ERANGE",
           -6: "GNEP_ENONFINITE"}
@@ -77,6 +77,7 @@ def load_library(build_if_missing=True):
     L.gnep_set_global_norm.argtypes = [vp, C.c_int64, C.c_int64, C.c_double]
     L.gnep_set_grad.argtypes = [vp, vp, C.c_int]
     L.gnep_create_shared.argtypes = [vp, C.POINTER(vp)]
+    L.gnep_evaluate.argtypes = [vp, C.POINTER(C.c_float)]
     L.gnep_lr_schedule.argtypes = [C.c_int64, C.c_int64, C.c_int64, C.c_double, C.c_double, C.POINTER(C.c_double)]
     L.gnep_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
     L.gnep_set_profiling.argtypes = [vp, C.c_int]
@@ -273,6 +274,12 @@ class Gnep:
         child._parent = self
         self._ck(self._L.gnep_create_shared(self._h, C.byref(child._h)))
         return child
+
+    def evaluate(self):
+        """(rmse_energy eV/atom, rmse_force eV/A, rmse_virial eV/atom) of the resident batch against its references."""
+        out = (C.c_float * 3)()
+        self._ck(self._L.gnep_evaluate(self._h, out))
+        return np.array(out[:], dtype=np.float32)
 
     # ---- profiling ----
     def set_profiling(self, on):

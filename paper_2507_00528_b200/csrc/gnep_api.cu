@@ -836,6 +836,19 @@ int gnep_loss_and_grad(gnep_handle *h, float *loss_terms, float *grad, int is_de
   return GNEP_OK;
 }
 
+int gnep_evaluate(gnep_handle *h, float *rmse) {
+  if (!h || !rmse) return fail(h, GNEP_EINVAL, "null argument");
+  if (!h->loaded) return fail(h, GNEP_ESTATE, "no batch loaded");
+  float t[5] = {0, 0, 0, 0, 0};
+  if (h->N > 0 || h->S > 0) {
+    RET_IF(enqueue_forward(h));
+    RET_IF(check_launch(h));
+    RET_IF(fetch_terms(h, t));
+  }
+  for (int i = 0; i < 3; ++i) rmse[i] = std::sqrt(std::max(t[1 + i], 0.f));   // t_e, t_f, t_v are the mean squares of Eq.10-12
+  return GNEP_OK;
+}
+
 int gnep_adam_step(gnep_handle *h, float lr, float beta1, float beta2, float eps) {
   if (!h) return fail(h, GNEP_EINVAL, "null handle");
   if (!(beta1 >= 0 && beta1 < 1 && beta2 >= 0 && beta2 < 1) || !(eps >= 0)) return fail(h, GNEP_EINVAL, "bad Adam constants");

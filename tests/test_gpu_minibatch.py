@@ -52,3 +52,30 @@ def test_minibatch_trajectory_matches_oracle(config, n_structs, bs):
     for h in handles[1:]:
         h.destroy()
     parent.destroy()
+
+
+def test_held_out_evaluation_on_a_shared_handle():
+    """gnep_evaluate: RMSEs of a test batch held by a shared handle, with and without a virial reference."""
+    from paper_2507_00528_b200 import Gnep
+    spec, sp, b, ob, theta, qs, labels = labelled_case(1, n_structs=5)
+    parent = Gnep(dict(spec, q_scale=qs))
+    off, pos, cells, types, E, F, W = _slice(b, labels, 0, 3)
+    parent.load_batch(off, pos, cells, types, E, F, W)
+    parent.set_params(theta.astype(np.float32))
+    test = parent.create_shared()
+    off, pos, cells, types, E, F, W = _slice(b, labels, 3, 5)
+    test.load_batch(off, pos, cells, types, E, F, W)
+    o = orc.Batch(sp, off, pos, cells, types); o.set_refs(E, F, W)
+    t_ref, _ = orc.loss_and_grad(sp, theta, qs, o)
+    np.testing.assert_allclose(test.evaluate(), np.sqrt(t_ref[1:4]), rtol=2e-5)
+    # independent restatement from the oracle's predictions: RMSE over structures / atoms x 3 / structures x 6
+    Ep, Fp, Wp = orc.predict(sp, theta, qs, o)
+    ns = np.diff(off)
+    want = [np.sqrt(np.mean(((Ep - E) / ns) ** 2)), np.sqrt(np.mean((Fp - F) ** 2)), np.sqrt(np.mean(((Wp - W) / ns[:, None]) ** 2))]
+    np.testing.assert_allclose(test.evaluate(), want, rtol=2e-5)
+    test.set_targets(E, F, None)
+    r = test.evaluate()
+    assert r[2] == 0.0 and r[0] == pytest.approx(want[0], rel=2e-5)
+    parent.train_epochs(1, 1e-3)                      # training on the parent moves the shared parameters ...
+    assert not np.allclose(test.evaluate()[:2], want[:2], rtol=1e-6)   # ... and the held-out errors with them
+    test.destroy(); parent.destroy()
