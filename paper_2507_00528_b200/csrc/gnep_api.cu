@@ -47,7 +47,9 @@ struct gnep_handle {
   int hasE = 0, hasF = 0, hasV = 0;
   double Ng = -1, Sg = -1, l2_share = 1.0;   // job-wide normalisers when structures are sharded over ranks
   std::vector<void *> batch_allocs;
-  int *perm = nullptr, *type_s = nullptr, *struct_s = nullptr, *segR = nullptr, *rowAs = nullptr, *revA = nullptr, *segA = nullptr, *atomA = nullptr;
+  int *perm = nullptr, *type_s = nullptr, *struct_s = nullptr, *segR = nullptr, *rowAs = nullptr, *segA = nullptr, *atomA = nullptr;
+  int *rowAu = nullptr, *segAu = nullptr, *atomAu = nullptr, *revAu = nullptr;   // unpadded angular list (force + gather kernels)
+  float4 *pairAu = nullptr;
   float4 *pairR = nullptr, *pairA = nullptr;
   int64_t *exp_row[2] = {nullptr, nullptr};
   int *exp_j[2] = {nullptr, nullptr}, *exp_sh[2] = {nullptr, nullptr};
@@ -238,9 +240,9 @@ int enqueue_forward(gnep_handle *h) {
   mark(h, "a2_network_forward");
   DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_force<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, 0, d, h->N, h->type_s, h->segR, h->pairR, h->etil, h->Fat, h->Wat));
   mark(h, "a3_radial_force");
-  DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_force<KT>, cdiv(h->N, ANG_WARPS * FRC_TA), ANG_WARPS * 32, smem_ang_force(d), d, h->N, h->type_s, h->segA, h->atomA, h->pairA, h->theta, h->Ep, h->Sn, h->fpair));
+  DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_force<KT>, cdiv(h->N, ANG_WARPS * FRC_TA), ANG_WARPS * 32, smem_ang_force(d), d, h->N, h->type_s, h->segAu, h->atomAu, h->pairAu, h->theta, h->Ep, h->Sn, h->fpair));
   mark(h, "a3_angular_force");
-  LAUNCH(h, k_force_gather, cdiv((int64_t)h->N * 16, 256), 256, 0, h->N, d.T + 1, h->segA, h->revA, h->pairA, h->fpair, h->Fat, h->Wat);
+  LAUNCH(h, k_force_gather, cdiv((int64_t)h->N * 16, 256), 256, 0, h->N, d.T + 1, h->segAu, h->revAu, h->pairAu, h->fpair, h->Fat, h->Wat);
   mark(h, "a3_force_gather");
   LAUNCH(h, k_struct_reduce, h->S, 128, 0, loss_cfg(h), h->srange, h->Ei, h->Fat, h->Wat, h->Eref, h->Fref_s, h->Wref, h->Es, h->Ws, h->e_s, h->u, h->omega, h->parts);
   LAUNCH(h, k_loss_final, 1, 256, 0, loss_cfg(h), h->parts, h->theta, h->terms, h->scales);
@@ -642,10 +644,11 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     BA(h->srange, srange.size()); BA(h->Eref, S); BA(h->Wref, (size_t)S * 6); BA(h->Fref_s, (size_t)N * 3);
     // the angular list is first built unpadded (u) and then copied into its final layout, in which every (atom, J)
     // segment is padded to a multiple of 4 pairs with zero-contribution dummies (k_pad_angular)
-    int *d_rowRs, *d_shA, *d_rowAu, *d_segAu, *d_atomAu; unsigned long long *d_ekey; float *d_er; float4 *d_pairAu;
+    // (the unpadded list stays resident: the force and gather kernels, lane = pair, have no use for the dummies)
+    int *d_rowRs, *d_shA; unsigned long long *d_ekey; float *d_er;
     CKT(talloc((void **)&d_rowRs, sizeof(int) * (N + 1))); CKT(talloc((void **)&d_shA, sizeof(int) * nA));
-    CKT(talloc((void **)&d_rowAu, sizeof(int) * (N + 1))); CKT(talloc((void **)&d_segAu, sizeof(int) * ((size_t)N * (T + 1) + 1)));
-    CKT(talloc((void **)&d_atomAu, sizeof(int) * nA)); CKT(talloc((void **)&d_pairAu, sizeof(float4) * nA));
+    BA(h->rowAu, N + 1); BA(h->segAu, (size_t)N * (T + 1) + 1); BA(h->atomAu, nA); BA(h->pairAu, nA); BA(h->revAu, nA);
+    int *d_rowAu = h->rowAu, *d_segAu = h->segAu, *d_atomAu = h->atomAu; float4 *d_pairAu = h->pairAu;
     CKT(talloc((void **)&d_ekey, sizeof(unsigned long long) * nR)); CKT(talloc((void **)&d_er, sizeof(float) * 3 * nR));
     CKT(cudaMemcpyAsync(h->exp_row[0], rowR.data(), sizeof(int64_t) * (N + 1), cudaMemcpyHostToDevice, st));
     CKT(cudaMemcpyAsync(h->exp_row[1], rowA.data(), sizeof(int64_t) * (N + 1), cudaMemcpyHostToDevice, st));
@@ -676,14 +679,12 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     rowAs[N] = (int)nAp;
     if (nAp >= (int64_t)1 << 31) { tfree(); free_batch(h); return fail(h, GNEP_ERANGE, "2^31 or more (padded) angular pairs"); }
     h->nAp = nAp;
-    int *d_shAp;
-    CKT(talloc((void **)&d_shAp, sizeof(int) * nAp));
-    BA(h->revA, nAp); BA(h->atomA, nAp); BA(h->pairA, nAp);
+    BA(h->atomA, nAp); BA(h->pairA, nAp);
     CKT(cudaMemcpyAsync(h->rowAs, rowAs.data(), sizeof(int) * (N + 1), cudaMemcpyHostToDevice, st));
     CKT(cudaMemcpyAsync(h->segA, segAp.data(), sizeof(int) * ((size_t)N * (T + 1) + 1), cudaMemcpyHostToDevice, st));
-    LAUNCH(h, k_pad_angular, cdiv((int64_t)N * 32, 256), 256, 0, N, T, d_segAu, h->segA, d_pairAu, d_shA, h->pairA, d_shAp, h->atomA,
+    LAUNCH(h, k_pad_angular, cdiv((int64_t)N * 32, 256), 256, 0, N, T, d_segAu, h->segA, d_pairAu, h->pairA, h->atomA,
            (float)(2.0 * h->spec.rc_angular));
-    LAUNCH(h, k_nbr_reverse, cdiv((int64_t)N * 32, 256), 256, 0, N, h->rowAs, h->pairA, d_shAp, h->revA);
+    LAUNCH(h, k_nbr_reverse, cdiv((int64_t)N * 32, 256), 256, 0, N, h->rowAu, h->pairAu, d_shA, h->revAu);
     CKT(cudaGetLastError());
     CKT(cudaStreamSynchronize(st));
     tfree();
@@ -720,7 +721,7 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     BA(h->q, npad * d.Ndes); BA(h->Sn, n * d.NA * GNEP_NLM); BA(h->x, npad * d.Nn); BA(h->Ei, n); BA(h->Ep, n * d.Ndes);
     BA(h->etil, n * T * d.KRp); BA(h->M1, n * T * d.KRp); BA(h->M2, n * T * d.KRp); BA(h->D, npad * d.Ndes); BA(h->Tn, n * d.NA * GNEP_NLM); BA(h->A1, n * T * d.KAp * GNEP_NLM); BA(h->A2, n * T * d.KAp * GNEP_NLM);
     BA(h->gbar, n * d.Ndes); BA(h->pbuf, npad * d.Nn); BA(h->eat, npad); BA(h->Wat, n * 6);
-    BA(h->Fat, n); BA(h->fpair, h->nAp); BA(h->u, n);
+    BA(h->Fat, n); BA(h->fpair, h->nA); BA(h->u, n);
     BA(h->Es, S); BA(h->Ws, (size_t)S * 6); BA(h->parts, (size_t)S * 3); BA(h->e_s, S); BA(h->omega, (size_t)S * 6);
     BA(h->partialCR, (size_t)std::max(h->n_chunks, 1) * d.NR * T * d.KRp);
     BA(h->partialCA, (size_t)std::max(h->rm.n_warps_ca, 1) * T * T * d.NA * d.KAp);

@@ -213,22 +213,21 @@ __global__ void k_nbr_scatter(int N, int T, const int *__restrict__ struct_of, c
 
 // Final layout of the internal angular list: every (atom, J) segment is padded to a multiple of 4 pairs so that the
 // 4-pair register tiles of the angular kernels never straddle a segment.  A dummy is float4(2 rcA, 0, 0, bits(a))
-// with the zero shift: the basis functions clamp d / rc at 1, where f_k = f_k' = 0 exactly, so a dummy contributes
-// exactly nothing anywhere; its reverse pair is a dummy of the same row.  Warp per atom.
+// : the basis functions clamp d / rc at 1, where f_k = f_k' = 0 exactly, so a dummy contributes exactly nothing.
+// Only the two moment sweeps use the padded list; the force and gather kernels (lane = pair) keep the unpadded one.
+// Warp per atom.
 __global__ void k_pad_angular(int N, int T, const int *__restrict__ segAu, const int *__restrict__ segAp,
-                              const float4 *__restrict__ pairAu, const int *__restrict__ shAu,
-                              float4 *__restrict__ pairA, int *__restrict__ shA, int *__restrict__ atomA, float rdummy) {
+                              const float4 *__restrict__ pairAu, float4 *__restrict__ pairA, int *__restrict__ atomA,
+                              float rdummy) {
   int a = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   int lane = threadIdx.x & 31;
   if (a >= N) return;
-  const int zero_shift = (128 << 16) | (128 << 8) | 128;
   for (int J = 0; J < T; ++J) {
     const int s0 = segAu[a * (T + 1) + J], n = segAu[a * (T + 1) + J + 1] - s0;
     const int d0 = segAp[a * (T + 1) + J], np = segAp[a * (T + 1) + J + 1] - d0;
     for (int e = lane; e < np; e += 32) {
       const bool real = e < n;
       pairA[d0 + e] = real ? pairAu[s0 + e] : make_float4(rdummy, 0.f, 0.f, __int_as_float(a));
-      shA[d0 + e] = real ? shAu[s0 + e] : zero_shift;
       atomA[d0 + e] = a;
     }
   }
