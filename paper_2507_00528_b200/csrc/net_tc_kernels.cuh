@@ -599,12 +599,15 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, int nraw, const float *__restrict__ theta,
       if (i_kind[j] == 1 && col == 0) i_kind[j] = 3;
     }
     const int e_off = 2 * GW_KS * (sp.Nn + sp.Ndes);
+    int nfl = 0;                                        // accumulation groups already added to the registers
     for (int it = 0; it < nst; ++it) {
       const int st = it % GW_OPST, use = it / GW_OPST, g = it / GW_FLUSH, gi = it - g * GW_FLUSH;
       const int rs = it % nraw, ruse = it / nraw;
       float *sb = smem + st * stage_fl;
       const float *rb = raw + rs * raw_fl;
-      if (gi == 0 && g >= 1) flush(g - 1);
+      // group g - 1 is added to the registers one stage late (at the second stage of group g), so that its last
+      // MMAs have finished by then; its TMEM set is not written again before group g + 1
+      if (gi == (GW_FLUSH > 1 ? 1 : 0) && nfl < g) { flush(nfl); ++nfl; }
       const int a0 = w0 + it * GW_KS;
       const int vlo = c0 - a0, vhi = c1 - a0;         // atoms [vlo, vhi) of the window belong to this CTA
       const bool whole = vlo <= 0 && vhi >= GW_KS;
@@ -653,7 +656,7 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, int nraw, const float *__restrict__ theta,
       mbar_arrive(full + st);
       mbar_arrive(rempty + rs);
     }
-    if (ngroups > 0) flush(ngroups - 1);
+    for (; nfl < ngroups; ++nfl) flush(nfl);
     esh[tid] = esum;
     // results: row mu lives in threads mu and 128 + mu
     asm volatile("bar.sync 1, %0;" ::"n"(GW_PROD) : "memory");
