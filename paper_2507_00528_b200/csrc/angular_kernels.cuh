@@ -64,40 +64,43 @@ __device__ __forceinline__ void split_sums(const NLane &nl, const float (&w)[8],
   for (int i = 0; i < 8; ++i) { if (i < nl.split) sa += w[i]; else sb += w[i]; }
 }
 
-// Epilogue contraction X = c . A (S = c.A1, T = c.A2) without a second pass over shared memory: when a segment's
-// register tile acc[KQ][3] (k in the lane's quarter, 3 lm) is complete, the lane adds its part
-//   Xp[n][i] += sum_r c[I][J][n][k_r] acc[r][i]
-// for all n; at the end of the atom the four k-quarters are summed by two butterfly shuffles and X[n][lm] goes to
-// shared memory once (Xs[n][24]) for the per-(n, l) contractions.  (The straightforward form re-reads the whole
-// moment matrix from shared memory for every n-group and made the sweeps shared-memory-bandwidth bound.)
-template <int KT, int KQ, int NQ>
-__device__ __forceinline__ void xpart_add(const DevSpec &sp, const float *ct, int I, int J, int kq, const float (&acc)[KQ][3],
-                                          float (&Xp)[NQ][3]) {
+// Epilogue contraction X = c . A (S = c.A1, T = c.A2) without a second pass over shared memory.  When a segment's
+// register tile acc[KQ][3] (k in the lane's quarter kq, 3 lm) is complete, the four lanes (kq = 0..3) that share the
+// same 3 lm exchange their tiles by shuffles, so that each holds A[all k][its 3 lm]; lane kq then owns the functions
+// n = kq, kq + 4, ... and adds  Xo[j][i] += sum_k c[I][J][n_j][k] A[k][lm_i].  At the end of the atom X[n][lm] goes to
+// shared memory once (Xs[n][24]) for the per-(n, l) contractions.  (Re-reading the moment matrix from shared memory for
+// every n-group, or summing partial X over the k-quarters by butterflies, both cost more instructions.)
+template <int KT, int KQ, int NJ>
+__device__ __forceinline__ void xown_add(const DevSpec &sp, const float *ct, int I, int J, int lane, int kq,
+                                         const float (&acc)[KQ][3], float (&Xo)[NJ][3]) {
 #pragma unroll
-  for (int r = 0; r < KQ; ++r) {
-    const int k = kq * KQ + r;
-    if (k < KT) {
-      const float *cp = ct + ((I * sp.T + J) * KT + k) * ANG_NQ;
+  for (int d = 0; d < 4; ++d) {
+    const int kb = ((kq + d) & 3) * KQ;             // first k of the tile held by lane kq + d
 #pragma unroll
-      for (int n = 0; n < NQ; ++n) {
-        const float c = cp[n];                      // zero for n >= NA (zero-padded table)
+    for (int r = 0; r < KQ; ++r) {
+      float a[3];
 #pragma unroll
-        for (int i = 0; i < 3; ++i) Xp[n][i] = fmaf(c, acc[r][i], Xp[n][i]);
+      for (int i = 0; i < 3; ++i) a[i] = d == 0 ? acc[r][i] : __shfl_sync(0xffffffffu, acc[r][i], (lane + 8 * d) & 31);
+      if (kb + r < KT) {
+        const float *cp = ct + ((I * sp.T + J) * KT + kb + r) * ANG_NQ + kq;
+#pragma unroll
+        for (int j = 0; j < NJ; ++j) {
+          const float c = cp[4 * j];                // n = kq + 4 j; zero beyond NA (zero-padded table)
+#pragma unroll
+          for (int i = 0; i < 3; ++i) Xo[j][i] = fmaf(c, a[i], Xo[j][i]);
+        }
       }
     }
   }
 }
-template <int NQ>
-__device__ __forceinline__ void xpart_finish(int kq, int lmq, float (&Xp)[NQ][3], float *Xs) {
+template <int NJ>
+__device__ __forceinline__ void xown_store(int kq, int lmq, float (&Xo)[NJ][3], float *Xs) {
 #pragma unroll
-  for (int n = 0; n < NQ; ++n)
+  for (int j = 0; j < NJ; ++j)
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
-      float v = Xp[n][i];
-      v += __shfl_xor_sync(0xffffffffu, v, 8);
-      v += __shfl_xor_sync(0xffffffffu, v, 16);
-      if ((n & 3) == kq) Xs[n * GNEP_NLM + 3 * lmq + i] = v;
-      Xp[n][i] = 0.f;
+      Xs[(kq + 4 * j) * GNEP_NLM + 3 * lmq + i] = Xo[j][i];     // rows up to 4 NJ - 1 <= ANG_NQ - 1 exist
+      Xo[j][i] = 0.f;
     }
   __syncwarp();
 }
@@ -136,18 +139,19 @@ k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   for (int r = 0; r < KQ; ++r)
 #pragma unroll
     for (int i = 0; i < 3; ++i) acc[r][i] = 0.f;
-  float Xp[NQ][3];
+  constexpr int NJ = (NQ + 3) / 4;
+  float Xo[NJ][3];
 #pragma unroll
-  for (int n = 0; n < NQ; ++n)
+  for (int j = 0; j < NJ; ++j)
 #pragma unroll
-    for (int i = 0; i < 3; ++i) Xp[n][i] = 0.f;
+    for (int i = 0; i < 3; ++i) Xo[j][i] = 0.f;
   for (int x = lane; x < (a_hi - a_lo) * sp.T; x += 32) sEnd[x] = segA[(a_lo + x / sp.T) * T1 + x % sp.T + 1];
   __syncwarp();
   int a = a_lo, J = 0;
   int seg_end = sEnd[0];
 
   auto flush_segment = [&]() {   // accumulators of (a, J) -> S partial sums and shared As, then reset
-    xpart_add<KT, KQ, NQ>(sp, ct, type_s[a], J, kq, acc, Xp);
+    xown_add<KT, KQ, NJ>(sp, ct, type_s[a], J, lane, kq, acc, Xo);
 #pragma unroll
     for (int r = 0; r < KQ; ++r) {
       int k = kq * KQ + r;
@@ -161,7 +165,7 @@ k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   auto atom_epilogue = [&]() {   // A1 -> global, S = c.A1, q_nl, q4 of atom a
     __syncwarp();
     for (int x = lane; x < nA / 4; x += 32) ((float4 *)(A1 + (size_t)a * nA))[x] = ((const float4 *)As)[x];
-    xpart_finish<NQ>(kq, lmq, Xp, Xs);
+    xown_store<NJ>(kq, lmq, Xo, Xs);
     float *Sa = S + (size_t)a * sp.NA * GNEP_NLM;
     float *qa = q + (size_t)a * sp.Ndes + sp.NR;
     for (int nb = 0; nb < sp.NA; nb += 10) {
@@ -286,18 +290,19 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   for (int r = 0; r < KQ; ++r)
 #pragma unroll
     for (int i = 0; i < 3; ++i) acc[r][i] = 0.f;
-  float Xp[NQ][3];
+  constexpr int NJ = (NQ + 3) / 4;
+  float Xo[NJ][3];
 #pragma unroll
-  for (int n = 0; n < NQ; ++n)
+  for (int j = 0; j < NJ; ++j)
 #pragma unroll
-    for (int i = 0; i < 3; ++i) Xp[n][i] = 0.f;
+    for (int i = 0; i < 3; ++i) Xo[j][i] = 0.f;
   for (int x = lane; x < (a_hi - a_lo) * sp.T; x += 32) sEnd[x] = segA[(a_lo + x / sp.T) * T1 + x % sp.T + 1];
   __syncwarp();
   int a = a_lo, J = 0;
   int seg_end = sEnd[0];
 
   auto flush_segment = [&]() {
-    xpart_add<KT, KQ, NQ>(sp, ct, type_s[a], J, kq, acc, Xp);
+    xown_add<KT, KQ, NJ>(sp, ct, type_s[a], J, lane, kq, acc, Xo);
 #pragma unroll
     for (int r = 0; r < KQ; ++r) {
       int k = kq * KQ + r;
@@ -311,7 +316,7 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   auto atom_epilogue = [&]() {   // A2 -> global, T = c.A2, D of atom a
     __syncwarp();
     for (int x = lane; x < nA / 4; x += 32) ((float4 *)(A2 + (size_t)a * nA))[x] = ((const float4 *)As)[x];
-    xpart_finish<NQ>(kq, lmq, Xp, Xs);
+    xown_store<NJ>(kq, lmq, Xo, Xs);
     const float *Sa = S + (size_t)a * sp.NA * GNEP_NLM;
     float *Ta = Tn + (size_t)a * sp.NA * GNEP_NLM;
     float *Da = D + (size_t)a * sp.Ndes + sp.NR;
