@@ -22,17 +22,23 @@
 #define ANG_NQ 16        // n padded to 16 in the transposed coefficient table
 #define ANG_SEGS (ANG_TA * GNEP_MAX_SPECIES_C)   // (atom, J) segments of a warp tile
 
-// transposed coefficients ct[((I*T+J)*KT + k)*ANG_NQ + n] (zero padded) for the S/T/Gamma contractions
+// coefficients for the S/T contractions, ct[(((I*T+J)*KT + k)*4 + q)*4 + j] = c[I][J][n = q + 4 j][k] (zero padded):
+// the functions n = q, q + 4, q + 8, q + 12 owned by one lane are one 16-byte load
 __device__ __forceinline__ void stage_coeff_t(float *dst, const float *src, int T, int NA, int K, int KT) {
   int tot = T * T * KT * ANG_NQ;
   for (int x = threadIdx.x; x < tot; x += blockDim.x) {
-    int n = x % ANG_NQ, r = x / ANG_NQ;
+    int j = x & 3, q = (x >> 2) & 3, r = x / ANG_NQ;
+    int n = q + 4 * j;
     int k = r % KT, ij = r / KT;
     dst[x] = (n < NA && k < K) ? src[(ij * NA + n) * K + k] : 0.f;
   }
 }
 
 __device__ __forceinline__ float dot4(const float4 &a, const float4 &b) { return a.x * b.x + a.y * b.y + a.z * b.z + a.w * b.w; }
+// acc += a . b as one FMA chain
+__device__ __forceinline__ void fma4(float &acc, const float4 &a, const float4 &b) {
+  acc = fmaf(a.x, b.x, acc); acc = fmaf(a.y, b.y, acc); acc = fmaf(a.z, b.z, acc); acc = fmaf(a.w, b.w, acc);
+}
 
 // Per-atom lane layout "(n, lmg)": lane = 3*nq + lmg (lanes 0..29), n = nb + nq for nb = 0, 10, ..., and the lane owns
 // lm in [8 lmg, 8 lmg + 8): lmg 0 = all of l=1 (i<3) and l=2; lmg 1 = all of l=3 (i<7) and the first slot of l=4;
@@ -82,13 +88,12 @@ __device__ __forceinline__ void xown_add(const DevSpec &sp, const float *ct, int
 #pragma unroll
       for (int i = 0; i < 3; ++i) a[i] = d == 0 ? acc[r][i] : __shfl_sync(0xffffffffu, acc[r][i], (lane + 8 * d) & 31);
       if (kb + r < KT) {
-        const float *cp = ct + ((I * sp.T + J) * KT + kb + r) * ANG_NQ + kq;
+        const float4 c4 = *(const float4 *)(ct + ((I * sp.T + J) * KT + kb + r) * ANG_NQ + 4 * kq);   // n = kq + 4 j
+        const float cv[4] = {c4.x, c4.y, c4.z, c4.w};                                                // zero beyond NA
 #pragma unroll
-        for (int j = 0; j < NJ; ++j) {
-          const float c = cp[4 * j];                // n = kq + 4 j; zero beyond NA (zero-padded table)
+        for (int j = 0; j < NJ; ++j)
 #pragma unroll
-          for (int i = 0; i < 3; ++i) Xo[j][i] = fmaf(c, a[i], Xo[j][i]);
-        }
+          for (int i = 0; i < 3; ++i) Xo[j][i] = fmaf(cv[j], a[i], Xo[j][i]);
       }
     }
   }
@@ -419,7 +424,7 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
           float4 X = *(const float4 *)(sX + (3 * lmq + i) * ANG_LD + 4 * g);
           float4 Y = *(const float4 *)(sY + (3 * lmq + i) * ANG_LD + 4 * g);
 #pragma unroll
-          for (int r = 0; r < KQ; ++r) acc[r][i] += dot4(f1[r], X) + dot4(f2[r], Y);
+          for (int r = 0; r < KQ; ++r) { fma4(acc[r][i], f1[r], X); fma4(acc[r][i], f2[r], Y); }
         }
       }
       pos = hi;
