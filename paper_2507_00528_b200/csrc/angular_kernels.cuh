@@ -155,8 +155,10 @@ k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   int a = a_lo, J = 0;
   int seg_end = sEnd[0];
 
+  int Icur = type_s[a_lo];       // species of atom a, requested when the previous atom ends
+  auto next_atom = [&]() { if (a < a_hi) Icur = type_s[a]; };
   auto flush_segment = [&]() {   // accumulators of (a, J) -> S partial sums and shared As, then reset
-    xown_add<KT, KQ, NJ>(sp, ct, type_s[a], J, lane, kq, acc, Xo);
+    xown_add<KT, KQ, NJ>(sp, ct, Icur, J, lane, kq, acc, Xo);
 #pragma unroll
     for (int r = 0; r < KQ; ++r) {
       int k = kq * KQ + r;
@@ -204,7 +206,7 @@ k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   };
   auto next_segment = [&]() {
     flush_segment();
-    if (++J == sp.T) { atom_epilogue(); J = 0; ++a; }
+    if (++J == sp.T) { atom_epilogue(); J = 0; ++a; next_atom(); }
     seg_end = a < a_hi ? sEnd[(a - a_lo) * sp.T + J] : 0x7fffffff;
   };
 
@@ -306,8 +308,21 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   int a = a_lo, J = 0;
   int seg_end = sEnd[0];
 
+  int Icur = type_s[a_lo];       // species of atom a, requested when the previous atom ends
+  // S of atom a in the (n, lmg) lane layout of the epilogue (first n-round), requested when the previous atom ends
+  float4 sn0 = make_float4(0.f, 0.f, 0.f, 0.f), sn1 = sn0;
+  auto next_atom = [&]() {
+    if (a < a_hi) {
+      Icur = type_s[a];
+      if (nl.act && nl.nq < sp.NA) {
+        const float *Sa_ = S + (size_t)a * sp.NA * GNEP_NLM + nl.nq * GNEP_NLM + 8 * nl.lmg;
+        sn0 = *(const float4 *)Sa_; sn1 = *(const float4 *)(Sa_ + 4);
+      }
+    }
+  };
+  next_atom();
   auto flush_segment = [&]() {
-    xown_add<KT, KQ, NJ>(sp, ct, type_s[a], J, lane, kq, acc, Xo);
+    xown_add<KT, KQ, NJ>(sp, ct, Icur, J, lane, kq, acc, Xo);
 #pragma unroll
     for (int r = 0; r < KQ; ++r) {
       int k = kq * KQ + r;
@@ -330,7 +345,8 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
       const bool on = nl.act && n < sp.NA;
       float tv[8], sv[8], da = 0.f, db = 0.f;
       if (on) {
-        float4 s0 = *(const float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg), s1 = *(const float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg + 4);
+        float4 s0 = sn0, s1 = sn1;
+        if (nb > 0) { s0 = *(const float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg); s1 = *(const float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg + 4); }
         sv[0] = s0.x; sv[1] = s0.y; sv[2] = s0.z; sv[3] = s0.w; sv[4] = s1.x; sv[5] = s1.y; sv[6] = s1.z; sv[7] = s1.w;
         {
           const float4 t0 = *(const float4 *)(Xs + n * GNEP_NLM + 8 * nl.lmg), t1 = *(const float4 *)(Xs + n * GNEP_NLM + 8 * nl.lmg + 4);
@@ -362,7 +378,7 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
   };
   auto next_segment = [&]() {
     flush_segment();
-    if (++J == sp.T) { atom_epilogue(); J = 0; ++a; }
+    if (++J == sp.T) { atom_epilogue(); J = 0; ++a; next_atom(); }
     seg_end = a < a_hi ? sEnd[(a - a_lo) * sp.T + J] : 0x7fffffff;
   };
 
