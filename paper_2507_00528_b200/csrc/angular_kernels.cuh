@@ -475,41 +475,56 @@ k_angular_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__
   const int T1 = sp.T + 1;
   const int P_lo = segA[a_lo * T1], P_hi = segA[(a_hi - 1) * T1 + sp.T];
   if (P_lo == P_hi) return;
-  {   // beta_nlm = E'_(n,l) 2C_lm S_nlm (+ E'_4 kappa4 dP4/ds_m), (n, lmg) lane layout
+  {   // beta_nlm = E'_(n,l) 2C_lm S_nlm (+ E'_4 kappa4 dP4/ds_m), (n, lmg) lane layout; the inputs of the next
+      // (atom, n-round) are requested before the current one is worked on
     const NLane nl = make_nlane(lane);
-    for (int a = a_lo; a < a_hi; ++a) {
-      const float *Sa = S + (size_t)a * nb, *Epa = Ep + (size_t)a * sp.Ndes;
-      for (int n0 = 0; n0 < sp.NA; n0 += 10) {
-        const int n = n0 + nl.nq;
-        if (nl.act && n < sp.NA) {
-          float4 s0 = *(const float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg), s1 = *(const float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg + 4);
-          float sv[8] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w}, bv[8];
-          const float ea = desc_of(sp, Epa, nl.la, n), eb = desc_of(sp, Epa, nl.lb, n);
+    const int rounds = (sp.NA + 9) / 10, nit = (a_hi - a_lo) * rounds;
+    float4 s0n = make_float4(0.f, 0.f, 0.f, 0.f), s1n = s0n;
+    float ean = 0.f, ebn = 0.f, e4n = 0.f;
+    auto request = [&](int it) {
+      const int a = a_lo + it / rounds, n = (it % rounds) * 10 + nl.nq;
+      if (it < nit && nl.act && n < sp.NA) {
+        const float *Sa = S + (size_t)a * nb + n * GNEP_NLM + 8 * nl.lmg, *Epa = Ep + (size_t)a * sp.Ndes;
+        s0n = *(const float4 *)Sa; s1n = *(const float4 *)(Sa + 4);
+        ean = desc_of(sp, Epa, nl.la, n); ebn = desc_of(sp, Epa, nl.lb, n);
+        if (sp.use4 && nl.lmg == 0) e4n = Epa[sp.NR + sp.L * sp.NA + n];
+      }
+    };
+    request(0);
+    for (int it = 0; it < nit; ++it) {
+      const int al = it / rounds, n = (it % rounds) * 10 + nl.nq;
+      const float4 s0 = s0n, s1 = s1n;
+      const float ea = ean, eb = ebn, e4 = c_kappa4 * e4n;
+      request(it + 1);
+      if (nl.act && n < sp.NA) {
+        float sv[8] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w}, bv[8];
 #pragma unroll
-          for (int i = 0; i < 8; ++i) bv[i] = (i < nl.split ? ea : eb) * nl.c2[i] * sv[i];
-          if (sp.use4 && nl.lmg == 0) {
-            float g4[5];
-            p4_grad(sv + 3, g4);
-            const float e4 = c_kappa4 * Epa[sp.NR + sp.L * sp.NA + n];
+        for (int i = 0; i < 8; ++i) bv[i] = (i < nl.split ? ea : eb) * nl.c2[i] * sv[i];
+        if (sp.use4 && nl.lmg == 0) {
+          float g4[5];
+          p4_grad(sv + 3, g4);
 #pragma unroll
-            for (int m = 0; m < 5; ++m) bv[3 + m] += e4 * g4[m];
-          }
-          float *dst = beta + (a - a_lo) * nb + n * GNEP_NLM + 8 * nl.lmg;
-          *(float4 *)dst = make_float4(bv[0], bv[1], bv[2], bv[3]);
-          *(float4 *)(dst + 4) = make_float4(bv[4], bv[5], bv[6], bv[7]);
+          for (int m = 0; m < 5; ++m) bv[3 + m] += e4 * g4[m];
         }
+        float *dst = beta + al * nb + n * GNEP_NLM + 8 * nl.lmg;
+        *(float4 *)dst = make_float4(bv[0], bv[1], bv[2], bv[3]);
+        *(float4 *)(dst + 4) = make_float4(bv[4], bv[5], bv[6], bv[7]);
       }
     }
   }
   __syncwarp();
+  // atomA packs (central atom | neighbour species << 28 | central species << 30); the next chunk's record is in flight
+  float4 rn = make_float4(1.f, 0.f, 0.f, 0.f);
+  int an = 0;
+  if (P_lo + lane < P_hi) { rn = pairA[P_lo + lane]; an = atomA[P_lo + lane]; }
   for (int p = P_lo + lane; p < P_hi; p += 32) {
-    float4 r = pairA[p];
-    const int a = atomA[p];
-    const int I = type_s[a];
+    const float4 r = rn;
+    const unsigned packed = (unsigned)an;
+    if (p + 32 < P_hi) { rn = pairA[p + 32]; an = atomA[p + 32]; }
+    const int a = (int)(packed & 0x0fffffffu), J = (int)((packed >> 28) & 3u), I = (int)(packed >> 30);
     const float *be = beta + (a - a_lo) * nb;
     float d, rinv;
     pair_len(r.x * r.x + r.y * r.y + r.z * r.z, d, rinv);
-    int J = type_s[__float_as_int(r.w)];
     float f[KT], fp[KT];
     cheb_ffp<KT>(d, sp.rcAinv, f, fp);
     const float *c = cs + (I * sp.T + J) * sp.NA * KT;

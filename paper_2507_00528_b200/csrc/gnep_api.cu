@@ -631,6 +631,7 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     std::vector<int64_t> rowR(N + 1, 0), rowA(N + 1, 0);
     for (int i = 0; i < N; ++i) { rowR[i + 1] = rowR[i] + cR[i]; rowA[i + 1] = rowA[i] + cA[i]; }
     const int64_t nR = rowR[N], nA = rowA[N];
+    if (N >= (1 << 28)) { tfree(); free_batch(h); return fail(h, GNEP_ERANGE, "2^28 or more atoms"); }
     if (nR >= (int64_t)1 << 31) { tfree(); free_batch(h); return fail(h, GNEP_ERANGE, "2^31 or more radial pairs"); }
     std::vector<int> rowRs(N + 1, 0), rowAs(N + 1, 0);
     for (int a = 0; a < N; ++a) { rowRs[a + 1] = rowRs[a] + cR[perm[a]]; rowAs[a + 1] = rowAs[a] + cA[perm[a]]; }

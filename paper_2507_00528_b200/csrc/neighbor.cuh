@@ -185,7 +185,7 @@ __global__ void k_nbr_scatter(int N, int T, const int *__restrict__ struct_of, c
       expA_j[baseA + rankCA] = j; expA_sh[baseA + rankCA] = sh;
       pairA[baseAs + rankIA] = rec;
       shA[baseAs + rankIA] = sh;
-      atomA[baseAs + rankIA] = a;
+      atomA[baseAs + rankIA] = a | (J << 28) | (type[i] << 30);   // central atom, neighbour species, central species
       cntJA[J] += 1;
     }
     cntJ[J] += 1;
