@@ -91,6 +91,27 @@ __device__ __forceinline__ void store_row4(float *__restrict__ row, int W, int c
   if (c + 3 < W) row[c + 3] = v.w;
 }
 
+// 8 consecutive values of a row (32-byte aligned, row length a multiple of 8): one 256-bit access -- half as many
+// requests as two 128-bit ones, which is what the row-per-thread pattern pays for (32 different lines per request)
+struct float8 { float4 lo, hi; };
+__device__ __forceinline__ float8 ldg256(const float *p) {
+  float8 r;
+  asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=f"(r.lo.x), "=f"(r.lo.y), "=f"(r.lo.z), "=f"(r.lo.w), "=f"(r.hi.x), "=f"(r.hi.y), "=f"(r.hi.z), "=f"(r.hi.w)
+               : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void stg256(float *p, const float4 &a, const float4 &b) {
+  asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "f"(a.x), "f"(a.y), "f"(a.z), "f"(a.w), "f"(b.x),
+               "f"(b.y), "f"(b.z), "f"(b.w)
+               : "memory");
+}
+__device__ __forceinline__ void store_row8(float *__restrict__ row, int W, int c, bool vec4, bool vec8, const float4 &a, const float4 &b) {
+  if (vec8 && c + 8 <= W) { stg256(row + c, a, b); return; }
+  store_row4(row, W, c, vec4, a);
+  store_row4(row, W, c + 4, vec4, b);
+}
+
 // ------------------------------------------------------------------------------------------------
 // a2 / a6: two chained contractions per 128-atom tile.  Thread r of a warpgroup owns atom row r (TMEM lane r).
 //   step 1  rows of `in_rows` (q or D), scaled by s, split hi/lo -> K-major operand tile [NdK/4][128][4]
@@ -161,7 +182,7 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
   const uint32_t id1 = idesc_tf32(128, NnP, 0, 0), id2 = idesc_tf32(128, NdN, 0, 0);
   uint64_t *bar1 = bars + 2 * wg, *bar2 = bar1 + 1;
   const float b1v = net[sp.Nn * sp.Ndes + 2 * sp.Nn];
-  const bool vecD = (sp.Ndes & 3) == 0, vecN = (sp.Nn & 3) == 0;
+  const bool vecD = (sp.Ndes & 3) == 0, vecN = (sp.Nn & 3) == 0, vecD8 = (sp.Ndes & 7) == 0, vecN8 = (sp.Nn & 7) == 0;
   const int TK = sp.T * sp.KRp;
   const bool vecT = (TK & 3) == 0;
 
@@ -260,7 +281,9 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
         if (valid) {
           float *xr = xbuf + (size_t)a * sp.Nn;
 #pragma unroll
-          for (int v = 0; v < 4; ++v) store_row4(xr, sp.Nn, m0 + 4 * v, vecN, make_float4(xs[4 * v], xs[4 * v + 1], xs[4 * v + 2], xs[4 * v + 3]));
+          for (int v = 0; v < 2; ++v)
+            store_row8(xr, sp.Nn, m0 + 8 * v, vecN, vecN8, make_float4(xs[8 * v], xs[8 * v + 1], xs[8 * v + 2], xs[8 * v + 3]),
+                       make_float4(xs[8 * v + 4], xs[8 * v + 5], xs[8 * v + 6], xs[8 * v + 7]));
         }
       } else {
         const float *xr = xbuf + (size_t)a * sp.Nn;
@@ -341,7 +364,9 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
         if (valid) {
           float *er = Ep + (size_t)a * sp.Ndes;
 #pragma unroll
-          for (int q4 = 0; q4 < 4; ++q4) store_row4(er, sp.Ndes, n0 + 4 * q4, vecD, make_float4(v[4 * q4], v[4 * q4 + 1], v[4 * q4 + 2], v[4 * q4 + 3]));
+          for (int q8 = 0; q8 < 2; ++q8)
+            store_row8(er, sp.Ndes, n0 + 8 * q8, vecD, vecD8, make_float4(v[8 * q8], v[8 * q8 + 1], v[8 * q8 + 2], v[8 * q8 + 3]),
+                       make_float4(v[8 * q8 + 4], v[8 * q8 + 5], v[8 * q8 + 6], v[8 * q8 + 7]));
         }
       } else {
         const float *er = Ep + (size_t)a * sp.Ndes;
@@ -353,11 +378,13 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
           enext[q4] = load_row4(er, sp.Ndes, n0 + 16 + 4 * q4, vecD, valid && n0 + 16 < NdN);
         }
 #pragma unroll
-        for (int q4 = 0; q4 < 4; ++q4) {
-          const float4 e4 = ecur[q4];
+        for (int q8 = 0; q8 < 2; ++q8) {
+          const float4 ea = ecur[2 * q8], eb = ecur[2 * q8 + 1];
+          const int o = 8 * q8;
           if (valid)
-            store_row4(gr, sp.Ndes, n0 + 4 * q4, vecD,
-                       make_float4(ev * e4.x + v[4 * q4], ev * e4.y + v[4 * q4 + 1], ev * e4.z + v[4 * q4 + 2], ev * e4.w + v[4 * q4 + 3]));
+            store_row8(gr, sp.Ndes, n0 + o, vecD, vecD8,
+                       make_float4(ev * ea.x + v[o], ev * ea.y + v[o + 1], ev * ea.z + v[o + 2], ev * ea.w + v[o + 3]),
+                       make_float4(ev * eb.x + v[o + 4], ev * eb.y + v[o + 5], ev * eb.z + v[o + 6], ev * eb.w + v[o + 7]));
         }
       }
     }
