@@ -11,6 +11,7 @@
 // Model constants passed by value to every kernel.
 struct DevSpec {
   int T, NR, KR, NA, KA, L, use4, Nn, Ndes, P;
+  int NnS;                    // row stride of the hidden-layer buffers x, p: Nn padded to 8 (32-byte rows, 256-bit accesses)
   int KRp, KAp;               // basis sizes padded to the template size of the pair kernels
   int offA, offNet, netSize;  // parameter-vector offsets (include/gnep.h layout)
   int ldW;                    // padded shared-memory row stride of W0 (odd -> conflict-free)

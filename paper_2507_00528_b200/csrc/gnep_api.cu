@@ -362,7 +362,7 @@ int gnep_create(const gnep_model_spec *spec, void *cuda_stream, gnep_handle **ou
   h->device = dev; h->num_sms = prop.multiProcessorCount;
   DevSpec &d = h->ds;
   d.T = s.n_species; d.NR = s.n_radial; d.KR = s.n_basis_radial; d.NA = s.n_angular; d.KA = s.n_basis_angular;
-  d.L = s.l_max; d.use4 = s.use_4body ? 1 : 0; d.Nn = s.n_neurons;
+  d.L = s.l_max; d.use4 = s.use_4body ? 1 : 0; d.Nn = s.n_neurons; d.NnS = (d.Nn + 7) & ~7;
   d.Ndes = d.NR + d.NA * d.L + (d.use4 ? d.NA : 0);
   d.KRp = padded_basis(d.KR); d.KAp = padded_basis(d.KA);
   d.offA = d.T * d.T * d.NR * d.KR;
@@ -719,9 +719,9 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     // ---- per-atom state ----
     const size_t n = N;
     const size_t npad = n + GW_PAD_ROWS;   // k_gradw_tc bulk-copies whole windows of rows: zeroed rows past the end
-    BA(h->q, npad * d.Ndes); BA(h->Sn, n * d.NA * GNEP_NLM); BA(h->x, npad * d.Nn); BA(h->Ei, n); BA(h->Ep, n * d.Ndes);
+    BA(h->q, npad * d.Ndes); BA(h->Sn, n * d.NA * GNEP_NLM); BA(h->x, npad * d.NnS); BA(h->Ei, n); BA(h->Ep, n * d.Ndes);
     BA(h->etil, n * T * d.KRp); BA(h->M1, n * T * d.KRp); BA(h->M2, n * T * d.KRp); BA(h->D, npad * d.Ndes); BA(h->Tn, n * d.NA * GNEP_NLM); BA(h->A1, n * T * d.KAp * GNEP_NLM); BA(h->A2, n * T * d.KAp * GNEP_NLM);
-    BA(h->gbar, n * d.Ndes); BA(h->pbuf, npad * d.Nn); BA(h->eat, npad); BA(h->Wat, n * 6);
+    BA(h->gbar, n * d.Ndes); BA(h->pbuf, npad * d.NnS); BA(h->eat, npad); BA(h->Wat, n * 6);
     BA(h->Fat, n); BA(h->fpair, h->nA); BA(h->u, n);
     BA(h->Es, S); BA(h->Ws, (size_t)S * 6); BA(h->parts, (size_t)S * 3); BA(h->e_s, S); BA(h->omega, (size_t)S * 6);
     BA(h->partialCR, (size_t)std::max(h->n_chunks, 1) * d.NR * T * d.KRp);
@@ -730,8 +730,8 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     BA(h->partialB, (size_t)std::max(h->n_gw, 1) * (2 * d.Nn + 1));
     CKT(cudaMemsetAsync(h->q + n * d.Ndes, 0, sizeof(float) * GW_PAD_ROWS * d.Ndes, st));
     CKT(cudaMemsetAsync(h->D + n * d.Ndes, 0, sizeof(float) * GW_PAD_ROWS * d.Ndes, st));
-    CKT(cudaMemsetAsync(h->x + n * d.Nn, 0, sizeof(float) * GW_PAD_ROWS * d.Nn, st));
-    CKT(cudaMemsetAsync(h->pbuf + n * d.Nn, 0, sizeof(float) * GW_PAD_ROWS * d.Nn, st));
+    CKT(cudaMemsetAsync(h->x, 0, sizeof(float) * npad * d.NnS, st));
+    CKT(cudaMemsetAsync(h->pbuf, 0, sizeof(float) * npad * d.NnS, st));
     CKT(cudaMemsetAsync(h->eat + n, 0, sizeof(float) * GW_PAD_ROWS, st));
 #undef BA
 #undef CKT

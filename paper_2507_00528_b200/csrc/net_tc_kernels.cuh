@@ -182,7 +182,7 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
   const uint32_t id1 = idesc_tf32(128, NnP, 0, 0), id2 = idesc_tf32(128, NdN, 0, 0);
   uint64_t *bar1 = bars + 2 * wg, *bar2 = bar1 + 1;
   const float b1v = net[sp.Nn * sp.Ndes + 2 * sp.Nn];
-  const bool vecD = (sp.Ndes & 3) == 0, vecN = (sp.Nn & 3) == 0, vecD8 = (sp.Ndes & 7) == 0, vecN8 = (sp.Nn & 7) == 0;
+  const bool vecD = (sp.Ndes & 3) == 0, vecN = (sp.Nn & 3) == 0, vecD8 = (sp.Ndes & 7) == 0;
   const int TK = sp.T * sp.KRp;
   const bool vecT = (TK & 3) == 0;
 
@@ -250,7 +250,7 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
     float4 xnext[4];   // backward: the x row is fetched one 16-neuron chunk ahead of its use
     if (BWD) {
 #pragma unroll
-      for (int v = 0; v < 4; ++v) xnext[v] = load_row4(xbuf + (size_t)a * sp.Nn, sp.Nn, 4 * v, vecN, valid);
+      for (int v = 0; v < 4; ++v) xnext[v] = load_row4(xbuf + (size_t)a * sp.NnS, sp.NnS, 4 * v, true, valid);
     }
     if (!mbar_wait(bar1, parity)) __trap();
     fence_after_sync();
@@ -279,20 +279,20 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
           split_fast(w1 * (1.f - xv * xv), ch[i], cl[i]);
         }
         if (valid) {
-          float *xr = xbuf + (size_t)a * sp.Nn;
+          float *xr = xbuf + (size_t)a * sp.NnS;
 #pragma unroll
           for (int v = 0; v < 2; ++v)
-            store_row8(xr, sp.Nn, m0 + 8 * v, vecN, vecN8, make_float4(xs[8 * v], xs[8 * v + 1], xs[8 * v + 2], xs[8 * v + 3]),
+            store_row8(xr, sp.NnS, m0 + 8 * v, true, true, make_float4(xs[8 * v], xs[8 * v + 1], xs[8 * v + 2], xs[8 * v + 3]),
                        make_float4(xs[8 * v + 4], xs[8 * v + 5], xs[8 * v + 6], xs[8 * v + 7]));
         }
       } else {
-        const float *xr = xbuf + (size_t)a * sp.Nn;
-        float *pr = pbuf + (size_t)a * sp.Nn;
+        const float *xr = xbuf + (size_t)a * sp.NnS;
+        float *pr = pbuf + (size_t)a * sp.NnS;
         float4 xcur[4];
 #pragma unroll
         for (int v = 0; v < 4; ++v) {
           xcur[v] = xnext[v];
-          xnext[v] = load_row4(xr, sp.Nn, m0 + 16 + 4 * v, vecN, valid && m0 + 16 < NnP);
+          xnext[v] = load_row4(xr, sp.NnS, m0 + 16 + 4 * v, true, valid && m0 + 16 < NnP);
         }
 #pragma unroll
         for (int v = 0; v < 4; ++v) {
@@ -303,7 +303,12 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
             const float d1 = 1.f - xv[i] * xv[i], d2 = -2.f * xv[i] * d1;
             split_fast(w1s[m0 + 4 * v + i] * d2 * z[4 * v + i], ch[4 * v + i], cl[4 * v + i]);
           }
-          if (valid) store_row4(pr, sp.Nn, m0 + 4 * v, vecN, make_float4(z[4 * v], z[4 * v + 1], z[4 * v + 2], z[4 * v + 3]));
+        }
+        if (valid) {
+#pragma unroll
+          for (int v = 0; v < 2; ++v)
+            store_row8(pr, sp.NnS, m0 + 8 * v, true, true, make_float4(z[8 * v], z[8 * v + 1], z[8 * v + 2], z[8 * v + 3]),
+                       make_float4(z[8 * v + 4], z[8 * v + 5], z[8 * v + 6], z[8 * v + 7]));
         }
       }
       {
@@ -449,7 +454,7 @@ __host__ __device__ inline int gw_ncols(const DevSpec &sp) { return pad_to(sp.Nd
 __host__ __device__ inline size_t gradw_stage_floats(const DevSpec &sp) {
   return 6 * (size_t)(GW_KS / 4) * 128 * 4 + 4 * (size_t)(GW_KS / 4) * gw_ncols(sp) * 4;
 }
-__host__ __device__ inline size_t gradw_raw_floats(const DevSpec &sp) { return (size_t)GW_KS * (2 * sp.Nn + 2 * sp.Ndes + 1); }
+__host__ __device__ inline size_t gradw_raw_floats(const DevSpec &sp) { return (size_t)GW_KS * (2 * sp.NnS + 2 * sp.Ndes + 1); }
 __host__ __device__ inline size_t gradw_fixed_bytes() { return ((GW_KS / 4) * 16 * 4 + GW_PROD) * sizeof(float) + 256; }
 __host__ __device__ inline int gradw_nraw(const DevSpec &sp) {
   const long long left = 227ll * 1024 - (long long)gradw_fixed_bytes() - (long long)(GW_OPST * gradw_stage_floats(sp) * sizeof(float));
@@ -484,7 +489,7 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, int nraw, const float *__restrict__ theta,
   const int NB = gw_ncols(sp);
   const int tileA = G4 * 128 * 4, tileB = G4 * NB * 4; // floats per operand tile
   const int stage_fl = 6 * tileA + 4 * tileB;
-  const int raw_fl = GW_KS * (2 * sp.Nn + 2 * sp.Ndes + 1);
+  const int raw_fl = GW_KS * (2 * sp.NnS + 2 * sp.Ndes + 1);
   // operand stage: Ah Al Bh Bl Vh Vl (rows = mu, 128) | Gh Gl Dh Dl (rows = nu, NB);  raw stage: x | p | q | D | e
   float *raw = smem + GW_OPST * stage_fl;
   float *ones = raw + nraw * raw_fl;                  // [G4][16][4]
@@ -527,7 +532,7 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, int nraw, const float *__restrict__ theta,
   if (warp == GW_PROD / 32 + 1) {
     // ================= bulk-copy issuer (one thread) =================
     if ((tid & 31) == 0) {
-      const uint32_t bx = (uint32_t)(GW_KS * sp.Nn * sizeof(float)), bq = (uint32_t)(GW_KS * sp.Ndes * sizeof(float));
+      const uint32_t bx = (uint32_t)(GW_KS * sp.NnS * sizeof(float)), bq = (uint32_t)(GW_KS * sp.Ndes * sizeof(float));
       const uint32_t be = (uint32_t)(GW_KS * sizeof(float));
       for (int it = 0; it < nst; ++it) {
         const int rs = it % nraw, use = it / nraw;
@@ -535,11 +540,11 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, int nraw, const float *__restrict__ theta,
         const size_t a0 = (size_t)(w0 + it * GW_KS);
         float *rb = raw + rs * raw_fl;
         mbar_expect_tx(rfull + rs, 2 * bx + 2 * bq + be);
-        bulk_g2s(rb, x + a0 * sp.Nn, bx, rfull + rs);
-        bulk_g2s(rb + GW_KS * sp.Nn, p + a0 * sp.Nn, bx, rfull + rs);
-        bulk_g2s(rb + 2 * GW_KS * sp.Nn, q + a0 * sp.Ndes, bq, rfull + rs);
-        bulk_g2s(rb + 2 * GW_KS * sp.Nn + GW_KS * sp.Ndes, D + a0 * sp.Ndes, bq, rfull + rs);
-        bulk_g2s(rb + 2 * GW_KS * (sp.Nn + sp.Ndes), eat + a0, be, rfull + rs);
+        bulk_g2s(rb, x + a0 * sp.NnS, bx, rfull + rs);
+        bulk_g2s(rb + GW_KS * sp.NnS, p + a0 * sp.NnS, bx, rfull + rs);
+        bulk_g2s(rb + 2 * GW_KS * sp.NnS, q + a0 * sp.Ndes, bq, rfull + rs);
+        bulk_g2s(rb + 2 * GW_KS * sp.NnS + GW_KS * sp.Ndes, D + a0 * sp.Ndes, bq, rfull + rs);
+        bulk_g2s(rb + 2 * GW_KS * (sp.NnS + sp.Ndes), eat + a0, be, rfull + rs);
       }
     }
   } else if (warp == GW_PROD / 32) {
@@ -620,12 +625,12 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, int nraw, const float *__restrict__ theta,
       const int wl = w < nA ? w : w - nA, W = w < nA ? sp.Nn : sp.Ndes;
       const int ag = i_kind[j] ? wl / W : 0, col = i_kind[j] ? wl - ag * W : 0;
       i_ag[j] = 4 * ag;
-      r_off[j] = (i_kind[j] == 1 ? 0 : 2 * GW_KS * sp.Nn) + 4 * ag * W + col;
+      r_off[j] = i_kind[j] == 1 ? 4 * ag * sp.NnS + col : 2 * GW_KS * sp.NnS + 4 * ag * W + col;
       s_off[j] = i_kind[j] == 1 ? (ag * 128 + col) * 4 : 6 * tileA + (ag * NB + col) * 4;
       i_cf[j] = i_kind[j] == 1 ? w1g[col] : (i_kind[j] == 2 ? qscale[col] : 0.f);
       if (i_kind[j] == 1 && col == 0) i_kind[j] = 3;
     }
-    const int e_off = 2 * GW_KS * (sp.Nn + sp.Ndes);
+    const int e_off = 2 * GW_KS * (sp.NnS + sp.Ndes);
     int nfl = 0;                                        // accumulation groups already added to the registers
     for (int it = 0; it < nst; ++it) {
       const int st = it % GW_OPST, use = it / GW_OPST, g = it / GW_FLUSH, gi = it - g * GW_FLUSH;
@@ -647,15 +652,15 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, int nraw, const float *__restrict__ theta,
         float *dst = sb + s_off[j];
         const float cf = i_cf[j];
         if (i_kind[j] & 1) {
-          const float *rx = rb + r_off[j], *rp = rx + GW_KS * sp.Nn;
+          const float *rx = rb + r_off[j], *rp = rx + GW_KS * sp.NnS;
           const float4 e4 = *(const float4 *)(rb + e_off + i_ag[j]);
           const float ee[4] = {e4.x, e4.y, e4.z, e4.w};
           float Av[4], Bv[4], Vv[4];
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
             const bool ok = whole || (i_ag[j] + i >= vlo && i_ag[j] + i < vhi);
-            const float xv = rx[i * sp.Nn];
-            const float pv = ok ? rp[i * sp.Nn] : 0.f, ev = ok ? ee[i] : 0.f;
+            const float xv = rx[i * sp.NnS];
+            const float pv = ok ? rp[i * sp.NnS] : 0.f, ev = ok ? ee[i] : 0.f;
             const float d1 = 1.f - xv * xv, d2 = -2.f * xv * d1;
             Av[i] = cf * (ev * d1 + d2 * pv);
             Bv[i] = ok ? cf * d1 : 0.f;
