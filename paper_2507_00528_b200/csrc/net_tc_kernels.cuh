@@ -106,6 +106,11 @@ __device__ __forceinline__ void stg256(float *p, const float4 &a, const float4 &
                "f"(b.y), "f"(b.z), "f"(b.w)
                : "memory");
 }
+__device__ __forceinline__ void load_row8(const float *__restrict__ row, int W, int c, bool vec4, bool vec8, bool valid, float4 &a, float4 &b) {
+  if (valid && vec8 && c + 8 <= W) { const float8 r = ldg256(row + c); a = r.lo; b = r.hi; return; }
+  a = load_row4(row, W, c, vec4, valid);
+  b = load_row4(row, W, c + 4, vec4, valid);
+}
 __device__ __forceinline__ void store_row8(float *__restrict__ row, int W, int c, bool vec4, bool vec8, const float4 &a, const float4 &b) {
   if (vec8 && c + 8 <= W) { stg256(row + c, a, b); return; }
   store_row4(row, W, c, vec4, a);
@@ -196,7 +201,7 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
     const bool ok = tile_ < tiles && a_ < sm.start[t + 1];
     const float *row_ = in_rows + (size_t)a_ * sp.Ndes;
 #pragma unroll
-    for (int c = 0; c < NET_PRE; ++c) pre[c] = load_row4(row_, sp.Ndes, 4 * c, vecD, ok && c < NdK / 4);
+    for (int c = 0; c < NET_PRE; c += 2) load_row8(row_, sp.Ndes, 4 * c, vecD, vecD8, ok && c < NdK / 4, pre[c], pre[c + 1]);
   };
   prefetch_row((blockIdx.x - sm.cta_base[t]) * 2 + wg);
   for (int tile = (blockIdx.x - sm.cta_base[t]) * 2 + wg; tile < tiles; tile += 2 * ncta, parity ^= 1u) {
@@ -250,7 +255,7 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
     float4 xnext[4];   // backward: the x row is fetched one 16-neuron chunk ahead of its use
     if (BWD) {
 #pragma unroll
-      for (int v = 0; v < 4; ++v) xnext[v] = load_row4(xbuf + (size_t)a * sp.NnS, sp.NnS, 4 * v, true, valid);
+      for (int v = 0; v < 4; v += 2) load_row8(xbuf + (size_t)a * sp.NnS, sp.NnS, 4 * v, true, true, valid, xnext[v], xnext[v + 1]);
     }
     if (!mbar_wait(bar1, parity)) __trap();
     fence_after_sync();
@@ -290,10 +295,9 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
         float *pr = pbuf + (size_t)a * sp.NnS;
         float4 xcur[4];
 #pragma unroll
-        for (int v = 0; v < 4; ++v) {
-          xcur[v] = xnext[v];
-          xnext[v] = load_row4(xr, sp.NnS, m0 + 16 + 4 * v, true, valid && m0 + 16 < NnP);
-        }
+        for (int v = 0; v < 4; ++v) xcur[v] = xnext[v];
+#pragma unroll
+        for (int v = 0; v < 4; v += 2) load_row8(xr, sp.NnS, m0 + 16 + 4 * v, true, true, valid && m0 + 16 < NnP, xnext[v], xnext[v + 1]);
 #pragma unroll
         for (int v = 0; v < 4; ++v) {
           const float4 x4 = xcur[v];
@@ -344,7 +348,7 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
     float4 enext[4];   // backward: E' row, one 16-descriptor chunk ahead
     if (BWD) {
 #pragma unroll
-      for (int v = 0; v < 4; ++v) enext[v] = load_row4(Ep + (size_t)a * sp.Ndes, sp.Ndes, 4 * v, vecD, valid);
+      for (int v = 0; v < 4; v += 2) load_row8(Ep + (size_t)a * sp.Ndes, sp.Ndes, 4 * v, vecD, vecD8, valid, enext[v], enext[v + 1]);
     }
     if (!mbar_wait(bar2, parity)) __trap();
     fence_after_sync();
@@ -378,10 +382,9 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
         float *gr = gbar + (size_t)a * sp.Ndes;
         float4 ecur[4];
 #pragma unroll
-        for (int q4 = 0; q4 < 4; ++q4) {
-          ecur[q4] = enext[q4];
-          enext[q4] = load_row4(er, sp.Ndes, n0 + 16 + 4 * q4, vecD, valid && n0 + 16 < NdN);
-        }
+        for (int q4 = 0; q4 < 4; ++q4) ecur[q4] = enext[q4];
+#pragma unroll
+        for (int q4 = 0; q4 < 4; q4 += 2) load_row8(er, sp.Ndes, n0 + 16 + 4 * q4, vecD, vecD8, valid && n0 + 16 < NdN, enext[q4], enext[q4 + 1]);
 #pragma unroll
         for (int q8 = 0; q8 < 2; ++q8) {
           const float4 ea = ecur[2 * q8], eb = ecur[2 * q8 + 1];
@@ -395,10 +398,11 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
     }
     if (!BWD) {   // etil[J][k] = sum_n E'_n cR[t][J][n][k]  (input of the radial force pass)
       float *et = etil + (size_t)a * TK;
-      for (int o = 0; o < TK; o += 4) {
-        float acc4[4] = {0.f, 0.f, 0.f, 0.f};
+      const bool vecT8 = (TK & 7) == 0;
+      for (int o = 0; o < TK; o += 8) {
+        float acc4[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
+        for (int i = 0; i < 8; ++i) {
           if (o + i < TK) {
             const float4 *c4 = (const float4 *)(cRs + (o + i) * 16);
             float s = 0.f;
@@ -410,7 +414,7 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
             acc4[i] = s;
           }
         }
-        if (valid) store_row4(et, TK, o, vecT, make_float4(acc4[0], acc4[1], acc4[2], acc4[3]));
+        if (valid) store_row8(et, TK, o, vecT, vecT8, make_float4(acc4[0], acc4[1], acc4[2], acc4[3]), make_float4(acc4[4], acc4[5], acc4[6], acc4[7]));
       }
     }
     fence_before_sync();   // the next tile's MMAs overwrite D1/D2 and the operand buffer after the barrier of step 1
