@@ -184,8 +184,7 @@ k_angular_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
           const float4 s0 = *(const float4 *)(Xs + n * GNEP_NLM + 8 * nl.lmg), s1 = *(const float4 *)(Xs + n * GNEP_NLM + 8 * nl.lmg + 4);
           sv[0] = s0.x; sv[1] = s0.y; sv[2] = s0.z; sv[3] = s0.w; sv[4] = s1.x; sv[5] = s1.y; sv[6] = s1.z; sv[7] = s1.w;
         }
-        *(float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg) = make_float4(sv[0], sv[1], sv[2], sv[3]);
-        *(float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg + 4) = make_float4(sv[4], sv[5], sv[6], sv[7]);
+        stg256(Sa + n * GNEP_NLM + 8 * nl.lmg, make_float4(sv[0], sv[1], sv[2], sv[3]), make_float4(sv[4], sv[5], sv[6], sv[7]));
         float w[8];
 #pragma unroll
         for (int i = 0; i < 8; ++i) w[i] = 0.5f * nl.c2[i] * sv[i] * sv[i];
@@ -316,7 +315,7 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
       Icur = type_s[a];
       if (nl.act && nl.nq < sp.NA) {
         const float *Sa_ = S + (size_t)a * sp.NA * GNEP_NLM + nl.nq * GNEP_NLM + 8 * nl.lmg;
-        sn0 = *(const float4 *)Sa_; sn1 = *(const float4 *)(Sa_ + 4);
+        const float8 s8 = ldg256(Sa_); sn0 = s8.lo; sn1 = s8.hi;
       }
     }
   };
@@ -346,14 +345,13 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
       float tv[8], sv[8], da = 0.f, db = 0.f;
       if (on) {
         float4 s0 = sn0, s1 = sn1;
-        if (nb > 0) { s0 = *(const float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg); s1 = *(const float4 *)(Sa + n * GNEP_NLM + 8 * nl.lmg + 4); }
+        if (nb > 0) { const float8 s8 = ldg256(Sa + n * GNEP_NLM + 8 * nl.lmg); s0 = s8.lo; s1 = s8.hi; }
         sv[0] = s0.x; sv[1] = s0.y; sv[2] = s0.z; sv[3] = s0.w; sv[4] = s1.x; sv[5] = s1.y; sv[6] = s1.z; sv[7] = s1.w;
         {
           const float4 t0 = *(const float4 *)(Xs + n * GNEP_NLM + 8 * nl.lmg), t1 = *(const float4 *)(Xs + n * GNEP_NLM + 8 * nl.lmg + 4);
           tv[0] = t0.x; tv[1] = t0.y; tv[2] = t0.z; tv[3] = t0.w; tv[4] = t1.x; tv[5] = t1.y; tv[6] = t1.z; tv[7] = t1.w;
         }
-        *(float4 *)(Ta + n * GNEP_NLM + 8 * nl.lmg) = make_float4(tv[0], tv[1], tv[2], tv[3]);
-        *(float4 *)(Ta + n * GNEP_NLM + 8 * nl.lmg + 4) = make_float4(tv[4], tv[5], tv[6], tv[7]);
+        stg256(Ta + n * GNEP_NLM + 8 * nl.lmg, make_float4(tv[0], tv[1], tv[2], tv[3]), make_float4(tv[4], tv[5], tv[6], tv[7]));
         float w[8];
 #pragma unroll
         for (int i = 0; i < 8; ++i) w[i] = nl.c2[i] * sv[i] * tv[i];
@@ -485,7 +483,7 @@ k_angular_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__
       const int a = a_lo + it / rounds, n = (it % rounds) * 10 + nl.nq;
       if (it < nit && nl.act && n < sp.NA) {
         const float *Sa = S + (size_t)a * nb + n * GNEP_NLM + 8 * nl.lmg, *Epa = Ep + (size_t)a * sp.Ndes;
-        s0n = *(const float4 *)Sa; s1n = *(const float4 *)(Sa + 4);
+        const float8 s8 = ldg256(Sa); s0n = s8.lo; s1n = s8.hi;
         ean = desc_of(sp, Epa, nl.la, n); ebn = desc_of(sp, Epa, nl.lb, n);
         if (sp.use4 && nl.lmg == 0) e4n = Epa[sp.NR + sp.L * sp.NA + n];
       }
@@ -627,7 +625,10 @@ k_cgrad_angular(DevSpec sp, int N, const int *__restrict__ type_s, const float *
         const float4 *a1 = (const float4 *)(A1 + (size_t)a * nA + row * GNEP_NLM);
         const float4 *a2 = (const float4 *)(A2 + (size_t)a * nA + row * GNEP_NLM);
 #pragma unroll
-        for (int v = 0; v < 6; ++v) { x1[v] = __ldg(a1 + v); x2[v] = __ldg(a2 + v); }
+        for (int v = 0; v < 6; v += 2) {
+          const float8 u1 = ldg256((const float *)(a1 + v)), u2 = ldg256((const float *)(a2 + v));
+          x1[v] = u1.lo; x1[v + 1] = u1.hi; x2[v] = u2.lo; x2[v + 1] = u2.hi;
+        }
       }
     }
     const float *Sa = S + (size_t)a * nb, *Ta = Tn + (size_t)a * nb;
@@ -636,8 +637,8 @@ k_cgrad_angular(DevSpec sp, int N, const int *__restrict__ type_s, const float *
       const int n = n0 + nl.nq;
       if (nl.act && n < sp.NA) {
         const int o = n * GNEP_NLM + 8 * nl.lmg;
-        float4 s0 = *(const float4 *)(Sa + o), s1 = *(const float4 *)(Sa + o + 4);
-        float4 t0 = *(const float4 *)(Ta + o), t1 = *(const float4 *)(Ta + o + 4);
+        const float8 s8 = ldg256(Sa + o), t8 = ldg256(Ta + o);
+        const float4 s0 = s8.lo, s1 = s8.hi, t0 = t8.lo, t1 = t8.hi;
         float sv[8] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
         float tv[8] = {t0.x, t0.y, t0.z, t0.w, t1.x, t1.y, t1.z, t1.w};
         const float ea = desc_of(sp, Epa, nl.la, n), eb = desc_of(sp, Epa, nl.lb, n);
@@ -671,7 +672,10 @@ k_cgrad_angular(DevSpec sp, int N, const int *__restrict__ type_s, const float *
         const float4 *a1 = (const float4 *)(A1 + (size_t)a * nA + row * GNEP_NLM);
         const float4 *a2 = (const float4 *)(A2 + (size_t)a * nA + row * GNEP_NLM);
 #pragma unroll
-        for (int v = 0; v < 6; ++v) { x1[v] = __ldg(a1 + v); x2[v] = __ldg(a2 + v); }
+        for (int v = 0; v < 6; v += 2) {
+          const float8 u1 = ldg256((const float *)(a1 + v)), u2 = ldg256((const float *)(a2 + v));
+          x1[v] = u1.lo; x1[v + 1] = u1.hi; x2[v] = u2.lo; x2[v + 1] = u2.hi;
+        }
       }
       const int J = row / KT, k = row - J * KT;
       float *dst = accS + ((I * sp.T + J) * sp.NA) * KT + k;

@@ -192,6 +192,21 @@ __device__ __forceinline__ void p4_hess_vec(const float *s, const float *t, floa
   h[4] = -18.f * s4 * t[0] + 108.f * s2 * t[1] + 108.f * s1 * t[2] - 18.f * s0 * t[4];
 }
 
+// 8 consecutive floats at a 32-byte aligned address as ONE 256-bit access (sm_100: LDG/STG.256): half as many requests
+// as two 128-bit ones, which is what row-per-thread / row-per-lane patterns pay for (a different line per lane)
+struct float8 { float4 lo, hi; };
+__device__ __forceinline__ float8 ldg256(const float *p) {
+  float8 r;
+  asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=f"(r.lo.x), "=f"(r.lo.y), "=f"(r.lo.z), "=f"(r.lo.w), "=f"(r.hi.x), "=f"(r.hi.y), "=f"(r.hi.z), "=f"(r.hi.w)
+               : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void stg256(float *p, const float4 &a, const float4 &b) {
+  asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "f"(a.x), "f"(a.y), "f"(a.z), "f"(a.w), "f"(b.x),
+               "f"(b.y), "f"(b.z), "f"(b.w)
+               : "memory");
+}
 // Fixed-order warp reduction of K per-lane accumulators through shared memory:
 // returns sum over lanes of acc[lane_k] to lane k (k < K), 0 elsewhere.  buf: K*33 floats per warp.
 template <int K>

@@ -91,21 +91,6 @@ __device__ __forceinline__ void store_row4(float *__restrict__ row, int W, int c
   if (c + 3 < W) row[c + 3] = v.w;
 }
 
-// 8 consecutive values of a row (32-byte aligned, row length a multiple of 8): one 256-bit access -- half as many
-// requests as two 128-bit ones, which is what the row-per-thread pattern pays for (32 different lines per request)
-struct float8 { float4 lo, hi; };
-__device__ __forceinline__ float8 ldg256(const float *p) {
-  float8 r;
-  asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-               : "=f"(r.lo.x), "=f"(r.lo.y), "=f"(r.lo.z), "=f"(r.lo.w), "=f"(r.hi.x), "=f"(r.hi.y), "=f"(r.hi.z), "=f"(r.hi.w)
-               : "l"(p));
-  return r;
-}
-__device__ __forceinline__ void stg256(float *p, const float4 &a, const float4 &b) {
-  asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "f"(a.x), "f"(a.y), "f"(a.z), "f"(a.w), "f"(b.x),
-               "f"(b.y), "f"(b.z), "f"(b.w)
-               : "memory");
-}
 __device__ __forceinline__ void load_row8(const float *__restrict__ row, int W, int c, bool vec4, bool vec8, bool valid, float4 &a, float4 &b) {
   if (valid && vec8 && c + 8 <= W) { const float8 r = ldg256(row + c); a = r.lo; b = r.hi; return; }
   a = load_row4(row, W, c, vec4, valid);
