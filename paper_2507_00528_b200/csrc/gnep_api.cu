@@ -634,13 +634,14 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     if (N >= (1 << 28)) { tfree(); free_batch(h); return fail(h, GNEP_ERANGE, "2^28 or more atoms"); }
     if (nR >= (int64_t)1 << 31) { tfree(); free_batch(h); return fail(h, GNEP_ERANGE, "2^31 or more radial pairs"); }
     std::vector<int> rowRs(N + 1, 0), rowAs(N + 1, 0);
-    for (int a = 0; a < N; ++a) { rowRs[a + 1] = rowRs[a] + cR[perm[a]]; rowAs[a + 1] = rowAs[a] + cA[perm[a]]; }
+    // radial rows start at even record indices (32-byte aligned): the walk reads two 16-byte records per 256-bit load
+    for (int a = 0; a < N; ++a) { rowRs[a + 1] = rowRs[a] + ((cR[perm[a]] + 1) & ~1); rowAs[a + 1] = rowAs[a] + cA[perm[a]]; }
     h->nR = nR; h->nA = nA;
     // ---- persistent batch arrays ----
     int rc_;
 #define BA(ptr, n) if ((rc_ = dalloc(h, &(ptr), (n), true)) != GNEP_OK) { tfree(); free_batch(h); return rc_; }
     BA(h->perm, N); BA(h->type_s, N); BA(h->struct_s, N); BA(h->segR, (size_t)N * (T + 1) + 1); BA(h->rowAs, N + 1); BA(h->segA, (size_t)N * (T + 1) + 1);
-    BA(h->pairR, nR);
+    BA(h->pairR, (size_t)rowRs[N] + 2);
     BA(h->exp_row[0], N + 1); BA(h->exp_row[1], N + 1); BA(h->exp_j[0], nR); BA(h->exp_sh[0], nR); BA(h->exp_j[1], nA); BA(h->exp_sh[1], nA);
     BA(h->srange, srange.size()); BA(h->Eref, S); BA(h->Wref, (size_t)S * 6); BA(h->Fref_s, (size_t)N * 3);
     // the angular list is first built unpadded (u) and then copied into its final layout, in which every (atom, J)

@@ -27,15 +27,21 @@ __device__ __forceinline__ void walk_row(const float4 *__restrict__ pairR, const
   const int pend = sg[T];
   const float4 dum = make_float4(1.f, 0.f, 0.f, 0.f);      // w = bits(0): a valid atom index for the gather
   float4 nb[RAD_PF];
+  // rows start at even record indices and p advances by RAD_PF: two records per 256-bit load (the second may lie past
+  // the row's end -- in the row's pad slot or the next row -- and is then ignored)
+  auto load2 = [&](int q, float4 &r0, float4 &r1) {
+    if (q < pend) { const float8 v = ldg256((const float *)(pairR + q)); r0 = v.lo; r1 = v.hi; }
+    else { r0 = dum; r1 = dum; }
+  };
 #pragma unroll
-  for (int i = 0; i < RAD_PF; ++i) nb[i] = p + i < pend ? pairR[p + i] : dum;
+  for (int i = 0; i < RAD_PF; i += 2) load2(p + i, nb[i], nb[i + 1]);
   auto gn = gather(nb[0]);
   while (p < pend) {
     float4 cb[RAD_PF];
 #pragma unroll
     for (int i = 0; i < RAD_PF; ++i) cb[i] = nb[i];
 #pragma unroll
-    for (int i = 0; i < RAD_PF; ++i) nb[i] = p + RAD_PF + i < pend ? pairR[p + RAD_PF + i] : dum;
+    for (int i = 0; i < RAD_PF; i += 2) load2(p + RAD_PF + i, nb[i], nb[i + 1]);
 #pragma unroll
     for (int i = 0; i < RAD_PF; ++i) {
       const auto gc = gn;
