@@ -593,7 +593,7 @@ k_force_gather(int N, int T1, const int *__restrict__ segA, const int *__restric
 // shared memory over the atoms it visits and writes one partial at the end (reduced by k_grad_reduce).
 // ------------------------------------------------------------------------------------------------
 template <int KT>
-__global__ void __launch_bounds__(ANG_WARPS * 32)
+__global__ void __launch_bounds__(ANG_WARPS * 32, 4)
 k_cgrad_angular(DevSpec sp, int N, const int *__restrict__ type_s, const float *__restrict__ Ep,
                 const float *__restrict__ gbar, const float *__restrict__ S, const float *__restrict__ Tn,
                 const float *__restrict__ A1, const float *__restrict__ A2, float *__restrict__ partial) {
@@ -617,7 +617,21 @@ k_cgrad_angular(DevSpec sp, int N, const int *__restrict__ type_s, const float *
   const int n_lo = half * nh, n_hi = min(sp.NA, n_lo + nh);
   for (int a = gw; a < N; a += nw) {
     const int I = type_s[a];
-    // the moment rows of the first round are requested before alpha/beta are formed, so that their latency is hidden
+    // requests in the order of use: the per-atom rows S, T, E', gbar of the first n-round (needed at once for
+    // alpha/beta), then the moment rows of the first contraction round, whose latency hides behind the alpha/beta work
+    const float *Sa = S + (size_t)a * nb, *Ta = Tn + (size_t)a * nb;
+    const float *Epa = Ep + (size_t)a * sp.Ndes, *gba = gbar + (size_t)a * sp.Ndes;
+    float8 s8, t8;
+    s8.lo = s8.hi = t8.lo = t8.hi = make_float4(0.f, 0.f, 0.f, 0.f);
+    float ea = 0.f, eb = 0.f, ga = 0.f, gb = 0.f, e4r = 0.f, gb4r = 0.f;
+    auto request = [&](int n) {
+      const int o = n * GNEP_NLM + 8 * nl.lmg;
+      s8 = ldg256(Sa + o); t8 = ldg256(Ta + o);
+      ea = desc_of(sp, Epa, nl.la, n); eb = desc_of(sp, Epa, nl.lb, n);
+      ga = desc_of(sp, gba, nl.la, n); gb = desc_of(sp, gba, nl.lb, n);
+      if (sp.use4 && nl.lmg == 0) { e4r = Epa[sp.NR + sp.L * sp.NA + n]; gb4r = gba[sp.NR + sp.L * sp.NA + n]; }
+    };
+    if (nl.act && nl.nq < sp.NA) request(nl.nq);
     float4 x1[6], x2[6];
     {
       const int row = lane >> 1;
@@ -631,18 +645,14 @@ k_cgrad_angular(DevSpec sp, int N, const int *__restrict__ type_s, const float *
         }
       }
     }
-    const float *Sa = S + (size_t)a * nb, *Ta = Tn + (size_t)a * nb;
-    const float *Epa = Ep + (size_t)a * sp.Ndes, *gba = gbar + (size_t)a * sp.Ndes;
     for (int n0 = 0; n0 < sp.NA; n0 += 10) {      // alpha, beta in the (n, lmg) lane layout
       const int n = n0 + nl.nq;
       if (nl.act && n < sp.NA) {
         const int o = n * GNEP_NLM + 8 * nl.lmg;
-        const float8 s8 = ldg256(Sa + o), t8 = ldg256(Ta + o);
+        if (n0 > 0) request(n);
         const float4 s0 = s8.lo, s1 = s8.hi, t0 = t8.lo, t1 = t8.hi;
         float sv[8] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
         float tv[8] = {t0.x, t0.y, t0.z, t0.w, t1.x, t1.y, t1.z, t1.w};
-        const float ea = desc_of(sp, Epa, nl.la, n), eb = desc_of(sp, Epa, nl.lb, n);
-        const float ga = desc_of(sp, gba, nl.la, n), gb = desc_of(sp, gba, nl.lb, n);
         float al[8], be[8];
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
@@ -651,11 +661,10 @@ k_cgrad_angular(DevSpec sp, int N, const int *__restrict__ type_s, const float *
           be[i] = nl.c2[i] * e1 * sv[i];
         }
         if (sp.use4 && nl.lmg == 0) {
-          const int v4 = sp.NR + sp.L * sp.NA + n;
           float g4[5], hv[5];
           p4_grad(sv + 3, g4);
           p4_hess_vec(sv + 3, tv + 3, hv);
-          const float e4 = c_kappa4 * Epa[v4], gb4 = c_kappa4 * gba[v4];
+          const float e4 = c_kappa4 * e4r, gb4 = c_kappa4 * gb4r;
 #pragma unroll
           for (int m = 0; m < 5; ++m) { al[3 + m] += gb4 * g4[m] + e4 * hv[m]; be[3 + m] += e4 * g4[m]; }
         }
