@@ -172,7 +172,7 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
   const uint32_t id1 = idesc_tf32(128, NnP, 0, 0), id2 = idesc_tf32(128, NdN, 0, 0);
   uint64_t *bar1 = bars + 2 * wg, *bar2 = bar1 + 1;
   const float b1v = net[sp.Nn * sp.Ndes + 2 * sp.Nn];
-  const bool vecD = (sp.Ndes & 3) == 0, vecN = (sp.Nn & 3) == 0, vecD8 = (sp.Ndes & 7) == 0;
+  const bool vecD = (sp.Ndes & 3) == 0, vecD8 = (sp.Ndes & 7) == 0;
   const int TK = sp.T * sp.KRp;
   const bool vecT = (TK & 3) == 0;
 
