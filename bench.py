@@ -295,9 +295,9 @@ def run_ours(args):
     else:
         roof = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
                 "traffic": None, "peak_source": hbm_src}
-    if args.config == 4 and not args.structs:      # the workload of the committed ncu capture (profiles/r1_v7_cfg4_traffic.md)
+    if args.config == 4 and not args.structs:      # the workload of the committed ncu capture (profiles/r1_v8_cfg4_traffic.md)
         try:
-            for ln in open(os.path.join(ROOT, "profiles", "r1_v7_cfg4_traffic.csv")):
+            for ln in open(os.path.join(ROOT, "profiles", "r1_v8_cfg4_traffic.csv")):
                 f = ln.strip().split(",")
                 if f[0] == top:
                     roof["traffic"] = int(f[-1]); roof["traffic_unit"] = "DRAM bytes per launch (ncu --set full)"
