@@ -168,11 +168,16 @@ __global__ void __launch_bounds__(256)
 k_adam(int P, float *__restrict__ theta, float *__restrict__ m, float *__restrict__ v,
        const float *__restrict__ grad, const long long *__restrict__ step, const float *__restrict__ lr_p, float beta1,
        float beta2, float eps) {
+  __shared__ float sc[2];
+  if (threadIdx.x == 0) {          // the bias corrections need fp64 pow: once per block, not once per parameter
+    const double t = (double)(*step + 1);
+    sc[0] = (float)(1.0 - pow((double)beta1, t)); sc[1] = (float)(1.0 - pow((double)beta2, t));
+  }
+  __syncthreads();
   int p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= P) return;
   const float lr = *lr_p;          // device scalar: a learning-rate schedule changes it without re-building the epoch graph
-  double t = (double)(*step + 1);
-  float c1 = (float)(1.0 - pow((double)beta1, t)), c2 = (float)(1.0 - pow((double)beta2, t));
+  const float c1 = sc[0], c2 = sc[1];
   float g = grad[p];
   float mm = beta1 * m[p] + (1.f - beta1) * g;
   float vv = beta2 * v[p] + (1.f - beta2) * g * g;
