@@ -453,7 +453,7 @@ k_angular_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__re
 // lane = pair over the packed pairs of FRC_TA atoms; beta of the tile's atoms lives in shared memory.
 // gam_lm = sum_n g_n beta_nlm, gamp_lm = sum_n g_n' beta_nlm, then one harmonic sweep.  Writes f_ij per pair.
 // ------------------------------------------------------------------------------------------------
-#define FRC_TA 16
+#define FRC_TA 8
 template <int KT>
 __global__ void __launch_bounds__(ANG_WARPS * 32)
 k_angular_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ segA,
