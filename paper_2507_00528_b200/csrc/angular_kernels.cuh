@@ -552,50 +552,7 @@ k_angular_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__
   }
 }
 
-// F_i += sum_{p in row i} (f_p - f_rev(p)),  W_i -= sum_p r_p (x) f_p   (Eq.3, Eq.4 for the angular part; no
-// atomics).  Half a warp per atom.
-__global__ void __launch_bounds__(256, 6)
-k_force_gather(int N, int T1, const int *__restrict__ segA, const int *__restrict__ revA,
-               const float4 *__restrict__ pairA, const float4 *__restrict__ fpair, float4 *__restrict__ Fat,
-               float *__restrict__ Wat) {
-  const int a = (blockIdx.x * blockDim.x + threadIdx.x) >> 4;
-  const int sub = threadIdx.x & 15;
-  float F[3] = {0.f, 0.f, 0.f}, W[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-  if (a < N) {
-    const int p0 = segA[a * T1], p1 = segA[a * T1 + T1 - 1];
-    // the kernel is a chain of dependent loads (row bounds -> reverse index -> reverse force): two 16-pair chunks are
-    // requested together so that most rows cost one round trip per level
-    for (int pb = p0 + sub; pb < p1; pb += 32) {
-      const int pc = pb + 16;
-      const bool two = pc < p1;
-      const int r0 = revA[pb], r1 = two ? revA[pc] : 0;
-      const float4 f0 = fpair[pb], x0 = pairA[pb];
-      float4 f1 = make_float4(0.f, 0.f, 0.f, 0.f), x1 = f1, g1 = f1;
-      if (two) { f1 = fpair[pc]; x1 = pairA[pc]; }
-      const float4 g0 = fpair[r0];
-      if (two) g1 = fpair[r1];
-      F[0] += (f0.x - g0.x) + (f1.x - g1.x); F[1] += (f0.y - g0.y) + (f1.y - g1.y); F[2] += (f0.z - g0.z) + (f1.z - g1.z);
-      W[0] -= x0.x * f0.x + x1.x * f1.x; W[1] -= x0.y * f0.y + x1.y * f1.y; W[2] -= x0.z * f0.z + x1.z * f1.z;
-      W[3] -= x0.x * f0.y + x1.x * f1.y; W[4] -= x0.y * f0.z + x1.y * f1.z; W[5] -= x0.z * f0.x + x1.z * f1.x;
-    }
-  }
-#pragma unroll
-  for (int o = 8; o > 0; o >>= 1) {
-#pragma unroll
-    for (int c = 0; c < 3; ++c) F[c] += __shfl_xor_sync(0xffffffffu, F[c], o);
-#pragma unroll
-    for (int c = 0; c < 6; ++c) W[c] += __shfl_xor_sync(0xffffffffu, W[c], o);
-  }
-  if (a < N && sub == 0) {
-    float4 o = Fat[a];
-    Fat[a] = make_float4(o.x + F[0], o.y + F[1], o.z + F[2], 0.f);
-#pragma unroll
-    for (int c = 0; c < 6; c += 2) {
-      float2 w = *(float2 *)(Wat + (size_t)a * 6 + c);
-      *(float2 *)(Wat + (size_t)a * 6 + c) = make_float2(w.x + W[c], w.y + W[c + 1]);
-    }
-  }
-}
+// (The gather F_i += sum_p (f_p - f_rev(p)), W_i -= sum_p r_p (x) f_p is done by k_radial_force, thread per atom.)
 
 // ------------------------------------------------------------------------------------------------
 // a7 (angular): dL/dcA[I][J][n][k] = sum_atoms sum_lm alpha_nlm A1[J][k][lm] + beta_nlm A2[J][k][lm]

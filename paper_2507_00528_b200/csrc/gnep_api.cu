@@ -238,12 +238,12 @@ int enqueue_forward(gnep_handle *h) {
   LAUNCH(h, k_net_tc<false>, h->n_cta_net, 256, smem_net_fwd(d), d, h->sm, h->theta, h->qscale, h->q, h->x, h->Ei, h->Ep, h->etil,
          (const int *)nullptr, (const float *)nullptr, (const float *)nullptr, (float *)nullptr, (float *)nullptr);
   mark(h, "a2_network_forward");
-  DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_force<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, 0, d, h->N, h->type_s, h->segR, h->pairR, h->etil, h->Fat, h->Wat));
-  mark(h, "a3_radial_force");
   DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_force<KT>, cdiv(h->N, ANG_WARPS * FRC_TA), ANG_WARPS * 32, smem_ang_force(d), d, h->N, h->type_s, h->segAu, h->atomAu, h->pairAu, h->theta, h->Ep, h->Sn, h->fpair));
   mark(h, "a3_angular_force");
-  LAUNCH(h, k_force_gather, cdiv((int64_t)h->N * 16, 256), 256, 0, h->N, d.T + 1, h->segAu, h->revAu, h->pairAu, h->fpair, h->Fat, h->Wat);
-  mark(h, "a3_force_gather");
+  // radial forces + the gather of the angular pair forces (thread per atom): writes F_i, W_i once
+  DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_force<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, 0, d, h->N, h->type_s, h->segR, h->pairR, h->etil,
+                            h->segAu, h->revAu, h->pairAu, h->fpair, h->Fat, h->Wat));
+  mark(h, "a3_radial_force");
   LAUNCH(h, k_struct_reduce, h->S, 128, 0, loss_cfg(h), h->srange, h->Ei, h->Fat, h->Wat, h->Eref, h->Fref_s, h->Wref, h->Es, h->Ws, h->e_s, h->u, h->omega, h->parts);
   LAUNCH(h, k_loss_final, 1, 256, 0, loss_cfg(h), h->parts, h->theta, h->terms, h->scales);
   mark(h, "a4_loss_and_seeds");

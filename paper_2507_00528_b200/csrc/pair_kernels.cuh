@@ -156,8 +156,9 @@ k_radial_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__res
 template <int KT>
 __global__ void __launch_bounds__(RAD_THREADS)
 k_radial_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ segR,
-               const float4 *__restrict__ pairR, const float *__restrict__ etil, float4 *__restrict__ Fat,
-               float *__restrict__ Wat) {
+               const float4 *__restrict__ pairR, const float *__restrict__ etil, const int *__restrict__ segA,
+               const int *__restrict__ revA, const float4 *__restrict__ pairA, const float4 *__restrict__ fpair,
+               float4 *__restrict__ Fat, float *__restrict__ Wat) {
   const int a = blockIdx.x * RAD_THREADS + threadIdx.x;
   if (a >= N) return;
   const int I = type_s[a];
@@ -195,6 +196,31 @@ k_radial_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__r
              W[0] -= r.x * fx; W[1] -= r.y * fy; W[2] -= r.z * fz;
              W[3] -= r.x * fy; W[4] -= r.y * fz; W[5] -= r.z * fx;
            });
+  // angular part (Eq.3, Eq.4): F_i += sum_{p in row i} (f_p - f_rev(p)),  W_i -= sum_p r_p (x) f_p with the pair forces
+  // f_p written by k_angular_force; the reverse forces are a dependent gather, so four pairs go through the two load
+  // levels together
+  if (fpair) {
+    const int q0 = segA[(size_t)a * (sp.T + 1)], q1 = segA[(size_t)a * (sp.T + 1) + sp.T];
+    for (int pb = q0; pb < q1; pb += 4) {
+      int rv[4];
+      float4 f[4], x[4], g[4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const bool ok = pb + i < q1;
+        rv[i] = ok ? revA[pb + i] : q0;
+        f[i] = ok ? fpair[pb + i] : make_float4(0.f, 0.f, 0.f, 0.f);
+        x[i] = ok ? pairA[pb + i] : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+#pragma unroll
+      for (int i = 0; i < 4; ++i) g[i] = pb + i < q1 ? fpair[rv[i]] : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        F[0] += f[i].x - g[i].x; F[1] += f[i].y - g[i].y; F[2] += f[i].z - g[i].z;
+        W[0] -= x[i].x * f[i].x; W[1] -= x[i].y * f[i].y; W[2] -= x[i].z * f[i].z;
+        W[3] -= x[i].x * f[i].y; W[4] -= x[i].y * f[i].z; W[5] -= x[i].z * f[i].x;
+      }
+    }
+  }
   Fat[a] = make_float4(F[0], F[1], F[2], 0.f);
 #pragma unroll
   for (int c = 0; c < 6; c += 2) *(float2 *)(Wat + (size_t)a * 6 + c) = make_float2(W[c], W[c + 1]);

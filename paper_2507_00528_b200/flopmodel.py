@@ -41,7 +41,7 @@ def phase_flops(spec, n_atoms, n_pairs_radial, n_pairs_angular):
     f["a2_network_forward"] = N * (4 * Nn * Nd + 2 * T * KR * NR + 12 * Nn)
     f["a3_radial_force"] = nR * (geom + _basis_ffp(KR) + 4 * KR + 30)
     f["a3_angular_force"] = nA * (geom + _basis_ffp(KA) + 4 * NA * KA + 4 * NA * NLM + HARM_BG + 9 * NLM + 40) + N * 3 * NA * NLM
-    f["a3_force_gather"] = nA * 3
+    f["a3_radial_force"] += nA * 3          # + the gather of the angular pair forces, done by the same kernel
     f["a4_loss_and_seeds"] = N * 20
     f["a5_radial_adjoint"] = nR * (geom + _basis_ffp(KR) + 2 * KR + 30) + N * 2 * T * KR * NR
     f["a5_angular_adjoint"] = nA * (geom + _basis_ffp(KA) + 2 * KA + HARM_BG + 8 * NLM + 4 * KA * NLM + 30) + N * (moments + 3 * NA * NLM)
@@ -69,7 +69,7 @@ def phase_bytes(spec, n_atoms, n_pairs_radial, n_pairs_angular):
     b["a2_network_forward"] = N * (4 * Nd + 4 * Nn + 4 + 4 * Nd + M_)
     b["a3_radial_force"] = (16 + 4 * KR) * nR + N * (M_ + 16 + 24)
     b["a3_angular_force"] = (16 + 4 + 16) * nA + N * (S_ + 4 * Nd)
-    b["a3_force_gather"] = (4 + 16 + 16 + 16) * nA + N * 2 * (16 + 24)
+    b["a3_radial_force"] += (4 + 16 + 16 + 16) * nA
     b["a4_loss_and_seeds"] = N * (4 + 16 + 24 + 12 + 16)
     b["a5_radial_adjoint"] = (16 + 16) * nR + N * (M_ + 4 * NR + 16)
     b["a5_angular_adjoint"] = (16 + 4 + 16) * nA + N * (2 * S_ + A_ + 4 * (Nd - NR) + 16)
