@@ -264,20 +264,16 @@ k_radial_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__res
   const AdjCtx ac = make_adj(u, omega, scales, a, struct_s[a]);
   const int *sg = segR + (size_t)a * (sp.T + 1);
   float *Mrow = M2 + (size_t)a * sp.T * KT;
-  // accumulated per Chebyshev term with w1 = (a.rhat) hdf, w2 = (a.rhat) hfcp:
-  //   aD[k] = sum w1 D_k, aT[k] = sum w2 T_k (k >= 1), aT[0] = sum w2;  M2[0] = 2 aT[0], M2[k] = aD[k] + aT[k] + aT[0]
-  float aD[KT], aT[KT];
+  // acc[k] = sum (a.rhat) f_k'(d),  f_0' = 2 hfcp, f_k' = D_k hdf + (T_k + 1) hfcp  (one accumulator per k keeps the
+  // kernel at 6 resident CTAs per SM; the walk lives on occupancy)
+  float acc[KT];
 #pragma unroll
-  for (int k = 0; k < KT; ++k) { aD[k] = 0.f; aT[k] = 0.f; }
+  for (int k = 0; k < KT; ++k) acc[k] = 0.f;
   walk_row(pairR, sg, sp.T,
            [&](int J) {
-             float m[KT];
-             m[0] = 2.f * aT[0];
+             store_row<KT>(Mrow + J * KT, acc);
 #pragma unroll
-             for (int k = 1; k < KT; ++k) m[k] = aD[k] + aT[k] + aT[0];
-             store_row<KT>(Mrow + J * KT, m);
-#pragma unroll
-             for (int k = 0; k < KT; ++k) { aD[k] = 0.f; aT[k] = 0.f; }
+             for (int k = 0; k < KT; ++k) acc[k] = 0.f;
            },
            [&](const float4 &r) { return u[__float_as_int(r.w)]; },
            [&](const float4 &r, const float4 &uj) {
@@ -288,9 +284,9 @@ k_radial_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__res
              const float ar = (ax * r.x + ay * r.y + az * r.z) * rinv;
              cheb_TD<KT>(d, sp.rcRinv, Tk, Dk, hfc, hfcp, hdf);
              const float w1 = ar * hdf, w2 = ar * hfcp;
-             aT[0] += w2;
+             acc[0] = fmaf(2.f, w2, acc[0]);
 #pragma unroll
-             for (int k = 1; k < KT; ++k) { aD[k] = fmaf(w1, Dk[k], aD[k]); aT[k] = fmaf(w2, Tk[k], aT[k]); }
+             for (int k = 1; k < KT; ++k) acc[k] = fmaf(w1, Dk[k], fmaf(w2, Tk[k], acc[k] + w2));
            });
   radial_contract<KT>(sp, cs, type_s[a], Mrow, D + (size_t)a * sp.Ndes);
 }
