@@ -169,12 +169,10 @@ k_radial_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__r
   load_row<KT>(etil + (size_t)a * TK, ei);
   walk_row(pairR, sg, sp.T,
            [&](int J) { if (J + 1 < sp.T) load_row<KT>(etil + (size_t)a * TK + (J + 1) * KT, ei); },
-           [&](const float4 &r) {
-             RowRegs<KT> g;
-             load_row<KT>(etil + (size_t)__float_as_int(r.w) * TK + I * KT, g.v);
-             return g;
-           },
-           [&](const float4 &r, const RowRegs<KT> &ej) {
+           [](const float4 &) { return 0; },
+           [&](const float4 &r, int) {
+             RowRegs<KT> ej;                              // requested first, used after the basis functions
+             load_row<KT>(etil + (size_t)__float_as_int(r.w) * TK + I * KT, ej.v);
              float d, rinv, Tk[KT], Dk[KT], hfc, hfcp, hdf;
              pair_len(r.x * r.x + r.y * r.y + r.z * r.z, d, rinv);
              cheb_TD<KT>(d, sp.rcRinv, Tk, Dk, hfc, hfcp, hdf);
