@@ -5,7 +5,6 @@
 #include <stdint.h>
 
 #define GNEP_NLM 24           // (l,m) slots for l = 1..4
-#define GNEP_WARPS 8          // warps per CTA of the warp-per-atom kernels
 #define GNEP_MAX_SPECIES_C 4   // == GNEP_MAX_SPECIES of include/gnep.h
 
 // Model constants passed by value to every kernel.
@@ -207,28 +206,6 @@ __device__ __forceinline__ void stg256(float *p, const float4 &a, const float4 &
                "f"(b.y), "f"(b.z), "f"(b.w)
                : "memory");
 }
-// Fixed-order warp reduction of K per-lane accumulators through shared memory:
-// returns sum over lanes of acc[lane_k] to lane k (k < K), 0 elsewhere.  buf: K*33 floats per warp.
-template <int K>
-__device__ __forceinline__ float warp_transpose_reduce(const float (&acc)[K], float *buf, int lane) {
-#pragma unroll
-  for (int k = 0; k < K; ++k) buf[k * 33 + lane] = acc[k];
-  __syncwarp();
-  float s = 0.f;
-  if (lane < K) {
-#pragma unroll 8
-    for (int i = 0; i < 32; ++i) s += buf[lane * 33 + i];
-  }
-  __syncwarp();
-  return s;
-}
-
-__device__ __forceinline__ float warp_sum(float v) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-  return v;
-}
-
 // stage the expansion coefficients c[I][J][n][k] into shared memory with k padded to KT (zeros)
 __device__ __forceinline__ void stage_coeff(float *dst, const float *src, int rows, int K, int KT) {
   for (int x = threadIdx.x; x < rows * KT; x += blockDim.x) {

@@ -214,7 +214,6 @@ inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 // ---- the forward half: descriptors, network, forces, per-structure sums (rows a1-a4) --------------
 int enqueue_descriptors(gnep_handle *h) {
   const DevSpec &d = h->ds;
-  int gridA = cdiv(h->N, GNEP_WARPS);
   DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_fwd<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, smem_radial(d), d, h->N, h->type_s, h->segR, h->pairR, h->theta, h->q, h->M1));
   mark(h, "a1_radial_descriptor");
   DISPATCH_KT(d.KAp, DISPATCH_NQ(d.NA, auto kf = k_angular_fwd<KT, NQ>; LAUNCH(h, kf, cdiv(h->N, ANG_WARPS * ANG_TA), ANG_WARPS * 32, smem_ang_fwd(d), d, h->N, h->type_s, h->segA, h->pairA, h->theta, h->q, h->Sn, h->A1)));
@@ -233,7 +232,6 @@ LossCfg loss_cfg(const gnep_handle *h) {
 
 int enqueue_forward(gnep_handle *h) {
   const DevSpec &d = h->ds;
-  int gridA = cdiv(h->N, GNEP_WARPS);
   RET_IF(enqueue_descriptors(h));
   LAUNCH(h, k_net_tc<false>, h->n_cta_net, 256, smem_net_fwd(d), d, h->sm, h->theta, h->qscale, h->q, h->x, h->Ei, h->Ep, h->etil,
          (const int *)nullptr, (const float *)nullptr, (const float *)nullptr, (float *)nullptr, (float *)nullptr);
@@ -253,7 +251,6 @@ int enqueue_forward(gnep_handle *h) {
 // ---- the backward half (rows a5-a8) ----------------------------------------------------------------
 int enqueue_backward(gnep_handle *h) {
   const DevSpec &d = h->ds;
-  int gridA = cdiv(h->N, GNEP_WARPS);
   DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_adj<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, smem_radial(d), d, h->N, h->type_s, h->struct_s, h->segR, h->pairR, h->theta, h->u, h->omega, h->scales, h->D, h->M2));
   mark(h, "a5_radial_adjoint");
   DISPATCH_KT(d.KAp, DISPATCH_NQ(d.NA, auto ka = k_angular_adj<KT, NQ>; LAUNCH(h, ka, cdiv(h->N, ANG_WARPS * ANG_TA), ANG_WARPS * 32, smem_ang_adj(d), d, h->N, h->type_s, h->struct_s, h->segA, h->atomA, h->pairA, h->theta, h->u, h->omega, h->scales, h->Sn, h->Tn, h->A2, h->D)));

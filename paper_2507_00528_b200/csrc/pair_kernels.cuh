@@ -9,11 +9,6 @@
 #pragma once
 #include "common.cuh"
 
-// per-warp dynamic shared memory helper
-__device__ __forceinline__ float *warp_smem(float *base, int per_warp_floats) {
-  return base + (threadIdx.x >> 5) * per_warp_floats;
-}
-
 #define RAD_THREADS 128
 #define RAD_PF 4        // pairs per prefetch group: the loads of a group are issued one whole group ahead
 
