@@ -79,3 +79,21 @@ def test_held_out_evaluation_on_a_shared_handle():
     parent.train_epochs(1, 1e-3)                      # training on the parent moves the shared parameters ...
     assert not np.allclose(test.evaluate()[:2], want[:2], rtol=1e-6)   # ... and the held-out errors with them
     test.destroy(); parent.destroy()
+
+
+def test_shared_handle_and_evaluate_error_paths():
+    import ctypes as C
+    from paper_2507_00528_b200 import Gnep, GnepError, load_library
+    import gnep_synth as gs
+    L = load_library()
+    out = C.c_void_p()
+    assert L.gnep_create_shared(None, C.byref(out)) == -1              # EINVAL: no parent
+    g = Gnep(dict(gs.MODEL_SPECS[0]))
+    child = g.create_shared()
+    with pytest.raises(GnepError) as e:
+        child.evaluate()                                                # ESTATE: the shared handle has no batch yet
+    assert e.value.code == -2
+    theta = gs.draw_params(dict(gs.MODEL_SPECS[0]), 0).astype(np.float32)
+    child.set_params(theta)                                             # parameters are one device buffer for both
+    np.testing.assert_array_equal(g.get_params(), theta)
+    child.destroy(); g.destroy()
