@@ -21,6 +21,7 @@ _STREAM_PARAMS_STUDENT = (1 << 40) + 1
 _STREAM_PARAMS_TEACHER = (1 << 40) + 2
 _STREAM_NOISE = (1 << 40) + 3
 _STREAM_SIZES = (1 << 40) + 4
+_STREAM_SPECIES = (1 << 40) + 5
 
 
 def _base(nr, kr, rcr, na, ka, rca, four, nn):
@@ -190,6 +191,15 @@ def make_batch(config, n_structs=None, first=0, workers=0):
                 positions=np.concatenate(P, axis=0) if P else np.zeros((0, 3)),
                 cells=np.stack(Cc, axis=0) if Cc else np.zeros((0, 9)),
                 types=np.concatenate(Tt, axis=0) if Tt else np.zeros((0,), dtype=np.int32))
+
+
+def relabel_species(types, n_species, config):
+    """Species ids for a model with `n_species` != 2 kinds of atoms on the same sites (test inputs for T = 1, 3, 4):
+    all zeros for one species, otherwise i.i.d. uniform draws from [0, n_species) on a stream of their own."""
+    n = len(types)
+    if n_species == 1:
+        return np.zeros(n, dtype=np.int32)
+    return _rng(config, _STREAM_SPECIES).integers(0, n_species, size=n).astype(np.int32)
 
 
 def draw_params(spec, config, which="student"):

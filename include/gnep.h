@@ -165,6 +165,13 @@ int gnep_set_opt_state(gnep_handle *h, const float *m, const float *v, int64_t s
 int gnep_batch_info(const gnep_handle *h, int64_t *n_atoms, int64_t *n_structs, int64_t *n_pairs_radial,
                     int64_t *n_pairs_angular);
 
+/* Measured plain-FP32 FMA peak of the device (the denominator of the ALU roofline next to the
+ * nominal 148 SM x 128 lanes x 2 x clock): a register-only FMA microbenchmark on every SM of the handle's device that
+ * runs for about min_ms milliseconds on the handle's stream (synchronises it).  tflops: HOST, achieved TFLOP/s
+ * (FMA = 2 flop); ms (may be NULL): the duration timed with CUDA events; implied_sm_mhz (may be NULL): the SM clock
+ * this rate corresponds to at 128 FP32 lanes per SM.  EINVAL unless 0 < min_ms <= 2000. */
+int gnep_measure_fp32_peak(gnep_handle *h, double min_ms, double *tflops, double *ms, double *implied_sm_mhz);
+
 /* Kernel launches issued by this handle since creation (for bench.py's gpu_launches). */
 int gnep_launch_count(const gnep_handle *h, int64_t *n);
 

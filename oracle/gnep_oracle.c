@@ -58,6 +58,7 @@ typedef struct {
   int *nsh[2];             /* 3 ints per pair */
   double *nr[2];           /* r_ij, 3 doubles per pair */
   double *Eref, *Fref, *Wref;   /* may be NULL */
+  double *we, *wf, *wv;         /* per-structure weights of the three loss terms (R40); NULL = all ones */
 } orc_batch;
 
 /* ------------------------------------------------------------------ sizes and layout (S:8(c).2) */
@@ -280,6 +281,7 @@ void orc_batch_destroy(orc_batch *b) {
   free(b->aoff); free(b->pos); free(b->cell); free(b->type);
   for (int w = 0; w < 2; ++w) { free(b->rptr[w]); free(b->nj[w]); free(b->nsh[w]); free(b->nr[w]); }
   free(b->Eref); free(b->Fref); free(b->Wref);
+  free(b->we); free(b->wf); free(b->wv);
   free(b);
 }
 
@@ -379,6 +381,24 @@ void orc_batch_get_neighbors(const orc_batch *b, int which, int64_t *rptr, int32
 void orc_batch_set_refs(orc_batch *b, const double *Eref, const double *Fref, const double *Wref) {
   free(b->Eref); free(b->Fref); free(b->Wref);
   b->Eref = dupd(Eref, b->S); b->Fref = dupd(Fref, (size_t)3 * b->N); b->Wref = dupd(Wref, (size_t)6 * b->S);
+}
+
+/* Per-structure loss weights (R40; the paper's sets mix structures with and without virials, and
+ * Eq.10-12 weigh every structure equally): a weight is the multiplicity of the structure in the training set, so a
+ * term is the weighted mean  sum_s w_s (...)_s / sum_s w_s  (forces: / (3 sum_s w_s N_s)); w = 0 masks a missing
+ * label, all ones (or NULL) is Eq.10-12 as printed.  Each array has S entries or is NULL. */
+void orc_batch_set_weights(orc_batch *b, const double *we, const double *wf, const double *wv) {
+  free(b->we); free(b->wf); free(b->wv);
+  b->we = dupd(we, b->S); b->wf = dupd(wf, b->S); b->wv = dupd(wv, b->S);
+}
+static double wgt(const double *w, int s) { return w ? w[s] : 1.0; }
+/* normalisers Z_E = sum w_e, Z_F = sum w_f N_s, Z_V = sum w_v  (= S, N, S without weights) */
+static void weight_norms(const orc_batch *b, double *Z) {
+  Z[0] = Z[1] = Z[2] = 0.0;
+  for (int s = 0; s < b->S; ++s) {
+    double Ns = b->aoff[s + 1] - b->aoff[s];
+    Z[0] += wgt(b->we, s); Z[1] += wgt(b->wf, s) * Ns; Z[2] += wgt(b->wv, s);
+  }
 }
 
 /* ------------------------------------------------------------------ per-atom forward pieces */
@@ -599,29 +619,34 @@ void orc_predict(const orc_spec *sp, const double *theta, const double *qs, cons
   }
 }
 
-/* loss terms from predictions: terms = {L, t_e, t_f, t_v, t_2}  (Eq.9-12; S:8(c).8) */
+/* loss terms from predictions: terms = {L, t_e, t_f, t_v, t_2}  (Eq.9-12; S:8(c).8; weights R40) */
 static void loss_terms(const orc_spec *sp, const double *theta, const orc_batch *b, const double *Es,
                        const double *F, const double *Ws, double *terms) {
   int64_t P = orc_num_params(sp);
-  double te = 0, tf = 0, tv = 0, t2 = 0;
-  if (b->Eref && b->S > 0) {
+  double te = 0, tf = 0, tv = 0, t2 = 0, Z[3];
+  weight_norms(b, Z);
+  if (b->Eref && Z[0] > 0) {
     for (int s = 0; s < b->S; ++s) {
       double Ns = b->aoff[s + 1] - b->aoff[s];
       double dE = Es[s] / Ns - b->Eref[s] / Ns;
-      te += dE * dE;
+      te += wgt(b->we, s) * dE * dE;
     }
-    te /= b->S;
+    te /= Z[0];
   }
-  if (b->Fref && b->N > 0) {
-    for (int64_t x = 0; x < (int64_t)3 * b->N; ++x) { double d = F[x] - b->Fref[x]; tf += d * d; }
-    tf /= 3.0 * b->N;
+  if (b->Fref && Z[1] > 0) {
+    for (int s = 0; s < b->S; ++s)
+      for (int64_t x = (int64_t)3 * b->aoff[s]; x < (int64_t)3 * b->aoff[s + 1]; ++x) {
+        double d = F[x] - b->Fref[x];
+        tf += wgt(b->wf, s) * d * d;
+      }
+    tf /= 3.0 * Z[1];
   }
-  if (b->Wref && b->S > 0) {
+  if (b->Wref && Z[2] > 0) {
     for (int s = 0; s < b->S; ++s) {
       double Ns = b->aoff[s + 1] - b->aoff[s];
-      for (int c = 0; c < 6; ++c) { double d = (Ws[6 * s + c] - b->Wref[6 * s + c]) / Ns; tv += d * d; }
+      for (int c = 0; c < 6; ++c) { double d = (Ws[6 * s + c] - b->Wref[6 * s + c]) / Ns; tv += wgt(b->wv, s) * d * d; }
     }
-    tv /= 6.0 * b->S;
+    tv /= 6.0 * Z[2];
   }
   for (int64_t p = 0; p < P; ++p) t2 += theta[p] * theta[p];
   t2 /= (double)P;
@@ -657,10 +682,13 @@ void orc_loss_and_grad(const orc_spec *sp, const double *theta, const double *qs
     me = terms[1] > 0 ? 0.5 / sqrt(terms[1]) : 0; mf = terms[2] > 0 ? 0.5 / sqrt(terms[2]) : 0;
     mv = terms[3] > 0 ? 0.5 / sqrt(terms[3]) : 0; m2 = terms[4] > 0 ? 0.5 / sqrt(terms[4]) : 0;
   }
+  double Z[3];
+  weight_norms(b, Z);
   double *u = (double *)calloc((size_t)3 * b->N + 1, sizeof(double));
-  if (b->Fref)
-    for (int64_t x = 0; x < (int64_t)3 * b->N; ++x)
-      u[x] = mf * 2.0 * sp->lam_f * (F[x] - b->Fref[x]) / (3.0 * b->N);
+  if (b->Fref && Z[1] > 0)
+    for (int s = 0; s < b->S; ++s)
+      for (int64_t x = (int64_t)3 * b->aoff[s]; x < (int64_t)3 * b->aoff[s + 1]; ++x)
+        u[x] = mf * 2.0 * sp->lam_f * wgt(b->wf, s) * (F[x] - b->Fref[x]) / (3.0 * Z[1]);
   for (int64_t p = 0; p < P; ++p) grad[p] = 0.0;
   int nmax = max_struct_atoms(b);
 #pragma omp parallel
@@ -680,10 +708,10 @@ void orc_loss_and_grad(const orc_spec *sp, const double *theta, const double *qs
       double Ns = a1 - a0;
       structure_forward(sp, &cx, theta, qs, b, s, &w, NULL, NULL, NULL);
       double e = 0.0, om[6] = {0, 0, 0, 0, 0, 0};
-      if (b->Eref) e = me * 2.0 * sp->lam_e * (Es[s] / Ns - b->Eref[s] / Ns) / (b->S * Ns);
-      if (b->Wref)
+      if (b->Eref && Z[0] > 0) e = me * 2.0 * sp->lam_e * wgt(b->we, s) * (Es[s] / Ns - b->Eref[s] / Ns) / (Z[0] * Ns);
+      if (b->Wref && Z[2] > 0)
         for (int c = 0; c < 6; ++c)
-          om[c] = mv * 2.0 * sp->lam_v * ((Ws[6 * s + c] - b->Wref[6 * s + c]) / Ns) / (6.0 * b->S * Ns);
+          om[c] = mv * 2.0 * sp->lam_v * wgt(b->wv, s) * ((Ws[6 * s + c] - b->Wref[6 * s + c]) / Ns) / (6.0 * Z[2] * Ns);
       for (int i = a0; i < a1; ++i) {
         int li = i - a0, I = b->type[i];
         const double *q = w.q + (size_t)li * Nd, *Sn = w.S + (size_t)li * NA * NLM_MAX;

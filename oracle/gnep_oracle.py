@@ -61,6 +61,7 @@ def lib():
         L.orc_batch_get_neighbors.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 4
         L.orc_batch_get_positions.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_batch_set_refs.argtypes = [C.c_void_p] * 4
+        L.orc_batch_set_weights.argtypes = [C.c_void_p] * 4
         L.orc_basis.argtypes = [C.c_double, C.c_int, C.c_double, C.c_void_p, C.c_void_p]
         L.orc_blm.argtypes = [C.c_double] * 3 + [C.c_void_p] * 2
         L.orc_blm_raw.argtypes = [C.c_double] * 3 + [C.c_void_p] * 2
@@ -163,6 +164,13 @@ class Batch:
     def set_refs(self, E, F, W):
         E, F, W = _f64(E), _f64(F), _f64(W)
         lib().orc_batch_set_refs(self.h, _p(E), _p(F), _p(W))
+
+    def set_weights(self, we=None, wf=None, wv=None):
+        """Per-structure weights of the energy / force / virial terms (R40); None = ones, 0 = no label."""
+        we, wf, wv = _f64(we), _f64(wf), _f64(wv)
+        for w in (we, wf, wv):
+            assert w is None or w.size == self.S
+        lib().orc_batch_set_weights(self.h, _p(we), _p(wf), _p(wv))
 
     def num_pairs(self, which):
         return int(lib().orc_batch_num_pairs(self.h, which))

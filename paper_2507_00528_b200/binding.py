@@ -19,7 +19,7 @@ EXPORTS = ["gnep_create", "gnep_destroy", "gnep_num_params", "gnep_num_descripto
            "gnep_descriptors", "gnep_predict", "gnep_loss_and_grad", "gnep_adam_step", "gnep_train_epochs",
            "gnep_get_opt_state", "gnep_set_opt_state", "gnep_batch_info", "gnep_launch_count",
            "gnep_set_profiling", "gnep_phase_times", "gnep_last_error", "gnep_set_global_norm", "gnep_set_grad",
-           "gnep_create_shared", "gnep_lr_schedule", "gnep_evaluate"]
+           "gnep_create_shared", "gnep_lr_schedule", "gnep_evaluate", "gnep_measure_fp32_peak"]
 
 ERRORS = {-1: "GNEP_EINVAL", -2: "GNEP_ESTATE", -3: "GNEP_ECUDA", -4: "GNEP_ENOMEM", -5: "GNEP_ERANGE",
           -6: "GNEP_ENONFINITE"}
@@ -80,6 +80,7 @@ def load_library(build_if_missing=True):
     L.gnep_evaluate.argtypes = [vp, C.POINTER(C.c_float)]
     L.gnep_lr_schedule.argtypes = [C.c_int64, C.c_int64, C.c_int64, C.c_double, C.c_double, C.POINTER(C.c_double)]
     L.gnep_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
+    L.gnep_measure_fp32_peak.argtypes = [vp, C.c_double] + [C.POINTER(C.c_double)] * 3
     L.gnep_set_profiling.argtypes = [vp, C.c_int]
     L.gnep_phase_times.argtypes = [vp, C.POINTER(C.c_char_p), C.POINTER(C.c_float), C.c_int32, C.POINTER(C.c_int32)]
     for name in EXPORTS:
@@ -107,6 +108,25 @@ def _ptr(a, dtype):
             return C.c_void_p(a.data_ptr()), 1, a
         a = a.numpy()
     a = np.ascontiguousarray(a, dtype=dtype)
+    return a.ctypes.data_as(C.c_void_p), 0, a
+
+
+def _out_ptr(a, dtype):
+    """Like _ptr for an OUTPUT buffer: the library writes into the caller's memory, so a buffer that would have to be
+    converted or copied (wrong dtype, non-contiguous, read-only) is an error, never a silent temporary."""
+    if a is None:
+        return None, None, None
+    if _is_torch(a):
+        import torch
+        want = {np.float32: torch.float32, np.float64: torch.float64, np.int32: torch.int32,
+                np.int64: torch.int64, np.int8: torch.int8}[dtype]
+        if a.dtype != want or not a.is_contiguous():
+            raise TypeError("output tensor must be contiguous %s" % want)
+        if a.is_cuda:
+            return C.c_void_p(a.data_ptr()), 1, a
+        a = a.numpy()
+    if not isinstance(a, np.ndarray) or a.dtype != np.dtype(dtype) or not a.flags.c_contiguous or not a.flags.writeable:
+        raise TypeError("output array must be a writeable C-contiguous numpy array of %s" % np.dtype(dtype))
     return a.ctypes.data_as(C.c_void_p), 0, a
 
 
@@ -182,7 +202,7 @@ class Gnep:
 
     def get_params(self, out=None):
         out = np.empty(self.num_params(), dtype=np.float32) if out is None else out
-        p, dev, _k = _ptr(out, np.float32)
+        p, dev, _k = _out_ptr(out, np.float32)
         self._ck(self._L.gnep_get_params(self._h, p, dev))
         return out
 
@@ -226,7 +246,7 @@ class Gnep:
     # ---- the hot path ----
     def descriptors(self, out=None):
         out = np.empty((self._n_atoms, self.num_descriptors()), dtype=np.float32) if out is None else out
-        p, dev, _k = _ptr(out, np.float32)
+        p, dev, _k = _out_ptr(out, np.float32)
         self._ck(self._L.gnep_descriptors(self._h, p, dev))
         return out
 
@@ -235,7 +255,7 @@ class Gnep:
             energy = np.empty(self._n_structs, dtype=np.float32)
             force = np.empty((self._n_atoms, 3), dtype=np.float32)
             virial = np.empty((self._n_structs, 6), dtype=np.float32)
-        pe, d1, _a = _ptr(energy, np.float32); pf, d2, _b = _ptr(force, np.float32); pw, d3, _c = _ptr(virial, np.float32)
+        pe, d1, _a = _out_ptr(energy, np.float32); pf, d2, _b = _out_ptr(force, np.float32); pw, d3, _c = _out_ptr(virial, np.float32)
         self._ck(self._L.gnep_predict(self._h, pe, pf, pw, _same_side([d1, d2, d3])))
         return energy, force, virial
 
@@ -243,7 +263,7 @@ class Gnep:
         terms = np.empty(5, dtype=np.float32) if want_terms else None
         if want_grad and grad is None:
             grad = np.empty(self.num_params(), dtype=np.float32)
-        pg, dev, _k = _ptr(grad, np.float32)
+        pg, dev, _k = _out_ptr(grad, np.float32)
         pt = None if terms is None else terms.ctypes.data_as(C.c_void_p)
         self._ck(self._L.gnep_loss_and_grad(self._h, pt, pg, dev or 0))
         return terms, grad
@@ -282,6 +302,12 @@ class Gnep:
         return np.array(out[:], dtype=np.float32)
 
     # ---- profiling ----
+    def measure_fp32_peak(self, min_ms=60.0):
+        """dict(tflops, ms, implied_sm_mhz) of the FP32 FMA microbenchmark (gnep_measure_fp32_peak)."""
+        v = [C.c_double() for _ in range(3)]
+        self._ck(self._L.gnep_measure_fp32_peak(self._h, float(min_ms), *[C.byref(x) for x in v]))
+        return dict(tflops=v[0].value, ms=v[1].value, implied_sm_mhz=v[2].value)
+
     def set_profiling(self, on):
         self._ck(self._L.gnep_set_profiling(self._h, int(on)))
 

@@ -16,6 +16,7 @@
 #include "pair_kernels.cuh"
 #include "angular_kernels.cuh"
 #include "reduce_kernels.cuh"
+#include "peak_kernels.cuh"
 
 namespace {
 
@@ -46,6 +47,7 @@ struct gnep_handle {
   int64_t nR = 0, nA = 0, nAp = 0;   // nAp: angular pairs including the padding dummies
   int hasE = 0, hasF = 0, hasV = 0;
   double Ng = -1, Sg = -1, l2_share = 1.0;   // job-wide normalisers when structures are sharded over ranks
+  bool eval_local = false;                   // set while gnep_evaluate runs: RMSEs of the resident batch, whatever the job norm
   std::vector<void *> batch_allocs;
   int *perm = nullptr, *type_s = nullptr, *struct_s = nullptr, *segR = nullptr, *rowAs = nullptr, *segA = nullptr, *atomA = nullptr;
   int *rowAu = nullptr, *segAu = nullptr, *atomAu = nullptr, *revAu = nullptr;   // unpadded angular list (force + gather kernels)
@@ -155,7 +157,9 @@ size_t smem_cgrad_rad(const DevSpec &d) { return cgrad_radial_smem_bytes(d); }
 template <class K>
 int set_smem(gnep_handle *h, K kernel, size_t bytes) {
   if (bytes > 227 * 1024) return fail(h, GNEP_EINVAL, "model too large for shared memory staging (n_neurons x n_descriptors)");
-  CK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+  // the attribute is process-wide per kernel: always the hardware maximum, so that a later, smaller model never lowers
+  // the limit under a live handle (each launch still asks only for what its own model needs)
+  CK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
   return GNEP_OK;
 }
 
@@ -226,7 +230,8 @@ LossCfg loss_cfg(const gnep_handle *h) {
   lc.S = h->S; lc.N = h->N; lc.T = h->ds.T; lc.P = h->ds.P;
   lc.hasE = h->hasE; lc.hasF = h->hasF; lc.hasV = h->hasV; lc.loss_mode = h->ds.loss_mode;
   lc.lam_e = h->spec.lambda_e; lc.lam_f = h->spec.lambda_f; lc.lam_v = h->spec.lambda_v; lc.lam_2 = h->spec.lambda_2;
-  lc.Ng = h->Ng >= 0 ? h->Ng : (double)h->N; lc.Sg = h->Sg >= 0 ? h->Sg : (double)h->S; lc.l2_share = h->l2_share;
+  const bool job = h->Ng >= 0 && !h->eval_local;   // gnep_evaluate always normalises by the resident batch itself
+  lc.Ng = job ? h->Ng : (double)h->N; lc.Sg = job ? h->Sg : (double)h->S; lc.l2_share = job ? h->l2_share : 1.0;
   return lc;
 }
 
@@ -378,7 +383,8 @@ int gnep_create(const gnep_model_spec *spec, void *cuda_stream, gnep_handle **ou
   }
   int rc;
   if ((rc = configure_kernels(h)) != GNEP_OK) return bail(rc);
-  // constants: 2 C_lm with C_lm = (2l+1)/(4 pi) Chat_lm (R11-R12), kappa4 (R14)
+  // constants: 2 C_lm with C_lm = (2l+1)/(4 pi) Chat_lm (R11-R12), kappa4 (R14).  Process-global __constant__
+  // memory, so the tables must not depend on this handle's spec (two live handles of different l_max share them)
   {
     const double chat[GNEP_NLM] = {1, 1, 1, 1.0 / 4, 3, 3, 3.0 / 4, 3.0 / 4, 1.0 / 4, 3.0 / 8, 3.0 / 8, 15.0 / 4, 15.0 / 4, 5.0 / 8,
                                    5.0 / 8, 1.0 / 64, 5.0 / 8, 5.0 / 8, 5.0 / 16, 5.0 / 16, 35.0 / 8, 35.0 / 8, 35.0 / 64, 35.0 / 64};
@@ -387,7 +393,7 @@ int gnep_create(const gnep_model_spec *spec, void *cuda_stream, gnep_handle **ou
     for (int lm = 0; lm < GNEP_NLM; ++lm) {
       int l = lm < 3 ? 1 : lm < 8 ? 2 : lm < 15 ? 3 : 4;
       lf[lm] = (float)l;
-      c2[lm] = l <= d.L ? (float)(2.0 * (2 * l + 1) / (4.0 * pi) * chat[lm]) : 0.f;
+      c2[lm] = (float)(2.0 * (2 * l + 1) / (4.0 * pi) * chat[lm]);   // the same for every handle: the kernels guard on sp.L
     }
     float k4 = (float)(-5.0 * std::sqrt(14.0) / (448.0 * pi * std::sqrt(pi)));
     if (cudaMemcpyToSymbol(c_C2, c2, sizeof(c2)) != cudaSuccess || cudaMemcpyToSymbol(c_lf, lf, sizeof(lf)) != cudaSuccess ||
@@ -659,6 +665,9 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
       CKT(cudaMemcpyAsync(h->struct_s, struct_s.data(), sizeof(int) * N, cudaMemcpyHostToDevice, st));
     }
     CKT(cudaMemcpyAsync(h->srange, srange.data(), sizeof(int) * srange.size(), cudaMemcpyHostToDevice, st));
+    // radial rows are padded to an even record count and the walk loads records in pairs: the pad slots (and the two
+    // records past the last row) must hold a valid neighbour index for the one-ahead gather of k_radial_adj
+    CKT(cudaMemsetAsync(h->pairR, 0, sizeof(float4) * ((size_t)rowRs[N] + 2), st));
     LAUNCH(h, k_nbr_fill, gN, 128, 0, N, d_struct_of, d_geo, d_wpos, d_binid, d_bin_start, d_bin_atoms, rcR2, rcA2, h->exp_row[0], d_ekey, d_er);
     LAUNCH(h, k_nbr_scatter, cdiv((int64_t)N * 32, 256), 256, 0, N, T, d_struct_of, d_geo, d_type, d_inv, h->exp_row[0], h->exp_row[1], d_rowRs,
            d_rowAu, d_ekey, d_er, h->exp_j[0], h->exp_sh[0], h->exp_j[1], h->exp_sh[1], h->pairR, d_pairAu, d_shA, h->segR, d_segAu, d_atomAu);
@@ -841,7 +850,10 @@ int gnep_evaluate(gnep_handle *h, float *rmse) {
   if (!h->loaded) return fail(h, GNEP_ESTATE, "no batch loaded");
   float t[5] = {0, 0, 0, 0, 0};
   if (h->N > 0 || h->S > 0) {
-    RET_IF(enqueue_forward(h));
+    h->eval_local = true;
+    int rc = enqueue_forward(h);
+    h->eval_local = false;
+    RET_IF(rc);
     RET_IF(check_launch(h));
     RET_IF(fetch_terms(h, t));
   }
@@ -904,6 +916,41 @@ int gnep_set_global_norm(gnep_handle *h, int64_t n_atoms_global, int64_t n_struc
 int gnep_set_grad(gnep_handle *h, const float *grad, int is_device) {
   if (!h || !grad) return fail(h, GNEP_EINVAL, "null argument");
   return copy_in(h, h->grad, grad, h->ds.P * sizeof(float), is_device);
+}
+
+int gnep_measure_fp32_peak(gnep_handle *h, double min_ms, double *tflops, double *ms_out, double *sm_mhz) {
+  if (!h || !tflops) return fail(h, GNEP_EINVAL, "null argument");
+  if (!(min_ms > 0) || min_ms > 2000) return fail(h, GNEP_EINVAL, "min_ms must be in (0, 2000]");
+  const int grid = h->num_sms * 8, block = 256;     // 2048 resident threads per SM
+  float *sink = nullptr;
+  CK(cudaMalloc((void **)&sink, sizeof(float) * (size_t)grid * block));
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  auto run = [&](int iters, float *ms) -> cudaError_t {
+    cudaEventRecord(e0, h->stream);
+    k_ffma_peak<<<grid, block, 0, h->stream>>>(iters, 0.999f, 1e-3f, sink);
+    h->launches++;
+    cudaEventRecord(e1, h->stream);
+    cudaError_t e = cudaEventSynchronize(e1);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(ms, e0, e1);
+    return e;
+  };
+  float ms = 0.f;
+  int iters = 4096;
+  cudaError_t e = run(iters, &ms);                  // warm-up and calibration
+  if (e == cudaSuccess) {
+    const double want = min_ms / std::max((double)ms, 1e-3) * iters;
+    iters = (int)std::min(std::max(want, 4096.0), 2.0e8);
+    e = run(iters, &ms);
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(sink);
+  if (e != cudaSuccess) return fail(h, GNEP_ECUDA, std::string("fp32 peak measurement: ") + cudaGetErrorString(e));
+  const double flops = 2.0 * PEAK_CHAINS * PEAK_UNROLL * (double)iters * (double)grid * block;
+  *tflops = flops / (ms * 1e-3) / 1e12;
+  if (ms_out) *ms_out = ms;
+  if (sm_mhz) *sm_mhz = *tflops * 1e12 / (2.0 * 128.0 * h->num_sms) / 1e6;   // the clock this rate implies at 128 lanes / SM
+  return GNEP_OK;
 }
 
 int gnep_launch_count(const gnep_handle *h, int64_t *n) {

@@ -22,8 +22,9 @@ __device__ __forceinline__ void walk_row(const float4 *__restrict__ pairR, const
   const int pend = sg[T];
   const float4 dum = make_float4(1.f, 0.f, 0.f, 0.f);      // w = bits(0): a valid atom index for the gather
   float4 nb[RAD_PF];
-  // rows start at even record indices and p advances by RAD_PF: two records per 256-bit load (the second may lie past
-  // the row's end -- in the row's pad slot or the next row -- and is then ignored)
+  // rows start at even record indices and p advances by RAD_PF: two records per 256-bit load.  The second may lie past
+  // the row's end -- in the row's pad slot (zeroed at load: w = bits(0), a valid index) or in the next row -- its body
+  // is skipped, but gather() still runs on it one pair ahead, so its w must always be a valid atom index
   auto load2 = [&](int q, float4 &r0, float4 &r1) {
     if (q < pend) { const float8 v = ldg256((const float *)(pairR + q)); r0 = v.lo; r1 = v.hi; }
     else { r0 = dum; r1 = dum; }

@@ -55,8 +55,13 @@ def setup_sharded(engine, dist, n_atoms_local, n_structs_local, device=None):
 def sharded_step(engine, dist, grad, lr, **adam):
     """One epoch on every rank: partial loss+gradient, all-reduce (sum) of the gradient, identical Adam step.
     `grad` is a float32 torch tensor of P entries on the engine's device, reused every step."""
-    engine.loss_and_grad(want_terms=False, grad=grad)
+    engine.loss_and_grad(want_terms=False, grad=grad)      # returns after the engine's stream has written `grad`
     dist.all_reduce(grad)
+    if getattr(grad, "is_cuda", False):
+        # the collective is ordered on torch's current stream, gnep_set_grad copies on the ENGINE's stream: finish the
+        # reduction before handing the buffer over (P floats, latency-bound; correct for any pairing of streams)
+        import torch
+        torch.cuda.current_stream(grad.device).synchronize()
     engine.set_grad(grad)
     engine.adam_step(lr, **adam)
 

@@ -25,6 +25,8 @@ def labelled_case(config, n_structs=None, spec_over=None, noise=True):
         spec.update(spec_over)
     sp = orc.make_spec(spec)
     b = gs.make_batch(config, n_structs=n_structs)
+    if spec["n_species"] != 2:
+        b["types"] = gs.relabel_species(b["types"], spec["n_species"], config)
     ob = orc.Batch(sp, b["atom_offsets"], b["positions"], b["cells"], b["types"])
     theta = gs.draw_params(spec, config, "student")
     teacher = gs.draw_params(spec, config, "teacher")

@@ -42,8 +42,12 @@ def test_minibatch_trajectory_matches_oracle(config, n_structs, bs):
             assert lr_schedule(s, n_warm, n_total, 1e-3, 1e-5) == pytest.approx(lr, rel=1e-14)
             t_ref, g_ref = orc.loss_and_grad(sp, th, qs, obatches[k])
             orc.adam_step(th, m, v, g_ref, s + 1, lr)
+            th_seen = handles[k].get_params().astype(np.float64)         # the parameters this step's loss is evaluated at
             terms = handles[k].train_epochs(1, lr)
-            assert abs(terms[0] - t_ref[0]) <= 2e-5 * abs(t_ref[0])     # the loss the step saw (same parameters so far)
+            # loss parity at 1e-5 on IDENTICAL parameters (the two trajectories drift apart at the 1e-6 level, which the
+            # final parameter check bounds; the loss of the oracle's own trajectory agrees to 1e-4)
+            assert abs(terms[0] - orc.loss(sp, th_seen, qs, obatches[k])[0]) <= 1e-5 * abs(t_ref[0])
+            assert abs(terms[0] - t_ref[0]) <= 1e-4 * abs(t_ref[0])
             s += 1
     for h in handles:                                                    # every handle sees the same shared state
         th_gpu = h.get_params().astype(np.float64)
@@ -67,15 +71,15 @@ def test_held_out_evaluation_on_a_shared_handle():
     test.load_batch(off, pos, cells, types, E, F, W)
     o = orc.Batch(sp, off, pos, cells, types); o.set_refs(E, F, W)
     t_ref, _ = orc.loss_and_grad(sp, theta, qs, o)
-    np.testing.assert_allclose(test.evaluate(), np.sqrt(t_ref[1:4]), rtol=2e-5)
+    np.testing.assert_allclose(test.evaluate(), np.sqrt(t_ref[1:4]), rtol=1e-5)
     # independent restatement from the oracle's predictions: RMSE over structures / atoms x 3 / structures x 6
     Ep, Fp, Wp = orc.predict(sp, theta, qs, o)
     ns = np.diff(off)
     want = [np.sqrt(np.mean(((Ep - E) / ns) ** 2)), np.sqrt(np.mean((Fp - F) ** 2)), np.sqrt(np.mean(((Wp - W) / ns[:, None]) ** 2))]
-    np.testing.assert_allclose(test.evaluate(), want, rtol=2e-5)
+    np.testing.assert_allclose(test.evaluate(), want, rtol=1e-5)
     test.set_targets(E, F, None)
     r = test.evaluate()
-    assert r[2] == 0.0 and r[0] == pytest.approx(want[0], rel=2e-5)
+    assert r[2] == 0.0 and r[0] == pytest.approx(want[0], rel=1e-5)
     parent.train_epochs(1, 1e-3)                      # training on the parent moves the shared parameters ...
     assert not np.allclose(test.evaluate()[:2], want[:2], rtol=1e-6)   # ... and the held-out errors with them
     test.destroy(); parent.destroy()
