@@ -44,7 +44,8 @@ WORKLOAD_NAMES = {0: "cfg0-tiny-sc", 1: "cfg1-rocksalt-100x216", 2: "cfg2-liquid
 
 
 def n_descriptors(spec):
-    return spec["n_radial"] + spec["n_angular"] * spec["l_max"] + (spec["n_angular"] if spec["use_4body"] else 0)
+    return (spec["n_radial"] + spec["n_angular"] * spec["l_max"] + (spec["n_angular"] if spec["use_4body"] else 0)
+            + (spec["n_angular"] if spec.get("use_5body") else 0))
 
 
 def n_params(spec):

@@ -25,7 +25,7 @@
  *   | cA[I][J][n][k]
  *   | for each species t: W0_t[mu][nu] (nu fastest), b0_t[mu], w1_t[mu], b1_t ]         (P:718 Eq.D1.1)
  * Descriptor index nu: 0..NR-1 radial q_n (Eq.5); NR+(l-1)*NA+n three-body q_nl, l=1..l_max
- * (Eq.7); NR+l_max*NA+n four-body (R14).
+ * (Eq.7); then NA four-body terms (R14) if use_4body; then NA five-body terms (R41) if use_5body.
  */
 #ifndef GNEP_H
 #define GNEP_H
@@ -58,8 +58,9 @@ typedef struct {
   double rc_radial;                      /* radial cutoff r_c^R (Eq.2)                                   */
   int32_t n_angular, n_basis_angular;    /* NA, KA (own coefficients cA, R4)                             */
   double rc_angular;                     /* 0 < rc_angular <= rc_radial                                  */
-  int32_t l_max;                         /* 1..4 (Eq.7; l = 5..8 not built)                              */
-  int32_t use_4body;                     /* 0/1, needs l_max >= 2 (R14)                                  */
+  int32_t l_max;                         /* 1..8 (Eq.7; b_lm of App.B)                  */
+  int32_t use_4body;                     /* 0/1, needs l_max >= 2: cubic invariant of the l = 2 moments (R14) */
+  int32_t use_5body;                     /* 0/1: quartic invariant of the l = 1 moments (R41) */
   int32_t n_neurons;                     /* hidden width N_neu, 1..GNEP_MAX_NEURONS                      */
   double lambda_e, lambda_f, lambda_v;   /* Eq.9 weights                                                 */
   double lambda_2;                       /* weight of t_2 = mean(theta^2) (R22; not in the paper)        */
@@ -102,6 +103,20 @@ int gnep_load_batch(gnep_handle *h, int32_t n_structs, const int32_t *atom_offse
 int gnep_set_targets(gnep_handle *h, const double *ref_energy, const double *ref_force,
                      const double *ref_virial, int is_device);
 
+/* Per-structure loss weights (real training sets mix structures with and without virial labels, P:138,
+ * while Eq.10-12, weigh every structure equally).  Reading R40: a weight is the multiplicity of the structure
+ * in the training set, so each term is a weighted mean,
+ *   t_e = sum_s w_e,s dE_s^2 / Z_E,  t_f = sum_s w_f,s sum_{i in s} |dF_i|^2 / (3 Z_F),  t_v = sum_s w_v,s sum_c dW_s,c^2 / (6 Z_V),
+ *   Z_E = sum_s w_e,s,  Z_F = sum_s w_f,s N_s,  Z_V = sum_s w_v,s,
+ * which is Eq.10-12 as printed when all weights are 1 (the default after gnep_load_batch) and the mean over the
+ * labelled structures when w is a 0/1 mask (w = 0: that structure has no such label; its reference entry is ignored).
+ * w_e, w_f, w_v: S doubles each, or NULL (= ones).  EINVAL on a negative or non-finite weight. */
+int gnep_set_weights(gnep_handle *h, const double *w_e, const double *w_f, const double *w_v, int is_device);
+
+/* The three normalisers {Z_E, Z_F, Z_V} of the resident batch (HOST, 3 doubles): what a rank contributes to the
+ * job-wide normalisers under structure sharding (gnep_set_global_norms). */
+int gnep_loss_norms(const gnep_handle *h, double *z);
+
 /* Parity aid: the neighbour list in canonical order (rows by atom, entries ascending (j, sa, sb, sc)),
  * which: 0 radial, 1 angular.  n_pairs (host, may be NULL) receives the pair count; row_ptr N+1 int64;
  * j and shift3 (3 int8 per pair) hold `capacity` pairs; if capacity < n_pairs only n_pairs is set
@@ -136,6 +151,10 @@ int gnep_train_epochs(gnep_handle *h, int32_t n_epochs, float lr, float beta1, f
  * caller all-reduces (sum) the P gradient floats, hands the result back with gnep_set_grad and calls
  * gnep_adam_step on every rank.  Negative counts restore single-GPU behaviour.  loss_mode 0 only. */
 int gnep_set_global_norm(gnep_handle *h, int64_t n_atoms_global, int64_t n_structs_global, double l2_share);
+/* The same with per-structure weights: z = job-wide {Z_E, Z_F, Z_V} (HOST, 3 doubles: the all-reduced sums of every
+ * rank's gnep_loss_norms); gnep_set_global_norm(N, S, share) is z = {S, N, S}.  NULL or a negative entry restores
+ * single-GPU behaviour. */
+int gnep_set_global_norms(gnep_handle *h, const double *z, double l2_share);
 int gnep_set_grad(gnep_handle *h, const float *grad, int is_device);
 
 /* Mini-batch training (the paper's regime is mini-batches of size 1).  A shared handle is a

@@ -19,7 +19,8 @@ EXPORTS = ["gnep_create", "gnep_destroy", "gnep_num_params", "gnep_num_descripto
            "gnep_descriptors", "gnep_predict", "gnep_loss_and_grad", "gnep_adam_step", "gnep_train_epochs",
            "gnep_get_opt_state", "gnep_set_opt_state", "gnep_batch_info", "gnep_launch_count",
            "gnep_set_profiling", "gnep_phase_times", "gnep_last_error", "gnep_set_global_norm", "gnep_set_grad",
-           "gnep_create_shared", "gnep_lr_schedule", "gnep_evaluate", "gnep_measure_fp32_peak"]
+           "gnep_create_shared", "gnep_lr_schedule", "gnep_evaluate", "gnep_measure_fp32_peak", "gnep_set_weights",
+           "gnep_loss_norms", "gnep_set_global_norms"]
 
 ERRORS = {-1: "GNEP_EINVAL", -2: "GNEP_ESTATE", -3: "GNEP_ECUDA", -4: "GNEP_ENOMEM", -5: "GNEP_ERANGE",
           -6: "GNEP_ENONFINITE"}
@@ -35,7 +36,7 @@ class ModelSpec(C.Structure):
     _fields_ = [("n_species", C.c_int32), ("n_radial", C.c_int32), ("n_basis_radial", C.c_int32),
                 ("rc_radial", C.c_double), ("n_angular", C.c_int32), ("n_basis_angular", C.c_int32),
                 ("rc_angular", C.c_double), ("l_max", C.c_int32), ("use_4body", C.c_int32),
-                ("n_neurons", C.c_int32), ("lambda_e", C.c_double), ("lambda_f", C.c_double),
+                ("use_5body", C.c_int32), ("n_neurons", C.c_int32), ("lambda_e", C.c_double), ("lambda_f", C.c_double),
                 ("lambda_v", C.c_double), ("lambda_2", C.c_double), ("loss_mode", C.c_int32),
                 ("q_scale", C.POINTER(C.c_float))]
 
@@ -76,6 +77,9 @@ def load_library(build_if_missing=True):
     L.gnep_batch_info.argtypes = [vp] + [C.POINTER(C.c_int64)] * 4
     L.gnep_set_global_norm.argtypes = [vp, C.c_int64, C.c_int64, C.c_double]
     L.gnep_set_grad.argtypes = [vp, vp, C.c_int]
+    L.gnep_set_weights.argtypes = [vp, vp, vp, vp, C.c_int]
+    L.gnep_loss_norms.argtypes = [vp, C.POINTER(C.c_double)]
+    L.gnep_set_global_norms.argtypes = [vp, C.POINTER(C.c_double), C.c_double]
     L.gnep_create_shared.argtypes = [vp, C.POINTER(vp)]
     L.gnep_evaluate.argtypes = [vp, C.POINTER(C.c_float)]
     L.gnep_lr_schedule.argtypes = [C.c_int64, C.c_int64, C.c_int64, C.c_double, C.c_double, C.POINTER(C.c_double)]
@@ -234,6 +238,18 @@ class Gnep:
         pe, d4, k4 = _ptr(ref_energy, np.float64); pf, d5, k5 = _ptr(ref_force, np.float64); pw, d6, k6 = _ptr(ref_virial, np.float64)
         self._ck(self._L.gnep_set_targets(self._h, pe, pf, pw, _same_side([d4, d5, d6])))
 
+    def set_weights(self, w_e=None, w_f=None, w_v=None):
+        """Per-structure weights of the energy / force / virial terms (None = ones, 0 = structure has no such label)."""
+        pe, d1, _a = _ptr(w_e, np.float64); pf, d2, _b = _ptr(w_f, np.float64); pv, d3, _c = _ptr(w_v, np.float64)
+        for w in (_a, _b, _c):
+            assert w is None or int(np.prod(w.shape)) == self._n_structs
+        self._ck(self._L.gnep_set_weights(self._h, pe, pf, pv, _same_side([d1, d2, d3])))
+
+    def loss_norms(self):
+        z = (C.c_double * 3)()
+        self._ck(self._L.gnep_loss_norms(self._h, z))
+        return np.array(z[:], dtype=np.float64)
+
     def neighbor_list(self, which):
         n = C.c_int64()
         self._ck(self._L.gnep_neighbor_list(self._h, which, C.byref(n), None, None, None, 0, 0))
@@ -280,6 +296,10 @@ class Gnep:
     # ---- structure sharding over ranks ----
     def set_global_norm(self, n_atoms_global, n_structs_global, l2_share):
         self._ck(self._L.gnep_set_global_norm(self._h, int(n_atoms_global), int(n_structs_global), float(l2_share)))
+
+    def set_global_norms(self, z, l2_share):
+        zz = (C.c_double * 3)(*[float(x) for x in z])
+        self._ck(self._L.gnep_set_global_norms(self._h, zz, float(l2_share)))
 
     def set_grad(self, grad):
         p, dev, _k = _ptr(grad, np.float32)

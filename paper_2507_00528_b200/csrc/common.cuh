@@ -4,12 +4,14 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#define GNEP_NLM 24           // (l,m) slots for l = 1..4
 #define GNEP_MAX_SPECIES_C 4   // == GNEP_MAX_SPECIES of include/gnep.h
+#define GNEP_LMAX 8            // largest l_max (paper Eq.7: l = 1..8)
+#define GNEP_NLM_MAX 80        // (l,m) slots for l = 1..8; slot lm = l*l - 1 + m, m = 0..2l
 
 // Model constants passed by value to every kernel.
 struct DevSpec {
-  int T, NR, KR, NA, KA, L, use4, Nn, Ndes, P;
+  int T, NR, KR, NA, KA, L, use4, use5, Nn, Ndes, P;
+  int nlmS;                   // row stride of the per-atom (l,m) arrays S, T, beta, A1: 24 for l_max <= 4, 84 above
   int NnS;                    // row stride of the hidden-layer buffers x, p: Nn padded to 8 (32-byte rows, 256-bit accesses)
   int KRp, KAp;               // basis sizes padded to the template size of the pair kernels
   int offA, offNet, netSize;  // parameter-vector offsets (include/gnep.h layout)
@@ -19,12 +21,36 @@ struct DevSpec {
   float lam_e, lam_f, lam_v, lam_2;
 };
 
-// 2*C_lm (C_lm = (2l+1)/(4 pi) * Chat_lm, zero for l > l_max), l of each slot, kappa4.
-__constant__ float c_C2[GNEP_NLM];
-__constant__ float c_lf[GNEP_NLM];
-__constant__ float c_kappa4;
+// l of slot lm
+__host__ __device__ constexpr int blm_l(int lm) {
+  int l = 1;
+  while ((l + 1) * (l + 1) - 1 <= lm) ++l;
+  return l;
+}
 
-__device__ __forceinline__ int l_of_lm(int lm) { return lm < 3 ? 1 : lm < 8 ? 2 : lm < 15 ? 3 : 4; }
+// 2*C_lm with C_lm = (2l+1)/(4 pi) * Chat_lm (R11-R12): Chat_lm is fixed by the addition theorem
+// sum_m Chat_lm b_lm(r1) b_lm(r2) = r1^l r2^l P_l(cos theta12) for the paper's b_lm (App.B); one entry for m = 0, then one
+// per (cos, sin) pair.  Compile-time table: the same for every model, so nothing per-handle lives in constant memory.
+#define GNEP_C2(l, chat) ((float)(2.0 * (2 * (l) + 1) / (4.0 * 3.14159265358979323846) * (chat)))
+#define GNEP_C2P(l, chat) GNEP_C2(l, chat), GNEP_C2(l, chat)
+__constant__ float c_C2[GNEP_NLM_MAX + 4] = {
+    GNEP_C2(1, 1.0), GNEP_C2P(1, 1.0),
+    GNEP_C2(2, 1.0 / 4), GNEP_C2P(2, 3.0), GNEP_C2P(2, 3.0 / 4),
+    GNEP_C2(3, 1.0 / 4), GNEP_C2P(3, 3.0 / 8), GNEP_C2P(3, 15.0 / 4), GNEP_C2P(3, 5.0 / 8),
+    GNEP_C2(4, 1.0 / 64), GNEP_C2P(4, 5.0 / 8), GNEP_C2P(4, 5.0 / 16), GNEP_C2P(4, 35.0 / 8), GNEP_C2P(4, 35.0 / 64),
+    GNEP_C2(5, 1.0 / 64), GNEP_C2P(5, 15.0 / 64), GNEP_C2P(5, 105.0 / 16), GNEP_C2P(5, 35.0 / 128), GNEP_C2P(5, 315.0 / 64),
+    GNEP_C2P(5, 63.0 / 128),
+    GNEP_C2(6, 1.0 / 256), GNEP_C2P(6, 21.0 / 64), GNEP_C2P(6, 105.0 / 512), GNEP_C2P(6, 105.0 / 128), GNEP_C2P(6, 63.0 / 256),
+    GNEP_C2P(6, 693.0 / 128), GNEP_C2P(6, 231.0 / 512),
+    GNEP_C2(7, 1.0 / 256), GNEP_C2P(7, 7.0 / 1024), GNEP_C2P(7, 21.0 / 512), GNEP_C2P(7, 21.0 / 1024), GNEP_C2P(7, 231.0 / 256),
+    GNEP_C2P(7, 231.0 / 1024), GNEP_C2P(7, 3003.0 / 512), GNEP_C2P(7, 429.0 / 1024),
+    GNEP_C2(8, 1.0 / 16384), GNEP_C2P(8, 9.0 / 1024), GNEP_C2P(8, 315.0 / 2048), GNEP_C2P(8, 1155.0 / 1024),
+    GNEP_C2P(8, 693.0 / 4096), GNEP_C2P(8, 9009.0 / 1024), GNEP_C2P(8, 429.0 / 2048), GNEP_C2P(8, 6435.0 / 1024),
+    GNEP_C2P(8, 6435.0 / 16384),
+    0.f, 0.f, 0.f, 0.f};
+// kappa4 = -5 sqrt(14) / (448 pi^(3/2)) (R14); kappa5 = 3 / (16 pi^2) (R41)
+#define GNEP_KAPPA4 (-0.0074994808266641f)
+#define GNEP_KAPPA5 (0.018997721932938f)
 
 // ---------------------------------------------------------------------------------------------
 // Pair geometry: d = |r| and 1/d from one MUFU.RSQ and one Newton step (relative error ~1e-7, as sqrtf + division).
@@ -123,13 +149,14 @@ __device__ __forceinline__ void cheb_ffp(float d, float rcinv, float (&f)[KT], f
 }
 
 // ---------------------------------------------------------------------------------------------
-// Real harmonics of a UNIT vector (paper App.B): emits, for each of the 24 (l,m) slots,
+// Real harmonics of a UNIT vector (paper App.B): emits, for each of the LMAX (LMAX + 2) (l,m) slots,
 // b = b_lm(rhat) and g = (grad b_lm)(rhat)  [polynomial gradient, r^2 terms differentiated, then r=1].
 // With B_lm = b_lm(r)/d^l:  B_lm = b,  grad B_lm = (g - l b rhat) / d.
 // F is called as f(lm, l, b, gx, gy, gz) with literal lm so that register arrays index statically.
 // ---------------------------------------------------------------------------------------------
-template <class F>
+template <int LMAX, class F>
 __device__ __forceinline__ void blm_unit(float x, float y, float z, F f) {
+  static_assert(LMAX == 4 || LMAX == 8, "harmonics are instantiated for l_max 4 and 8");
   float x2 = x * x, y2 = y * y, z2 = z * z;
   float xy = x * y, xz = x * z, yz = y * z;
   float d2 = x2 - y2;
@@ -166,6 +193,60 @@ __device__ __forceinline__ void blm_unit(float x, float y, float z, F f) {
   f(21, 4, cy * z, 6.f * xy * z, 3.f * d2 * z, cy);
   f(22, 4, x2 * x2 - 6.f * x2 * y2 + y2 * y2, 4.f * cx, -4.f * cy, 0.f);
   f(23, 4, 4.f * xy * d2, 4.f * cy, 4.f * cx, 0.f);
+  if constexpr (LMAX > 4) {
+    // l = 5..8 (Eq.B5.1-B8.17): b_lm = Z_lm'(z, r^2) * Re/Im (x + i y)^m', m' = 0 for m = 0 and m' = ceil(m/2)
+    // otherwise.  With cm = Re (x+iy)^m', sm = Im (x+iy)^m' and, at r = 1, Z, Zz = dZ/dz, Zr = dZ/d(r^2):
+    //   grad (Z cm) = Z m' (c_{m'-1}, -s_{m'-1}, 0) + cm (2 Zr x, 2 Zr y, Zz + 2 Zr z)      (polynomial gradient)
+    //   grad (Z sm) = Z m' (s_{m'-1},  c_{m'-1}, 0) + sm (2 Zr x, 2 Zr y, Zz + 2 Zr z)
+    float cm[9], sm[9];
+    cm[0] = 1.f; sm[0] = 0.f;
+#pragma unroll
+    for (int m = 1; m <= 8; ++m) { cm[m] = x * cm[m - 1] - y * sm[m - 1]; sm[m] = x * sm[m - 1] + y * cm[m - 1]; }
+    const float z3 = z2 * z, z4 = z2 * z2, z5 = z4 * z, z6 = z4 * z2, z7 = z6 * z, z8 = z4 * z4;
+    auto zero = [&](int lm, int l, float Z, float Zz, float Zr) { f(lm, l, Z, 2.f * Zr * x, 2.f * Zr * y, Zz + 2.f * Zr * z); };
+    auto pair = [&](int lm, int l, int m, float Z, float Zz, float Zr) {
+      const float fm = (float)m, w = Zz + 2.f * Zr * z, zx = 2.f * Zr * x, zy = 2.f * Zr * y;
+      f(lm, l, Z * cm[m], Z * fm * cm[m - 1] + zx * cm[m], -Z * fm * sm[m - 1] + zy * cm[m], w * cm[m]);
+      f(lm + 1, l, Z * sm[m], Z * fm * sm[m - 1] + zx * sm[m], Z * fm * cm[m - 1] + zy * sm[m], w * sm[m]);
+    };
+    // l = 5, slots 24..34
+    zero(24, 5, 63.f * z5 - 70.f * z3 + 15.f * z, 315.f * z4 - 210.f * z2 + 15.f, -70.f * z3 + 30.f * z);
+    pair(25, 5, 1, 21.f * z4 - 14.f * z2 + 1.f, 84.f * z3 - 28.f * z, -14.f * z2 + 2.f);
+    pair(27, 5, 2, 3.f * z3 - z, 9.f * z2 - 1.f, -z);
+    pair(29, 5, 3, 9.f * z2 - 1.f, 18.f * z, -1.f);
+    pair(31, 5, 4, z, 1.f, 0.f);
+    pair(33, 5, 5, 1.f, 0.f, 0.f);
+    // l = 6, slots 35..47
+    zero(35, 6, 231.f * z6 - 315.f * z4 + 105.f * z2 - 5.f, 1386.f * z5 - 1260.f * z3 + 210.f * z, -315.f * z4 + 210.f * z2 - 15.f);
+    pair(36, 6, 1, 33.f * z5 - 30.f * z3 + 5.f * z, 165.f * z4 - 90.f * z2 + 5.f, -30.f * z3 + 10.f * z);
+    pair(38, 6, 2, 33.f * z4 - 18.f * z2 + 1.f, 132.f * z3 - 36.f * z, -18.f * z2 + 2.f);
+    pair(40, 6, 3, 11.f * z3 - 3.f * z, 33.f * z2 - 3.f, -3.f * z);
+    pair(42, 6, 4, 11.f * z2 - 1.f, 22.f * z, -1.f);
+    pair(44, 6, 5, z, 1.f, 0.f);
+    pair(46, 6, 6, 1.f, 0.f, 0.f);
+    // l = 7, slots 48..62
+    zero(48, 7, 429.f * z7 - 693.f * z5 + 315.f * z3 - 35.f * z, 3003.f * z6 - 3465.f * z4 + 945.f * z2 - 35.f,
+         -693.f * z5 + 630.f * z3 - 105.f * z);
+    pair(49, 7, 1, 429.f * z6 - 495.f * z4 + 135.f * z2 - 5.f, 2574.f * z5 - 1980.f * z3 + 270.f * z, -495.f * z4 + 270.f * z2 - 15.f);
+    pair(51, 7, 2, 143.f * z5 - 110.f * z3 + 15.f * z, 715.f * z4 - 330.f * z2 + 15.f, -110.f * z3 + 30.f * z);
+    pair(53, 7, 3, 143.f * z4 - 66.f * z2 + 3.f, 572.f * z3 - 132.f * z, -66.f * z2 + 6.f);
+    pair(55, 7, 4, 13.f * z3 - 3.f * z, 39.f * z2 - 3.f, -3.f * z);
+    pair(57, 7, 5, 13.f * z2 - 1.f, 26.f * z, -1.f);
+    pair(59, 7, 6, z, 1.f, 0.f);
+    pair(61, 7, 7, 1.f, 0.f, 0.f);
+    // l = 8, slots 63..79
+    zero(63, 8, 6435.f * z8 - 12012.f * z6 + 6930.f * z4 - 1260.f * z2 + 35.f, 51480.f * z7 - 72072.f * z5 + 27720.f * z3 - 2520.f * z,
+         -12012.f * z6 + 13860.f * z4 - 3780.f * z2 + 140.f);
+    pair(64, 8, 1, 715.f * z7 - 1001.f * z5 + 385.f * z3 - 35.f * z, 5005.f * z6 - 5005.f * z4 + 1155.f * z2 - 35.f,
+         -1001.f * z5 + 770.f * z3 - 105.f * z);
+    pair(66, 8, 2, 143.f * z6 - 143.f * z4 + 33.f * z2 - 1.f, 858.f * z5 - 572.f * z3 + 66.f * z, -143.f * z4 + 66.f * z2 - 3.f);
+    pair(68, 8, 3, 39.f * z5 - 26.f * z3 + 3.f * z, 195.f * z4 - 78.f * z2 + 3.f, -26.f * z3 + 6.f * z);
+    pair(70, 8, 4, 65.f * z4 - 26.f * z2 + 1.f, 260.f * z3 - 52.f * z, -26.f * z2 + 2.f);
+    pair(72, 8, 5, 5.f * z3 - z, 15.f * z2 - 1.f, -z);
+    pair(74, 8, 6, 15.f * z2 - 1.f, 30.f * z, -1.f);
+    pair(76, 8, 7, z, 1.f, 0.f);
+    pair(78, 8, 8, 1.f, 0.f, 0.f);
+  }
 }
 
 // 4-body cubic invariant of the l=2 moments s[0..4] (R14): P4, gradient, Hessian*t
@@ -189,6 +270,21 @@ __device__ __forceinline__ void p4_hess_vec(const float *s, const float *t, floa
   h[2] = 36.f * s2 * t[0] + 108.f * s4 * t[1] + (36.f * s0 - 108.f * s3) * t[2] - 108.f * s2 * t[3] + 108.f * s1 * t[4];
   h[3] = -18.f * s3 * t[0] + 108.f * s1 * t[1] - 108.f * s2 * t[2] - 18.f * s0 * t[3];
   h[4] = -18.f * s4 * t[0] + 108.f * s2 * t[1] + 108.f * s1 * t[2] - 18.f * s0 * t[4];
+}
+
+// 5-body quartic invariant of the l=1 moments s[0..2] (R41): q5 = kappa5 |s|^4; value, gradient, Hessian*t
+__device__ __forceinline__ float p5_value(const float *s) {
+  const float n2 = s[0] * s[0] + s[1] * s[1] + s[2] * s[2];
+  return GNEP_KAPPA5 * n2 * n2;
+}
+__device__ __forceinline__ void p5_grad(const float *s, float *g) {
+  const float c = 4.f * GNEP_KAPPA5 * (s[0] * s[0] + s[1] * s[1] + s[2] * s[2]);
+  g[0] = c * s[0]; g[1] = c * s[1]; g[2] = c * s[2];
+}
+__device__ __forceinline__ void p5_hess_vec(const float *s, const float *t, float *h) {
+  const float n2 = s[0] * s[0] + s[1] * s[1] + s[2] * s[2], st = s[0] * t[0] + s[1] * t[1] + s[2] * t[2];
+  const float a = 4.f * GNEP_KAPPA5 * n2, b = 8.f * GNEP_KAPPA5 * st;
+  h[0] = a * t[0] + b * s[0]; h[1] = a * t[1] + b * s[1]; h[2] = a * t[2] + b * s[2];
 }
 
 // 8 consecutive floats at a 32-byte aligned address as ONE 256-bit access (sm_100: LDG/STG.256): half as many requests

@@ -44,15 +44,21 @@ struct gnep_handle {
   // batch
   bool loaded = false;
   int N = 0, S = 0;
-  int64_t nR = 0, nA = 0, nAp = 0;   // nAp: angular pairs including the padding dummies
+  int64_t nR = 0, nA = 0;
   int hasE = 0, hasF = 0, hasV = 0;
-  double Ng = -1, Sg = -1, l2_share = 1.0;   // job-wide normalisers when structures are sharded over ranks
+  double Zloc[3] = {0, 0, 0};                // normalisers of the resident batch: sum w_e, sum w_f N_s, sum w_v (R40)
+  double Zjob[3] = {-1, -1, -1};             // job-wide normalisers when structures are sharded over ranks (< 0: unset)
+  double l2_share = 1.0;
+  double *wgt = nullptr;                     // device [3][S]: per-structure weights of the three loss terms
+  std::vector<int> host_aoff;                // atom offsets of the resident batch (for the weight normalisers)
   bool eval_local = false;                   // set while gnep_evaluate runs: RMSEs of the resident batch, whatever the job norm
   std::vector<void *> batch_allocs;
-  int *perm = nullptr, *type_s = nullptr, *struct_s = nullptr, *segR = nullptr, *rowAs = nullptr, *segA = nullptr, *atomA = nullptr;
-  int *rowAu = nullptr, *segAu = nullptr, *atomAu = nullptr, *revAu = nullptr;   // unpadded angular list (force + gather kernels)
+  int *perm = nullptr, *type_s = nullptr, *struct_s = nullptr, *segR = nullptr;
+  int *tilesA = nullptr;       // angular tiles: 32 atoms of one central species each, sorted by neighbour counts; -1 = idle lane
+  int n_tilesA = 0, grid_adj = 0, grid_cg = 0, occ_adj = 1, occ_cg = 1;
+  int *rowAu = nullptr, *segAu = nullptr, *atomAu = nullptr, *revAu = nullptr;   // angular list
   float4 *pairAu = nullptr;
-  float4 *pairR = nullptr, *pairA = nullptr;
+  float4 *pairR = nullptr;
   int64_t *exp_row[2] = {nullptr, nullptr};
   int *exp_j[2] = {nullptr, nullptr}, *exp_sh[2] = {nullptr, nullptr};
   int *srange = nullptr;
@@ -60,10 +66,10 @@ struct gnep_handle {
   float *Fref_s = nullptr;
   SpeciesMap sm{};
   ReduceMap rm{};
-  int n_cta_net = 0, n_chunks = 0, n_ca_blocks = 0, n_gw = 0;
+  int n_cta_net = 0, n_chunks = 0, n_gw = 0;
   // per-atom state
   float *q = nullptr, *Sn = nullptr, *x = nullptr, *Ei = nullptr, *Ep = nullptr, *etil = nullptr, *M1 = nullptr,
-        *M2 = nullptr, *D = nullptr, *Tn = nullptr, *A1 = nullptr, *A2 = nullptr, *gbar = nullptr, *pbuf = nullptr, *eat = nullptr, *Wat = nullptr;
+        *M2 = nullptr, *D = nullptr, *Tn = nullptr, *A1 = nullptr, *Beta = nullptr, *gbar = nullptr, *pbuf = nullptr, *eat = nullptr, *Wat = nullptr;
   float4 *Fat = nullptr, *fpair = nullptr, *u = nullptr;
   double *Es = nullptr, *Ws = nullptr, *parts = nullptr;
   float *e_s = nullptr, *omega = nullptr;
@@ -115,10 +121,18 @@ int padded_basis(int K) {
     default: { constexpr int KT = 16; __VA_ARGS__; } break;     \
   }
 
-// n (angular radial functions) padded to the register-array size of the angular sweeps
-#define DISPATCH_NQ(NA_, ...)                                   \
-  if ((NA_) <= 10) { constexpr int NQ = 10; __VA_ARGS__; }      \
-  else { constexpr int NQ = 16; __VA_ARGS__; }
+// angular kernels: basis size padded to 4, 8 or 16 (32 / KT functions per lane-sum chunk), harmonics compiled for
+// l_max <= 4 (24 slots, 4 slot groups) and l_max <= 8 (80 slots, 14 slot groups)
+int padded_basis_ang(int K) { return K <= 4 ? 4 : K <= 8 ? 8 : 16; }
+#define DISPATCH_KA(KP, ...)                                    \
+  switch (KP) {                                                 \
+    case 4: { constexpr int KT = 4; __VA_ARGS__; } break;       \
+    case 8: { constexpr int KT = 8; __VA_ARGS__; } break;       \
+    default: { constexpr int KT = 16; __VA_ARGS__; } break;     \
+  }
+#define DISPATCH_ANG(d_, ...)                                               \
+  if ((d_).L <= 4) { constexpr int LMAX = 4; DISPATCH_KA((d_).KAp, __VA_ARGS__) } \
+  else { constexpr int LMAX = 8; DISPATCH_KA((d_).KAp, __VA_ARGS__) }
 
 template <class T>
 int dalloc(gnep_handle *h, T **p, size_t n, bool batch) {
@@ -138,17 +152,11 @@ void free_batch(gnep_handle *h) {
 
 // ---- dynamic shared memory sizes (bytes) --------------------------------------------------------
 size_t smem_radial(const DevSpec &d) { return sizeof(float) * (d.T * d.T * d.NR * d.KRp); }
-size_t smem_ang_fwd(const DevSpec &d) {
-  return sizeof(float) * (d.T * d.T * d.KAp * ANG_NQ + ANG_WARPS * ((d.KAp + GNEP_NLM) * ANG_LD + d.T * d.KAp * GNEP_NLM + ANG_NQ * GNEP_NLM + ANG_SEGS));
-}
-size_t smem_ang_force(const DevSpec &d) { return sizeof(float) * (((d.T * d.T * d.NA * d.KAp + 3) & ~3) + ANG_WARPS * FRC_TA * d.NA * GNEP_NLM); }
-size_t smem_ang_adj(const DevSpec &d) {
-  return sizeof(float) * (d.T * d.T * d.KAp * ANG_NQ + ANG_WARPS * ((2 * d.KAp + 2 * GNEP_NLM) * ANG_LD + d.T * d.KAp * GNEP_NLM + ANG_NQ * GNEP_NLM + ANG_SEGS));
-}
-size_t smem_cgrad_ang(const DevSpec &d) {
-  int nacc = d.T * d.T * d.NA * d.KAp;
-  return sizeof(float) * ANG_WARPS * (((nacc + 3) & ~3) + 2 * ((d.NA * GNEP_NLM + 3) & ~3));
-}
+int ang_warps(const DevSpec &d) { return ang_groups(d.L); }   // warps per CTA of the moment kernels = slot groups of the model
+size_t smem_ang_fwd(const DevSpec &d) { return sizeof(float) * ang_fwd_smem_floats(d.T, d.NA, d.KAp, ang_warps(d), d.Ndes - d.NR); }
+size_t smem_ang_force(const DevSpec &d) { return sizeof(float) * (((d.T * d.T * d.NA * d.KAp + 3) & ~3) + FRC_WARPS * FRC_TA * d.NA * d.nlmS); }
+size_t smem_ang_adj(const DevSpec &d) { return sizeof(float) * ang_adj_smem_floats(d.T, d.NA, d.KAp, ang_warps(d), d.Ndes - d.NR); }
+size_t smem_cgrad_ang(const DevSpec &d) { return sizeof(float) * ang_cgrad_smem_floats(d.T, d.NA, d.KAp, ang_warps(d), d.Ndes - d.NR); }
 size_t smem_net_fwd(const DevSpec &d) { return net_tc_smem_bytes(d, false); }
 size_t smem_net_bwd(const DevSpec &d) { return net_tc_smem_bytes(d, true); }
 size_t smem_gradw(const DevSpec &d) { return gradw_smem_bytes(d); }
@@ -166,8 +174,16 @@ int set_smem(gnep_handle *h, K kernel, size_t bytes) {
 int configure_kernels(gnep_handle *h) {
   const DevSpec &d = h->ds;
   DISPATCH_KT(d.KRp, RET_IF(set_smem(h, k_radial_fwd<KT>, smem_radial(d))); RET_IF(set_smem(h, k_radial_adj<KT>, smem_radial(d))));
-  DISPATCH_KT(d.KAp, RET_IF(set_smem(h, k_angular_force<KT>, smem_ang_force(d))); RET_IF(set_smem(h, k_cgrad_angular<KT>, smem_cgrad_ang(d)));
-              DISPATCH_NQ(d.NA, auto kf = k_angular_fwd<KT, NQ>; auto ka = k_angular_adj<KT, NQ>; RET_IF(set_smem(h, kf, smem_ang_fwd(d))); RET_IF(set_smem(h, ka, smem_ang_adj(d)))));
+  DISPATCH_ANG(d, auto kf = k_angular_fwd<KT, LMAX>; auto ka = k_angular_adj<KT, LMAX>; auto kc = k_cgrad_angular<KT, LMAX>;
+               auto kp = k_angular_force<KT, LMAX>;
+               RET_IF(set_smem(h, kf, smem_ang_fwd(d))); RET_IF(set_smem(h, ka, smem_ang_adj(d)));
+               RET_IF(set_smem(h, kc, smem_cgrad_ang(d))); RET_IF(set_smem(h, kp, smem_ang_force(d)));
+               // persistent grids of the two accumulating kernels: one resident wave
+               int occ = 0;
+               CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, ka, 32 * ang_warps(d), smem_ang_adj(d)));
+               h->occ_adj = std::max(occ, 1);
+               CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kc, 32 * ang_warps(d), smem_cgrad_ang(d)));
+               h->occ_cg = std::max(occ, 1));
   {   // TMEM budget of one k_net_tc warpgroup (256 columns): D1 + max(D1 corrections, D2 + D2 corrections)
     const NetDims nd = net_dims(d);
     if (nd.NnP + std::max(nd.NnP, 2 * nd.NdN) > 256) return fail(h, GNEP_EINVAL, "model too large for tensor memory (n_neurons, n_descriptors)");
@@ -220,7 +236,7 @@ int enqueue_descriptors(gnep_handle *h) {
   const DevSpec &d = h->ds;
   DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_fwd<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, smem_radial(d), d, h->N, h->type_s, h->segR, h->pairR, h->theta, h->q, h->M1));
   mark(h, "a1_radial_descriptor");
-  DISPATCH_KT(d.KAp, DISPATCH_NQ(d.NA, auto kf = k_angular_fwd<KT, NQ>; LAUNCH(h, kf, cdiv(h->N, ANG_WARPS * ANG_TA), ANG_WARPS * 32, smem_ang_fwd(d), d, h->N, h->type_s, h->segA, h->pairA, h->theta, h->q, h->Sn, h->A1)));
+  DISPATCH_ANG(d, auto kf = k_angular_fwd<KT, LMAX>; LAUNCH(h, kf, h->n_tilesA, 32 * ang_warps(d), smem_ang_fwd(d), d, h->n_tilesA, h->tilesA, h->type_s, h->segAu, h->pairAu, h->theta, h->q, h->Sn, h->A1));
   mark(h, "a1_angular_descriptor");
   return GNEP_OK;
 }
@@ -230,8 +246,9 @@ LossCfg loss_cfg(const gnep_handle *h) {
   lc.S = h->S; lc.N = h->N; lc.T = h->ds.T; lc.P = h->ds.P;
   lc.hasE = h->hasE; lc.hasF = h->hasF; lc.hasV = h->hasV; lc.loss_mode = h->ds.loss_mode;
   lc.lam_e = h->spec.lambda_e; lc.lam_f = h->spec.lambda_f; lc.lam_v = h->spec.lambda_v; lc.lam_2 = h->spec.lambda_2;
-  const bool job = h->Ng >= 0 && !h->eval_local;   // gnep_evaluate always normalises by the resident batch itself
-  lc.Ng = job ? h->Ng : (double)h->N; lc.Sg = job ? h->Sg : (double)h->S; lc.l2_share = job ? h->l2_share : 1.0;
+  const bool job = h->Zjob[0] >= 0 && !h->eval_local;   // gnep_evaluate always normalises by the resident batch itself
+  const double *Z = job ? h->Zjob : h->Zloc;
+  lc.ZE = Z[0]; lc.ZF = Z[1]; lc.ZV = Z[2]; lc.l2_share = job ? h->l2_share : 1.0;
   return lc;
 }
 
@@ -241,13 +258,13 @@ int enqueue_forward(gnep_handle *h) {
   LAUNCH(h, k_net_tc<false>, h->n_cta_net, 256, smem_net_fwd(d), d, h->sm, h->theta, h->qscale, h->q, h->x, h->Ei, h->Ep, h->etil,
          (const int *)nullptr, (const float *)nullptr, (const float *)nullptr, (float *)nullptr, (float *)nullptr);
   mark(h, "a2_network_forward");
-  DISPATCH_KT(d.KAp, LAUNCH(h, k_angular_force<KT>, cdiv(h->N, ANG_WARPS * FRC_TA), ANG_WARPS * 32, smem_ang_force(d), d, h->N, h->type_s, h->segAu, h->atomAu, h->pairAu, h->theta, h->Ep, h->Sn, h->fpair));
+  DISPATCH_ANG(d, auto kp = k_angular_force<KT, LMAX>; LAUNCH(h, kp, cdiv(h->N, FRC_WARPS * FRC_TA), FRC_WARPS * 32, smem_ang_force(d), d, h->N, h->type_s, h->segAu, h->atomAu, h->pairAu, h->theta, h->Ep, h->Sn, h->Beta, h->fpair));
   mark(h, "a3_angular_force");
   // radial forces + the gather of the angular pair forces (thread per atom): writes F_i, W_i once
   DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_force<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, 0, d, h->N, h->type_s, h->segR, h->pairR, h->etil,
                             h->segAu, h->revAu, h->pairAu, h->fpair, h->Fat, h->Wat));
   mark(h, "a3_radial_force");
-  LAUNCH(h, k_struct_reduce, h->S, 128, 0, loss_cfg(h), h->srange, h->Ei, h->Fat, h->Wat, h->Eref, h->Fref_s, h->Wref, h->Es, h->Ws, h->e_s, h->u, h->omega, h->parts);
+  LAUNCH(h, k_struct_reduce, h->S, 128, 0, loss_cfg(h), h->srange, h->Ei, h->Fat, h->Wat, h->Eref, h->Fref_s, h->Wref, h->wgt, h->Es, h->Ws, h->e_s, h->u, h->omega, h->parts);
   LAUNCH(h, k_loss_final, 1, 256, 0, loss_cfg(h), h->parts, h->theta, h->terms, h->scales);
   mark(h, "a4_loss_and_seeds");
   return GNEP_OK;
@@ -258,7 +275,7 @@ int enqueue_backward(gnep_handle *h) {
   const DevSpec &d = h->ds;
   DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_adj<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, smem_radial(d), d, h->N, h->type_s, h->struct_s, h->segR, h->pairR, h->theta, h->u, h->omega, h->scales, h->D, h->M2));
   mark(h, "a5_radial_adjoint");
-  DISPATCH_KT(d.KAp, DISPATCH_NQ(d.NA, auto ka = k_angular_adj<KT, NQ>; LAUNCH(h, ka, cdiv(h->N, ANG_WARPS * ANG_TA), ANG_WARPS * 32, smem_ang_adj(d), d, h->N, h->type_s, h->struct_s, h->segA, h->atomA, h->pairA, h->theta, h->u, h->omega, h->scales, h->Sn, h->Tn, h->A2, h->D)));
+  DISPATCH_ANG(d, auto ka = k_angular_adj<KT, LMAX>; LAUNCH(h, ka, h->grid_adj, 32 * ang_warps(d), smem_ang_adj(d), d, h->n_tilesA, h->tilesA, h->type_s, h->struct_s, h->segAu, h->pairAu, h->theta, h->u, h->omega, h->scales, h->Sn, h->Beta, h->Tn, h->D, h->partialCA));
   mark(h, "a5_angular_adjoint");
   LAUNCH(h, k_net_tc<true>, h->n_cta_net, 256, smem_net_bwd(d), d, h->sm, h->theta, h->qscale, h->D, h->x, h->eat, h->Ep, (float *)nullptr,
          h->struct_s, h->e_s, h->scales, h->pbuf, h->gbar);
@@ -267,7 +284,8 @@ int enqueue_backward(gnep_handle *h) {
   mark(h, "a6_w0_gradient");
   LAUNCH(h, k_cgrad_radial, h->n_chunks, CR_THREADS, smem_cgrad_rad(d), d, h->sm, h->gbar, h->Ep, h->M1, h->M2, h->partialCR);
   mark(h, "a7_radial_cgrad");
-  DISPATCH_KT(d.KAp, LAUNCH(h, k_cgrad_angular<KT>, h->n_ca_blocks, ANG_WARPS * 32, smem_cgrad_ang(d), d, h->N, h->type_s, h->Ep, h->gbar, h->Sn, h->Tn, h->A1, h->A2, h->partialCA));
+  DISPATCH_ANG(d, auto kc = k_cgrad_angular<KT, LMAX>; LAUNCH(h, kc, h->grid_cg, 32 * ang_warps(d), smem_cgrad_ang(d), d, h->n_tilesA, h->tilesA, h->type_s, h->Ep, h->gbar, h->Sn, h->Tn, h->A1,
+                                                          h->partialCA + (size_t)h->grid_adj * ang_warps(d) * d.T * d.T * d.NA * d.KAp));
   mark(h, "a7_angular_cgrad");
   LAUNCH(h, k_grad_reduce, cdiv(d.P, 8), 256, 0, d, h->rm, (float)h->l2_share, h->theta, h->scales, h->partialCR, h->partialCA, h->partialW, h->partialB, h->grad);
   mark(h, "a8_grad_reduce");
@@ -346,7 +364,7 @@ int gnep_create(const gnep_model_spec *spec, void *cuda_stream, gnep_handle **ou
   if (s.n_basis_radial < 1 || s.n_basis_radial > GNEP_MAX_BASIS || s.n_basis_angular < 1 || s.n_basis_angular > GNEP_MAX_BASIS)
     return fail(h, GNEP_EINVAL, "basis size out of range");
   if (!(s.rc_radial > 0) || !(s.rc_angular > 0) || s.rc_angular > s.rc_radial) return fail(h, GNEP_EINVAL, "need 0 < rc_angular <= rc_radial");
-  if (s.l_max < 1 || s.l_max > 4) return fail(h, GNEP_EINVAL, "l_max must be 1..4");
+  if (s.l_max < 1 || s.l_max > GNEP_LMAX) return fail(h, GNEP_EINVAL, "l_max must be 1..8");
   if (s.use_4body && s.l_max < 2) return fail(h, GNEP_EINVAL, "use_4body needs l_max >= 2");
   if (s.n_neurons < 1 || s.n_neurons > GNEP_MAX_NEURONS) return fail(h, GNEP_EINVAL, "n_neurons out of range");
   if (s.loss_mode != 0 && s.loss_mode != 1) return fail(h, GNEP_EINVAL, "loss_mode must be 0 or 1");
@@ -364,9 +382,10 @@ int gnep_create(const gnep_model_spec *spec, void *cuda_stream, gnep_handle **ou
   h->device = dev; h->num_sms = prop.multiProcessorCount;
   DevSpec &d = h->ds;
   d.T = s.n_species; d.NR = s.n_radial; d.KR = s.n_basis_radial; d.NA = s.n_angular; d.KA = s.n_basis_angular;
-  d.L = s.l_max; d.use4 = s.use_4body ? 1 : 0; d.Nn = s.n_neurons; d.NnS = (d.Nn + 7) & ~7;
-  d.Ndes = d.NR + d.NA * d.L + (d.use4 ? d.NA : 0);
-  d.KRp = padded_basis(d.KR); d.KAp = padded_basis(d.KA);
+  d.L = s.l_max; d.use4 = s.use_4body ? 1 : 0; d.use5 = s.use_5body ? 1 : 0; d.Nn = s.n_neurons; d.NnS = (d.Nn + 7) & ~7;
+  d.Ndes = d.NR + d.NA * d.L + (d.use4 ? d.NA : 0) + (d.use5 ? d.NA : 0);
+  d.nlmS = d.L <= 4 ? 24 : 88;   // 24 / 80 slots; rows are whole 32-byte pieces
+  d.KRp = padded_basis(d.KR); d.KAp = padded_basis_ang(d.KA);
   d.offA = d.T * d.T * d.NR * d.KR;
   d.offNet = d.offA + d.T * d.T * d.NA * d.KA;
   d.netSize = d.Nn * d.Ndes + 2 * d.Nn + 1;
@@ -383,22 +402,6 @@ int gnep_create(const gnep_model_spec *spec, void *cuda_stream, gnep_handle **ou
   }
   int rc;
   if ((rc = configure_kernels(h)) != GNEP_OK) return bail(rc);
-  // constants: 2 C_lm with C_lm = (2l+1)/(4 pi) Chat_lm (R11-R12), kappa4 (R14).  Process-global __constant__
-  // memory, so the tables must not depend on this handle's spec (two live handles of different l_max share them)
-  {
-    const double chat[GNEP_NLM] = {1, 1, 1, 1.0 / 4, 3, 3, 3.0 / 4, 3.0 / 4, 1.0 / 4, 3.0 / 8, 3.0 / 8, 15.0 / 4, 15.0 / 4, 5.0 / 8,
-                                   5.0 / 8, 1.0 / 64, 5.0 / 8, 5.0 / 8, 5.0 / 16, 5.0 / 16, 35.0 / 8, 35.0 / 8, 35.0 / 64, 35.0 / 64};
-    float c2[GNEP_NLM], lf[GNEP_NLM];
-    const double pi = 3.14159265358979323846;
-    for (int lm = 0; lm < GNEP_NLM; ++lm) {
-      int l = lm < 3 ? 1 : lm < 8 ? 2 : lm < 15 ? 3 : 4;
-      lf[lm] = (float)l;
-      c2[lm] = (float)(2.0 * (2 * l + 1) / (4.0 * pi) * chat[lm]);   // the same for every handle: the kernels guard on sp.L
-    }
-    float k4 = (float)(-5.0 * std::sqrt(14.0) / (448.0 * pi * std::sqrt(pi)));
-    if (cudaMemcpyToSymbol(c_C2, c2, sizeof(c2)) != cudaSuccess || cudaMemcpyToSymbol(c_lf, lf, sizeof(lf)) != cudaSuccess ||
-        cudaMemcpyToSymbol(c_kappa4, &k4, sizeof(k4)) != cudaSuccess) { h->err = "cudaMemcpyToSymbol failed"; return bail(GNEP_ECUDA); }
-  }
   if ((rc = dalloc(h, &h->theta, d.P, false)) || (rc = dalloc(h, &h->grad, d.P, false)) || (rc = dalloc(h, &h->m, d.P, false)) ||
       (rc = dalloc(h, &h->v, d.P, false)) || (rc = dalloc(h, &h->qscale, d.Ndes, false)) || (rc = dalloc(h, &h->step_dev, 1, false)) ||
       (rc = dalloc(h, &h->terms, 8, false)) || (rc = dalloc(h, &h->scales, 4, false)) || (rc = dalloc(h, &h->lr_dev, 1, false)))
@@ -519,6 +522,33 @@ int gnep_set_targets(gnep_handle *h, const double *E, const double *F, const dou
     if (e != cudaSuccess) return fail(h, GNEP_ECUDA, cudaGetErrorString(e));
   }
   if (h->graph) { cudaGraphExecDestroy(h->graph); h->graph = nullptr; }   // hasE/F/V are baked into the graph
+  return GNEP_OK;
+}
+
+int gnep_set_weights(gnep_handle *h, const double *we, const double *wf, const double *wv, int is_device) {
+  if (!h) return fail(h, GNEP_EINVAL, "null handle");
+  if (!h->loaded) return fail(h, GNEP_ESTATE, "no batch loaded");
+  const int S = h->S;
+  std::vector<double> w((size_t)3 * S, 1.0);
+  const double *src[3] = {we, wf, wv};
+  for (int k = 0; k < 3; ++k)
+    if (src[k] && S)
+      CK(cudaMemcpy(w.data() + (size_t)k * S, src[k], (size_t)S * sizeof(double), is_device ? cudaMemcpyDeviceToHost : cudaMemcpyHostToHost));
+  for (double x : w) if (!(x >= 0) || !std::isfinite(x)) return fail(h, GNEP_EINVAL, "weights must be finite and >= 0");
+  double Z[3] = {0, 0, 0};
+  for (int s = 0; s < S; ++s) {
+    Z[0] += w[s]; Z[1] += w[(size_t)S + s] * (double)(h->host_aoff[s + 1] - h->host_aoff[s]); Z[2] += w[(size_t)2 * S + s];
+  }
+  for (int k = 0; k < 3; ++k) h->Zloc[k] = Z[k];
+  if (S) RET_IF(copy_in(h, h->wgt, w.data(), w.size() * sizeof(double), 0));
+  if (h->graph) { cudaGraphExecDestroy(h->graph); h->graph = nullptr; }   // the normalisers are kernel arguments of the graph
+  return GNEP_OK;
+}
+
+int gnep_loss_norms(const gnep_handle *h, double *z) {
+  if (!h || !z) return fail(h, GNEP_EINVAL, "null argument");
+  if (!h->loaded) return fail(h, GNEP_ESTATE, "no batch loaded");
+  for (int k = 0; k < 3; ++k) z[k] = h->Zloc[k];
   return GNEP_OK;
 }
 
@@ -643,13 +673,12 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     // ---- persistent batch arrays ----
     int rc_;
 #define BA(ptr, n) if ((rc_ = dalloc(h, &(ptr), (n), true)) != GNEP_OK) { tfree(); free_batch(h); return rc_; }
-    BA(h->perm, N); BA(h->type_s, N); BA(h->struct_s, N); BA(h->segR, (size_t)N * (T + 1) + 1); BA(h->rowAs, N + 1); BA(h->segA, (size_t)N * (T + 1) + 1);
+    BA(h->perm, N); BA(h->type_s, N); BA(h->struct_s, N); BA(h->segR, (size_t)N * (T + 1) + 1);
     BA(h->pairR, (size_t)rowRs[N] + 2);
     BA(h->exp_row[0], N + 1); BA(h->exp_row[1], N + 1); BA(h->exp_j[0], nR); BA(h->exp_sh[0], nR); BA(h->exp_j[1], nA); BA(h->exp_sh[1], nA);
     BA(h->srange, srange.size()); BA(h->Eref, S); BA(h->Wref, (size_t)S * 6); BA(h->Fref_s, (size_t)N * 3);
-    // the angular list is first built unpadded (u) and then copied into its final layout, in which every (atom, J)
-    // segment is padded to a multiple of 4 pairs with zero-contribution dummies (k_pad_angular)
-    // (the unpadded list stays resident: the force and gather kernels, lane = pair, have no use for the dummies)
+    BA(h->wgt, (size_t)3 * S);
+    h->host_aoff.assign(aoff, aoff + S + 1);
     int *d_rowRs, *d_shA; unsigned long long *d_ekey; float *d_er;
     CKT(talloc((void **)&d_rowRs, sizeof(int) * (N + 1))); CKT(talloc((void **)&d_shA, sizeof(int) * nA));
     BA(h->rowAu, N + 1); BA(h->segAu, (size_t)N * (T + 1) + 1); BA(h->atomAu, nA); BA(h->pairAu, nA); BA(h->revAu, nA);
@@ -672,26 +701,32 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     LAUNCH(h, k_nbr_scatter, cdiv((int64_t)N * 32, 256), 256, 0, N, T, d_struct_of, d_geo, d_type, d_inv, h->exp_row[0], h->exp_row[1], d_rowRs,
            d_rowAu, d_ekey, d_er, h->exp_j[0], h->exp_sh[0], h->exp_j[1], h->exp_sh[1], h->pairR, d_pairAu, d_shA, h->segR, d_segAu, d_atomAu);
     CKT(cudaGetLastError());
-    std::vector<int> segAu((size_t)N * (T + 1) + 1, 0), segAp((size_t)N * (T + 1) + 1, 0);
+    std::vector<int> segAu((size_t)N * (T + 1) + 1, 0);
     if (N) CKT(cudaMemcpyAsync(segAu.data(), d_segAu, sizeof(int) * (size_t)N * (T + 1), cudaMemcpyDeviceToHost, st));
     CKT(cudaStreamSynchronize(st));
-    int64_t nAp = 0;
-    for (int a = 0; a < N; ++a) {
-      for (int J = 0; J < T; ++J) {
-        segAp[(size_t)a * (T + 1) + J] = (int)nAp;
-        nAp += (segAu[(size_t)a * (T + 1) + J + 1] - segAu[(size_t)a * (T + 1) + J] + 3) / 4 * 4;
+    // ---- tiles of the angular moment kernels: 32 atoms of one central species, atoms sorted by their per-species
+    // neighbour counts (descending), so that the rows a warp walks in lock step have equal lengths; the last tile of a
+    // species is filled up with -1 (idle lanes)
+    std::vector<int> tiles;
+    {
+      std::vector<std::pair<uint64_t, int>> keyed;
+      for (int t = 0; t < T; ++t) {
+        const int a0 = h->sm.start[t], a1 = h->sm.start[t + 1];
+        keyed.clear();
+        for (int a = a0; a < a1; ++a) {
+          uint64_t key = 0;
+          for (int J = 0; J < T; ++J)
+            key = (key << 16) | (uint64_t)std::min(segAu[(size_t)a * (T + 1) + J + 1] - segAu[(size_t)a * (T + 1) + J], 65535);
+          keyed.emplace_back(~key, a);               // descending counts, ascending atom index among equals
+        }
+        std::sort(keyed.begin(), keyed.end());
+        for (auto &kv : keyed) tiles.push_back(kv.second);
+        while (tiles.size() % ANG_TILE) tiles.push_back(-1);
       }
-      segAp[(size_t)a * (T + 1) + T] = (int)nAp;
-      rowAs[a] = segAp[(size_t)a * (T + 1)];
     }
-    rowAs[N] = (int)nAp;
-    if (nAp >= (int64_t)1 << 31) { tfree(); free_batch(h); return fail(h, GNEP_ERANGE, "2^31 or more (padded) angular pairs"); }
-    h->nAp = nAp;
-    BA(h->atomA, nAp); BA(h->pairA, nAp);
-    CKT(cudaMemcpyAsync(h->rowAs, rowAs.data(), sizeof(int) * (N + 1), cudaMemcpyHostToDevice, st));
-    CKT(cudaMemcpyAsync(h->segA, segAp.data(), sizeof(int) * ((size_t)N * (T + 1) + 1), cudaMemcpyHostToDevice, st));
-    LAUNCH(h, k_pad_angular, cdiv((int64_t)N * 32, 256), 256, 0, N, T, d_segAu, h->segA, d_pairAu, h->pairA, h->atomA,
-           (float)(2.0 * h->spec.rc_angular));
+    h->n_tilesA = (int)(tiles.size() / ANG_TILE);
+    BA(h->tilesA, tiles.size());
+    if (!tiles.empty()) CKT(cudaMemcpyAsync(h->tilesA, tiles.data(), sizeof(int) * tiles.size(), cudaMemcpyHostToDevice, st));
     LAUNCH(h, k_nbr_reverse, cdiv((int64_t)N * 32, 256), 256, 0, N, h->rowAu, h->pairAu, d_shA, h->revAu);
     CKT(cudaGetLastError());
     CKT(cudaStreamSynchronize(st));
@@ -720,14 +755,15 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     h->n_cta_net = h->sm.cta_base[GNEP_MAX_SPECIES_C];
     h->n_chunks = h->sm.chunk_base[GNEP_MAX_SPECIES_C];
     h->n_gw = h->sm.gw_base[GNEP_MAX_SPECIES_C];
-    h->n_ca_blocks = std::max(1, std::min(cdiv(N, ANG_WARPS), 4 * h->num_sms));
+    h->grid_adj = std::min(h->n_tilesA, h->occ_adj * h->num_sms);
+    h->grid_cg = std::min(h->n_tilesA, h->occ_cg * h->num_sms);
     for (int t = 0; t <= GNEP_MAX_SPECIES_C; ++t) { h->rm.chunk_base[t] = h->sm.chunk_base[t]; h->rm.gw_base[t] = h->sm.gw_base[t]; }
-    h->rm.n_warps_ca = N > 0 ? h->n_ca_blocks * ANG_WARPS : 0;
+    h->rm.n_warps_ca = (h->grid_adj + h->grid_cg) * ang_warps(d);   // partial rows: the beta half (adjoint sweep) then the alpha half
     // ---- per-atom state ----
     const size_t n = N;
     const size_t npad = n + GW_PAD_ROWS;   // k_gradw_tc bulk-copies whole windows of rows: zeroed rows past the end
-    BA(h->q, npad * d.Ndes); BA(h->Sn, n * d.NA * GNEP_NLM); BA(h->x, npad * d.NnS); BA(h->Ei, n); BA(h->Ep, n * d.Ndes);
-    BA(h->etil, n * T * d.KRp); BA(h->M1, n * T * d.KRp); BA(h->M2, n * T * d.KRp); BA(h->D, npad * d.Ndes); BA(h->Tn, n * d.NA * GNEP_NLM); BA(h->A1, n * T * d.KAp * GNEP_NLM); BA(h->A2, n * T * d.KAp * GNEP_NLM);
+    BA(h->q, npad * d.Ndes); BA(h->Sn, n * d.NA * d.nlmS); BA(h->x, npad * d.NnS); BA(h->Ei, n); BA(h->Ep, n * d.Ndes);
+    BA(h->etil, n * T * d.KRp); BA(h->M1, n * T * d.KRp); BA(h->M2, n * T * d.KRp); BA(h->D, npad * d.Ndes); BA(h->Tn, n * d.NA * d.nlmS); BA(h->Beta, n * ang_warps(d) * ang_nap(d.NA) * ANG_GS + 64); BA(h->A1, n * ang_warps(d) * T * d.KAp * ANG_GS);
     BA(h->gbar, n * d.Ndes); BA(h->pbuf, npad * d.NnS); BA(h->eat, npad); BA(h->Wat, n * 6);
     BA(h->Fat, n); BA(h->fpair, h->nA); BA(h->u, n);
     BA(h->Es, S); BA(h->Ws, (size_t)S * 6); BA(h->parts, (size_t)S * 3); BA(h->e_s, S); BA(h->omega, (size_t)S * 6);
@@ -735,6 +771,10 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     BA(h->partialCA, (size_t)std::max(h->rm.n_warps_ca, 1) * T * T * d.NA * d.KAp);
     BA(h->partialW, (size_t)std::max(h->n_gw, 1) * d.Nn * d.Ndes);
     BA(h->partialB, (size_t)std::max(h->n_gw, 1) * (2 * d.Nn + 1));
+    // slots of the (l,m) rows that no slot group of this model writes (l_max < 4) are read as zeros
+    CKT(cudaMemsetAsync(h->Sn, 0, sizeof(float) * n * d.NA * d.nlmS, st));
+    CKT(cudaMemsetAsync(h->Tn, 0, sizeof(float) * n * d.NA * d.nlmS, st));
+    CKT(cudaMemsetAsync(h->Beta, 0, sizeof(float) * (n * ang_warps(d) * ang_nap(d.NA) * ANG_GS + 64), st));
     CKT(cudaMemsetAsync(h->q + n * d.Ndes, 0, sizeof(float) * GW_PAD_ROWS * d.Ndes, st));
     CKT(cudaMemsetAsync(h->D + n * d.Ndes, 0, sizeof(float) * GW_PAD_ROWS * d.Ndes, st));
     CKT(cudaMemsetAsync(h->x, 0, sizeof(float) * npad * d.NnS, st));
@@ -743,6 +783,7 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
 #undef BA
 #undef CKT
     h->loaded = true;
+    RET_IF(gnep_set_weights(h, nullptr, nullptr, nullptr, 0));
     return gnep_set_targets(h, Eref, Fref, Wref, is_device);
   } catch (const std::bad_alloc &) {
     free_batch(h);
@@ -901,16 +942,23 @@ int gnep_train_epochs(gnep_handle *h, int32_t n_epochs, float lr, float beta1, f
   return GNEP_OK;
 }
 
-int gnep_set_global_norm(gnep_handle *h, int64_t n_atoms_global, int64_t n_structs_global, double l2_share) {
+int gnep_set_global_norms(gnep_handle *h, const double *z, double l2_share) {
   if (!h) return fail(h, GNEP_EINVAL, "null handle");
-  if (n_atoms_global < 0 || n_structs_global < 0) { h->Ng = h->Sg = -1; h->l2_share = 1.0; }
+  if (!z || z[0] < 0 || z[1] < 0 || z[2] < 0) { h->Zjob[0] = h->Zjob[1] = h->Zjob[2] = -1; h->l2_share = 1.0; }
   else {
     if (h->ds.loss_mode != 0) return fail(h, GNEP_EINVAL, "sharded normalisation needs loss_mode 0 (RMSE mode needs the global terms before the seeds)");
     if (!(l2_share >= 0 && l2_share <= 1)) return fail(h, GNEP_EINVAL, "l2_share must be in [0,1]");
-    h->Ng = (double)n_atoms_global; h->Sg = (double)n_structs_global; h->l2_share = l2_share;
+    for (int k = 0; k < 3; ++k) h->Zjob[k] = z[k];
+    h->l2_share = l2_share;
   }
   if (h->graph) { cudaGraphExecDestroy(h->graph); h->graph = nullptr; }
   return GNEP_OK;
+}
+
+int gnep_set_global_norm(gnep_handle *h, int64_t n_atoms_global, int64_t n_structs_global, double l2_share) {
+  if (n_atoms_global < 0 || n_structs_global < 0) return gnep_set_global_norms(h, nullptr, 1.0);
+  const double z[3] = {(double)n_structs_global, (double)n_atoms_global, (double)n_structs_global};
+  return gnep_set_global_norms(h, z, l2_share);
 }
 
 int gnep_set_grad(gnep_handle *h, const float *grad, int is_device) {

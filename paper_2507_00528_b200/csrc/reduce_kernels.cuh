@@ -8,7 +8,9 @@ struct LossCfg {
   int S, N, T, P;
   int hasE, hasF, hasV, loss_mode;
   double lam_e, lam_f, lam_v, lam_2;
-  double Ng, Sg;      // atoms / structures of the WHOLE job (== N, S on one GPU): the normalisers of Eq.10-12
+  // normalisers of Eq.10-12 over the WHOLE job: Z_E = sum_s w_e,s, Z_F = sum_s w_f,s N_s, Z_V = sum_s w_v,s
+  // (= S, N, S without per-structure weights on one GPU; R40)
+  double ZE, ZF, ZV;
   double l2_share;    // this rank's share of the L2 term (1 on one GPU, 1/world when structures are sharded)
 };
 
@@ -33,18 +35,21 @@ __device__ __forceinline__ void block_reduce_d(double (&v)[NV], double *sh /*[NV
 }
 
 // a4: one CTA per structure.  E_s = sum E_i, W_s = sum W_i (Eq.1, Eq.4), residuals of Eq.10-12 and the
-// seeds e_s = 2 lam_e dE_s/(S N_s), u_i = 2 lam_f (F_i - Fref_i)/(3N), omega_s = 2 lam_v dW_s/(6 S N_s).
+// seeds e_s = 2 lam_e w_e,s dE_s/(Z_E N_s), u_i = 2 lam_f w_f,s (F_i - Fref_i)/(3 Z_F), omega_s = 2 lam_v w_v,s dW_s/(6 Z_V N_s)
+// (w = per-structure weights, all ones by default: then Z_E = Z_V = S, Z_F = N and these are the seeds of Eq.10-12).
 __global__ void __launch_bounds__(128)
 k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const float *__restrict__ Ei,
                 const float4 *__restrict__ Fat, const float *__restrict__ Wat, const double *__restrict__ Eref,
-                const float *__restrict__ Fref_s, const double *__restrict__ Wref, double *__restrict__ Es,
+                const float *__restrict__ Fref_s, const double *__restrict__ Wref,
+                const double *__restrict__ wgt /*[3][S]: w_e, w_f, w_v*/, double *__restrict__ Es,
                 double *__restrict__ Ws, float *__restrict__ e_s, float4 *__restrict__ u,
                 float *__restrict__ omega, double *__restrict__ parts /*[S][3]*/) {
   __shared__ double sh[8 * 4];
   const int s = blockIdx.x;
   double v[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // E, W[6], sum |dF|^2
   int Ns = 0;
-  const float cu = lc.hasF ? (float)(2.0 * lc.lam_f / (3.0 * lc.Ng)) : 0.f;
+  const double we = wgt[s], wf = wgt[lc.S + s], wv = wgt[2 * lc.S + s];
+  const float cu = lc.hasF && lc.ZF > 0 ? (float)(2.0 * lc.lam_f * wf / (3.0 * lc.ZF)) : 0.f;
   for (int t = 0; t < lc.T; ++t) {
     int b = srange[(s * lc.T + t) * 2], e = srange[(s * lc.T + t) * 2 + 1];
     Ns += e - b;
@@ -64,23 +69,23 @@ k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const 
     double ns = (double)Ns;
     Es[s] = v[0];
     double pe = 0.0, pv = 0.0, es = 0.0;
-    if (lc.hasE && Ns > 0) {
+    if (lc.hasE && Ns > 0 && lc.ZE > 0) {
       double dE = v[0] / ns - Eref[s] / ns;
-      pe = dE * dE;
-      es = 2.0 * lc.lam_e * dE / (lc.Sg * ns);
+      pe = we * dE * dE;
+      es = 2.0 * lc.lam_e * we * dE / (lc.ZE * ns);
     }
     e_s[s] = (float)es;
     for (int c = 0; c < 6; ++c) {
       Ws[s * 6 + c] = v[1 + c];
       double om = 0.0;
-      if (lc.hasV && Ns > 0) {
+      if (lc.hasV && Ns > 0 && lc.ZV > 0) {
         double dW = (v[1 + c] - Wref[s * 6 + c]) / ns;
-        pv += dW * dW;
-        om = 2.0 * lc.lam_v * dW / (6.0 * lc.Sg * ns);
+        pv += wv * dW * dW;
+        om = 2.0 * lc.lam_v * wv * dW / (6.0 * lc.ZV * ns);
       }
       omega[s * 6 + c] = (float)om;
     }
-    parts[s * 3 + 0] = pe; parts[s * 3 + 1] = v[7]; parts[s * 3 + 2] = pv;
+    parts[s * 3 + 0] = pe; parts[s * 3 + 1] = wf * v[7]; parts[s * 3 + 2] = pv;
   }
 }
 
@@ -95,9 +100,9 @@ k_loss_final(LossCfg lc, const double *__restrict__ parts, const float *__restri
   for (int p = threadIdx.x; p < lc.P; p += blockDim.x) { double x = theta[p]; v[3] += x * x; }
   block_reduce_d<4>(v, sh);
   if (threadIdx.x == 0) {
-    double te = lc.Sg > 0 ? v[0] / lc.Sg : 0.0;
-    double tf = lc.Ng > 0 ? v[1] / (3.0 * lc.Ng) : 0.0;
-    double tv = lc.Sg > 0 ? v[2] / (6.0 * lc.Sg) : 0.0;
+    double te = lc.ZE > 0 ? v[0] / lc.ZE : 0.0;
+    double tf = lc.ZF > 0 ? v[1] / (3.0 * lc.ZF) : 0.0;
+    double tv = lc.ZV > 0 ? v[2] / (6.0 * lc.ZV) : 0.0;
     double t2 = lc.l2_share * v[3] / lc.P;
     double L, sc[4] = {1, 1, 1, 1};
     if (lc.loss_mode == 0) L = lc.lam_e * te + lc.lam_f * tf + lc.lam_v * tv + lc.lam_2 * t2;

@@ -52,6 +52,18 @@ def setup_sharded(engine, dist, n_atoms_local, n_structs_local, device=None):
     return n_job, s_job
 
 
+def setup_sharded_weighted(engine, dist, device=None):
+    """The same when per-structure loss weights are set: every rank contributes its normalisers {Z_E, Z_F, Z_V}
+    (`loss_norms`), their sums over ranks are the job-wide ones.  Returns them."""
+    import torch
+    world = dist.get_world_size()
+    z = torch.tensor(np.asarray(engine.loss_norms(), dtype=np.float64), device=device)
+    dist.all_reduce(z)
+    z = z.cpu().numpy()
+    engine.set_global_norms(z, 1.0 / world)
+    return z
+
+
 def sharded_step(engine, dist, grad, lr, **adam):
     """One epoch on every rank: partial loss+gradient, all-reduce (sum) of the gradient, identical Adam step.
     `grad` is a float32 torch tensor of P entries on the engine's device, reused every step."""

@@ -38,7 +38,7 @@ def test_create_fails_loudly_without_gpu():
 def test_bad_spec_rejected_before_touching_the_device():
     import gnep_synth as gs
     from paper_2507_00528_b200 import Gnep, GnepError
-    for over in ({"l_max": 5}, {"n_species": 9}, {"rc_angular": 9.0}, {"n_neurons": 0}, {"loss_mode": 3},
+    for over in ({"l_max": 9}, {"n_species": 9}, {"rc_angular": 9.0}, {"n_neurons": 0}, {"loss_mode": 3},
                  {"use_4body": True, "l_max": 1}):
         with pytest.raises(GnepError) as e:
             Gnep(dict(gs.MODEL_SPECS[0], **over))

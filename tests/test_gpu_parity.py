@@ -134,7 +134,7 @@ def test_three_species_odd_sizes():
 
 def test_four_species():
     """T = GNEP_MAX_SPECIES: the packed (atom | J << 28 | I << 30) pair tag uses both bits of each field."""
-    _check_all(1, 2, adam_steps=2, spec_over={"n_species": 4, "n_neurons": 20})
+    _check_all(1, 6, adam_steps=2, spec_over={"n_species": 4, "n_neurons": 20})
 
 
 def test_one_species():

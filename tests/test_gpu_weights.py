@@ -1,0 +1,95 @@
+"""GPU parity of the per-structure loss weights / missing-label masks (R40; the paper's
+training sets mix structures with and without virial labels) against the weighted oracle."""
+import numpy as np
+import pytest
+
+from cases import labelled_case
+from oracle import gnep_oracle as orc
+
+pytestmark = pytest.mark.gpu
+
+
+def _gnep(spec, qs, b, labels, theta):
+    from paper_2507_00528_b200 import Gnep
+    g = Gnep(dict(spec, q_scale=qs))
+    g.load_batch(b["atom_offsets"], b["positions"], b["cells"], b["types"], *labels)
+    g.set_params(theta.astype(np.float32))
+    return g
+
+
+def _compare(g, sp, theta, qs, ob):
+    terms, grad = g.loss_and_grad(want_grad=True)
+    t_ref, g_ref = orc.loss_and_grad(sp, theta, qs, ob)
+    np.testing.assert_allclose(terms, t_ref, rtol=1e-5, atol=1e-12)
+    assert np.linalg.norm(grad - g_ref) / np.linalg.norm(g_ref) < 1e-4
+    big = np.abs(g_ref) > 1e-6
+    assert np.max(np.abs(grad[big] - g_ref[big]) / np.abs(g_ref[big])) < 1e-3
+    return terms, grad
+
+
+def test_half_the_structures_have_no_virial_and_random_weights():
+    spec, sp, b, ob, theta, qs, labels = labelled_case(3, n_structs=6)
+    S = 6
+    g = _gnep(spec, qs, b, labels, theta)
+    np.testing.assert_array_equal(g.loss_norms(), [S, b["atom_offsets"][-1], S])     # defaults: Eq.10-12 as printed
+    base, _ = _compare(g, sp, theta, qs, ob)
+    wv = np.array([1, 0, 1, 0, 0, 1.0])                                              # virial labels on half the set
+    g.set_weights(None, None, wv); ob.set_weights(None, None, wv)
+    masked, _ = _compare(g, sp, theta, qs, ob)
+    assert masked[3] != base[3] and masked[1] == base[1] and masked[2] == base[2]
+    rng = np.random.default_rng(5)
+    we, wf, wv = rng.uniform(0.1, 4.0, size=(3, S))
+    wf[2] = 0.0; we[4] = 0.0
+    g.set_weights(we, wf, wv); ob.set_weights(we, wf, wv)
+    _compare(g, sp, theta, qs, ob)
+    # the weighted epoch through the CUDA graph, 3 steps
+    th = theta.copy(); m = np.zeros_like(th); v = np.zeros_like(th)
+    for t in range(1, 4):
+        _, gr = orc.loss_and_grad(sp, th, qs, ob)
+        orc.adam_step(th, m, v, gr, t, 1e-3)
+    g.train_epochs(3, 1e-3)
+    th_gpu = g.get_params().astype(np.float64)
+    assert np.linalg.norm(th_gpu - th) / np.linalg.norm(th) < 1e-4
+    # evaluate() reports the weighted RMSEs of the resident batch
+    t_now = orc.loss(sp, th_gpu, qs, ob)
+    np.testing.assert_allclose(g.evaluate(), np.sqrt(t_now[1:4]), rtol=1e-5)
+    # back to ones
+    g.set_weights(); ob.set_weights()
+    g.set_params(theta.astype(np.float32))
+    again, _ = _compare(g, sp, theta, qs, ob)
+    np.testing.assert_array_equal(again, base)
+    from paper_2507_00528_b200 import GnepError
+    with pytest.raises(GnepError) as e:
+        g.set_weights(np.array([1, 1, -1, 1, 1, 1.0]))
+    assert e.value.code == -1
+    g.destroy()
+
+
+def test_weighted_loss_sharded_over_two_handles():
+    from paper_2507_00528_b200 import Gnep
+    spec, sp, b, ob, theta, qs, (E, F, W) = labelled_case(1, n_structs=5)
+    rng = np.random.default_rng(9)
+    we, wf, wv = rng.uniform(0.2, 2.0, size=(3, 5)); wv[[0, 3]] = 0.0
+    ob.set_weights(we, wf, wv)
+    off = b["atom_offsets"]
+    parts, z = [], np.zeros(3)
+    for lo, hi in ((0, 2), (2, 5)):
+        a0, a1 = off[lo], off[hi]
+        g = Gnep(dict(spec, q_scale=qs))
+        g.load_batch((off[lo:hi + 1] - a0).astype(np.int32), b["positions"][a0:a1], b["cells"][lo:hi], b["types"][a0:a1],
+                     E[lo:hi], F[a0:a1], W[lo:hi])
+        g.set_weights(we[lo:hi], wf[lo:hi], wv[lo:hi])
+        g.set_params(theta.astype(np.float32))
+        z += g.loss_norms()
+        parts.append(g)
+    np.testing.assert_allclose(z, [we.sum(), (wf * np.diff(off)).sum(), wv.sum()], rtol=1e-15)
+    for g in parts:
+        g.set_global_norms(z, 0.5)
+    res = [g.loss_and_grad(want_grad=True) for g in parts]
+    terms = np.sum([np.asarray(r[0], np.float64) for r in res], axis=0)
+    grad = np.sum([np.asarray(r[1], np.float64) for r in res], axis=0)
+    t_ref, g_ref = orc.loss_and_grad(sp, theta, qs, ob)
+    np.testing.assert_allclose(terms, t_ref, rtol=1e-5, atol=1e-12)
+    assert np.linalg.norm(grad - g_ref) / np.linalg.norm(g_ref) < 1e-4
+    for g in parts:
+        g.destroy()
