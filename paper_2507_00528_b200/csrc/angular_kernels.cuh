@@ -65,15 +65,20 @@ struct LaneSum {
 };
 
 // ------------------------------------------------------------------------------------------------
-// Memory layouts of the moment kernels.  A row-per-thread access costs one L1 wavefront per lane whatever its width, so
-// everything a thread (atom a, slot group G) reads or writes by itself is one contiguous, 32-byte aligned block moved
-// with 256-bit accesses ("group-major"):
-//   A1g [a][G][J][k][6]      moments of the species segment J               (k_angular_fwd -> k_cgrad_angular)
-//   Bg  [a][G][n][6], n < NAp = NA rounded up to 4                           (k_angular_force -> k_angular_adj)
-// while the per-atom rows S[a][n][nlmS], T[a][n][nlmS] stay row-major: they are assembled in shared memory by the
-// slot-group threads and written (and read) whole by one thread per (atom, n).
+// Memory traffic of the tile kernels.  A load or store whose 32 lanes touch 32 different lines costs one L1 wavefront
+// (about two cycles) per lane whatever its width, and a thread-per-atom kernel that does its own global accesses is bound
+// by exactly that.  So the tile kernels move data COOPERATIVELY: consecutive lanes take consecutive 32-byte pieces of
+// one atom's rows (S, T, beta: [a][n][nlmS] row-major; q, D, E', gbar: the atom's descriptor row), and the data meets
+// the per-thread view in shared memory "slot arrays"  X[(n*6 + i) * SST + G*32 + al],  SST = threads + 1:
+//   - the owner thread (atom al, slot group G) reads / updates its 6 slots of every n without bank conflicts,
+//   - one thread per (atom, n) gathers a whole (l,m) row across the groups without bank conflicts,
+//   - the cooperative copies (lanes along an atom's rows) see only occasional two-way conflicts.
+// Pair records are read once per pair (not once per slot group): phase 1 evaluates the radial basis, the unit vector
+// and the pair adjoint for a chunk of ANG_PC pairs per atom into shared memory, phase 2 (the slot-group threads) adds
+// the harmonics of its group and the K x 6 outer products.  Only the A1 moment blocks, which their own thread reads
+// back in k_cgrad_angular, stay thread-private in global memory: A1g[a][G][J][k][6], 256-bit accesses.
 // ------------------------------------------------------------------------------------------------
-__host__ __device__ inline int ang_nap(int NA) { return (NA + 3) & ~3; }
+#define ANG_PC 8          // pairs per atom per staged chunk
 
 template <int N8>
 __device__ __forceinline__ void st_block(float *__restrict__ p, const float (&v)[8 * N8]) {   // N8 x 8 floats, 32-byte aligned
@@ -91,29 +96,111 @@ __device__ __forceinline__ void ld_block(const float *__restrict__ p, float (&v)
     v[8 * c + 4] = t.hi.x; v[8 * c + 5] = t.hi.y; v[8 * c + 6] = t.hi.z; v[8 * c + 7] = t.hi.w;
   }
 }
-
-// One (atom, n) row of S or T gathered from the per-thread shared slots part[(n*6 + i) * nthr + G*32 + lane] of the
-// ng slot-group threads of the atom (slots of groups that do not exist read as zero)
-template <int LMAX>
-__device__ __forceinline__ void gather_row(const float *part, int n, int nthr, int ng, int lane, float (&s)[LMAX * (LMAX + 2)]) {
-#pragma unroll
-  for (int lm = 0; lm < LMAX * (LMAX + 2); ++lm)
-    s[lm] = lm / ANG_GS < ng ? part[(n * ANG_GS + lm % ANG_GS) * nthr + (lm / ANG_GS) * 32 + lane] : 0.f;
-}
-// ... written row-major with 256-bit stores (row stride NS is a multiple of 8 floats; the slots past NLM are zero)
-template <int LMAX>
-__device__ __forceinline__ void store_row_lm(float *__restrict__ row, const float (&s)[LMAX * (LMAX + 2)], int NS) {
-  constexpr int NLM = LMAX * (LMAX + 2);
-#pragma unroll
-  for (int c = 0; c < NLM / 8; ++c)
-    stg256(row + 8 * c, make_float4(s[8 * c], s[8 * c + 1], s[8 * c + 2], s[8 * c + 3]),
-           make_float4(s[8 * c + 4], s[8 * c + 5], s[8 * c + 6], s[8 * c + 7]));
-  (void)NS;
-}
 template <int LMAX>
 __device__ __forceinline__ void load_row_lm(const float *__restrict__ row, float (&s)[LMAX * (LMAX + 2)]) {
   ld_block<LMAX * (LMAX + 2) / 8>(row, s);
 }
+
+// per-tile bookkeeping in shared memory: atom ids (-1 = idle lane), species-segment bounds of each atom's angular row,
+// longest segment of the tile per neighbour species
+struct TileInfo {
+  int at[ANG_TILE];
+  int seg[ANG_TILE][GNEP_MAX_SPECIES_C + 1];
+  int maxlen[GNEP_MAX_SPECIES_C];
+};
+// called by every thread; the caller synchronises the CTA afterwards
+__device__ __forceinline__ void tile_setup(TileInfo *ti, const DevSpec &sp, const int *__restrict__ tiles, int tile,
+                                           const int *__restrict__ segA) {
+  if (threadIdx.x < 32) {
+    const int lane = threadIdx.x, a = tiles[tile * ANG_TILE + lane];
+    ti->at[lane] = a;
+    int prev = a >= 0 ? segA[(size_t)a * (sp.T + 1)] : 0;
+    ti->seg[lane][0] = prev;
+    for (int J = 0; J < sp.T; ++J) {
+      const int e = a >= 0 ? segA[(size_t)a * (sp.T + 1) + J + 1] : 0;
+      ti->seg[lane][J + 1] = e;
+      int m = e - prev;
+      prev = e;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+      if (lane == 0) ti->maxlen[J] = m;
+    }
+  }
+}
+
+// slot of (n, lm) of atom al in a slot array
+__device__ __forceinline__ int slot_of(int n, int lm, int sst, int al) { return (n * ANG_GS + lm % ANG_GS) * sst + (lm / ANG_GS) * 32 + al; }
+
+// cooperative global -> slot array: the tile's rows g[a][n][NS] (NA*NS floats per atom, NS = row stride of LMAX)
+template <int LMAX>
+__device__ __forceinline__ void coop_load_rows(const DevSpec &sp, const TileInfo *ti, const float *__restrict__ g, float *X, int sst, int ng) {
+  constexpr int NS = LMAX <= 4 ? 24 : 88;
+  const int len8 = sp.NA * NS / 8;
+  for (int x = threadIdx.x; x < ANG_TILE * len8; x += blockDim.x) {
+    const int al = x / len8, c8 = x - al * len8, a = ti->at[al];
+    if (a < 0) continue;
+    const float8 v8 = ldg256(g + (size_t)a * sp.NA * NS + 8 * c8);
+    const float v[8] = {v8.lo.x, v8.lo.y, v8.lo.z, v8.lo.w, v8.hi.x, v8.hi.y, v8.hi.z, v8.hi.w};
+#pragma unroll
+    for (int e = 0; e < 8; ++e) {
+      const int e8 = 8 * c8 + e, n = e8 / NS, lm = e8 - n * NS;
+      if (lm < ng * ANG_GS) X[slot_of(n, lm, sst, al)] = v[e];
+    }
+  }
+}
+// cooperative slot array -> global rows (slots of groups that do not exist are written as zero)
+template <int LMAX>
+__device__ __forceinline__ void coop_store_rows(const DevSpec &sp, const TileInfo *ti, const float *X, int sst, int ng, float *__restrict__ g) {
+  constexpr int NS = LMAX <= 4 ? 24 : 88;
+  const int len8 = sp.NA * NS / 8;
+  for (int x = threadIdx.x; x < ANG_TILE * len8; x += blockDim.x) {
+    const int al = x / len8, c8 = x - al * len8, a = ti->at[al];
+    if (a < 0) continue;
+    float v[8];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) {
+      const int e8 = 8 * c8 + e, n = e8 / NS, lm = e8 - n * NS;
+      v[e] = lm < ng * ANG_GS ? X[slot_of(n, lm, sst, al)] : 0.f;
+    }
+    stg256(g + (size_t)a * sp.NA * NS + 8 * c8, make_float4(v[0], v[1], v[2], v[3]), make_float4(v[4], v[5], v[6], v[7]));
+  }
+}
+// one (atom, n) row gathered from a slot array
+template <int LMAX>
+__device__ __forceinline__ void gather_row(const float *X, int n, int sst, int ng, int al, float (&s)[LMAX * (LMAX + 2)]) {
+#pragma unroll
+  for (int lm = 0; lm < LMAX * (LMAX + 2); ++lm) s[lm] = lm / ANG_GS < ng ? X[slot_of(n, lm, sst, al)] : 0.f;
+}
+
+// the harmonics of slot group G of a unit vector: B[i] = B_lm, lm = 6G + i (and, with the pair adjoint (ax,ay,az), ar =
+// a.rhat: Y[i] = grad B_lm . a = ((grad b_lm).a - l b_lm ar) / d).  G is warp-uniform; the unused harmonics of every
+// case are removed at compile time.
+template <int LMAX, int G>
+__device__ __forceinline__ void harm_case(float hx, float hy, float hz, float (&B)[ANG_GS]) {
+  blm_unit<LMAX>(hx, hy, hz, [&](int lm, int, float b, float, float, float) {
+    if (lm >= G * ANG_GS && lm < (G + 1) * ANG_GS) B[lm - G * ANG_GS] = b;
+  });
+}
+template <int LMAX, int G>
+__device__ __forceinline__ void harm_case(float hx, float hy, float hz, float rinv, float ax, float ay, float az, float ar,
+                                          float (&X)[ANG_GS], float (&Y)[ANG_GS]) {
+  blm_unit<LMAX>(hx, hy, hz, [&](int lm, int l, float b, float gx, float gy, float gz) {
+    if (lm >= G * ANG_GS && lm < (G + 1) * ANG_GS) {
+      X[lm - G * ANG_GS] = b;
+      Y[lm - G * ANG_GS] = rinv * ((gx * ax + gy * ay + gz * az) - (float)l * b * ar);
+    }
+  });
+}
+#define ANG_CASE(LMAX, g, CALL) \
+  case g: if constexpr (ang_groups(LMAX) > g) { constexpr int G = g; CALL; } break;
+#define ANG_GROUP_SWITCH(LMAX, w, CALL)                                                                        \
+  switch (w) {                                                                                                 \
+    ANG_CASE(LMAX, 0, CALL) ANG_CASE(LMAX, 1, CALL) ANG_CASE(LMAX, 2, CALL) ANG_CASE(LMAX, 3, CALL)            \
+    ANG_CASE(LMAX, 4, CALL) ANG_CASE(LMAX, 5, CALL) ANG_CASE(LMAX, 6, CALL) ANG_CASE(LMAX, 7, CALL)            \
+    ANG_CASE(LMAX, 8, CALL) ANG_CASE(LMAX, 9, CALL) ANG_CASE(LMAX, 10, CALL) ANG_CASE(LMAX, 11, CALL)          \
+    ANG_CASE(LMAX, 12, CALL) ANG_CASE(LMAX, 13, CALL)                                                          \
+    default: break;                                                                                            \
+  }
 
 // q_nl = sum_m C_lm S_nlm^2 (Eq.7), q4_n = kappa4 P4(S_n2m) (R14), q5_n = kappa5 |S_n1|^4 (R41); out: the atom's angular
 // descriptor entries nu - NR
@@ -155,90 +242,41 @@ __device__ __forceinline__ void finish_D(const DevSpec &sp, const float (&s)[LMA
   }
 }
 // the tile's angular descriptor entries, assembled in shared memory rows[al * stride + nu], go out with coalesced stores
-__device__ __forceinline__ void copy_out_rows(const DevSpec &sp, const int *at, const float *rows, int stride, float *__restrict__ dst) {
+__device__ __forceinline__ void copy_out_rows(const DevSpec &sp, const TileInfo *ti, const float *rows, int stride, float *__restrict__ dst) {
   const int nqa = sp.Ndes - sp.NR;
   for (int x = threadIdx.x; x < ANG_TILE * nqa; x += blockDim.x) {
-    const int al = x / nqa, v = x - al * nqa, a = at[al];
+    const int al = x / nqa, v = x - al * nqa, a = ti->at[al];
     if (a >= 0) dst[(size_t)a * sp.Ndes + sp.NR + v] = rows[al * stride + v];
+  }
+}
+// X[n] (+)= c[I][J][n][.] . acc[.][6]: the thread-local contraction of a finished species segment into the thread's slots
+template <int KT>
+__device__ __forceinline__ void contract_segment(const DevSpec &sp, const float *c, const float (&acc)[KT * ANG_GS], float *x_t, int sst, bool first) {
+  for (int n = 0; n < sp.NA; ++n) {
+    float s[ANG_GS];
+#pragma unroll
+    for (int i = 0; i < ANG_GS; ++i) s[i] = first ? 0.f : x_t[(n * ANG_GS + i) * sst];
+#pragma unroll
+    for (int k4 = 0; k4 < KT; k4 += 4) {
+      const float4 c4 = *(const float4 *)(c + n * KT + k4);
+      const float cv[4] = {c4.x, c4.y, c4.z, c4.w};
+#pragma unroll
+      for (int kk = 0; kk < 4; ++kk)
+#pragma unroll
+        for (int i = 0; i < ANG_GS; ++i) s[i] = fmaf(cv[kk], acc[(k4 + kk) * ANG_GS + i], s[i]);
+    }
+#pragma unroll
+    for (int i = 0; i < ANG_GS; ++i) x_t[(n * ANG_GS + i) * sst] = s[i];
   }
 }
 
 // ------------------------------------------------------------------------------------------------
 // a1 (angular): A1 moments, S_nlm (Eq.8), q_nl (Eq.7), many-body terms (R14, R41)
 // ------------------------------------------------------------------------------------------------
-template <int KT, int LMAX, int G>
-__device__ __forceinline__ void ang_fwd_thread(const DevSpec &sp, const float *cs, float *Spart, int nthr, int ng, int a,
-                                               const int *__restrict__ type_s, const int *__restrict__ segA,
-                                               const float4 *__restrict__ pairA, float *__restrict__ A1g) {
-  const int I = type_s[a];
-  const int *sg = segA + (size_t)a * (sp.T + 1);
-  float *A1a = A1g + ((size_t)a * ng + G) * sp.T * KT * ANG_GS;
-  float *sp_t = Spart + threadIdx.x;
-  int pbeg = sg[0];
-  for (int J = 0; J < sp.T; ++J) {
-    const int pend = sg[J + 1];
-    float acc[KT * ANG_GS];
-#pragma unroll
-    for (int x = 0; x < KT * ANG_GS; ++x) acc[x] = 0.f;
-    float4 rn = pbeg < pend ? pairA[pbeg] : make_float4(1.f, 0.f, 0.f, 0.f);
-    for (int p = pbeg; p < pend; ++p) {
-      const float4 r = rn;
-      if (p + 1 < pend) rn = pairA[p + 1];                   // the next record is in flight during this pair
-      float d, rinv;
-      pair_len(r.x * r.x + r.y * r.y + r.z * r.z, d, rinv);
-      float f[KT];
-      cheb_f<KT>(d, sp.rcAinv, f);
-      float B[ANG_GS];
-#pragma unroll
-      for (int i = 0; i < ANG_GS; ++i) B[i] = 0.f;
-      blm_unit<LMAX>(r.x * rinv, r.y * rinv, r.z * rinv, [&](int lm, int, float b, float, float, float) {
-        if (lm >= G * ANG_GS && lm < (G + 1) * ANG_GS) B[lm - G * ANG_GS] = b;
-      });
-#pragma unroll
-      for (int k = 0; k < KT; ++k)
-#pragma unroll
-        for (int i = 0; i < ANG_GS; ++i) acc[k * ANG_GS + i] = fmaf(f[k], B[i], acc[k * ANG_GS + i]);
-    }
-    pbeg = pend;
-    st_block<KT * ANG_GS / 8>(A1a + (size_t)J * KT * ANG_GS, acc);
-    // S += c[I][J] . A1[J]  (thread-local: this thread owns its 6 slots of every n); the running sums live in the
-    // thread's shared slots, where the finishing step picks the complete rows up
-    const float *c = cs + (size_t)(I * sp.T + J) * sp.NA * KT;
-    const bool first = J == 0;
-    for (int n = 0; n < sp.NA; ++n) {
-      float s[ANG_GS];
-#pragma unroll
-      for (int i = 0; i < ANG_GS; ++i) s[i] = first ? 0.f : sp_t[(n * ANG_GS + i) * nthr];
-#pragma unroll
-      for (int k4 = 0; k4 < KT; k4 += 4) {
-        const float4 c4 = *(const float4 *)(c + n * KT + k4);
-        const float cv[4] = {c4.x, c4.y, c4.z, c4.w};
-#pragma unroll
-        for (int kk = 0; kk < 4; ++kk)
-#pragma unroll
-          for (int i = 0; i < ANG_GS; ++i) s[i] = fmaf(cv[kk], acc[(k4 + kk) * ANG_GS + i], s[i]);
-      }
-#pragma unroll
-      for (int i = 0; i < ANG_GS; ++i) sp_t[(n * ANG_GS + i) * nthr] = s[i];
-    }
-  }
-}
-
-// warp w of the CTA runs the code of slot group w (the groups beyond ang_groups(LMAX) are never instantiated)
-#define ANG_CASE(LMAX, g, CALL) \
-  case g: if constexpr (ang_groups(LMAX) > g) { constexpr int G = g; CALL; } break;
-#define ANG_GROUP_SWITCH(LMAX, w, CALL)                                                                        \
-  switch (w) {                                                                                                 \
-    ANG_CASE(LMAX, 0, CALL) ANG_CASE(LMAX, 1, CALL) ANG_CASE(LMAX, 2, CALL) ANG_CASE(LMAX, 3, CALL)            \
-    ANG_CASE(LMAX, 4, CALL) ANG_CASE(LMAX, 5, CALL) ANG_CASE(LMAX, 6, CALL) ANG_CASE(LMAX, 7, CALL)            \
-    ANG_CASE(LMAX, 8, CALL) ANG_CASE(LMAX, 9, CALL) ANG_CASE(LMAX, 10, CALL) ANG_CASE(LMAX, 11, CALL)          \
-    ANG_CASE(LMAX, 12, CALL) ANG_CASE(LMAX, 13, CALL)                                                          \
-    default: break;                                                                                            \
-  }
-
-// shared-memory floats: coefficients | per-thread S slots [NA*6][threads] | descriptor rows [32][nqa|1] | atom ids [32]
+// shared-memory floats: coefficients | S slots [NA*6][SST] | descriptor rows [32][nqa|1] | pair stage [PC][32][KT+4] | TileInfo
 __host__ __device__ inline int ang_fwd_smem_floats(int T, int NA, int KT, int nwarps, int nqa) {
-  return ((T * T * NA * KT + 3) & ~3) + NA * ANG_GS * 32 * nwarps + ANG_TILE * (nqa | 1) + ANG_TILE;
+  return ((T * T * NA * KT + 3) & ~3) + ((NA * ANG_GS * (32 * nwarps + 1) + 3) & ~3) + ((ANG_TILE * (nqa | 1) + 3) & ~3) +
+         ANG_PC * 32 * (KT + 4) + (int)(sizeof(TileInfo) / 4);
 }
 
 template <int KT, int LMAX>
@@ -247,193 +285,212 @@ k_angular_fwd(DevSpec sp, int n_tiles, const int *__restrict__ tiles, const int 
               const int *__restrict__ segA, const float4 *__restrict__ pairA, const float *__restrict__ theta,
               float *__restrict__ q, float *__restrict__ S, float *__restrict__ A1g) {
   extern __shared__ __align__(128) float smem[];
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nthr = blockDim.x, ng = nthr >> 5;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nthr = blockDim.x, ng = nthr >> 5, sst = nthr + 1;
   const int nqa = sp.Ndes - sp.NR, qst = nqa | 1;
   float *cs = smem;                                             // [T*T*NA][KT]
-  float *Spart = smem + ((sp.T * sp.T * sp.NA * KT + 3) & ~3);  // [NA*6][threads]
-  float *QS = Spart + sp.NA * ANG_GS * nthr;                    // [32][qst]
-  int *at = (int *)(QS + ANG_TILE * qst);
+  float *Sst = cs + ((sp.T * sp.T * sp.NA * KT + 3) & ~3);      // S slots
+  float *QS = Sst + ((sp.NA * ANG_GS * sst + 3) & ~3);          // [32][qst]
+  float4 *PS = (float4 *)(QS + ((ANG_TILE * qst + 3) & ~3));    // [KT/4 + 1][PC][32]: f_k, then (hx, hy, hz, -)
+  TileInfo *ti = (TileInfo *)(PS + ANG_PC * 32 * (KT / 4 + 1));
   stage_coeff(cs, theta + sp.offA, sp.T * sp.T * sp.NA, sp.KA, KT);
-  const int a = tiles[blockIdx.x * ANG_TILE + lane];
-  if (w == 0) at[lane] = a;
+  tile_setup(ti, sp, tiles, blockIdx.x, segA);
   __syncthreads();
-  if (a >= 0) {
-    ANG_GROUP_SWITCH(LMAX, w, (ang_fwd_thread<KT, LMAX, G>(sp, cs, Spart, nthr, ng, a, type_s, segA, pairA, A1g)));
+  const int a = ti->at[lane];
+  const int I = type_s[ti->at[0]];
+  float *s_t = Sst + threadIdx.x;
+  float *A1a = A1g + ((size_t)max(a, 0) * ng + w) * sp.T * KT * ANG_GS;
+  for (int J = 0; J < sp.T; ++J) {
+    float acc[KT * ANG_GS];
+#pragma unroll
+    for (int x = 0; x < KT * ANG_GS; ++x) acc[x] = 0.f;
+    const int lo = ti->seg[lane][J], len = ti->seg[lane][J + 1] - lo, mlen = ti->maxlen[J];
+    for (int c0 = 0; c0 < mlen; c0 += ANG_PC) {
+      __syncthreads();                                          // the stage is free
+      for (int p = w; p < ANG_PC; p += ng)                      // phase 1: radial basis and unit vector, once per pair
+        if (c0 + p < len) {
+          const float4 r = pairA[lo + c0 + p];
+          float d, rinv, f[KT];
+          pair_len(r.x * r.x + r.y * r.y + r.z * r.z, d, rinv);
+          cheb_f<KT>(d, sp.rcAinv, f);
+#pragma unroll
+          for (int k4 = 0; k4 < KT / 4; ++k4) PS[(k4 * ANG_PC + p) * 32 + lane] = make_float4(f[4 * k4], f[4 * k4 + 1], f[4 * k4 + 2], f[4 * k4 + 3]);
+          PS[((KT / 4) * ANG_PC + p) * 32 + lane] = make_float4(r.x * rinv, r.y * rinv, r.z * rinv, 0.f);
+        }
+      __syncthreads();
+      const int np = min(ANG_PC, len - c0);                     // phase 2: harmonics of this group, K x 6 outer products
+      for (int p = 0; p < np; ++p) {
+        float f[KT], B[ANG_GS];
+#pragma unroll
+        for (int k4 = 0; k4 < KT / 4; ++k4) {
+          const float4 f4 = PS[(k4 * ANG_PC + p) * 32 + lane];
+          f[4 * k4] = f4.x; f[4 * k4 + 1] = f4.y; f[4 * k4 + 2] = f4.z; f[4 * k4 + 3] = f4.w;
+        }
+        const float4 h = PS[((KT / 4) * ANG_PC + p) * 32 + lane];
+#pragma unroll
+        for (int i = 0; i < ANG_GS; ++i) B[i] = 0.f;
+        ANG_GROUP_SWITCH(LMAX, w, (harm_case<LMAX, G>(h.x, h.y, h.z, B)));
+#pragma unroll
+        for (int k = 0; k < KT; ++k)
+#pragma unroll
+          for (int i = 0; i < ANG_GS; ++i) acc[k * ANG_GS + i] = fmaf(f[k], B[i], acc[k * ANG_GS + i]);
+      }
+    }
+    if (a >= 0) {
+      st_block<KT * ANG_GS / 8>(A1a + (size_t)J * KT * ANG_GS, acc);
+      contract_segment<KT>(sp, cs + (size_t)(I * sp.T + J) * sp.NA * KT, acc, s_t, sst, J == 0);
+    }
   }
-  __syncthreads();                                              // the S rows of the tile are complete in shared memory
+  __syncthreads();                                              // the S rows of the tile are complete in the slot array
   if (a >= 0)
     for (int n = w; n < sp.NA; n += ng) {
       float s[LMAX * (LMAX + 2)];
-      gather_row<LMAX>(Spart, n, nthr, ng, lane, s);
-      store_row_lm<LMAX>(S + ((size_t)a * sp.NA + n) * sp.nlmS, s, sp.nlmS);
+      gather_row<LMAX>(Sst, n, sst, ng, lane, s);
       finish_q<LMAX>(sp, s, QS + lane * qst, n);
     }
+  coop_store_rows<LMAX>(sp, ti, Sst, sst, ng, S);
   __syncthreads();
-  copy_out_rows(sp, at, QS, qst, q);
+  copy_out_rows(sp, ti, QS, qst, q);
 }
 
 // ------------------------------------------------------------------------------------------------
 // a5 (angular) + the beta half of a7: A2 moments with the pair adjoint a_ij, T_nlm = c.A2, D_(n,l), D_4, D_5, and
 // dL/dcA[I][J][n][k] += sum_lm beta_nlm A2[J][k][lm]  (beta = E' dq/dS was written by k_angular_force)
 // ------------------------------------------------------------------------------------------------
-template <int KT, int LMAX, int G>
-__device__ __forceinline__ void ang_adj_thread(const DevSpec &sp, const float *cs, float *Tpart, int nthr, int ng, LaneSum<KT> &ls,
-                                               int a, const int *__restrict__ type_s, const int *__restrict__ struct_s,
-                                               const int *__restrict__ segA, const float4 *__restrict__ pairA,
-                                               const float4 *__restrict__ u, const float *__restrict__ omega,
-                                               const float *__restrict__ scales, const float *__restrict__ Bg, bool act) {
-  const int I = type_s[a];
-  const int *sg = segA + (size_t)a * (sp.T + 1);
-  const AdjCtx ac = make_adj(u, omega, scales, a, struct_s[a]);
-  const float *Ba = Bg + ((size_t)a * ng + G) * ang_nap(sp.NA) * ANG_GS;
-  float *tp_t = Tpart + threadIdx.x;
-  float *accw_I = ls.accw;                                      // [T][NA*KT] block of this central species
-  int pbeg = act ? sg[0] : 0;
-  for (int J = 0; J < sp.T; ++J) {
-    const int pend = act ? sg[J + 1] : 0;
-    float acc[KT][ANG_GS];
-#pragma unroll
-    for (int k = 0; k < KT; ++k)
-#pragma unroll
-      for (int i = 0; i < ANG_GS; ++i) acc[k][i] = 0.f;
-    // records two pairs ahead, the gather of u_j one pair ahead
-    const float4 rdum = make_float4(1.f, 0.f, 0.f, __int_as_float(a));
-    float4 r1 = pbeg < pend ? pairA[pbeg] : rdum;
-    float4 r2 = pbeg + 1 < pend ? pairA[pbeg + 1] : rdum;
-    float4 uj1 = u[__float_as_int(r1.w)];
-    for (int p = pbeg; p < pend; ++p) {
-      const float4 r = r1, uj = uj1;
-      r1 = r2;
-      uj1 = u[__float_as_int(r1.w)];
-      r2 = p + 2 < pend ? pairA[p + 2] : rdum;
-      float d, rinv, ax, ay, az;
-      pair_len(r.x * r.x + r.y * r.y + r.z * r.z, d, rinv);
-      pair_adjoint(ac, uj, r, ax, ay, az);
-      const float hx = r.x * rinv, hy = r.y * rinv, hz = r.z * rinv;
-      const float ar = ax * hx + ay * hy + az * hz;
-      float f[KT], fp[KT];
-      cheb_ffp<KT>(d, sp.rcAinv, f, fp);
-      float X[ANG_GS], Y[ANG_GS];
-#pragma unroll
-      for (int i = 0; i < ANG_GS; ++i) { X[i] = 0.f; Y[i] = 0.f; }
-      blm_unit<LMAX>(hx, hy, hz, [&](int lm, int l, float b, float gx, float gy, float gz) {
-        if (lm >= G * ANG_GS && lm < (G + 1) * ANG_GS) {
-          X[lm - G * ANG_GS] = b;
-          Y[lm - G * ANG_GS] = rinv * ((gx * ax + gy * ay + gz * az) - (float)l * b * ar);
-        }
-      });
-#pragma unroll
-      for (int k = 0; k < KT; ++k) {
-        const float f1 = fp[k] * ar;
-#pragma unroll
-        for (int i = 0; i < ANG_GS; ++i) acc[k][i] = fmaf(f1, X[i], fmaf(f[k], Y[i], acc[k][i]));
-      }
-    }
-    pbeg = pend;
-    const float *c = cs + (size_t)(I * sp.T + J) * sp.NA * KT;
-    const bool first = J == 0;
-    // T += c[I][J] . A2[J], running sums in the thread's shared slots
-    if (act)
-      for (int n = 0; n < sp.NA; ++n) {
-        float t[ANG_GS];
-#pragma unroll
-        for (int i = 0; i < ANG_GS; ++i) t[i] = first ? 0.f : tp_t[(n * ANG_GS + i) * nthr];
-#pragma unroll
-        for (int k4 = 0; k4 < KT; k4 += 4) {
-          const float4 c4 = *(const float4 *)(c + n * KT + k4);
-          const float cv[4] = {c4.x, c4.y, c4.z, c4.w};
-#pragma unroll
-          for (int kk = 0; kk < 4; ++kk)
-#pragma unroll
-            for (int i = 0; i < ANG_GS; ++i) t[i] = fmaf(cv[kk], acc[k4 + kk][i], t[i]);
-        }
-#pragma unroll
-        for (int i = 0; i < ANG_GS; ++i) tp_t[(n * ANG_GS + i) * nthr] = t[i];
-      }
-    // dL/dcA[I][J][n][k] += sum_{lm in group} beta_nlm A2[J][k][lm], summed over the 32 atoms of the warp
-    ls.accw = accw_I + J * sp.NA * KT;
-    constexpr int NPC = LaneSum<KT>::NPC;                       // functions per chunk: their beta slots are one aligned block
-    for (int ch = 0; ch * NPC < sp.NA; ++ch) {
-      float be[NPC * ANG_GS];
-      if (act) {
-        if constexpr ((NPC * ANG_GS) % 8 == 0) ld_block<NPC * ANG_GS / 8>(Ba + ch * NPC * ANG_GS, be);
-        else {
-#pragma unroll
-          for (int v = 0; v < NPC * ANG_GS; v += 4) {
-            const float4 t4 = *(const float4 *)(Ba + ch * NPC * ANG_GS + v);
-            be[v] = t4.x; be[v + 1] = t4.y; be[v + 2] = t4.z; be[v + 3] = t4.w;
-          }
-        }
-      } else {
-#pragma unroll
-        for (int v = 0; v < NPC * ANG_GS; ++v) be[v] = 0.f;
-      }
-#pragma unroll
-      for (int nn = 0; nn < NPC; ++nn) {
-        float g[KT];
-#pragma unroll
-        for (int k = 0; k < KT; ++k) {
-          g[k] = 0.f;
-#pragma unroll
-          for (int i = 0; i < ANG_GS; ++i) g[k] = fmaf(be[nn * ANG_GS + i], acc[k][i], g[k]);   // (beta rows past NA are zero)
-        }
-        ls.put(nn, g);
-      }
-      ls.flush(ch, sp.NA * KT);
-    }
-  }
-  ls.accw = accw_I;
-}
-
-// shared-memory floats of k_angular_adj: coefficients | per-thread T slots | D rows [32][nqa|1] | per-warp scratch [32][33]
-// | per-warp accumulators [T*T][NA*KT] | atom ids
+// shared-memory floats: coefficients | T slots | beta slots (S slots for the finishing step) | D rows [32][nqa|1] | pair stage
+// [PC][32][2KT+8] | per-warp scratch [32][33] | per-warp accumulators [T*T][NA*KT] | TileInfo
 __host__ __device__ inline int ang_adj_smem_floats(int T, int NA, int KT, int nwarps, int nqa) {
-  return ((T * T * NA * KT + 3) & ~3) + NA * ANG_GS * 32 * nwarps + ANG_TILE * (nqa | 1) + nwarps * 32 * 33 +
-         nwarps * T * T * NA * KT + ANG_TILE;
+  return ((T * T * NA * KT + 3) & ~3) + 2 * ((NA * ANG_GS * (32 * nwarps + 1) + 3) & ~3) + ((ANG_TILE * (nqa | 1) + 3) & ~3) +
+         ANG_PC * 32 * (2 * KT + 8) + nwarps * 32 * 33 + ((nwarps * T * T * NA * KT + 3) & ~3) + (int)(sizeof(TileInfo) / 4);
 }
 
 template <int KT, int LMAX>
-__global__ void __launch_bounds__(32 * ang_groups(LMAX), LMAX <= 4 ? 4 : 1)
+__global__ void __launch_bounds__(32 * ang_groups(LMAX), LMAX <= 4 ? 2 : 1)
 k_angular_adj(DevSpec sp, int n_tiles, const int *__restrict__ tiles, const int *__restrict__ type_s,
               const int *__restrict__ struct_s, const int *__restrict__ segA, const float4 *__restrict__ pairA,
               const float *__restrict__ theta, const float4 *__restrict__ u, const float *__restrict__ omega,
-              const float *__restrict__ scales, const float *__restrict__ S, const float *__restrict__ Bg,
+              const float *__restrict__ scales, const float *__restrict__ S, const float *__restrict__ Beta,
               float *__restrict__ Tn, float *__restrict__ D, float *__restrict__ partial) {
   extern __shared__ __align__(128) float smem[];
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nthr = blockDim.x, ng = nthr >> 5;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nthr = blockDim.x, ng = nthr >> 5, sst = nthr + 1;
   const int ncs = (sp.T * sp.T * sp.NA * KT + 3) & ~3, nv = sp.NA * KT, nacc = sp.T * sp.T * nv;
-  const int nqa = sp.Ndes - sp.NR, qst = nqa | 1;
+  const int nqa = sp.Ndes - sp.NR, qst = nqa | 1, nslot = (sp.NA * ANG_GS * sst + 3) & ~3;
   float *cs = smem;
-  float *Tpart = cs + ncs;                                      // [NA*6][threads]
-  float *DS = Tpart + sp.NA * ANG_GS * nthr;                    // [32][qst]
-  float *scr = DS + ANG_TILE * qst + w * 32 * 33;               // per warp [32][33]
-  float *accw = DS + ANG_TILE * qst + ng * 32 * 33 + w * nacc;  // per warp [T*T][NA*KT]
-  int *at = (int *)(DS + ANG_TILE * qst + ng * 32 * 33 + ng * nacc);
+  float *Tst = cs + ncs;
+  float *Bst = Tst + nslot;
+  float *DS = Bst + nslot;
+  float4 *PS = (float4 *)(DS + ((ANG_TILE * qst + 3) & ~3));    // [2 KT/4 + 2][PC][32]: f_k' (a.rhat), f_k, (rhat, 1/d), (a, a.rhat)
+  float *scr = (float *)(PS + ANG_PC * 32 * (KT / 2 + 2)) + w * 32 * 33;
+  float *accw = (float *)(PS + ANG_PC * 32 * (KT / 2 + 2)) + ng * 32 * 33 + w * nacc;
+  TileInfo *ti = (TileInfo *)((float *)(PS + ANG_PC * 32 * (KT / 2 + 2)) + ng * 32 * 33 + ((ng * nacc + 3) & ~3));
   stage_coeff(cs, theta + sp.offA, sp.T * sp.T * sp.NA, sp.KA, KT);
   for (int o = lane; o < nacc; o += 32) accw[o] = 0.f;
+  const float sfF = scales[1], svV = scales[2];
   for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-    const int a = tiles[tile * ANG_TILE + lane];
-    const int a0 = tiles[tile * ANG_TILE];                      // lane 0 of a tile is always a real atom
-    __syncthreads();                                            // coefficients staged; previous tile's rows copied out
-    if (w == 0) at[lane] = a;
-    const int I = type_s[a0];
-    LaneSum<KT> ls{scr, accw + I * sp.T * nv, lane};
+    __syncthreads();                                            // the previous tile is done with every shared array
+    tile_setup(ti, sp, tiles, tile, segA);
+    __syncthreads();
+    const int a = ti->at[lane];
     const bool act = a >= 0;
-    const int aa = act ? a : a0;                                // idle lanes walk no pairs but join the lane sums
-    ANG_GROUP_SWITCH(LMAX, w, (ang_adj_thread<KT, LMAX, G>(sp, cs, Tpart, nthr, ng, ls, aa, type_s, struct_s, segA, pairA, u, omega,
-                                                            scales, Bg, act)));
-    __syncthreads();                                            // the T rows of the tile are complete in shared memory
+    const int I = type_s[ti->at[0]];
+    coop_load_rows<LMAX>(sp, ti, Beta, Bst, sst, ng);           // (visible after the first chunk barrier / the flush barrier)
+    // this lane's atom: adjoint seed u_i and the structure's omega, used by phase 1
+    float4 ui = make_float4(0.f, 0.f, 0.f, 0.f);
+    float om[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    if (act) {
+      ui = u[a];
+      const float *o6 = omega + (size_t)struct_s[a] * 6;
+#pragma unroll
+      for (int c = 0; c < 6; ++c) om[c] = svV * o6[c];
+    }
+    float *t_t = Tst + threadIdx.x;
+    const float *b_t = Bst + threadIdx.x;
+    LaneSum<KT> ls{scr, accw, lane};
+    for (int J = 0; J < sp.T; ++J) {
+      float acc[KT * ANG_GS];
+#pragma unroll
+      for (int x = 0; x < KT * ANG_GS; ++x) acc[x] = 0.f;
+      const int lo = ti->seg[lane][J], len = ti->seg[lane][J + 1] - lo, mlen = ti->maxlen[J];
+      for (int c0 = 0; c0 < mlen; c0 += ANG_PC) {
+        __syncthreads();
+        for (int p = w; p < ANG_PC; p += ng)                    // phase 1: one record, one gather, one basis evaluation per pair
+          if (c0 + p < len) {
+            const float4 r = pairA[lo + c0 + p];
+            const float4 uj = u[__float_as_int(r.w)];
+            float d, rinv, f[KT], fp[KT];
+            pair_len(r.x * r.x + r.y * r.y + r.z * r.z, d, rinv);
+            const float ax = sfF * (ui.x - uj.x) - (om[0] * r.x + om[5] * r.z);
+            const float ay = sfF * (ui.y - uj.y) - (om[1] * r.y + om[3] * r.x);
+            const float az = sfF * (ui.z - uj.z) - (om[2] * r.z + om[4] * r.y);
+            const float hx = r.x * rinv, hy = r.y * rinv, hz = r.z * rinv;
+            const float ar = ax * hx + ay * hy + az * hz;
+            cheb_ffp<KT>(d, sp.rcAinv, f, fp);
+#pragma unroll
+            for (int k4 = 0; k4 < KT / 4; ++k4) {
+              PS[(k4 * ANG_PC + p) * 32 + lane] = make_float4(fp[4 * k4] * ar, fp[4 * k4 + 1] * ar, fp[4 * k4 + 2] * ar, fp[4 * k4 + 3] * ar);
+              PS[((KT / 4 + k4) * ANG_PC + p) * 32 + lane] = make_float4(f[4 * k4], f[4 * k4 + 1], f[4 * k4 + 2], f[4 * k4 + 3]);
+            }
+            PS[((KT / 2) * ANG_PC + p) * 32 + lane] = make_float4(hx, hy, hz, rinv);
+            PS[((KT / 2 + 1) * ANG_PC + p) * 32 + lane] = make_float4(ax, ay, az, ar);
+          }
+        __syncthreads();
+        const int np = min(ANG_PC, len - c0);
+        for (int p = 0; p < np; ++p) {                          // phase 2
+          float f1[KT], f2[KT], X[ANG_GS], Y[ANG_GS];
+#pragma unroll
+          for (int k4 = 0; k4 < KT / 4; ++k4) {
+            const float4 u4 = PS[(k4 * ANG_PC + p) * 32 + lane], v4 = PS[((KT / 4 + k4) * ANG_PC + p) * 32 + lane];
+            f1[4 * k4] = u4.x; f1[4 * k4 + 1] = u4.y; f1[4 * k4 + 2] = u4.z; f1[4 * k4 + 3] = u4.w;
+            f2[4 * k4] = v4.x; f2[4 * k4 + 1] = v4.y; f2[4 * k4 + 2] = v4.z; f2[4 * k4 + 3] = v4.w;
+          }
+          const float4 h = PS[((KT / 2) * ANG_PC + p) * 32 + lane], av = PS[((KT / 2 + 1) * ANG_PC + p) * 32 + lane];
+#pragma unroll
+          for (int i = 0; i < ANG_GS; ++i) { X[i] = 0.f; Y[i] = 0.f; }
+          ANG_GROUP_SWITCH(LMAX, w, (harm_case<LMAX, G>(h.x, h.y, h.z, h.w, av.x, av.y, av.z, av.w, X, Y)));
+#pragma unroll
+          for (int k = 0; k < KT; ++k)
+#pragma unroll
+            for (int i = 0; i < ANG_GS; ++i) acc[k * ANG_GS + i] = fmaf(f1[k], X[i], fmaf(f2[k], Y[i], acc[k * ANG_GS + i]));
+        }
+      }
+      __syncthreads();                                          // beta slots are loaded (needed when the tile has no pairs at all)
+      if (act) contract_segment<KT>(sp, cs + (size_t)(I * sp.T + J) * sp.NA * KT, acc, t_t, sst, J == 0);
+      // dL/dcA[I][J][n][k] += sum_{lm in group} beta_nlm A2[J][k][lm], summed over the 32 atoms of the warp
+      ls.accw = accw + (I * sp.T + J) * nv;
+      constexpr int NPC = LaneSum<KT>::NPC;
+      for (int ch = 0; ch * NPC < sp.NA; ++ch) {
+#pragma unroll
+        for (int nn = 0; nn < NPC; ++nn) {
+          const int n = ch * NPC + nn;
+          float g[KT];
+#pragma unroll
+          for (int k = 0; k < KT; ++k) g[k] = 0.f;
+          if (act && n < sp.NA) {
+            float be[ANG_GS];
+#pragma unroll
+            for (int i = 0; i < ANG_GS; ++i) be[i] = b_t[(n * ANG_GS + i) * sst];
+#pragma unroll
+            for (int k = 0; k < KT; ++k)
+#pragma unroll
+              for (int i = 0; i < ANG_GS; ++i) g[k] = fmaf(be[i], acc[k * ANG_GS + i], g[k]);
+          }
+          ls.put(nn, g);
+        }
+        ls.flush(ch, nv);
+      }
+    }
+    __syncthreads();                                            // T slots complete, beta slots no longer needed
+    coop_load_rows<LMAX>(sp, ti, S, Bst, sst, ng);              // S rows for D = sum_m 2C S T
+    __syncthreads();
     if (act)
       for (int n = w; n < sp.NA; n += ng) {
         float s[LMAX * (LMAX + 2)], t[LMAX * (LMAX + 2)];
-        const size_t row = ((size_t)a * sp.NA + n) * sp.nlmS;
-        load_row_lm<LMAX>(S + row, s);
-        gather_row<LMAX>(Tpart, n, nthr, ng, lane, t);
-        store_row_lm<LMAX>(Tn + row, t, sp.nlmS);
+        gather_row<LMAX>(Bst, n, sst, ng, lane, s);
+        gather_row<LMAX>(Tst, n, sst, ng, lane, t);
         finish_D<LMAX>(sp, s, t, DS + lane * qst, n);
       }
+    coop_store_rows<LMAX>(sp, ti, Tst, sst, ng, Tn);
     __syncthreads();
-    copy_out_rows(sp, at, DS, qst, D);
+    copy_out_rows(sp, ti, DS, qst, D);
   }
   __syncwarp();
   float *dst = partial + (size_t)(blockIdx.x * ng + w) * nacc;
@@ -477,6 +534,9 @@ __device__ __forceinline__ void beta_row(const DevSpec &sp, const float *__restr
   }
 #pragma unroll
   for (int v = 0; v < NLM; v += 4) *(float4 *)(out_s + v) = make_float4(b[v], b[v + 1], b[v + 2], b[v + 3]);
+  constexpr int NS = LMAX <= 4 ? 24 : 88;                       // the row's padding slots are zero
+#pragma unroll
+  for (int v = NLM; v < NS; v += 4) *(float4 *)(out_s + v) = make_float4(0.f, 0.f, 0.f, 0.f);
 }
 
 // contribution of the harmonics lm in [LO, HI) to the pair force: gam_lm = sum_n g_n beta_nlm, gamp_lm = sum_n g_n' beta_nlm
@@ -516,7 +576,7 @@ template <int KT, int LMAX>
 __global__ void __launch_bounds__(FRC_WARPS * 32)
 k_angular_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ segA,
                 const int *__restrict__ atomA, const float4 *__restrict__ pairA, const float *__restrict__ theta,
-                const float *__restrict__ Ep, const float *__restrict__ S, float *__restrict__ Bg,
+                const float *__restrict__ Ep, const float *__restrict__ S, float *__restrict__ Beta,
                 float4 *__restrict__ fpair) {
   extern __shared__ __align__(128) float smem[];
   float *cs = smem;
@@ -531,27 +591,16 @@ k_angular_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__
   const int a_hi = min(a_lo + FRC_TA, N);
   const int T1 = sp.T + 1;
   const int P_lo = segA[a_lo * T1], P_hi = segA[(a_hi - 1) * T1 + sp.T];
-  // beta of the tile's atoms: one (atom, n) row per lane and round, into shared memory ...
+  // beta of the warp's atoms: one (atom, n) row per lane and round, into shared memory ...
   for (int it = lane; it < (a_hi - a_lo) * sp.NA; it += 32) {
     const int al = it / sp.NA, n = it - al * sp.NA;
     beta_row<LMAX>(sp, S + ((size_t)(a_lo + al) * sp.NA + n) * NS, Ep + (size_t)(a_lo + al) * sp.Ndes, n, beta + al * nb + n * NS);
   }
   __syncwarp();
-  // ... and out to global memory in the group-major layout of the adjoint sweep, Bg[a][G][n < NAp][6], 32 bytes per
-  // lane and store (rows n >= NA are zero)
-  {
-    const int ng = ang_groups(sp.L), nap = ang_nap(sp.NA), per_atom = ng * nap * ANG_GS / 8;
-    for (int it = lane; it < (a_hi - a_lo) * per_atom; it += 32) {
-      const int al = it / per_atom, c8 = it - al * per_atom;
-      const int G = c8 / (nap * ANG_GS / 8), e0 = (c8 - G * (nap * ANG_GS / 8)) * 8;
-      float v[8];
-#pragma unroll
-      for (int e = 0; e < 8; ++e) {
-        const int n = (e0 + e) / ANG_GS, i = (e0 + e) - n * ANG_GS;
-        v[e] = n < sp.NA ? beta[al * nb + n * NS + G * ANG_GS + i] : 0.f;
-      }
-      stg256(Bg + ((size_t)(a_lo + al) * ng + G) * nap * ANG_GS + e0, make_float4(v[0], v[1], v[2], v[3]), make_float4(v[4], v[5], v[6], v[7]));
-    }
+  // ... and out to global memory, row-major like S, for the adjoint sweep (32 bytes per lane and store)
+  for (int it = lane; it < (a_hi - a_lo) * (nb / 8); it += 32) {
+    const float4 *src = (const float4 *)(beta + 8 * it);
+    stg256(Beta + (size_t)a_lo * nb + 8 * it, src[0], src[1]);
   }
   if (P_lo == P_hi) return;
   // atomA packs (central atom | neighbour species << 28 | central species << 30); the next chunk's record is in flight
@@ -587,9 +636,9 @@ k_angular_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__
 // ------------------------------------------------------------------------------------------------
 // a7 (angular), alpha half: dL/dcA[I][J][n][k] += sum_atoms sum_lm alpha_nlm A1[J][k][lm]
 //   alpha_nlm = gbar_(n,l) 2C_lm S_nlm + E'_(n,l) 2C_lm T_nlm (+ 4-body: gbar_4 k4 dP4/ds_m + E'_4 k4 (H4 T)_m, 5-body alike)
-// No pair sweep (the A1 moments were stored by k_angular_fwd).  Per tile: the E' and gbar rows are staged in shared memory
-// with coalesced loads, one thread per (atom, n) builds the alpha row from the S and T rows, then the slot-group threads
-// contract their alpha slots with their A1 block and the lane sums go to the per-warp accumulators as in the adjoint sweep.
+// No pair sweep (the A1 moments were stored by k_angular_fwd).  Per tile: the S, T rows and the E', gbar rows are staged in
+// shared memory with coalesced loads, one thread per (atom, n) builds the alpha row, then the slot-group threads contract
+// their alpha slots with their A1 block and the lane sums go to the per-warp accumulators as in the adjoint sweep.
 // ------------------------------------------------------------------------------------------------
 template <int LMAX>
 __device__ __forceinline__ void alpha_row(const DevSpec &sp, const float (&s)[LMAX * (LMAX + 2)], const float (&t)[LMAX * (LMAX + 2)],
@@ -620,94 +669,90 @@ __device__ __forceinline__ void alpha_row(const DevSpec &sp, const float (&s)[LM
   }
 }
 
-template <int KT, int G>
-__device__ __forceinline__ void ang_cgrad_thread(const DevSpec &sp, LaneSum<KT> &ls, const float *AL, int nthr, int ng, int a, bool act,
-                                                 const float *__restrict__ A1g) {
-  const float *A1a = A1g + ((size_t)a * ng + G) * sp.T * KT * ANG_GS;
-  const float *al_t = AL + threadIdx.x;                         // alpha slots of this thread: AL[(n*6 + i) * nthr + tid]
-  float *accw_I = ls.accw;
-  constexpr int NPC = LaneSum<KT>::NPC;
-  for (int J = 0; J < sp.T; ++J) {
-    float a1[KT * ANG_GS];
-    if (act) ld_block<KT * ANG_GS / 8>(A1a + (size_t)J * KT * ANG_GS, a1);
-    else {
-#pragma unroll
-      for (int x = 0; x < KT * ANG_GS; ++x) a1[x] = 0.f;
-    }
-    ls.accw = accw_I + J * sp.NA * KT;
-    for (int ch = 0; ch * NPC < sp.NA; ++ch) {
-#pragma unroll
-      for (int nn = 0; nn < NPC; ++nn) {
-        const int n = ch * NPC + nn;
-        float g[KT];
-#pragma unroll
-        for (int k = 0; k < KT; ++k) g[k] = 0.f;
-        if (n < sp.NA) {
-          float al[ANG_GS];
-#pragma unroll
-          for (int i = 0; i < ANG_GS; ++i) al[i] = al_t[(n * ANG_GS + i) * nthr];
-#pragma unroll
-          for (int k = 0; k < KT; ++k)
-#pragma unroll
-            for (int i = 0; i < ANG_GS; ++i) g[k] = fmaf(al[i], a1[k * ANG_GS + i], g[k]);
-        }
-        ls.put(nn, g);
-      }
-      ls.flush(ch, sp.NA * KT);
-    }
-  }
-  ls.accw = accw_I;
-}
-
-// shared-memory floats of k_cgrad_angular: alpha slots [NA*6][threads] | E' and gbar rows 2 x [32][nqa|1] | per-warp scratch
-// | per-warp accumulators | atom ids
+// shared-memory floats of k_cgrad_angular: S slots | T slots (then alpha) | E' and gbar rows 2 x [32][nqa|1] | per-warp
+// scratch | per-warp accumulators | TileInfo
 __host__ __device__ inline int ang_cgrad_smem_floats(int T, int NA, int KT, int nwarps, int nqa) {
-  return NA * ANG_GS * 32 * nwarps + 2 * ANG_TILE * (nqa | 1) + nwarps * 32 * 33 + nwarps * T * T * NA * KT + ANG_TILE;
+  return 2 * ((NA * ANG_GS * (32 * nwarps + 1) + 3) & ~3) + ((2 * ANG_TILE * (nqa | 1) + 3) & ~3) + nwarps * 32 * 33 +
+         ((nwarps * T * T * NA * KT + 3) & ~3) + (int)(sizeof(TileInfo) / 4);
 }
 
 template <int KT, int LMAX>
-__global__ void __launch_bounds__(32 * ang_groups(LMAX), LMAX <= 4 ? 4 : 1)
+__global__ void __launch_bounds__(32 * ang_groups(LMAX), LMAX <= 4 ? 2 : 1)
 k_cgrad_angular(DevSpec sp, int n_tiles, const int *__restrict__ tiles, const int *__restrict__ type_s,
-                const float *__restrict__ Ep, const float *__restrict__ gbar, const float *__restrict__ S,
-                const float *__restrict__ Tn, const float *__restrict__ A1g, float *__restrict__ partial) {
+                const int *__restrict__ segA, const float *__restrict__ Ep, const float *__restrict__ gbar,
+                const float *__restrict__ S, const float *__restrict__ Tn, const float *__restrict__ A1g,
+                float *__restrict__ partial) {
   extern __shared__ __align__(128) float smem[];
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nthr = blockDim.x, ng = nthr >> 5;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nthr = blockDim.x, ng = nthr >> 5, sst = nthr + 1;
   const int nv = sp.NA * KT, nacc = sp.T * sp.T * nv;
-  const int nqa = sp.Ndes - sp.NR, qst = nqa | 1;
-  float *AL = smem;                                             // [NA*6][threads]
-  float *EG = AL + sp.NA * ANG_GS * nthr;                       // E' rows [32][qst], gbar rows [32][qst]
-  float *scr = EG + 2 * ANG_TILE * qst + w * 32 * 33;
-  float *accw = EG + 2 * ANG_TILE * qst + ng * 32 * 33 + w * nacc;
-  int *at = (int *)(EG + 2 * ANG_TILE * qst + ng * 32 * 33 + ng * nacc);
+  const int nqa = sp.Ndes - sp.NR, qst = nqa | 1, nslot = (sp.NA * ANG_GS * sst + 3) & ~3;
+  float *Sst = smem;
+  float *Tst = Sst + nslot;                                     // T, then alpha
+  float *EG = Tst + nslot;                                      // E' rows [32][qst], gbar rows [32][qst]
+  float *scr = EG + ((2 * ANG_TILE * qst + 3) & ~3) + w * 32 * 33;
+  float *accw = EG + ((2 * ANG_TILE * qst + 3) & ~3) + ng * 32 * 33 + w * nacc;
+  TileInfo *ti = (TileInfo *)(EG + ((2 * ANG_TILE * qst + 3) & ~3) + ng * 32 * 33 + ((ng * nacc + 3) & ~3));
   for (int o = lane; o < nacc; o += 32) accw[o] = 0.f;
   for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-    const int a = tiles[tile * ANG_TILE + lane];
-    const int a0 = tiles[tile * ANG_TILE];
-    __syncthreads();                                            // the previous tile's alpha slots and rows are no longer read
-    if (w == 0) at[lane] = a;
+    __syncthreads();                                            // the previous tile is done with every shared array
+    tile_setup(ti, sp, tiles, tile, segA);
     __syncthreads();
-    for (int x = threadIdx.x; x < ANG_TILE * nqa; x += nthr) {  // stage the angular parts of the E' and gbar rows
-      const int al = x / nqa, v = x - al * nqa, aa = at[al];
+    const int a = ti->at[lane];
+    const bool act = a >= 0;
+    const int I = type_s[ti->at[0]];
+    // this thread's A1 blocks are requested first: their latency hides behind the alpha rows
+    const float *A1a = A1g + ((size_t)max(a, 0) * ng + w) * sp.T * KT * ANG_GS;
+    coop_load_rows<LMAX>(sp, ti, S, Sst, sst, ng);
+    coop_load_rows<LMAX>(sp, ti, Tn, Tst, sst, ng);
+    for (int x = threadIdx.x; x < ANG_TILE * nqa; x += nthr) {  // the angular parts of the E' and gbar rows
+      const int al = x / nqa, v = x - al * nqa, aa = ti->at[al];
       EG[al * qst + v] = aa >= 0 ? Ep[(size_t)aa * sp.Ndes + sp.NR + v] : 0.f;
       EG[(ANG_TILE + al) * qst + v] = aa >= 0 ? gbar[(size_t)aa * sp.Ndes + sp.NR + v] : 0.f;
     }
     __syncthreads();
-    const bool act = a >= 0;
     if (act)
-      for (int n = w; n < sp.NA; n += ng) {                     // alpha row of (atom, n) -> the slot owners' shared slots
+      for (int n = w; n < sp.NA; n += ng) {                     // alpha row of (atom, n) overwrites the T slots of that row
         float s[LMAX * (LMAX + 2)], t[LMAX * (LMAX + 2)], al[LMAX * (LMAX + 2)];
-        const size_t row = ((size_t)a * sp.NA + n) * sp.nlmS;
-        load_row_lm<LMAX>(S + row, s);
-        load_row_lm<LMAX>(Tn + row, t);
+        gather_row<LMAX>(Sst, n, sst, ng, lane, s);
+        gather_row<LMAX>(Tst, n, sst, ng, lane, t);
         alpha_row<LMAX>(sp, s, t, EG + lane * qst, EG + (ANG_TILE + lane) * qst, n, al);
 #pragma unroll
         for (int lm = 0; lm < LMAX * (LMAX + 2); ++lm)
-          if (lm / ANG_GS < ng) AL[(n * ANG_GS + lm % ANG_GS) * nthr + (lm / ANG_GS) * 32 + lane] = al[lm];
+          if (lm / ANG_GS < ng) Tst[slot_of(n, lm, sst, lane)] = al[lm];
       }
     __syncthreads();
-    const int I = type_s[a0];
-    LaneSum<KT> ls{scr, accw + I * sp.T * nv, lane};
-    ANG_GROUP_SWITCH(LMAX, w, (ang_cgrad_thread<KT, G>(sp, ls, AL, nthr, ng, act ? a : a0, act, A1g)));
+    const float *al_t = Tst + threadIdx.x;
+    LaneSum<KT> ls{scr, accw, lane};
+    constexpr int NPC = LaneSum<KT>::NPC;
+    for (int J = 0; J < sp.T; ++J) {
+      float a1[KT * ANG_GS];
+      if (act) ld_block<KT * ANG_GS / 8>(A1a + (size_t)J * KT * ANG_GS, a1);
+      else {
+#pragma unroll
+        for (int x = 0; x < KT * ANG_GS; ++x) a1[x] = 0.f;
+      }
+      ls.accw = accw + (I * sp.T + J) * nv;
+      for (int ch = 0; ch * NPC < sp.NA; ++ch) {
+#pragma unroll
+        for (int nn = 0; nn < NPC; ++nn) {
+          const int n = ch * NPC + nn;
+          float g[KT];
+#pragma unroll
+          for (int k = 0; k < KT; ++k) g[k] = 0.f;
+          if (act && n < sp.NA) {
+            float al[ANG_GS];
+#pragma unroll
+            for (int i = 0; i < ANG_GS; ++i) al[i] = al_t[(n * ANG_GS + i) * sst];
+#pragma unroll
+            for (int k = 0; k < KT; ++k)
+#pragma unroll
+              for (int i = 0; i < ANG_GS; ++i) g[k] = fmaf(al[i], a1[k * ANG_GS + i], g[k]);
+          }
+          ls.put(nn, g);
+        }
+        ls.flush(ch, nv);
+      }
+    }
   }
   __syncwarp();
   float *dst = partial + (size_t)(blockIdx.x * ng + w) * nacc;

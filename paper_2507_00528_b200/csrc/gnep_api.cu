@@ -15,6 +15,7 @@
 #include "net_kernels.cuh"   // includes net_tc_kernels.cuh (tensor-core network)
 #include "pair_kernels.cuh"
 #include "angular_kernels.cuh"
+#include "angular_warp_kernels.cuh"
 #include "reduce_kernels.cuh"
 #include "peak_kernels.cuh"
 
@@ -54,8 +55,13 @@ struct gnep_handle {
   bool eval_local = false;                   // set while gnep_evaluate runs: RMSEs of the resident batch, whatever the job norm
   std::vector<void *> batch_allocs;
   int *perm = nullptr, *type_s = nullptr, *struct_s = nullptr, *segR = nullptr;
-  int *tilesA = nullptr;       // angular tiles: 32 atoms of one central species each, sorted by neighbour counts; -1 = idle lane
+  // angular moment kernels, two mappings: warp tiles over a padded pair list (l_max <= 4, the fast
+  // path) or slot-group tiles of 32 atoms (any l_max; always used above 4)
+  bool tile_path = false;
+  int *tilesA = nullptr;       // slot-group path: 32 atoms of one central species per tile, sorted by neighbour counts; -1 = idle lane
   int n_tilesA = 0, grid_adj = 0, grid_cg = 0, occ_adj = 1, occ_cg = 1;
+  int *segA = nullptr, *atomA = nullptr;   // warp-tile path: angular list with every (atom, J) segment padded to 4 pairs
+  float4 *pairA = nullptr;
   int *rowAu = nullptr, *segAu = nullptr, *atomAu = nullptr, *revAu = nullptr;   // angular list
   float4 *pairAu = nullptr;
   float4 *pairR = nullptr;
@@ -69,7 +75,7 @@ struct gnep_handle {
   int n_cta_net = 0, n_chunks = 0, n_gw = 0;
   // per-atom state
   float *q = nullptr, *Sn = nullptr, *x = nullptr, *Ei = nullptr, *Ep = nullptr, *etil = nullptr, *M1 = nullptr,
-        *M2 = nullptr, *D = nullptr, *Tn = nullptr, *A1 = nullptr, *Beta = nullptr, *gbar = nullptr, *pbuf = nullptr, *eat = nullptr, *Wat = nullptr;
+        *M2 = nullptr, *D = nullptr, *Tn = nullptr, *A1 = nullptr, *A2 = nullptr, *Beta = nullptr, *gbar = nullptr, *pbuf = nullptr, *eat = nullptr, *Wat = nullptr;
   float4 *Fat = nullptr, *fpair = nullptr, *u = nullptr;
   double *Es = nullptr, *Ws = nullptr, *parts = nullptr;
   float *e_s = nullptr, *omega = nullptr;
@@ -130,6 +136,10 @@ int padded_basis_ang(int K) { return K <= 4 ? 4 : K <= 8 ? 8 : 16; }
     case 8: { constexpr int KT = 8; __VA_ARGS__; } break;       \
     default: { constexpr int KT = 16; __VA_ARGS__; } break;     \
   }
+// warp-tile kernels: n (angular radial functions) padded to the register-array size of the sweeps
+#define DISPATCH_NQ(NA_, ...)                                   \
+  if ((NA_) <= 10) { constexpr int NQ = 10; __VA_ARGS__; }      \
+  else { constexpr int NQ = 16; __VA_ARGS__; }
 #define DISPATCH_ANG(d_, ...)                                               \
   if ((d_).L <= 4) { constexpr int LMAX = 4; DISPATCH_KA((d_).KAp, __VA_ARGS__) } \
   else { constexpr int LMAX = 8; DISPATCH_KA((d_).KAp, __VA_ARGS__) }
@@ -157,6 +167,15 @@ size_t smem_ang_fwd(const DevSpec &d) { return sizeof(float) * ang_fwd_smem_floa
 size_t smem_ang_force(const DevSpec &d) { return sizeof(float) * (((d.T * d.T * d.NA * d.KAp + 3) & ~3) + FRC_WARPS * FRC_TA * d.NA * d.nlmS); }
 size_t smem_ang_adj(const DevSpec &d) { return sizeof(float) * ang_adj_smem_floats(d.T, d.NA, d.KAp, ang_warps(d), d.Ndes - d.NR); }
 size_t smem_cgrad_ang(const DevSpec &d) { return sizeof(float) * ang_cgrad_smem_floats(d.T, d.NA, d.KAp, ang_warps(d), d.Ndes - d.NR); }
+size_t smem_angw_fwd(const DevSpec &d) {
+  return sizeof(float) * (d.T * d.T * d.KAp * ANG_NQ + ANG_WARPS * ((d.KAp + ANGW_NLM) * ANG_LD + d.T * d.KAp * ANGW_NLM + ANG_NQ * ANGW_NLM + ANG_SEGS));
+}
+size_t smem_angw_adj(const DevSpec &d) {
+  return sizeof(float) * (d.T * d.T * d.KAp * ANG_NQ + ANG_WARPS * ((2 * d.KAp + 2 * ANGW_NLM) * ANG_LD + d.T * d.KAp * ANGW_NLM + ANG_NQ * ANGW_NLM + ANG_SEGS));
+}
+size_t smem_angw_cgrad(const DevSpec &d) {
+  return sizeof(float) * ANG_WARPS * (((d.T * d.T * d.NA * d.KAp + 3) & ~3) + 2 * ((d.NA * ANGW_NLM + 3) & ~3));
+}
 size_t smem_net_fwd(const DevSpec &d) { return net_tc_smem_bytes(d, false); }
 size_t smem_net_bwd(const DevSpec &d) { return net_tc_smem_bytes(d, true); }
 size_t smem_gradw(const DevSpec &d) { return gradw_smem_bytes(d); }
@@ -184,6 +203,11 @@ int configure_kernels(gnep_handle *h) {
                h->occ_adj = std::max(occ, 1);
                CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kc, 32 * ang_warps(d), smem_cgrad_ang(d)));
                h->occ_cg = std::max(occ, 1));
+  if (!h->tile_path) {
+    DISPATCH_KA(d.KAp, RET_IF(set_smem(h, k_angw_cgrad<KT>, smem_angw_cgrad(d)));
+                DISPATCH_NQ(d.NA, auto kf = k_angw_fwd<KT, NQ>; auto ka = k_angw_adj<KT, NQ>; RET_IF(set_smem(h, kf, smem_angw_fwd(d)));
+                            RET_IF(set_smem(h, ka, smem_angw_adj(d)))));
+  }
   {   // TMEM budget of one k_net_tc warpgroup (256 columns): D1 + max(D1 corrections, D2 + D2 corrections)
     const NetDims nd = net_dims(d);
     if (nd.NnP + std::max(nd.NnP, 2 * nd.NdN) > 256) return fail(h, GNEP_EINVAL, "model too large for tensor memory (n_neurons, n_descriptors)");
@@ -236,6 +260,9 @@ int enqueue_descriptors(gnep_handle *h) {
   const DevSpec &d = h->ds;
   DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_fwd<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, smem_radial(d), d, h->N, h->type_s, h->segR, h->pairR, h->theta, h->q, h->M1));
   mark(h, "a1_radial_descriptor");
+  if (!h->tile_path) {
+    DISPATCH_KA(d.KAp, DISPATCH_NQ(d.NA, auto kf = k_angw_fwd<KT, NQ>; LAUNCH(h, kf, cdiv(h->N, ANG_WARPS * ANG_TA), ANG_WARPS * 32, smem_angw_fwd(d), d, h->N, h->type_s, h->segA, h->pairA, h->theta, h->q, h->Sn, h->A1)));
+  } else
   DISPATCH_ANG(d, auto kf = k_angular_fwd<KT, LMAX>; LAUNCH(h, kf, h->n_tilesA, 32 * ang_warps(d), smem_ang_fwd(d), d, h->n_tilesA, h->tilesA, h->type_s, h->segAu, h->pairAu, h->theta, h->q, h->Sn, h->A1));
   mark(h, "a1_angular_descriptor");
   return GNEP_OK;
@@ -275,6 +302,9 @@ int enqueue_backward(gnep_handle *h) {
   const DevSpec &d = h->ds;
   DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_adj<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, smem_radial(d), d, h->N, h->type_s, h->struct_s, h->segR, h->pairR, h->theta, h->u, h->omega, h->scales, h->D, h->M2));
   mark(h, "a5_radial_adjoint");
+  if (!h->tile_path) {
+    DISPATCH_KA(d.KAp, DISPATCH_NQ(d.NA, auto ka = k_angw_adj<KT, NQ>; LAUNCH(h, ka, cdiv(h->N, ANG_WARPS * ANG_TA), ANG_WARPS * 32, smem_angw_adj(d), d, h->N, h->type_s, h->struct_s, h->segA, h->atomA, h->pairA, h->theta, h->u, h->omega, h->scales, h->Sn, h->Tn, h->A2, h->D)));
+  } else
   DISPATCH_ANG(d, auto ka = k_angular_adj<KT, LMAX>; LAUNCH(h, ka, h->grid_adj, 32 * ang_warps(d), smem_ang_adj(d), d, h->n_tilesA, h->tilesA, h->type_s, h->struct_s, h->segAu, h->pairAu, h->theta, h->u, h->omega, h->scales, h->Sn, h->Beta, h->Tn, h->D, h->partialCA));
   mark(h, "a5_angular_adjoint");
   LAUNCH(h, k_net_tc<true>, h->n_cta_net, 256, smem_net_bwd(d), d, h->sm, h->theta, h->qscale, h->D, h->x, h->eat, h->Ep, (float *)nullptr,
@@ -284,7 +314,10 @@ int enqueue_backward(gnep_handle *h) {
   mark(h, "a6_w0_gradient");
   LAUNCH(h, k_cgrad_radial, h->n_chunks, CR_THREADS, smem_cgrad_rad(d), d, h->sm, h->gbar, h->Ep, h->M1, h->M2, h->partialCR);
   mark(h, "a7_radial_cgrad");
-  DISPATCH_ANG(d, auto kc = k_cgrad_angular<KT, LMAX>; LAUNCH(h, kc, h->grid_cg, 32 * ang_warps(d), smem_cgrad_ang(d), d, h->n_tilesA, h->tilesA, h->type_s, h->Ep, h->gbar, h->Sn, h->Tn, h->A1,
+  if (!h->tile_path) {
+    DISPATCH_KA(d.KAp, LAUNCH(h, k_angw_cgrad<KT>, h->grid_cg, ANG_WARPS * 32, smem_angw_cgrad(d), d, h->N, h->type_s, h->Ep, h->gbar, h->Sn, h->Tn, h->A1, h->A2, h->partialCA));
+  } else
+  DISPATCH_ANG(d, auto kc = k_cgrad_angular<KT, LMAX>; LAUNCH(h, kc, h->grid_cg, 32 * ang_warps(d), smem_cgrad_ang(d), d, h->n_tilesA, h->tilesA, h->type_s, h->segAu, h->Ep, h->gbar, h->Sn, h->Tn, h->A1,
                                                           h->partialCA + (size_t)h->grid_adj * ang_warps(d) * d.T * d.T * d.NA * d.KAp));
   mark(h, "a7_angular_cgrad");
   LAUNCH(h, k_grad_reduce, cdiv(d.P, 8), 256, 0, d, h->rm, (float)h->l2_share, h->theta, h->scales, h->partialCR, h->partialCA, h->partialW, h->partialB, h->grad);
@@ -399,6 +432,10 @@ int gnep_create(const gnep_model_spec *spec, void *cuda_stream, gnep_handle **ou
   else {
     if (cudaStreamCreate(&h->stream) != cudaSuccess) { h->err = "cudaStreamCreate failed"; return bail(GNEP_ECUDA); }
     h->own_stream = true;
+  }
+  {   // GNEP_ANGULAR_MAPPING=groups forces the slot-group kernels for l_max <= 4 as well (they are the only ones above 4)
+    const char *m = getenv("GNEP_ANGULAR_MAPPING");
+    h->tile_path = d.L > 4 || (m && std::string(m) == "groups");
   }
   int rc;
   if ((rc = configure_kernels(h)) != GNEP_OK) return bail(rc);
@@ -708,7 +745,7 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     // neighbour counts (descending), so that the rows a warp walks in lock step have equal lengths; the last tile of a
     // species is filled up with -1 (idle lanes)
     std::vector<int> tiles;
-    {
+    if (h->tile_path) {
       std::vector<std::pair<uint64_t, int>> keyed;
       for (int t = 0; t < T; ++t) {
         const int a0 = h->sm.start[t], a1 = h->sm.start[t + 1];
@@ -727,6 +764,25 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     h->n_tilesA = (int)(tiles.size() / ANG_TILE);
     BA(h->tilesA, tiles.size());
     if (!tiles.empty()) CKT(cudaMemcpyAsync(h->tilesA, tiles.data(), sizeof(int) * tiles.size(), cudaMemcpyHostToDevice, st));
+    // ---- warp-tile path: the angular list once more with every (atom, J) segment padded to a multiple of 4 pairs by
+    // zero-contribution dummies (k_pad_angular), so that the 4-pair register tiles of the sweeps never straddle a segment
+    std::vector<int> segAp;
+    if (!h->tile_path) {
+      segAp.assign((size_t)N * (T + 1) + 1, 0);
+      int64_t nAp = 0;
+      for (int a = 0; a < N; ++a) {
+        for (int J = 0; J < T; ++J) {
+          segAp[(size_t)a * (T + 1) + J] = (int)nAp;
+          nAp += (segAu[(size_t)a * (T + 1) + J + 1] - segAu[(size_t)a * (T + 1) + J] + 3) / 4 * 4;
+        }
+        segAp[(size_t)a * (T + 1) + T] = (int)nAp;
+      }
+      if (nAp >= (int64_t)1 << 31) { tfree(); free_batch(h); return fail(h, GNEP_ERANGE, "2^31 or more (padded) angular pairs"); }
+      BA(h->segA, (size_t)N * (T + 1) + 1); BA(h->atomA, nAp); BA(h->pairA, nAp);
+      CKT(cudaMemcpyAsync(h->segA, segAp.data(), sizeof(int) * ((size_t)N * (T + 1) + 1), cudaMemcpyHostToDevice, st));
+      LAUNCH(h, k_pad_angular, cdiv((int64_t)N * 32, 256), 256, 0, N, T, d_segAu, h->segA, d_pairAu, h->pairA, h->atomA,
+             (float)(2.0 * h->spec.rc_angular));
+    }
     LAUNCH(h, k_nbr_reverse, cdiv((int64_t)N * 32, 256), 256, 0, N, h->rowAu, h->pairAu, d_shA, h->revAu);
     CKT(cudaGetLastError());
     CKT(cudaStreamSynchronize(st));
@@ -755,15 +811,22 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     h->n_cta_net = h->sm.cta_base[GNEP_MAX_SPECIES_C];
     h->n_chunks = h->sm.chunk_base[GNEP_MAX_SPECIES_C];
     h->n_gw = h->sm.gw_base[GNEP_MAX_SPECIES_C];
-    h->grid_adj = std::min(h->n_tilesA, h->occ_adj * h->num_sms);
-    h->grid_cg = std::min(h->n_tilesA, h->occ_cg * h->num_sms);
+    if (h->tile_path) {
+      h->grid_adj = std::min(h->n_tilesA, h->occ_adj * h->num_sms);
+      h->grid_cg = std::min(h->n_tilesA, h->occ_cg * h->num_sms);
+    } else {   // only k_angw_cgrad keeps accumulators: persistent warps, four CTAs per SM
+      h->grid_adj = 0;
+      h->grid_cg = std::max(1, std::min(cdiv(N, ANG_WARPS), 4 * h->num_sms));
+    }
     for (int t = 0; t <= GNEP_MAX_SPECIES_C; ++t) { h->rm.chunk_base[t] = h->sm.chunk_base[t]; h->rm.gw_base[t] = h->sm.gw_base[t]; }
-    h->rm.n_warps_ca = (h->grid_adj + h->grid_cg) * ang_warps(d);   // partial rows: the beta half (adjoint sweep) then the alpha half
+    const int ca_warps = h->tile_path ? ang_warps(d) : ANG_WARPS;
+    h->rm.n_warps_ca = N > 0 ? (h->grid_adj + h->grid_cg) * ca_warps : 0;   // partial rows: the beta half (adjoint sweep) then the alpha half
     // ---- per-atom state ----
     const size_t n = N;
     const size_t npad = n + GW_PAD_ROWS;   // k_gradw_tc bulk-copies whole windows of rows: zeroed rows past the end
     BA(h->q, npad * d.Ndes); BA(h->Sn, n * d.NA * d.nlmS); BA(h->x, npad * d.NnS); BA(h->Ei, n); BA(h->Ep, n * d.Ndes);
-    BA(h->etil, n * T * d.KRp); BA(h->M1, n * T * d.KRp); BA(h->M2, n * T * d.KRp); BA(h->D, npad * d.Ndes); BA(h->Tn, n * d.NA * d.nlmS); BA(h->Beta, n * ang_warps(d) * ang_nap(d.NA) * ANG_GS + 64); BA(h->A1, n * ang_warps(d) * T * d.KAp * ANG_GS);
+    BA(h->etil, n * T * d.KRp); BA(h->M1, n * T * d.KRp); BA(h->M2, n * T * d.KRp); BA(h->D, npad * d.Ndes); BA(h->Tn, n * d.NA * d.nlmS); BA(h->Beta, n * d.NA * d.nlmS); BA(h->A1, h->tile_path ? n * ang_warps(d) * T * d.KAp * ANG_GS : n * T * d.KAp * ANGW_NLM);
+    if (!h->tile_path) BA(h->A2, n * T * d.KAp * ANGW_NLM);
     BA(h->gbar, n * d.Ndes); BA(h->pbuf, npad * d.NnS); BA(h->eat, npad); BA(h->Wat, n * 6);
     BA(h->Fat, n); BA(h->fpair, h->nA); BA(h->u, n);
     BA(h->Es, S); BA(h->Ws, (size_t)S * 6); BA(h->parts, (size_t)S * 3); BA(h->e_s, S); BA(h->omega, (size_t)S * 6);
@@ -774,7 +837,6 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     // slots of the (l,m) rows that no slot group of this model writes (l_max < 4) are read as zeros
     CKT(cudaMemsetAsync(h->Sn, 0, sizeof(float) * n * d.NA * d.nlmS, st));
     CKT(cudaMemsetAsync(h->Tn, 0, sizeof(float) * n * d.NA * d.nlmS, st));
-    CKT(cudaMemsetAsync(h->Beta, 0, sizeof(float) * (n * ang_warps(d) * ang_nap(d.NA) * ANG_GS + 64), st));
     CKT(cudaMemsetAsync(h->q + n * d.Ndes, 0, sizeof(float) * GW_PAD_ROWS * d.Ndes, st));
     CKT(cudaMemsetAsync(h->D + n * d.Ndes, 0, sizeof(float) * GW_PAD_ROWS * d.Ndes, st));
     CKT(cudaMemsetAsync(h->x, 0, sizeof(float) * npad * d.NnS, st));
