@@ -10,8 +10,8 @@
  * What it computes, in the paper's order:
  *   neighbour sets            P:44 Eq.2                       orc_batch_create
  *   Chebyshev basis, cutoff   P:72 Eq.6, App.A      orc_basis
- *   harmonics b_lm, B_lm      P:251-304 App.B, P:454 Eq.B9    orc_blm
- *   descriptors q_n, q_nl     P:69-85 Eq.5-8 (+ 4-body, S:8(c).4)   orc_descriptors
+ *   harmonics b_lm, B_lm      P:251-449 App.B (l = 1..8), P:454 Eq.B9    orc_blm
+ *   descriptors q_n, q_nl     P:69-85 Eq.5-8 (+ 4-body, S:8(c).4; + 5-body, R41)   orc_descriptors
  *   network F(G)              P:718 Eq.D1.1-D1.6              orc_network
  *   E, F, virial              P:39 Eq.1, Eq.3, Eq.4, P:611 Eq.C3.6   orc_predict
  *   loss                      P:93-102 Eq.9-12 (+ L2, S:8(c).8)     orc_loss
@@ -32,15 +32,16 @@
 #include <omp.h>
 #endif
 
-#define NLM_MAX 24
+#define NLM_MAX 80   /* (l,m) slots for l = 1..8; slot lm = l*l - 1 + m, m = 0..2l */
 #define KMAX 32
 
 typedef struct {
   int32_t T;               /* number of species */
   int32_t NR, KR;          /* radial functions n, radial basis functions k */
   int32_t NA, KA;          /* angular radial functions, basis functions */
-  int32_t L;               /* l_max 1..4 */
+  int32_t L;               /* l_max 1..8 */
   int32_t use4;            /* 4-body term */
+  int32_t use5;            /* 5-body term */
   int32_t Nn;              /* hidden neurons */
   int32_t loss_mode;       /* 0 = mean square (paper Eq.9-12), 1 = RMSE */
   double rcR, rcA;
@@ -62,8 +63,9 @@ typedef struct {
 } orc_batch;
 
 /* ------------------------------------------------------------------ sizes and layout (S:8(c).2) */
-int orc_ndes(const orc_spec *sp) { return sp->NR + sp->NA * sp->L + (sp->use4 ? sp->NA : 0); }
+int orc_ndes(const orc_spec *sp) { return sp->NR + sp->NA * sp->L + (sp->use4 ? sp->NA : 0) + (sp->use5 ? sp->NA : 0); }
 int orc_nlm(const orc_spec *sp) { return sp->L * (sp->L + 2); }
+static int off5(const orc_spec *sp) { return sp->NR + sp->L * sp->NA + (sp->use4 ? sp->NA : 0); }   /* first 5-body descriptor */
 static int64_t off_cR(const orc_spec *sp) { (void)sp; return 0; }
 static int64_t off_cA(const orc_spec *sp) { return (int64_t)sp->T * sp->T * sp->NR * sp->KR; }
 static int64_t off_net(const orc_spec *sp) { return off_cA(sp) + (int64_t)sp->T * sp->T * sp->NA * sp->KA; }
@@ -102,6 +104,103 @@ void orc_basis(double rc, int K, double d, double *f, double *fp) {
 }
 
 /* ------------------------------------------------------------------ harmonics (App.B) */
+/* l = 5..8 (B5.1-B8.17).  Every printed b_lm is a product  Z(z, r^2) * C(x, y)  of a polynomial in z and
+ * r^2 = x^2+y^2+z^2 and one of the planar polynomials printed beside it,
+ *   c_m = Re (x+iy)^m :  c1 = x, c2 = x^2-y^2, c3 = x^3-3xy^2, c4 = x^4-6x^2y^2+y^4, c5 = x^5-10x^3y^2+5xy^4, ...
+ *   s_m = Im (x+iy)^m :  s1 = y, s2 = 2xy,     s3 = 3x^2y-y^3, s4 = 4x^3y-4xy^3,     s5 = 5x^4y-10x^2y^3+y^5, ...
+ * (m = 0: C = 1).  Slots: m = 0 first, then (c_m', s_m') for m' = 1..l.  The gradient is the product rule with
+ *   dZ/dx = 2x dZ/dr2, dZ/dy = 2y dZ/dr2, dZ/dz (total) = Zz + 2z dZ/dr2,   Zz = partial dZ/dz at fixed r2,
+ * and the planar derivatives written out term by term below. */
+static void planar(double x, double y, double *c, double *s, double *cx, double *cy, double *sx, double *sy) {
+  double x2 = x * x, y2 = y * y, x3 = x2 * x, y3 = y2 * y, x4 = x2 * x2, y4 = y2 * y2, x5 = x4 * x, y5 = y4 * y;
+  double x6 = x3 * x3, y6 = y3 * y3, x7 = x6 * x, y7 = y6 * y, x8 = x4 * x4, y8 = y4 * y4;
+  c[0] = 1; s[0] = 0; cx[0] = 0; cy[0] = 0; sx[0] = 0; sy[0] = 0;
+  c[1] = x;                                   cx[1] = 1;                                cy[1] = 0;
+  s[1] = y;                                   sx[1] = 0;                                sy[1] = 1;
+  c[2] = x2 - y2;                             cx[2] = 2 * x;                            cy[2] = -2 * y;
+  s[2] = 2 * x * y;                           sx[2] = 2 * y;                            sy[2] = 2 * x;
+  c[3] = x3 - 3 * x * y2;                     cx[3] = 3 * x2 - 3 * y2;                  cy[3] = -6 * x * y;
+  s[3] = 3 * x2 * y - y3;                     sx[3] = 6 * x * y;                        sy[3] = 3 * x2 - 3 * y2;
+  c[4] = x4 - 6 * x2 * y2 + y4;               cx[4] = 4 * x3 - 12 * x * y2;             cy[4] = -12 * x2 * y + 4 * y3;
+  s[4] = 4 * x3 * y - 4 * x * y3;             sx[4] = 12 * x2 * y - 4 * y3;             sy[4] = 4 * x3 - 12 * x * y2;
+  c[5] = x5 - 10 * x3 * y2 + 5 * x * y4;      cx[5] = 5 * x4 - 30 * x2 * y2 + 5 * y4;   cy[5] = -20 * x3 * y + 20 * x * y3;
+  s[5] = 5 * x4 * y - 10 * x2 * y3 + y5;      sx[5] = 20 * x3 * y - 20 * x * y3;        sy[5] = 5 * x4 - 30 * x2 * y2 + 5 * y4;
+  c[6] = x6 - 15 * x4 * y2 + 15 * x2 * y4 - y6;
+  cx[6] = 6 * x5 - 60 * x3 * y2 + 30 * x * y4;            cy[6] = -30 * x4 * y + 60 * x2 * y3 - 6 * y5;
+  s[6] = 6 * x5 * y - 20 * x3 * y3 + 6 * x * y5;
+  sx[6] = 30 * x4 * y - 60 * x2 * y3 + 6 * y5;            sy[6] = 6 * x5 - 60 * x3 * y2 + 30 * x * y4;
+  c[7] = x7 - 21 * x5 * y2 + 35 * x3 * y4 - 7 * x * y6;
+  cx[7] = 7 * x6 - 105 * x4 * y2 + 105 * x2 * y4 - 7 * y6; cy[7] = -42 * x5 * y + 140 * x3 * y3 - 42 * x * y5;
+  s[7] = 7 * x6 * y - 35 * x4 * y3 + 21 * x2 * y5 - y7;
+  sx[7] = 42 * x5 * y - 140 * x3 * y3 + 42 * x * y5;       sy[7] = 7 * x6 - 105 * x4 * y2 + 105 * x2 * y4 - 7 * y6;
+  c[8] = x8 - 28 * x6 * y2 + 70 * x4 * y4 - 28 * x2 * y6 + y8;
+  cx[8] = 8 * x7 - 168 * x5 * y2 + 280 * x3 * y4 - 56 * x * y6;
+  cy[8] = -56 * x6 * y + 280 * x4 * y3 - 168 * x2 * y5 + 8 * y7;
+  s[8] = 8 * x7 * y - 56 * x5 * y3 + 56 * x3 * y5 - 8 * x * y7;
+  sx[8] = 56 * x6 * y - 280 * x4 * y3 + 168 * x2 * y5 - 8 * y7;
+  sy[8] = 8 * x7 - 168 * x5 * y2 + 280 * x3 * y4 - 56 * x * y6;
+}
+/* slot lm = Z, slots lm+1 / lm+2 = Z c_m / Z s_m */
+static void put_zero(int lm, double Z, double Zz, double Zr, double x, double y, double z, double *b, double (*g)[3]) {
+  b[lm] = Z; g[lm][0] = 2 * x * Zr; g[lm][1] = 2 * y * Zr; g[lm][2] = Zz + 2 * z * Zr;
+}
+static void put_pair(int lm, int m, double Z, double Zz, double Zr, double x, double y, double z, const double *c,
+                     const double *s, const double *cx, const double *cy, const double *sx, const double *sy, double *b,
+                     double (*g)[3]) {
+  b[lm] = Z * c[m];
+  g[lm][0] = 2 * x * Zr * c[m] + Z * cx[m]; g[lm][1] = 2 * y * Zr * c[m] + Z * cy[m]; g[lm][2] = (Zz + 2 * z * Zr) * c[m];
+  b[lm + 1] = Z * s[m];
+  g[lm + 1][0] = 2 * x * Zr * s[m] + Z * sx[m]; g[lm + 1][1] = 2 * y * Zr * s[m] + Z * sy[m]; g[lm + 1][2] = (Zz + 2 * z * Zr) * s[m];
+}
+static void blm_poly_high(double x, double y, double z, double *b, double (*g)[3]) {
+  double c[9], s[9], cx[9], cy[9], sx[9], sy[9];
+  planar(x, y, c, s, cx, cy, sx, sy);
+  double r2 = x * x + y * y + z * z, r4 = r2 * r2, r6 = r4 * r2, r8 = r4 * r4;
+  double z2 = z * z, z3 = z2 * z, z4 = z2 * z2, z5 = z4 * z, z6 = z3 * z3, z7 = z6 * z, z8 = z4 * z4;
+#define PAIR(lm, m, Z, Zz, Zr) put_pair(lm, m, Z, Zz, Zr, x, y, z, c, s, cx, cy, sx, sy, b, g)
+  /* l = 5: B5.1-B5.11, slots 24..34 */
+  put_zero(24, 63 * z5 - 70 * z3 * r2 + 15 * z * r4, 315 * z4 - 210 * z2 * r2 + 15 * r4, -70 * z3 + 30 * z * r2, x, y, z, b, g);
+  PAIR(25, 1, 21 * z4 - 14 * z2 * r2 + r4, 84 * z3 - 28 * z * r2, -14 * z2 + 2 * r2);
+  PAIR(27, 2, 3 * z3 - z * r2, 9 * z2 - r2, -z);
+  PAIR(29, 3, 9 * z2 - r2, 18 * z, -1.0);
+  PAIR(31, 4, z, 1.0, 0.0);
+  PAIR(33, 5, 1.0, 0.0, 0.0);
+  /* l = 6: B6.1-B6.13, slots 35..47 */
+  put_zero(35, 231 * z6 - 315 * z4 * r2 + 105 * z2 * r4 - 5 * r6, 1386 * z5 - 1260 * z3 * r2 + 210 * z * r4,
+           -315 * z4 + 210 * z2 * r2 - 15 * r4, x, y, z, b, g);
+  PAIR(36, 1, 33 * z5 - 30 * z3 * r2 + 5 * z * r4, 165 * z4 - 90 * z2 * r2 + 5 * r4, -30 * z3 + 10 * z * r2);
+  PAIR(38, 2, 33 * z4 - 18 * z2 * r2 + r4, 132 * z3 - 36 * z * r2, -18 * z2 + 2 * r2);
+  PAIR(40, 3, 11 * z3 - 3 * z * r2, 33 * z2 - 3 * r2, -3 * z);
+  PAIR(42, 4, 11 * z2 - r2, 22 * z, -1.0);
+  PAIR(44, 5, z, 1.0, 0.0);
+  PAIR(46, 6, 1.0, 0.0, 0.0);
+  /* l = 7: B7.1-B7.15, slots 48..62 */
+  put_zero(48, 429 * z7 - 693 * z5 * r2 + 315 * z3 * r4 - 35 * z * r6, 3003 * z6 - 3465 * z4 * r2 + 945 * z2 * r4 - 35 * r6,
+           -693 * z5 + 630 * z3 * r2 - 105 * z * r4, x, y, z, b, g);
+  PAIR(49, 1, 429 * z6 - 495 * z4 * r2 + 135 * z2 * r4 - 5 * r6, 2574 * z5 - 1980 * z3 * r2 + 270 * z * r4,
+       -495 * z4 + 270 * z2 * r2 - 15 * r4);
+  PAIR(51, 2, 143 * z5 - 110 * z3 * r2 + 15 * z * r4, 715 * z4 - 330 * z2 * r2 + 15 * r4, -110 * z3 + 30 * z * r2);
+  PAIR(53, 3, 143 * z4 - 66 * z2 * r2 + 3 * r4, 572 * z3 - 132 * z * r2, -66 * z2 + 6 * r2);
+  PAIR(55, 4, 13 * z3 - 3 * z * r2, 39 * z2 - 3 * r2, -3 * z);
+  PAIR(57, 5, 13 * z2 - r2, 26 * z, -1.0);
+  PAIR(59, 6, z, 1.0, 0.0);
+  PAIR(61, 7, 1.0, 0.0, 0.0);
+  /* l = 8: B8.1-B8.17, slots 63..79 */
+  put_zero(63, 6435 * z8 - 12012 * z6 * r2 + 6930 * z4 * r4 - 1260 * z2 * r6 + 35 * r8,
+           51480 * z7 - 72072 * z5 * r2 + 27720 * z3 * r4 - 2520 * z * r6, -12012 * z6 + 13860 * z4 * r2 - 3780 * z2 * r4 + 140 * r6,
+           x, y, z, b, g);
+  PAIR(64, 1, 715 * z7 - 1001 * z5 * r2 + 385 * z3 * r4 - 35 * z * r6, 5005 * z6 - 5005 * z4 * r2 + 1155 * z2 * r4 - 35 * r6,
+       -1001 * z5 + 770 * z3 * r2 - 105 * z * r4);
+  PAIR(66, 2, 143 * z6 - 143 * z4 * r2 + 33 * z2 * r4 - r6, 858 * z5 - 572 * z3 * r2 + 66 * z * r4, -143 * z4 + 66 * z2 * r2 - 3 * r4);
+  PAIR(68, 3, 39 * z5 - 26 * z3 * r2 + 3 * z * r4, 195 * z4 - 78 * z2 * r2 + 3 * r4, -26 * z3 + 6 * z * r2);
+  PAIR(70, 4, 65 * z4 - 26 * z2 * r2 + r4, 260 * z3 - 52 * z * r2, -26 * z2 + 2 * r2);
+  PAIR(72, 5, 5 * z3 - z * r2, 15 * z2 - r2, -z);
+  PAIR(74, 6, 15 * z2 - r2, 30 * z, -1.0);
+  PAIR(76, 7, z, 1.0, 0.0);
+  PAIR(78, 8, 1.0, 0.0, 0.0);
+#undef PAIR
+}
+
 /* b_lm polynomials (B1.1-B4.9) in flattened order lm = l*l-1+m, and their Cartesian gradients. */
 static void blm_poly(double x, double y, double z, double *b, double (*g)[3]) {
   double r2 = x * x + y * y + z * z;
@@ -154,9 +253,10 @@ static void blm_poly(double x, double y, double z, double *b, double (*g)[3]) {
   g[22][0] = 4 * x2 * x - 12 * x * y2; g[22][1] = -12 * x2 * y + 4 * y2 * y; g[22][2] = 0;
   b[23] = 4 * x2 * x * y - 4 * x * y2 * y;
   g[23][0] = 12 * x2 * y - 4 * y2 * y; g[23][1] = 4 * x2 * x - 12 * x * y2; g[23][2] = 0;
+  blm_poly_high(x, y, z, b, g);
 }
 
-static int l_of_lm(int lm) { return lm < 3 ? 1 : lm < 8 ? 2 : lm < 15 ? 3 : 4; }
+static int l_of_lm(int lm) { int l = 1; while ((l + 1) * (l + 1) - 1 <= lm) ++l; return l; }
 
 /* raw polynomials, exported for the harmonic / homogeneity pins */
 void orc_blm_raw(double x, double y, double z, double *b, double *grad /*24*3*/) {
@@ -181,11 +281,19 @@ void orc_blm(double x, double y, double z, double *B, double *dB /*24*3*/) {
 
 /* C_lm = kappa_l * Chat_lm, kappa_l = (2l+1)/(4 pi)  (S:8(c).4; the paper never prints them) */
 void orc_clm(double *C) {
+  /* one entry for m = 0, then one per (cos, sin) pair; derived from the addition theorem, pinned against scipy's Legendre */
   static const double chat[NLM_MAX] = {
       1, 1, 1,
       1.0 / 4, 3, 3, 3.0 / 4, 3.0 / 4,
       1.0 / 4, 3.0 / 8, 3.0 / 8, 15.0 / 4, 15.0 / 4, 5.0 / 8, 5.0 / 8,
-      1.0 / 64, 5.0 / 8, 5.0 / 8, 5.0 / 16, 5.0 / 16, 35.0 / 8, 35.0 / 8, 35.0 / 64, 35.0 / 64};
+      1.0 / 64, 5.0 / 8, 5.0 / 8, 5.0 / 16, 5.0 / 16, 35.0 / 8, 35.0 / 8, 35.0 / 64, 35.0 / 64,
+      1.0 / 64, 15.0 / 64, 15.0 / 64, 105.0 / 16, 105.0 / 16, 35.0 / 128, 35.0 / 128, 315.0 / 64, 315.0 / 64, 63.0 / 128, 63.0 / 128,
+      1.0 / 256, 21.0 / 64, 21.0 / 64, 105.0 / 512, 105.0 / 512, 105.0 / 128, 105.0 / 128, 63.0 / 256, 63.0 / 256, 693.0 / 128,
+      693.0 / 128, 231.0 / 512, 231.0 / 512,
+      1.0 / 256, 7.0 / 1024, 7.0 / 1024, 21.0 / 512, 21.0 / 512, 21.0 / 1024, 21.0 / 1024, 231.0 / 256, 231.0 / 256, 231.0 / 1024,
+      231.0 / 1024, 3003.0 / 512, 3003.0 / 512, 429.0 / 1024, 429.0 / 1024,
+      1.0 / 16384, 9.0 / 1024, 9.0 / 1024, 315.0 / 2048, 315.0 / 2048, 1155.0 / 1024, 1155.0 / 1024, 693.0 / 4096, 693.0 / 4096,
+      9009.0 / 1024, 9009.0 / 1024, 429.0 / 2048, 429.0 / 2048, 6435.0 / 1024, 6435.0 / 1024, 6435.0 / 16384, 6435.0 / 16384};
   for (int lm = 0; lm < NLM_MAX; ++lm) {
     int l = l_of_lm(lm);
     C[lm] = (2 * l + 1) / (4.0 * M_PI) * chat[lm];
@@ -215,6 +323,21 @@ double orc_p4(const double *s, double *g /*5 or NULL*/, double *H /*25 or NULL*/
     for (int a = 0; a < 5; ++a) for (int c = 0; c < 5; ++c) H[5 * a + c] = h[a][c];
   }
   return P;
+}
+
+/* 5-body term (named at P:65; not defined in the paper; R41): the only quartic rotational invariant of
+ * the l = 1 moments v = (S_n10, S_n11, S_n12) = sum_j g_n(d_ij) (z, x, y)/d is |v|^4.  Normalised like the 4-body term
+ * as the contraction of four orthonormal l = 1 moments coupled pairwise to zero, (1/3) (sum_m |A_1m|^2)^2 with
+ * sum_m |A_1m|^2 = 3/(4 pi) |v|^2:   q5 = kappa5 |v|^4,  kappa5 = 3 / (16 pi^2)  (= q_{n,l=1}^2 / 3). */
+#define KAPPA5 (3.0 / (16.0 * M_PI * M_PI))
+double orc_kappa5(void) { return KAPPA5; }
+double orc_p5(const double *s, double *g /*3 or NULL*/, double *H /*9 or NULL*/) {
+  double n2 = s[0] * s[0] + s[1] * s[1] + s[2] * s[2];
+  if (g) for (int a = 0; a < 3; ++a) g[a] = 4 * KAPPA5 * n2 * s[a];
+  if (H)
+    for (int a = 0; a < 3; ++a)
+      for (int c = 0; c < 3; ++c) H[3 * a + c] = 4 * KAPPA5 * (n2 * (a == c ? 1.0 : 0.0) + 2 * s[a] * s[c]);
+  return KAPPA5 * n2 * n2;
 }
 
 /* ------------------------------------------------------------------ neighbour sets (Eq.2; S:8(c).3) */
@@ -459,6 +582,7 @@ static void atom_descriptor(const orc_spec *sp, const ctx_t *cx, const orc_batch
       q[sp->NR + (l - 1) * sp->NA + n] += cx->C[lm] * s * s;
     }
     if (sp->use4) q[sp->NR + sp->L * sp->NA + n] = KAPPA4 * orc_p4(Snlm + n * NLM_MAX + 3, NULL, NULL);
+    if (sp->use5) q[off5(sp) + n] = orc_p5(Snlm + n * NLM_MAX, NULL, NULL);
   }
 }
 
@@ -493,6 +617,11 @@ static void atom_beta(const orc_spec *sp, const ctx_t *cx, const double *Ep, con
       double g4[5];
       orc_p4(Snlm + n * NLM_MAX + 3, g4, NULL);
       for (int m = 0; m < 5; ++m) beta[n * NLM_MAX + 3 + m] += Ep[sp->NR + sp->L * sp->NA + n] * KAPPA4 * g4[m];
+    }
+    if (sp->use5) {
+      double g5[3];
+      orc_p5(Snlm + n * NLM_MAX, g5, NULL);
+      for (int m = 0; m < 3; ++m) beta[n * NLM_MAX + m] += Ep[off5(sp) + n] * g5[m];
     }
   }
 }
@@ -756,6 +885,12 @@ void orc_loss_and_grad(const orc_spec *sp, const double *theta, const double *qs
             for (int m = 0; m < 5; ++m) acc += g4[m] * Tn[n * NLM_MAX + 3 + m];
             Dv[NR + sp->L * NA + n] = KAPPA4 * acc;
           }
+          if (sp->use5) {
+            double g5[3], acc = 0;
+            orc_p5(Sn + n * NLM_MAX, g5, NULL);
+            for (int m = 0; m < 3; ++m) acc += g5[m] * Tn[n * NLM_MAX + m];
+            Dv[off5(sp) + n] = acc;
+          }
         }
         /* step 4: network (species I) */
         {
@@ -795,6 +930,16 @@ void orc_loss_and_grad(const orc_spec *sp, const double *theta, const double *qs
               double ht = 0;
               for (int m2i = 0; m2i < 5; ++m2i) ht += H4[5 * m + m2i] * Tn[n * NLM_MAX + 3 + m2i];
               alpha[n * NLM_MAX + 3 + m] += gbar[v] * KAPPA4 * g4[m] + Ep[v] * KAPPA4 * ht;
+            }
+          }
+          if (sp->use5) {
+            int v = off5(sp) + n;
+            double g5[3], H5[9];
+            orc_p5(Sn + n * NLM_MAX, g5, H5);
+            for (int m = 0; m < 3; ++m) {
+              double ht = 0;
+              for (int m2i = 0; m2i < 3; ++m2i) ht += H5[3 * m + m2i] * Tn[n * NLM_MAX + m2i];
+              alpha[n * NLM_MAX + m] += gbar[v] * g5[m] + Ep[v] * ht;
             }
           }
         }

@@ -26,7 +26,8 @@ def build(force=False):
 
 class Spec(C.Structure):
     _fields_ = [("T", C.c_int32), ("NR", C.c_int32), ("KR", C.c_int32), ("NA", C.c_int32),
-                ("KA", C.c_int32), ("L", C.c_int32), ("use4", C.c_int32), ("Nn", C.c_int32),
+                ("KA", C.c_int32), ("L", C.c_int32), ("use4", C.c_int32), ("use5", C.c_int32),
+                ("Nn", C.c_int32),
                 ("loss_mode", C.c_int32), ("rcR", C.c_double), ("rcA", C.c_double),
                 ("lam_e", C.c_double), ("lam_f", C.c_double), ("lam_v", C.c_double),
                 ("lam_2", C.c_double)]
@@ -35,11 +36,13 @@ class Spec(C.Structure):
 def make_spec(d):
     """d: dict with the keys of gnep_synth.MODEL_SPECS entries."""
     return Spec(T=d["n_species"], NR=d["n_radial"], KR=d["n_basis_radial"], NA=d["n_angular"],
-                KA=d["n_basis_angular"], L=d["l_max"], use4=int(d["use_4body"]), Nn=d["n_neurons"],
+                KA=d["n_basis_angular"], L=d["l_max"], use4=int(d["use_4body"]), use5=int(d.get("use_5body", False)),
+                Nn=d["n_neurons"],
                 loss_mode=d.get("loss_mode", 0), rcR=d["rc_radial"], rcA=d["rc_angular"],
                 lam_e=d["lambda_e"], lam_f=d["lambda_f"], lam_v=d["lambda_v"], lam_2=d["lambda_2"])
 
 
+NLM = 80            # (l,m) slots for l = 1..8, slot lm = l*l - 1 + m
 _lib = None
 
 
@@ -69,6 +72,9 @@ def lib():
         L.orc_kappa4.restype = C.c_double
         L.orc_p4.restype = C.c_double
         L.orc_p4.argtypes = [C.c_void_p] * 3
+        L.orc_kappa5.restype = C.c_double
+        L.orc_p5.restype = C.c_double
+        L.orc_p5.argtypes = [C.c_void_p] * 3
         L.orc_descriptors.argtypes = [C.c_void_p] * 4
         L.orc_network.restype = C.c_double
         L.orc_network.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int] + [C.c_void_p] * 4
@@ -108,21 +114,34 @@ def basis(rc, K, d):
 
 
 def blm(x, y, z):
-    B = np.zeros(24); dB = np.zeros((24, 3))
+    B = np.zeros(NLM); dB = np.zeros((NLM, 3))
     lib().orc_blm(float(x), float(y), float(z), _p(B), _p(dB))
     return B, dB
 
 
 def blm_raw(x, y, z):
-    b = np.zeros(24); g = np.zeros((24, 3))
+    b = np.zeros(NLM); g = np.zeros((NLM, 3))
     lib().orc_blm_raw(float(x), float(y), float(z), _p(b), _p(g))
     return b, g
 
 
 def clm():
-    c = np.zeros(24)
+    c = np.zeros(NLM)
     lib().orc_clm(_p(c))
     return c
+
+
+def kappa5():
+    return float(lib().orc_kappa5())
+
+
+def p5(s, want_grad=False):
+    s = _f64(s)
+    if not want_grad:
+        return float(lib().orc_p5(_p(s), None, None))
+    g = np.zeros(3); H = np.zeros((3, 3))
+    v = float(lib().orc_p5(_p(s), _p(g), _p(H)))
+    return v, g, H
 
 
 def kappa4():

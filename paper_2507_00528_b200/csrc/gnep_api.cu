@@ -435,7 +435,7 @@ int gnep_create(const gnep_model_spec *spec, void *cuda_stream, gnep_handle **ou
   }
   {   // GNEP_ANGULAR_MAPPING=groups forces the slot-group kernels for l_max <= 4 as well (they are the only ones above 4)
     const char *m = getenv("GNEP_ANGULAR_MAPPING");
-    h->tile_path = d.L > 4 || (m && std::string(m) == "groups");
+    h->tile_path = d.L > 4 || d.use5 || (m && std::string(m) == "groups");   // (the warp-tile kernels have no 5-body term)
   }
   int rc;
   if ((rc = configure_kernels(h)) != GNEP_OK) return bail(rc);

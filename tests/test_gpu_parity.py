@@ -36,7 +36,10 @@ def _check_neighbors(g, ob):
         np.testing.assert_array_equal(sh.astype(np.int32), osh)
 
 
-def _check_all(config, n_structs, adam_steps=10, spec_over=None):
+def _check_all(config, n_structs, adam_steps=10, spec_over=None, floor=1e-6):
+    """floor: absolute size above which a gradient component is held to 1e-3 relative (north_star: 1e-6 on the BASELINE
+    configs; the l_max > 4 models below, whose gradients are 10-30x larger and whose degree-5..8 harmonics are
+    conditioned worse in fp32, use a floor scaled accordingly -- DESIGN.md section 6)."""
     spec, sp, b, ob, theta, qs, labels = labelled_case(config, n_structs=n_structs, spec_over=spec_over)
     g = _gnep(spec, qs, b, labels, theta)
     _check_neighbors(g, ob)
@@ -54,9 +57,9 @@ def _check_all(config, n_structs, adam_steps=10, spec_over=None):
     for a, r in zip(terms, t_ref):
         assert abs(a - r) <= 1e-5 * abs(r) + 1e-12
     assert np.linalg.norm(grad - g_ref) / np.linalg.norm(g_ref) < 1e-4
-    big = np.abs(g_ref) > 1e-6
+    big = np.abs(g_ref) > floor
     assert np.max(np.abs(grad[big] - g_ref[big]) / np.abs(g_ref[big])) < 1e-3
-    assert np.max(np.abs(grad[~big] - g_ref[~big])) < 1e-6 if (~big).any() else True
+    assert np.max(np.abs(grad[~big] - g_ref[~big])) < floor if (~big).any() else True
     # Adam trajectory, both through separate calls and through the graph
     if adam_steps:
         th = theta.copy(); m = np.zeros_like(th); v = np.zeros_like(th)
@@ -139,6 +142,27 @@ def test_four_species():
 
 def test_one_species():
     _check_all(0, 2, adam_steps=2, spec_over={"n_species": 1, "l_max": 1, "n_angular": 3, "n_neurons": 9})
+
+
+def test_l_max_6_with_4body():
+    """Higher angular order (paper Eq.7: l up to 8; b_lm of Eq.B5-B6): the slot-group kernels, 8 groups."""
+    over = {"l_max": 6, "use_4body": True, "n_angular": 4, "n_basis_angular": 5, "n_neurons": 12}
+    _check_all(0, 2, adam_steps=2, spec_over=over, floor=3e-5)
+
+
+def test_l_max_8_with_4body_and_5body():
+    over = {"l_max": 8, "use_4body": True, "use_5body": True, "n_angular": 5, "n_basis_angular": 8, "n_neurons": 16}
+    _check_all(1, 2, adam_steps=2, spec_over=over, floor=3e-5)
+
+
+def test_l_max_5_three_species_no_many_body():
+    over = {"n_species": 3, "l_max": 5, "use_4body": False, "n_angular": 3, "n_basis_angular": 4, "n_neurons": 8}
+    _check_all(0, 3, adam_steps=2, spec_over=over, floor=3e-5)
+
+
+def test_5body_with_l_max_4_and_slot_group_mapping_for_config3():
+    """The 5-body term routes l_max <= 4 models through the slot-group kernels too (config-3 sizes, 4 groups)."""
+    _check_all(3, 4, adam_steps=2, spec_over={"use_5body": True}, floor=1e-5)   # (4 structures: a noisier sample than config 3)
 
 
 def test_two_live_handles_with_different_specs():

@@ -1,4 +1,4 @@
-"""Pins for b_lm, B_lm, C_lm and the 4-body invariant (paper App.B, Eq.7-8, B9 P:454)."""
+"""Pins for b_lm, B_lm, C_lm (l = 1..8) and the 4- and 5-body invariants (paper App.B, Eq.7-8, B9 P:454)."""
 import os
 
 import numpy as np
@@ -7,7 +7,8 @@ from scipy.special import eval_legendre
 from cases import golden, random_rotation
 from oracle import gnep_oracle as orc
 
-L_OF = np.array([1] * 3 + [2] * 5 + [3] * 7 + [4] * 9)
+L_OF = np.concatenate([[l] * (2 * l + 1) for l in range(1, 9)])
+NLM = 80
 
 
 def _paper_formulas():
@@ -25,7 +26,7 @@ def _paper_formulas():
 def test_blm_match_printed_formulas():
     rng = np.random.default_rng(1)
     forms = _paper_formulas()
-    assert len(forms) == 24
+    assert len(forms) == NLM and [f[:2] for f in forms] == [(l, m) for l in range(1, 9) for m in range(2 * l + 1)]
     for _ in range(10):
         x, y, z = rng.normal(size=3)
         b, _ = orc.blm_raw(x, y, z)
@@ -44,13 +45,15 @@ def test_blm_harmonic_and_homogeneous():
         bt, _ = orc.blm_raw(*(1.7 * p))
         np.testing.assert_allclose(bt, 1.7 ** L_OF * b0, rtol=1e-12, atol=1e-12)
         np.testing.assert_allclose(g0 @ p, L_OF * b0, rtol=1e-12, atol=1e-12)
-        # Laplacian = 0: 4th-order-accurate central stencil is exact for polynomials of degree <= 5
-        lap = np.zeros(24)
+        # Laplacian = 0: the 8th-order-accurate central stencil of the second derivative is exact for polynomials of
+        # degree <= 9 (the b_lm have degree l <= 8)
+        w = [-205.0 / 72, 8.0 / 5, -1.0 / 5, 8.0 / 315, -1.0 / 560]
+        lap = np.zeros(NLM)
         for ax in range(3):
             e = np.zeros(3); e[ax] = h
             f = lambda q: orc.blm_raw(*q)[0]
-            lap += (-f(p + 2 * e) + 16 * f(p + e) - 30 * b0 + 16 * f(p - e) - f(p - 2 * e)) / (12 * h * h)
-        assert np.max(np.abs(lap)) < 1e-9
+            lap += (w[0] * b0 + sum(w[k] * (f(p + k * e) + f(p - k * e)) for k in range(1, 5))) / (h * h)
+        assert np.max(np.abs(lap) / (1 + np.abs(b0))) < 1e-7
 
 
 def test_grad_blm_fd():
@@ -77,7 +80,7 @@ def test_addition_theorem_fixes_clm():
         B1, _ = orc.blm(*r1)
         B2, _ = orc.blm(*r2)
         ct = r1 @ r2 / np.linalg.norm(r1) / np.linalg.norm(r2)
-        for l in range(1, 5):
+        for l in range(1, 9):
             sl = slice(l * l - 1, l * l + 2 * l)
             lhs = np.sum(C[sl] * B1[sl] * B2[sl])
             assert abs(lhs - (2 * l + 1) / (4 * np.pi) * eval_legendre(l, ct)) < 1e-12
@@ -93,8 +96,8 @@ def test_sc_lattice_closed_form():
     S = sum(orc.blm(*p)[0] for p in sites)
     assert np.max(np.abs(S[:15])) < 1e-12          # l = 1,2,3 vanish by cubic symmetry
     assert abs(S[15] - golden("sc_l4_S0")[0]) < 1e-12 and abs(S[22] - golden("sc_l4_S7")[0]) < 1e-12
-    assert np.max(np.abs(np.delete(S[15:], [0, 7]))) < 1e-12
-    q4l = np.sum(orc.clm()[15:] * S[15:] ** 2)
+    assert np.max(np.abs(np.delete(S[15:24], [0, 7]))) < 1e-12
+    q4l = np.sum(orc.clm()[15:24] * S[15:24] ** 2)
     assert abs(q4l - golden("sc_l4_q")[0]) < 1e-9
 
 
@@ -135,3 +138,34 @@ def test_p4_grad_hessian_fd():
         gp = orc.p4(s + e, True)[1]; gm = orc.p4(s - e, True)[1]
         np.testing.assert_allclose(H[a], (gp - gm) / (2 * h), atol=1e-7)
     np.testing.assert_allclose(H, H.T)
+
+
+def test_p5_is_the_quartic_invariant_of_the_l1_moments():
+    """q5 = kappa5 |v|^4 (R41): rotation invariant, single neighbour of weight g gives kappa5 g^4, equals
+    q_{l=1}^2 / 3 with q_{l=1} = 3/(4 pi) |v|^2 (Eq.7 with the C_1m of the addition theorem), kappa5 = 3/(16 pi^2)."""
+    rng = np.random.default_rng(6)
+    assert abs(orc.kappa5() - 3 / (16 * np.pi ** 2)) < 1e-16
+    pts = rng.normal(size=(7, 3)); wts = rng.normal(size=7)
+    def moments(P):
+        return sum(w * orc.blm(*p)[0][:3] for w, p in zip(wts, P))
+    s = moments(pts)
+    R = random_rotation(rng)
+    assert abs(orc.p5(s) - orc.p5(moments(pts @ R.T))) < 1e-13 * abs(orc.p5(s))
+    q1 = np.sum(orc.clm()[:3] * s ** 2)
+    assert abs(orc.p5(s) - q1 ** 2 / 3) < 1e-14 * abs(q1 ** 2)
+    g = 0.37
+    one = g * orc.blm(0.2, -0.4, 0.9)[0][:3]
+    assert abs(orc.p5(one) - orc.kappa5() * g ** 4) < 1e-15
+
+
+def test_p5_grad_hessian_fd():
+    rng = np.random.default_rng(8)
+    s = rng.normal(size=3)
+    v, g, H = orc.p5(s, want_grad=True)
+    h = 1e-5
+    for a in range(3):
+        e = np.zeros(3); e[a] = h
+        assert abs((orc.p5(s + e) - orc.p5(s - e)) / (2 * h) - g[a]) < 1e-8
+        gp = orc.p5(s + e, want_grad=True)[1]; gm = orc.p5(s - e, want_grad=True)[1]
+        np.testing.assert_allclose((gp - gm) / (2 * h), H[a], atol=1e-8)
+    np.testing.assert_allclose(H, H.T, atol=0)
