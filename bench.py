@@ -40,6 +40,9 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-structs", type=int, default=0, help="structures in the oracle sample (0 = auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--minibatch", type=int, default=0,
+                    help="structures per mini-batch: time the paper's training regime (P:142: mini-batches of size 1), one "
+                         "Adam step per mini-batch through shared handles, instead of the full-batch epoch")
     return ap.parse_args()
 
 
@@ -276,40 +279,58 @@ def run_ours(args):
             acc[name] = acc.get(name, 0.0) + t_ms / nprof
     g.set_profiling(0)
     tot_phase = sum(acc.values())
-    flops = fm.phase_flops(spec, N_local, info["n_pairs_radial"], info["n_pairs_angular"])
-    byts = fm.phase_bytes(spec, N_local, info["n_pairs_radial"], info["n_pairs_angular"])
+    npr, npa = info["n_pairs_radial"], info["n_pairs_angular"]
+    mflops = fm.method_flops(spec, N_local, npr, npa); mbytes = fm.method_bytes(spec, N_local, npr, npa)
+    dflops = fm.phase_flops(spec, N_local, npr, npa); dbytes = fm.phase_bytes(spec, N_local, npr, npa)
+    if "a1_descriptor_contraction" in acc:     # descriptor pair sweeps hoisted to load time: only the contraction is in the epoch
+        cf, cb = fm.contraction_phase(spec, N_local)
+        for dct, val in ((mflops, cf), (dflops, cf), (mbytes, cb), (dbytes, cb)):
+            dct["a1_descriptor_contraction"] = val
+            dct.pop("a1_radial_descriptor", None); dct.pop("a1_angular_descriptor", None)
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except Exception:
         pass
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
-    hbm_src = "measured (MEASURED_PEAKS.json)" if "hbm_gbs" in peaks else "fallback (B200_PROFILING.md)"
-    fp32_peak = fm.fp32_peak_tflops()
+    hbm_src = "measured copy bandwidth (MEASURED_PEAKS.json)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
+    # FP32 FMA peak measured in this run (register-only FMA chains on every SM, ~60 ms, CUDA events) next to the nominal one
+    pk = g.measure_fp32_peak(60.0)
+    fp32_meas, fp32_nom = pk["tflops"], fm.fp32_peak_tflops()
     top = max(acc, key=acc.get)
     t_top = acc[top] * 1e-3
-    tf = flops[top] / t_top / 1e12; gbs = byts[top] / t_top / 1e9
-    if tf / fp32_peak >= gbs / hbm_peak:
-        roof = {"bound": "alu", "achieved": tf, "peak": fp32_peak, "unit": "TFLOP/s", "frac": tf / fp32_peak,
-                "traffic": None, "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md section 5)"}
+    bound = fm.PHASE_BOUND.get(top, "alu")
+    # committed ncu capture of this workload, if any: DRAM bytes of the dominant kernel per launch
+    traffic, traffic_src = None, None
+    tfile = os.path.join(ROOT, "profiles", "r2_cfg%d_traffic.csv" % args.config)
+    if not args.structs and os.path.exists(tfile):
+        for ln in open(tfile):
+            f = ln.strip().split(",")
+            if f and f[0] == top:
+                traffic = int(float(f[-1])); traffic_src = "committed capture profiles/%s (ncu --set full, not re-measured in this run)" % os.path.basename(tfile)
+    if bound == "hbm":
+        ach = mbytes[top] / t_top / 1e9
+        roof = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "traffic": traffic,
+                "peak_source": hbm_src}
     else:
-        roof = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
-                "traffic": None, "peak_source": hbm_src}
-    if args.config == 4 and not args.structs:      # the workload of the committed ncu capture (profiles/r1_v8_cfg4_traffic.md)
-        try:
-            for ln in open(os.path.join(ROOT, "profiles", "r1_v8_cfg4_traffic.csv")):
-                f = ln.strip().split(",")
-                if f[0] == top:
-                    roof["traffic"] = int(f[-1]); roof["traffic_unit"] = "DRAM bytes per launch (ncu --set full)"
-                    roof["algorithmic_bytes"] = int(byts[top])
-        except OSError:
-            pass
-    roof["kernel"] = top
-    roof["kernel_ms"] = acc[top]
-    roof["kernel_share_of_step"] = acc[top] / tot_phase
-    path_tf = sum(flops.values()) / (ms_step * 1e-3) / 1e12 * (N_local / max(N_local, 1))
-    phases = {k: {"ms": round(v, 4), "tflops": round(flops[k] / (v * 1e-3) / 1e12, 3) if v > 0 else None,
-                  "gbs": round(byts[k] / (v * 1e-3) / 1e9, 1) if v > 0 else None} for k, v in acc.items()}
+        ach = mflops[top] / t_top / 1e12
+        roof = {"bound": "alu", "achieved": ach, "peak": fp32_meas, "unit": "TFLOP/s", "frac": ach / fp32_meas, "traffic": traffic,
+                "peak_source": "FP32 FMA microbenchmark in this run (gnep_measure_fp32_peak, %.0f ms, implied SM clock %.0f MHz)" % (pk["ms"], pk["implied_sm_mhz"]),
+                "frac_of_nominal_peak": ach / fp32_nom, "peak_nominal": fp32_nom,
+                "peak_nominal_source": "148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz (B200_PROFILING.md unit counts)"}
+    roof.update({"kernel": top, "kernel_ms": acc[top], "kernel_share_of_step": acc[top] / tot_phase,
+                 "count": "method-algorithmic (SURVEY 8(d).3, flopmodel.method_flops / method_bytes)",
+                 "method_flops": mflops[top], "method_bytes": mbytes[top], "design_flops": dflops[top], "design_bytes": dbytes[top],
+                 "bound_from": "ncu captures under profiles/ (flopmodel.PHASE_BOUND), not from a comparison of fractions"})
+    if traffic_src:
+        roof["traffic_source"] = traffic_src
+    path_tf = sum(mflops.values()) / (ms_step * 1e-3) / 1e12
+    path_tf_design = sum(dflops.values()) / (ms_step * 1e-3) / 1e12
+    phases = {k: {"ms": round(v, 4), "bound": fm.PHASE_BOUND.get(k),
+                  "method_tflops": round(mflops[k] / (v * 1e-3) / 1e12, 3) if v > 0 else None,
+                  "method_gbs": round(mbytes[k] / (v * 1e-3) / 1e9, 1) if v > 0 else None,
+                  "design_tflops": round(dflops[k] / (v * 1e-3) / 1e12, 3) if v > 0 else None,
+                  "design_gbs": round(dbytes[k] / (v * 1e-3) / 1e9, 1) if v > 0 else None} for k, v in acc.items()}
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -325,7 +346,10 @@ def run_ours(args):
                    "generate_s": round(setup_t["gen_s"], 2), "load_batch_s": round(setup_t["load_batch_s"], 3)},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
         "roofline": roof,
-        "path": {"algorithmic_tflops": path_tf, "frac_of_fp32_peak": path_tf / fp32_peak, "flop_per_atom_env": sum(flops.values()) / max(N_local, 1),
+        "path": {"method_tflops": path_tf, "frac_of_fp32_peak_measured": path_tf / fp32_meas, "frac_of_fp32_peak_nominal": path_tf / fp32_nom,
+                 "method_flop_per_atom_env": sum(mflops.values()) / max(N_local, 1), "method_bytes_per_atom_env": sum(mbytes.values()) / max(N_local, 1),
+                 "design_tflops": path_tf_design, "design_flop_per_atom_env": sum(dflops.values()) / max(N_local, 1),
+                 "fp32_peak_measured_tflops": fp32_meas, "fp32_peak_nominal_tflops": fp32_nom, "fp32_peak_implied_sm_mhz": pk["implied_sm_mhz"],
                  "phase_sum_ms": tot_phase},
         "phases": phases,
         "loss_terms_last": [float(x) for x in last_terms],
@@ -342,10 +366,99 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_minibatch(args):
+    """The paper's regime (Fig.1 caption: mini-batches of size 1; Eq.17 schedule): every mini-batch is a resident
+    batch on a shared handle, a step = one CUDA-graph replay of loss + gradient + Adam at lr(s).  One JSON line in the
+    same contract; `ms_per_step` is per mini-batch step."""
+    import torch
+    from paper_2507_00528_b200 import Gnep, lr_schedule
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_stream(torch.cuda.Stream())
+    cfg, B = args.config, args.minibatch
+    spec = dict(gs.MODEL_SPECS[cfg])
+    nb = max(1, min(64, (args.structs or gs.N_STRUCTS[cfg]) // B))
+    b = gs.make_batch(cfg, n_structs=nb * B)
+    off = b["atom_offsets"]
+    parent = Gnep(spec, stream=torch.cuda.current_stream())
+    theta = gs.draw_params(spec, cfg, "student").astype(np.float32)
+    teacher = gs.draw_params(spec, cfg, "teacher").astype(np.float32)
+    parent.load_batch(off, b["positions"], b["cells"], b["types"])
+    parent.set_params(theta)
+    qs = gs.q_scale_from(parent.descriptors())
+    parent.set_q_scale(qs)
+    parent.set_params(teacher)
+    E, F, W = gs.add_label_noise(cfg, off, *parent.predict())
+    parent.set_params(theta)
+    handles, host = [], []
+    for k in range(nb):
+        lo, hi = k * B, (k + 1) * B
+        a0, a1 = off[lo], off[hi]
+        h = parent if k == 0 else parent.create_shared()
+        arrs = ((off[lo:hi + 1] - a0).astype(np.int32), b["positions"][a0:a1], b["cells"][lo:hi], b["types"][a0:a1],
+                E[lo:hi].astype(np.float64), F[a0:a1].astype(np.float64), W[lo:hi].astype(np.float64))
+        h.load_batch(*arrs)
+        handles.append(h); host.append(arrs)
+    n_total = args.warmup + args.steps
+
+    def step(s, want_terms):
+        lr = lr_schedule(s, max(1, n_total // 10), n_total, LR, 1e-2 * LR)
+        return handles[s % nb].train_epochs(1, lr, want_terms=want_terms)
+
+    for s in range(args.warmup):
+        step(s, False)
+    sampler = ClockSampler(int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.synchronize()
+    sampler.start()
+    l0 = sum(h.launch_count() for h in handles)
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    e0.record()
+    atoms = 0
+    for s in range(args.warmup, n_total):
+        step(s, False)
+        atoms += int(host[s % nb][0][-1])
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    launches = sum(h.launch_count() for h in handles) - l0
+    # end to end: the mini-batch arrives from HOST memory every step (neighbour build included), the loss goes back
+    t0 = time.perf_counter()
+    e0.record()
+    atoms2, h2d = 0, 0
+    for s in range(args.steps):
+        arrs = host[s % nb]
+        handles[s % nb].load_batch(*arrs)
+        terms = step(s, True)
+        atoms2 += int(arrs[0][-1]); h2d += sum(a.nbytes for a in arrs)
+    e1.record()
+    torch.cuda.synchronize()
+    ms2 = max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3)
+    out = {"metric": METRIC, "value": atoms / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+           "data": "synthetic",
+           "config": {"workload": "%s/minibatch-%d" % (gs.WORKLOAD_NAMES[cfg], B), "minibatches_resident": nb,
+                      "atoms_per_step": atoms / args.steps, "steps_per_s": args.steps / (ms * 1e-3),
+                      "step": "gnep_train_epochs(1) on a shared handle: CUDA graph of loss+grad+Adam at lr(s) (Eq.17)",
+                      "regime": "paper P:142 (mini-batch training); launch/latency-bound, no roofline claimed"},
+           "clocks": clocks, "gpu_launches": int(launches), "roofline": None,
+           "e2e": {"value": atoms2 / (ms2 * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d // args.steps, "d2h_bytes_per_step": 20,
+                   "what": "gnep_load_batch(host arrays of the mini-batch, neighbour build) + train step + loss terms to host"},
+           "loss_terms_last": [float(x) for x in terms]}
+    for h in handles[1:]:
+        h.destroy()
+    parent.destroy()
+    print(json.dumps(out))
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         run_reference(args)
+    elif args.minibatch:
+        if int(os.environ.get("RANK", "0")) == 0:
+            run_minibatch(args)
     else:
         run_ours(args)
 

@@ -128,48 +128,79 @@ __device__ __forceinline__ void tile_setup(TileInfo *ti, const DevSpec &sp, cons
   }
 }
 
-// slot of (n, lm) of atom al in a slot array
+// slot of (n, lm) of atom al in a slot array; the stride SST = 32 * ang_groups(LMAX) + 1 is a compile-time constant (also
+// for models with l_max < LMAX, which simply leave the upper groups' slots unused), so that slot offsets are immediates
+template <int LMAX> struct AngDims {
+  static constexpr int NG = ang_groups(LMAX), NTH = 32 * NG, SST = NTH + 1, NLM = LMAX * (LMAX + 2), NS = LMAX <= 4 ? 24 : 88;
+};
+__host__ __device__ constexpr int ang_sst(int lmax) { return 32 * ang_groups(lmax) + 1; }
 __device__ __forceinline__ int slot_of(int n, int lm, int sst, int al) { return (n * ANG_GS + lm % ANG_GS) * sst + (lm / ANG_GS) * 32 + al; }
 
-// cooperative global -> slot array: the tile's rows g[a][n][NS] (NA*NS floats per atom, NS = row stride of LMAX)
+// cooperative global -> slot array: the tile's rows g[a][n][NS] (NA*NS floats per atom); lanes run along an atom's rows,
+// 32 bytes each.  A piece is 8 consecutive slots of one row, so its slot offsets from the row's base are immediates.
+template <int LMAX, int PART>
+__device__ __forceinline__ void piece_to_slots(float *Xn, const float8 &v8, int ng) {
+  constexpr int SST = AngDims<LMAX>::SST;
+  const float v[8] = {v8.lo.x, v8.lo.y, v8.lo.z, v8.lo.w, v8.hi.x, v8.hi.y, v8.hi.z, v8.hi.w};
+#pragma unroll
+  for (int e = 0; e < 8; ++e) {
+    constexpr int dummy = 0; (void)dummy;
+    const int lm = 8 * PART + e;
+    if (lm < AngDims<LMAX>::NG * ANG_GS && lm / ANG_GS < ng) Xn[(lm % ANG_GS) * SST + (lm / ANG_GS) * 32] = v[e];
+  }
+}
+template <int LMAX, int PART>
+__device__ __forceinline__ void slots_to_piece(const float *Xn, float (&v)[8], int ng) {
+  constexpr int SST = AngDims<LMAX>::SST;
+#pragma unroll
+  for (int e = 0; e < 8; ++e) {
+    const int lm = 8 * PART + e;
+    v[e] = (lm < AngDims<LMAX>::NG * ANG_GS && lm / ANG_GS < ng) ? Xn[(lm % ANG_GS) * SST + (lm / ANG_GS) * 32] : 0.f;
+  }
+}
+#define ANG_PART_CASE(LMAX, pt, CALL) case pt: if constexpr (AngDims<LMAX>::NS / 8 > pt) { constexpr int PART = pt; CALL; } break;
+#define ANG_PART_SWITCH(LMAX, part, CALL)                                                                       \
+  switch (part) {                                                                                               \
+    ANG_PART_CASE(LMAX, 0, CALL) ANG_PART_CASE(LMAX, 1, CALL) ANG_PART_CASE(LMAX, 2, CALL) ANG_PART_CASE(LMAX, 3, CALL)   \
+    ANG_PART_CASE(LMAX, 4, CALL) ANG_PART_CASE(LMAX, 5, CALL) ANG_PART_CASE(LMAX, 6, CALL) ANG_PART_CASE(LMAX, 7, CALL)   \
+    ANG_PART_CASE(LMAX, 8, CALL) ANG_PART_CASE(LMAX, 9, CALL) ANG_PART_CASE(LMAX, 10, CALL)                               \
+    default: break;                                                                                             \
+  }
 template <int LMAX>
-__device__ __forceinline__ void coop_load_rows(const DevSpec &sp, const TileInfo *ti, const float *__restrict__ g, float *X, int sst, int ng) {
-  constexpr int NS = LMAX <= 4 ? 24 : 88;
-  const int len8 = sp.NA * NS / 8;
+__device__ __forceinline__ void coop_load_rows(const DevSpec &sp, const TileInfo *ti, const float *__restrict__ g, float *X, int ng) {
+  constexpr int NS = AngDims<LMAX>::NS, P8 = NS / 8, SST = AngDims<LMAX>::SST;
+  const int len8 = sp.NA * P8;
   for (int x = threadIdx.x; x < ANG_TILE * len8; x += blockDim.x) {
     const int al = x / len8, c8 = x - al * len8, a = ti->at[al];
     if (a < 0) continue;
+    const int n = c8 / P8, part = c8 - n * P8;
     const float8 v8 = ldg256(g + (size_t)a * sp.NA * NS + 8 * c8);
-    const float v[8] = {v8.lo.x, v8.lo.y, v8.lo.z, v8.lo.w, v8.hi.x, v8.hi.y, v8.hi.z, v8.hi.w};
-#pragma unroll
-    for (int e = 0; e < 8; ++e) {
-      const int e8 = 8 * c8 + e, n = e8 / NS, lm = e8 - n * NS;
-      if (lm < ng * ANG_GS) X[slot_of(n, lm, sst, al)] = v[e];
-    }
+    float *Xn = X + n * ANG_GS * SST + al;
+    ANG_PART_SWITCH(LMAX, part, (piece_to_slots<LMAX, PART>(Xn, v8, ng)));
   }
 }
 // cooperative slot array -> global rows (slots of groups that do not exist are written as zero)
 template <int LMAX>
-__device__ __forceinline__ void coop_store_rows(const DevSpec &sp, const TileInfo *ti, const float *X, int sst, int ng, float *__restrict__ g) {
-  constexpr int NS = LMAX <= 4 ? 24 : 88;
-  const int len8 = sp.NA * NS / 8;
+__device__ __forceinline__ void coop_store_rows(const DevSpec &sp, const TileInfo *ti, const float *X, int ng, float *__restrict__ g) {
+  constexpr int NS = AngDims<LMAX>::NS, P8 = NS / 8, SST = AngDims<LMAX>::SST;
+  const int len8 = sp.NA * P8;
   for (int x = threadIdx.x; x < ANG_TILE * len8; x += blockDim.x) {
     const int al = x / len8, c8 = x - al * len8, a = ti->at[al];
     if (a < 0) continue;
+    const int n = c8 / P8, part = c8 - n * P8;
+    const float *Xn = X + n * ANG_GS * SST + al;
     float v[8];
-#pragma unroll
-    for (int e = 0; e < 8; ++e) {
-      const int e8 = 8 * c8 + e, n = e8 / NS, lm = e8 - n * NS;
-      v[e] = lm < ng * ANG_GS ? X[slot_of(n, lm, sst, al)] : 0.f;
-    }
+    ANG_PART_SWITCH(LMAX, part, (slots_to_piece<LMAX, PART>(Xn, v, ng)));
     stg256(g + (size_t)a * sp.NA * NS + 8 * c8, make_float4(v[0], v[1], v[2], v[3]), make_float4(v[4], v[5], v[6], v[7]));
   }
 }
 // one (atom, n) row gathered from a slot array
 template <int LMAX>
-__device__ __forceinline__ void gather_row(const float *X, int n, int sst, int ng, int al, float (&s)[LMAX * (LMAX + 2)]) {
+__device__ __forceinline__ void gather_row(const float *X, int n, int ng, int al, float (&s)[LMAX * (LMAX + 2)]) {
+  constexpr int SST = AngDims<LMAX>::SST;
+  const float *Xn = X + n * ANG_GS * SST + al;
 #pragma unroll
-  for (int lm = 0; lm < LMAX * (LMAX + 2); ++lm) s[lm] = lm / ANG_GS < ng ? X[slot_of(n, lm, sst, al)] : 0.f;
+  for (int lm = 0; lm < LMAX * (LMAX + 2); ++lm) s[lm] = lm / ANG_GS < ng ? Xn[(lm % ANG_GS) * SST + (lm / ANG_GS) * 32] : 0.f;
 }
 
 // the harmonics of slot group G of a unit vector: B[i] = B_lm, lm = 6G + i (and, with the pair adjoint (ax,ay,az), ar =
@@ -250,15 +281,15 @@ __device__ __forceinline__ void copy_out_rows(const DevSpec &sp, const TileInfo 
   }
 }
 // X[n] (+)= c[I][J][n][.] . acc[.][6]: the thread-local contraction of a finished species segment into the thread's slots
-template <int KT>
-__device__ __forceinline__ void contract_segment(const DevSpec &sp, const float *c, const float (&acc)[KT * ANG_GS], float *x_t, int sst, bool first) {
-  for (int n = 0; n < sp.NA; ++n) {
+template <int KT, int SST>
+__device__ __forceinline__ void contract_segment(const DevSpec &sp, const float *c, const float (&acc)[KT * ANG_GS], float *x_t, bool first) {
+  for (int n = 0; n < sp.NA; ++n, x_t += ANG_GS * SST, c += KT) {
     float s[ANG_GS];
 #pragma unroll
-    for (int i = 0; i < ANG_GS; ++i) s[i] = first ? 0.f : x_t[(n * ANG_GS + i) * sst];
+    for (int i = 0; i < ANG_GS; ++i) s[i] = first ? 0.f : x_t[i * SST];
 #pragma unroll
     for (int k4 = 0; k4 < KT; k4 += 4) {
-      const float4 c4 = *(const float4 *)(c + n * KT + k4);
+      const float4 c4 = *(const float4 *)(c + k4);
       const float cv[4] = {c4.x, c4.y, c4.z, c4.w};
 #pragma unroll
       for (int kk = 0; kk < 4; ++kk)
@@ -266,32 +297,35 @@ __device__ __forceinline__ void contract_segment(const DevSpec &sp, const float 
         for (int i = 0; i < ANG_GS; ++i) s[i] = fmaf(cv[kk], acc[(k4 + kk) * ANG_GS + i], s[i]);
     }
 #pragma unroll
-    for (int i = 0; i < ANG_GS; ++i) x_t[(n * ANG_GS + i) * sst] = s[i];
+    for (int i = 0; i < ANG_GS; ++i) x_t[i * SST] = s[i];
   }
 }
 
 // ------------------------------------------------------------------------------------------------
 // a1 (angular): A1 moments, S_nlm (Eq.8), q_nl (Eq.7), many-body terms (R14, R41)
 // ------------------------------------------------------------------------------------------------
-// shared-memory floats: coefficients | S slots [NA*6][SST] | descriptor rows [32][nqa|1] | pair stage [PC][32][KT+4] | TileInfo
-__host__ __device__ inline int ang_fwd_smem_floats(int T, int NA, int KT, int nwarps, int nqa) {
-  return ((T * T * NA * KT + 3) & ~3) + ((NA * ANG_GS * (32 * nwarps + 1) + 3) & ~3) + ((ANG_TILE * (nqa | 1) + 3) & ~3) +
-         ANG_PC * 32 * (KT + 4) + (int)(sizeof(TileInfo) / 4);
+// shared-memory floats: coefficients | S slots [NA*6][SST] | descriptor rows [32][nqa|1] | pair stage 2 x [PC][32][KT+4] | TileInfo
+__host__ __device__ inline int ang_fwd_smem_floats(int T, int NA, int KT, int lmax, int nqa) {
+  return ((T * T * NA * KT + 3) & ~3) + ((NA * ANG_GS * ang_sst(lmax) + 3) & ~3) + ((ANG_TILE * (nqa | 1) + 3) & ~3) +
+         2 * ANG_PC * 32 * (KT + 4) + (int)(sizeof(TileInfo) / 4);
 }
 
 template <int KT, int LMAX>
-__global__ void __launch_bounds__(32 * ang_groups(LMAX), LMAX <= 4 ? 4 : 1)
+__global__ void __launch_bounds__(32 * ang_groups(LMAX), LMAX <= 4 ? 3 : 1)
 k_angular_fwd(DevSpec sp, int n_tiles, const int *__restrict__ tiles, const int *__restrict__ type_s,
               const int *__restrict__ segA, const float4 *__restrict__ pairA, const float *__restrict__ theta,
               float *__restrict__ q, float *__restrict__ S, float *__restrict__ A1g) {
   extern __shared__ __align__(128) float smem[];
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nthr = blockDim.x, ng = nthr >> 5, sst = nthr + 1;
+  constexpr int SST = AngDims<LMAX>::SST, NF4 = KT / 4 + 1, PSZ = ANG_PC * 32 * NF4;
+  // the CTA always has ang_groups(LMAX) warps; those beyond the model's ng slot groups (l_max < LMAX) only help with phase 1
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5, ng = ang_groups(sp.L);
+  const bool grp = w < ng;
   const int nqa = sp.Ndes - sp.NR, qst = nqa | 1;
   float *cs = smem;                                             // [T*T*NA][KT]
   float *Sst = cs + ((sp.T * sp.T * sp.NA * KT + 3) & ~3);      // S slots
-  float *QS = Sst + ((sp.NA * ANG_GS * sst + 3) & ~3);          // [32][qst]
-  float4 *PS = (float4 *)(QS + ((ANG_TILE * qst + 3) & ~3));    // [KT/4 + 1][PC][32]: f_k, then (hx, hy, hz, -)
-  TileInfo *ti = (TileInfo *)(PS + ANG_PC * 32 * (KT / 4 + 1));
+  float *QS = Sst + ((sp.NA * ANG_GS * SST + 3) & ~3);          // [32][qst]
+  float4 *PS = (float4 *)(QS + ((ANG_TILE * qst + 3) & ~3));    // 2 x [KT/4 + 1][PC][32]: f_k, then (hx, hy, hz, -)
+  TileInfo *ti = (TileInfo *)(PS + 2 * PSZ);
   stage_coeff(cs, theta + sp.offA, sp.T * sp.T * sp.NA, sp.KA, KT);
   tile_setup(ti, sp, tiles, blockIdx.x, segA);
   __syncthreads();
@@ -299,33 +333,38 @@ k_angular_fwd(DevSpec sp, int n_tiles, const int *__restrict__ tiles, const int 
   const int I = type_s[ti->at[0]];
   float *s_t = Sst + threadIdx.x;
   float *A1a = A1g + ((size_t)max(a, 0) * ng + w) * sp.T * KT * ANG_GS;
+  int buf = 0;
   for (int J = 0; J < sp.T; ++J) {
     float acc[KT * ANG_GS];
 #pragma unroll
     for (int x = 0; x < KT * ANG_GS; ++x) acc[x] = 0.f;
     const int lo = ti->seg[lane][J], len = ti->seg[lane][J + 1] - lo, mlen = ti->maxlen[J];
-    for (int c0 = 0; c0 < mlen; c0 += ANG_PC) {
-      __syncthreads();                                          // the stage is free
-      for (int p = w; p < ANG_PC; p += ng)                      // phase 1: radial basis and unit vector, once per pair
+    for (int c0 = 0; c0 < mlen; c0 += ANG_PC, buf ^= 1) {
+      float4 *ps = PS + buf * PSZ + lane;
+      // phase 1: radial basis and unit vector, once per pair (warp w takes the pairs w, w + ng, ... of the chunk).  The
+      // stage is double-buffered: the barrier below also orders this chunk's writes after everybody's reads of the chunk
+      // before the previous one.
+      for (int p = w; p < ANG_PC; p += nw)
         if (c0 + p < len) {
           const float4 r = pairA[lo + c0 + p];
           float d, rinv, f[KT];
           pair_len(r.x * r.x + r.y * r.y + r.z * r.z, d, rinv);
           cheb_f<KT>(d, sp.rcAinv, f);
 #pragma unroll
-          for (int k4 = 0; k4 < KT / 4; ++k4) PS[(k4 * ANG_PC + p) * 32 + lane] = make_float4(f[4 * k4], f[4 * k4 + 1], f[4 * k4 + 2], f[4 * k4 + 3]);
-          PS[((KT / 4) * ANG_PC + p) * 32 + lane] = make_float4(r.x * rinv, r.y * rinv, r.z * rinv, 0.f);
+          for (int k4 = 0; k4 < KT / 4; ++k4) ps[(k4 * ANG_PC + p) * 32] = make_float4(f[4 * k4], f[4 * k4 + 1], f[4 * k4 + 2], f[4 * k4 + 3]);
+          ps[((KT / 4) * ANG_PC + p) * 32] = make_float4(r.x * rinv, r.y * rinv, r.z * rinv, 0.f);
         }
       __syncthreads();
-      const int np = min(ANG_PC, len - c0);                     // phase 2: harmonics of this group, K x 6 outer products
-      for (int p = 0; p < np; ++p) {
+      const int np = grp ? min(ANG_PC, len - c0) : 0;           // phase 2: harmonics of this group, K x 6 outer products
+      const float4 *pp = ps;
+      for (int p = 0; p < np; ++p, pp += 32) {
         float f[KT], B[ANG_GS];
 #pragma unroll
         for (int k4 = 0; k4 < KT / 4; ++k4) {
-          const float4 f4 = PS[(k4 * ANG_PC + p) * 32 + lane];
+          const float4 f4 = pp[k4 * ANG_PC * 32];
           f[4 * k4] = f4.x; f[4 * k4 + 1] = f4.y; f[4 * k4 + 2] = f4.z; f[4 * k4 + 3] = f4.w;
         }
-        const float4 h = PS[((KT / 4) * ANG_PC + p) * 32 + lane];
+        const float4 h = pp[(KT / 4) * ANG_PC * 32];
 #pragma unroll
         for (int i = 0; i < ANG_GS; ++i) B[i] = 0.f;
         ANG_GROUP_SWITCH(LMAX, w, (harm_case<LMAX, G>(h.x, h.y, h.z, B)));
@@ -335,19 +374,19 @@ k_angular_fwd(DevSpec sp, int n_tiles, const int *__restrict__ tiles, const int 
           for (int i = 0; i < ANG_GS; ++i) acc[k * ANG_GS + i] = fmaf(f[k], B[i], acc[k * ANG_GS + i]);
       }
     }
-    if (a >= 0) {
+    if (a >= 0 && grp) {
       st_block<KT * ANG_GS / 8>(A1a + (size_t)J * KT * ANG_GS, acc);
-      contract_segment<KT>(sp, cs + (size_t)(I * sp.T + J) * sp.NA * KT, acc, s_t, sst, J == 0);
+      contract_segment<KT, SST>(sp, cs + (size_t)(I * sp.T + J) * sp.NA * KT, acc, s_t, J == 0);
     }
   }
   __syncthreads();                                              // the S rows of the tile are complete in the slot array
   if (a >= 0)
-    for (int n = w; n < sp.NA; n += ng) {
+    for (int n = w; n < sp.NA; n += nw) {
       float s[LMAX * (LMAX + 2)];
-      gather_row<LMAX>(Sst, n, sst, ng, lane, s);
+      gather_row<LMAX>(Sst, n, ng, lane, s);
       finish_q<LMAX>(sp, s, QS + lane * qst, n);
     }
-  coop_store_rows<LMAX>(sp, ti, Sst, sst, ng, S);
+  coop_store_rows<LMAX>(sp, ti, Sst, ng, S);
   __syncthreads();
   copy_out_rows(sp, ti, QS, qst, q);
 }
@@ -356,11 +395,14 @@ k_angular_fwd(DevSpec sp, int n_tiles, const int *__restrict__ tiles, const int 
 // a5 (angular) + the beta half of a7: A2 moments with the pair adjoint a_ij, T_nlm = c.A2, D_(n,l), D_4, D_5, and
 // dL/dcA[I][J][n][k] += sum_lm beta_nlm A2[J][k][lm]  (beta = E' dq/dS was written by k_angular_force)
 // ------------------------------------------------------------------------------------------------
+#define ANG_PCA 4         // pairs per atom per staged chunk of the adjoint sweep (its stage holds 2K+8 floats per pair)
+
 // shared-memory floats: coefficients | T slots | beta slots (S slots for the finishing step) | D rows [32][nqa|1] | pair stage
-// [PC][32][2KT+8] | per-warp scratch [32][33] | per-warp accumulators [T*T][NA*KT] | TileInfo
-__host__ __device__ inline int ang_adj_smem_floats(int T, int NA, int KT, int nwarps, int nqa) {
-  return ((T * T * NA * KT + 3) & ~3) + 2 * ((NA * ANG_GS * (32 * nwarps + 1) + 3) & ~3) + ((ANG_TILE * (nqa | 1) + 3) & ~3) +
-         ANG_PC * 32 * (2 * KT + 8) + nwarps * 32 * 33 + ((nwarps * T * T * NA * KT + 3) & ~3) + (int)(sizeof(TileInfo) / 4);
+// 2 x [PCA][32][2KT+8] | per-warp scratch [32][33] | per-warp accumulators [T*T][NA*KT] | TileInfo
+__host__ __device__ inline int ang_adj_smem_floats(int T, int NA, int KT, int lmax, int nqa) {
+  const int nwarps = ang_groups(lmax);
+  return ((T * T * NA * KT + 3) & ~3) + 2 * ((NA * ANG_GS * ang_sst(lmax) + 3) & ~3) + ((ANG_TILE * (nqa | 1) + 3) & ~3) +
+         2 * ANG_PCA * 32 * (2 * KT + 8) + nwarps * 32 * 33 + ((nwarps * T * T * NA * KT + 3) & ~3) + (int)(sizeof(TileInfo) / 4);
 }
 
 template <int KT, int LMAX>
@@ -371,20 +413,24 @@ k_angular_adj(DevSpec sp, int n_tiles, const int *__restrict__ tiles, const int 
               const float *__restrict__ scales, const float *__restrict__ S, const float *__restrict__ Beta,
               float *__restrict__ Tn, float *__restrict__ D, float *__restrict__ partial) {
   extern __shared__ __align__(128) float smem[];
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nthr = blockDim.x, ng = nthr >> 5, sst = nthr + 1;
+  constexpr int SST = AngDims<LMAX>::SST, NGM = AngDims<LMAX>::NG, NF4 = KT / 2 + 2, PSZ = ANG_PCA * 32 * NF4;
+  constexpr int PPT = (ANG_PCA + NGM - 1) / NGM;                 // pairs per thread and chunk in phase 1 (1 with 4 or more warps)
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5, ng = ang_groups(sp.L);   // nw == NGM
+  const bool grp = w < ng;
   const int ncs = (sp.T * sp.T * sp.NA * KT + 3) & ~3, nv = sp.NA * KT, nacc = sp.T * sp.T * nv;
-  const int nqa = sp.Ndes - sp.NR, qst = nqa | 1, nslot = (sp.NA * ANG_GS * sst + 3) & ~3;
+  const int nqa = sp.Ndes - sp.NR, qst = nqa | 1, nslot = (sp.NA * ANG_GS * SST + 3) & ~3;
   float *cs = smem;
   float *Tst = cs + ncs;
   float *Bst = Tst + nslot;
   float *DS = Bst + nslot;
-  float4 *PS = (float4 *)(DS + ((ANG_TILE * qst + 3) & ~3));    // [2 KT/4 + 2][PC][32]: f_k' (a.rhat), f_k, (rhat, 1/d), (a, a.rhat)
-  float *scr = (float *)(PS + ANG_PC * 32 * (KT / 2 + 2)) + w * 32 * 33;
-  float *accw = (float *)(PS + ANG_PC * 32 * (KT / 2 + 2)) + ng * 32 * 33 + w * nacc;
-  TileInfo *ti = (TileInfo *)((float *)(PS + ANG_PC * 32 * (KT / 2 + 2)) + ng * 32 * 33 + ((ng * nacc + 3) & ~3));
+  float4 *PS = (float4 *)(DS + ((ANG_TILE * qst + 3) & ~3));    // 2 x [2 KT/4 + 2][PCA][32]: f_k' (a.rhat), f_k, (rhat, 1/d), (a, a.rhat)
+  float *scr = (float *)(PS + 2 * PSZ) + w * 32 * 33;
+  float *accw = (float *)(PS + 2 * PSZ) + NGM * 32 * 33 + w * nacc;
+  TileInfo *ti = (TileInfo *)((float *)(PS + 2 * PSZ) + NGM * 32 * 33 + ((NGM * nacc + 3) & ~3));
   stage_coeff(cs, theta + sp.offA, sp.T * sp.T * sp.NA, sp.KA, KT);
   for (int o = lane; o < nacc; o += 32) accw[o] = 0.f;
   const float sfF = scales[1], svV = scales[2];
+  int buf = 0;
   for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
     __syncthreads();                                            // the previous tile is done with every shared array
     tile_setup(ti, sp, tiles, tile, segA);
@@ -392,7 +438,23 @@ k_angular_adj(DevSpec sp, int n_tiles, const int *__restrict__ tiles, const int 
     const int a = ti->at[lane];
     const bool act = a >= 0;
     const int I = type_s[ti->at[0]];
-    coop_load_rows<LMAX>(sp, ti, Beta, Bst, sst, ng);           // (visible after the first chunk barrier / the flush barrier)
+    // Phase 1 of a chunk belongs to warp w for the pairs w, w + ng, ... < PCA of every atom (lane).  Their records and the
+    // gathered u_j are requested one chunk ahead (the first chunk of the next species segment before the flush of the
+    // current one), so that no global latency is exposed in the chunk loop.
+    float4 rq[PPT], uq[PPT];
+    auto request = [&](int J, int c0) {
+#pragma unroll
+      for (int t = 0; t < PPT; ++t) {
+        const int p = w + t * nw;
+        const bool on = J < sp.T && p < ANG_PCA && c0 + p < ti->seg[lane][J + 1] - ti->seg[lane][J];
+        rq[t] = on ? pairA[ti->seg[lane][J] + c0 + p] : make_float4(1.f, 0.f, 0.f, __int_as_float(max(a, 0)));
+        uq[t] = u[__float_as_int(rq[t].w)];
+      }
+    };
+    int Jn = 0;                                                 // first species segment that has pairs in this tile
+    while (Jn < sp.T && ti->maxlen[Jn] == 0) ++Jn;
+    request(Jn, 0);
+    coop_load_rows<LMAX>(sp, ti, Beta, Bst, ng);                // (visible after the first chunk barrier / the flush barrier)
     // this lane's atom: adjoint seed u_i and the structure's omega, used by phase 1
     float4 ui = make_float4(0.f, 0.f, 0.f, 0.f);
     float om[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
@@ -409,13 +471,14 @@ k_angular_adj(DevSpec sp, int n_tiles, const int *__restrict__ tiles, const int 
       float acc[KT * ANG_GS];
 #pragma unroll
       for (int x = 0; x < KT * ANG_GS; ++x) acc[x] = 0.f;
-      const int lo = ti->seg[lane][J], len = ti->seg[lane][J + 1] - lo, mlen = ti->maxlen[J];
-      for (int c0 = 0; c0 < mlen; c0 += ANG_PC) {
-        __syncthreads();
-        for (int p = w; p < ANG_PC; p += ng)                    // phase 1: one record, one gather, one basis evaluation per pair
-          if (c0 + p < len) {
-            const float4 r = pairA[lo + c0 + p];
-            const float4 uj = u[__float_as_int(r.w)];
+      const int len = ti->seg[lane][J + 1] - ti->seg[lane][J], mlen = ti->maxlen[J];
+      for (int c0 = 0; c0 < mlen; c0 += ANG_PCA, buf ^= 1) {
+        float4 *ps = PS + buf * PSZ + lane;
+#pragma unroll
+        for (int t = 0; t < PPT; ++t) {                         // phase 1: one record, one gather, one basis evaluation per pair
+          const int p = w + t * nw;
+          if (p < ANG_PCA && c0 + p < len) {
+            const float4 r = rq[t], uj = uq[t];
             float d, rinv, f[KT], fp[KT];
             pair_len(r.x * r.x + r.y * r.y + r.z * r.z, d, rinv);
             const float ax = sfF * (ui.x - uj.x) - (om[0] * r.x + om[5] * r.z);
@@ -426,23 +489,31 @@ k_angular_adj(DevSpec sp, int n_tiles, const int *__restrict__ tiles, const int 
             cheb_ffp<KT>(d, sp.rcAinv, f, fp);
 #pragma unroll
             for (int k4 = 0; k4 < KT / 4; ++k4) {
-              PS[(k4 * ANG_PC + p) * 32 + lane] = make_float4(fp[4 * k4] * ar, fp[4 * k4 + 1] * ar, fp[4 * k4 + 2] * ar, fp[4 * k4 + 3] * ar);
-              PS[((KT / 4 + k4) * ANG_PC + p) * 32 + lane] = make_float4(f[4 * k4], f[4 * k4 + 1], f[4 * k4 + 2], f[4 * k4 + 3]);
+              ps[(k4 * ANG_PCA + p) * 32] = make_float4(fp[4 * k4] * ar, fp[4 * k4 + 1] * ar, fp[4 * k4 + 2] * ar, fp[4 * k4 + 3] * ar);
+              ps[((KT / 4 + k4) * ANG_PCA + p) * 32] = make_float4(f[4 * k4], f[4 * k4 + 1], f[4 * k4 + 2], f[4 * k4 + 3]);
             }
-            PS[((KT / 2) * ANG_PC + p) * 32 + lane] = make_float4(hx, hy, hz, rinv);
-            PS[((KT / 2 + 1) * ANG_PC + p) * 32 + lane] = make_float4(ax, ay, az, ar);
+            ps[((KT / 2) * ANG_PCA + p) * 32] = make_float4(hx, hy, hz, rinv);
+            ps[((KT / 2 + 1) * ANG_PCA + p) * 32] = make_float4(ax, ay, az, ar);
           }
+        }
+        if (c0 + ANG_PCA < mlen) request(J, c0 + ANG_PCA);      // next chunk of this segment, or the next segment's first
+        else {
+          Jn = J + 1;
+          while (Jn < sp.T && ti->maxlen[Jn] == 0) ++Jn;
+          request(Jn, 0);
+        }
         __syncthreads();
-        const int np = min(ANG_PC, len - c0);
-        for (int p = 0; p < np; ++p) {                          // phase 2
+        const int np = grp ? min(ANG_PCA, len - c0) : 0;
+        const float4 *pp = ps;
+        for (int p = 0; p < np; ++p, pp += 32) {                // phase 2
           float f1[KT], f2[KT], X[ANG_GS], Y[ANG_GS];
 #pragma unroll
           for (int k4 = 0; k4 < KT / 4; ++k4) {
-            const float4 u4 = PS[(k4 * ANG_PC + p) * 32 + lane], v4 = PS[((KT / 4 + k4) * ANG_PC + p) * 32 + lane];
+            const float4 u4 = pp[k4 * ANG_PCA * 32], v4 = pp[(KT / 4 + k4) * ANG_PCA * 32];
             f1[4 * k4] = u4.x; f1[4 * k4 + 1] = u4.y; f1[4 * k4 + 2] = u4.z; f1[4 * k4 + 3] = u4.w;
             f2[4 * k4] = v4.x; f2[4 * k4 + 1] = v4.y; f2[4 * k4 + 2] = v4.z; f2[4 * k4 + 3] = v4.w;
           }
-          const float4 h = PS[((KT / 2) * ANG_PC + p) * 32 + lane], av = PS[((KT / 2 + 1) * ANG_PC + p) * 32 + lane];
+          const float4 h = pp[(KT / 2) * ANG_PCA * 32], av = pp[(KT / 2 + 1) * ANG_PCA * 32];
 #pragma unroll
           for (int i = 0; i < ANG_GS; ++i) { X[i] = 0.f; Y[i] = 0.f; }
           ANG_GROUP_SWITCH(LMAX, w, (harm_case<LMAX, G>(h.x, h.y, h.z, h.w, av.x, av.y, av.z, av.w, X, Y)));
@@ -452,14 +523,16 @@ k_angular_adj(DevSpec sp, int n_tiles, const int *__restrict__ tiles, const int 
             for (int i = 0; i < ANG_GS; ++i) acc[k * ANG_GS + i] = fmaf(f1[k], X[i], fmaf(f2[k], Y[i], acc[k * ANG_GS + i]));
         }
       }
-      __syncthreads();                                          // beta slots are loaded (needed when the tile has no pairs at all)
-      if (act) contract_segment<KT>(sp, cs + (size_t)(I * sp.T + J) * sp.NA * KT, acc, t_t, sst, J == 0);
+      if (J == 0) __syncthreads();                              // beta slots are loaded (also when the first segment is empty)
+      if (!grp) continue;
+      if (act) contract_segment<KT, SST>(sp, cs + (size_t)(I * sp.T + J) * sp.NA * KT, acc, t_t, J == 0);
       // dL/dcA[I][J][n][k] += sum_{lm in group} beta_nlm A2[J][k][lm], summed over the 32 atoms of the warp
       ls.accw = accw + (I * sp.T + J) * nv;
       constexpr int NPC = LaneSum<KT>::NPC;
+      const float *bn = b_t;
       for (int ch = 0; ch * NPC < sp.NA; ++ch) {
 #pragma unroll
-        for (int nn = 0; nn < NPC; ++nn) {
+        for (int nn = 0; nn < NPC; ++nn, bn += ANG_GS * SST) {
           const int n = ch * NPC + nn;
           float g[KT];
 #pragma unroll
@@ -467,7 +540,7 @@ k_angular_adj(DevSpec sp, int n_tiles, const int *__restrict__ tiles, const int 
           if (act && n < sp.NA) {
             float be[ANG_GS];
 #pragma unroll
-            for (int i = 0; i < ANG_GS; ++i) be[i] = b_t[(n * ANG_GS + i) * sst];
+            for (int i = 0; i < ANG_GS; ++i) be[i] = bn[i * SST];
 #pragma unroll
             for (int k = 0; k < KT; ++k)
 #pragma unroll
@@ -479,21 +552,21 @@ k_angular_adj(DevSpec sp, int n_tiles, const int *__restrict__ tiles, const int 
       }
     }
     __syncthreads();                                            // T slots complete, beta slots no longer needed
-    coop_load_rows<LMAX>(sp, ti, S, Bst, sst, ng);              // S rows for D = sum_m 2C S T
+    coop_load_rows<LMAX>(sp, ti, S, Bst, ng);                   // S rows for D = sum_m 2C S T
     __syncthreads();
     if (act)
-      for (int n = w; n < sp.NA; n += ng) {
+      for (int n = w; n < sp.NA; n += nw) {
         float s[LMAX * (LMAX + 2)], t[LMAX * (LMAX + 2)];
-        gather_row<LMAX>(Bst, n, sst, ng, lane, s);
-        gather_row<LMAX>(Tst, n, sst, ng, lane, t);
+        gather_row<LMAX>(Bst, n, ng, lane, s);
+        gather_row<LMAX>(Tst, n, ng, lane, t);
         finish_D<LMAX>(sp, s, t, DS + lane * qst, n);
       }
-    coop_store_rows<LMAX>(sp, ti, Tst, sst, ng, Tn);
+    coop_store_rows<LMAX>(sp, ti, Tst, ng, Tn);
     __syncthreads();
     copy_out_rows(sp, ti, DS, qst, D);
   }
   __syncwarp();
-  float *dst = partial + (size_t)(blockIdx.x * ng + w) * nacc;
+  float *dst = partial + (size_t)(blockIdx.x * nw + w) * nacc;
   for (int o = lane; o < nacc; o += 32) dst[o] = accw[o];
 }
 
@@ -671,8 +744,9 @@ __device__ __forceinline__ void alpha_row(const DevSpec &sp, const float (&s)[LM
 
 // shared-memory floats of k_cgrad_angular: S slots | T slots (then alpha) | E' and gbar rows 2 x [32][nqa|1] | per-warp
 // scratch | per-warp accumulators | TileInfo
-__host__ __device__ inline int ang_cgrad_smem_floats(int T, int NA, int KT, int nwarps, int nqa) {
-  return 2 * ((NA * ANG_GS * (32 * nwarps + 1) + 3) & ~3) + ((2 * ANG_TILE * (nqa | 1) + 3) & ~3) + nwarps * 32 * 33 +
+__host__ __device__ inline int ang_cgrad_smem_floats(int T, int NA, int KT, int lmax, int nqa) {
+  const int nwarps = ang_groups(lmax);
+  return 2 * ((NA * ANG_GS * ang_sst(lmax) + 3) & ~3) + ((2 * ANG_TILE * (nqa | 1) + 3) & ~3) + nwarps * 32 * 33 +
          ((nwarps * T * T * NA * KT + 3) & ~3) + (int)(sizeof(TileInfo) / 4);
 }
 
@@ -683,15 +757,17 @@ k_cgrad_angular(DevSpec sp, int n_tiles, const int *__restrict__ tiles, const in
                 const float *__restrict__ S, const float *__restrict__ Tn, const float *__restrict__ A1g,
                 float *__restrict__ partial) {
   extern __shared__ __align__(128) float smem[];
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nthr = blockDim.x, ng = nthr >> 5, sst = nthr + 1;
+  constexpr int SST = AngDims<LMAX>::SST;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nthr = blockDim.x, nw = nthr >> 5, ng = ang_groups(sp.L);
+  const bool grp = w < ng;
   const int nv = sp.NA * KT, nacc = sp.T * sp.T * nv;
-  const int nqa = sp.Ndes - sp.NR, qst = nqa | 1, nslot = (sp.NA * ANG_GS * sst + 3) & ~3;
+  const int nqa = sp.Ndes - sp.NR, qst = nqa | 1, nslot = (sp.NA * ANG_GS * SST + 3) & ~3;
   float *Sst = smem;
   float *Tst = Sst + nslot;                                     // T, then alpha
   float *EG = Tst + nslot;                                      // E' rows [32][qst], gbar rows [32][qst]
   float *scr = EG + ((2 * ANG_TILE * qst + 3) & ~3) + w * 32 * 33;
-  float *accw = EG + ((2 * ANG_TILE * qst + 3) & ~3) + ng * 32 * 33 + w * nacc;
-  TileInfo *ti = (TileInfo *)(EG + ((2 * ANG_TILE * qst + 3) & ~3) + ng * 32 * 33 + ((ng * nacc + 3) & ~3));
+  float *accw = EG + ((2 * ANG_TILE * qst + 3) & ~3) + nw * 32 * 33 + w * nacc;
+  TileInfo *ti = (TileInfo *)(EG + ((2 * ANG_TILE * qst + 3) & ~3) + nw * 32 * 33 + ((nw * nacc + 3) & ~3));
   for (int o = lane; o < nacc; o += 32) accw[o] = 0.f;
   for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
     __syncthreads();                                            // the previous tile is done with every shared array
@@ -702,8 +778,8 @@ k_cgrad_angular(DevSpec sp, int n_tiles, const int *__restrict__ tiles, const in
     const int I = type_s[ti->at[0]];
     // this thread's A1 blocks are requested first: their latency hides behind the alpha rows
     const float *A1a = A1g + ((size_t)max(a, 0) * ng + w) * sp.T * KT * ANG_GS;
-    coop_load_rows<LMAX>(sp, ti, S, Sst, sst, ng);
-    coop_load_rows<LMAX>(sp, ti, Tn, Tst, sst, ng);
+    coop_load_rows<LMAX>(sp, ti, S, Sst, ng);
+    coop_load_rows<LMAX>(sp, ti, Tn, Tst, ng);
     for (int x = threadIdx.x; x < ANG_TILE * nqa; x += nthr) {  // the angular parts of the E' and gbar rows
       const int al = x / nqa, v = x - al * nqa, aa = ti->at[al];
       EG[al * qst + v] = aa >= 0 ? Ep[(size_t)aa * sp.Ndes + sp.NR + v] : 0.f;
@@ -711,20 +787,21 @@ k_cgrad_angular(DevSpec sp, int n_tiles, const int *__restrict__ tiles, const in
     }
     __syncthreads();
     if (act)
-      for (int n = w; n < sp.NA; n += ng) {                     // alpha row of (atom, n) overwrites the T slots of that row
+      for (int n = w; n < sp.NA; n += nw) {                     // alpha row of (atom, n) overwrites the T slots of that row
         float s[LMAX * (LMAX + 2)], t[LMAX * (LMAX + 2)], al[LMAX * (LMAX + 2)];
-        gather_row<LMAX>(Sst, n, sst, ng, lane, s);
-        gather_row<LMAX>(Tst, n, sst, ng, lane, t);
+        gather_row<LMAX>(Sst, n, ng, lane, s);
+        gather_row<LMAX>(Tst, n, ng, lane, t);
         alpha_row<LMAX>(sp, s, t, EG + lane * qst, EG + (ANG_TILE + lane) * qst, n, al);
+        float *Xn = Tst + n * ANG_GS * SST + lane;
 #pragma unroll
         for (int lm = 0; lm < LMAX * (LMAX + 2); ++lm)
-          if (lm / ANG_GS < ng) Tst[slot_of(n, lm, sst, lane)] = al[lm];
+          if (lm / ANG_GS < ng) Xn[(lm % ANG_GS) * SST + (lm / ANG_GS) * 32] = al[lm];
       }
     __syncthreads();
     const float *al_t = Tst + threadIdx.x;
     LaneSum<KT> ls{scr, accw, lane};
     constexpr int NPC = LaneSum<KT>::NPC;
-    for (int J = 0; J < sp.T; ++J) {
+    for (int J = 0; J < sp.T && grp; ++J) {
       float a1[KT * ANG_GS];
       if (act) ld_block<KT * ANG_GS / 8>(A1a + (size_t)J * KT * ANG_GS, a1);
       else {
@@ -742,7 +819,7 @@ k_cgrad_angular(DevSpec sp, int n_tiles, const int *__restrict__ tiles, const in
           if (act && n < sp.NA) {
             float al[ANG_GS];
 #pragma unroll
-            for (int i = 0; i < ANG_GS; ++i) al[i] = al_t[(n * ANG_GS + i) * sst];
+            for (int i = 0; i < ANG_GS; ++i) al[i] = al_t[(n * ANG_GS + i) * SST];
 #pragma unroll
             for (int k = 0; k < KT; ++k)
 #pragma unroll
@@ -755,6 +832,6 @@ k_cgrad_angular(DevSpec sp, int n_tiles, const int *__restrict__ tiles, const in
     }
   }
   __syncwarp();
-  float *dst = partial + (size_t)(blockIdx.x * ng + w) * nacc;
+  float *dst = partial + (size_t)(blockIdx.x * nw + w) * nacc;
   for (int o = lane; o < nacc; o += 32) dst[o] = accw[o];
 }

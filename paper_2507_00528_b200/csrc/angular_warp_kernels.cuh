@@ -259,6 +259,121 @@ k_angw_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restr
 }
 
 // ------------------------------------------------------------------------------------------------
+// a1, per epoch: the whole descriptor pass as contractions with the RESIDENT moments,
+//   q_n = sum_{J,k} cR[I][J][n][k] M1[J][k] (Eq.5-6),  S_nlm = sum_{J,k} cA[I][J][n][k] A1[J][k][lm] (Eq.8), q_nl (Eq.7), 4-body.
+// M1 = sum_j f_k and A1 = sum_j f_k B_lm depend on the geometry only (positions are fixed during training): the
+// pair sweeps that build them (k_radial_fwd, k_angw_fwd) run once per loaded batch.  Warp per atom (grid-stride).  The
+// atom's A1 block (T*KT*24 floats, contiguous) and M1 row arrive as full-width loads requested one atom ahead and are
+// parked in a per-warp shared buffer; the contraction reads them as 32-byte pieces shared by the lanes of a slot group,
+// lane = (n, lmg) as in the epilogues above (8 (l,m) slots of one n per lane), cA[I][J][n][.] as float4.
+// ------------------------------------------------------------------------------------------------
+__host__ __device__ inline int angw_S_smem_floats(int T, int NA, int KT, int NR, int KRp) {
+  return T * T * NA * KT + ((T * T * NR * KRp + 3) & ~3) + ANG_WARPS * (T * KT * ANGW_NLM + ((T * KRp + 7) & ~7));
+}
+template <int KT>
+__global__ void __launch_bounds__(ANG_WARPS * 32)
+k_angw_S(DevSpec sp, int N, const int *__restrict__ type_s, const float *__restrict__ theta, const float *__restrict__ M1,
+         const float *__restrict__ A1, float *__restrict__ q, float *__restrict__ S) {
+  constexpr int NP = (GNEP_MAX_SPECIES_C * KT * 3 + 31) / 32;    // 32-byte pieces of an A1 block per lane, at most
+  extern __shared__ __align__(128) float smem[];
+  const int nA = sp.T * KT * ANGW_NLM, nM = sp.T * sp.KRp;
+  float *csA = smem;                                             // [T*T*NA][KT]
+  float *csR = csA + sp.T * sp.T * sp.NA * KT;                   // [T*T*NR][KRp]
+  float *stage = csR + ((sp.T * sp.T * sp.NR * sp.KRp + 3) & ~3) + (threadIdx.x >> 5) * (nA + ((nM + 7) & ~7));
+  float *m1s = stage + nA;
+  stage_coeff(csA, theta + sp.offA, sp.T * sp.T * sp.NA, sp.KA, KT);
+  // cR transposed to [I][J][k][n]: the lanes (n) of the radial contraction read consecutive words
+  for (int x = threadIdx.x; x < sp.T * sp.T * sp.NR * sp.KRp; x += blockDim.x) {
+    const int n = x % sp.NR, k = (x / sp.NR) % sp.KRp, ij = x / (sp.NR * sp.KRp);
+    csR[x] = k < sp.KR ? theta[((size_t)ij * sp.NR + n) * sp.KR + k] : 0.f;
+  }
+  __syncthreads();
+  const int lane = threadIdx.x & 31;
+  const NLane nl = make_nlane(lane);
+  const int gw = blockIdx.x * ANG_WARPS + (threadIdx.x >> 5), nw = gridDim.x * ANG_WARPS;
+  const int pieces = nA / 8;
+  float8 pre[NP];
+  float mpre[2] = {0.f, 0.f};                                    // the M1 row: T * KRp <= 64 floats
+  int Ipre = 0;
+  auto request = [&](int a_) {
+    if (a_ >= N) return;
+    Ipre = type_s[a_];
+#pragma unroll
+    for (int v = 0; v < NP; ++v)
+      if (lane + 32 * v < pieces) pre[v] = ldg256(A1 + (size_t)a_ * nA + 8 * (lane + 32 * v));
+    if (lane < nM) mpre[0] = M1[(size_t)a_ * nM + lane];
+    if (lane + 32 < nM) mpre[1] = M1[(size_t)a_ * nM + lane + 32];
+  };
+  request(gw);
+  for (int a = gw; a < N; a += nw) {
+#pragma unroll
+    for (int v = 0; v < NP; ++v)
+      if (lane + 32 * v < pieces) {
+        *(float4 *)(stage + 8 * (lane + 32 * v)) = pre[v].lo;
+        *(float4 *)(stage + 8 * (lane + 32 * v) + 4) = pre[v].hi;
+      }
+    if (lane < nM) m1s[lane] = mpre[0];
+    if (lane + 32 < nM) m1s[lane + 32] = mpre[1];
+    const int I = Ipre;
+    __syncwarp();
+    request(a + nw);                                             // the next atom's block is in flight during this contraction
+    float *Sa = S + (size_t)a * sp.NA * ANGW_NLM;
+    float *qa = q + (size_t)a * sp.Ndes + sp.NR;
+    if (lane < sp.NR) {                                          // radial descriptors
+      float acc = 0.f;
+      const float *c = csR + (size_t)I * sp.T * sp.KRp * sp.NR + lane;
+      for (int jk = 0; jk < nM; jk += 2) {                       // (KRp is even)
+        const float2 m2 = *(const float2 *)(m1s + jk);
+        acc = fmaf(c[jk * sp.NR], m2.x, acc);
+        acc = fmaf(c[(jk + 1) * sp.NR], m2.y, acc);
+      }
+      q[(size_t)a * sp.Ndes + lane] = acc;
+    }
+    for (int nb = 0; nb < sp.NA; nb += 10) {
+      const int n = nb + nl.nq;
+      const bool on = nl.act && n < sp.NA;
+      float sv[8], qa_ = 0.f, qb_ = 0.f;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) sv[i] = 0.f;
+      if (on) {
+        for (int J = 0; J < sp.T; ++J) {
+          const float *c = csA + ((size_t)(I * sp.T + J) * sp.NA + n) * KT;
+          const float *row = stage + (size_t)J * KT * ANGW_NLM + 8 * nl.lmg;
+#pragma unroll
+          for (int k4 = 0; k4 < KT; k4 += 4) {
+            const float4 c4 = *(const float4 *)(c + k4);
+            const float cv[4] = {c4.x, c4.y, c4.z, c4.w};
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk) {
+              const float4 lo = *(const float4 *)(row + (k4 + kk) * ANGW_NLM), hi = *(const float4 *)(row + (k4 + kk) * ANGW_NLM + 4);
+              sv[0] = fmaf(cv[kk], lo.x, sv[0]); sv[1] = fmaf(cv[kk], lo.y, sv[1]); sv[2] = fmaf(cv[kk], lo.z, sv[2]);
+              sv[3] = fmaf(cv[kk], lo.w, sv[3]); sv[4] = fmaf(cv[kk], hi.x, sv[4]); sv[5] = fmaf(cv[kk], hi.y, sv[5]);
+              sv[6] = fmaf(cv[kk], hi.z, sv[6]); sv[7] = fmaf(cv[kk], hi.w, sv[7]);
+            }
+          }
+        }
+        stg256(Sa + n * ANGW_NLM + 8 * nl.lmg, make_float4(sv[0], sv[1], sv[2], sv[3]), make_float4(sv[4], sv[5], sv[6], sv[7]));
+        float w[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) w[i] = 0.5f * nl.c2[i] * sv[i] * sv[i];
+        split_sums(nl, w, qa_, qb_);
+      }
+      const float nxt = __shfl_down_sync(0xffffffffu, qa_, 1);     // the l=4 remainder held by (n, lmg 2)
+      if (on && nl.lmg == 0) {
+        qa[n] = qa_;
+        if (sp.L >= 2) qa[sp.NA + n] = qb_;
+        if (sp.use4) qa[sp.NA * sp.L + n] = GNEP_KAPPA4 * p4_value(sv + 3);
+      }
+      if (on && nl.lmg == 1) {
+        if (sp.L >= 3) qa[2 * sp.NA + n] = qa_;
+        if (sp.L >= 4) qa[3 * sp.NA + n] = qb_ + nxt;
+      }
+    }
+    __syncwarp();                                                // the stage is rewritten for the next atom
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
 // a5 (angular): A2 moments with the pair adjoint a_ij, T_nlm = c.A2, D_(n,l) = sum_m 2 C_lm S_nlm T_nlm, D_4
 // ------------------------------------------------------------------------------------------------
 template <int KT, int NQ>

@@ -59,7 +59,7 @@ struct gnep_handle {
   // path) or slot-group tiles of 32 atoms (any l_max; always used above 4)
   bool tile_path = false;
   int *tilesA = nullptr;       // slot-group path: 32 atoms of one central species per tile, sorted by neighbour counts; -1 = idle lane
-  int n_tilesA = 0, grid_adj = 0, grid_cg = 0, occ_adj = 1, occ_cg = 1;
+  int n_tilesA = 0, grid_adj = 0, grid_cg = 0, occ_adj = 1, occ_cg = 1, occ_S = 4;
   int *segA = nullptr, *atomA = nullptr;   // warp-tile path: angular list with every (atom, J) segment padded to 4 pairs
   float4 *pairA = nullptr;
   int *rowAu = nullptr, *segAu = nullptr, *atomAu = nullptr, *revAu = nullptr;   // angular list
@@ -162,14 +162,16 @@ void free_batch(gnep_handle *h) {
 
 // ---- dynamic shared memory sizes (bytes) --------------------------------------------------------
 size_t smem_radial(const DevSpec &d) { return sizeof(float) * (d.T * d.T * d.NR * d.KRp); }
-int ang_warps(const DevSpec &d) { return ang_groups(d.L); }   // warps per CTA of the moment kernels = slot groups of the model
-size_t smem_ang_fwd(const DevSpec &d) { return sizeof(float) * ang_fwd_smem_floats(d.T, d.NA, d.KAp, ang_warps(d), d.Ndes - d.NR); }
+int ang_lmax(const DevSpec &d) { return d.L <= 4 ? 4 : 8; }               // harmonics instantiation of the slot-group kernels
+int ang_warps(const DevSpec &d) { return ang_groups(ang_lmax(d)); }       // warps per CTA (the model uses ang_groups(L) slot groups)
+size_t smem_ang_fwd(const DevSpec &d) { return sizeof(float) * ang_fwd_smem_floats(d.T, d.NA, d.KAp, ang_lmax(d), d.Ndes - d.NR); }
 size_t smem_ang_force(const DevSpec &d) { return sizeof(float) * (((d.T * d.T * d.NA * d.KAp + 3) & ~3) + FRC_WARPS * FRC_TA * d.NA * d.nlmS); }
-size_t smem_ang_adj(const DevSpec &d) { return sizeof(float) * ang_adj_smem_floats(d.T, d.NA, d.KAp, ang_warps(d), d.Ndes - d.NR); }
-size_t smem_cgrad_ang(const DevSpec &d) { return sizeof(float) * ang_cgrad_smem_floats(d.T, d.NA, d.KAp, ang_warps(d), d.Ndes - d.NR); }
+size_t smem_ang_adj(const DevSpec &d) { return sizeof(float) * ang_adj_smem_floats(d.T, d.NA, d.KAp, ang_lmax(d), d.Ndes - d.NR); }
+size_t smem_cgrad_ang(const DevSpec &d) { return sizeof(float) * ang_cgrad_smem_floats(d.T, d.NA, d.KAp, ang_lmax(d), d.Ndes - d.NR); }
 size_t smem_angw_fwd(const DevSpec &d) {
   return sizeof(float) * (d.T * d.T * d.KAp * ANG_NQ + ANG_WARPS * ((d.KAp + ANGW_NLM) * ANG_LD + d.T * d.KAp * ANGW_NLM + ANG_NQ * ANGW_NLM + ANG_SEGS));
 }
+size_t smem_angw_S(const DevSpec &d) { return sizeof(float) * (size_t)angw_S_smem_floats(d.T, d.NA, d.KAp, d.NR, d.KRp); }
 size_t smem_angw_adj(const DevSpec &d) {
   return sizeof(float) * (d.T * d.T * d.KAp * ANG_NQ + ANG_WARPS * ((2 * d.KAp + 2 * ANGW_NLM) * ANG_LD + d.T * d.KAp * ANGW_NLM + ANG_NQ * ANGW_NLM + ANG_SEGS));
 }
@@ -192,7 +194,8 @@ int set_smem(gnep_handle *h, K kernel, size_t bytes) {
 
 int configure_kernels(gnep_handle *h) {
   const DevSpec &d = h->ds;
-  DISPATCH_KT(d.KRp, RET_IF(set_smem(h, k_radial_fwd<KT>, smem_radial(d))); RET_IF(set_smem(h, k_radial_adj<KT>, smem_radial(d))));
+  DISPATCH_KT(d.KRp, RET_IF(set_smem(h, k_radial_fwd<KT>, smem_radial(d))); RET_IF(set_smem(h, k_radial_adj<KT>, smem_radial(d)));
+              RET_IF(set_smem(h, k_radial_q<KT>, smem_radial(d))));
   DISPATCH_ANG(d, auto kf = k_angular_fwd<KT, LMAX>; auto ka = k_angular_adj<KT, LMAX>; auto kc = k_cgrad_angular<KT, LMAX>;
                auto kp = k_angular_force<KT, LMAX>;
                RET_IF(set_smem(h, kf, smem_ang_fwd(d))); RET_IF(set_smem(h, ka, smem_ang_adj(d)));
@@ -204,7 +207,10 @@ int configure_kernels(gnep_handle *h) {
                CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kc, 32 * ang_warps(d), smem_cgrad_ang(d)));
                h->occ_cg = std::max(occ, 1));
   if (!h->tile_path) {
-    DISPATCH_KA(d.KAp, RET_IF(set_smem(h, k_angw_cgrad<KT>, smem_angw_cgrad(d)));
+    DISPATCH_KA(d.KAp, RET_IF(set_smem(h, k_angw_cgrad<KT>, smem_angw_cgrad(d))); RET_IF(set_smem(h, k_angw_S<KT>, smem_angw_S(d)));
+                int occ = 0;
+                CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_angw_S<KT>, ANG_WARPS * 32, smem_angw_S(d)));
+                h->occ_S = std::max(occ, 1);
                 DISPATCH_NQ(d.NA, auto kf = k_angw_fwd<KT, NQ>; auto ka = k_angw_adj<KT, NQ>; RET_IF(set_smem(h, kf, smem_angw_fwd(d)));
                             RET_IF(set_smem(h, ka, smem_angw_adj(d)))));
   }
@@ -256,13 +262,27 @@ inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
   } while (0)
 
 // ---- the forward half: descriptors, network, forces, per-structure sums (rows a1-a4) --------------
-int enqueue_descriptors(gnep_handle *h) {
+// Geometry-only moments of the resident batch: M1[J][k] = sum_j f_k(d_ij) and, on the warp-tile path,
+// A1[J][k][lm] = sum_j f_k B_lm.  They do not depend on theta and positions are fixed during training, so the pair
+// sweeps that build them run ONCE, at the end of gnep_load_batch; the epoch's descriptor pass contracts them with c.
+int enqueue_geometry_moments(gnep_handle *h) {
   const DevSpec &d = h->ds;
   DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_fwd<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, smem_radial(d), d, h->N, h->type_s, h->segR, h->pairR, h->theta, h->q, h->M1));
-  mark(h, "a1_radial_descriptor");
   if (!h->tile_path) {
     DISPATCH_KA(d.KAp, DISPATCH_NQ(d.NA, auto kf = k_angw_fwd<KT, NQ>; LAUNCH(h, kf, cdiv(h->N, ANG_WARPS * ANG_TA), ANG_WARPS * 32, smem_angw_fwd(d), d, h->N, h->type_s, h->segA, h->pairA, h->theta, h->q, h->Sn, h->A1)));
-  } else
+  }
+  return GNEP_OK;
+}
+
+int enqueue_descriptors(gnep_handle *h) {
+  const DevSpec &d = h->ds;
+  if (!h->tile_path) {   // one kernel: radial and angular contractions with the resident moments
+    DISPATCH_KA(d.KAp, LAUNCH(h, k_angw_S<KT>, std::max(1, std::min(cdiv(h->N, ANG_WARPS), h->occ_S * h->num_sms)), ANG_WARPS * 32, smem_angw_S(d), d, h->N, h->type_s, h->theta, h->M1, h->A1, h->q, h->Sn));
+    mark(h, "a1_descriptor_contraction");
+    return GNEP_OK;
+  }
+  DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_q<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, smem_radial(d), d, h->N, h->type_s, h->theta, h->M1, h->q));
+  mark(h, "a1_radial_descriptor");
   DISPATCH_ANG(d, auto kf = k_angular_fwd<KT, LMAX>; LAUNCH(h, kf, h->n_tilesA, 32 * ang_warps(d), smem_ang_fwd(d), d, h->n_tilesA, h->tilesA, h->type_s, h->segAu, h->pairAu, h->theta, h->q, h->Sn, h->A1));
   mark(h, "a1_angular_descriptor");
   return GNEP_OK;
@@ -825,7 +845,7 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     const size_t n = N;
     const size_t npad = n + GW_PAD_ROWS;   // k_gradw_tc bulk-copies whole windows of rows: zeroed rows past the end
     BA(h->q, npad * d.Ndes); BA(h->Sn, n * d.NA * d.nlmS); BA(h->x, npad * d.NnS); BA(h->Ei, n); BA(h->Ep, n * d.Ndes);
-    BA(h->etil, n * T * d.KRp); BA(h->M1, n * T * d.KRp); BA(h->M2, n * T * d.KRp); BA(h->D, npad * d.Ndes); BA(h->Tn, n * d.NA * d.nlmS); BA(h->Beta, n * d.NA * d.nlmS); BA(h->A1, h->tile_path ? n * ang_warps(d) * T * d.KAp * ANG_GS : n * T * d.KAp * ANGW_NLM);
+    BA(h->etil, n * T * d.KRp); BA(h->M1, n * T * d.KRp); BA(h->M2, n * T * d.KRp); BA(h->D, npad * d.Ndes); BA(h->Tn, n * d.NA * d.nlmS); BA(h->Beta, n * d.NA * d.nlmS); BA(h->A1, h->tile_path ? n * ang_groups(d.L) * T * d.KAp * ANG_GS : n * T * d.KAp * ANGW_NLM);
     if (!h->tile_path) BA(h->A2, n * T * d.KAp * ANGW_NLM);
     BA(h->gbar, n * d.Ndes); BA(h->pbuf, npad * d.NnS); BA(h->eat, npad); BA(h->Wat, n * 6);
     BA(h->Fat, n); BA(h->fpair, h->nA); BA(h->u, n);
@@ -845,6 +865,7 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
 #undef BA
 #undef CKT
     h->loaded = true;
+    if (N > 0) { RET_IF(enqueue_geometry_moments(h)); RET_IF(check_launch(h)); }
     RET_IF(gnep_set_weights(h, nullptr, nullptr, nullptr, 0));
     return gnep_set_targets(h, Eref, Fref, Wref, is_device);
   } catch (const std::bad_alloc &) {

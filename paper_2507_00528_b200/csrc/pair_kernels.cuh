@@ -5,7 +5,9 @@
 // W_i), so a thread that walks its own row needs no cross-lane reduction at all, every lane is busy (rows of
 // neighbouring atoms have nearly equal lengths) and the per-pair work is the ~70-110 instructions of the basis
 // functions.  The 16-byte pair loads of a warp touch 32 different rows: each 32-byte sector is fetched once and its
-// second half is an L1 hit in the next iteration.
+// second half is an L1 hit in the next iteration.  (Handing the atoms to the threads sorted by row length, so that the
+// rows of a warp end together, was measured and dropped: a global sort loses the locality of the gathers, +60 % on the
+// force sweep, and a sort inside each 128-atom window still costs 2-10 %: the lanes' rows are no longer adjacent.)
 #pragma once
 #include "common.cuh"
 
@@ -141,6 +143,21 @@ k_radial_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__res
              for (int k = 1; k < KT; ++k) acc[k] = fmaf(hfc, Tk[k], acc[k]);
            });
   radial_contract<KT>(sp, cs, type_s[a], Mrow, q + (size_t)a * sp.Ndes);
+}
+
+// a1 (radial), per epoch: q_n = sum_{J,k} cR[I][J][n][k] M1[J][k] from the resident moments.  M1 depends on the geometry
+// only (positions are fixed during training), so the pair sweep above runs once per loaded batch.
+template <int KT>
+__global__ void __launch_bounds__(RAD_THREADS)
+k_radial_q(DevSpec sp, int N, const int *__restrict__ type_s, const float *__restrict__ theta, const float *__restrict__ M1,
+           float *__restrict__ q) {
+  extern __shared__ __align__(128) float smem[];
+  float *cs = smem;                                          // [T*T*NR][KT]
+  stage_coeff(cs, theta, sp.T * sp.T * sp.NR, sp.KR, KT);
+  __syncthreads();
+  const int a = blockIdx.x * RAD_THREADS + threadIdx.x;
+  if (a >= N) return;
+  radial_contract<KT>(sp, cs, type_s[a], M1 + (size_t)a * sp.T * KT, q + (size_t)a * sp.Ndes);
 }
 
 // ------------------------------------------------------------------------------------------------

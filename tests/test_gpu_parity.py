@@ -162,7 +162,7 @@ def test_l_max_5_three_species_no_many_body():
 
 def test_5body_with_l_max_4_and_slot_group_mapping_for_config3():
     """The 5-body term routes l_max <= 4 models through the slot-group kernels too (config-3 sizes, 4 groups)."""
-    _check_all(3, 4, adam_steps=2, spec_over={"use_5body": True}, floor=1e-5)   # (4 structures: a noisier sample than config 3)
+    _check_all(3, 4, adam_steps=2, spec_over={"use_5body": True, "n_neurons": 40}, floor=1e-5)   # (4 structures: a noisier sample than config 3)
 
 
 def test_two_live_handles_with_different_specs():
