@@ -268,108 +268,140 @@ k_angw_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restr
 // lane = (n, lmg) as in the epilogues above (8 (l,m) slots of one n per lane), cA[I][J][n][.] as float4.
 // ------------------------------------------------------------------------------------------------
 __host__ __device__ inline int angw_S_smem_floats(int T, int NA, int KT, int NR, int KRp) {
-  return T * T * NA * KT + ((T * T * NR * KRp + 3) & ~3) + ANG_WARPS * (T * KT * ANGW_NLM + ((T * KRp + 7) & ~7));
+  return T * T * NA * KT + ((T * T * NR * KRp + 3) & ~3) + ANG_WARPS * 2 * (T * KT * ANGW_NLM + ((T * KRp + 7) & ~7));
 }
-template <int KT>
-__global__ void __launch_bounds__(ANG_WARPS * 32)
+// Two atoms per warp and iteration: lanes 0..14 work on the first, 16..30 on the second; within a half lane = (n pair, lmg):
+// two functions n and 8 (l,m) slots each, so that one 32-byte piece of an A1 row feeds 16 FMAs.
+template <int KT, int TMAX>
+__global__ void __launch_bounds__(ANG_WARPS * 32, TMAX <= 2 ? 4 : 2)
 k_angw_S(DevSpec sp, int N, const int *__restrict__ type_s, const float *__restrict__ theta, const float *__restrict__ M1,
          const float *__restrict__ A1, float *__restrict__ q, float *__restrict__ S) {
-  constexpr int NP = (GNEP_MAX_SPECIES_C * KT * 3 + 31) / 32;    // 32-byte pieces of an A1 block per lane, at most
+  constexpr int NP = (2 * TMAX * KT * 3 + 31) / 32;                // 32-byte pieces of two A1 blocks per lane (T <= TMAX species)
   extern __shared__ __align__(128) float smem[];
-  const int nA = sp.T * KT * ANGW_NLM, nM = sp.T * sp.KRp;
+  const int nA = sp.T * KT * ANGW_NLM, nM = sp.T * sp.KRp, nMs = (nM + 7) & ~7;
   float *csA = smem;                                             // [T*T*NA][KT]
-  float *csR = csA + sp.T * sp.T * sp.NA * KT;                   // [T*T*NR][KRp]
-  float *stage = csR + ((sp.T * sp.T * sp.NR * sp.KRp + 3) & ~3) + (threadIdx.x >> 5) * (nA + ((nM + 7) & ~7));
-  float *m1s = stage + nA;
+  float *csR = csA + sp.T * sp.T * sp.NA * KT;                   // [T*T][KRp][NR] (transposed: lanes n read consecutive words)
+  float *stage = csR + ((sp.T * sp.T * sp.NR * sp.KRp + 3) & ~3) + (threadIdx.x >> 5) * 2 * (nA + nMs);   // two A1 blocks
+  float *m1s = stage + 2 * nA;                                   // two M1 rows
   stage_coeff(csA, theta + sp.offA, sp.T * sp.T * sp.NA, sp.KA, KT);
-  // cR transposed to [I][J][k][n]: the lanes (n) of the radial contraction read consecutive words
   for (int x = threadIdx.x; x < sp.T * sp.T * sp.NR * sp.KRp; x += blockDim.x) {
     const int n = x % sp.NR, k = (x / sp.NR) % sp.KRp, ij = x / (sp.NR * sp.KRp);
     csR[x] = k < sp.KR ? theta[((size_t)ij * sp.NR + n) * sp.KR + k] : 0.f;
   }
   __syncthreads();
-  const int lane = threadIdx.x & 31;
-  const NLane nl = make_nlane(lane);
+  const int lane = threadIdx.x & 31, half = lane >> 4, hl = lane & 15;
+  const int nq = hl / 3, lmg = hl - 3 * nq;                      // n pair 0..4 (hl 15 idles), slot group
+  const bool act = hl < 15;
+  float c2[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) c2[i] = c_C2[8 * (lmg < 3 ? lmg : 0) + i];
+  const int split = lmg == 0 ? 3 : lmg == 1 ? 7 : 8;             // slots below `split` belong to the lane's first l
   const int gw = blockIdx.x * ANG_WARPS + (threadIdx.x >> 5), nw = gridDim.x * ANG_WARPS;
-  const int pieces = nA / 8;
+  const int pieces = nA / 8;                                     // of ONE block
   float8 pre[NP];
-  float mpre[2] = {0.f, 0.f};                                    // the M1 row: T * KRp <= 64 floats
+  constexpr int NMP = TMAX <= 2 ? 2 : 4;
+  float mpre[NMP];                                               // two M1 rows of T * KRp <= 16 TMAX floats
+#pragma unroll
+  for (int v = 0; v < NMP; ++v) mpre[v] = 0.f;
   int Ipre = 0;
-  auto request = [&](int a_) {
-    if (a_ >= N) return;
-    Ipre = type_s[a_];
+  // the pair of atoms (2 it, 2 it + 1): their A1 blocks are adjacent in memory, 2 * pieces pieces in all
+  auto request = [&](int it) {
+    const int a0 = 2 * it;
+    if (a0 >= N) return;
+    const int np2 = (a0 + 1 < N ? 2 : 1) * pieces;
+    Ipre = type_s[min(a0 + half, N - 1)];
 #pragma unroll
     for (int v = 0; v < NP; ++v)
-      if (lane + 32 * v < pieces) pre[v] = ldg256(A1 + (size_t)a_ * nA + 8 * (lane + 32 * v));
-    if (lane < nM) mpre[0] = M1[(size_t)a_ * nM + lane];
-    if (lane + 32 < nM) mpre[1] = M1[(size_t)a_ * nM + lane + 32];
+      if (lane + 32 * v < np2) pre[v] = ldg256(A1 + (size_t)a0 * nA + 8 * (lane + 32 * v));
+    const int nm2 = (a0 + 1 < N ? 2 : 1) * nM;
+#pragma unroll
+    for (int v = 0; v < NMP; ++v)
+      if (lane + 32 * v < nm2) mpre[v] = M1[(size_t)a0 * nM + lane + 32 * v];
   };
+  const int n_it = (N + 1) >> 1;
   request(gw);
-  for (int a = gw; a < N; a += nw) {
+  for (int it = gw; it < n_it; it += nw) {
+    const int np2 = (2 * it + 1 < N ? 2 : 1) * pieces, nm2 = (2 * it + 1 < N ? 2 : 1) * nM;
 #pragma unroll
     for (int v = 0; v < NP; ++v)
-      if (lane + 32 * v < pieces) {
+      if (lane + 32 * v < np2) {
         *(float4 *)(stage + 8 * (lane + 32 * v)) = pre[v].lo;
         *(float4 *)(stage + 8 * (lane + 32 * v) + 4) = pre[v].hi;
       }
-    if (lane < nM) m1s[lane] = mpre[0];
-    if (lane + 32 < nM) m1s[lane + 32] = mpre[1];
+#pragma unroll
+    for (int v = 0; v < NMP; ++v) {
+      const int x = lane + 32 * v;                               // (the two rows are parked nMs apart)
+      if (x < nm2) m1s[(x >= nM ? nMs - nM : 0) + x] = mpre[v];
+    }
     const int I = Ipre;
     __syncwarp();
-    request(a + nw);                                             // the next atom's block is in flight during this contraction
+    request(it + nw);                                            // the next pair's blocks are in flight during this contraction
+    const int a = 2 * it + half;
+    const bool on_a = a < N;
     float *Sa = S + (size_t)a * sp.NA * ANGW_NLM;
     float *qa = q + (size_t)a * sp.Ndes + sp.NR;
-    if (lane < sp.NR) {                                          // radial descriptors
+    if (on_a && hl < sp.NR) {                                    // radial descriptors: lane = n (NR <= 16)
       float acc = 0.f;
-      const float *c = csR + (size_t)I * sp.T * sp.KRp * sp.NR + lane;
+      const float *c = csR + (size_t)I * sp.T * sp.KRp * sp.NR + hl;
+      const float *m = m1s + half * nMs;
       for (int jk = 0; jk < nM; jk += 2) {                       // (KRp is even)
-        const float2 m2 = *(const float2 *)(m1s + jk);
+        const float2 m2 = *(const float2 *)(m + jk);
         acc = fmaf(c[jk * sp.NR], m2.x, acc);
         acc = fmaf(c[(jk + 1) * sp.NR], m2.y, acc);
       }
-      q[(size_t)a * sp.Ndes + lane] = acc;
+      q[(size_t)a * sp.Ndes + hl] = acc;
     }
     for (int nb = 0; nb < sp.NA; nb += 10) {
-      const int n = nb + nl.nq;
-      const bool on = nl.act && n < sp.NA;
-      float sv[8], qa_ = 0.f, qb_ = 0.f;
+      const int n0 = nb + 2 * nq;
+      const bool on0 = on_a && act && n0 < sp.NA, on1 = on0 && n0 + 1 < sp.NA;
+      float sv[2][8];
 #pragma unroll
-      for (int i = 0; i < 8; ++i) sv[i] = 0.f;
-      if (on) {
+      for (int i = 0; i < 8; ++i) { sv[0][i] = 0.f; sv[1][i] = 0.f; }
+      if (on0) {
         for (int J = 0; J < sp.T; ++J) {
-          const float *c = csA + ((size_t)(I * sp.T + J) * sp.NA + n) * KT;
-          const float *row = stage + (size_t)J * KT * ANGW_NLM + 8 * nl.lmg;
+          const float *c = csA + ((size_t)(I * sp.T + J) * sp.NA + n0) * KT;
+          const float *c1 = on1 ? c + KT : c;
+          const float *row = stage + (size_t)half * nA + (size_t)J * KT * ANGW_NLM + 8 * lmg;
 #pragma unroll
           for (int k4 = 0; k4 < KT; k4 += 4) {
-            const float4 c4 = *(const float4 *)(c + k4);
-            const float cv[4] = {c4.x, c4.y, c4.z, c4.w};
+            const float4 ca = *(const float4 *)(c + k4), cb = *(const float4 *)(c1 + k4);
+            const float cv0[4] = {ca.x, ca.y, ca.z, ca.w}, cv1[4] = {cb.x, cb.y, cb.z, cb.w};
 #pragma unroll
             for (int kk = 0; kk < 4; ++kk) {
               const float4 lo = *(const float4 *)(row + (k4 + kk) * ANGW_NLM), hi = *(const float4 *)(row + (k4 + kk) * ANGW_NLM + 4);
-              sv[0] = fmaf(cv[kk], lo.x, sv[0]); sv[1] = fmaf(cv[kk], lo.y, sv[1]); sv[2] = fmaf(cv[kk], lo.z, sv[2]);
-              sv[3] = fmaf(cv[kk], lo.w, sv[3]); sv[4] = fmaf(cv[kk], hi.x, sv[4]); sv[5] = fmaf(cv[kk], hi.y, sv[5]);
-              sv[6] = fmaf(cv[kk], hi.z, sv[6]); sv[7] = fmaf(cv[kk], hi.w, sv[7]);
+              const float av[8] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
+#pragma unroll
+              for (int i = 0; i < 8; ++i) { sv[0][i] = fmaf(cv0[kk], av[i], sv[0][i]); sv[1][i] = fmaf(cv1[kk], av[i], sv[1][i]); }
             }
           }
         }
-        stg256(Sa + n * ANGW_NLM + 8 * nl.lmg, make_float4(sv[0], sv[1], sv[2], sv[3]), make_float4(sv[4], sv[5], sv[6], sv[7]));
-        float w[8];
+      }
 #pragma unroll
-        for (int i = 0; i < 8; ++i) w[i] = 0.5f * nl.c2[i] * sv[i] * sv[i];
-        split_sums(nl, w, qa_, qb_);
-      }
-      const float nxt = __shfl_down_sync(0xffffffffu, qa_, 1);     // the l=4 remainder held by (n, lmg 2)
-      if (on && nl.lmg == 0) {
-        qa[n] = qa_;
-        if (sp.L >= 2) qa[sp.NA + n] = qb_;
-        if (sp.use4) qa[sp.NA * sp.L + n] = GNEP_KAPPA4 * p4_value(sv + 3);
-      }
-      if (on && nl.lmg == 1) {
-        if (sp.L >= 3) qa[2 * sp.NA + n] = qa_;
-        if (sp.L >= 4) qa[3 * sp.NA + n] = qb_ + nxt;
+      for (int e = 0; e < 2; ++e) {
+        const int n = n0 + e;
+        const bool on = e == 0 ? on0 : on1;
+        float qa_ = 0.f, qb_ = 0.f;
+        if (on) {
+          stg256(Sa + n * ANGW_NLM + 8 * lmg, make_float4(sv[e][0], sv[e][1], sv[e][2], sv[e][3]), make_float4(sv[e][4], sv[e][5], sv[e][6], sv[e][7]));
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const float w = 0.5f * c2[i] * sv[e][i] * sv[e][i];
+            if (i < split) qa_ += w; else qb_ += w;
+          }
+        }
+        const float nxt = __shfl_down_sync(0xffffffffu, qa_, 1);   // the l=4 remainder held by (n, lmg 2)
+        if (on && lmg == 0) {
+          qa[n] = qa_;
+          if (sp.L >= 2) qa[sp.NA + n] = qb_;
+          if (sp.use4) qa[sp.NA * sp.L + n] = GNEP_KAPPA4 * p4_value(sv[e] + 3);
+        }
+        if (on && lmg == 1) {
+          if (sp.L >= 3) qa[2 * sp.NA + n] = qa_;
+          if (sp.L >= 4) qa[3 * sp.NA + n] = qb_ + nxt;
+        }
       }
     }
-    __syncwarp();                                                // the stage is rewritten for the next atom
+    __syncwarp();                                                // the stage is rewritten for the next pair
   }
 }
 

@@ -140,6 +140,9 @@ int padded_basis_ang(int K) { return K <= 4 ? 4 : K <= 8 ? 8 : 16; }
 #define DISPATCH_NQ(NA_, ...)                                   \
   if ((NA_) <= 10) { constexpr int NQ = 10; __VA_ARGS__; }      \
   else { constexpr int NQ = 16; __VA_ARGS__; }
+#define DISPATCH_TMAX(T_, ...)                                  \
+  if ((T_) <= 2) { constexpr int TMAX = 2; __VA_ARGS__; }       \
+  else { constexpr int TMAX = 4; __VA_ARGS__; }
 #define DISPATCH_ANG(d_, ...)                                               \
   if ((d_).L <= 4) { constexpr int LMAX = 4; DISPATCH_KA((d_).KAp, __VA_ARGS__) } \
   else { constexpr int LMAX = 8; DISPATCH_KA((d_).KAp, __VA_ARGS__) }
@@ -207,10 +210,10 @@ int configure_kernels(gnep_handle *h) {
                CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kc, 32 * ang_warps(d), smem_cgrad_ang(d)));
                h->occ_cg = std::max(occ, 1));
   if (!h->tile_path) {
-    DISPATCH_KA(d.KAp, RET_IF(set_smem(h, k_angw_cgrad<KT>, smem_angw_cgrad(d))); RET_IF(set_smem(h, k_angw_S<KT>, smem_angw_S(d)));
-                int occ = 0;
-                CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_angw_S<KT>, ANG_WARPS * 32, smem_angw_S(d)));
-                h->occ_S = std::max(occ, 1);
+    DISPATCH_KA(d.KAp, RET_IF(set_smem(h, k_angw_cgrad<KT>, smem_angw_cgrad(d))); DISPATCH_TMAX(d.T, auto ks = k_angw_S<KT, TMAX>; RET_IF(set_smem(h, ks, smem_angw_S(d)));
+                              int occ = 0;
+                              CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, ks, ANG_WARPS * 32, smem_angw_S(d)));
+                              h->occ_S = std::max(occ, 1));
                 DISPATCH_NQ(d.NA, auto kf = k_angw_fwd<KT, NQ>; auto ka = k_angw_adj<KT, NQ>; RET_IF(set_smem(h, kf, smem_angw_fwd(d)));
                             RET_IF(set_smem(h, ka, smem_angw_adj(d)))));
   }
@@ -277,7 +280,7 @@ int enqueue_geometry_moments(gnep_handle *h) {
 int enqueue_descriptors(gnep_handle *h) {
   const DevSpec &d = h->ds;
   if (!h->tile_path) {   // one kernel: radial and angular contractions with the resident moments
-    DISPATCH_KA(d.KAp, LAUNCH(h, k_angw_S<KT>, std::max(1, std::min(cdiv(h->N, ANG_WARPS), h->occ_S * h->num_sms)), ANG_WARPS * 32, smem_angw_S(d), d, h->N, h->type_s, h->theta, h->M1, h->A1, h->q, h->Sn));
+    DISPATCH_KA(d.KAp, DISPATCH_TMAX(d.T, auto ks = k_angw_S<KT, TMAX>; LAUNCH(h, ks, std::max(1, std::min(cdiv(h->N, 2 * ANG_WARPS), h->occ_S * h->num_sms)), ANG_WARPS * 32, smem_angw_S(d), d, h->N, h->type_s, h->theta, h->M1, h->A1, h->q, h->Sn)));
     mark(h, "a1_descriptor_contraction");
     return GNEP_OK;
   }
