@@ -1,4 +1,4 @@
-// net_kernels.cuh -- the "K = atoms" contraction of the radial coefficient gradient (row a7-radial of DESIGN.md).
+// cgrad_radial.cuh -- the radial expansion-coefficient gradient (row a7 of DESIGN.md) as a K = atoms contraction.
 // The network itself (rows a2, a6) lives in net_tc_kernels.cuh (tensor cores).
 #pragma once
 #include "common.cuh"

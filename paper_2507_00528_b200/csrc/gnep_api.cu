@@ -12,7 +12,7 @@
 
 #include "common.cuh"
 #include "neighbor.cuh"
-#include "net_kernels.cuh"   // includes net_tc_kernels.cuh (tensor-core network)
+#include "cgrad_radial.cuh"   // includes net_tc_kernels.cuh (tensor-core network)
 #include "pair_kernels.cuh"
 #include "angular_kernels.cuh"
 #include "angular_warp_kernels.cuh"
