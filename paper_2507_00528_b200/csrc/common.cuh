@@ -12,7 +12,7 @@
 struct DevSpec {
   int T, NR, KR, NA, KA, L, use4, use5, Nn, Ndes, P;
   int nlmS;                   // row stride of the per-atom (l,m) arrays S, T, beta, A1: 24 for l_max <= 4, 84 above
-  int NnS;                    // row stride of the hidden-layer buffers x, p: Nn padded to 8 (32-byte rows, 256-bit accesses)
+  int NnS;                    // neurons per atom in the hidden-layer buffers x, p: Nn padded to 16 (XT layout, net_tc_kernels.cuh)
   int KRp, KAp;               // basis sizes padded to the template size of the pair kernels
   int offA, offNet, netSize;  // parameter-vector offsets (include/gnep.h layout)
   int ldW;                    // padded shared-memory row stride of W0 (odd -> conflict-free)

@@ -438,7 +438,7 @@ int gnep_create(const gnep_model_spec *spec, void *cuda_stream, gnep_handle **ou
   h->device = dev; h->num_sms = prop.multiProcessorCount;
   DevSpec &d = h->ds;
   d.T = s.n_species; d.NR = s.n_radial; d.KR = s.n_basis_radial; d.NA = s.n_angular; d.KA = s.n_basis_angular;
-  d.L = s.l_max; d.use4 = s.use_4body ? 1 : 0; d.use5 = s.use_5body ? 1 : 0; d.Nn = s.n_neurons; d.NnS = (d.Nn + 7) & ~7;
+  d.L = s.l_max; d.use4 = s.use_4body ? 1 : 0; d.use5 = s.use_5body ? 1 : 0; d.Nn = s.n_neurons; d.NnS = (d.Nn + 15) & ~15;
   d.Ndes = d.NR + d.NA * d.L + (d.use4 ? d.NA : 0) + (d.use5 ? d.NA : 0);
   d.nlmS = d.L <= 4 ? 24 : 88;   // 24 / 80 slots; rows are whole 32-byte pieces
   d.KRp = padded_basis(d.KR); d.KAp = padded_basis_ang(d.KA);
@@ -846,11 +846,12 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     h->rm.n_warps_ca = N > 0 ? (h->grid_adj + h->grid_cg) * ca_warps : 0;   // partial rows: the beta half (adjoint sweep) then the alpha half
     // ---- per-atom state ----
     const size_t n = N;
-    const size_t npad = n + GW_PAD_ROWS;   // k_gradw_tc bulk-copies whole windows of rows: zeroed rows past the end
-    BA(h->q, npad * d.Ndes); BA(h->Sn, n * d.NA * d.nlmS); BA(h->x, npad * d.NnS); BA(h->Ei, n); BA(h->Ep, n * d.Ndes);
+    const size_t npad = n + GW_PAD_ROWS;
+    const size_t nxt = (npad + 127) / 128 * 128;   // x, p: whole 128-atom blocks of the XT layout (net_tc_kernels.cuh)   // k_gradw_tc bulk-copies whole windows of rows: zeroed rows past the end
+    BA(h->q, npad * d.Ndes); BA(h->Sn, n * d.NA * d.nlmS); BA(h->x, nxt * d.NnS); BA(h->Ei, n); BA(h->Ep, n * d.Ndes);
     BA(h->etil, n * T * d.KRp); BA(h->M1, n * T * d.KRp); BA(h->M2, n * T * d.KRp); BA(h->D, npad * d.Ndes); BA(h->Tn, n * d.NA * d.nlmS); BA(h->Beta, n * d.NA * d.nlmS); BA(h->A1, h->tile_path ? n * ang_groups(d.L) * T * d.KAp * ANG_GS : n * T * d.KAp * ANGW_NLM);
     if (!h->tile_path) BA(h->A2, n * T * d.KAp * ANGW_NLM);
-    BA(h->gbar, n * d.Ndes); BA(h->pbuf, npad * d.NnS); BA(h->eat, npad); BA(h->Wat, n * 6);
+    BA(h->gbar, n * d.Ndes); BA(h->pbuf, nxt * d.NnS); BA(h->eat, npad); BA(h->Wat, n * 6);
     BA(h->Fat, n); BA(h->fpair, h->nA); BA(h->u, n);
     BA(h->Es, S); BA(h->Ws, (size_t)S * 6); BA(h->parts, (size_t)S * 3); BA(h->e_s, S); BA(h->omega, (size_t)S * 6);
     BA(h->partialCR, (size_t)std::max(h->n_chunks, 1) * d.NR * T * d.KRp);
@@ -862,8 +863,8 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     CKT(cudaMemsetAsync(h->Tn, 0, sizeof(float) * n * d.NA * d.nlmS, st));
     CKT(cudaMemsetAsync(h->q + n * d.Ndes, 0, sizeof(float) * GW_PAD_ROWS * d.Ndes, st));
     CKT(cudaMemsetAsync(h->D + n * d.Ndes, 0, sizeof(float) * GW_PAD_ROWS * d.Ndes, st));
-    CKT(cudaMemsetAsync(h->x, 0, sizeof(float) * npad * d.NnS, st));
-    CKT(cudaMemsetAsync(h->pbuf, 0, sizeof(float) * npad * d.NnS, st));
+    CKT(cudaMemsetAsync(h->x, 0, sizeof(float) * nxt * d.NnS, st));
+    CKT(cudaMemsetAsync(h->pbuf, 0, sizeof(float) * nxt * d.NnS, st));
     CKT(cudaMemsetAsync(h->eat + n, 0, sizeof(float) * GW_PAD_ROWS, st));
 #undef BA
 #undef CKT

@@ -30,6 +30,16 @@ __device__ __forceinline__ int species_of_block(const int *base, int T, int b) {
 
 __host__ __device__ inline int pad_to(int x, int m) { return (x + m - 1) / m * m; }
 
+// Layout of the hidden-layer buffers x = tanh(z) and p (written by k_net_tc, read by k_net_tc<true> and k_gradw_tc):
+// blocks of 128 atoms (absolute sorted index), inside a block one [128 atoms][16 neurons] panel per chunk of 16 neurons,
+//   XT[(a >> 7)][mu >> 4][a & 127][mu & 15],   NnS = Nn padded to 16 neurons per atom.
+// A thread-per-atom access of one chunk is then 64 contiguous bytes per lane with consecutive lanes adjacent (a warp
+// moves 2 KB of consecutive memory instead of touching 32 rows 4 NnS bytes apart), and a window of 16 consecutive atoms is
+// one contiguous kilobyte per chunk for the bulk copies of k_gradw_tc.
+__host__ __device__ inline size_t xt_off(int a, int mu, int NnS) {
+  return ((size_t)(a >> 7) * (NnS >> 4) + (mu >> 4)) * 2048 + (size_t)(a & 127) * 16 + (mu & 15);
+}
+
 // padded problem sizes of the tensor-core kernels
 struct NetDims {
   int NnP;   // neurons padded to 16: N of the first contraction, K of the second
@@ -240,7 +250,7 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
     float4 xnext[4];   // backward: the x row is fetched one 16-neuron chunk ahead of its use
     if (BWD) {
 #pragma unroll
-      for (int v = 0; v < 4; v += 2) load_row8(xbuf + (size_t)a * sp.NnS, sp.NnS, 4 * v, true, true, valid, xnext[v], xnext[v + 1]);
+      for (int v = 0; v < 4; v += 2) load_row8(xbuf + xt_off(a, 0, sp.NnS), 16, 4 * v, true, true, valid, xnext[v], xnext[v + 1]);
     }
     if (!mbar_wait(bar1, parity)) __trap();
     fence_after_sync();
@@ -269,20 +279,20 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
           split_fast(w1 * (1.f - xv * xv), ch[i], cl[i]);
         }
         if (valid) {
-          float *xr = xbuf + (size_t)a * sp.NnS;
+          float *xr = xbuf + xt_off(a, m0, sp.NnS);
 #pragma unroll
           for (int v = 0; v < 2; ++v)
-            store_row8(xr, sp.NnS, m0 + 8 * v, true, true, make_float4(xs[8 * v], xs[8 * v + 1], xs[8 * v + 2], xs[8 * v + 3]),
+            store_row8(xr, 16, 8 * v, true, true, make_float4(xs[8 * v], xs[8 * v + 1], xs[8 * v + 2], xs[8 * v + 3]),
                        make_float4(xs[8 * v + 4], xs[8 * v + 5], xs[8 * v + 6], xs[8 * v + 7]));
         }
       } else {
-        const float *xr = xbuf + (size_t)a * sp.NnS;
-        float *pr = pbuf + (size_t)a * sp.NnS;
+        const float *xr = xbuf + xt_off(a, m0 + 16, sp.NnS);   // the next chunk's panel
+        float *pr = pbuf + xt_off(a, m0, sp.NnS);
         float4 xcur[4];
 #pragma unroll
         for (int v = 0; v < 4; ++v) xcur[v] = xnext[v];
 #pragma unroll
-        for (int v = 0; v < 4; v += 2) load_row8(xr, sp.NnS, m0 + 16 + 4 * v, true, true, valid && m0 + 16 < NnP, xnext[v], xnext[v + 1]);
+        for (int v = 0; v < 4; v += 2) load_row8(xr, 16, 4 * v, true, true, valid && m0 + 16 < NnP, xnext[v], xnext[v + 1]);
 #pragma unroll
         for (int v = 0; v < 4; ++v) {
           const float4 x4 = xcur[v];
@@ -296,7 +306,7 @@ k_net_tc(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float
         if (valid) {
 #pragma unroll
           for (int v = 0; v < 2; ++v)
-            store_row8(pr, sp.NnS, m0 + 8 * v, true, true, make_float4(z[8 * v], z[8 * v + 1], z[8 * v + 2], z[8 * v + 3]),
+            store_row8(pr, 16, 8 * v, true, true, make_float4(z[8 * v], z[8 * v + 1], z[8 * v + 2], z[8 * v + 3]),
                        make_float4(z[8 * v + 4], z[8 * v + 5], z[8 * v + 6], z[8 * v + 7]));
         }
       }
@@ -522,15 +532,17 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, int nraw, const float *__restrict__ theta,
     // ================= bulk-copy issuer (one thread) =================
     if ((tid & 31) == 0) {
       const uint32_t bx = (uint32_t)(GW_KS * sp.NnS * sizeof(float)), bq = (uint32_t)(GW_KS * sp.Ndes * sizeof(float));
-      const uint32_t be = (uint32_t)(GW_KS * sizeof(float));
+      const uint32_t be = (uint32_t)(GW_KS * sizeof(float)), bx16 = (uint32_t)(GW_KS * 16 * sizeof(float));
       for (int it = 0; it < nst; ++it) {
         const int rs = it % nraw, use = it / nraw;
         if (use > 0 && !mbar_wait(rempty + rs, (uint32_t)((use - 1) & 1))) __trap();
         const size_t a0 = (size_t)(w0 + it * GW_KS);
         float *rb = raw + rs * raw_fl;
         mbar_expect_tx(rfull + rs, 2 * bx + 2 * bq + be);
-        bulk_g2s(rb, x + a0 * sp.NnS, bx, rfull + rs);
-        bulk_g2s(rb + GW_KS * sp.NnS, p + a0 * sp.NnS, bx, rfull + rs);
+        for (int c = 0; c < (sp.NnS >> 4); ++c) {     // one contiguous [16 atoms][16 neurons] piece per chunk (XT layout)
+          bulk_g2s(rb + c * GW_KS * 16, x + xt_off((int)a0, 16 * c, sp.NnS), bx16, rfull + rs);
+          bulk_g2s(rb + GW_KS * sp.NnS + c * GW_KS * 16, p + xt_off((int)a0, 16 * c, sp.NnS), bx16, rfull + rs);
+        }
         bulk_g2s(rb + 2 * GW_KS * sp.NnS, q + a0 * sp.Ndes, bq, rfull + rs);
         bulk_g2s(rb + 2 * GW_KS * sp.NnS + GW_KS * sp.Ndes, D + a0 * sp.Ndes, bq, rfull + rs);
         bulk_g2s(rb + 2 * GW_KS * (sp.NnS + sp.Ndes), eat + a0, be, rfull + rs);
@@ -614,7 +626,8 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, int nraw, const float *__restrict__ theta,
       const int wl = w < nA ? w : w - nA, W = w < nA ? sp.Nn : sp.Ndes;
       const int ag = i_kind[j] ? wl / W : 0, col = i_kind[j] ? wl - ag * W : 0;
       i_ag[j] = 4 * ag;
-      r_off[j] = i_kind[j] == 1 ? 4 * ag * sp.NnS + col : 2 * GW_KS * sp.NnS + 4 * ag * W + col;
+      // raw x / p stage: [neuron chunk][16 atoms][16 neurons]; raw q / D stage: [16 atoms][N_des]
+      r_off[j] = i_kind[j] == 1 ? (col >> 4) * GW_KS * 16 + 4 * ag * 16 + (col & 15) : 2 * GW_KS * sp.NnS + 4 * ag * W + col;
       s_off[j] = i_kind[j] == 1 ? (ag * 128 + col) * 4 : 6 * tileA + (ag * NB + col) * 4;
       i_cf[j] = i_kind[j] == 1 ? w1g[col] : (i_kind[j] == 2 ? qscale[col] : 0.f);
       if (i_kind[j] == 1 && col == 0) i_kind[j] = 3;
@@ -648,8 +661,8 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, int nraw, const float *__restrict__ theta,
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
             const bool ok = whole || (i_ag[j] + i >= vlo && i_ag[j] + i < vhi);
-            const float xv = rx[i * sp.NnS];
-            const float pv = ok ? rp[i * sp.NnS] : 0.f, ev = ok ? ee[i] : 0.f;
+            const float xv = rx[i * 16];
+            const float pv = ok ? rp[i * 16] : 0.f, ev = ok ? ee[i] : 0.f;
             const float d1 = 1.f - xv * xv, d2 = -2.f * xv * d1;
             Av[i] = cf * (ev * d1 + d2 * pv);
             Bv[i] = ok ? cf * d1 : 0.f;
