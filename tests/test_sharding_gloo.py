@@ -41,11 +41,25 @@ class OracleEngine:
         self.theta = theta.copy()
         self.m = np.zeros_like(theta); self.v = np.zeros_like(theta); self.step = 0
         self.n_atoms, self.n_structs = int(a1 - a0), hi - lo
-        self.norm = (self.n_atoms, self.n_structs, 1.0)
+        self.weights = None
+        self.zjob, self.share = self.loss_norms(), 1.0
         self.grad = None
 
+    def set_weights(self, we, wf, wv):
+        self.weights = (np.asarray(we, float), np.asarray(wf, float), np.asarray(wv, float))
+        self.zjob = self.loss_norms()
+
+    def loss_norms(self):
+        """{Z_E, Z_F, Z_V} of this rank's structures (R40): sum w_e, sum w_f N_s, sum w_v."""
+        ns = np.diff(self.offsets).astype(float)
+        we, wf, wv = self.weights if self.weights is not None else (np.ones_like(ns),) * 3
+        return np.array([we.sum(), (wf * ns).sum(), wv.sum()])
+
     def set_global_norm(self, n_job, s_job, l2_share):
-        self.norm = (n_job, s_job, l2_share)
+        self.zjob, self.share = np.array([s_job, n_job, s_job], float), l2_share
+
+    def set_global_norms(self, z, l2_share):
+        self.zjob, self.share = np.asarray(z, float), l2_share
 
     def _term(self, which):
         lam = dict(lambda_e=0.0, lambda_f=0.0, lambda_v=0.0, lambda_2=0.0)
@@ -53,13 +67,14 @@ class OracleEngine:
         sp = orc.make_spec(dict(self.spec, **lam))
         ob = orc.Batch(sp, self.offsets, self.pos, self.cells, self.types)
         ob.set_refs(*self.refs)
+        if self.weights is not None:
+            ob.set_weights(*self.weights)
         t, g = orc.loss_and_grad(sp, self.theta, self.qs, ob)
         return t[0], g
 
     def loss_and_grad(self, want_terms=False, grad=None):
-        n_job, s_job, share = self.norm
-        w = dict(lambda_e=self.n_structs / s_job, lambda_f=self.n_atoms / n_job, lambda_v=self.n_structs / s_job,
-                 lambda_2=share)
+        zl, zj = self.loss_norms(), self.zjob
+        w = dict(lambda_e=zl[0] / zj[0], lambda_f=zl[1] / zj[1], lambda_v=zl[2] / zj[2], lambda_2=self.share)
         tot, g = 0.0, np.zeros_like(self.theta)
         for k, wk in w.items():
             t, gk = self._term(k)
@@ -90,7 +105,10 @@ def _case():
     return spec, sp, b, ob, theta, qs, labels
 
 
-def _rank_main(rank, world, port, out_dir):
+WEIGHTS = (np.array([1.0, 0.5, 2.0, 1.5]), np.array([2.0, 1.0, 0.0, 1.0]), np.array([1.0, 0.0, 0.0, 3.0]))
+
+
+def _rank_main(rank, world, port, out_dir, weighted=False):
     os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
@@ -98,8 +116,14 @@ def _rank_main(rank, world, port, out_dir):
         n_s = len(b["atom_offsets"]) - 1
         bounds = sharding.shard_bounds(np.diff(b["atom_offsets"]), world)
         eng = OracleEngine(spec, b, bounds[rank], bounds[rank + 1], theta, qs, labels)
-        n_job, s_job = sharding.setup_sharded(eng, dist, eng.n_atoms, eng.n_structs)
-        assert (n_job, s_job) == (int(b["atom_offsets"][-1]), n_s)
+        if weighted:
+            eng.set_weights(*[w[bounds[rank]:bounds[rank + 1]] for w in WEIGHTS])
+            z = sharding.setup_sharded_weighted(eng, dist)
+            ns = np.diff(b["atom_offsets"])
+            np.testing.assert_allclose(z, [WEIGHTS[0].sum(), (WEIGHTS[1] * ns).sum(), WEIGHTS[2].sum()], rtol=1e-14)
+        else:
+            n_job, s_job = sharding.setup_sharded(eng, dist, eng.n_atoms, eng.n_structs)
+            assert (n_job, s_job) == (int(b["atom_offsets"][-1]), n_s)
         grad = torch.empty(len(theta), dtype=torch.float32)
         part = eng.loss_and_grad(grad=grad)
         total = sharding.reduce_loss_terms(dist, [part])[0]
@@ -123,6 +147,24 @@ def test_two_rank_epoch_matches_single_process(tmp_path):
     assert abs(float(r0["loss"]) - t0[0]) <= 1e-6 * abs(t0[0])            # partial loss terms sum to the job's loss
     assert np.array_equal(r0["theta"], r1["theta"])                         # replicas stay identical
     assert np.linalg.norm(r0["grad"] - g) <= 1e-5 * np.linalg.norm(g)       # fp32 all-reduce of the partial gradients
+    assert np.linalg.norm(r0["theta"] - th) <= 1e-6 * np.linalg.norm(th)
+
+
+def test_two_rank_weighted_epoch_matches_single_process(tmp_path):
+    """Per-structure weights (R40): every rank contributes its normalisers, the job-wide ones come from one all-reduce."""
+    world, port = 2, 31500 + os.getpid() % 2000
+    mp.spawn(_rank_main, args=(world, port, str(tmp_path), True), nprocs=world, join=True)
+    spec, sp, b, ob, theta, qs, labels = _case()
+    ob.set_weights(*WEIGHTS)
+    th = theta.copy(); m = np.zeros_like(th); v = np.zeros_like(th)
+    t0, _ = orc.loss_and_grad(sp, th, qs, ob)
+    for step in (1, 2):
+        _, g = orc.loss_and_grad(sp, th, qs, ob)
+        orc.adam_step(th, m, v, g, step, LR)
+    r0 = np.load(tmp_path / "rank0.npz"); r1 = np.load(tmp_path / "rank1.npz")
+    assert abs(float(r0["loss"]) - t0[0]) <= 1e-6 * abs(t0[0])
+    assert np.array_equal(r0["theta"], r1["theta"])
+    assert np.linalg.norm(r0["grad"] - g) <= 1e-5 * np.linalg.norm(g)
     assert np.linalg.norm(r0["theta"] - th) <= 1e-6 * np.linalg.norm(th)
 
 
