@@ -647,7 +647,7 @@ __device__ __forceinline__ void force_block(const DevSpec &sp, const float *__re
 
 template <int KT, int LMAX>
 __global__ void __launch_bounds__(FRC_WARPS * 32)
-k_angular_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ segA,
+k_angular_force(DevSpec sp, int N, int ta /* atoms per warp, <= FRC_TA */, const int *__restrict__ type_s, const int *__restrict__ segA,
                 const int *__restrict__ atomA, const float4 *__restrict__ pairA, const float *__restrict__ theta,
                 const float *__restrict__ Ep, const float *__restrict__ S, float *__restrict__ Beta,
                 float4 *__restrict__ fpair) {
@@ -659,9 +659,9 @@ k_angular_force(DevSpec sp, int N, const int *__restrict__ type_s, const int *__
   stage_coeff(cs, theta + sp.offA, sp.T * sp.T * sp.NA, sp.KA, KT);
   __syncthreads();
   const int lane = threadIdx.x & 31;
-  const int a_lo = (blockIdx.x * FRC_WARPS + (threadIdx.x >> 5)) * FRC_TA;
+  const int a_lo = (blockIdx.x * FRC_WARPS + (threadIdx.x >> 5)) * ta;
   if (a_lo >= N) return;
-  const int a_hi = min(a_lo + FRC_TA, N);
+  const int a_hi = min(a_lo + ta, N);
   const int T1 = sp.T + 1;
   const int P_lo = segA[a_lo * T1], P_hi = segA[(a_hi - 1) * T1 + sp.T];
   // beta of the warp's atoms: one (atom, n) row per lane and round, into shared memory ...

@@ -116,7 +116,7 @@ __device__ __forceinline__ void xown_store(int kq, int lmq, float (&Xo)[NJ][3], 
 // ------------------------------------------------------------------------------------------------
 template <int KT, int NQ>
 __global__ void __launch_bounds__(ANG_WARPS * 32)
-k_angw_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ segA,
+k_angw_fwd(DevSpec sp, int N, int ta /* atoms per warp, <= ANG_TA */, const int *__restrict__ type_s, const int *__restrict__ segA,
               const float4 *__restrict__ pairA, const float *__restrict__ theta, float *__restrict__ q,
               float *__restrict__ S, float *__restrict__ A1) {
   constexpr int KQ = (KT + 3) / 4;      // k per lane: lane = (k quarter kq, lm eighth lmq) holds a KQ x 3 register tile
@@ -133,9 +133,9 @@ k_angw_fwd(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restr
   stage_coeff_t(ct, theta + sp.offA, sp.T, sp.NA, sp.KA, KT);
   __syncthreads();
   const int lane = threadIdx.x & 31;
-  const int a_lo = (blockIdx.x * ANG_WARPS + (threadIdx.x >> 5)) * ANG_TA;
+  const int a_lo = (blockIdx.x * ANG_WARPS + (threadIdx.x >> 5)) * ta;
   if (a_lo >= N) return;
-  const int a_hi = min(a_lo + ANG_TA, N);
+  const int a_hi = min(a_lo + ta, N);
   const int T1 = sp.T + 1;
   const int P_lo = segA[a_lo * T1], P_hi = segA[(a_hi - 1) * T1 + sp.T];
   const int kq = lane >> 3, lmq = lane & 7;
@@ -410,7 +410,7 @@ k_angw_S(DevSpec sp, int N, const int *__restrict__ type_s, const float *__restr
 // ------------------------------------------------------------------------------------------------
 template <int KT, int NQ>
 __global__ void __launch_bounds__(ANG_WARPS * 32)
-k_angw_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ struct_s,
+k_angw_adj(DevSpec sp, int N, int ta /* atoms per warp, <= ANG_TA */, const int *__restrict__ type_s, const int *__restrict__ struct_s,
               const int *__restrict__ segA, const int *__restrict__ atomA, const float4 *__restrict__ pairA,
               const float *__restrict__ theta, const float4 *__restrict__ u, const float *__restrict__ omega,
               const float *__restrict__ scales, const float *__restrict__ S, float *__restrict__ Tn,
@@ -431,9 +431,9 @@ k_angw_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restr
   stage_coeff_t(ct, theta + sp.offA, sp.T, sp.NA, sp.KA, KT);
   __syncthreads();
   const int lane = threadIdx.x & 31;
-  const int a_lo = (blockIdx.x * ANG_WARPS + (threadIdx.x >> 5)) * ANG_TA;
+  const int a_lo = (blockIdx.x * ANG_WARPS + (threadIdx.x >> 5)) * ta;
   if (a_lo >= N) return;
-  const int a_hi = min(a_lo + ANG_TA, N);
+  const int a_hi = min(a_lo + ta, N);
   const int T1 = sp.T + 1;
   const int P_lo = segA[a_lo * T1], P_hi = segA[(a_hi - 1) * T1 + sp.T];
   const int kq = lane >> 3, lmq = lane & 7;

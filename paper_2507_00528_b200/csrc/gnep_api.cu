@@ -60,6 +60,9 @@ struct gnep_handle {
   bool tile_path = false;
   int *tilesA = nullptr;       // slot-group path: 32 atoms of one central species per tile, sorted by neighbour counts; -1 = idle lane
   int n_tilesA = 0, grid_adj = 0, grid_cg = 0, occ_adj = 1, occ_cg = 1, occ_S = 4;
+  bool fuse_adam = false; float fuse_b1 = 0.f, fuse_b2 = 0.f, fuse_eps = 0.f;   // set while gnep_train_epochs captures its graph
+  bool rad_split = false;                  // radial a3/a5 with RAD_SPLIT lanes per atom (small batches)
+  int ta_ang = ANG_TA, ta_frc = FRC_TA;   // atoms per warp of the warp-tile sweeps: fewer for small batches, so that every SM gets warps
   int *segA = nullptr, *atomA = nullptr;   // warp-tile path: angular list with every (atom, J) segment padded to 4 pairs
   float4 *pairA = nullptr;
   int *rowAu = nullptr, *segAu = nullptr, *atomAu = nullptr, *revAu = nullptr;   // angular list
@@ -197,7 +200,7 @@ int set_smem(gnep_handle *h, K kernel, size_t bytes) {
 
 int configure_kernels(gnep_handle *h) {
   const DevSpec &d = h->ds;
-  DISPATCH_KT(d.KRp, RET_IF(set_smem(h, k_radial_fwd<KT>, smem_radial(d))); RET_IF(set_smem(h, k_radial_adj<KT>, smem_radial(d)));
+  DISPATCH_KT(d.KRp, RET_IF(set_smem(h, k_radial_fwd<KT>, smem_radial(d))); RET_IF(set_smem(h, k_radial_adj<KT>, smem_radial(d))); RET_IF(set_smem(h, k_radial_adj_split<KT>, smem_radial(d)));
               RET_IF(set_smem(h, k_radial_q<KT>, smem_radial(d))));
   DISPATCH_ANG(d, auto kf = k_angular_fwd<KT, LMAX>; auto ka = k_angular_adj<KT, LMAX>; auto kc = k_cgrad_angular<KT, LMAX>;
                auto kp = k_angular_force<KT, LMAX>;
@@ -272,7 +275,7 @@ int enqueue_geometry_moments(gnep_handle *h) {
   const DevSpec &d = h->ds;
   DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_fwd<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, smem_radial(d), d, h->N, h->type_s, h->segR, h->pairR, h->theta, h->q, h->M1));
   if (!h->tile_path) {
-    DISPATCH_KA(d.KAp, DISPATCH_NQ(d.NA, auto kf = k_angw_fwd<KT, NQ>; LAUNCH(h, kf, cdiv(h->N, ANG_WARPS * ANG_TA), ANG_WARPS * 32, smem_angw_fwd(d), d, h->N, h->type_s, h->segA, h->pairA, h->theta, h->q, h->Sn, h->A1)));
+    DISPATCH_KA(d.KAp, DISPATCH_NQ(d.NA, auto kf = k_angw_fwd<KT, NQ>; LAUNCH(h, kf, cdiv(h->N, ANG_WARPS * h->ta_ang), ANG_WARPS * 32, smem_angw_fwd(d), d, h->N, h->ta_ang, h->type_s, h->segA, h->pairA, h->theta, h->q, h->Sn, h->A1)));
   }
   return GNEP_OK;
 }
@@ -308,14 +311,25 @@ int enqueue_forward(gnep_handle *h) {
   LAUNCH(h, k_net_tc<false>, h->n_cta_net, 256, smem_net_fwd(d), d, h->sm, h->theta, h->qscale, h->q, h->x, h->Ei, h->Ep, h->etil,
          (const int *)nullptr, (const float *)nullptr, (const float *)nullptr, (float *)nullptr, (float *)nullptr);
   mark(h, "a2_network_forward");
-  DISPATCH_ANG(d, auto kp = k_angular_force<KT, LMAX>; LAUNCH(h, kp, cdiv(h->N, FRC_WARPS * FRC_TA), FRC_WARPS * 32, smem_ang_force(d), d, h->N, h->type_s, h->segAu, h->atomAu, h->pairAu, h->theta, h->Ep, h->Sn, h->Beta, h->fpair));
+  DISPATCH_ANG(d, auto kp = k_angular_force<KT, LMAX>; LAUNCH(h, kp, cdiv(h->N, FRC_WARPS * h->ta_frc), FRC_WARPS * 32, smem_ang_force(d), d, h->N, h->ta_frc, h->type_s, h->segAu, h->atomAu, h->pairAu, h->theta, h->Ep, h->Sn, h->Beta, h->fpair));
   mark(h, "a3_angular_force");
   // radial forces + the gather of the angular pair forces (thread per atom): writes F_i, W_i once
-  DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_force<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, 0, d, h->N, h->type_s, h->segR, h->pairR, h->etil,
-                            h->segAu, h->revAu, h->pairAu, h->fpair, h->Fat, h->Wat));
+  if (h->rad_split) {
+    DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_force_split<KT>, cdiv((int64_t)h->N * RAD_SPLIT, RAD_THREADS), RAD_THREADS, 0, d, h->N, h->type_s, h->segR, h->pairR, h->etil,
+                              h->segAu, h->revAu, h->pairAu, h->fpair, h->Fat, h->Wat));
+  } else {
+    DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_force<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, 0, d, h->N, h->type_s, h->segR, h->pairR, h->etil,
+                              h->segAu, h->revAu, h->pairAu, h->fpair, h->Fat, h->Wat));
+  }
   mark(h, "a3_radial_force");
-  LAUNCH(h, k_struct_reduce, h->S, 128, 0, loss_cfg(h), h->srange, h->Ei, h->Fat, h->Wat, h->Eref, h->Fref_s, h->Wref, h->wgt, h->Es, h->Ws, h->e_s, h->u, h->omega, h->parts);
-  LAUNCH(h, k_loss_final, 1, 256, 0, loss_cfg(h), h->parts, h->theta, h->terms, h->scales);
+  // terms[5..6] = the Adam bias corrections of this step, terms[7] = the ticket counter of k_struct_reduce (zero at rest)
+  const AdamPre ap = {h->step_dev, h->terms + 5, h->fuse_b1, h->fuse_b2, h->fuse_adam ? 1 : 0};
+  if (h->S > 0) {
+    LAUNCH(h, k_struct_reduce, h->S, 128, 0, loss_cfg(h), h->srange, h->Ei, h->Fat, h->Wat, h->Eref, h->Fref_s, h->Wref, h->wgt, h->Es, h->Ws, h->e_s, h->u, h->omega, h->parts,
+           (unsigned *)(h->terms + 7), h->theta, h->terms, h->scales, ap);
+  } else {
+    LAUNCH(h, k_loss_final, 1, 128, 0, loss_cfg(h), h->parts, h->theta, h->terms, h->scales, ap);
+  }
   mark(h, "a4_loss_and_seeds");
   return GNEP_OK;
 }
@@ -323,10 +337,14 @@ int enqueue_forward(gnep_handle *h) {
 // ---- the backward half (rows a5-a8) ----------------------------------------------------------------
 int enqueue_backward(gnep_handle *h) {
   const DevSpec &d = h->ds;
-  DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_adj<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, smem_radial(d), d, h->N, h->type_s, h->struct_s, h->segR, h->pairR, h->theta, h->u, h->omega, h->scales, h->D, h->M2));
+  if (h->rad_split) {
+    DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_adj_split<KT>, cdiv((int64_t)h->N * RAD_SPLIT, RAD_THREADS), RAD_THREADS, smem_radial(d), d, h->N, h->type_s, h->struct_s, h->segR, h->pairR, h->theta, h->u, h->omega, h->scales, h->D, h->M2));
+  } else {
+    DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_adj<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, smem_radial(d), d, h->N, h->type_s, h->struct_s, h->segR, h->pairR, h->theta, h->u, h->omega, h->scales, h->D, h->M2));
+  }
   mark(h, "a5_radial_adjoint");
   if (!h->tile_path) {
-    DISPATCH_KA(d.KAp, DISPATCH_NQ(d.NA, auto ka = k_angw_adj<KT, NQ>; LAUNCH(h, ka, cdiv(h->N, ANG_WARPS * ANG_TA), ANG_WARPS * 32, smem_angw_adj(d), d, h->N, h->type_s, h->struct_s, h->segA, h->atomA, h->pairA, h->theta, h->u, h->omega, h->scales, h->Sn, h->Tn, h->A2, h->D)));
+    DISPATCH_KA(d.KAp, DISPATCH_NQ(d.NA, auto ka = k_angw_adj<KT, NQ>; LAUNCH(h, ka, cdiv(h->N, ANG_WARPS * h->ta_ang), ANG_WARPS * 32, smem_angw_adj(d), d, h->N, h->ta_ang, h->type_s, h->struct_s, h->segA, h->atomA, h->pairA, h->theta, h->u, h->omega, h->scales, h->Sn, h->Tn, h->A2, h->D)));
   } else
   DISPATCH_ANG(d, auto ka = k_angular_adj<KT, LMAX>; LAUNCH(h, ka, h->grid_adj, 32 * ang_warps(d), smem_ang_adj(d), d, h->n_tilesA, h->tilesA, h->type_s, h->struct_s, h->segAu, h->pairAu, h->theta, h->u, h->omega, h->scales, h->Sn, h->Beta, h->Tn, h->D, h->partialCA));
   mark(h, "a5_angular_adjoint");
@@ -343,7 +361,9 @@ int enqueue_backward(gnep_handle *h) {
   DISPATCH_ANG(d, auto kc = k_cgrad_angular<KT, LMAX>; LAUNCH(h, kc, h->grid_cg, 32 * ang_warps(d), smem_cgrad_ang(d), d, h->n_tilesA, h->tilesA, h->type_s, h->segAu, h->Ep, h->gbar, h->Sn, h->Tn, h->A1,
                                                           h->partialCA + (size_t)h->grid_adj * ang_warps(d) * d.T * d.T * d.NA * d.KAp));
   mark(h, "a7_angular_cgrad");
-  LAUNCH(h, k_grad_reduce, cdiv(d.P, 8), 256, 0, d, h->rm, (float)h->l2_share, h->theta, h->scales, h->partialCR, h->partialCA, h->partialW, h->partialB, h->grad);
+  // inside a captured training step the Adam update (a9) rides on the reduction: the thread that sums a parameter's partials updates it
+  const AdamFuse af = {h->m, h->v, h->terms + 5, h->lr_dev, h->fuse_b1, h->fuse_b2, h->fuse_eps, h->fuse_adam ? 1 : 0};
+  LAUNCH(h, k_grad_reduce, cdiv(d.P, 8), 256, 0, d, h->rm, (float)h->l2_share, h->theta, h->scales, h->partialCR, h->partialCA, h->partialW, h->partialB, h->grad, af);
   mark(h, "a8_grad_reduce");
   return GNEP_OK;
 }
@@ -841,6 +861,13 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
       h->grid_adj = 0;
       h->grid_cg = std::max(1, std::min(cdiv(N, ANG_WARPS), 4 * h->num_sms));
     }
+    // a mini-batch of a few hundred atoms would fill a handful of warps at the full tile size: shrink the atom tile until
+    // there are about four CTAs per SM (large batches keep the full tile, whose per-warp prologue is amortised best)
+    h->ta_ang = std::max(1, std::min(ANG_TA, cdiv(N, 4 * h->num_sms * ANG_WARPS)));
+    h->ta_frc = std::max(1, std::min(FRC_TA, cdiv(N, 5 * h->num_sms * FRC_WARPS)));
+    // one thread per atom needs about two CTAs per SM to hide its latencies; below that, RAD_SPLIT lanes per atom
+    h->rad_split = N < 2 * h->num_sms * RAD_THREADS;
+    if (const char *e = getenv("GNEP_RADIAL_SPLIT")) h->rad_split = atoi(e) != 0;
     for (int t = 0; t <= GNEP_MAX_SPECIES_C; ++t) { h->rm.chunk_base[t] = h->sm.chunk_base[t]; h->rm.gw_base[t] = h->sm.gw_base[t]; }
     const int ca_warps = h->tile_path ? ang_warps(d) : ANG_WARPS;
     h->rm.n_warps_ca = N > 0 ? (h->grid_adj + h->grid_cg) * ca_warps : 0;   // partial rows: the beta half (adjoint sweep) then the alpha half
@@ -1009,9 +1036,10 @@ int gnep_train_epochs(gnep_handle *h, int32_t n_epochs, float lr, float beta1, f
     int64_t before = h->launches;
     cudaGraph_t g = nullptr;
     CK(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
+    h->fuse_adam = true; h->fuse_b1 = beta1; h->fuse_b2 = beta2; h->fuse_eps = eps;   // a9 inside a4 / a8 (reduce_kernels.cuh)
     int rc = enqueue_forward(h);
     if (rc == GNEP_OK) rc = enqueue_backward(h);
-    if (rc == GNEP_OK) rc = enqueue_adam(h, beta1, beta2, eps);
+    h->fuse_adam = false;
     cudaError_t e = cudaStreamEndCapture(h->stream, &g);
     h->prof = prof;
     h->graph_launches = h->launches - before;

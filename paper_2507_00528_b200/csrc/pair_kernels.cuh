@@ -301,3 +301,140 @@ k_radial_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__res
            });
   radial_contract<KT>(sp, cs, type_s[a], Mrow, D + (size_t)a * sp.Ndes);
 }
+
+// ------------------------------------------------------------------------------------------------
+// Small-batch variants of a3 / a5 (radial): RAD_SPLIT LANES PER ATOM.  A mini-batch of a few hundred atoms (the paper
+// trains with batch size 1) gives the thread-per-atom kernels a handful of warps, each walking 60-odd pairs one
+// after the other: pure latency.  Here the lanes of an atom take every RAD_SPLIT-th pair of a species segment (eight
+// consecutive records = 128 contiguous bytes per atom and round) and add their sums by butterflies.  Same arithmetic
+// per pair as the kernels above; chosen by the host when the batch cannot fill the SMs with one thread per atom.
+// ------------------------------------------------------------------------------------------------
+#define RAD_SPLIT 8
+__device__ __forceinline__ float split_sum(float x) {
+#pragma unroll
+  for (int o = 1; o < RAD_SPLIT; o <<= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+  return x;
+}
+
+template <int KT>
+__global__ void __launch_bounds__(RAD_THREADS)
+k_radial_force_split(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ segR,
+                     const float4 *__restrict__ pairR, const float *__restrict__ etil, const int *__restrict__ segA,
+                     const int *__restrict__ revA, const float4 *__restrict__ pairA, const float4 *__restrict__ fpair,
+                     float4 *__restrict__ Fat, float *__restrict__ Wat) {
+  const int gt = blockIdx.x * RAD_THREADS + threadIdx.x;
+  const int a = gt / RAD_SPLIT, sub = gt % RAD_SPLIT;
+  const bool on = a < N;                          // whole warps stay in the butterflies
+  float F[3] = {0.f, 0.f, 0.f}, W[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  if (on) {
+    const int I = type_s[a];
+    const int TK = sp.T * KT;
+    const int *sg = segR + (size_t)a * (sp.T + 1);
+    for (int J = 0; J < sp.T; ++J) {
+      float ei[KT];
+      load_row<KT>(etil + (size_t)a * TK + J * KT, ei);
+      for (int p = sg[J] + sub; p < sg[J + 1]; p += RAD_SPLIT) {
+        const float4 r = pairR[p];
+        float ej[KT];
+        load_row<KT>(etil + (size_t)__float_as_int(r.w) * TK + I * KT, ej);
+        float d, rinv, Tk[KT], Dk[KT], hfc, hfcp, hdf;
+        pair_len(r.x * r.x + r.y * r.y + r.z * r.z, d, rinv);
+        cheb_TD<KT>(d, sp.rcRinv, Tk, Dk, hfc, hfcp, hdf);
+        float sD = 0.f, sT = 2.f * (ei[0] + ej[0]);
+#pragma unroll
+        for (int k = 1; k < KT; ++k) {
+          const float es = ei[k] + ej[k];
+          sD = fmaf(es, Dk[k], sD);
+          sT = fmaf(es, Tk[k] + 1.f, sT);
+        }
+        const float tot = sD * hdf + sT * hfcp;
+        const float hx = r.x * rinv, hy = r.y * rinv, hz = r.z * rinv;
+        F[0] += tot * hx; F[1] += tot * hy; F[2] += tot * hz;
+        const float hf = 0.5f * tot;              // half of the pair's symmetric total, as in k_radial_force
+        const float fx = hf * hx, fy = hf * hy, fz = hf * hz;
+        W[0] -= r.x * fx; W[1] -= r.y * fy; W[2] -= r.z * fz;
+        W[3] -= r.x * fy; W[4] -= r.y * fz; W[5] -= r.z * fx;
+      }
+    }
+    if (fpair) {
+      const int q0 = segA[(size_t)a * (sp.T + 1)], q1 = segA[(size_t)a * (sp.T + 1) + sp.T];
+      for (int p = q0 + sub; p < q1; p += RAD_SPLIT) {
+        const float4 f = fpair[p], x = pairA[p], g = fpair[revA[p]];
+        F[0] += f.x - g.x; F[1] += f.y - g.y; F[2] += f.z - g.z;
+        W[0] -= x.x * f.x; W[1] -= x.y * f.y; W[2] -= x.z * f.z;
+        W[3] -= x.x * f.y; W[4] -= x.y * f.z; W[5] -= x.z * f.x;
+      }
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < 3; ++c) F[c] = split_sum(F[c]);
+#pragma unroll
+  for (int c = 0; c < 6; ++c) W[c] = split_sum(W[c]);
+  if (on && sub == 0) {
+    Fat[a] = make_float4(F[0], F[1], F[2], 0.f);
+#pragma unroll
+    for (int c = 0; c < 6; c += 2) *(float2 *)(Wat + (size_t)a * 6 + c) = make_float2(W[c], W[c + 1]);
+  }
+}
+
+template <int KT>
+__global__ void __launch_bounds__(RAD_THREADS)
+k_radial_adj_split(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ struct_s,
+                   const int *__restrict__ segR, const float4 *__restrict__ pairR, const float *__restrict__ theta,
+                   const float4 *__restrict__ u, const float *__restrict__ omega, const float *__restrict__ scales,
+                   float *__restrict__ D, float *__restrict__ M2) {
+  extern __shared__ __align__(128) float smem[];
+  float *cs = smem;
+  stage_coeff(cs, theta, sp.T * sp.T * sp.NR, sp.KR, KT);
+  __syncthreads();
+  const int gt = blockIdx.x * RAD_THREADS + threadIdx.x;
+  const int a = gt / RAD_SPLIT, sub = gt % RAD_SPLIT;
+  const bool on = a < N;
+  const int ac = on ? a : 0;
+  const int I = N > 0 ? type_s[ac] : 0;
+  AdjCtx ctx = {};
+  if (on) ctx = make_adj(u, omega, scales, a, struct_s[a]);
+  const int *sg = segR + (size_t)ac * (sp.T + 1);
+  float o[2] = {0.f, 0.f};                        // D_n of the lane's two functions n = sub, sub + RAD_SPLIT
+  for (int J = 0; J < sp.T; ++J) {
+    float acc[KT];
+#pragma unroll
+    for (int k = 0; k < KT; ++k) acc[k] = 0.f;
+    if (on)
+      for (int p = sg[J] + sub; p < sg[J + 1]; p += RAD_SPLIT) {
+        const float4 r = pairR[p];
+        const float4 uj = u[__float_as_int(r.w)];
+        float d, rinv, Tk[KT], Dk[KT], hfc, hfcp, hdf;
+        pair_len(r.x * r.x + r.y * r.y + r.z * r.z, d, rinv);
+        float ax, ay, az;
+        pair_adjoint(ctx, uj, r, ax, ay, az);
+        const float ar = (ax * r.x + ay * r.y + az * r.z) * rinv;
+        cheb_TD<KT>(d, sp.rcRinv, Tk, Dk, hfc, hfcp, hdf);
+        const float w1 = ar * hdf, w2 = ar * hfcp;
+        acc[0] = fmaf(2.f, w2, acc[0]);
+#pragma unroll
+        for (int k = 1; k < KT; ++k) acc[k] = fmaf(w1, Dk[k], fmaf(w2, Tk[k], acc[k] + w2));
+      }
+#pragma unroll
+    for (int k = 0; k < KT; ++k) acc[k] = split_sum(acc[k]);       // every lane of the atom now holds M2[J][.]
+    if (on && sub == 0) store_row<KT>(M2 + (size_t)a * sp.T * KT + J * KT, acc);
+    const float *c = cs + (size_t)(I * sp.T + J) * sp.NR * KT;
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+      const int n = sub + i * RAD_SPLIT;
+      if (n < sp.NR) {
+        float cv[KT];
+        load_row<KT>(c + n * KT, cv);
+#pragma unroll
+        for (int k = 0; k < KT; ++k) o[i] = fmaf(cv[k], acc[k], o[i]);
+      }
+    }
+  }
+  if (on) {
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+      const int n = sub + i * RAD_SPLIT;
+      if (n < sp.NR) D[(size_t)a * sp.Ndes + n] = o[i];
+    }
+  }
+}

@@ -34,17 +34,68 @@ __device__ __forceinline__ void block_reduce_d(double (&v)[NV], double *sh /*[NV
   __syncthreads();
 }
 
+// Adam bookkeeping folded into the epoch's kernels when a whole training step is enqueued (gnep_train_epochs): the last
+// CTA of k_struct_reduce advances the step counter and writes the two bias corrections (fp64 pow, once per step), and
+// k_grad_reduce applies the update to the parameter it has just reduced.  `on == 0`: plain loss / gradient evaluation.
+struct AdamPre { long long *step; float *bc; float beta1, beta2; int on; };
+struct AdamFuse { float *m, *v; const float *bc, *lr; float beta1, beta2, eps; int on; };
+
+// a4: loss terms {L, t_e, t_f, t_v, t_2} (Eq.9-12 + L2) and the per-term seed multipliers, by ONE CTA (any size)
+// scales = {se, sf, sv, s2}: all 1 in mean-square mode, 1/(2 sqrt t_x) in RMSE mode (0 if t_x = 0).
+// `parts` was written by other CTAs of the same launch: read around L1.
+__device__ __forceinline__ void loss_final(const LossCfg &lc, const double *parts, const float *__restrict__ theta,
+                                           float *__restrict__ terms, float *__restrict__ scales, const AdamPre &ap,
+                                           double *sh) {
+  double v[4] = {0, 0, 0, 0};
+  for (int s = threadIdx.x; s < lc.S; s += blockDim.x) { v[0] += __ldcg(parts + s * 3); v[1] += __ldcg(parts + s * 3 + 1); v[2] += __ldcg(parts + s * 3 + 2); }
+  {   // sum theta^2: four independent fp64 chains per thread
+    double w[4] = {0, 0, 0, 0};
+    const int P4 = lc.P >> 2;
+    for (int p = threadIdx.x; p < P4; p += blockDim.x) {
+      const float4 x = ((const float4 *)theta)[p];
+      w[0] += (double)x.x * x.x; w[1] += (double)x.y * x.y; w[2] += (double)x.z * x.z; w[3] += (double)x.w * x.w;
+    }
+    for (int p = 4 * P4 + threadIdx.x; p < lc.P; p += blockDim.x) { double x = theta[p]; w[0] += x * x; }
+    v[3] = (w[0] + w[1]) + (w[2] + w[3]);
+  }
+  block_reduce_d<4>(v, sh);
+  if (threadIdx.x == 0) {
+    double te = lc.ZE > 0 ? v[0] / lc.ZE : 0.0;
+    double tf = lc.ZF > 0 ? v[1] / (3.0 * lc.ZF) : 0.0;
+    double tv = lc.ZV > 0 ? v[2] / (6.0 * lc.ZV) : 0.0;
+    double t2 = lc.l2_share * v[3] / lc.P;
+    double L, sc[4] = {1, 1, 1, 1};
+    if (lc.loss_mode == 0) L = lc.lam_e * te + lc.lam_f * tf + lc.lam_v * tv + lc.lam_2 * t2;
+    else {
+      L = lc.lam_e * sqrt(te) + lc.lam_f * sqrt(tf) + lc.lam_v * sqrt(tv) + lc.lam_2 * sqrt(t2);
+      sc[0] = te > 0 ? 0.5 / sqrt(te) : 0; sc[1] = tf > 0 ? 0.5 / sqrt(tf) : 0;
+      sc[2] = tv > 0 ? 0.5 / sqrt(tv) : 0; sc[3] = t2 > 0 ? 0.5 / sqrt(t2) : 0;
+    }
+    terms[0] = (float)L; terms[1] = (float)te; terms[2] = (float)tf; terms[3] = (float)tv; terms[4] = (float)t2;
+    for (int i = 0; i < 4; ++i) scales[i] = (float)sc[i];
+    if (ap.on) {
+      const long long t = *ap.step + 1;
+      *ap.step = t;
+      ap.bc[0] = (float)(1.0 - pow((double)ap.beta1, (double)t)); ap.bc[1] = (float)(1.0 - pow((double)ap.beta2, (double)t));
+    }
+  }
+}
+
 // a4: one CTA per structure.  E_s = sum E_i, W_s = sum W_i (Eq.1, Eq.4), residuals of Eq.10-12 and the
 // seeds e_s = 2 lam_e w_e,s dE_s/(Z_E N_s), u_i = 2 lam_f w_f,s (F_i - Fref_i)/(3 Z_F), omega_s = 2 lam_v w_v,s dW_s/(6 Z_V N_s)
 // (w = per-structure weights, all ones by default: then Z_E = Z_V = S, Z_F = N and these are the seeds of Eq.10-12).
+// The CTA that finishes last (a ticket counter, reset for the next launch) adds the per-structure parts in structure
+// order -- a fixed order whichever CTA it is -- and writes the loss terms: no second launch.
 __global__ void __launch_bounds__(128)
 k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const float *__restrict__ Ei,
                 const float4 *__restrict__ Fat, const float *__restrict__ Wat, const double *__restrict__ Eref,
                 const float *__restrict__ Fref_s, const double *__restrict__ Wref,
                 const double *__restrict__ wgt /*[3][S]: w_e, w_f, w_v*/, double *__restrict__ Es,
                 double *__restrict__ Ws, float *__restrict__ e_s, float4 *__restrict__ u,
-                float *__restrict__ omega, double *__restrict__ parts /*[S][3]*/) {
+                float *__restrict__ omega, double *parts /*[S][3]*/, unsigned *ticket,
+                const float *__restrict__ theta, float *__restrict__ terms, float *__restrict__ scales, AdamPre ap) {
   __shared__ double sh[8 * 4];
+  __shared__ int last;
   const int s = blockIdx.x;
   double v[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // E, W[6], sum |dF|^2
   int Ns = 0;
@@ -86,34 +137,22 @@ k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const 
       omega[s * 6 + c] = (float)om;
     }
     parts[s * 3 + 0] = pe; parts[s * 3 + 1] = wf * v[7]; parts[s * 3 + 2] = pv;
+    __threadfence();                                           // parts visible before the ticket is taken
+    last = atomicAdd(ticket, 1u) == gridDim.x - 1;
   }
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  loss_final(lc, parts, theta, terms, scales, ap, sh);
+  if (threadIdx.x == 0) *ticket = 0u;
 }
 
-// a4: loss terms {L, t_e, t_f, t_v, t_2} (Eq.9-12 + L2) and the per-term seed multipliers
-// scales = {se, sf, sv, s2}: all 1 in mean-square mode, 1/(2 sqrt t_x) in RMSE mode (0 if t_x = 0).
-__global__ void __launch_bounds__(256)
-k_loss_final(LossCfg lc, const double *__restrict__ parts, const float *__restrict__ theta,
-             float *__restrict__ terms, float *__restrict__ scales) {
-  __shared__ double sh[4 * 8];
-  double v[4] = {0, 0, 0, 0};
-  for (int s = threadIdx.x; s < lc.S; s += blockDim.x) { v[0] += parts[s * 3]; v[1] += parts[s * 3 + 1]; v[2] += parts[s * 3 + 2]; }
-  for (int p = threadIdx.x; p < lc.P; p += blockDim.x) { double x = theta[p]; v[3] += x * x; }
-  block_reduce_d<4>(v, sh);
-  if (threadIdx.x == 0) {
-    double te = lc.ZE > 0 ? v[0] / lc.ZE : 0.0;
-    double tf = lc.ZF > 0 ? v[1] / (3.0 * lc.ZF) : 0.0;
-    double tv = lc.ZV > 0 ? v[2] / (6.0 * lc.ZV) : 0.0;
-    double t2 = lc.l2_share * v[3] / lc.P;
-    double L, sc[4] = {1, 1, 1, 1};
-    if (lc.loss_mode == 0) L = lc.lam_e * te + lc.lam_f * tf + lc.lam_v * tv + lc.lam_2 * t2;
-    else {
-      L = lc.lam_e * sqrt(te) + lc.lam_f * sqrt(tf) + lc.lam_v * sqrt(tv) + lc.lam_2 * sqrt(t2);
-      sc[0] = te > 0 ? 0.5 / sqrt(te) : 0; sc[1] = tf > 0 ? 0.5 / sqrt(tf) : 0;
-      sc[2] = tv > 0 ? 0.5 / sqrt(tv) : 0; sc[3] = t2 > 0 ? 0.5 / sqrt(t2) : 0;
-    }
-    terms[0] = (float)L; terms[1] = (float)te; terms[2] = (float)tf; terms[3] = (float)tv; terms[4] = (float)t2;
-    for (int i = 0; i < 4; ++i) scales[i] = (float)sc[i];
-  }
+// a4 without structures (an empty batch still has its L2 term): the loss terms alone
+__global__ void __launch_bounds__(128)
+k_loss_final(LossCfg lc, const double *parts, const float *__restrict__ theta, float *__restrict__ terms,
+             float *__restrict__ scales, AdamPre ap) {
+  __shared__ double sh[8 * 4];
+  loss_final(lc, parts, theta, terms, scales, ap, sh);
 }
 
 // a8: grad[p] = sum over the partial buffers that cover p (fixed order, fp64) + 2 lam_2 s2 theta_p / P.
@@ -125,9 +164,10 @@ struct ReduceMap {
 // Block = 8 consecutive parameters x 32 row lanes: every lane sums rows lane, lane+32, ... of its parameter's partial
 // buffer in fp64, the 32 lane sums are added in lane order by one thread (fixed order -> bit-reproducible).
 __global__ void __launch_bounds__(256)
-k_grad_reduce(DevSpec sp, ReduceMap rm, float l2_share, const float *__restrict__ theta, const float *__restrict__ scales,
+k_grad_reduce(DevSpec sp, ReduceMap rm, float l2_share, float *theta, const float *__restrict__ scales,
               const float *__restrict__ partialCR, const float *__restrict__ partialCA,
-              const float *__restrict__ partialW, const float *__restrict__ partialB, float *__restrict__ grad) {
+              const float *__restrict__ partialW, const float *__restrict__ partialB, float *__restrict__ grad,
+              AdamFuse af) {
   __shared__ double sh[32][9];
   const int tx = threadIdx.x & 7, ty = threadIdx.x >> 3;
   const int p = blockIdx.x * 8 + tx;
@@ -163,8 +203,17 @@ k_grad_reduce(DevSpec sp, ReduceMap rm, float l2_share, const float *__restrict_
     double t = 0.0;
 #pragma unroll
     for (int r = 0; r < 32; ++r) t += sh[r][tx];
-    t += 2.0 * (double)l2_share * (double)sp.lam_2 * (double)scales[3] * (double)theta[p] / (double)sp.P;
-    grad[p] = (float)t;
+    const float th = theta[p];
+    t += 2.0 * (double)l2_share * (double)sp.lam_2 * (double)scales[3] * (double)th / (double)sp.P;
+    const float g = (float)t;
+    grad[p] = g;
+    if (af.on) {                             // a9 on the parameter just reduced (same arithmetic as k_adam)
+      const float c1 = af.bc[0], c2 = af.bc[1], lr = *af.lr;
+      const float mm = af.beta1 * af.m[p] + (1.f - af.beta1) * g;
+      const float vv = af.beta2 * af.v[p] + (1.f - af.beta2) * g * g;
+      af.m[p] = mm; af.v[p] = vv;
+      theta[p] = th - lr * (mm / c1) / (sqrtf(vv / c2) + af.eps);
+    }
   }
 }
 
