@@ -325,7 +325,7 @@ int enqueue_forward(gnep_handle *h) {
   // terms[5..6] = the Adam bias corrections of this step, terms[7] = the ticket counter of k_struct_reduce (zero at rest)
   const AdamPre ap = {h->step_dev, h->terms + 5, h->fuse_b1, h->fuse_b2, h->fuse_adam ? 1 : 0};
   if (h->S > 0) {
-    LAUNCH(h, k_struct_reduce, h->S, 128, 0, loss_cfg(h), h->srange, h->Ei, h->Fat, h->Wat, h->Eref, h->Fref_s, h->Wref, h->wgt, h->Es, h->Ws, h->e_s, h->u, h->omega, h->parts,
+    LAUNCH(h, k_struct_reduce, h->S + LOSS_T2_CTAS, 128, 0, loss_cfg(h), h->srange, h->Ei, h->Fat, h->Wat, h->Eref, h->Fref_s, h->Wref, h->wgt, h->Es, h->Ws, h->e_s, h->u, h->omega, h->parts,
            (unsigned *)(h->terms + 7), h->theta, h->terms, h->scales, ap);
   } else {
     LAUNCH(h, k_loss_final, 1, 128, 0, loss_cfg(h), h->parts, h->theta, h->terms, h->scales, ap);
@@ -841,7 +841,7 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
       int nc = tiles > 0 ? std::max(1, std::min(cdiv(tiles, 2), (int)((double)h->num_sms * tiles / std::max(tiles_total, 1) + 0.5))) : 0;
       h->sm.cta_base[t + 1] = h->sm.cta_base[t] + nc;
       // k_cgrad_radial: K-chunks
-      int want = nt > 0 ? std::max(1, std::min(cdiv(nt, 256), (int)((4.0 * h->num_sms * nt) / std::max(N, 1) + 0.5))) : 0;
+      int want = nt > 0 ? std::max(1, std::min(cdiv(nt, 32), (int)((4.0 * h->num_sms * nt) / std::max(N, 1) + 0.5))) : 0;
       int ca = want > 0 ? ((cdiv(nt, want) + 31) / 32) * 32 : 32;
       h->sm.chunk_atoms[t] = ca;
       h->sm.chunk_base[t + 1] = h->sm.chunk_base[t] + (nt > 0 ? cdiv(nt, ca) : 0);
@@ -880,7 +880,7 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     if (!h->tile_path) BA(h->A2, n * T * d.KAp * ANGW_NLM);
     BA(h->gbar, n * d.Ndes); BA(h->pbuf, nxt * d.NnS); BA(h->eat, npad); BA(h->Wat, n * 6);
     BA(h->Fat, n); BA(h->fpair, h->nA); BA(h->u, n);
-    BA(h->Es, S); BA(h->Ws, (size_t)S * 6); BA(h->parts, (size_t)S * 3); BA(h->e_s, S); BA(h->omega, (size_t)S * 6);
+    BA(h->Es, S); BA(h->Ws, (size_t)S * 6); BA(h->parts, (size_t)S * 3 + LOSS_T2_CTAS); BA(h->e_s, S); BA(h->omega, (size_t)S * 6);
     BA(h->partialCR, (size_t)std::max(h->n_chunks, 1) * d.NR * T * d.KRp);
     BA(h->partialCA, (size_t)std::max(h->rm.n_warps_ca, 1) * T * T * d.NA * d.KAp);
     BA(h->partialW, (size_t)std::max(h->n_gw, 1) * d.Nn * d.Ndes);

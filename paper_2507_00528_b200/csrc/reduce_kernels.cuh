@@ -43,22 +43,31 @@ struct AdamFuse { float *m, *v; const float *bc, *lr; float beta1, beta2, eps; i
 // a4: loss terms {L, t_e, t_f, t_v, t_2} (Eq.9-12 + L2) and the per-term seed multipliers, by ONE CTA (any size)
 // scales = {se, sf, sv, s2}: all 1 in mean-square mode, 1/(2 sqrt t_x) in RMSE mode (0 if t_x = 0).
 // `parts` was written by other CTAs of the same launch: read around L1.
-__device__ __forceinline__ void loss_final(const LossCfg &lc, const double *parts, const float *__restrict__ theta,
-                                           float *__restrict__ terms, float *__restrict__ scales, const AdamPre &ap,
-                                           double *sh) {
+#define LOSS_T2_CTAS 8      // extra CTAs of k_struct_reduce that sum theta^2 (the L2 term) in slices
+
+// sum of theta[p]^2 over p = first, first + stride, ... (float4 groups), fp64, fixed order per thread
+__device__ __forceinline__ double theta_sq(const float *__restrict__ theta, int P, int first, int stride) {
+  double w[4] = {0, 0, 0, 0};
+  const int P4 = P >> 2;
+  for (int p = first; p < P4; p += stride) {
+    const float4 x = ((const float4 *)theta)[p];
+    w[0] += (double)x.x * x.x; w[1] += (double)x.y * x.y; w[2] += (double)x.z * x.z; w[3] += (double)x.w * x.w;
+  }
+  for (int p = 4 * P4 + first; p < P; p += stride) { double x = theta[p]; w[0] += x * x; }
+  return (w[0] + w[1]) + (w[2] + w[3]);
+}
+
+__device__ __forceinline__ void loss_final(const LossCfg &lc, const double *parts, const double *t2parts, int nt2,
+                                           const float *__restrict__ theta, float *__restrict__ terms,
+                                           float *__restrict__ scales, const AdamPre &ap, double *sh) {
   double v[4] = {0, 0, 0, 0};
   for (int s = threadIdx.x; s < lc.S; s += blockDim.x) { v[0] += __ldcg(parts + s * 3); v[1] += __ldcg(parts + s * 3 + 1); v[2] += __ldcg(parts + s * 3 + 2); }
-  {   // sum theta^2: four independent fp64 chains per thread
-    double w[4] = {0, 0, 0, 0};
-    const int P4 = lc.P >> 2;
-    for (int p = threadIdx.x; p < P4; p += blockDim.x) {
-      const float4 x = ((const float4 *)theta)[p];
-      w[0] += (double)x.x * x.x; w[1] += (double)x.y * x.y; w[2] += (double)x.z * x.z; w[3] += (double)x.w * x.w;
-    }
-    for (int p = 4 * P4 + threadIdx.x; p < lc.P; p += blockDim.x) { double x = theta[p]; w[0] += x * x; }
-    v[3] = (w[0] + w[1]) + (w[2] + w[3]);
-  }
+  if (nt2 > 0) { if (threadIdx.x == 0) for (int i = 0; i < nt2; ++i) v[3] += __ldcg(t2parts + i); }
+  else v[3] = theta_sq(theta, lc.P, threadIdx.x, blockDim.x);
   block_reduce_d<4>(v, sh);
+  const long long t = ap.on ? *ap.step + 1 : 0;       // read by every thread before thread 0 advances it
+  __syncthreads();
+  if (ap.on && threadIdx.x == 32) ap.bc[1] = (float)(1.0 - pow((double)ap.beta2, (double)t));   // the two fp64 pows side by side
   if (threadIdx.x == 0) {
     double te = lc.ZE > 0 ? v[0] / lc.ZE : 0.0;
     double tf = lc.ZF > 0 ? v[1] / (3.0 * lc.ZF) : 0.0;
@@ -73,30 +82,43 @@ __device__ __forceinline__ void loss_final(const LossCfg &lc, const double *part
     }
     terms[0] = (float)L; terms[1] = (float)te; terms[2] = (float)tf; terms[3] = (float)tv; terms[4] = (float)t2;
     for (int i = 0; i < 4; ++i) scales[i] = (float)sc[i];
-    if (ap.on) {
-      const long long t = *ap.step + 1;
-      *ap.step = t;
-      ap.bc[0] = (float)(1.0 - pow((double)ap.beta1, (double)t)); ap.bc[1] = (float)(1.0 - pow((double)ap.beta2, (double)t));
-    }
+    if (ap.on) { *ap.step = t; ap.bc[0] = (float)(1.0 - pow((double)ap.beta1, (double)t)); }
   }
 }
 
 // a4: one CTA per structure.  E_s = sum E_i, W_s = sum W_i (Eq.1, Eq.4), residuals of Eq.10-12 and the
 // seeds e_s = 2 lam_e w_e,s dE_s/(Z_E N_s), u_i = 2 lam_f w_f,s (F_i - Fref_i)/(3 Z_F), omega_s = 2 lam_v w_v,s dW_s/(6 Z_V N_s)
 // (w = per-structure weights, all ones by default: then Z_E = Z_V = S, Z_F = N and these are the seeds of Eq.10-12).
-// The CTA that finishes last (a ticket counter, reset for the next launch) adds the per-structure parts in structure
-// order -- a fixed order whichever CTA it is -- and writes the loss terms: no second launch.
+// CTAs S .. S + LOSS_T2_CTAS - 1 each sum a slice of theta^2 instead.  The CTA that finishes last (a ticket counter,
+// reset for the next launch) adds the per-structure parts in structure order and the theta^2 slices in slice order --
+// a fixed order whichever CTA it is -- and writes the loss terms: no second launch.
 __global__ void __launch_bounds__(128)
 k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const float *__restrict__ Ei,
                 const float4 *__restrict__ Fat, const float *__restrict__ Wat, const double *__restrict__ Eref,
                 const float *__restrict__ Fref_s, const double *__restrict__ Wref,
                 const double *__restrict__ wgt /*[3][S]: w_e, w_f, w_v*/, double *__restrict__ Es,
                 double *__restrict__ Ws, float *__restrict__ e_s, float4 *__restrict__ u,
-                float *__restrict__ omega, double *parts /*[S][3]*/, unsigned *ticket,
+                float *__restrict__ omega, double *parts /*[S][3] + [LOSS_T2_CTAS]*/, unsigned *ticket,
                 const float *__restrict__ theta, float *__restrict__ terms, float *__restrict__ scales, AdamPre ap) {
   __shared__ double sh[8 * 4];
   __shared__ int last;
   const int s = blockIdx.x;
+  double *t2parts = parts + (size_t)lc.S * 3;
+  if (s >= lc.S) {                          // a theta^2 slice
+    double w[1] = {theta_sq(theta, lc.P, (s - lc.S) * blockDim.x + threadIdx.x, LOSS_T2_CTAS * blockDim.x)};
+    block_reduce_d<1>(w, sh);
+    if (threadIdx.x == 0) {
+      t2parts[s - lc.S] = w[0];
+      __threadfence();
+      last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    loss_final(lc, parts, t2parts, LOSS_T2_CTAS, theta, terms, scales, ap, sh);
+    if (threadIdx.x == 0) *ticket = 0u;
+    return;
+  }
   double v[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // E, W[6], sum |dF|^2
   int Ns = 0;
   const double we = wgt[s], wf = wgt[lc.S + s], wv = wgt[2 * lc.S + s];
@@ -143,7 +165,7 @@ k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const 
   __syncthreads();
   if (!last) return;
   __threadfence();
-  loss_final(lc, parts, theta, terms, scales, ap, sh);
+  loss_final(lc, parts, t2parts, LOSS_T2_CTAS, theta, terms, scales, ap, sh);
   if (threadIdx.x == 0) *ticket = 0u;
 }
 
@@ -152,7 +174,7 @@ __global__ void __launch_bounds__(128)
 k_loss_final(LossCfg lc, const double *parts, const float *__restrict__ theta, float *__restrict__ terms,
              float *__restrict__ scales, AdamPre ap) {
   __shared__ double sh[8 * 4];
-  loss_final(lc, parts, theta, terms, scales, ap, sh);
+  loss_final(lc, parts, nullptr, 0, theta, terms, scales, ap, sh);
 }
 
 // a8: grad[p] = sum over the partial buffers that cover p (fixed order, fp64) + 2 lam_2 s2 theta_p / P.
