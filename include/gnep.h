@@ -19,6 +19,10 @@
  *     loss_terms == NULL and host-free arguments do not.
  *   - units: Angstrom, eV, eV/Angstrom; virial in eV (total per structure).
  *   - one handle = one model + one resident batch.  Not thread-safe per handle.
+ *   - two environment variables choose between kernel sets that compute the same thing (for tests and
+ *     measurements; results agree to rounding): GNEP_ANGULAR_MAPPING=groups (read by gnep_create) runs the
+ *     slot-group angular kernels for l_max <= 4 too; GNEP_SMALL_BATCH=0|1 (read by gnep_load_batch) forces
+ *     the large-batch / small-batch mappings instead of choosing by the batch size.
  *
  * Parameter vector theta (P floats, R6/S:8(c).2):
  *   [ cR[I][J][n][k] (k fastest; I = species of the central atom, J = of the neighbour)

@@ -861,13 +861,15 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
       h->grid_adj = 0;
       h->grid_cg = std::max(1, std::min(cdiv(N, ANG_WARPS), 4 * h->num_sms));
     }
-    // a mini-batch of a few hundred atoms would fill a handful of warps at the full tile size: shrink the atom tile until
-    // there are about four CTAs per SM (large batches keep the full tile, whose per-warp prologue is amortised best)
-    h->ta_ang = std::max(1, std::min(ANG_TA, cdiv(N, 4 * h->num_sms * ANG_WARPS)));
-    h->ta_frc = std::max(1, std::min(FRC_TA, cdiv(N, 5 * h->num_sms * FRC_WARPS)));
-    // one thread per atom needs about two CTAs per SM to hide its latencies; below that, RAD_SPLIT lanes per atom
-    h->rad_split = N < 2 * h->num_sms * RAD_THREADS;
-    if (const char *e = getenv("GNEP_RADIAL_SPLIT")) h->rad_split = atoi(e) != 0;
+    // A mini-batch of a few hundred atoms (the paper trains with batch size 1) cannot fill the SMs with the
+    // large-batch mappings (one thread per atom in the radial sweeps, ANG_TA atoms per warp in the angular ones): below
+    // two CTAs per SM of the radial kernels the atom tiles shrink until there are about four CTAs per SM and the radial
+    // force / adjoint sweeps use RAD_SPLIT lanes per atom.  GNEP_SMALL_BATCH=0/1 forces either set (tests run both).
+    bool small = N < 2 * h->num_sms * RAD_THREADS;
+    if (const char *e = getenv("GNEP_SMALL_BATCH")) small = atoi(e) != 0;
+    h->ta_ang = small ? std::max(1, std::min(ANG_TA, cdiv(N, 4 * h->num_sms * ANG_WARPS))) : ANG_TA;
+    h->ta_frc = small ? std::max(1, std::min(FRC_TA, cdiv(N, 5 * h->num_sms * FRC_WARPS))) : FRC_TA;
+    h->rad_split = small;
     for (int t = 0; t <= GNEP_MAX_SPECIES_C; ++t) { h->rm.chunk_base[t] = h->sm.chunk_base[t]; h->rm.gw_base[t] = h->sm.gw_base[t]; }
     const int ca_warps = h->tile_path ? ang_warps(d) : ANG_WARPS;
     h->rm.n_warps_ca = N > 0 ? (h->grid_adj + h->grid_cg) * ca_warps : 0;   // partial rows: the beta half (adjoint sweep) then the alpha half

@@ -85,11 +85,20 @@ def _check_all(config, n_structs, adam_steps=10, spec_over=None, floor=1e-6):
     g.destroy()
 
 
-def test_config0_full():
+@pytest.fixture(params=["large", "small"])
+def kernel_set(request, monkeypatch):
+    """Both kernel sets on the same small case: the large-batch mappings (one thread per atom in the radial sweeps,
+    16 / 8 atoms per warp in the angular ones) that the bench configurations run, and the small-batch ones (8 lanes per
+    atom, one atom per warp) that a batch of this size would get by itself.  Read by gnep_load_batch."""
+    monkeypatch.setenv("GNEP_SMALL_BATCH", "1" if request.param == "small" else "0")
+    return request.param
+
+
+def test_config0_full(kernel_set):
     _check_all(0, None)
 
 
-def test_config1_sample_with_4body():
+def test_config1_sample_with_4body(kernel_set):
     _check_all(1, 6)
 
 
@@ -97,7 +106,7 @@ def test_config2_liquid_sample():
     _check_all(2, 4, adam_steps=3)
 
 
-def test_config3_mixed_sample():
+def test_config3_mixed_sample(kernel_set):
     _check_all(3, 9, adam_steps=3)
 
 
@@ -128,7 +137,7 @@ def test_small_l_and_odd_sizes():
     _check_all(0, 2, adam_steps=2, spec_over=over)
 
 
-def test_three_species_odd_sizes():
+def test_three_species_odd_sizes(kernel_set):
     """T = 3 (nine c^{IJ} blocks, three networks), l_max = 3 with the 4-body term, odd sizes."""
     over = {"n_species": 3, "l_max": 3, "use_4body": True, "n_radial": 4, "n_basis_radial": 7, "n_angular": 5,
             "n_basis_angular": 5, "n_neurons": 13}
