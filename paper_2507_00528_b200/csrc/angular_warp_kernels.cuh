@@ -45,6 +45,18 @@ __device__ __forceinline__ void fma4(float &acc, const float4 &a, const float4 &
   acc = fmaf(a.x, b.x, acc); acc = fmaf(a.y, b.y, acc); acc = fmaf(a.z, b.z, acc); acc = fmaf(a.w, b.w, acc);
 }
 
+// Packed FP32 FMA (sm_100 FFMA2, fma.rn.f32x2): two independent IEEE fp32 FMAs in ONE issue slot.  The sweeps are bound
+// by issue slots, not by the FMA pipe, so the outer products are written on register pairs.
+// (k0, k1) += F(k0, k1; pair p) x_p over the four pairs of a group; Fa = (k0p0, k1p0, k0p1, k1p1), Fb = (k0p2, ..., k1p3)
+__device__ __forceinline__ void fma4x2(float &a0, float &a1, const float4 &Fa, const float4 &Fb, const float4 &X) {
+  float2 t = make_float2(a0, a1);
+  t = __ffma2_rn(make_float2(Fa.x, Fa.y), make_float2(X.x, X.x), t);
+  t = __ffma2_rn(make_float2(Fa.z, Fa.w), make_float2(X.y, X.y), t);
+  t = __ffma2_rn(make_float2(Fb.x, Fb.y), make_float2(X.z, X.z), t);
+  t = __ffma2_rn(make_float2(Fb.z, Fb.w), make_float2(X.w, X.w), t);
+  a0 = t.x; a1 = t.y;
+}
+
 // Per-atom lane layout "(n, lmg)": lane = 3*nq + lmg (lanes 0..29), n = nb + nq for nb = 0, 10, ..., and the lane owns
 // lm in [8 lmg, 8 lmg + 8): lmg 0 = all of l=1 (i<3) and l=2; lmg 1 = all of l=3 (i<7) and the first slot of l=4;
 // lmg 2 = the rest of l=4.  Everything per-atom (S, T, beta, alpha, q_nl, D_nl) is produced in this layout with static
@@ -92,9 +104,15 @@ __device__ __forceinline__ void xown_add(const DevSpec &sp, const float *ct, int
         const float4 c4 = *(const float4 *)(ct + ((I * sp.T + J) * KT + kb + r) * ANG_NQ + 4 * kq);   // n = kq + 4 j
         const float cv[4] = {c4.x, c4.y, c4.z, c4.w};                                                // zero beyond NA
 #pragma unroll
-        for (int j = 0; j < NJ; ++j)
+        for (int j = 0; j + 1 < NJ; j += 2)         // two functions n per packed FMA
 #pragma unroll
-          for (int i = 0; i < 3; ++i) Xo[j][i] = fmaf(cv[j], a[i], Xo[j][i]);
+          for (int i = 0; i < 3; ++i) {
+            const float2 t = __ffma2_rn(make_float2(cv[j], cv[j + 1]), make_float2(a[i], a[i]), make_float2(Xo[j][i], Xo[j + 1][i]));
+            Xo[j][i] = t.x; Xo[j + 1][i] = t.y;
+          }
+        if (NJ & 1)
+#pragma unroll
+          for (int i = 0; i < 3; ++i) Xo[NJ - 1][i] = fmaf(cv[NJ - 1], a[i], Xo[NJ - 1][i]);
       }
     }
   }
@@ -416,6 +434,7 @@ k_angw_adj(DevSpec sp, int N, int ta /* atoms per warp, <= ANG_TA */, const int 
               const float *__restrict__ scales, const float *__restrict__ S, float *__restrict__ Tn,
               float *__restrict__ A2, float *__restrict__ D) {
   constexpr int KQ = (KT + 3) / 4;      // k per lane: lane = (k quarter kq, lm eighth lmq) holds a KQ x 3 register tile
+  constexpr bool KPAIR = (KQ % 2 == 0); // radial factors stored as k pairs, outer products on packed FMAs
   extern __shared__ __align__(128) float smem[];
   float *ct = smem;
   const int nct = sp.T * sp.T * KT * ANG_NQ;
@@ -554,15 +573,31 @@ k_angw_adj(DevSpec sp, int N, int ta /* atoms per warp, <= ANG_TA */, const int 
       float ar = ax * hx + ay * hy + az * hz;
       float f[KT], fp[KT];
       cheb_ffp<KT>(d, sp.rcAinv, f, fp);
+      if constexpr (KPAIR) {   // rows of k pairs: [k/2][slot][2]
 #pragma unroll
-      for (int k = 0; k < KT; ++k) { sf1[k * ANG_LD + lane] = fp[k] * ar; sf2[k * ANG_LD + lane] = f[k]; }
+        for (int k = 0; k < KT; k += 2) {
+          *(float2 *)(sf1 + k * ANG_LD + 2 * lane) = make_float2(fp[k] * ar, fp[k + 1] * ar);
+          *(float2 *)(sf2 + k * ANG_LD + 2 * lane) = make_float2(f[k], f[k + 1]);
+        }
+      } else {
+#pragma unroll
+        for (int k = 0; k < KT; ++k) { sf1[k * ANG_LD + lane] = fp[k] * ar; sf2[k * ANG_LD + lane] = f[k]; }
+      }
       blm_unit<4>(hx, hy, hz, [&](int lm, int l, float b, float gx, float gy, float gz) {
         sX[lm * ANG_LD + lane] = b;
         sY[lm * ANG_LD + lane] = rinv * ((gx * ax + gy * ay + gz * az) - (float)l * b * ar);
       });
     } else {
+      if constexpr (KPAIR) {
 #pragma unroll
-      for (int k = 0; k < KT; ++k) { sf1[k * ANG_LD + lane] = 0.f; sf2[k * ANG_LD + lane] = 0.f; }
+        for (int k = 0; k < KT; k += 2) {
+          *(float2 *)(sf1 + k * ANG_LD + 2 * lane) = make_float2(0.f, 0.f);
+          *(float2 *)(sf2 + k * ANG_LD + 2 * lane) = make_float2(0.f, 0.f);
+        }
+      } else {
+#pragma unroll
+        for (int k = 0; k < KT; ++k) { sf1[k * ANG_LD + lane] = 0.f; sf2[k * ANG_LD + lane] = 0.f; }
+      }
 #pragma unroll
       for (int lm = 0; lm < ANGW_NLM; ++lm) { sX[lm * ANG_LD + lane] = 0.f; sY[lm * ANG_LD + lane] = 0.f; }
     }
@@ -572,6 +607,27 @@ k_angw_adj(DevSpec sp, int N, int ta /* atoms per warp, <= ANG_TA */, const int 
     while (pos < chunk_end) {
       while (seg_end <= pos) next_segment();
       const int hi = min(seg_end, chunk_end);
+      if constexpr (KPAIR) {
+        for (int g = (pos - c0) >> 2; g < (hi - c0) >> 2; ++g) {   // whole 4-pair groups only (padded segments)
+          float4 f1a[KQ / 2], f1b[KQ / 2], f2a[KQ / 2], f2b[KQ / 2];
+#pragma unroll
+          for (int rp = 0; rp < KQ / 2; ++rp) {                     // the lane's k pairs (k0, k0 + 1), four pair slots each
+            const int o = (kq * KQ + 2 * rp) * ANG_LD + 8 * g;
+            f1a[rp] = *(const float4 *)(sf1 + o); f1b[rp] = *(const float4 *)(sf1 + o + 4);
+            f2a[rp] = *(const float4 *)(sf2 + o); f2b[rp] = *(const float4 *)(sf2 + o + 4);
+          }
+#pragma unroll
+          for (int i = 0; i < 3; ++i) {
+            const float4 X = *(const float4 *)(sX + (3 * lmq + i) * ANG_LD + 4 * g);
+            const float4 Y = *(const float4 *)(sY + (3 * lmq + i) * ANG_LD + 4 * g);
+#pragma unroll
+            for (int rp = 0; rp < KQ / 2; ++rp) {
+              fma4x2(acc[2 * rp][i], acc[2 * rp + 1][i], f1a[rp], f1b[rp], X);
+              fma4x2(acc[2 * rp][i], acc[2 * rp + 1][i], f2a[rp], f2b[rp], Y);
+            }
+          }
+        }
+      } else
       for (int g = (pos - c0) >> 2; g < (hi - c0) >> 2; ++g) {   // whole 4-pair groups only (padded segments)
         float4 f1[KQ], f2[KQ];
 #pragma unroll
