@@ -616,31 +616,34 @@ __device__ __forceinline__ void beta_row(const DevSpec &sp, const float *__restr
 // over that slot range, then the harmonic sweep.  LO and HI - LO are multiples of 4 (16-byte loads of the beta rows).
 template <int KT, int LMAX, int LO, int HI>
 __device__ __forceinline__ void force_block(const DevSpec &sp, const float *__restrict__ be, int NS, const float *__restrict__ c,
-                                            const float (&f)[KT], const float (&fp)[KT], float hx, float hy, float hz,
+                                            const float2 (&ffp)[KT], float hx, float hy, float hz,
                                             float &sB, float &sl, float &vx, float &vy, float &vz) {
   constexpr int NB = HI - LO;
   static_assert(LO % 4 == 0 && NB % 4 == 0, "slot blocks are float4-aligned");
-  float gam[NB], gamp[NB];
+  // (gam, gamp) and (g_n, g_n') live in register pairs: every FMA of the two sums is one packed FP32 FMA (FFMA2) with
+  // the coefficient / the beta entry as the broadcast operand -- half the issue slots of the scalar form
+  float2 gg[NB];
 #pragma unroll
-  for (int i = 0; i < NB; ++i) { gam[i] = 0.f; gamp[i] = 0.f; }
+  for (int i = 0; i < NB; ++i) gg[i] = make_float2(0.f, 0.f);
   for (int n = 0; n < sp.NA; ++n) {
-    float g = 0.f, gp = 0.f;
+    float2 g2 = make_float2(0.f, 0.f);
 #pragma unroll
-    for (int k = 0; k < KT; ++k) { const float cv = c[n * KT + k]; g = fmaf(cv, f[k], g); gp = fmaf(cv, fp[k], gp); }
+    for (int k = 0; k < KT; ++k) { const float cv = c[n * KT + k]; g2 = __ffma2_rn(make_float2(cv, cv), ffp[k], g2); }
 #pragma unroll
     for (int v = 0; v < NB / 4; ++v) {
       const float4 b4 = *(const float4 *)(be + n * NS + LO + 4 * v);
-      gam[4 * v] = fmaf(g, b4.x, gam[4 * v]); gam[4 * v + 1] = fmaf(g, b4.y, gam[4 * v + 1]);
-      gam[4 * v + 2] = fmaf(g, b4.z, gam[4 * v + 2]); gam[4 * v + 3] = fmaf(g, b4.w, gam[4 * v + 3]);
-      gamp[4 * v] = fmaf(gp, b4.x, gamp[4 * v]); gamp[4 * v + 1] = fmaf(gp, b4.y, gamp[4 * v + 1]);
-      gamp[4 * v + 2] = fmaf(gp, b4.z, gamp[4 * v + 2]); gamp[4 * v + 3] = fmaf(gp, b4.w, gamp[4 * v + 3]);
+      gg[4 * v] = __ffma2_rn(g2, make_float2(b4.x, b4.x), gg[4 * v]);
+      gg[4 * v + 1] = __ffma2_rn(g2, make_float2(b4.y, b4.y), gg[4 * v + 1]);
+      gg[4 * v + 2] = __ffma2_rn(g2, make_float2(b4.z, b4.z), gg[4 * v + 2]);
+      gg[4 * v + 3] = __ffma2_rn(g2, make_float2(b4.w, b4.w), gg[4 * v + 3]);
     }
   }
   blm_unit<LMAX>(hx, hy, hz, [&](int lm, int l, float b, float gx, float gy, float gz) {
     if (lm >= LO && lm < HI) {
-      sB = fmaf(gamp[lm - LO], b, sB);
-      sl = fmaf((float)l * gam[lm - LO], b, sl);
-      vx = fmaf(gam[lm - LO], gx, vx); vy = fmaf(gam[lm - LO], gy, vy); vz = fmaf(gam[lm - LO], gz, vz);
+      const float gam = gg[lm - LO].x, gamp = gg[lm - LO].y;
+      sB = fmaf(gamp, b, sB);
+      sl = fmaf((float)l * gam, b, sl);
+      vx = fmaf(gam, gx, vx); vy = fmaf(gam, gy, vy); vz = fmaf(gam, gz, vz);
     }
   });
 }
@@ -688,16 +691,16 @@ k_angular_force(DevSpec sp, int N, int ta /* atoms per warp, <= FRC_TA */, const
     const float *be = beta + (a - a_lo) * nb;
     float d, rinv;
     pair_len(r.x * r.x + r.y * r.y + r.z * r.z, d, rinv);
-    float f[KT], fp[KT];
-    cheb_ffp<KT>(d, sp.rcAinv, f, fp);
+    float2 ffp[KT];                                  // (f_k, f_k') pairs
+    cheb_ffp2<KT>(d, sp.rcAinv, ffp);
     const float *c = cs + (I * sp.T + J) * sp.NA * KT;
     const float hx = r.x * rinv, hy = r.y * rinv, hz = r.z * rinv;
     float sB = 0.f, sl = 0.f, vx = 0.f, vy = 0.f, vz = 0.f;
-    force_block<KT, LMAX, 0, 24>(sp, be, NS, c, f, fp, hx, hy, hz, sB, sl, vx, vy, vz);              // l = 1..4
+    force_block<KT, LMAX, 0, 24>(sp, be, NS, c, ffp, hx, hy, hz, sB, sl, vx, vy, vz);              // l = 1..4
     if constexpr (LMAX > 4) {
-      if (sp.L >= 5) force_block<KT, LMAX, 24, 48>(sp, be, NS, c, f, fp, hx, hy, hz, sB, sl, vx, vy, vz);   // l = 5, 6
-      if (sp.L >= 7) force_block<KT, LMAX, 48, 64>(sp, be, NS, c, f, fp, hx, hy, hz, sB, sl, vx, vy, vz);   // l = 7 and slot 63
-      if (sp.L >= 8) force_block<KT, LMAX, 64, 80>(sp, be, NS, c, f, fp, hx, hy, hz, sB, sl, vx, vy, vz);   // rest of l = 8
+      if (sp.L >= 5) force_block<KT, LMAX, 24, 48>(sp, be, NS, c, ffp, hx, hy, hz, sB, sl, vx, vy, vz);   // l = 5, 6
+      if (sp.L >= 7) force_block<KT, LMAX, 48, 64>(sp, be, NS, c, ffp, hx, hy, hz, sB, sl, vx, vy, vz);   // l = 7 and slot 63
+      if (sp.L >= 8) force_block<KT, LMAX, 64, 80>(sp, be, NS, c, ffp, hx, hy, hz, sB, sl, vx, vy, vz);   // rest of l = 8
     }
     fpair[p] = make_float4(hx * sB + rinv * (vx - hx * sl), hy * sB + rinv * (vy - hy * sl),
                            hz * sB + rinv * (vz - hz * sl), 0.f);

@@ -148,6 +148,34 @@ __device__ __forceinline__ void cheb_ffp(float d, float rcinv, float (&f)[KT], f
   }
 }
 
+// (f_k, f_k') as register pairs, built with packed FP32 FMAs (sm_100 FFMA2: two fp32 FMAs per issue slot): the pair
+// (T_k, D_k) runs through one recurrence, (T_k, D_k) = 2 xi (T_k-1, D_k-1) - (T_k-2, D_k-2) + (0, 2 T_k-1), and
+// (f_k, f_k') = (hfc, hdf) (T_k, D_k) + (hfc, hfcp (T_k + 1)).  Same values as cheb_ffp up to rounding order.
+template <int KT>
+__device__ __forceinline__ void cheb_ffp2(float d, float rcinv, float2 (&ffp)[KT]) {
+  const float t = fminf(d * rcinv, 1.f);
+  const float x = t - 1.f;
+  const float xi = 2.f * x * x - 1.f;
+  float sn, cs;
+  sincospi01(t, sn, cs);
+  const bool in = t < 1.f;
+  const float hfc = in ? 0.25f * (1.f + cs) : 0.f;
+  const float hfcp = in ? -0.25f * GNEP_PI_F * rcinv * sn : 0.f;
+  const float hdf = hfc * 4.f * x * rcinv;
+  const float2 sc = make_float2(hfc, hdf), xx = make_float2(2.f * xi, 2.f * xi);
+  auto combine = [&](const float2 &td) { return __ffma2_rn(sc, td, make_float2(hfc, fmaf(hfcp, td.x, hfcp))); };
+  float2 p2 = make_float2(1.f, 0.f), p1 = make_float2(xi, 1.f);
+  ffp[0] = make_float2(2.f * hfc, 2.f * hfcp);
+  if (KT > 1) ffp[1] = combine(p1);
+#pragma unroll
+  for (int k = 2; k < KT; ++k) {
+    float2 c = __ffma2_rn(xx, p1, make_float2(-p2.x, -p2.y));
+    c.y = fmaf(2.f, p1.x, c.y);
+    ffp[k] = combine(c);
+    p2 = p1; p1 = c;
+  }
+}
+
 // ---------------------------------------------------------------------------------------------
 // Real harmonics of a UNIT vector (paper App.B): emits, for each of the LMAX (LMAX + 2) (l,m) slots,
 // b = b_lm(rhat) and g = (grad b_lm)(rhat)  [polynomial gradient, r^2 terms differentiated, then r=1].
