@@ -756,16 +756,20 @@ k_angw_cgrad(DevSpec sp, int N, const int *__restrict__ type_s, const float *__r
       const int J = row / KT, k = row - J * KT;
       float *dst = accS + ((I * sp.T + J) * sp.NA) * KT + k;
       for (int n = n_lo; n < n_hi; ++n) {
-        float sa[2] = {0.f, 0.f}, sb[2] = {0.f, 0.f};   // four independent FMA chains
+        float2 sa[2], sb[2];                              // four independent chains of packed FMAs (even / odd lm partial sums)
+        sa[0] = sa[1] = sb[0] = sb[1] = make_float2(0.f, 0.f);
 #pragma unroll
         for (int v = 0; v < 6; ++v) {
           const float4 al4 = *(const float4 *)(sAl + n * ANGW_NLM + 4 * v);
           const float4 be4 = *(const float4 *)(sBe + n * ANGW_NLM + 4 * v);
-          float &s = sa[v & 1], &t = sb[v & 1];
-          s = fmaf(al4.x, x1[v].x, s); s = fmaf(al4.y, x1[v].y, s); s = fmaf(al4.z, x1[v].z, s); s = fmaf(al4.w, x1[v].w, s);
-          t = fmaf(be4.x, x2[v].x, t); t = fmaf(be4.y, x2[v].y, t); t = fmaf(be4.z, x2[v].z, t); t = fmaf(be4.w, x2[v].w, t);
+          float2 &s = sa[v & 1], &t = sb[v & 1];
+          s = __ffma2_rn(make_float2(al4.x, al4.y), make_float2(x1[v].x, x1[v].y), s);
+          s = __ffma2_rn(make_float2(al4.z, al4.w), make_float2(x1[v].z, x1[v].w), s);
+          t = __ffma2_rn(make_float2(be4.x, be4.y), make_float2(x2[v].x, x2[v].y), t);
+          t = __ffma2_rn(make_float2(be4.z, be4.w), make_float2(x2[v].z, x2[v].w), t);
         }
-        dst[n * KT] += (sa[0] + sa[1]) + (sb[0] + sb[1]);
+        const float2 st = __fadd2_rn(__fadd2_rn(sa[0], sa[1]), __fadd2_rn(sb[0], sb[1]));
+        dst[n * KT] += st.x + st.y;
       }
     }
     __syncwarp();
