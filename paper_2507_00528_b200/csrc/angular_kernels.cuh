@@ -638,14 +638,16 @@ __device__ __forceinline__ void force_block(const DevSpec &sp, const float *__re
       gg[4 * v + 3] = __ffma2_rn(g2, make_float2(b4.w, b4.w), gg[4 * v + 3]);
     }
   }
+  float2 slB = make_float2(sl, sB), vxy = make_float2(vx, vy);
   blm_unit<LMAX>(hx, hy, hz, [&](int lm, int l, float b, float gx, float gy, float gz) {
     if (lm >= LO && lm < HI) {
-      const float gam = gg[lm - LO].x, gamp = gg[lm - LO].y;
-      sB = fmaf(gamp, b, sB);
-      sl = fmaf((float)l * gam, b, sl);
-      vx = fmaf(gam, gx, vx); vy = fmaf(gam, gy, vy); vz = fmaf(gam, gz, vz);
+      const float2 g = gg[lm - LO];                                  // (gam, gamp)
+      slB = __ffma2_rn(g, make_float2((float)l * b, b), slB);        // sl += l gam b,  sB += gamp b
+      vxy = __ffma2_rn(make_float2(g.x, g.x), make_float2(gx, gy), vxy);
+      vz = fmaf(g.x, gz, vz);
     }
   });
+  sl = slB.x; sB = slB.y; vx = vxy.x; vy = vxy.y;
 }
 
 template <int KT, int LMAX>
