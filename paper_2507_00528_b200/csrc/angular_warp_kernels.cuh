@@ -583,9 +583,12 @@ k_angw_adj(DevSpec sp, int N, int ta /* atoms per warp, <= ANG_TA */, const int 
 #pragma unroll
         for (int k = 0; k < KT; ++k) { sf1[k * ANG_LD + lane] = fp[k] * ar; sf2[k * ANG_LD + lane] = f[k]; }
       }
+      // Y_lm = (grad B_lm . a - l B_lm (a.rhat)) / d with a / d and l (a.rhat) / d formed once per pair: four FMAs per slot
+      const float bx = ax * rinv, by = ay * rinv, bz = az * rinv, br = ar * rinv;
+      const float lar[4] = {-br, -2.f * br, -3.f * br, -4.f * br};
       blm_unit<4>(hx, hy, hz, [&](int lm, int l, float b, float gx, float gy, float gz) {
         sX[lm * ANG_LD + lane] = b;
-        sY[lm * ANG_LD + lane] = rinv * ((gx * ax + gy * ay + gz * az) - (float)l * b * ar);
+        sY[lm * ANG_LD + lane] = fmaf(lar[l - 1], b, fmaf(gz, bz, fmaf(gy, by, gx * bx)));
       });
     } else {
       if constexpr (KPAIR) {
