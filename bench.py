@@ -301,13 +301,15 @@ def run_ours(args):
     t_top = acc[top] * 1e-3
     bound = fm.PHASE_BOUND.get(top, "alu")
     # committed ncu capture of this workload, if any: DRAM bytes of the dominant kernel per launch
-    traffic, traffic_src = None, None
+    traffic, traffic_src, capture = None, None, None
     tfile = os.path.join(ROOT, "profiles", "r2_cfg%d_traffic.csv" % args.config)
     if not args.structs and os.path.exists(tfile):
         for ln in open(tfile):
             f = ln.strip().split(",")
             if f and f[0] == top:
                 traffic = int(float(f[-1])); traffic_src = "committed capture profiles/%s (ncu --set full, not re-measured in this run)" % os.path.basename(tfile)
+                if len(f) >= 8:     # pipe utilisations of the same capture: what the kernel is really bound by
+                    capture = {"fma_pipe_pct": float(f[2]), "issue_slots_pct": float(f[3]), "shared_memory_pipe_pct": float(f[4])}
     if bound == "hbm":
         ach = mbytes[top] / t_top / 1e9
         roof = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "traffic": traffic,
@@ -324,6 +326,8 @@ def run_ours(args):
                  "bound_from": "ncu captures under profiles/ (flopmodel.PHASE_BOUND), not from a comparison of fractions"})
     if traffic_src:
         roof["traffic_source"] = traffic_src
+    if capture:
+        roof["counters_from_committed_capture"] = capture
     path_tf = sum(mflops.values()) / (ms_step * 1e-3) / 1e12
     path_tf_design = sum(dflops.values()) / (ms_step * 1e-3) / 1e12
     phases = {k: {"ms": round(v, 4), "bound": fm.PHASE_BOUND.get(k),
