@@ -137,6 +137,14 @@ def test_small_l_and_odd_sizes():
     _check_all(0, 2, adam_steps=2, spec_over=over)
 
 
+@pytest.mark.parametrize("ka,kr", [(4, 4), (12, 16), (3, 6)])
+def test_basis_sizes_of_every_kernel_instantiation(ka, kr, kernel_set):
+    """The angular warp kernels are instantiated for KA padded to 4, 8 and 16 (the packed-FMA k pairs exist for 8 and 16,
+    4 keeps the scalar path), the radial ones for KR padded to 4, 6, 8, 12, 16: one case per remaining size."""
+    over = {"n_basis_angular": ka, "n_basis_radial": kr, "n_angular": 6, "n_neurons": 14}
+    _check_all(0, 3, adam_steps=2, spec_over=over, floor=1e-5)
+
+
 def test_three_species_odd_sizes(kernel_set):
     """T = 3 (nine c^{IJ} blocks, three networks), l_max = 3 with the 4-body term, odd sizes."""
     over = {"n_species": 3, "l_max": 3, "use_4body": True, "n_radial": 4, "n_basis_radial": 7, "n_angular": 5,
