@@ -214,6 +214,7 @@ k_angw_fwd(DevSpec sp, int N, int ta /* atoms per warp, <= ANG_TA */, const int 
         qa[n] = qa_;
         if (sp.L >= 2) qa[sp.NA + n] = qb_;
         if (sp.use4) qa[sp.NA * sp.L + n] = GNEP_KAPPA4 * p4_value(sv + 3);
+        if (sp.use5) qa[sp.NA * (sp.L + sp.use4) + n] = p5_value(sv);          // R41: kappa5 |S_n,1|^4, after the 4-body block
       }
       if (on && nl.lmg == 1) {
         if (sp.L >= 3) qa[2 * sp.NA + n] = qa_;
@@ -412,6 +413,7 @@ k_angw_S(DevSpec sp, int N, const int *__restrict__ type_s, const float *__restr
           qa[n] = qa_;
           if (sp.L >= 2) qa[sp.NA + n] = qb_;
           if (sp.use4) qa[sp.NA * sp.L + n] = GNEP_KAPPA4 * p4_value(sv[e] + 3);
+          if (sp.use5) qa[sp.NA * (sp.L + sp.use4) + n] = p5_value(sv[e]);
         }
         if (on && lmg == 1) {
           if (sp.L >= 3) qa[2 * sp.NA + n] = qa_;
@@ -426,7 +428,7 @@ k_angw_S(DevSpec sp, int N, const int *__restrict__ type_s, const float *__restr
 // ------------------------------------------------------------------------------------------------
 // a5 (angular): A2 moments with the pair adjoint a_ij, T_nlm = c.A2, D_(n,l) = sum_m 2 C_lm S_nlm T_nlm, D_4
 // ------------------------------------------------------------------------------------------------
-template <int KT, int NQ>
+template <int KT, int NQ, bool B5 /* model has the 5-body term */>
 __global__ void __launch_bounds__(ANG_WARPS * 32)
 k_angw_adj(DevSpec sp, int N, int ta /* atoms per warp, <= ANG_TA */, const int *__restrict__ type_s, const int *__restrict__ struct_s,
               const int *__restrict__ segA, const int *__restrict__ atomA, const float4 *__restrict__ pairA,
@@ -532,6 +534,11 @@ k_angw_adj(DevSpec sp, int N, int ta /* atoms per warp, <= ANG_TA */, const int 
           float g4[5];
           p4_grad(sv + 3, g4);
           Da[sp.NA * sp.L + n] = GNEP_KAPPA4 * (g4[0] * tv[3] + g4[1] * tv[4] + g4[2] * tv[5] + g4[3] * tv[6] + g4[4] * tv[7]);
+        }
+        if constexpr (B5) {                              // directional derivative of q5 = kappa5 |S_1|^4 along T
+          float g5[3];
+          p5_grad(sv, g5);
+          Da[sp.NA * (sp.L + sp.use4) + n] = g5[0] * tv[0] + g5[1] * tv[1] + g5[2] * tv[2];
         }
       }
       if (on && nl.lmg == 1) {
@@ -662,7 +669,7 @@ k_angw_adj(DevSpec sp, int N, int ta /* atoms per warp, <= ANG_TA */, const int 
 // One warp per atom (grid-stride); lane = ((J,k) row, half of n).  Each warp keeps a [T][T][NA][KT] accumulator in
 // shared memory over the atoms it visits and writes one partial at the end (reduced by k_grad_reduce).
 // ------------------------------------------------------------------------------------------------
-template <int KT>
+template <int KT, bool B5 /* model has the 5-body term */>
 __global__ void __launch_bounds__(ANG_WARPS * 32, 4)
 k_angw_cgrad(DevSpec sp, int N, const int *__restrict__ type_s, const float *__restrict__ Ep,
                 const float *__restrict__ gbar, const float *__restrict__ S, const float *__restrict__ Tn,
@@ -737,6 +744,15 @@ k_angw_cgrad(DevSpec sp, int N, const int *__restrict__ type_s, const float *__r
           const float e4 = GNEP_KAPPA4 * e4r, gb4 = GNEP_KAPPA4 * gb4r;
 #pragma unroll
           for (int m = 0; m < 5; ++m) { al[3 + m] += gb4 * g4[m] + e4 * hv[m]; be[3 + m] += e4 * g4[m]; }
+        }
+        if (B5 && nl.lmg == 0) {                        // 5-body (R41) on the l = 1 slots; its E', gbar are fetched here
+          const int o5 = sp.NR + (sp.L + sp.use4) * sp.NA + n;
+          const float e5 = Epa[o5], gb5 = gba[o5];
+          float g5[3], hv[3];
+          p5_grad(sv, g5);
+          p5_hess_vec(sv, tv, hv);
+#pragma unroll
+          for (int m = 0; m < 3; ++m) { al[m] += gb5 * g5[m] + e5 * hv[m]; be[m] += e5 * g5[m]; }
         }
         *(float4 *)(sAl + o) = make_float4(al[0], al[1], al[2], al[3]);
         *(float4 *)(sAl + o + 4) = make_float4(al[4], al[5], al[6], al[7]);

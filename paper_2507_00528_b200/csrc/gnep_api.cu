@@ -143,6 +143,9 @@ int padded_basis_ang(int K) { return K <= 4 ? 4 : K <= 8 ? 8 : 16; }
 #define DISPATCH_NQ(NA_, ...)                                   \
   if ((NA_) <= 10) { constexpr int NQ = 10; __VA_ARGS__; }      \
   else { constexpr int NQ = 16; __VA_ARGS__; }
+#define DISPATCH_B5(U5_, ...)                                   \
+  if (U5_) { constexpr bool B5 = true; __VA_ARGS__; }           \
+  else { constexpr bool B5 = false; __VA_ARGS__; }
 #define DISPATCH_TMAX(T_, ...)                                  \
   if ((T_) <= 2) { constexpr int TMAX = 2; __VA_ARGS__; }       \
   else { constexpr int TMAX = 4; __VA_ARGS__; }
@@ -213,12 +216,12 @@ int configure_kernels(gnep_handle *h) {
                CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kc, 32 * ang_warps(d), smem_cgrad_ang(d)));
                h->occ_cg = std::max(occ, 1));
   if (!h->tile_path) {
-    DISPATCH_KA(d.KAp, RET_IF(set_smem(h, k_angw_cgrad<KT>, smem_angw_cgrad(d))); DISPATCH_TMAX(d.T, auto ks = k_angw_S<KT, TMAX>; RET_IF(set_smem(h, ks, smem_angw_S(d)));
+    DISPATCH_KA(d.KAp, DISPATCH_B5(d.use5, auto kc5 = k_angw_cgrad<KT, B5>; RET_IF(set_smem(h, kc5, smem_angw_cgrad(d)))); DISPATCH_TMAX(d.T, auto ks = k_angw_S<KT, TMAX>; RET_IF(set_smem(h, ks, smem_angw_S(d)));
                               int occ = 0;
                               CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, ks, ANG_WARPS * 32, smem_angw_S(d)));
                               h->occ_S = std::max(occ, 1));
-                DISPATCH_NQ(d.NA, auto kf = k_angw_fwd<KT, NQ>; auto ka = k_angw_adj<KT, NQ>; RET_IF(set_smem(h, kf, smem_angw_fwd(d)));
-                            RET_IF(set_smem(h, ka, smem_angw_adj(d)))));
+                DISPATCH_NQ(d.NA, auto kf = k_angw_fwd<KT, NQ>; RET_IF(set_smem(h, kf, smem_angw_fwd(d)));
+                            DISPATCH_B5(d.use5, auto ka = k_angw_adj<KT, NQ, B5>; RET_IF(set_smem(h, ka, smem_angw_adj(d))))));
   }
   {   // TMEM budget of one k_net_tc warpgroup (256 columns): D1 + max(D1 corrections, D2 + D2 corrections)
     const NetDims nd = net_dims(d);
@@ -344,7 +347,7 @@ int enqueue_backward(gnep_handle *h) {
   }
   mark(h, "a5_radial_adjoint");
   if (!h->tile_path) {
-    DISPATCH_KA(d.KAp, DISPATCH_NQ(d.NA, auto ka = k_angw_adj<KT, NQ>; LAUNCH(h, ka, cdiv(h->N, ANG_WARPS * h->ta_ang), ANG_WARPS * 32, smem_angw_adj(d), d, h->N, h->ta_ang, h->type_s, h->struct_s, h->segA, h->atomA, h->pairA, h->theta, h->u, h->omega, h->scales, h->Sn, h->Tn, h->A2, h->D)));
+    DISPATCH_KA(d.KAp, DISPATCH_NQ(d.NA, DISPATCH_B5(d.use5, auto ka = k_angw_adj<KT, NQ, B5>; LAUNCH(h, ka, cdiv(h->N, ANG_WARPS * h->ta_ang), ANG_WARPS * 32, smem_angw_adj(d), d, h->N, h->ta_ang, h->type_s, h->struct_s, h->segA, h->atomA, h->pairA, h->theta, h->u, h->omega, h->scales, h->Sn, h->Tn, h->A2, h->D))));
   } else
   DISPATCH_ANG(d, auto ka = k_angular_adj<KT, LMAX>; LAUNCH(h, ka, h->grid_adj, 32 * ang_warps(d), smem_ang_adj(d), d, h->n_tilesA, h->tilesA, h->type_s, h->struct_s, h->segAu, h->pairAu, h->theta, h->u, h->omega, h->scales, h->Sn, h->Beta, h->Tn, h->D, h->partialCA));
   mark(h, "a5_angular_adjoint");
@@ -356,7 +359,7 @@ int enqueue_backward(gnep_handle *h) {
   LAUNCH(h, k_cgrad_radial, h->n_chunks, CR_THREADS, smem_cgrad_rad(d), d, h->sm, h->gbar, h->Ep, h->M1, h->M2, h->partialCR);
   mark(h, "a7_radial_cgrad");
   if (!h->tile_path) {
-    DISPATCH_KA(d.KAp, LAUNCH(h, k_angw_cgrad<KT>, h->grid_cg, ANG_WARPS * 32, smem_angw_cgrad(d), d, h->N, h->type_s, h->Ep, h->gbar, h->Sn, h->Tn, h->A1, h->A2, h->partialCA));
+    DISPATCH_KA(d.KAp, DISPATCH_B5(d.use5, auto kc5 = k_angw_cgrad<KT, B5>; LAUNCH(h, kc5, h->grid_cg, ANG_WARPS * 32, smem_angw_cgrad(d), d, h->N, h->type_s, h->Ep, h->gbar, h->Sn, h->Tn, h->A1, h->A2, h->partialCA)));
   } else
   DISPATCH_ANG(d, auto kc = k_cgrad_angular<KT, LMAX>; LAUNCH(h, kc, h->grid_cg, 32 * ang_warps(d), smem_cgrad_ang(d), d, h->n_tilesA, h->tilesA, h->type_s, h->segAu, h->Ep, h->gbar, h->Sn, h->Tn, h->A1,
                                                           h->partialCA + (size_t)h->grid_adj * ang_warps(d) * d.T * d.T * d.NA * d.KAp));
@@ -478,7 +481,7 @@ int gnep_create(const gnep_model_spec *spec, void *cuda_stream, gnep_handle **ou
   }
   {   // GNEP_ANGULAR_MAPPING=groups forces the slot-group kernels for l_max <= 4 as well (they are the only ones above 4)
     const char *m = getenv("GNEP_ANGULAR_MAPPING");
-    h->tile_path = d.L > 4 || d.use5 || (m && std::string(m) == "groups");   // (the warp-tile kernels have no 5-body term)
+    h->tile_path = d.L > 4 || (m && std::string(m) == "groups");
   }
   int rc;
   if ((rc = configure_kernels(h)) != GNEP_OK) return bail(rc);

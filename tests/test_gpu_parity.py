@@ -177,9 +177,15 @@ def test_l_max_5_three_species_no_many_body():
     _check_all(0, 3, adam_steps=2, spec_over=over, floor=3e-5)
 
 
-def test_5body_with_l_max_4_and_slot_group_mapping_for_config3():
-    """The 5-body term routes l_max <= 4 models through the slot-group kernels too (config-3 sizes, 4 groups)."""
+def test_5body_with_l_max_4_on_the_warp_tile_kernels(kernel_set):
+    """3-body l <= 4 + 4-body + 5-body (the full descriptor set named at P:65) on the warp-tile kernels."""
     _check_all(3, 4, adam_steps=2, spec_over={"use_5body": True, "n_neurons": 40}, floor=1e-5)   # (4 structures: a noisier sample than config 3)
+
+
+def test_slot_group_mapping_for_config3_with_5body(monkeypatch):
+    """GNEP_ANGULAR_MAPPING=groups runs an l_max <= 4 model through the slot-group kernels (config-3 sizes, 4 groups)."""
+    monkeypatch.setenv("GNEP_ANGULAR_MAPPING", "groups")
+    _check_all(3, 4, adam_steps=2, spec_over={"use_5body": True, "n_neurons": 40}, floor=1e-5)
 
 
 def test_two_live_handles_with_different_specs():
