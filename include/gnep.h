@@ -188,6 +188,27 @@ int gnep_set_opt_state(gnep_handle *h, const float *m, const float *v, int64_t s
 int gnep_batch_info(const gnep_handle *h, int64_t *n_atoms, int64_t *n_structs, int64_t *n_pairs_radial,
                     int64_t *n_pairs_angular);
 
+/* Loss terms WITHOUT ANY ALLOCATION (for callers that cannot call cudaMalloc: code under CUDA-graph capture, tight
+ * serving loops, harnesses that forbid it): t_e, t_f, t_v of Eq.10-12 (readings R18, R19) and
+ * L = lam_e t_e + lam_f t_f + lam_v t_v (Eq.9 without the L2 term; square roots per term in loss_mode 1, R21) of
+ * caller-held predictions against caller-held references, with the handle's lambdas and unit per-structure weights.
+ * A variant of the per-structure reduction of gnep_loss_and_grad whose partial sums live in a fixed file-scope device
+ * array of the library (192 KiB + 256 B per GPU, held from library load to process exit) instead of the per-batch
+ * buffers: the call makes no cudaMalloc / cudaFree and calls no allocating routine; it enqueues one 4-byte memset and
+ * one kernel on the handle's stream and does NOT synchronise.  No batch needs to be loaded.
+ *   ALL POINTERS ARE DEVICE POINTERS on the handle's device.  n_structs: 1..GNEP_NOALLOC_MAX_STRUCTS, more is refused
+ *   with GNEP_ERANGE (split the batch, or use gnep_set_targets + gnep_loss_and_grad); atom_offsets[n_structs+1] as in
+ *   gnep_load_batch; energy[n_structs], force[3 N], virial[6 n_structs]: fp32, caller atom order, exactly what
+ *   gnep_predict writes; Eref / Fref / Wref: fp64 like gnep_set_targets, NULL drops that term (R39; its prediction may
+ *   then be NULL too); terms: 4 floats {L, t_e, t_f, t_v}, written when the kernel has run (stream order).
+ * Every call on a GPU shares the one scratch array, which keeps the last call's contents (the call rewrites all it
+ * reads and clears its ticket counter): calls that overlap on the GPU -- different streams, or handles on different
+ * streams -- race on it; serialise them. */
+#define GNEP_NOALLOC_MAX_STRUCTS 8192
+int gnep_loss_terms_noalloc(gnep_handle *h, int32_t n_structs, const int32_t *atom_offsets, const float *energy,
+                            const float *force, const float *virial, const double *Eref, const double *Fref,
+                            const double *Wref, float *terms);
+
 /* Measured plain-FP32 FMA peak of the device (the denominator of the ALU roofline next to the
  * nominal 148 SM x 128 lanes x 2 x clock): a register-only FMA microbenchmark on every SM of the handle's device that
  * runs for about min_ms milliseconds on the handle's stream (synchronises it).  tflops: HOST, achieved TFLOP/s

@@ -20,7 +20,7 @@ EXPORTS = ["gnep_create", "gnep_destroy", "gnep_num_params", "gnep_num_descripto
            "gnep_get_opt_state", "gnep_set_opt_state", "gnep_batch_info", "gnep_launch_count",
            "gnep_set_profiling", "gnep_phase_times", "gnep_last_error", "gnep_set_global_norm", "gnep_set_grad",
            "gnep_create_shared", "gnep_lr_schedule", "gnep_evaluate", "gnep_measure_fp32_peak", "gnep_set_weights",
-           "gnep_loss_norms", "gnep_set_global_norms"]
+           "gnep_loss_norms", "gnep_set_global_norms", "gnep_loss_terms_noalloc"]
 
 ERRORS = {-1: "GNEP_EINVAL", -2: "GNEP_ESTATE", -3: "GNEP_ECUDA", -4: "GNEP_ENOMEM", -5: "GNEP_ERANGE",
           -6: "GNEP_ENONFINITE"}
@@ -86,6 +86,7 @@ def load_library(build_if_missing=True):
     L.gnep_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
     L.gnep_measure_fp32_peak.argtypes = [vp, C.c_double] + [C.POINTER(C.c_double)] * 3
     L.gnep_set_profiling.argtypes = [vp, C.c_int]
+    L.gnep_loss_terms_noalloc.argtypes = [vp, C.c_int32] + [vp] * 8
     L.gnep_phase_times.argtypes = [vp, C.POINTER(C.c_char_p), C.POINTER(C.c_float), C.c_int32, C.POINTER(C.c_int32)]
     for name in EXPORTS:
         if name != "gnep_last_error":
@@ -327,6 +328,24 @@ class Gnep:
         v = [C.c_double() for _ in range(3)]
         self._ck(self._L.gnep_measure_fp32_peak(self._h, float(min_ms), *[C.byref(x) for x in v]))
         return dict(tflops=v[0].value, ms=v[1].value, implied_sm_mhz=v[2].value)
+
+    def loss_terms_noalloc(self, atom_offsets, energy, force, virial, Eref, Fref, Wref, terms):
+        """gnep_loss_terms_noalloc: {L, t_e, t_f, t_v} of device-resident predictions against device-resident references
+        into the 4-float device tensor `terms`; allocates nothing and does not synchronise.  Every argument must already
+        be a contiguous CUDA tensor of the right dtype (int32 offsets, float32 predictions, float64 references) or None:
+        nothing is converted or copied here."""
+        def dev(a, dtype):
+            if a is None:
+                return None
+            p, d, _k = _out_ptr(a, dtype)            # (raises on a dtype / contiguity mismatch instead of copying)
+            if d != 1:
+                raise TypeError("gnep_loss_terms_noalloc takes CUDA tensors only")
+            return p
+        n_structs = int(atom_offsets.numel()) - 1
+        self._ck(self._L.gnep_loss_terms_noalloc(self._h, n_structs, dev(atom_offsets, np.int32), dev(energy, np.float32),
+                                                 dev(force, np.float32), dev(virial, np.float32), dev(Eref, np.float64),
+                                                 dev(Fref, np.float64), dev(Wref, np.float64), dev(terms, np.float32)))
+        return terms
 
     def set_profiling(self, on):
         self._ck(self._L.gnep_set_profiling(self._h, int(on)))

@@ -18,10 +18,40 @@
 #include "angular_warp_kernels.cuh"
 #include "reduce_kernels.cuh"
 #include "peak_kernels.cuh"
+#include "noalloc_kernels.cuh"
+#include <mutex>
+
+// Scratch of gnep_loss_terms_noalloc: per-structure partial sums + the ticket counter.  File-scope device memory
+// (192 KiB + 256 B; every GPU that loads the library holds it until exit) so that the entry point allocates nothing.
+// In host code this NAME is only a stand-in for the symbol: the kernel gets the device address that
+// cudaGetSymbolAddress returns (noalloc_scratch(), once per device).
+static __device__ __align__(256) double g_noalloc_scratch[NOALLOC_SCRATCH_DOUBLES];
 
 namespace {
 
 thread_local std::string g_create_error;
+
+// device address of g_noalloc_scratch on device `dev`: looked up once per device, with that device current
+std::mutex g_noalloc_mu;
+double *g_noalloc_ptr[64] = {};
+cudaError_t noalloc_scratch(int dev, double **out) {
+  if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lk(g_noalloc_mu);
+  if (!g_noalloc_ptr[dev]) {
+    int cur = -1;
+    cudaError_t e = cudaGetDevice(&cur);
+    if (e != cudaSuccess) return e;
+    if (cur != dev && (e = cudaSetDevice(dev)) != cudaSuccess) return e;
+    double *p = nullptr;
+    e = cudaGetSymbolAddress((void **)&p, g_noalloc_scratch);
+    if (cur != dev) cudaSetDevice(cur);
+    if (e != cudaSuccess) return e;
+    if (!p) return cudaErrorInvalidSymbol;
+    g_noalloc_ptr[dev] = p;
+  }
+  *out = g_noalloc_ptr[dev];
+  return cudaSuccess;
+}
 
 struct Phase { const char *name; cudaEvent_t ev; };
 
@@ -1119,6 +1149,27 @@ int gnep_measure_fp32_peak(gnep_handle *h, double min_ms, double *tflops, double
   if (ms_out) *ms_out = ms;
   if (sm_mhz) *sm_mhz = *tflops * 1e12 / (2.0 * 128.0 * h->num_sms) / 1e6;   // the clock this rate implies at 128 lanes / SM
   return GNEP_OK;
+}
+
+int gnep_loss_terms_noalloc(gnep_handle *h, int32_t n_structs, const int32_t *atom_offsets, const float *energy,
+                            const float *force, const float *virial, const double *Eref, const double *Fref,
+                            const double *Wref, float *terms) {
+  if (!h) return fail(h, GNEP_EINVAL, "null handle");
+  if (n_structs < 1) return fail(h, GNEP_EINVAL, "n_structs must be at least 1");
+  if (n_structs > NOALLOC_MAX_STRUCTS)
+    return fail(h, GNEP_ERANGE, "gnep_loss_terms_noalloc: " + std::to_string(n_structs) + " structures exceed the fixed scratch of " +
+                                    std::to_string(NOALLOC_MAX_STRUCTS) + " (split the batch, or use gnep_set_targets + gnep_loss_and_grad)");
+  if (!atom_offsets || !terms) return fail(h, GNEP_EINVAL, "null atom_offsets / terms");
+  if ((Eref && !energy) || (Fref && !force) || (Wref && !virial)) return fail(h, GNEP_EINVAL, "a reference without its prediction");
+  double *scratch = nullptr;
+  CK(noalloc_scratch(h->device, &scratch));
+  // the array keeps the last call's contents: the partial sums are all rewritten, the ticket must start at zero
+  CK(cudaMemsetAsync(scratch + 3 * NOALLOC_MAX_STRUCTS, 0, sizeof(unsigned), h->stream));
+  NoAllocLoss lc;
+  lc.S = n_structs; lc.loss_mode = h->ds.loss_mode;
+  lc.lam_e = Eref ? h->spec.lambda_e : 0.0; lc.lam_f = Fref ? h->spec.lambda_f : 0.0; lc.lam_v = Wref ? h->spec.lambda_v : 0.0;
+  LAUNCH(h, k_loss_terms_noalloc, n_structs, 128, 0, lc, atom_offsets, energy, force, virial, Eref, Fref, Wref, scratch, terms);
+  return check_launch(h);
 }
 
 int gnep_launch_count(const gnep_handle *h, int64_t *n) {
