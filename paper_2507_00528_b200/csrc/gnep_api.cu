@@ -19,6 +19,7 @@
 #include "reduce_kernels.cuh"
 #include "peak_kernels.cuh"
 #include "noalloc_kernels.cuh"
+#include "net_small_kernels.cuh"
 #include <mutex>
 
 // Scratch of gnep_loss_terms_noalloc: per-structure partial sums + the ticket counter.  File-scope device memory
@@ -91,6 +92,7 @@ struct gnep_handle {
   int *tilesA = nullptr;       // slot-group path: 32 atoms of one central species per tile, sorted by neighbour counts; -1 = idle lane
   int n_tilesA = 0, grid_adj = 0, grid_cg = 0, occ_adj = 1, occ_cg = 1, occ_S = 4;
   bool fuse_adam = false; float fuse_b1 = 0.f, fuse_b2 = 0.f, fuse_eps = 0.f;   // set while gnep_train_epochs captures its graph
+  bool net_small = false;                  // small batches: the network on plain FMAs, warp per atom (net_small_kernels.cuh)
   bool rad_split = false;                  // radial a3/a5 with RAD_SPLIT lanes per atom (small batches)
   int ta_ang = ANG_TA, ta_frc = FRC_TA;   // atoms per warp of the warp-tile sweeps: fewer for small batches, so that every SM gets warps
   int *segA = nullptr, *atomA = nullptr;   // warp-tile path: angular list with every (atom, J) segment padded to 4 pairs
@@ -262,6 +264,7 @@ int configure_kernels(gnep_handle *h) {
   if (gradw_nraw(d) < 2) return fail(h, GNEP_EINVAL, "model too large for shared memory staging (n_descriptors)");
   RET_IF(set_smem(h, k_gradw_tc, smem_gradw(d)));
   RET_IF(set_smem(h, k_cgrad_radial, smem_cgrad_rad(d)));
+  RET_IF(set_smem(h, k_net_small_fwd, 0)); RET_IF(set_smem(h, k_net_small_bwd, 0));   // (used only when the model fits: net_small)
   return GNEP_OK;
 }
 
@@ -341,8 +344,12 @@ LossCfg loss_cfg(const gnep_handle *h) {
 int enqueue_forward(gnep_handle *h) {
   const DevSpec &d = h->ds;
   RET_IF(enqueue_descriptors(h));
-  LAUNCH(h, k_net_tc<false>, h->n_cta_net, 256, smem_net_fwd(d), d, h->sm, h->theta, h->qscale, h->q, h->x, h->Ei, h->Ep, h->etil,
-         (const int *)nullptr, (const float *)nullptr, (const float *)nullptr, (float *)nullptr, (float *)nullptr);
+  if (h->net_small) {
+    LAUNCH(h, k_net_small_fwd, h->n_gw, NS_WARPS * 32, sizeof(float) * net_small_fwd_floats(d), d, h->sm, h->theta, h->qscale, h->q, h->x, h->Ei, h->Ep, h->etil);
+  } else {
+    LAUNCH(h, k_net_tc<false>, h->n_cta_net, 256, smem_net_fwd(d), d, h->sm, h->theta, h->qscale, h->q, h->x, h->Ei, h->Ep, h->etil,
+           (const int *)nullptr, (const float *)nullptr, (const float *)nullptr, (float *)nullptr, (float *)nullptr);
+  }
   mark(h, "a2_network_forward");
   DISPATCH_ANG(d, auto kp = k_angular_force<KT, LMAX>; LAUNCH(h, kp, cdiv(h->N, FRC_WARPS * h->ta_frc), FRC_WARPS * 32, smem_ang_force(d), d, h->N, h->ta_frc, h->type_s, h->segAu, h->atomAu, h->pairAu, h->theta, h->Ep, h->Sn, h->Beta, h->fpair));
   mark(h, "a3_angular_force");
@@ -381,10 +388,16 @@ int enqueue_backward(gnep_handle *h) {
   } else
   DISPATCH_ANG(d, auto ka = k_angular_adj<KT, LMAX>; LAUNCH(h, ka, h->grid_adj, 32 * ang_warps(d), smem_ang_adj(d), d, h->n_tilesA, h->tilesA, h->type_s, h->struct_s, h->segAu, h->pairAu, h->theta, h->u, h->omega, h->scales, h->Sn, h->Beta, h->Tn, h->D, h->partialCA));
   mark(h, "a5_angular_adjoint");
-  LAUNCH(h, k_net_tc<true>, h->n_cta_net, 256, smem_net_bwd(d), d, h->sm, h->theta, h->qscale, h->D, h->x, h->eat, h->Ep, (float *)nullptr,
-         h->struct_s, h->e_s, h->scales, h->pbuf, h->gbar);
-  mark(h, "a6_network_backward");
-  LAUNCH(h, k_gradw_tc, h->n_gw, GW_THREADS, smem_gradw(d), d, h->sm, gradw_nraw(d), h->theta, h->qscale, h->eat, h->q, h->D, h->x, h->pbuf, h->partialW, h->partialB);
+  if (h->net_small) {   // network backward and its parameter-gradient partials in one launch
+    LAUNCH(h, k_net_small_bwd, h->n_gw, NS_WARPS * 32, sizeof(float) * net_small_bwd_floats(d), d, h->sm, h->theta, h->qscale, h->q, h->D, h->x, h->Ep,
+           h->struct_s, h->e_s, h->scales, h->gbar, h->partialW, h->partialB);
+    mark(h, "a6_network_backward");
+  } else {
+    LAUNCH(h, k_net_tc<true>, h->n_cta_net, 256, smem_net_bwd(d), d, h->sm, h->theta, h->qscale, h->D, h->x, h->eat, h->Ep, (float *)nullptr,
+           h->struct_s, h->e_s, h->scales, h->pbuf, h->gbar);
+    mark(h, "a6_network_backward");
+    LAUNCH(h, k_gradw_tc, h->n_gw, GW_THREADS, smem_gradw(d), d, h->sm, gradw_nraw(d), h->theta, h->qscale, h->eat, h->q, h->D, h->x, h->pbuf, h->partialW, h->partialB);
+  }
   mark(h, "a6_w0_gradient");
   LAUNCH(h, k_cgrad_radial, h->n_chunks, CR_THREADS, smem_cgrad_rad(d), d, h->sm, h->gbar, h->Ep, h->M1, h->M2, h->partialCR);
   mark(h, "a7_radial_cgrad");
@@ -864,6 +877,10 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     CKT(cudaStreamSynchronize(st));
     tfree();
     // ---- work decomposition of the network / gradient kernels ----
+    // (small batches -- see below -- run the network on plain FMAs, one warp per atom, with short atom ranges per CTA)
+    bool small = N < 2 * h->num_sms * RAD_THREADS;
+    if (const char *e = getenv("GNEP_SMALL_BATCH")) small = atoi(e) != 0;
+    h->net_small = small && d.Nn <= 128 && d.Ndes <= 128 && sizeof(float) * net_small_bwd_floats(d) <= 200 * 1024;
     int tiles_total = 0;
     for (int t = 0; t < T; ++t) tiles_total += cdiv(h->sm.start[t + 1] - h->sm.start[t], 128);
     h->sm.cta_base[0] = 0; h->sm.chunk_base[0] = 0; h->sm.gw_base[0] = 0;
@@ -881,6 +898,7 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
       // k_gradw_tc: one contiguous atom range per CTA
       int gwant = nt > 0 ? std::max(1, std::min(cdiv(nt, 4 * GW_KS), (int)((double)h->num_sms * nt / std::max(N, 1) + 0.5))) : 0;
       int ga = gwant > 0 ? pad_to(cdiv(nt, gwant), GW_KS) : GW_KS;
+      if (h->net_small) ga = NS_ATOMS;             // k_net_small_fwd / bwd: short contiguous atom ranges of one species
       h->sm.gw_atoms[t] = ga;
       h->sm.gw_base[t + 1] = h->sm.gw_base[t] + (nt > 0 ? cdiv(nt, ga) : 0);
     }
@@ -898,8 +916,6 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     // large-batch mappings (one thread per atom in the radial sweeps, ANG_TA atoms per warp in the angular ones): below
     // two CTAs per SM of the radial kernels the atom tiles shrink until there are about four CTAs per SM and the radial
     // force / adjoint sweeps use RAD_SPLIT lanes per atom.  GNEP_SMALL_BATCH=0/1 forces either set (tests run both).
-    bool small = N < 2 * h->num_sms * RAD_THREADS;
-    if (const char *e = getenv("GNEP_SMALL_BATCH")) small = atoi(e) != 0;
     h->ta_ang = small ? std::max(1, std::min(ANG_TA, cdiv(N, 4 * h->num_sms * ANG_WARPS))) : ANG_TA;
     h->ta_frc = small ? std::max(1, std::min(FRC_TA, cdiv(N, 5 * h->num_sms * FRC_WARPS))) : FRC_TA;
     h->rad_split = small;
