@@ -363,9 +363,9 @@ int enqueue_forward(gnep_handle *h) {
   }
   mark(h, "a3_radial_force");
   // terms[5..6] = the Adam bias corrections of this step, terms[7] = the ticket counter of k_struct_reduce (zero at rest)
-  const AdamPre ap = {h->step_dev, h->terms + 5, h->fuse_b1, h->fuse_b2, h->fuse_adam ? 1 : 0};
+  const AdamPre ap = {h->step_dev, h->terms + 5, h->fuse_b1, h->fuse_b2, std::log((double)h->fuse_b1), std::log((double)h->fuse_b2), h->fuse_adam ? 1 : 0};
   if (h->S > 0) {
-    LAUNCH(h, k_struct_reduce, h->S + LOSS_T2_CTAS, 128, 0, loss_cfg(h), h->srange, h->Ei, h->Fat, h->Wat, h->Eref, h->Fref_s, h->Wref, h->wgt, h->Es, h->Ws, h->e_s, h->u, h->omega, h->parts,
+    LAUNCH(h, k_struct_reduce, h->S <= 4 ? 1 : h->S + LOSS_T2_CTAS, 128, 0, loss_cfg(h), h->srange, h->Ei, h->Fat, h->Wat, h->Eref, h->Fref_s, h->Wref, h->wgt, h->Es, h->Ws, h->e_s, h->u, h->omega, h->parts,
            (unsigned *)(h->terms + 7), h->theta, h->terms, h->scales, ap);
   } else {
     LAUNCH(h, k_loss_final, 1, 128, 0, loss_cfg(h), h->parts, h->theta, h->terms, h->scales, ap);

@@ -25,11 +25,16 @@ __device__ __forceinline__ void block_reduce_d(double (&v)[NV], double *sh /*[NV
     if (lane == 0) sh[i * nw + warp] = x;
   }
   __syncthreads();
+  if (nw == 4) {                     // the usual 128-thread CTA: independent chains, no loop
 #pragma unroll
-  for (int i = 0; i < NV; ++i) {
-    double x = 0.0;
-    for (int w = 0; w < nw; ++w) x += sh[i * nw + w];
-    v[i] = x;
+    for (int i = 0; i < NV; ++i) v[i] = (sh[i * 4] + sh[i * 4 + 1]) + (sh[i * 4 + 2] + sh[i * 4 + 3]);
+  } else {
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      double x = 0.0;
+      for (int w = 0; w < nw; ++w) x += sh[i * nw + w];
+      v[i] = x;
+    }
   }
   __syncthreads();
 }
@@ -37,7 +42,10 @@ __device__ __forceinline__ void block_reduce_d(double (&v)[NV], double *sh /*[NV
 // Adam bookkeeping folded into the epoch's kernels when a whole training step is enqueued (gnep_train_epochs): the last
 // CTA of k_struct_reduce advances the step counter and writes the two bias corrections (fp64 pow, once per step), and
 // k_grad_reduce applies the update to the parameter it has just reduced.  `on == 0`: plain loss / gradient evaluation.
-struct AdamPre { long long *step; float *bc; float beta1, beta2; int on; };
+// lnb1, lnb2 = log(beta) from the host in fp64: 1 - beta^t = -expm1(t log beta), whose fp32 evaluation is accurate to
+// ~1e-7 RELATIVE also where beta^t is close to 1 (a float pow would lose the difference; a double pow costs a
+// microsecond of dependent fp64 instructions at the end of a kernel that one thread runs alone).
+struct AdamPre { long long *step; float *bc; float beta1, beta2; double lnb1, lnb2; int on; };
 struct AdamFuse { float *m, *v; const float *bc, *lr; float beta1, beta2, eps; int on; };
 
 // a4: loss terms {L, t_e, t_f, t_v, t_2} (Eq.9-12 + L2) and the per-term seed multipliers, by ONE CTA (any size)
@@ -57,22 +65,34 @@ __device__ __forceinline__ double theta_sq(const float *__restrict__ theta, int 
   return (w[0] + w[1]) + (w[2] + w[3]);
 }
 
-__device__ __forceinline__ void loss_final(const LossCfg &lc, const double *parts, const double *t2parts, int nt2,
-                                           const float *__restrict__ theta, float *__restrict__ terms,
+// nt2 > 0: theta^2 arrives as nt2 slices; nt2 == 0: the CTA sums it here; nt2 < 0: this thread's share is t2_own.
+// step0 = the step counter as read at the top of the kernel (its load is off the critical path there).
+__device__ __forceinline__ void loss_final(const LossCfg &lc, const double *parts, const double *t2parts, int nt2, double t2_own,
+                                           long long step0, const float *__restrict__ theta, float *__restrict__ terms,
                                            float *__restrict__ scales, const AdamPre &ap, double *sh) {
   double v[4] = {0, 0, 0, 0};
   for (int s = threadIdx.x; s < lc.S; s += blockDim.x) { v[0] += __ldcg(parts + s * 3); v[1] += __ldcg(parts + s * 3 + 1); v[2] += __ldcg(parts + s * 3 + 2); }
   if (nt2 > 0) { if (threadIdx.x == 0) for (int i = 0; i < nt2; ++i) v[3] += __ldcg(t2parts + i); }
-  else v[3] = theta_sq(theta, lc.P, threadIdx.x, blockDim.x);
+  else if (nt2 == 0) v[3] = theta_sq(theta, lc.P, threadIdx.x, blockDim.x);
+  else v[3] = t2_own;
   block_reduce_d<4>(v, sh);
-  const long long t = ap.on ? *ap.step + 1 : 0;       // read by every thread before thread 0 advances it
-  __syncthreads();
-  if (ap.on && threadIdx.x == 32) ap.bc[1] = (float)(1.0 - pow((double)ap.beta2, (double)t));   // the two fp64 pows side by side
+  const long long t = step0 + 1;
+  if (ap.on && threadIdx.x == 32) {                    // bias corrections 1 - beta^t of this step
+    ap.bc[0] = -expm1f((float)((double)t * ap.lnb1));
+    ap.bc[1] = -expm1f((float)((double)t * ap.lnb2));
+  }
+  // the four fp64 divisions side by side on lanes 0..3 (a division is ~40 dependent instructions), gathered by lane 0
+  double term = 0.0;
+  if (threadIdx.x < 4) {
+    const int i = threadIdx.x;
+    const double den = i == 0 ? lc.ZE : i == 1 ? 3.0 * lc.ZF : i == 2 ? 6.0 * lc.ZV : (double)lc.P;
+    const double num = i == 0 ? v[0] : i == 1 ? v[1] : i == 2 ? v[2] : lc.l2_share * v[3];
+    term = den > 0 ? num / den : 0.0;
+  }
+  if (threadIdx.x < 32) {
+    const double te = __shfl_sync(0xffffffffu, term, 0), tf = __shfl_sync(0xffffffffu, term, 1);
+    const double tv = __shfl_sync(0xffffffffu, term, 2), t2 = __shfl_sync(0xffffffffu, term, 3);
   if (threadIdx.x == 0) {
-    double te = lc.ZE > 0 ? v[0] / lc.ZE : 0.0;
-    double tf = lc.ZF > 0 ? v[1] / (3.0 * lc.ZF) : 0.0;
-    double tv = lc.ZV > 0 ? v[2] / (6.0 * lc.ZV) : 0.0;
-    double t2 = lc.l2_share * v[3] / lc.P;
     double L, sc[4] = {1, 1, 1, 1};
     if (lc.loss_mode == 0) L = lc.lam_e * te + lc.lam_f * tf + lc.lam_v * tv + lc.lam_2 * t2;
     else {
@@ -82,7 +102,8 @@ __device__ __forceinline__ void loss_final(const LossCfg &lc, const double *part
     }
     terms[0] = (float)L; terms[1] = (float)te; terms[2] = (float)tf; terms[3] = (float)tv; terms[4] = (float)t2;
     for (int i = 0; i < 4; ++i) scales[i] = (float)sc[i];
-    if (ap.on) { *ap.step = t; ap.bc[0] = (float)(1.0 - pow((double)ap.beta1, (double)t)); }
+    if (ap.on) *ap.step = t;
+  }
   }
 }
 
@@ -102,8 +123,13 @@ k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const 
                 const float *__restrict__ theta, float *__restrict__ terms, float *__restrict__ scales, AdamPre ap) {
   __shared__ double sh[8 * 4];
   __shared__ int last;
-  const int s = blockIdx.x;
+  // A batch of a few structures (size-1 mini-batches) is launched as ONE CTA that walks all structures and then
+  // writes the loss terms itself: no ticket, no fences, no tail of a second CTA in the chain of dependent launches.
+  const bool solo = gridDim.x == 1;
   double *t2parts = parts + (size_t)lc.S * 3;
+  const long long step0 = ap.on ? *ap.step : 0;         // (every CTA reads it before the last one advances it)
+  const double t2_own = solo ? theta_sq(theta, lc.P, threadIdx.x, blockDim.x) : 0.0;   // loads overlap the first structure's
+  for (int s = blockIdx.x; s < (solo ? lc.S : blockIdx.x + 1); ++s) {
   if (s >= lc.S) {                          // a theta^2 slice
     double w[1] = {theta_sq(theta, lc.P, (s - lc.S) * blockDim.x + threadIdx.x, LOSS_T2_CTAS * blockDim.x)};
     block_reduce_d<1>(w, sh);
@@ -115,7 +141,7 @@ k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const 
     __syncthreads();
     if (!last) return;
     __threadfence();
-    loss_final(lc, parts, t2parts, LOSS_T2_CTAS, theta, terms, scales, ap, sh);
+    loss_final(lc, parts, t2parts, LOSS_T2_CTAS, 0.0, step0, theta, terms, scales, ap, sh);
     if (threadIdx.x == 0) *ticket = 0u;
     return;
   }
@@ -123,6 +149,13 @@ k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const 
   int Ns = 0;
   const double we = wgt[s], wf = wgt[lc.S + s], wv = wgt[2 * lc.S + s];
   const float cu = lc.hasF && lc.ZF > 0 ? (float)(2.0 * lc.lam_f * wf / (3.0 * lc.ZF)) : 0.f;
+  double eref = 0.0, wref[6] = {0, 0, 0, 0, 0, 0};      // requested now, used by thread 0 after the reduction
+  if (threadIdx.x == 0) {
+    if (lc.hasE) eref = Eref[s];
+    if (lc.hasV)
+#pragma unroll
+      for (int c = 0; c < 6; ++c) wref[c] = Wref[s * 6 + c];
+  }
   for (int t = 0; t < lc.T; ++t) {
     int b = srange[(s * lc.T + t) * 2], e = srange[(s * lc.T + t) * 2 + 1];
     Ns += e - b;
@@ -139,33 +172,44 @@ k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const 
   }
   block_reduce_d<8>(v, sh);
   if (threadIdx.x == 0) {
-    double ns = (double)Ns;
     Es[s] = v[0];
+    // per-atom residuals through ONE reciprocal of N_s (an fp64 division is ~40 dependent instructions on this one thread)
+    const double inv_ns = Ns > 0 ? 1.0 / (double)Ns : 0.0;
     double pe = 0.0, pv = 0.0, es = 0.0;
     if (lc.hasE && Ns > 0 && lc.ZE > 0) {
-      double dE = v[0] / ns - Eref[s] / ns;
+      const double dE = (v[0] - eref) * inv_ns;
       pe = we * dE * dE;
-      es = 2.0 * lc.lam_e * we * dE / (lc.ZE * ns);
+      es = (2.0 * lc.lam_e * we / lc.ZE) * inv_ns * dE;
     }
     e_s[s] = (float)es;
+    const bool onV = lc.hasV && Ns > 0 && lc.ZV > 0;
+    const double k_om = onV ? (2.0 * lc.lam_v * wv / (6.0 * lc.ZV)) * inv_ns : 0.0;
+#pragma unroll
     for (int c = 0; c < 6; ++c) {
       Ws[s * 6 + c] = v[1 + c];
       double om = 0.0;
-      if (lc.hasV && Ns > 0 && lc.ZV > 0) {
-        double dW = (v[1 + c] - Wref[s * 6 + c]) / ns;
+      if (onV) {
+        const double dW = (v[1 + c] - wref[c]) * inv_ns;
         pv += wv * dW * dW;
-        om = 2.0 * lc.lam_v * wv * dW / (6.0 * lc.ZV * ns);
+        om = k_om * dW;
       }
       omega[s * 6 + c] = (float)om;
     }
     parts[s * 3 + 0] = pe; parts[s * 3 + 1] = wf * v[7]; parts[s * 3 + 2] = pv;
-    __threadfence();                                           // parts visible before the ticket is taken
-    last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+    if (!solo) {
+      __threadfence();                                         // parts visible before the ticket is taken
+      last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+    }
   }
   __syncthreads();
+  }   // structures of this CTA
+  if (solo) {                               // (parts were written by this CTA: ordered by the barrier above)
+    loss_final(lc, parts, nullptr, -1, t2_own, step0, theta, terms, scales, ap, sh);
+    return;
+  }
   if (!last) return;
   __threadfence();
-  loss_final(lc, parts, t2parts, LOSS_T2_CTAS, theta, terms, scales, ap, sh);
+  loss_final(lc, parts, t2parts, LOSS_T2_CTAS, 0.0, step0, theta, terms, scales, ap, sh);
   if (threadIdx.x == 0) *ticket = 0u;
 }
 
@@ -174,7 +218,7 @@ __global__ void __launch_bounds__(128)
 k_loss_final(LossCfg lc, const double *parts, const float *__restrict__ theta, float *__restrict__ terms,
              float *__restrict__ scales, AdamPre ap) {
   __shared__ double sh[8 * 4];
-  loss_final(lc, parts, nullptr, 0, theta, terms, scales, ap, sh);
+  loss_final(lc, parts, nullptr, 0, 0.0, ap.on ? *ap.step : 0, theta, terms, scales, ap, sh);
 }
 
 // a8: grad[p] = sum over the partial buffers that cover p (fixed order, fp64) + 2 lam_2 s2 theta_p / P.
