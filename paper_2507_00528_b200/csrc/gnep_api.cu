@@ -345,7 +345,7 @@ int enqueue_forward(gnep_handle *h) {
   const DevSpec &d = h->ds;
   RET_IF(enqueue_descriptors(h));
   if (h->net_small) {
-    LAUNCH(h, k_net_small_fwd, h->n_gw, NS_WARPS * 32, sizeof(float) * net_small_fwd_floats(d), d, h->sm, h->theta, h->qscale, h->q, h->x, h->Ei, h->Ep, h->etil);
+    LAUNCH(h, k_net_small_fwd, h->n_gw, NS_THREADS, sizeof(float) * net_small_fwd_floats(d), d, h->sm, h->theta, h->qscale, h->q, h->x, h->Ei, h->Ep, h->etil);
   } else {
     LAUNCH(h, k_net_tc<false>, h->n_cta_net, 256, smem_net_fwd(d), d, h->sm, h->theta, h->qscale, h->q, h->x, h->Ei, h->Ep, h->etil,
            (const int *)nullptr, (const float *)nullptr, (const float *)nullptr, (float *)nullptr, (float *)nullptr);
@@ -389,7 +389,7 @@ int enqueue_backward(gnep_handle *h) {
   DISPATCH_ANG(d, auto ka = k_angular_adj<KT, LMAX>; LAUNCH(h, ka, h->grid_adj, 32 * ang_warps(d), smem_ang_adj(d), d, h->n_tilesA, h->tilesA, h->type_s, h->struct_s, h->segAu, h->pairAu, h->theta, h->u, h->omega, h->scales, h->Sn, h->Beta, h->Tn, h->D, h->partialCA));
   mark(h, "a5_angular_adjoint");
   if (h->net_small) {   // network backward and its parameter-gradient partials in one launch
-    LAUNCH(h, k_net_small_bwd, h->n_gw, NS_WARPS * 32, sizeof(float) * net_small_bwd_floats(d), d, h->sm, h->theta, h->qscale, h->q, h->D, h->x, h->Ep,
+    LAUNCH(h, k_net_small_bwd, h->n_gw, NS_THREADS, sizeof(float) * net_small_bwd_floats(d), d, h->sm, h->theta, h->qscale, h->q, h->D, h->x, h->Ep,
            h->struct_s, h->e_s, h->scales, h->gbar, h->partialW, h->partialB);
     mark(h, "a6_network_backward");
   } else {

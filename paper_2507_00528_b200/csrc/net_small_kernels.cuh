@@ -3,9 +3,11 @@
 // The tensor-core kernels of net_tc_kernels.cuh work on 128-atom tiles: a mini-batch of a few hundred atoms (the paper
 // trains with batch size 1) gives them one or two tiles, and each launch then costs its fixed chain of TMEM
 // allocation, weight staging and commit / wait round trips (13-15 us for a single tile, three launches per step).
-// Here ONE WARP works on one atom (lane = neuron in the first contraction, lane = descriptor in the second), every
-// species' network sits in shared memory (row stride odd: the column reads of the second contraction are
-// conflict-free), and the backward kernel also forms the parameter-gradient partials, so a6 is one launch, not two.
+// Here a group of 128 THREADS works on one atom (thread = neuron in the first contraction, thread = descriptor in the
+// second: every dot product of the two contractions runs at once), a CTA holds four such groups and one species' network
+// in shared memory (row stride odd: row and column reads are both conflict-free), and the backward kernel also forms the
+// parameter-gradient partials, so a6 is one launch, not two.  With so few warps per SM these kernels are bound by the
+// number of instructions a warp executes one after the other: the mapping keeps that number small.
 // Same formulas as net_tc_kernels.cuh (Eq.D1.1, D1.5-D1.17, C3.8), plain fp32 dot products.
 // Chosen by the host for small batches when the networks fit (gnep_api.cu); results agree with the tensor-core path to
 // rounding and both are parity-tested against the oracle (tests/test_gpu_parity.py runs its core cases under both).
@@ -13,109 +15,109 @@
 #include "common.cuh"
 #include "net_tc_kernels.cuh"
 
-#define NS_WARPS 4          // warps (= atoms in flight) per CTA
-#define NS_ATOMS 4          // atoms per CTA (contiguous, one species): SpeciesMap.gw_atoms of a small batch
+#define NS_GROUP 128        // threads per atom
+#define NS_ATOMS 4          // atoms per CTA and round (contiguous, one species): SpeciesMap.gw_atoms of a small batch
+#define NS_THREADS (NS_GROUP * NS_ATOMS)
 
 // W0 of one species (Nn x Ndes, row-major, contiguous at `net`) into shared memory with row stride ld; element
 // x = mu * Ndes + nu is walked with incremental (mu, nu): no integer division in the loop, loads independent
 __device__ __forceinline__ void ns_stage_w0(float *W0s, const float *__restrict__ net, int Nn, int Ndes, int ld) {
-  const int nW = Nn * Ndes, step = NS_WARPS * 32;
+  const int nW = Nn * Ndes;
   int mu = threadIdx.x / Ndes, nu = threadIdx.x - mu * Ndes;
-  const int dmu = step / Ndes, dnu = step - dmu * Ndes;
+  const int dmu = NS_THREADS / Ndes, dnu = NS_THREADS - dmu * Ndes;
 #pragma unroll 4
-  for (int x = threadIdx.x; x < nW; x += step) {
+  for (int x = threadIdx.x; x < nW; x += NS_THREADS) {
     W0s[mu * ld + nu] = net[x];
     mu += dmu; nu += dnu;
     if (nu >= Ndes) { nu -= Ndes; ++mu; }
   }
 }
-// sum_i w[i * ws] * v[i * vs], i < n, on four independent chains (the loads of a chain step do not wait for the FMAs)
-__device__ __forceinline__ float ns_dot(const float *w, int ws, const float *v, int vs, int n) {
+// sum_i w[i * ws] * v[i], i < n, on four independent chains (the loads of a chain step do not wait for the FMAs)
+__device__ __forceinline__ float ns_dot(const float *w, int ws, const float *v, int n) {
   float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
   int i = 0;
-  for (; i + 3 < n; i += 4) {
-    const float w0 = w[i * ws], w1 = w[(i + 1) * ws], w2 = w[(i + 2) * ws], w3 = w[(i + 3) * ws];
-    const float v0 = v[i * vs], v1 = v[(i + 1) * vs], v2 = v[(i + 2) * vs], v3 = v[(i + 3) * vs];
-    a0 = fmaf(w0, v0, a0); a1 = fmaf(w1, v1, a1); a2 = fmaf(w2, v2, a2); a3 = fmaf(w3, v3, a3);
+  for (; i + 3 < n; i += 4, w += 4 * ws) {
+    const float w0 = w[0], w1 = w[ws], w2 = w[2 * ws], w3 = w[3 * ws];
+    const float4 v4 = make_float4(v[i], v[i + 1], v[i + 2], v[i + 3]);
+    a0 = fmaf(w0, v4.x, a0); a1 = fmaf(w1, v4.y, a1); a2 = fmaf(w2, v4.z, a2); a3 = fmaf(w3, v4.w, a3);
   }
-  for (; i < n; ++i) a0 = fmaf(w[i * ws], v[i * vs], a0);
+  for (; i < n; ++i, w += ws) a0 = fmaf(w[0], v[i], a0);
   return (a0 + a1) + (a2 + a3);
 }
 
-// shared-memory floats of the forward kernel: cR[t] as [jk][16], the species' network, q_scale, per-warp rows
+// shared-memory floats of the forward kernel: cR[t] as [jk][16], the species' network, q_scale, per-atom rows
 __host__ __device__ inline size_t net_small_fwd_floats(const DevSpec &sp) {
   return (size_t)sp.T * sp.KRp * 16 + (size_t)sp.Nn * sp.ldW + (size_t)(2 * sp.Nn + 1) + sp.Ndes +
-         (size_t)NS_WARPS * (2 * sp.Ndes + sp.Nn);
+         (size_t)NS_ATOMS * (2 * sp.Ndes + sp.Nn + 4);
 }
-// backward kernel: the species' network, w1, q_scale, per-warp rows sD, sG (Ndes each) and Hc, Av, Bv (Nn each), the W0
-// gradient accumulator of the CTA and the cross-warp sums of the b0 / w1 / b1 partials
+// backward kernel: the species' network, w1, q_scale, per-atom rows sD, sG (Ndes each) and Hc, Av, Bv (Nn each), the W0
+// gradient accumulator of the CTA and the cross-group sums of the b0 / w1 / b1 partials
 __host__ __device__ inline size_t net_small_bwd_floats(const DevSpec &sp) {
-  return (size_t)sp.Nn * sp.ldW + (size_t)sp.Nn + sp.Ndes + (size_t)NS_WARPS * (2 * sp.Ndes + 3 * sp.Nn) +
-         (size_t)sp.Nn * sp.Ndes + (size_t)NS_WARPS * (2 * sp.Nn + 1);
+  return (size_t)sp.Nn * sp.ldW + (size_t)sp.Nn + sp.Ndes + (size_t)NS_ATOMS * (2 * sp.Ndes + 3 * sp.Nn) +
+         (size_t)sp.Nn * sp.Ndes + (size_t)NS_ATOMS * (2 * sp.Nn + 1);
 }
 
 // ------------------------------------------------------------------------------------------------
 // a2: x = tanh(W0 (s o q) + b0), E_i = w1.x + b1, E' = s o (C W0) with C = w1 (1 - x^2), etil = E'[0..NR) . cR
-// A CTA owns a contiguous atom range of ONE species (SpeciesMap.gw_base / gw_atoms), its warps take one atom each.
+// A CTA owns a contiguous atom range of ONE species (SpeciesMap.gw_base / gw_atoms), NS_ATOMS atoms per round.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(NS_WARPS * 32)
+__global__ void __launch_bounds__(NS_THREADS)
 k_net_small_fwd(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float *__restrict__ qscale,
                 const float *__restrict__ q, float *__restrict__ xbuf, float *__restrict__ Ei, float *__restrict__ Ep,
                 float *__restrict__ etil) {
   extern __shared__ __align__(128) float smem[];
-  const int ld = sp.ldW, TK = sp.T * sp.KRp, nW = sp.Nn * sp.Ndes;
+  const int ld = sp.ldW, TK = sp.T * sp.KRp, nW = sp.Nn * sp.Ndes, nrow = 2 * sp.Ndes + sp.Nn + 4;
+  const int grp = threadIdx.x >> 7, tig = threadIdx.x & (NS_GROUP - 1);
   float *cRs = smem;                                   // [jk = J*KRp + k][16]: cR[t][J][n][k], zero padded
   float *W0s = cRs + (size_t)TK * 16;                  // [mu][ld]
   float *bw = W0s + (size_t)sp.Nn * ld;                // [b0 (Nn) | w1 (Nn) | b1]
   float *qss = bw + (2 * sp.Nn + 1);                   // [Ndes]
-  float *rows = qss + sp.Ndes + (size_t)(threadIdx.x >> 5) * (2 * sp.Ndes + sp.Nn);
-  float *sq = rows, *Es = sq + sp.Ndes, *Cs = Es + sp.Ndes;   // per warp: s o q, E', C
+  float *sq = qss + sp.Ndes + (size_t)grp * nrow, *Es = sq + sp.Ndes, *Cs = Es + sp.Ndes, *ep4 = Cs + sp.Nn;   // per atom: s o q, E', C, E partials
   const int t = species_of_block(sm.gw_base, sp.T, blockIdx.x);
   const float *net = theta + sp.offNet + (size_t)t * sp.netSize;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int c0 = sm.start[t] + (blockIdx.x - sm.gw_base[t]) * sm.gw_atoms[t];
   const int c1 = min(c0 + sm.gw_atoms[t], sm.start[t + 1]);
   // the first atom's row is requested before the staging loops (it does not depend on them)
-  float qpre[4] = {0.f, 0.f, 0.f, 0.f};
-  if (c0 + warp < c1)
-#pragma unroll
-    for (int i = 0; i < 4; ++i) if (lane + 32 * i < sp.Ndes) qpre[i] = q[(size_t)(c0 + warp) * sp.Ndes + lane + 32 * i];
+  float qv = (c0 + grp < c1 && tig < sp.Ndes) ? q[(size_t)(c0 + grp) * sp.Ndes + tig] : 0.f;
   ns_stage_w0(W0s, net, sp.Nn, sp.Ndes, ld);
-  for (int x = threadIdx.x; x < 2 * sp.Nn + 1; x += blockDim.x) bw[x] = net[nW + x];
-  for (int x = threadIdx.x; x < sp.Ndes; x += blockDim.x) qss[x] = qscale[x];
-  for (int x = threadIdx.x; x < TK * 16; x += blockDim.x) {
+  for (int x = threadIdx.x; x < 2 * sp.Nn + 1; x += NS_THREADS) bw[x] = net[nW + x];
+  for (int x = threadIdx.x; x < sp.Ndes; x += NS_THREADS) qss[x] = qscale[x];
+  for (int x = threadIdx.x; x < TK * 16; x += NS_THREADS) {
     const int n = x & 15, jk = x >> 4, J = jk / sp.KRp, k = jk - J * sp.KRp;
     cRs[x] = (n < sp.NR && k < sp.KR) ? theta[(((size_t)t * sp.T + J) * sp.NR + n) * sp.KR + k] : 0.f;
   }
   __syncthreads();
-  for (int a = c0 + warp; a < c1; a += NS_WARPS) {
-#pragma unroll
-    for (int i = 0; i < 4; ++i) if (lane + 32 * i < sp.Ndes) sq[lane + 32 * i] = qpre[i] * qss[lane + 32 * i];
-    if (a + NS_WARPS < c1)
-#pragma unroll
-      for (int i = 0; i < 4; ++i) if (lane + 32 * i < sp.Ndes) qpre[i] = q[(size_t)(a + NS_WARPS) * sp.Ndes + lane + 32 * i];
-    __syncwarp();
-    float eacc = 0.f;
-    for (int mu = lane; mu < sp.Nn; mu += 32) {          // first contraction: lane = neuron (row of W0, odd stride)
-      const float z = bw[mu] + ns_dot(W0s + (size_t)mu * ld, 1, sq, 1, sp.Ndes);
-      const float xv = tanh_fast(z), w1 = bw[sp.Nn + mu];
-      xbuf[xt_off(a, mu, sp.NnS)] = xv;
-      eacc = fmaf(w1, xv, eacc);
-      Cs[mu] = w1 * (1.f - xv * xv);
+  for (int r0 = c0; r0 < c1; r0 += NS_ATOMS) {
+    const int a = r0 + grp;
+    const bool on = a < c1;
+    if (on && tig < sp.Ndes) sq[tig] = qv * qss[tig];
+    if (a + NS_ATOMS < c1 && tig < sp.Ndes) qv = q[(size_t)(a + NS_ATOMS) * sp.Ndes + tig];
+    __syncthreads();
+    float e = 0.f;
+    if (on && tig < sp.Nn) {                             // first contraction: thread = neuron (row of W0, odd stride)
+      const float z = bw[tig] + ns_dot(W0s + (size_t)tig * ld, 1, sq, sp.Ndes);
+      const float xv = tanh_fast(z), w1 = bw[sp.Nn + tig];
+      xbuf[xt_off(a, tig, sp.NnS)] = xv;
+      e = w1 * xv;
+      Cs[tig] = w1 * (1.f - xv * xv);
     }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) eacc += __shfl_xor_sync(0xffffffffu, eacc, o);
-    if (lane == 0) Ei[a] = eacc + bw[2 * sp.Nn];
-    __syncwarp();
-    for (int nu = lane; nu < sp.Ndes; nu += 32) {        // second contraction: lane = descriptor (column of W0)
-      const float e = ns_dot(W0s + nu, ld, Cs, 1, sp.Nn) * qss[nu];
-      Ep[(size_t)a * sp.Ndes + nu] = e;
-      Es[nu] = e;
+    for (int o = 16; o > 0; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+    if ((tig & 31) == 0) ep4[tig >> 5] = e;
+    __syncthreads();
+    if (on) {
+      if (tig == 0) Ei[a] = (ep4[0] + ep4[1]) + (ep4[2] + ep4[3]) + bw[2 * sp.Nn];
+      if (tig < sp.Ndes) {                               // second contraction: thread = descriptor (column of W0)
+        const float ev = ns_dot(W0s + tig, ld, Cs, sp.Nn) * qss[tig];
+        Ep[(size_t)a * sp.Ndes + tig] = ev;
+        Es[tig] = ev;
+      }
     }
-    __syncwarp();
-    for (int jk = lane; jk < TK; jk += 32)               // etil[J][k] = sum_n E'_n cR[t][J][n][k]  (input of the radial force pass)
-      etil[(size_t)a * TK + jk] = ns_dot(cRs + (size_t)jk * 16, 1, Es, 1, sp.NR);
-    __syncwarp();
+    __syncthreads();
+    if (on && tig < TK)                                  // etil[J][k] = sum_n E'_n cR[t][J][n][k]  (input of the radial force pass)
+      etil[(size_t)a * TK + tig] = ns_dot(cRs + (size_t)tig * 16, 1, Es, sp.NR);
+    for (int jk = tig + NS_GROUP; on && jk < TK; jk += NS_GROUP) etil[(size_t)a * TK + jk] = ns_dot(cRs + (size_t)jk * 16, 1, Es, sp.NR);
+    __syncthreads();
   }
 }
 
@@ -124,87 +126,74 @@ k_net_small_fwd(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, cons
 // and the parameter-gradient partials of this CTA's atoms (D1.7-D1.17):
 //   dL/dW0 = sum A (x) G + Bc (x) sD,  dL/db0 = sum A,  dL/dw1 = sum V,  dL/db1 = sum e,
 //   G = s o q, sD = s o D, A = w1 (e d1 + d2 p), Bc = w1 d1, V = e x + d1 p, e = s_e e_struct.
-// Same atom ranges as the forward kernel; after a round (one atom per warp) all threads add the round's rank-2 updates to
-// the CTA's W0-gradient accumulator in shared memory (element y = tid + 128 i).  One partial row per CTA, summed in row
-// order by k_grad_reduce.
+// Same atom ranges as the forward kernel; after a round all threads add the round's rank-2 updates to the CTA's
+// W0-gradient accumulator in shared memory (element y = tid + 512 i).  One partial row per CTA, summed in row order by
+// k_grad_reduce.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(NS_WARPS * 32)
+__global__ void __launch_bounds__(NS_THREADS)
 k_net_small_bwd(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float *__restrict__ qscale,
                 const float *__restrict__ q, const float *__restrict__ D, const float *__restrict__ xbuf,
                 const float *__restrict__ Ep, const int *__restrict__ struct_s, const float *__restrict__ e_s,
                 const float *__restrict__ scales, float *__restrict__ gbar, float *__restrict__ partialW,
                 float *__restrict__ partialB) {
   extern __shared__ __align__(128) float smem[];
-  const int ld = sp.ldW, nW = sp.Nn * sp.Ndes, nrow = 2 * sp.Ndes + 3 * sp.Nn;
+  const int ld = sp.ldW, nW = sp.Nn * sp.Ndes, nrow = 2 * sp.Ndes + 3 * sp.Nn, nb = 2 * sp.Nn + 1;
+  const int grp = threadIdx.x >> 7, tig = threadIdx.x & (NS_GROUP - 1);
   float *W0s = smem;                                   // [mu][ld] of this CTA's species
   float *w1s = W0s + (size_t)sp.Nn * ld;               // [Nn]
   float *qss = w1s + sp.Nn;                            // [Ndes]
-  float *rows0 = qss + sp.Ndes;                        // per warp: sD | sG | Hc | Av | Bv
-  float *accW = rows0 + (size_t)NS_WARPS * nrow;       // [Nn * Ndes]
-  float *red = accW + nW;                              // [warp][b0 (Nn) | w1 (Nn) | b1]
+  float *rows0 = qss + sp.Ndes;                        // per atom: sD | sG | Hc | Av | Bv
+  float *accW = rows0 + (size_t)NS_ATOMS * nrow;       // [Nn * Ndes]
+  float *red = accW + nW;                              // [atom slot][b0 (Nn) | w1 (Nn) | b1]
   const int t = species_of_block(sm.gw_base, sp.T, blockIdx.x);
   const float *net = theta + sp.offNet + (size_t)t * sp.netSize;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int c0 = sm.start[t] + (blockIdx.x - sm.gw_base[t]) * sm.gw_atoms[t];
   const int c1 = min(c0 + sm.gw_atoms[t], sm.start[t + 1]);
   ns_stage_w0(W0s, net, sp.Nn, sp.Ndes, ld);
-  for (int x = threadIdx.x; x < sp.Nn; x += blockDim.x) w1s[x] = net[nW + sp.Nn + x];
-  for (int x = threadIdx.x; x < sp.Ndes; x += blockDim.x) qss[x] = qscale[x];
-  for (int x = threadIdx.x; x < nW; x += blockDim.x) accW[x] = 0.f;
-  __syncthreads();
-  float *sD = rows0 + (size_t)warp * nrow, *sG = sD + sp.Ndes, *Hc = sG + sp.Ndes, *Av = Hc + sp.Nn, *Bv = Av + sp.Nn;
+  for (int x = threadIdx.x; x < sp.Nn; x += NS_THREADS) w1s[x] = net[nW + sp.Nn + x];
+  for (int x = threadIdx.x; x < sp.Ndes; x += NS_THREADS) qss[x] = qscale[x];
+  for (int x = threadIdx.x; x < nW; x += NS_THREADS) accW[x] = 0.f;
+  float *sD = rows0 + (size_t)grp * nrow, *sG = sD + sp.Ndes, *Hc = sG + sp.Ndes, *Av = Hc + sp.Nn, *Bv = Av + sp.Nn;
   const float se = scales[0];
-  float accA[4] = {0.f, 0.f, 0.f, 0.f}, accV[4] = {0.f, 0.f, 0.f, 0.f}, acce = 0.f;   // neurons lane, lane + 32, ... (Nn <= 128)
-  const int step = NS_WARPS * 32;
+  float accA = 0.f, accV = 0.f, acce = 0.f;            // of neuron tig (of the group's atoms)
   const int mu_first = threadIdx.x / sp.Ndes, nu_first = threadIdx.x - mu_first * sp.Ndes;
-  const int dmu = step / sp.Ndes, dnu = step - dmu * sp.Ndes;
-  for (int r0 = c0; r0 < c1; r0 += NS_WARPS) {
-    const int a = r0 + warp;
-    if (a < c1) {
-      const float e = se * e_s[struct_s[a]];
-      acce += e;                                       // (every lane holds it; lane 0's copy is used)
-      float xv[4], epv[4];
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {                    // requested before the contractions that need them
-        xv[i] = lane + 32 * i < sp.Nn ? xbuf[xt_off(a, lane + 32 * i, sp.NnS)] : 0.f;
-        epv[i] = lane + 32 * i < sp.Ndes ? Ep[(size_t)a * sp.Ndes + lane + 32 * i] : 0.f;
+  const int dmu = NS_THREADS / sp.Ndes, dnu = NS_THREADS - dmu * sp.Ndes;
+  __syncthreads();
+  for (int r0 = c0; r0 < c1; r0 += NS_ATOMS) {
+    const int a = r0 + grp;
+    const bool on = a < c1;
+    float e = 0.f, xv = 0.f, epv = 0.f;
+    if (on) {
+      e = se * e_s[struct_s[a]];
+      if (tig < sp.Nn) xv = xbuf[xt_off(a, tig, sp.NnS)];
+      if (tig < sp.Ndes) {
+        const float s = qss[tig];
+        epv = Ep[(size_t)a * sp.Ndes + tig];
+        sD[tig] = D[(size_t)a * sp.Ndes + tig] * s;
+        sG[tig] = q[(size_t)a * sp.Ndes + tig] * s;
       }
-      for (int nu = lane; nu < sp.Ndes; nu += 32) {
-        const float s = qss[nu];
-        sD[nu] = D[(size_t)a * sp.Ndes + nu] * s;
-        sG[nu] = q[(size_t)a * sp.Ndes + nu] * s;
-      }
-      __syncwarp();
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        const int mu = lane + 32 * i;
-        if (mu < sp.Nn) {
-          const float p = ns_dot(W0s + (size_t)mu * ld, 1, sD, 1, sp.Ndes), w1 = w1s[mu];
-          const float d1 = 1.f - xv[i] * xv[i], d2 = -2.f * xv[i] * d1;
-          const float A = w1 * (e * d1 + d2 * p);
-          Hc[mu] = w1 * d2 * p; Av[mu] = A; Bv[mu] = w1 * d1;
-          accA[i] += A;
-          accV[i] += e * xv[i] + d1 * p;
-        }
-      }
-      __syncwarp();
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        const int nu = lane + 32 * i;
-        if (nu < sp.Ndes) gbar[(size_t)a * sp.Ndes + nu] = e * epv[i] + ns_dot(W0s + nu, ld, Hc, 1, sp.Nn) * qss[nu];
-      }
+      acce += e;
     }
     __syncthreads();
+    if (on && tig < sp.Nn) {
+      const float p = ns_dot(W0s + (size_t)tig * ld, 1, sD, sp.Ndes), w1 = w1s[tig];
+      const float d1 = 1.f - xv * xv, d2 = -2.f * xv * d1;
+      const float A = w1 * (e * d1 + d2 * p);
+      Hc[tig] = w1 * d2 * p; Av[tig] = A; Bv[tig] = w1 * d1;
+      accA += A;
+      accV += e * xv + d1 * p;
+    }
+    __syncthreads();
+    if (on && tig < sp.Ndes) gbar[(size_t)a * sp.Ndes + tig] = e * epv + ns_dot(W0s + tig, ld, Hc, sp.Nn) * qss[tig];
     // the round's rank-2 updates to the elements this thread owns
-    const int nw_on = min(NS_WARPS, c1 - r0);
+    const int n_on = min(NS_ATOMS, c1 - r0);
     int mu = mu_first, nu = nu_first;
-#pragma unroll 2
-    for (int y = threadIdx.x; y < nW; y += step) {
+    for (int y = threadIdx.x; y < nW; y += NS_THREADS) {
       float s = accW[y];
 #pragma unroll
-      for (int w = 0; w < NS_WARPS; ++w) {
-        if (w < nw_on) {
-          const float *rw = rows0 + (size_t)w * nrow;   // sD | sG | Hc | Av | Bv of warp w's atom
+      for (int w = 0; w < NS_ATOMS; ++w) {
+        if (w < n_on) {
+          const float *rw = rows0 + (size_t)w * nrow;   // sD | sG | Hc | Av | Bv of atom slot w
           s = fmaf(rw[2 * sp.Ndes + sp.Nn + mu], rw[sp.Ndes + nu], fmaf(rw[2 * sp.Ndes + 2 * sp.Nn + mu], rw[nu], s));
         }
       }
@@ -214,18 +203,15 @@ k_net_small_bwd(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, cons
     }
     __syncthreads();
   }
-  for (int y = threadIdx.x; y < nW; y += step) partialW[(size_t)blockIdx.x * nW + y] = accW[y];
-  float *rd = red + (size_t)warp * (2 * sp.Nn + 1);
-#pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const int mu = lane + 32 * i;
-    if (mu < sp.Nn) { rd[mu] = accA[i]; rd[sp.Nn + mu] = accV[i]; }
-  }
-  if (lane == 0) rd[2 * sp.Nn] = acce;
+  for (int y = threadIdx.x; y < nW; y += NS_THREADS) partialW[(size_t)blockIdx.x * nW + y] = accW[y];
+  float *rd = red + (size_t)grp * nb;
+  if (tig < sp.Nn) { rd[tig] = accA; rd[sp.Nn + tig] = accV; }
+  if (tig == 0) rd[2 * sp.Nn] = acce;
   __syncthreads();
-  for (int x = threadIdx.x; x < 2 * sp.Nn + 1; x += blockDim.x) {
+  for (int x = threadIdx.x; x < nb; x += NS_THREADS) {
     float s = 0.f;
-    for (int w = 0; w < NS_WARPS; ++w) s += red[(size_t)w * (2 * sp.Nn + 1) + x];
-    partialB[(size_t)blockIdx.x * (2 * sp.Nn + 1) + x] = s;
+#pragma unroll
+    for (int w = 0; w < NS_ATOMS; ++w) s += red[(size_t)w * nb + x];
+    partialB[(size_t)blockIdx.x * nb + x] = s;
   }
 }
