@@ -93,6 +93,7 @@ struct gnep_handle {
   int n_tilesA = 0, grid_adj = 0, grid_cg = 0, occ_adj = 1, occ_cg = 1, occ_S = 4;
   bool fuse_adam = false; float fuse_b1 = 0.f, fuse_b2 = 0.f, fuse_eps = 0.f;   // set while gnep_train_epochs captures its graph
   bool net_small = false;                  // small batches: the network on plain FMAs, warp per atom (net_small_kernels.cuh)
+  int rad_lanes = RAD_SPLIT;               // lanes per atom of the split radial sweeps
   bool rad_split = false;                  // radial a3/a5 with RAD_SPLIT lanes per atom (small batches)
   int ta_ang = ANG_TA, ta_frc = FRC_TA;   // atoms per warp of the warp-tile sweeps: fewer for small batches, so that every SM gets warps
   int *segA = nullptr, *atomA = nullptr;   // warp-tile path: angular list with every (atom, J) segment padded to 4 pairs
@@ -175,6 +176,9 @@ int padded_basis_ang(int K) { return K <= 4 ? 4 : K <= 8 ? 8 : 16; }
 #define DISPATCH_NQ(NA_, ...)                                   \
   if ((NA_) <= 10) { constexpr int NQ = 10; __VA_ARGS__; }      \
   else { constexpr int NQ = 16; __VA_ARGS__; }
+#define DISPATCH_SPLIT(L_, ...)                                          \
+  if ((L_) == RAD_SPLIT_WIDE) { constexpr int SPLIT = RAD_SPLIT_WIDE; __VA_ARGS__; } \
+  else { constexpr int SPLIT = RAD_SPLIT; __VA_ARGS__; }
 #define DISPATCH_B5(U5_, ...)                                   \
   if (U5_) { constexpr bool B5 = true; __VA_ARGS__; }           \
   else { constexpr bool B5 = false; __VA_ARGS__; }
@@ -235,7 +239,7 @@ int set_smem(gnep_handle *h, K kernel, size_t bytes) {
 
 int configure_kernels(gnep_handle *h) {
   const DevSpec &d = h->ds;
-  DISPATCH_KT(d.KRp, RET_IF(set_smem(h, k_radial_fwd<KT>, smem_radial(d))); RET_IF(set_smem(h, k_radial_adj<KT>, smem_radial(d))); RET_IF(set_smem(h, k_radial_adj_split<KT>, smem_radial(d)));
+  DISPATCH_KT(d.KRp, RET_IF(set_smem(h, k_radial_fwd<KT>, smem_radial(d))); RET_IF(set_smem(h, k_radial_adj<KT>, smem_radial(d))); { auto k8 = k_radial_adj_split<KT, RAD_SPLIT>; auto k32 = k_radial_adj_split<KT, RAD_SPLIT_WIDE>; RET_IF(set_smem(h, k8, smem_radial(d))); RET_IF(set_smem(h, k32, smem_radial(d))); }
               RET_IF(set_smem(h, k_radial_q<KT>, smem_radial(d))));
   DISPATCH_ANG(d, auto kf = k_angular_fwd<KT, LMAX>; auto ka = k_angular_adj<KT, LMAX>; auto kc = k_cgrad_angular<KT, LMAX>;
                auto kp = k_angular_force<KT, LMAX>;
@@ -355,8 +359,8 @@ int enqueue_forward(gnep_handle *h) {
   mark(h, "a3_angular_force");
   // radial forces + the gather of the angular pair forces (thread per atom): writes F_i, W_i once
   if (h->rad_split) {
-    DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_force_split<KT>, cdiv((int64_t)h->N * RAD_SPLIT, RAD_THREADS), RAD_THREADS, 0, d, h->N, h->type_s, h->segR, h->pairR, h->etil,
-                              h->segAu, h->revAu, h->pairAu, h->fpair, h->Fat, h->Wat));
+    DISPATCH_KT(d.KRp, DISPATCH_SPLIT(h->rad_lanes, auto kf = k_radial_force_split<KT, SPLIT>; LAUNCH(h, kf, cdiv((int64_t)h->N * SPLIT, RAD_THREADS), RAD_THREADS, 0, d, h->N, h->type_s, h->segR, h->pairR, h->etil,
+                              h->segAu, h->revAu, h->pairAu, h->fpair, h->Fat, h->Wat)));
   } else {
     DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_force<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, 0, d, h->N, h->type_s, h->segR, h->pairR, h->etil,
                               h->segAu, h->revAu, h->pairAu, h->fpair, h->Fat, h->Wat));
@@ -378,7 +382,7 @@ int enqueue_forward(gnep_handle *h) {
 int enqueue_backward(gnep_handle *h) {
   const DevSpec &d = h->ds;
   if (h->rad_split) {
-    DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_adj_split<KT>, cdiv((int64_t)h->N * RAD_SPLIT, RAD_THREADS), RAD_THREADS, smem_radial(d), d, h->N, h->type_s, h->struct_s, h->segR, h->pairR, h->theta, h->u, h->omega, h->scales, h->D, h->M2));
+    DISPATCH_KT(d.KRp, DISPATCH_SPLIT(h->rad_lanes, auto ka = k_radial_adj_split<KT, SPLIT>; LAUNCH(h, ka, cdiv((int64_t)h->N * SPLIT, RAD_THREADS), RAD_THREADS, smem_radial(d), d, h->N, h->type_s, h->struct_s, h->segR, h->pairR, h->theta, h->u, h->omega, h->scales, h->D, h->M2)));
   } else {
     DISPATCH_KT(d.KRp, LAUNCH(h, k_radial_adj<KT>, cdiv(h->N, RAD_THREADS), RAD_THREADS, smem_radial(d), d, h->N, h->type_s, h->struct_s, h->segR, h->pairR, h->theta, h->u, h->omega, h->scales, h->D, h->M2));
   }
@@ -919,6 +923,7 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     h->ta_ang = small ? std::max(1, std::min(ANG_TA, cdiv(N, 4 * h->num_sms * ANG_WARPS))) : ANG_TA;
     h->ta_frc = small ? std::max(1, std::min(FRC_TA, cdiv(N, 5 * h->num_sms * FRC_WARPS))) : FRC_TA;
     h->rad_split = small;
+    h->rad_lanes = (int64_t)N * RAD_SPLIT_WIDE <= (int64_t)4 * h->num_sms * RAD_THREADS ? RAD_SPLIT_WIDE : RAD_SPLIT;
     for (int t = 0; t <= GNEP_MAX_SPECIES_C; ++t) { h->rm.chunk_base[t] = h->sm.chunk_base[t]; h->rm.gw_base[t] = h->sm.gw_base[t]; }
     const int ca_warps = h->tile_path ? ang_warps(d) : ANG_WARPS;
     h->rm.n_warps_ca = N > 0 ? (h->grid_adj + h->grid_cg) * ca_warps : 0;   // partial rows: the beta half (adjoint sweep) then the alpha half

@@ -309,21 +309,23 @@ k_radial_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__res
 // consecutive records = 128 contiguous bytes per atom and round) and add their sums by butterflies.  Same arithmetic
 // per pair as the kernels above; chosen by the host when the batch cannot fill the SMs with one thread per atom.
 // ------------------------------------------------------------------------------------------------
-#define RAD_SPLIT 8
+#define RAD_SPLIT 8          // lanes per atom ...
+#define RAD_SPLIT_WIDE 32    // ... and for batches so small that even that leaves SMs idle: one warp per atom
+template <int SPLIT>
 __device__ __forceinline__ float split_sum(float x) {
 #pragma unroll
-  for (int o = 1; o < RAD_SPLIT; o <<= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+  for (int o = 1; o < SPLIT; o <<= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
   return x;
 }
 
-template <int KT>
+template <int KT, int SPLIT>
 __global__ void __launch_bounds__(RAD_THREADS)
 k_radial_force_split(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ segR,
                      const float4 *__restrict__ pairR, const float *__restrict__ etil, const int *__restrict__ segA,
                      const int *__restrict__ revA, const float4 *__restrict__ pairA, const float4 *__restrict__ fpair,
                      float4 *__restrict__ Fat, float *__restrict__ Wat) {
   const int gt = blockIdx.x * RAD_THREADS + threadIdx.x;
-  const int a = gt / RAD_SPLIT, sub = gt % RAD_SPLIT;
+  const int a = gt / SPLIT, sub = gt % SPLIT;
   const bool on = a < N;                          // whole warps stay in the butterflies
   float F[3] = {0.f, 0.f, 0.f}, W[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   if (on) {
@@ -333,7 +335,7 @@ k_radial_force_split(DevSpec sp, int N, const int *__restrict__ type_s, const in
     for (int J = 0; J < sp.T; ++J) {
       float ei[KT];
       load_row<KT>(etil + (size_t)a * TK + J * KT, ei);
-      for (int p = sg[J] + sub; p < sg[J + 1]; p += RAD_SPLIT) {
+      for (int p = sg[J] + sub; p < sg[J + 1]; p += SPLIT) {
         const float4 r = pairR[p];
         float ej[KT];
         load_row<KT>(etil + (size_t)__float_as_int(r.w) * TK + I * KT, ej);
@@ -358,7 +360,7 @@ k_radial_force_split(DevSpec sp, int N, const int *__restrict__ type_s, const in
     }
     if (fpair) {
       const int q0 = segA[(size_t)a * (sp.T + 1)], q1 = segA[(size_t)a * (sp.T + 1) + sp.T];
-      for (int p = q0 + sub; p < q1; p += RAD_SPLIT) {
+      for (int p = q0 + sub; p < q1; p += SPLIT) {
         const float4 f = fpair[p], x = pairA[p], g = fpair[revA[p]];
         F[0] += f.x - g.x; F[1] += f.y - g.y; F[2] += f.z - g.z;
         W[0] -= x.x * f.x; W[1] -= x.y * f.y; W[2] -= x.z * f.z;
@@ -367,9 +369,9 @@ k_radial_force_split(DevSpec sp, int N, const int *__restrict__ type_s, const in
     }
   }
 #pragma unroll
-  for (int c = 0; c < 3; ++c) F[c] = split_sum(F[c]);
+  for (int c = 0; c < 3; ++c) F[c] = split_sum<SPLIT>(F[c]);
 #pragma unroll
-  for (int c = 0; c < 6; ++c) W[c] = split_sum(W[c]);
+  for (int c = 0; c < 6; ++c) W[c] = split_sum<SPLIT>(W[c]);
   if (on && sub == 0) {
     Fat[a] = make_float4(F[0], F[1], F[2], 0.f);
 #pragma unroll
@@ -377,7 +379,7 @@ k_radial_force_split(DevSpec sp, int N, const int *__restrict__ type_s, const in
   }
 }
 
-template <int KT>
+template <int KT, int SPLIT>
 __global__ void __launch_bounds__(RAD_THREADS)
 k_radial_adj_split(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ struct_s,
                    const int *__restrict__ segR, const float4 *__restrict__ pairR, const float *__restrict__ theta,
@@ -388,20 +390,20 @@ k_radial_adj_split(DevSpec sp, int N, const int *__restrict__ type_s, const int 
   stage_coeff(cs, theta, sp.T * sp.T * sp.NR, sp.KR, KT);
   __syncthreads();
   const int gt = blockIdx.x * RAD_THREADS + threadIdx.x;
-  const int a = gt / RAD_SPLIT, sub = gt % RAD_SPLIT;
+  const int a = gt / SPLIT, sub = gt % SPLIT;
   const bool on = a < N;
   const int ac = on ? a : 0;
   const int I = N > 0 ? type_s[ac] : 0;
   AdjCtx ctx = {};
   if (on) ctx = make_adj(u, omega, scales, a, struct_s[a]);
   const int *sg = segR + (size_t)ac * (sp.T + 1);
-  float o[2] = {0.f, 0.f};                        // D_n of the lane's two functions n = sub, sub + RAD_SPLIT
+  float o[2] = {0.f, 0.f};                        // D_n of the lane's two functions n = sub, sub + SPLIT
   for (int J = 0; J < sp.T; ++J) {
     float acc[KT];
 #pragma unroll
     for (int k = 0; k < KT; ++k) acc[k] = 0.f;
     if (on)
-      for (int p = sg[J] + sub; p < sg[J + 1]; p += RAD_SPLIT) {
+      for (int p = sg[J] + sub; p < sg[J + 1]; p += SPLIT) {
         const float4 r = pairR[p];
         const float4 uj = u[__float_as_int(r.w)];
         float d, rinv, Tk[KT], Dk[KT], hfc, hfcp, hdf;
@@ -416,12 +418,12 @@ k_radial_adj_split(DevSpec sp, int N, const int *__restrict__ type_s, const int 
         for (int k = 1; k < KT; ++k) acc[k] = fmaf(w1, Dk[k], fmaf(w2, Tk[k], acc[k] + w2));
       }
 #pragma unroll
-    for (int k = 0; k < KT; ++k) acc[k] = split_sum(acc[k]);       // every lane of the atom now holds M2[J][.]
+    for (int k = 0; k < KT; ++k) acc[k] = split_sum<SPLIT>(acc[k]);       // every lane of the atom now holds M2[J][.]
     if (on && sub == 0) store_row<KT>(M2 + (size_t)a * sp.T * KT + J * KT, acc);
     const float *c = cs + (size_t)(I * sp.T + J) * sp.NR * KT;
 #pragma unroll
     for (int i = 0; i < 2; ++i) {
-      const int n = sub + i * RAD_SPLIT;
+      const int n = sub + i * SPLIT;
       if (n < sp.NR) {
         float cv[KT];
         load_row<KT>(c + n * KT, cv);
@@ -433,7 +435,7 @@ k_radial_adj_split(DevSpec sp, int N, const int *__restrict__ type_s, const int 
   if (on) {
 #pragma unroll
     for (int i = 0; i < 2; ++i) {
-      const int n = sub + i * RAD_SPLIT;
+      const int n = sub + i * SPLIT;
       if (n < sp.NR) D[(size_t)a * sp.Ndes + n] = o[i];
     }
   }
