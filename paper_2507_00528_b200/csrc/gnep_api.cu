@@ -394,7 +394,7 @@ int enqueue_backward(gnep_handle *h) {
   mark(h, "a5_angular_adjoint");
   if (h->net_small) {   // network backward and its parameter-gradient partials in one launch
     LAUNCH(h, k_net_small_bwd, h->n_gw, NS_THREADS, sizeof(float) * net_small_bwd_floats(d), d, h->sm, h->theta, h->qscale, h->q, h->D, h->x, h->Ep,
-           h->struct_s, h->e_s, h->scales, h->gbar, h->partialW, h->partialB);
+           h->struct_s, h->e_s, h->scales, h->M1, h->M2, h->gbar, h->partialW, h->partialB, h->partialCR);
     mark(h, "a6_network_backward");
   } else {
     LAUNCH(h, k_net_tc<true>, h->n_cta_net, 256, smem_net_bwd(d), d, h->sm, h->theta, h->qscale, h->D, h->x, h->eat, h->Ep, (float *)nullptr,
@@ -403,7 +403,8 @@ int enqueue_backward(gnep_handle *h) {
     LAUNCH(h, k_gradw_tc, h->n_gw, GW_THREADS, smem_gradw(d), d, h->sm, gradw_nraw(d), h->theta, h->qscale, h->eat, h->q, h->D, h->x, h->pbuf, h->partialW, h->partialB);
   }
   mark(h, "a6_w0_gradient");
-  LAUNCH(h, k_cgrad_radial, h->n_chunks, CR_THREADS, smem_cgrad_rad(d), d, h->sm, h->gbar, h->Ep, h->M1, h->M2, h->partialCR);
+  if (!h->net_small)   // (the small-batch network backward forms these partials itself)
+    LAUNCH(h, k_cgrad_radial, h->n_chunks, CR_THREADS, smem_cgrad_rad(d), d, h->sm, h->gbar, h->Ep, h->M1, h->M2, h->partialCR);
   mark(h, "a7_radial_cgrad");
   if (!h->tile_path) {
     DISPATCH_KA(d.KAp, DISPATCH_B5(d.use5, auto kc5 = k_angw_cgrad<KT, B5>; LAUNCH(h, kc5, h->grid_cg, ANG_WARPS * 32, smem_angw_cgrad(d), d, h->N, h->type_s, h->Ep, h->gbar, h->Sn, h->Tn, h->A1, h->A2, h->partialCA)));
@@ -906,6 +907,8 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
       h->sm.gw_atoms[t] = ga;
       h->sm.gw_base[t + 1] = h->sm.gw_base[t] + (nt > 0 ? cdiv(nt, ga) : 0);
     }
+    if (h->net_small)   // the radial c-gradient partials come from k_net_small_bwd: one row per CTA of that kernel
+      for (int t = 0; t <= GNEP_MAX_SPECIES_C; ++t) h->sm.chunk_base[t] = h->sm.gw_base[t];
     h->n_cta_net = h->sm.cta_base[GNEP_MAX_SPECIES_C];
     h->n_chunks = h->sm.chunk_base[GNEP_MAX_SPECIES_C];
     h->n_gw = h->sm.gw_base[GNEP_MAX_SPECIES_C];

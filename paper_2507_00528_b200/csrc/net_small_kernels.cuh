@@ -54,7 +54,8 @@ __host__ __device__ inline size_t net_small_fwd_floats(const DevSpec &sp) {
 // gradient accumulator of the CTA and the cross-group sums of the b0 / w1 / b1 partials
 __host__ __device__ inline size_t net_small_bwd_floats(const DevSpec &sp) {
   return (size_t)sp.Nn * sp.ldW + (size_t)sp.Nn + sp.Ndes + (size_t)NS_ATOMS * (2 * sp.Ndes + 3 * sp.Nn) +
-         (size_t)sp.Nn * sp.Ndes + (size_t)NS_ATOMS * (2 * sp.Nn + 1);
+         (size_t)sp.Nn * sp.Ndes + (size_t)NS_ATOMS * (2 * sp.Nn + 1) +
+         (size_t)NS_ATOMS * (2 * sp.NR + 2 * sp.T * sp.KRp) + (size_t)sp.NR * sp.T * sp.KRp;   // radial c-gradient rows and accumulator
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -129,15 +130,20 @@ k_net_small_fwd(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, cons
 // Same atom ranges as the forward kernel; after a round all threads add the round's rank-2 updates to the CTA's
 // W0-gradient accumulator in shared memory (element y = tid + 512 i).  One partial row per CTA, summed in row order by
 // k_grad_reduce.
+// a7 (radial) rides along: dL/dcR[t][J][n][k] += gbar_n M1[J][k] + E'_n M2[J][k] per atom (cgrad_radial.cuh), the same
+// kind of rank-2 update on a [NR][T*KRp] accumulator; its partial row has the layout of k_cgrad_radial's ([n][J][k]),
+// one row per CTA (the host points the chunk table of k_grad_reduce at these CTAs).
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(NS_THREADS)
 k_net_small_bwd(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float *__restrict__ qscale,
                 const float *__restrict__ q, const float *__restrict__ D, const float *__restrict__ xbuf,
                 const float *__restrict__ Ep, const int *__restrict__ struct_s, const float *__restrict__ e_s,
-                const float *__restrict__ scales, float *__restrict__ gbar, float *__restrict__ partialW,
-                float *__restrict__ partialB) {
+                const float *__restrict__ scales, const float *__restrict__ M1, const float *__restrict__ M2,
+                float *__restrict__ gbar, float *__restrict__ partialW, float *__restrict__ partialB,
+                float *__restrict__ partialCR) {
   extern __shared__ __align__(128) float smem[];
   const int ld = sp.ldW, nW = sp.Nn * sp.Ndes, nrow = 2 * sp.Ndes + 3 * sp.Nn, nb = 2 * sp.Nn + 1;
+  const int TK = sp.T * sp.KRp, ncr = 2 * sp.NR + 2 * TK, nC = sp.NR * TK;
   const int grp = threadIdx.x >> 7, tig = threadIdx.x & (NS_GROUP - 1);
   float *W0s = smem;                                   // [mu][ld] of this CTA's species
   float *w1s = W0s + (size_t)sp.Nn * ld;               // [Nn]
@@ -145,6 +151,9 @@ k_net_small_bwd(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, cons
   float *rows0 = qss + sp.Ndes;                        // per atom: sD | sG | Hc | Av | Bv
   float *accW = rows0 + (size_t)NS_ATOMS * nrow;       // [Nn * Ndes]
   float *red = accW + nW;                              // [atom slot][b0 (Nn) | w1 (Nn) | b1]
+  float *crow0 = red + (size_t)NS_ATOMS * nb;          // per atom: gbar[0..NR) | E'[0..NR) | M1[TK] | M2[TK]
+  float *accC = crow0 + (size_t)NS_ATOMS * ncr;        // [NR][TK]
+  float *crow = crow0 + (size_t)grp * ncr;
   const int t = species_of_block(sm.gw_base, sp.T, blockIdx.x);
   const float *net = theta + sp.offNet + (size_t)t * sp.netSize;
   const int c0 = sm.start[t] + (blockIdx.x - sm.gw_base[t]) * sm.gw_atoms[t];
@@ -153,6 +162,7 @@ k_net_small_bwd(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, cons
   for (int x = threadIdx.x; x < sp.Nn; x += NS_THREADS) w1s[x] = net[nW + sp.Nn + x];
   for (int x = threadIdx.x; x < sp.Ndes; x += NS_THREADS) qss[x] = qscale[x];
   for (int x = threadIdx.x; x < nW; x += NS_THREADS) accW[x] = 0.f;
+  for (int x = threadIdx.x; x < nC; x += NS_THREADS) accC[x] = 0.f;
   float *sD = rows0 + (size_t)grp * nrow, *sG = sD + sp.Ndes, *Hc = sG + sp.Ndes, *Av = Hc + sp.Nn, *Bv = Av + sp.Nn;
   const float se = scales[0];
   float accA = 0.f, accV = 0.f, acce = 0.f;            // of neuron tig (of the group's atoms)
@@ -171,7 +181,9 @@ k_net_small_bwd(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, cons
         epv = Ep[(size_t)a * sp.Ndes + tig];
         sD[tig] = D[(size_t)a * sp.Ndes + tig] * s;
         sG[tig] = q[(size_t)a * sp.Ndes + tig] * s;
+        if (tig < sp.NR) crow[sp.NR + tig] = epv;
       }
+      for (int jk = tig; jk < TK; jk += NS_GROUP) { crow[2 * sp.NR + jk] = M1[(size_t)a * TK + jk]; crow[2 * sp.NR + TK + jk] = M2[(size_t)a * TK + jk]; }
       acce += e;
     }
     __syncthreads();
@@ -184,7 +196,11 @@ k_net_small_bwd(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, cons
       accV += e * xv + d1 * p;
     }
     __syncthreads();
-    if (on && tig < sp.Ndes) gbar[(size_t)a * sp.Ndes + tig] = e * epv + ns_dot(W0s + tig, ld, Hc, sp.Nn) * qss[tig];
+    if (on && tig < sp.Ndes) {
+      const float gb = e * epv + ns_dot(W0s + tig, ld, Hc, sp.Nn) * qss[tig];
+      gbar[(size_t)a * sp.Ndes + tig] = gb;
+      if (tig < sp.NR) crow[tig] = gb;
+    }
     // the round's rank-2 updates to the elements this thread owns
     const int n_on = min(NS_ATOMS, c1 - r0);
     int mu = mu_first, nu = nu_first;
@@ -201,8 +217,22 @@ k_net_small_bwd(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, cons
       mu += dmu; nu += dnu;
       if (nu >= sp.Ndes) { nu -= sp.Ndes; ++mu; }
     }
+    __syncthreads();                                     // (the gbar entries of this round are in the rows now)
+    for (int y = threadIdx.x; y < nC; y += NS_THREADS) { // a7 radial: element (n, jk)
+      const int n = y / TK, jk = y - n * TK;
+      float s = accC[y];
+#pragma unroll
+      for (int w = 0; w < NS_ATOMS; ++w) {
+        if (w < n_on) {
+          const float *cw = crow0 + (size_t)w * ncr;
+          s = fmaf(cw[n], cw[2 * sp.NR + jk], fmaf(cw[sp.NR + n], cw[2 * sp.NR + TK + jk], s));
+        }
+      }
+      accC[y] = s;
+    }
     __syncthreads();
   }
+  for (int y = threadIdx.x; y < nC; y += NS_THREADS) partialCR[(size_t)blockIdx.x * nC + y] = accC[y];
   for (int y = threadIdx.x; y < nW; y += NS_THREADS) partialW[(size_t)blockIdx.x * nW + y] = accW[y];
   float *rd = red + (size_t)grp * nb;
   if (tig < sp.Nn) { rd[tig] = accA; rd[sp.Nn + tig] = accV; }
