@@ -347,9 +347,12 @@ LossCfg loss_cfg(const gnep_handle *h) {
 
 int enqueue_forward(gnep_handle *h) {
   const DevSpec &d = h->ds;
-  RET_IF(enqueue_descriptors(h));
+  const bool fuse_desc = h->net_small && !h->tile_path;   // small batches: the descriptor contraction inside the network kernel
+  if (!fuse_desc) RET_IF(enqueue_descriptors(h));
   if (h->net_small) {
-    LAUNCH(h, k_net_small_fwd, h->n_gw, NS_THREADS, sizeof(float) * net_small_fwd_floats(d), d, h->sm, h->theta, h->qscale, h->q, h->x, h->Ei, h->Ep, h->etil);
+    LAUNCH(h, k_net_small_fwd, h->n_gw, NS_THREADS, sizeof(float) * net_small_fwd_floats(d), d, h->sm, h->theta, h->qscale, h->q, h->x, h->Ei, h->Ep, h->etil,
+           fuse_desc ? h->A1 : (const float *)nullptr, h->M1, h->Sn);
+    if (fuse_desc) mark(h, "a1_descriptor_contraction");
   } else {
     LAUNCH(h, k_net_tc<false>, h->n_cta_net, 256, smem_net_fwd(d), d, h->sm, h->theta, h->qscale, h->q, h->x, h->Ei, h->Ep, h->etil,
            (const int *)nullptr, (const float *)nullptr, (const float *)nullptr, (float *)nullptr, (float *)nullptr);
@@ -885,7 +888,8 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     // (small batches -- see below -- run the network on plain FMAs, one warp per atom, with short atom ranges per CTA)
     bool small = N < 2 * h->num_sms * RAD_THREADS;
     if (const char *e = getenv("GNEP_SMALL_BATCH")) small = atoi(e) != 0;
-    h->net_small = small && d.Nn <= 128 && d.Ndes <= 128 && sizeof(float) * net_small_bwd_floats(d) <= 200 * 1024;
+    h->net_small = small && d.Nn <= 128 && d.Ndes <= 128 && sizeof(float) * net_small_bwd_floats(d) <= 200 * 1024 &&
+                   sizeof(float) * net_small_fwd_floats(d) <= 200 * 1024;
     int tiles_total = 0;
     for (int t = 0; t < T; ++t) tiles_total += cdiv(h->sm.start[t + 1] - h->sm.start[t], 128);
     h->sm.cta_base[0] = 0; h->sm.chunk_base[0] = 0; h->sm.gw_base[0] = 0;

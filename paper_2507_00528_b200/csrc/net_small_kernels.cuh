@@ -45,10 +45,12 @@ __device__ __forceinline__ float ns_dot(const float *w, int ws, const float *v, 
   return (a0 + a1) + (a2 + a3);
 }
 
-// shared-memory floats of the forward kernel: cR[t] as [jk][16], the species' network, q_scale, per-atom rows
+// shared-memory floats of the forward kernel: cR[t] as [jk][16], the species' network, q_scale, per-atom rows; with the
+// descriptor contraction fused in (warp-tile angular path): cA[t], and per atom the A1 block, the M1 row, S and q
 __host__ __device__ inline size_t net_small_fwd_floats(const DevSpec &sp) {
   return (size_t)sp.T * sp.KRp * 16 + (size_t)sp.Nn * sp.ldW + (size_t)(2 * sp.Nn + 1) + sp.Ndes +
-         (size_t)NS_ATOMS * (2 * sp.Ndes + sp.Nn + 4);
+         (size_t)NS_ATOMS * (2 * sp.Ndes + sp.Nn + 4) + (size_t)sp.T * sp.NA * sp.KAp +
+         (size_t)NS_ATOMS * (sp.T * sp.KAp * 24 + sp.T * sp.KRp + sp.NA * 24 + sp.Ndes);
 }
 // backward kernel: the species' network, w1, q_scale, per-atom rows sD, sG (Ndes each) and Hc, Av, Bv (Nn each), the W0
 // gradient accumulator of the CTA and the cross-group sums of the b0 / w1 / b1 partials
@@ -61,11 +63,15 @@ __host__ __device__ inline size_t net_small_bwd_floats(const DevSpec &sp) {
 // ------------------------------------------------------------------------------------------------
 // a2: x = tanh(W0 (s o q) + b0), E_i = w1.x + b1, E' = s o (C W0) with C = w1 (1 - x^2), etil = E'[0..NR) . cR
 // A CTA owns a contiguous atom range of ONE species (SpeciesMap.gw_base / gw_atoms), NS_ATOMS atoms per round.
+// With A1 != nullptr (angular warp-tile path, l_max <= 4) the per-epoch descriptor contraction a1 is done here too, from
+// the resident geometry moments (angular_warp_kernels.cuh, k_angw_S): q_n = cR.M1 (Eq.5-6), S_nlm = cA.A1 (Eq.8, thread
+// = (n, lm)), q_nl = sum_m C_lm S^2 (Eq.7), the 4-body (R14) and 5-body (R41) terms; q and S are written for the later
+// kernels and the network reads q from shared memory: one launch instead of two.
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(NS_THREADS)
 k_net_small_fwd(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, const float *__restrict__ qscale,
-                const float *__restrict__ q, float *__restrict__ xbuf, float *__restrict__ Ei, float *__restrict__ Ep,
-                float *__restrict__ etil) {
+                float *q, float *__restrict__ xbuf, float *__restrict__ Ei, float *__restrict__ Ep,
+                float *__restrict__ etil, const float *__restrict__ A1, const float *__restrict__ M1, float *__restrict__ S) {
   extern __shared__ __align__(128) float smem[];
   const int ld = sp.ldW, TK = sp.T * sp.KRp, nW = sp.Nn * sp.Ndes, nrow = 2 * sp.Ndes + sp.Nn + 4;
   const int grp = threadIdx.x >> 7, tig = threadIdx.x & (NS_GROUP - 1);
@@ -74,12 +80,27 @@ k_net_small_fwd(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, cons
   float *bw = W0s + (size_t)sp.Nn * ld;                // [b0 (Nn) | w1 (Nn) | b1]
   float *qss = bw + (2 * sp.Nn + 1);                   // [Ndes]
   float *sq = qss + sp.Ndes + (size_t)grp * nrow, *Es = sq + sp.Ndes, *Cs = Es + sp.Ndes, *ep4 = Cs + sp.Nn;   // per atom: s o q, E', C, E partials
+  const bool fuse = A1 != nullptr;
+  const int nA1 = sp.T * sp.KAp * 24, nS = sp.NA * 24, ndr = nA1 + TK + nS + sp.Ndes;
+  float *cAs = qss + sp.Ndes + (size_t)NS_ATOMS * nrow;            // [J][n][k(KAp)] of this species, zero padded
+  float *A1s = cAs + (size_t)sp.T * sp.NA * sp.KAp + (size_t)grp * ndr, *m1s = A1s + nA1, *Ss = m1s + TK, *qrow = Ss + nS;
   const int t = species_of_block(sm.gw_base, sp.T, blockIdx.x);
   const float *net = theta + sp.offNet + (size_t)t * sp.netSize;
   const int c0 = sm.start[t] + (blockIdx.x - sm.gw_base[t]) * sm.gw_atoms[t];
   const int c1 = min(c0 + sm.gw_atoms[t], sm.start[t + 1]);
   // the first atom's row is requested before the staging loops (it does not depend on them)
-  float qv = (c0 + grp < c1 && tig < sp.Ndes) ? q[(size_t)(c0 + grp) * sp.Ndes + tig] : 0.f;
+  float qv = (!fuse && c0 + grp < c1 && tig < sp.Ndes) ? q[(size_t)(c0 + grp) * sp.Ndes + tig] : 0.f;
+  if (fuse) {
+    if (c0 + grp < c1) {                                 // the first atom's moments: requested before the staging loops too
+      const int a = c0 + grp;
+      for (int x = tig; x < nA1; x += NS_GROUP) A1s[x] = A1[(size_t)a * nA1 + x];
+      for (int x = tig; x < TK; x += NS_GROUP) m1s[x] = M1[(size_t)a * TK + x];
+    }
+    for (int x = threadIdx.x; x < sp.T * sp.NA * sp.KAp; x += NS_THREADS) {
+      const int k = x % sp.KAp, jn = x / sp.KAp;         // jn = J * NA + n
+      cAs[x] = k < sp.KA ? theta[sp.offA + ((size_t)t * sp.T * sp.NA + jn) * sp.KA + k] : 0.f;
+    }
+  }
   ns_stage_w0(W0s, net, sp.Nn, sp.Ndes, ld);
   for (int x = threadIdx.x; x < 2 * sp.Nn + 1; x += NS_THREADS) bw[x] = net[nW + x];
   for (int x = threadIdx.x; x < sp.Ndes; x += NS_THREADS) qss[x] = qscale[x];
@@ -91,8 +112,49 @@ k_net_small_fwd(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, cons
   for (int r0 = c0; r0 < c1; r0 += NS_ATOMS) {
     const int a = r0 + grp;
     const bool on = a < c1;
-    if (on && tig < sp.Ndes) sq[tig] = qv * qss[tig];
-    if (a + NS_ATOMS < c1 && tig < sp.Ndes) qv = q[(size_t)(a + NS_ATOMS) * sp.Ndes + tig];
+    if (fuse) {
+      if (on && r0 > c0) {
+        for (int x = tig; x < nA1; x += NS_GROUP) A1s[x] = A1[(size_t)a * nA1 + x];
+        for (int x = tig; x < TK; x += NS_GROUP) m1s[x] = M1[(size_t)a * TK + x];
+      }
+      __syncthreads();
+      if (on) {
+        for (int y = tig; y < nS; y += NS_GROUP) {       // S[n][lm] = sum_{J,k} cA[t][J][n][k] A1[J][k][lm]
+          const int n = y / 24, lm = y - n * 24;
+          float s0 = 0.f, s1 = 0.f;
+          for (int J = 0; J < sp.T; ++J) {
+            const float *c = cAs + (size_t)(J * sp.NA + n) * sp.KAp, *m = A1s + (size_t)J * sp.KAp * 24 + lm;
+            for (int k = 0; k < sp.KAp; k += 2) { s0 = fmaf(c[k], m[k * 24], s0); s1 = fmaf(c[k + 1], m[(k + 1) * 24], s1); }
+          }
+          Ss[y] = s0 + s1;
+          S[(size_t)a * nS + y] = s0 + s1;
+        }
+        if (tig < sp.NR) {                               // q_n = sum_{J,k} cR[t][J][n][k] M1[J][k]
+          float s0 = 0.f;
+          for (int jk = 0; jk < TK; ++jk) s0 = fmaf(cRs[jk * 16 + tig], m1s[jk], s0);
+          qrow[tig] = s0;
+        }
+      }
+      __syncthreads();
+      if (on) {
+        const int nl = sp.NA * sp.L;
+        if (tig < nl) {                                  // q_nl = sum_m C_lm S_nlm^2, descriptor index NR + (l-1) NA + n
+          const int l = tig / sp.NA + 1, n = tig - (l - 1) * sp.NA;
+          float v = 0.f;
+          for (int lm = l * l - 1; lm < l * l + 2 * l; ++lm) { const float sv = Ss[n * 24 + lm]; v = fmaf(0.5f * c_C2[lm] * sv, sv, v); }
+          qrow[sp.NR + tig] = v;
+        } else if (sp.use4 && tig < nl + sp.NA) {
+          qrow[sp.NR + tig] = GNEP_KAPPA4 * p4_value(Ss + (tig - nl) * 24 + 3);
+        } else if (sp.use5 && tig < nl + (sp.use4 + 1) * sp.NA) {
+          qrow[sp.NR + tig] = p5_value(Ss + (tig - nl - sp.use4 * sp.NA) * 24);
+        }
+      }
+      __syncthreads();
+      if (on && tig < sp.Ndes) { const float qx = qrow[tig]; q[(size_t)a * sp.Ndes + tig] = qx; sq[tig] = qx * qss[tig]; }
+    } else {
+      if (on && tig < sp.Ndes) sq[tig] = qv * qss[tig];
+      if (a + NS_ATOMS < c1 && tig < sp.Ndes) qv = q[(size_t)(a + NS_ATOMS) * sp.Ndes + tig];
+    }
     __syncthreads();
     float e = 0.f;
     if (on && tig < sp.Nn) {                             // first contraction: thread = neuron (row of W0, odd stride)
