@@ -342,6 +342,8 @@ LossCfg loss_cfg(const gnep_handle *h) {
   const bool job = h->Zjob[0] >= 0 && !h->eval_local;   // gnep_evaluate always normalises by the resident batch itself
   const double *Z = job ? h->Zjob : h->Zloc;
   lc.ZE = Z[0]; lc.ZF = Z[1]; lc.ZV = Z[2]; lc.l2_share = job ? h->l2_share : 1.0;
+  lc.rZE = Z[0] > 0 ? 1.0 / Z[0] : 0.0; lc.rZF3 = Z[1] > 0 ? 1.0 / (3.0 * Z[1]) : 0.0; lc.rZV6 = Z[2] > 0 ? 1.0 / (6.0 * Z[2]) : 0.0;
+  lc.rP = lc.P > 0 ? 1.0 / (double)lc.P : 0.0;
   return lc;
 }
 

@@ -11,6 +11,7 @@ struct LossCfg {
   // normalisers of Eq.10-12 over the WHOLE job: Z_E = sum_s w_e,s, Z_F = sum_s w_f,s N_s, Z_V = sum_s w_v,s
   // (= S, N, S without per-structure weights on one GPU; R40)
   double ZE, ZF, ZV;
+  double rZE, rZF3, rZV6, rP;   // 1/Z_E, 1/(3 Z_F), 1/(6 Z_V), 1/P from the host (0 where Z = 0): no fp64 division on the device
   double l2_share;    // this rank's share of the L2 term (1 on one GPU, 1/world when structures are sharded)
 };
 
@@ -65,34 +66,18 @@ __device__ __forceinline__ double theta_sq(const float *__restrict__ theta, int 
   return (w[0] + w[1]) + (w[2] + w[3]);
 }
 
-// nt2 > 0: theta^2 arrives as nt2 slices; nt2 == 0: the CTA sums it here; nt2 < 0: this thread's share is t2_own.
-// step0 = the step counter as read at the top of the kernel (its load is off the critical path there).
-__device__ __forceinline__ void loss_final(const LossCfg &lc, const double *parts, const double *t2parts, int nt2, double t2_own,
-                                           long long step0, const float *__restrict__ theta, float *__restrict__ terms,
-                                           float *__restrict__ scales, const AdamPre &ap, double *sh) {
-  double v[4] = {0, 0, 0, 0};
-  for (int s = threadIdx.x; s < lc.S; s += blockDim.x) { v[0] += __ldcg(parts + s * 3); v[1] += __ldcg(parts + s * 3 + 1); v[2] += __ldcg(parts + s * 3 + 2); }
-  if (nt2 > 0) { if (threadIdx.x == 0) for (int i = 0; i < nt2; ++i) v[3] += __ldcg(t2parts + i); }
-  else if (nt2 == 0) v[3] = theta_sq(theta, lc.P, threadIdx.x, blockDim.x);
-  else v[3] = t2_own;
-  block_reduce_d<4>(v, sh);
+// The loss terms {L, t_e, t_f, t_v, t_2} (Eq.9-12 + L2) and the per-term seed multipliers from the four batch sums, by
+// thread 0 (thread 32 writes the Adam bias corrections of this step next to it).  scales = {se, sf, sv, s2}: all 1 in
+// mean-square mode, 1/(2 sqrt t_x) in RMSE mode (0 if t_x = 0).
+__device__ __forceinline__ void loss_write(const LossCfg &lc, double se, double sf, double sv, double s2, long long step0,
+                                           float *__restrict__ terms, float *__restrict__ scales, const AdamPre &ap) {
   const long long t = step0 + 1;
-  if (ap.on && threadIdx.x == 32) {                    // bias corrections 1 - beta^t of this step
+  if (ap.on && threadIdx.x == 32) {                    // bias corrections 1 - beta^t
     ap.bc[0] = -expm1f((float)((double)t * ap.lnb1));
     ap.bc[1] = -expm1f((float)((double)t * ap.lnb2));
   }
-  // the four fp64 divisions side by side on lanes 0..3 (a division is ~40 dependent instructions), gathered by lane 0
-  double term = 0.0;
-  if (threadIdx.x < 4) {
-    const int i = threadIdx.x;
-    const double den = i == 0 ? lc.ZE : i == 1 ? 3.0 * lc.ZF : i == 2 ? 6.0 * lc.ZV : (double)lc.P;
-    const double num = i == 0 ? v[0] : i == 1 ? v[1] : i == 2 ? v[2] : lc.l2_share * v[3];
-    term = den > 0 ? num / den : 0.0;
-  }
-  if (threadIdx.x < 32) {
-    const double te = __shfl_sync(0xffffffffu, term, 0), tf = __shfl_sync(0xffffffffu, term, 1);
-    const double tv = __shfl_sync(0xffffffffu, term, 2), t2 = __shfl_sync(0xffffffffu, term, 3);
   if (threadIdx.x == 0) {
+    const double te = se * lc.rZE, tf = sf * lc.rZF3, tv = sv * lc.rZV6, t2 = lc.l2_share * s2 * lc.rP;
     double L, sc[4] = {1, 1, 1, 1};
     if (lc.loss_mode == 0) L = lc.lam_e * te + lc.lam_f * tf + lc.lam_v * tv + lc.lam_2 * t2;
     else {
@@ -104,7 +89,20 @@ __device__ __forceinline__ void loss_final(const LossCfg &lc, const double *part
     for (int i = 0; i < 4; ++i) scales[i] = (float)sc[i];
     if (ap.on) *ap.step = t;
   }
-  }
+}
+
+// nt2 > 0: theta^2 arrives as nt2 slices; nt2 == 0: the CTA sums it here; nt2 < 0: this thread's share is t2_own.
+// step0 = the step counter as read at the top of the kernel (its load is off the critical path there).
+__device__ __forceinline__ void loss_final(const LossCfg &lc, const double *parts, const double *t2parts, int nt2, double t2_own,
+                                           long long step0, const float *__restrict__ theta, float *__restrict__ terms,
+                                           float *__restrict__ scales, const AdamPre &ap, double *sh) {
+  double v[4] = {0, 0, 0, 0};
+  for (int s = threadIdx.x; s < lc.S; s += blockDim.x) { v[0] += __ldcg(parts + s * 3); v[1] += __ldcg(parts + s * 3 + 1); v[2] += __ldcg(parts + s * 3 + 2); }
+  if (nt2 > 0) { if (threadIdx.x == 0) for (int i = 0; i < nt2; ++i) v[3] += __ldcg(t2parts + i); }
+  else if (nt2 == 0) v[3] = theta_sq(theta, lc.P, threadIdx.x, blockDim.x);
+  else v[3] = t2_own;
+  block_reduce_d<4>(v, sh);
+  loss_write(lc, v[0], v[1], v[2], v[3], step0, terms, scales, ap);
 }
 
 // a4: one CTA per structure.  E_s = sum E_i, W_s = sum W_i (Eq.1, Eq.4), residuals of Eq.10-12 and the
@@ -121,8 +119,9 @@ k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const 
                 double *__restrict__ Ws, float *__restrict__ e_s, float4 *__restrict__ u,
                 float *__restrict__ omega, double *parts /*[S][3] + [LOSS_T2_CTAS]*/, unsigned *ticket,
                 const float *__restrict__ theta, float *__restrict__ terms, float *__restrict__ scales, AdamPre ap) {
-  __shared__ double sh[8 * 4];
+  __shared__ double sh[9 * 4];
   __shared__ int last;
+  double solo_sum[4] = {0, 0, 0, 0};       // thread 0, solo: the batch sums stay in registers
   // A batch of a few structures (size-1 mini-batches) is launched as ONE CTA that walks all structures and then
   // writes the loss terms itself: no ticket, no fences, no tail of a second CTA in the chain of dependent launches.
   const bool solo = gridDim.x == 1;
@@ -145,7 +144,8 @@ k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const 
     if (threadIdx.x == 0) *ticket = 0u;
     return;
   }
-  double v[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // E, W[6], sum |dF|^2
+  double v[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};   // E, W[6], sum |dF|^2, and (solo, first structure) this thread's share of theta^2
+  if (solo && s == 0) v[8] = t2_own;
   int Ns = 0;
   const double we = wgt[s], wf = wgt[lc.S + s], wv = wgt[2 * lc.S + s];
   const float cu = lc.hasF && lc.ZF > 0 ? (float)(2.0 * lc.lam_f * wf / (3.0 * lc.ZF)) : 0.f;
@@ -170,7 +170,7 @@ k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const 
       u[a] = make_float4(cu * dx, cu * dy, cu * dz, 0.f);
     }
   }
-  block_reduce_d<8>(v, sh);
+  block_reduce_d<9>(v, sh);
   if (threadIdx.x == 0) {
     Es[s] = v[0];
     // per-atom residuals through ONE reciprocal of N_s (an fp64 division is ~40 dependent instructions on this one thread)
@@ -179,11 +179,11 @@ k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const 
     if (lc.hasE && Ns > 0 && lc.ZE > 0) {
       const double dE = (v[0] - eref) * inv_ns;
       pe = we * dE * dE;
-      es = (2.0 * lc.lam_e * we / lc.ZE) * inv_ns * dE;
+      es = 2.0 * lc.lam_e * we * lc.rZE * inv_ns * dE;
     }
     e_s[s] = (float)es;
     const bool onV = lc.hasV && Ns > 0 && lc.ZV > 0;
-    const double k_om = onV ? (2.0 * lc.lam_v * wv / (6.0 * lc.ZV)) * inv_ns : 0.0;
+    const double k_om = onV ? 2.0 * lc.lam_v * wv * lc.rZV6 * inv_ns : 0.0;
 #pragma unroll
     for (int c = 0; c < 6; ++c) {
       Ws[s * 6 + c] = v[1 + c];
@@ -196,6 +196,7 @@ k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const 
       omega[s * 6 + c] = (float)om;
     }
     parts[s * 3 + 0] = pe; parts[s * 3 + 1] = wf * v[7]; parts[s * 3 + 2] = pv;
+    solo_sum[0] += pe; solo_sum[1] += wf * v[7]; solo_sum[2] += pv; solo_sum[3] += v[8];
     if (!solo) {
       __threadfence();                                         // parts visible before the ticket is taken
       last = atomicAdd(ticket, 1u) == gridDim.x - 1;
@@ -203,8 +204,8 @@ k_struct_reduce(LossCfg lc, const int *__restrict__ srange /*[S][T][2]*/, const 
   }
   __syncthreads();
   }   // structures of this CTA
-  if (solo) {                               // (parts were written by this CTA: ordered by the barrier above)
-    loss_final(lc, parts, nullptr, -1, t2_own, step0, theta, terms, scales, ap, sh);
+  if (solo) {                               // thread 0 holds every sum
+    loss_write(lc, solo_sum[0], solo_sum[1], solo_sum[2], solo_sum[3], step0, terms, scales, ap);
     return;
   }
   if (!last) return;
