@@ -114,7 +114,7 @@ def test_config4_liquid_sample():
     _check_all(4, 3, adam_steps=2)
 
 
-def test_rmse_mode_and_missing_virial():
+def test_rmse_mode_and_missing_virial(kernel_set):
     spec, sp, b, ob, theta, qs, (E, F, W) = labelled_case(0, n_structs=3, spec_over={"loss_mode": 1})
     g = _gnep(spec, qs, b, (E, F, W), theta)
     terms, grad = g.loss_and_grad(want_grad=True)
@@ -131,7 +131,7 @@ def test_rmse_mode_and_missing_virial():
     g.destroy()
 
 
-def test_small_l_and_odd_sizes():
+def test_small_l_and_odd_sizes(kernel_set):
     """l_max = 2 without 4-body, odd function / basis counts (padding paths)."""
     over = {"l_max": 2, "n_radial": 3, "n_basis_radial": 5, "n_angular": 11, "n_basis_angular": 7, "n_neurons": 37}
     _check_all(0, 2, adam_steps=2, spec_over=over)
@@ -152,12 +152,12 @@ def test_three_species_odd_sizes(kernel_set):
     _check_all(0, 3, adam_steps=2, spec_over=over)
 
 
-def test_four_species():
+def test_four_species(kernel_set):
     """T = GNEP_MAX_SPECIES: the packed (atom | J << 28 | I << 30) pair tag uses both bits of each field."""
     _check_all(1, 6, adam_steps=2, spec_over={"n_species": 4, "n_neurons": 20})
 
 
-def test_one_species():
+def test_one_species(kernel_set):
     _check_all(0, 2, adam_steps=2, spec_over={"n_species": 1, "l_max": 1, "n_angular": 3, "n_neurons": 9})
 
 
