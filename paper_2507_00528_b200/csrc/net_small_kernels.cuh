@@ -19,6 +19,19 @@
 #define NS_ATOMS 4          // atoms per CTA and round (contiguous, one species): SpeciesMap.gw_atoms of a small batch
 #define NS_THREADS (NS_GROUP * NS_ATOMS)
 
+// species t and atom range [c0, c1) of CTA `bid` (SpeciesMap.gw_base / gw_atoms / start) with STATIC indices into the
+// kernel-parameter struct: a dynamic index makes the compiler copy the struct to local memory (a fifth of the
+// instructions of these short kernels)
+__device__ __forceinline__ void ns_range(const SpeciesMap &sm, int T, int bid, int &t, int &c0, int &c1) {
+  int base = sm.gw_base[0], start = sm.start[0], end = sm.start[1], ga = sm.gw_atoms[0];
+  t = 0;
+#pragma unroll
+  for (int i = 1; i < GNEP_MAX_SPECIES_C; ++i)
+    if (i < T && bid >= sm.gw_base[i]) { t = i; base = sm.gw_base[i]; start = sm.start[i]; end = sm.start[i + 1]; ga = sm.gw_atoms[i]; }
+  c0 = start + (bid - base) * ga;
+  c1 = min(c0 + ga, end);
+}
+
 // W0 of one species (Nn x Ndes, row-major, contiguous at `net`) into shared memory with row stride ld; element
 // x = mu * Ndes + nu is walked with incremental (mu, nu): no integer division in the loop, loads independent
 __device__ __forceinline__ void ns_stage_w0(float *W0s, const float *__restrict__ net, int Nn, int Ndes, int ld) {
@@ -84,10 +97,9 @@ k_net_small_fwd(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, cons
   const int nA1 = sp.T * sp.KAp * 24, nS = sp.NA * 24, ndr = nA1 + TK + nS + sp.Ndes;
   float *cAs = qss + sp.Ndes + (size_t)NS_ATOMS * nrow;            // [J][n][k(KAp)] of this species, zero padded
   float *A1s = cAs + (size_t)sp.T * sp.NA * sp.KAp + (size_t)grp * ndr, *m1s = A1s + nA1, *Ss = m1s + TK, *qrow = Ss + nS;
-  const int t = species_of_block(sm.gw_base, sp.T, blockIdx.x);
+  int t, c0, c1;
+  ns_range(sm, sp.T, blockIdx.x, t, c0, c1);
   const float *net = theta + sp.offNet + (size_t)t * sp.netSize;
-  const int c0 = sm.start[t] + (blockIdx.x - sm.gw_base[t]) * sm.gw_atoms[t];
-  const int c1 = min(c0 + sm.gw_atoms[t], sm.start[t + 1]);
   // the first atom's row is requested before the staging loops (it does not depend on them)
   float qv = (!fuse && c0 + grp < c1 && tig < sp.Ndes) ? q[(size_t)(c0 + grp) * sp.Ndes + tig] : 0.f;
   if (fuse) {
@@ -216,10 +228,9 @@ k_net_small_bwd(DevSpec sp, SpeciesMap sm, const float *__restrict__ theta, cons
   float *crow0 = red + (size_t)NS_ATOMS * nb;          // per atom: gbar[0..NR) | E'[0..NR) | M1[TK] | M2[TK]
   float *accC = crow0 + (size_t)NS_ATOMS * ncr;        // [NR][TK]
   float *crow = crow0 + (size_t)grp * ncr;
-  const int t = species_of_block(sm.gw_base, sp.T, blockIdx.x);
+  int t, c0, c1;
+  ns_range(sm, sp.T, blockIdx.x, t, c0, c1);
   const float *net = theta + sp.offNet + (size_t)t * sp.netSize;
-  const int c0 = sm.start[t] + (blockIdx.x - sm.gw_base[t]) * sm.gw_atoms[t];
-  const int c1 = min(c0 + sm.gw_atoms[t], sm.start[t + 1]);
   ns_stage_w0(W0s, net, sp.Nn, sp.Ndes, ld);
   for (int x = threadIdx.x; x < sp.Nn; x += NS_THREADS) w1s[x] = net[nW + sp.Nn + x];
   for (int x = threadIdx.x; x < sp.Ndes; x += NS_THREADS) qss[x] = qscale[x];
