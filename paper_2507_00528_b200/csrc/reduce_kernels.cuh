@@ -223,6 +223,15 @@ k_loss_final(LossCfg lc, const double *parts, const float *__restrict__ theta, f
 }
 
 // a8: grad[p] = sum over the partial buffers that cover p (fixed order, fp64) + 2 lam_2 s2 theta_p / P.
+// a[i] of a small array inside a kernel-parameter struct through static indices (a dynamic index would make the
+// compiler copy the whole struct to local memory)
+template <int NMAX>
+__device__ __forceinline__ int pick(const int (&a)[NMAX], int i) {
+  int v = a[0];
+#pragma unroll
+  for (int j = 1; j < NMAX; ++j) v = i == j ? a[j] : v;
+  return v;
+}
 struct ReduceMap {
   int chunk_base[GNEP_MAX_SPECIES_C + 1];   // K-chunks (W0, cR partials) per species
   int gw_base[GNEP_MAX_SPECIES_C + 1];      // k_gradw_tc CTAs (W0, b0, w1, b1 partials) per species
@@ -247,7 +256,7 @@ k_grad_reduce(DevSpec sp, ReduceMap rm, float l2_share, float *theta, const floa
       int J = r % sp.T, I = r / sp.T;
       stride = (size_t)sp.NR * sp.T * sp.KRp;
       base = partialCR + n * sp.T * sp.KRp + J * sp.KRp + k;
-      r0 = rm.chunk_base[I]; r1 = rm.chunk_base[I + 1];
+      r0 = pick(rm.chunk_base, I); r1 = pick(rm.chunk_base, I + 1);
     } else if (p < sp.offNet) {              // cA[I][J][n][k]
       int x = p - sp.offA;
       int k = x % sp.KA, r = x / sp.KA;      // r = (I*T+J)*NA + n
@@ -258,7 +267,7 @@ k_grad_reduce(DevSpec sp, ReduceMap rm, float l2_share, float *theta, const floa
       int x = p - sp.offNet;
       int t = x / sp.netSize, y = x - t * sp.netSize;
       int nW = sp.Nn * sp.Ndes;
-      r0 = rm.gw_base[t]; r1 = rm.gw_base[t + 1];
+      r0 = pick(rm.gw_base, t); r1 = pick(rm.gw_base, t + 1);
       if (y < nW) { stride = nW; base = partialW + y; }
       else { stride = 2 * sp.Nn + 1; base = partialB + (y - nW); }
     }
