@@ -58,7 +58,7 @@ def test_minibatch_trajectory_matches_oracle(config, n_structs, bs):
     parent.destroy()
 
 
-def test_held_out_evaluation_on_a_shared_handle():
+def test_held_out_evaluation_on_a_shared_handle(kernel_set):
     """gnep_evaluate: RMSEs of a test batch held by a shared handle, with and without a virial reference."""
     from paper_2507_00528_b200 import Gnep
     spec, sp, b, ob, theta, qs, labels = labelled_case(1, n_structs=5)

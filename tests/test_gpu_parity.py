@@ -85,15 +85,6 @@ def _check_all(config, n_structs, adam_steps=10, spec_over=None, floor=1e-6):
     g.destroy()
 
 
-@pytest.fixture(params=["large", "small"])
-def kernel_set(request, monkeypatch):
-    """Both kernel sets on the same small case: the large-batch mappings (one thread per atom in the radial sweeps,
-    16 / 8 atoms per warp in the angular ones) that the bench configurations run, and the small-batch ones (8 lanes per
-    atom, one atom per warp) that a batch of this size would get by itself.  Read by gnep_load_batch."""
-    monkeypatch.setenv("GNEP_SMALL_BATCH", "1" if request.param == "small" else "0")
-    return request.param
-
-
 def test_config0_full(kernel_set):
     _check_all(0, None)
 
@@ -161,18 +152,18 @@ def test_one_species(kernel_set):
     _check_all(0, 2, adam_steps=2, spec_over={"n_species": 1, "l_max": 1, "n_angular": 3, "n_neurons": 9})
 
 
-def test_l_max_6_with_4body():
+def test_l_max_6_with_4body(kernel_set):
     """Higher angular order (paper Eq.7: l up to 8; b_lm of Eq.B5-B6): the slot-group kernels, 8 groups."""
     over = {"l_max": 6, "use_4body": True, "n_angular": 4, "n_basis_angular": 5, "n_neurons": 12}
     _check_all(0, 2, adam_steps=2, spec_over=over, floor=3e-5)
 
 
-def test_l_max_8_with_4body_and_5body():
+def test_l_max_8_with_4body_and_5body(kernel_set):
     over = {"l_max": 8, "use_4body": True, "use_5body": True, "n_angular": 5, "n_basis_angular": 8, "n_neurons": 16}
     _check_all(1, 2, adam_steps=2, spec_over=over, floor=3e-5)
 
 
-def test_l_max_5_three_species_no_many_body():
+def test_l_max_5_three_species_no_many_body(kernel_set):
     over = {"n_species": 3, "l_max": 5, "use_4body": False, "n_angular": 3, "n_basis_angular": 4, "n_neurons": 8}
     _check_all(0, 3, adam_steps=2, spec_over=over, floor=3e-5)
 
@@ -182,7 +173,7 @@ def test_5body_with_l_max_4_on_the_warp_tile_kernels(kernel_set):
     _check_all(3, 4, adam_steps=2, spec_over={"use_5body": True, "n_neurons": 40}, floor=1e-5)   # (4 structures: a noisier sample than config 3)
 
 
-def test_slot_group_mapping_for_config3_with_5body(monkeypatch):
+def test_slot_group_mapping_for_config3_with_5body(monkeypatch, kernel_set):
     """GNEP_ANGULAR_MAPPING=groups runs an l_max <= 4 model through the slot-group kernels (config-3 sizes, 4 groups)."""
     monkeypatch.setenv("GNEP_ANGULAR_MAPPING", "groups")
     _check_all(3, 4, adam_steps=2, spec_over={"use_5body": True, "n_neurons": 40}, floor=1e-5)

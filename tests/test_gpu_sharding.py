@@ -22,7 +22,7 @@ def _shard(b, labels, lo, hi):
 
 
 @pytest.mark.parametrize("config,n_structs,world", [(1, 6, 2), (3, 7, 3)])
-def test_sharded_epoch_matches_single_batch_oracle(config, n_structs, world):
+def test_sharded_epoch_matches_single_batch_oracle(config, n_structs, world, kernel_set):
     from paper_2507_00528_b200 import Gnep
     spec, sp, b, ob, theta, qs, labels = labelled_case(config, n_structs=n_structs)
     off = b["atom_offsets"]

@@ -27,7 +27,7 @@ def _compare(g, sp, theta, qs, ob):
     return terms, grad
 
 
-def test_half_the_structures_have_no_virial_and_random_weights():
+def test_half_the_structures_have_no_virial_and_random_weights(kernel_set):
     spec, sp, b, ob, theta, qs, labels = labelled_case(3, n_structs=6)
     S = 6
     g = _gnep(spec, qs, b, labels, theta)
