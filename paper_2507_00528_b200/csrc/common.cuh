@@ -325,6 +325,15 @@ __device__ __forceinline__ float8 ldg256(const float *p) {
                : "l"(p));
   return r;
 }
+// the same for data that is streamed once (pair lists): no L1 allocation, so that the lines of the per-atom rows the
+// sweep gathers (etil_j, u_j) stay resident in L1
+__device__ __forceinline__ float8 ldg256_stream(const float *p) {
+  float8 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=f"(r.lo.x), "=f"(r.lo.y), "=f"(r.lo.z), "=f"(r.lo.w), "=f"(r.hi.x), "=f"(r.hi.y), "=f"(r.hi.z), "=f"(r.hi.w)
+               : "l"(p));
+  return r;
+}
 __device__ __forceinline__ void stg256(float *p, const float4 &a, const float4 &b) {
   asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "f"(a.x), "f"(a.y), "f"(a.z), "f"(a.w), "f"(b.x),
                "f"(b.y), "f"(b.z), "f"(b.w)

@@ -28,7 +28,7 @@ __device__ __forceinline__ void walk_row(const float4 *__restrict__ pairR, const
   // the row's end -- in the row's pad slot (zeroed at load: w = bits(0), a valid index) or in the next row -- its body
   // is skipped, but gather() still runs on it one pair ahead, so its w must always be a valid atom index
   auto load2 = [&](int q, float4 &r0, float4 &r1) {
-    if (q < pend) { const float8 v = ldg256((const float *)(pairR + q)); r0 = v.lo; r1 = v.hi; }
+    if (q < pend) { const float8 v = ldg256_stream((const float *)(pairR + q)); r0 = v.lo; r1 = v.hi; }
     else { r0 = dum; r1 = dum; }
   };
 #pragma unroll
