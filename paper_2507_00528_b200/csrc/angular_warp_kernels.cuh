@@ -343,9 +343,9 @@ k_angw_S(DevSpec sp, int N, const int *__restrict__ type_s, const float *__restr
     const int np2 = (2 * it + 1 < N ? 2 : 1) * pieces, nm2 = (2 * it + 1 < N ? 2 : 1) * nM;
 #pragma unroll
     for (int v = 0; v < NP; ++v)
-      if (lane + 32 * v < np2) {
-        *(float4 *)(stage + 8 * (lane + 32 * v)) = pre[v].lo;
-        *(float4 *)(stage + 8 * (lane + 32 * v) + 4) = pre[v].hi;
+      if (lane + 32 * v < np2) {     // piece p = 8 floats of a row: low quads in one plane, high quads in the other, so that
+        *(float4 *)(stage + 4 * (lane + 32 * v)) = pre[v].lo;          // both stores are contiguous across the lanes (a 32-byte
+        *(float4 *)(stage + nA + 4 * (lane + 32 * v)) = pre[v].hi;     // stride per lane is a two-way bank conflict)
       }
 #pragma unroll
     for (int v = 0; v < NMP; ++v) {
@@ -380,14 +380,14 @@ k_angw_S(DevSpec sp, int N, const int *__restrict__ type_s, const float *__restr
         for (int J = 0; J < sp.T; ++J) {
           const float *c = csA + ((size_t)(I * sp.T + J) * sp.NA + n0) * KT;
           const float *c1 = on1 ? c + KT : c;
-          const float *row = stage + (size_t)half * nA + (size_t)J * KT * ANGW_NLM + 8 * lmg;
+          const float *row = stage + 4 * ((half * nA) / 8 + J * KT * 3 + lmg);   // low quad of piece (J, k = 0, lmg); + 12 per k; high plane + nA
 #pragma unroll
           for (int k4 = 0; k4 < KT; k4 += 4) {
             const float4 ca = *(const float4 *)(c + k4), cb = *(const float4 *)(c1 + k4);
             const float cv0[4] = {ca.x, ca.y, ca.z, ca.w}, cv1[4] = {cb.x, cb.y, cb.z, cb.w};
 #pragma unroll
             for (int kk = 0; kk < 4; ++kk) {
-              const float4 lo = *(const float4 *)(row + (k4 + kk) * ANGW_NLM), hi = *(const float4 *)(row + (k4 + kk) * ANGW_NLM + 4);
+              const float4 lo = *(const float4 *)(row + (k4 + kk) * 12), hi = *(const float4 *)(row + nA + (k4 + kk) * 12);
               const float av[8] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
 #pragma unroll
               for (int i = 0; i < 8; ++i) { sv[0][i] = fmaf(cv0[kk], av[i], sv[0][i]); sv[1][i] = fmaf(cv1[kk], av[i], sv[1][i]); }
