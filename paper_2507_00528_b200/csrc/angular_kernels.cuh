@@ -676,10 +676,11 @@ k_angular_force(DevSpec sp, int N, int ta /* atoms per warp, <= FRC_TA */, const
   }
   __syncwarp();
   // ... and out to global memory, row-major like S, for the adjoint sweep (32 bytes per lane and store)
-  for (int it = lane; it < (a_hi - a_lo) * (nb / 8); it += 32) {
-    const float4 *src = (const float4 *)(beta + 8 * it);
-    stg256(Beta + (size_t)a_lo * nb + 8 * it, src[0], src[1]);
-  }
+  if (Beta)                                      // (only the slot-group adjoint sweep reads it: nullptr on the warp-tile path)
+    for (int it = lane; it < (a_hi - a_lo) * (nb / 8); it += 32) {
+      const float4 *src = (const float4 *)(beta + 8 * it);
+      stg256(Beta + (size_t)a_lo * nb + 8 * it, src[0], src[1]);
+    }
   if (P_lo == P_hi) return;
   // atomA packs (central atom | neighbour species << 28 | central species << 30); the next chunk's record is in flight
   float4 rn = make_float4(1.f, 0.f, 0.f, 0.f);

@@ -360,7 +360,7 @@ int enqueue_forward(gnep_handle *h) {
            (const int *)nullptr, (const float *)nullptr, (const float *)nullptr, (float *)nullptr, (float *)nullptr);
   }
   mark(h, "a2_network_forward");
-  DISPATCH_ANG(d, auto kp = k_angular_force<KT, LMAX>; LAUNCH(h, kp, cdiv(h->N, FRC_WARPS * h->ta_frc), FRC_WARPS * 32, smem_ang_force(d), d, h->N, h->ta_frc, h->type_s, h->segAu, h->atomAu, h->pairAu, h->theta, h->Ep, h->Sn, h->Beta, h->fpair));
+  DISPATCH_ANG(d, auto kp = k_angular_force<KT, LMAX>; LAUNCH(h, kp, cdiv(h->N, FRC_WARPS * h->ta_frc), FRC_WARPS * 32, smem_ang_force(d), d, h->N, h->ta_frc, h->type_s, h->segAu, h->atomAu, h->pairAu, h->theta, h->Ep, h->Sn, h->tile_path ? h->Beta : (float *)nullptr, h->fpair));
   mark(h, "a3_angular_force");
   // radial forces + the gather of the angular pair forces (thread per atom): writes F_i, W_i once
   if (h->rad_split) {
@@ -941,7 +941,7 @@ int gnep_load_batch(gnep_handle *h, int32_t S, const int32_t *aoff, const double
     const size_t npad = n + GW_PAD_ROWS;
     const size_t nxt = (npad + 127) / 128 * 128;   // x, p: whole 128-atom blocks of the XT layout (net_tc_kernels.cuh)   // k_gradw_tc bulk-copies whole windows of rows: zeroed rows past the end
     BA(h->q, npad * d.Ndes); BA(h->Sn, n * d.NA * d.nlmS); BA(h->x, nxt * d.NnS); BA(h->Ei, n); BA(h->Ep, n * d.Ndes);
-    BA(h->etil, n * T * d.KRp); BA(h->M1, n * T * d.KRp); BA(h->M2, n * T * d.KRp); BA(h->D, npad * d.Ndes); BA(h->Tn, n * d.NA * d.nlmS); BA(h->Beta, n * d.NA * d.nlmS); BA(h->A1, h->tile_path ? n * ang_groups(d.L) * T * d.KAp * ANG_GS : n * T * d.KAp * ANGW_NLM);
+    BA(h->etil, n * T * d.KRp); BA(h->M1, n * T * d.KRp); BA(h->M2, n * T * d.KRp); BA(h->D, npad * d.Ndes); BA(h->Tn, n * d.NA * d.nlmS); if (h->tile_path) BA(h->Beta, n * d.NA * d.nlmS);   /* (read by the slot-group adjoint sweep only) */ BA(h->A1, h->tile_path ? n * ang_groups(d.L) * T * d.KAp * ANG_GS : n * T * d.KAp * ANGW_NLM);
     if (!h->tile_path) BA(h->A2, n * T * d.KAp * ANGW_NLM);
     BA(h->gbar, n * d.Ndes); BA(h->pbuf, nxt * d.NnS); BA(h->eat, npad); BA(h->Wat, n * 6);
     BA(h->Fat, n); BA(h->fpair, h->nA); BA(h->u, n);
