@@ -40,19 +40,29 @@ k_cgrad_radial(DevSpec sp, SpeciesMap sm, const float *__restrict__ gbar, const 
   for (int i = 0; i < 4; ++i)
 #pragma unroll
     for (int j = 0; j < 4; ++j) acc[i][j] = 0.f;
+  const int atA0 = threadIdx.x / NRp, nA0 = threadIdx.x - atA0 * NRp, datA = CR_THREADS / NRp, dnA = CR_THREADS - datA * NRp;
+  const int atM0 = threadIdx.x / TKp, jkM0 = threadIdx.x - atM0 * TKp, datM = CR_THREADS / TKp, djkM = CR_THREADS - datM * TKp;
   for (int s0 = c0; s0 < c1; s0 += CR_SUB) {
     const int ns_ = min(CR_SUB, c1 - s0);
-    for (int x = threadIdx.x; x < ns_ * NRp; x += CR_THREADS) {
-      const int at = x / NRp, n = x - at * NRp;
-      const bool ok = n < sp.NR;
-      gb[x] = ok ? gbar[(size_t)(s0 + at) * sp.Ndes + n] : 0.f;
-      ep[x] = ok ? Ep[(size_t)(s0 + at) * sp.Ndes + n] : 0.f;
-    }
-    for (int x = threadIdx.x; x < ns_ * TKp; x += CR_THREADS) {
-      const int at = x / TKp, jk = x - at * TKp;
-      const bool ok = jk < TK;
-      m1[x] = ok ? M1[(size_t)(s0 + at) * TK + jk] : 0.f;
-      m2[x] = ok ? M2[(size_t)(s0 + at) * TK + jk] : 0.f;
+    {   // (at, n) and (at, jk) advance incrementally: no integer division per element (it cost as much as the FMAs)
+      int at = atA0, n = nA0;
+#pragma unroll 4
+      for (int x = threadIdx.x; x < ns_ * NRp; x += CR_THREADS) {
+        const bool ok = n < sp.NR;
+        gb[x] = ok ? gbar[(size_t)(s0 + at) * sp.Ndes + n] : 0.f;
+        ep[x] = ok ? Ep[(size_t)(s0 + at) * sp.Ndes + n] : 0.f;
+        at += datA; n += dnA;
+        if (n >= NRp) { n -= NRp; ++at; }
+      }
+      at = atM0; int jk = jkM0;
+#pragma unroll 4
+      for (int x = threadIdx.x; x < ns_ * TKp; x += CR_THREADS) {
+        const bool ok = jk < TK;
+        m1[x] = ok ? M1[(size_t)(s0 + at) * TK + jk] : 0.f;
+        m2[x] = ok ? M2[(size_t)(s0 + at) * TK + jk] : 0.f;
+        at += datM; jk += djkM;
+        if (jk >= TKp) { jk -= TKp; ++at; }
+      }
     }
     __syncthreads();
     if (on)
