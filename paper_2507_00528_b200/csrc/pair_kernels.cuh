@@ -261,7 +261,7 @@ __device__ __forceinline__ void pair_adjoint(const AdjCtx &c, const float4 &uj, 
 // a5 (radial): M2[a][J][k] = sum_j f_k'(d_ij) (a_ij . rhat_ij) ;  D_n = sum_{J,k} cR[I][J][n][k] M2[J][k]
 // ------------------------------------------------------------------------------------------------
 template <int KT>
-__global__ void __launch_bounds__(RAD_THREADS)
+__global__ void __launch_bounds__(RAD_THREADS, KT <= 12 ? 6 : 4)
 k_radial_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__restrict__ struct_s,
              const int *__restrict__ segR, const float4 *__restrict__ pairR, const float *__restrict__ theta,
              const float4 *__restrict__ u, const float *__restrict__ omega, const float *__restrict__ scales,
@@ -275,14 +275,19 @@ k_radial_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__res
   const AdjCtx ac = make_adj(u, omega, scales, a, struct_s[a]);
   const int *sg = segR + (size_t)a * (sp.T + 1);
   float *Mrow = M2 + (size_t)a * sp.T * KT;
-  // acc[k] = sum (a.rhat) f_k'(d),  f_0' = 2 hfcp, f_k' = D_k hdf + (T_k + 1) hfcp  (one accumulator per k keeps the
-  // kernel at 6 resident CTAs per SM; the walk lives on occupancy)
+  // M2[k] = sum (a.rhat) f_k'(d),  f_k' = D_k hdf + (T_k + 1) hfcp for every k (T_0 = 1, D_0 = 0); accumulated per
+  // Chebyshev term as in k_radial_fwd: acc[k] = sum w1 D_k + w2 T_k, acc[0] = sum w2, M2[k] = acc[k] + acc[0] when the
+  // segment ends (one accumulator per k keeps the kernel at 6 resident CTAs per SM; the walk lives on occupancy)
   float acc[KT];
 #pragma unroll
   for (int k = 0; k < KT; ++k) acc[k] = 0.f;
   walk_row(pairR, sg, sp.T,
-           [&](int J) {
-             store_row<KT>(Mrow + J * KT, acc);
+           [&](int J) {                                     // M2[k] = acc[k] + acc[0]  (the "+ 1" of T_k + 1; T_0 = 1)
+             float m[KT];
+             m[0] = 2.f * acc[0];
+#pragma unroll
+             for (int k = 1; k < KT; ++k) m[k] = acc[k] + acc[0];
+             store_row<KT>(Mrow + J * KT, m);
 #pragma unroll
              for (int k = 0; k < KT; ++k) acc[k] = 0.f;
            },
@@ -295,9 +300,9 @@ k_radial_adj(DevSpec sp, int N, const int *__restrict__ type_s, const int *__res
              const float ar = (ax * r.x + ay * r.y + az * r.z) * rinv;
              cheb_TD<KT>(d, sp.rcRinv, Tk, Dk, hfc, hfcp, hdf);
              const float w1 = ar * hdf, w2 = ar * hfcp;
-             acc[0] = fmaf(2.f, w2, acc[0]);
+             acc[0] += w2;
 #pragma unroll
-             for (int k = 1; k < KT; ++k) acc[k] = fmaf(w1, Dk[k], fmaf(w2, Tk[k], acc[k] + w2));
+             for (int k = 1; k < KT; ++k) acc[k] = fmaf(w1, Dk[k], fmaf(w2, Tk[k], acc[k]));
            });
   radial_contract<KT>(sp, cs, type_s[a], Mrow, D + (size_t)a * sp.Ndes);
 }
@@ -413,12 +418,15 @@ k_radial_adj_split(DevSpec sp, int N, const int *__restrict__ type_s, const int 
         const float ar = (ax * r.x + ay * r.y + az * r.z) * rinv;
         cheb_TD<KT>(d, sp.rcRinv, Tk, Dk, hfc, hfcp, hdf);
         const float w1 = ar * hdf, w2 = ar * hfcp;
-        acc[0] = fmaf(2.f, w2, acc[0]);
+        acc[0] += w2;
 #pragma unroll
-        for (int k = 1; k < KT; ++k) acc[k] = fmaf(w1, Dk[k], fmaf(w2, Tk[k], acc[k] + w2));
+        for (int k = 1; k < KT; ++k) acc[k] = fmaf(w1, Dk[k], fmaf(w2, Tk[k], acc[k]));
       }
 #pragma unroll
-    for (int k = 0; k < KT; ++k) acc[k] = split_sum<SPLIT>(acc[k]);       // every lane of the atom now holds M2[J][.]
+    for (int k = 0; k < KT; ++k) acc[k] = split_sum<SPLIT>(acc[k]);
+#pragma unroll
+    for (int k = 1; k < KT; ++k) acc[k] += acc[0];                        // the "+ 1" of T_k + 1 (as in k_radial_adj)
+    acc[0] *= 2.f;                                                        // every lane of the atom now holds M2[J][.]
     if (on && sub == 0) store_row<KT>(M2 + (size_t)a * sp.T * KT + J * KT, acc);
     const float *c = cs + (size_t)(I * sp.T + J) * sp.NR * KT;
 #pragma unroll
