@@ -634,9 +634,9 @@ k_gradw_tc(DevSpec sp, SpeciesMap sm, int nraw, const float *__restrict__ theta,
     }
     const int e_off = 2 * GW_KS * (sp.NnS + sp.Ndes);
     int nfl = 0;                                        // accumulation groups already added to the registers
-    for (int it = 0; it < nst; ++it) {
+    int rs = 0, ruse = 0;                               // raw stage of window `it` and how often it has been used: it % nraw,
+    for (int it = 0; it < nst; ++it, rs = rs + 1 == nraw ? 0 : rs + 1, ruse += rs == 0) {   // it / nraw without the division
       const int st = it % GW_OPST, use = it / GW_OPST, g = it / GW_FLUSH, gi = it - g * GW_FLUSH;
-      const int rs = it % nraw, ruse = it / nraw;
       float *sb = smem + st * stage_fl;
       const float *rb = raw + rs * raw_fl;
       // group g - 1 is added to the registers one stage late (at the second stage of group g), so that its last
